@@ -1,0 +1,343 @@
+"""Pins for the CPU oracle (-m "not gpu").
+
+The paper prints no worked numerical example for this path, so each
+pin is something the mathematics fixes independently of oracle/staggered_oracle.c:
+a dense matrix built from the definition in numpy, closed forms, invariants and dense solves.
+Each test names the mistake it would catch.
+"""
+import numpy as np
+import pytest
+
+import lqcd_inputs as gen
+import oracle
+from dense_reference import dense_dirac, dense_normal_operator, parity_mask
+
+
+def rel(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+# ----------------------------------------------------------------------------------------------
+# Operator: dense brute force (stencil, phases, BC, N=2 wrap, dagger, 1/2)
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (4, 4, 4, 4), (4, 2, 6, 2)])
+@pytest.mark.parametrize("ap", [True, False])
+def test_dirac_matches_dense_matrix(dims, ap):
+    rng = np.random.default_rng(1)
+    U = gen.haar_like_links(dims, rng)
+    psi = gen.gaussian_spinor(dims, rng)
+    D = dense_dirac(dims, U, ap)
+    want = (D @ psi.reshape(-1)).reshape(-1, 3)
+    got = oracle.dirac_full(dims, U, psi, antiperiodic_t=ap)
+    assert rel(got, want) < 1e-14
+    # structure of the dense matrix itself: anti-Hermitian, no even-even / odd-odd block (Eq. 7)
+    assert np.abs(D + D.conj().T).max() == 0.0
+    par = np.repeat(parity_mask(dims), 3)
+    assert np.abs(D[np.ix_(par == 0, par == 0)]).max() == 0.0
+    assert np.abs(D[np.ix_(par == 1, par == 1)]).max() == 0.0
+
+
+def test_dirac_columns_at_2x4():
+    """oracle . e_j = column j of the dense matrix, every j (BASELINE.json config 1, 2^4)."""
+    dims = (2, 2, 2, 2)
+    U = gen.haar_like_links(dims, 1)
+    D = dense_dirac(dims, U, True)
+    V = gen.volume(dims)
+    for j in range(3 * V):
+        e = np.zeros(3 * V, dtype=np.complex128)
+        e[j] = 1.0
+        col = oracle.dirac_full(dims, U, e.reshape(V, 3)).reshape(-1)
+        assert np.abs(col - D[:, j]).max() < 1e-15
+
+
+def test_half_lattice_views_and_parity_naming():
+    """dslash_half(out_parity) = the (out, in) block of the dense matrix (reading R5)."""
+    dims = (4, 4, 2, 4)
+    rng = np.random.default_rng(7)
+    U = gen.haar_like_links(dims, rng)
+    _, D_eo, D_oe = dense_normal_operator(dims, U, 0.1)
+    in_e = gen.gaussian_half_spinor(dims, rng)
+    in_o = gen.gaussian_half_spinor(dims, rng)
+    out_o = oracle.dslash_half(dims, U, 1, in_e)
+    out_e = oracle.dslash_half(dims, U, 0, in_o)
+    assert rel(out_o.reshape(-1), D_oe @ in_e.reshape(-1)) < 1e-14
+    assert rel(out_e.reshape(-1), D_eo @ in_o.reshape(-1)) < 1e-14
+    # half <-> full round trip uses idxh = lex // 2 (Eq. 9)
+    lex_e = gen.half_index_of_parity(dims, 0)
+    full = oracle.half_to_full(dims, 0, in_e)
+    assert np.array_equal(full[lex_e], in_e)
+    assert np.abs(np.delete(full, lex_e, axis=0)).max() == 0.0
+    assert np.array_equal(oracle.full_to_half(dims, 0, full), in_e)
+
+
+# ----------------------------------------------------------------------------------------------
+# Closed forms
+# ----------------------------------------------------------------------------------------------
+def test_free_field_plane_wave_spectrum():
+    """U=1: every plane wave on even sites is an eigenvector of A with eigenvalue
+    m^2 + sum_mu sin^2 p_mu, p_{0,1,2} = 2 pi n/N, p_3 = (2n+1) pi/N3 (antiperiodic).
+    Catches a missing 1/2 (x4), a wrong phase convention, a wrong BC."""
+    dims = (4, 4, 6, 4)
+    U = gen.unit_links(dims)
+    m = 0.37
+    coords = gen.site_coords(dims)
+    lex_e = gen.half_index_of_parity(dims, 0)
+    xe = coords[lex_e]
+    colour = np.array([0.3 - 0.2j, 1.0 + 0.5j, -0.7j])
+    worst = 0.0
+    for n in [(0, 0, 0, 0), (1, 0, 0, 0), (0, 1, 2, 1), (3, 2, 5, 3), (2, 3, 1, 2), (1, 1, 1, 0)]:
+        p = np.array([2 * np.pi * n[0] / dims[0], 2 * np.pi * n[1] / dims[1],
+                      2 * np.pi * n[2] / dims[2], (2 * n[3] + 1) * np.pi / dims[3]])
+        phi = np.exp(1j * (xe @ p))[:, None] * colour[None, :]
+        lam = m * m + np.sum(np.sin(p) ** 2)
+        out = oracle.mdagm(dims, U, m, phi)
+        worst = max(worst, rel(out, lam * phi))
+    assert worst < 1e-13
+    # periodic variant: p_3 = 2 pi n / N3
+    p = np.array([2 * np.pi / 4, 0.0, 2 * np.pi * 2 / 6, 2 * np.pi * 3 / 4])
+    phi = np.exp(1j * (xe @ p))[:, None] * colour[None, :]
+    out = oracle.mdagm(dims, U, m, phi, antiperiodic_t=False)
+    assert rel(out, (m * m + np.sum(np.sin(p) ** 2)) * phi) < 1e-13
+
+
+def test_constant_spinor_boundary_closed_form():
+    """U=1, psi = constant c: (D psi)(x) = +eta_3(x) c at x3=0, -eta_3(x) c at x3=N3-1,
+    0 elsewhere; identically 0 with periodic BC.  Catches a sign or slice error in the BC."""
+    dims = (4, 2, 4, 6)
+    U = gen.unit_links(dims)
+    c = np.array([1.0 + 2.0j, -0.5j, 0.25])
+    V = gen.volume(dims)
+    psi = np.tile(c, (V, 1))
+    coords = gen.site_coords(dims)
+    eta3 = (-1.0) ** (coords[:, 0] + coords[:, 1] + coords[:, 2])
+    want = np.zeros((V, 3), dtype=np.complex128)
+    want[coords[:, 3] == 0] = (eta3[coords[:, 3] == 0])[:, None] * c
+    want[coords[:, 3] == dims[3] - 1] = -(eta3[coords[:, 3] == dims[3] - 1])[:, None] * c
+    got = oracle.dirac_full(dims, U, psi, antiperiodic_t=True)
+    assert np.abs(got - want).max() == 0.0
+    assert np.abs(oracle.dirac_full(dims, U, psi, antiperiodic_t=False)).max() == 0.0
+
+
+# ----------------------------------------------------------------------------------------------
+# Invariants
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 2, 8)])
+def test_antihermiticity_D_oe_dagger_is_minus_D_eo(dims):
+    """<phi, D_eo psi> + <D_oe phi, psi> = 0 (Eq. 7), real and imaginary parts."""
+    rng = np.random.default_rng(11)
+    U = gen.smooth_links(dims, 0.5, rng)
+    phi_e = gen.gaussian_half_spinor(dims, rng)
+    psi_o = gen.gaussian_half_spinor(dims, rng)
+    lhs = np.vdot(phi_e, oracle.dslash_half(dims, U, 0, psi_o))
+    rhs = np.vdot(oracle.dslash_half(dims, U, 1, phi_e), psi_o)
+    scale = np.linalg.norm(phi_e) * np.linalg.norm(psi_o)
+    assert abs(lhs + rhs) / scale < 1e-13
+    assert abs(lhs) / scale > 1e-4  # the identity is not vacuous
+
+
+def test_gauge_covariance():
+    """U'_mu(x) = g(x) U_mu(x) g(x+mu)^dagger, psi' = g psi  =>  D[U'] psi' = g D[U] psi."""
+    dims = (4, 4, 4, 6)
+    rng = np.random.default_rng(5)
+    U = gen.smooth_links(dims, 0.3, rng)
+    psi = gen.gaussian_spinor(dims, rng)
+    V = gen.volume(dims)
+    g = gen.haar_like_links(dims, rng)[:, 0]           # one SU(3) per site
+    coords = gen.site_coords(dims)
+    Up = np.empty_like(U)
+    for mu in range(4):
+        fwd = coords.copy()
+        fwd[:, mu] = (fwd[:, mu] + 1) % dims[mu]
+        lex_f = fwd[:, 0] + dims[0] * (fwd[:, 1] + dims[1] * (fwd[:, 2] + dims[2] * fwd[:, 3]))
+        Up[:, mu] = np.einsum("nab,nbc,ndc->nad", g, U[:, mu], g[lex_f].conj())
+    psip = np.einsum("nab,nb->na", g, psi)
+    lhs = oracle.dirac_full(dims, Up, psip)
+    rhs = np.einsum("nab,nb->na", g, oracle.dirac_full(dims, U, psi))
+    assert rel(lhs, rhs) < 1e-13
+    assert V == psi.shape[0]
+
+
+def test_normal_operator_positive_definite_and_matches_dense():
+    """A = m^2 - D_eo D_oe: Hermitian, eigenvalues >= m^2; oracle.mdagm = dense A."""
+    dims = (4, 4, 4, 4)
+    rng = np.random.default_rng(3)
+    U = gen.haar_like_links(dims, rng)
+    m = 0.05
+    A, _, _ = dense_normal_operator(dims, U, m)
+    assert np.abs(A - A.conj().T).max() < 1e-14
+    ev = np.linalg.eigvalsh(A)
+    assert ev.min() >= m * m * (1 - 1e-9)
+    v = gen.gaussian_half_spinor(dims, rng)
+    assert rel(oracle.mdagm(dims, U, m, v).reshape(-1), A @ v.reshape(-1)) < 1e-13
+    assert rel(oracle.mdagm(dims, U, m, v, sigma=0.7).reshape(-1), (A + 0.7 * np.eye(A.shape[0])) @ v.reshape(-1)) < 1e-13
+
+
+def test_norm_ratio_statistical_sanity():
+    """Gaussian psi: ||D psi||^2 / ||psi||^2 ~ 2 (8 hops x (1/2)^2) -- sanity, loose."""
+    dims = (4, 4, 4, 4)
+    rng = np.random.default_rng(9)
+    U = gen.haar_like_links(dims, rng)
+    psi = gen.gaussian_spinor(dims, rng)
+    ratio = np.linalg.norm(oracle.dirac_full(dims, U, psi)) ** 2 / np.linalg.norm(psi) ** 2
+    assert 1.7 < ratio < 2.3
+
+
+# ----------------------------------------------------------------------------------------------
+# Row-3 reconstruction
+# ----------------------------------------------------------------------------------------------
+def test_row3_reconstruction_against_generator():
+    """The generators fix det=1 by a phase on the Gram-Schmidt row 2 (no wedge product), so
+    r2 = (r0 ^ r1)^* must reproduce their row 2 to round-off."""
+    dims = (4, 4, 2, 2)
+    for U in (gen.haar_like_links(dims, 21), gen.smooth_links(dims, 0.5, 22)):
+        R = oracle.reconstruct_row3(U)
+        assert np.array_equal(R[..., :2, :], U[..., :2, :])
+        assert np.abs(R[..., 2, :] - U[..., 2, :]).max() < 5e-15
+        eye = np.einsum("nmab,nmcb->nmac", R, R.conj())
+        assert np.abs(eye - np.eye(3)).max() < 5e-15
+        assert np.abs(np.linalg.det(R) - 1.0).max() < 5e-15
+    # and a hand example: rows e0, e1 -> e2 ; rows (i e0), e1 -> conj(i) e2 = -i e2
+    M = np.zeros((1, 3, 3), dtype=np.complex128)
+    M[0, 0, 0] = 1j
+    M[0, 1, 1] = 1.0
+    assert np.allclose(oracle.reconstruct_row3(M)[0, 2], [0, 0, -1j])
+
+
+# ----------------------------------------------------------------------------------------------
+# CG (reading R10) and multi-shift CG (reading R11)
+# ----------------------------------------------------------------------------------------------
+def test_cg_against_dense_solve():
+    dims = (4, 4, 4, 4)
+    rng = np.random.default_rng(2)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m = 0.1
+    A, _, _ = dense_normal_operator(dims, U, m)
+    x_dense = np.linalg.solve(A, b.reshape(-1))
+    res = oracle.cg(dims, U, m, b, 1e-12, 2000, hist_len=2000)
+    assert res["converged"]
+    assert res["true_relres"] < 5e-12
+    assert rel(res["x"].reshape(-1), x_dense) < 1e-9
+    # the recursive residual history is what the stopping rule saw
+    k = res["iters"]
+    assert res["rnorm"][k - 1] <= 1e-12 * np.linalg.norm(b)
+    assert res["rnorm"][k - 2] > 1e-12 * np.linalg.norm(b)
+    # A-norm of the error decreases monotonically (textbook CG property): replay with max_iter
+    errs = []
+    for it in (1, 2, 3, 5, 8, 13):
+        xi = oracle.cg(dims, U, m, b, 1e-30, it)["x"].reshape(-1)
+        e = xi - x_dense
+        errs.append(np.real(np.vdot(e, A @ e)))
+    assert all(errs[i + 1] < errs[i] for i in range(len(errs) - 1))
+
+
+def test_cg_first_step_closed_form():
+    """alpha_0 = <b,b>/<b,Ab>, x_1 = alpha_0 b, beta_0 = |r_1|^2/|b|^2 -- against the dense A."""
+    dims = (2, 2, 2, 2)
+    rng = np.random.default_rng(4)
+    U = gen.haar_like_links(dims, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m = 0.3
+    A, _, _ = dense_normal_operator(dims, U, m)
+    bv = b.reshape(-1)
+    a0 = np.real(np.vdot(bv, bv)) / np.real(np.vdot(bv, A @ bv))
+    r1 = bv - a0 * (A @ bv)
+    res = oracle.cg(dims, U, m, b, 1e-30, 2, hist_len=2)
+    assert abs(res["alpha"][0] - a0) < 1e-14 * abs(a0)
+    assert abs(res["rnorm"][0] - np.linalg.norm(r1)) < 1e-13 * np.linalg.norm(r1)
+    assert abs(res["beta"][0] - np.vdot(r1, r1).real / np.vdot(bv, bv).real) < 1e-13
+    x1 = oracle.cg(dims, U, m, b, 1e-30, 1)["x"].reshape(-1)
+    assert rel(x1, a0 * bv) < 1e-15
+
+
+def test_cg_exact_termination_and_special_cases():
+    # 2^4: dim = 24; in exact arithmetic CG terminates within 24 iterations, in fp64 loss of
+    # orthogonality costs a few more at tol 1e-10
+    dims = (2, 2, 2, 2)
+    rng = np.random.default_rng(6)
+    U = gen.haar_like_links(dims, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    res = oracle.cg(dims, U, 0.5, b, 1e-10, 100)
+    assert res["converged"] and res["iters"] <= 24 + 4
+    # free field + plane-wave rhs: an eigenvector -> exactly 1 iteration, x = b / lambda
+    dims = (4, 4, 4, 4)
+    Uf = gen.unit_links(dims)
+    xe = gen.site_coords(dims)[gen.half_index_of_parity(dims, 0)]
+    p = np.array([2 * np.pi / 4, 0.0, 2 * np.pi * 2 / 4, 3 * np.pi / 4])
+    bw = np.exp(1j * (xe @ p))[:, None] * np.array([1.0, 2.0j, -0.5])[None, :]
+    m = 0.2
+    res = oracle.cg(dims, Uf, m, bw, 1e-12, 50)
+    assert res["iters"] == 1
+    assert rel(res["x"], bw / (m * m + np.sum(np.sin(p) ** 2))) < 1e-13
+    # m -> infinity: x -> b / m^2
+    b2 = gen.gaussian_half_spinor(dims, rng)
+    res = oracle.cg(dims, Uf, 1e4, b2, 1e-12, 50)
+    assert rel(res["x"], b2 / 1e8) < 1e-7
+    # zero rhs
+    res = oracle.cg(dims, Uf, m, np.zeros_like(b2), 1e-12, 50)
+    assert res["iters"] == 0 and np.abs(res["x"]).max() == 0.0
+    # max_iter reached is reported, not hidden
+    res = oracle.cg(dims, gen.smooth_links(dims, 0.5, 8), 0.01, b2, 1e-14, 3)
+    assert not res["converged"] and res["iters"] == 3
+
+
+def test_multishift_against_dense_and_single_shift():
+    dims = (4, 4, 4, 4)
+    rng = np.random.default_rng(4)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m = 0.05
+    shifts = np.array([0.3, 1e-3, 1.0, 0.02])        # unsorted on purpose: base = the minimum
+    A, _, _ = dense_normal_operator(dims, U, m)
+    res = oracle.cg_multishift(dims, U, m, shifts, b, 1e-11, 5000)
+    assert res["converged"]
+    eye = np.eye(A.shape[0])
+    for i, s in enumerate(shifts):
+        xd = np.linalg.solve(A + s * eye, b.reshape(-1))
+        assert rel(res["x"][i].reshape(-1), xd) < 1e-8
+        assert res["true_relres"][i] < 3e-11
+    # larger shifts freeze earlier (zeta_i decreases faster for larger delta_i)
+    order = np.argsort(shifts)
+    assert all(res["conv_iter"][order[j]] >= res["conv_iter"][order[j + 1]] for j in range(3))
+    assert res["conv_iter"].max() == res["iters"]
+    # single-shift CG on A + sigma == CG with mass^2 -> m^2 + sigma
+    s = shifts[0]
+    single = oracle.cg(dims, U, np.sqrt(m * m + s), b, 1e-11, 5000)
+    assert rel(res["x"][0], single["x"]) < 1e-8
+    assert abs(single["iters"] - res["conv_iter"][0]) <= 2
+
+
+def test_multishift_residual_identity_and_first_zeta():
+    """b - (A + sigma_i) x_i = zeta_i r while shift i is active; zeta_i after step 0 =
+    1/(1 + delta_i alpha_0).  Catches any slip in the zeta/alpha_i/beta_i recurrences."""
+    dims = (4, 4, 2, 4)
+    rng = np.random.default_rng(12)
+    U = gen.smooth_links(dims, 0.4, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m = 0.03
+    shifts = gen.rhmc_shifts(8)
+    assert np.allclose(shifts[[0, 1, 7]], [1e-4, 3.72759372e-4, 1.0])
+    bn = np.linalg.norm(b)
+    for it in (1, 2, 3, 7, 20):
+        res = oracle.cg_multishift(dims, U, m, shifts, b, 1e-30, it, hist_len=it)
+        assert res["iters"] == it and not res["converged"]
+        for i, s in enumerate(shifts):
+            true_r = b - oracle.mdagm(dims, U, m, res["x"][i], sigma=s)
+            assert np.linalg.norm(true_r - res["zeta"][i] * res["r"]) < 1e-12 * bn
+        if it == 1:
+            a0 = res["alpha"][0]
+            assert np.allclose(res["zeta"], 1.0 / (1.0 + (shifts - shifts.min()) * a0), rtol=1e-14)
+    # the base system's alpha/beta/|r| history is plain CG on A + sigma_min
+    ms = oracle.cg_multishift(dims, U, m, shifts, b, 1e-30, 10, hist_len=10)
+    sg = oracle.cg(dims, U, np.sqrt(m * m + shifts.min()), b, 1e-30, 10, hist_len=10)
+    assert np.allclose(ms["alpha"], sg["alpha"], rtol=1e-10)
+    assert np.allclose(ms["rnorm"], sg["rnorm"], rtol=1e-10)
+    assert np.allclose(ms["beta"][:9], sg["beta"][:9], rtol=1e-10)
+
+
+def test_multishift_rejects_bad_shifts():
+    dims = (2, 2, 2, 2)
+    U = gen.unit_links(dims)
+    b = gen.gaussian_half_spinor(dims, 1)
+    with pytest.raises(ValueError):
+        oracle.cg_multishift(dims, U, 0.1, [0.1, -0.2], b, 1e-8, 10)
