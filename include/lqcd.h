@@ -1,0 +1,170 @@
+/*
+ * lqcd.h -- C ABI of the B200-native staggered Dslash / CG / multi-shift CG library
+ *           (liblqcd_b200.so, built from paper_1701_00426_b200/csrc/ for sm_100a).
+ *
+ * The calls follow the paper's statement of the problem (arxiv/paper_1701_00426, cited as
+ * PAPER.md:LINE):
+ *   - lqcd_dslash          : D_eo / D_oe of Eq. 7; the paper's
+ *                            acc_Deo(u, out, in, backfield) of Listing 2
+ *   - lqcd_mdagm           : m^2 - D_eo D_oe of Eq. 8
+ *   - lqcd_cg              : "the conjugate gradient" on Eq. 8
+ *   - lqcd_cg_multishift   : the "multishift inverter routine" for Eq. 6
+ *
+ *   - lqcd_pack_* / unpack : canonical <-> native SoA, parity-split fields (PAPER.md:245-272,
+ *                            Figs 1-2, Eq. 9) with optional 2-row ("12-real") links whose third
+ *                            row is rebuilt in registers as r2 = (r0 ^ r1)^*
+ * What the paper leaves unstated (stencil, phases, boundary conditions, CG recurrences) is
+ * fixed by the readings R1..R19 of DESIGN.md.
+ *
+ * General conventions
+ *   - Plain C; no torch / C++ types.  Every function returns an int status (LQCD_OK = 0) unless
+ *     stated otherwise.  No exceptions, no abort(), nothing written to stdout/stderr.
+ *   - "dev" pointers are CUDA device pointers on the context's device, >= 16-byte aligned,
+ *     owned by the caller (e.g. torch.empty(...).data_ptr()).  The library never allocates or
+ *     frees field memory; it owns only the context (host struct, < 64 KiB of device scalars,
+ *     one pinned flag word).  "host" pointers are ordinary host memory (pinned or not).
+ *   - All device work is enqueued on the CUDA stream given to lqcd_create.  Functions marked
+ *     "async" return after enqueueing; functions marked "blocking" synchronise that stream.
+ *   - out/in buffers of one call must not alias unless stated.
+ *   - Errors: bad arguments are detected before any launch (LQCD_ERR_ARG / _WORKSPACE);
+ *     CUDA failures give LQCD_ERR_CUDA; lqcd_last_error() returns a message.
+ *
+ * Canonical layout (interchange format; identical to lqcd_inputs/fields.py and the oracle):
+ *   lex   = x0 + N0*(x1 + N1*(x2 + N2*x3))                       (numerator of Eq. 9)
+ *   links : complex128 U[lex][mu][row][col], mu = 0..3, row-major 3x3 (rows = r0,r1,r2)
+ *   half spinor of parity p = (x0+x1+x2+x3)%2 : complex128 phi[idxh][c], idxh = lex/2  (Eq. 9)
+ * Canonical arrays are ALWAYS complex128, also for an LQCD_F32 context (packing rounds to
+ * nearest; unpacking widens exactly).
+ *
+ * Native layout: private to the library; sizes from
+ * lqcd_spinor_bytes / lqcd_links_bytes.
+ */
+#ifndef LQCD_H
+#define LQCD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lqcd_ctx lqcd_ctx; /* opaque, library-owned */
+
+enum { LQCD_OK = 0, LQCD_ERR_ARG = 1, LQCD_ERR_UNSUPPORTED = 2, LQCD_ERR_CUDA = 3,
+       LQCD_ERR_NOT_CONVERGED = 4, LQCD_ERR_WORKSPACE = 5 };
+enum { LQCD_F64 = 0, LQCD_F32 = 1 };          /* arithmetic and storage type of native fields */
+enum { LQCD_RECON_18 = 0, LQCD_RECON_12 = 1 };/* links stored as 3 rows / 2 rows */
+enum { LQCD_EVEN = 0, LQCD_ODD = 1 };         /* parity of the OUTPUT sites (reading R5)        */
+#define LQCD_MAX_SHIFTS 32
+
+/* Library version string (static storage). */
+const char *lqcd_version(void);
+
+/*
+ * Create a context.
+ *   dims            N0..N3 (x0 fastest), each even and >= 2 (PAPER.md:249 and footnote d);
+ *                   N0*N1*N2*N3 < 2^31
+ *   prec            LQCD_F64 | LQCD_F32   (single-precision variants)
+ *   recon           LQCD_RECON_18 | LQCD_RECON_12
+ *   antiperiodic_t  1: fermion field antiperiodic across the x3 boundary (reading R4), 0: periodic
+ *   device          CUDA device ordinal
+ *   cuda_stream     a cudaStream_t (as void*), or NULL for the legacy default stream
+ * Errors: LQCD_ERR_ARG (null ctx, bad dims/enums), LQCD_ERR_CUDA (no device / allocation).
+ */
+int lqcd_create(lqcd_ctx **ctx, const int dims[4], int prec, int recon, int antiperiodic_t,
+                int device, void *cuda_stream);
+int lqcd_destroy(lqcd_ctx *ctx); /* blocking; frees only library-owned memory */
+
+/* Message for the last non-OK status returned with this context ("" if none).
+ * With ctx == NULL: message of the last failed lqcd_create on this thread. */
+const char *lqcd_last_error(const lqcd_ctx *ctx);
+
+/*
+ * Private tuning knobs (block sizes, layout variant, cache policy); see DESIGN.md "Tuning".
+ * Unknown names -> LQCD_ERR_ARG.  "layout" may only be changed before any field is packed.
+ */
+int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value);
+long lqcd_get_option(const lqcd_ctx *ctx, const char *name); /* -1 if unknown */
+
+/* Sizes in bytes of native buffers the caller must allocate (0 if ctx is NULL). */
+size_t lqcd_spinor_bytes(const lqcd_ctx *ctx); /* one half-lattice colour vector              */
+size_t lqcd_links_bytes(const lqcd_ctx *ctx);  /* whole link field, both parities, 4 directions */
+size_t lqcd_workspace_bytes(const lqcd_ctx *ctx, int nshift); /* solver workspace, nshift>=1   */
+
+/* Hand the solvers (and lqcd_mdagm) a caller-owned device workspace of >= lqcd_workspace_bytes
+ * bytes for the largest nshift that will be used.  Errors: LQCD_ERR_ARG, LQCD_ERR_WORKSPACE. */
+int lqcd_set_workspace(lqcd_ctx *ctx, void *dev_ptr, size_t bytes);
+
+/* Canonical <-> native, on the device.  async. */
+int lqcd_pack_links(lqcd_ctx *ctx, void *native_dev, const void *canonical_dev /* c128 [V][4][3][3] */);
+int lqcd_pack_spinor(lqcd_ctx *ctx, int parity, void *native_dev, const void *canonical_dev /* c128 [V/2][3] */);
+int lqcd_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical_dev, const void *native_dev);
+
+/*
+ * out = D in on the sites of `parity` (Eq. 7; readings R1-R5):
+ *   (D psi)(x) = 1/2 sum_mu eta_mu(x) [ s+ U_mu(x) psi(x+mu) - s- U_mu(x-mu)^dagger psi(x-mu) ]
+ * parity = LQCD_EVEN: out_e = D_eo in_o;  parity = LQCD_ODD: out_o = D_oe in_e.
+ * out, in: native half spinors (device); links: native link field (device).  async.
+ * Errors: LQCD_ERR_ARG (null pointer, parity not 0/1, out == in), LQCD_ERR_CUDA.
+ */
+int lqcd_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links);
+
+/*
+ * out_e = (mass^2 + sigma) in_e - D_eo (D_oe in_e)   (Eq. 8, shifted as in Eq. 6).
+ * Needs a workspace (one odd-site temporary).  async.
+ */
+int lqcd_mdagm(lqcd_ctx *ctx, void *out_e, const void *in_e, const void *links, double mass,
+               double sigma);
+
+/*
+ * Solve (mass^2 - D_eo D_oe) x_e = b_e by CG from x = 0 until ||r|| <= tol ||b|| (reading R10).
+ *   x_e, b_e    native even-site vectors (device)
+ *   iters       host, out: iterations performed (may be NULL)
+ *   rel_resid   host, out: TRUE residual ||b - A x|| / ||b|| recomputed at exit (may be NULL)
+ * blocking.  Returns LQCD_ERR_NOT_CONVERGED when max_iter is hit (outputs still filled, x at the
+ * last iterate); LQCD_ERR_ARG for tol <= 0, max_iter < 1, null pointers; LQCD_ERR_WORKSPACE.
+ */
+int lqcd_cg(lqcd_ctx *ctx, void *x_e, const void *b_e, const void *links, double mass,
+            double tol, int max_iter, int *iters, double *rel_resid);
+
+/*
+ * Solve (mass^2 + shifts[i] - D_eo D_oe) x_i = rhs_e for i = 0..nshift-1 with ONE operator
+ * application per iteration (reading R11): shift i is frozen (sticky) once
+ * |zeta_i| ||r|| <= tol ||rhs||; the loop ends when every shift is frozen.
+ *   shifts        host, nshift doubles >= 0, any order; 1 <= nshift <= LQCD_MAX_SHIFTS
+ *   rhs_e         native even-site vector (device)
+ *   solutions_e   host array of nshift device pointers to native even-site vectors (out)
+ *   iters         host, out: total iterations (may be NULL)
+ *   conv_iter     host, out [nshift]: iteration at which each shift froze (may be NULL)
+ *   rel_resid     host, out [nshift]: TRUE residuals at exit (may be NULL)
+ * blocking.  Error behaviour as lqcd_cg; a negative shift is LQCD_ERR_ARG.
+ */
+int lqcd_cg_multishift(lqcd_ctx *ctx, int nshift, const double *shifts, const void *rhs_e,
+                       void *const *solutions_e, const void *links, double mass, double tol,
+                       int max_iter, int *iters, int *conv_iter, double *rel_resid);
+
+/*
+ * After lqcd_cg / lqcd_cg_multishift: copy up to `n` entries of the per-iteration history
+ * (alpha_k, beta_k, ||r_{k+1}||) of the last solve to host arrays (any may be NULL).
+ * Returns the number of entries available (<= 64), or a negative status.
+ */
+int lqcd_solver_history(lqcd_ctx *ctx, int n, double *alpha, double *beta, double *rnorm);
+
+/*
+ * End-to-end entry points on HOST buffers in the canonical layout: host->device copy, pack,
+ * compute on the GPU, unpack, device->host copy, all inside the call.  blocking.
+ * They allocate and free their own device staging memory (cudaMalloc), unlike the calls above.
+ */
+int lqcd_dslash_host(lqcd_ctx *ctx, int parity, void *out_host /* c128 [V/2][3] */,
+                     const void *in_host /* c128 [V/2][3] */,
+                     const void *links_host /* c128 [V][4][3][3] */);
+int lqcd_cg_multishift_host(lqcd_ctx *ctx, int nshift, const double *shifts,
+                            const void *rhs_host /* c128 [V/2][3] */,
+                            void *solutions_host /* c128 [nshift][V/2][3] */,
+                            const void *links_host, double mass, double tol, int max_iter,
+                            int *iters, int *conv_iter, double *rel_resid);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQCD_H */

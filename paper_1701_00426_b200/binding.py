@@ -1,0 +1,240 @@
+"""ctypes binding of include/lqcd.h -- same names, argument marshalling only.
+
+`lib` is the raw ctypes handle (lib.lqcd_dslash(...) etc. with C signatures).  `Lattice` is a
+small convenience wrapper that owns a context plus the torch tensors used as device memory; it
+does no arithmetic.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+lib_path = os.path.join(HERE, "liblqcd_b200.so")
+
+OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOT_CONVERGED, ERR_WORKSPACE = range(6)
+F64, F32 = 0, 1
+RECON_18, RECON_12 = 0, 1
+EVEN, ODD = 0, 1
+MAX_SHIFTS = 32
+
+
+class LqcdError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"lqcd error {code}: {msg}")
+        self.code = code
+
+
+def _load():
+    if not os.path.exists(lib_path):
+        raise ImportError(
+            f"{lib_path} is missing: build it with `python -m paper_1701_00426_b200.build` "
+            "(or __graft_entry__.build()).  There is no fallback path.")
+    return C.CDLL(lib_path)
+
+
+lib = _load()
+
+_vp, _i, _d, _sz = C.c_void_p, C.c_int, C.c_double, C.c_size_t
+_pi, _pd = C.POINTER(C.c_int), C.POINTER(C.c_double)
+_sig = {
+    "lqcd_version": (C.c_char_p, []),
+    "lqcd_create": (_i, [C.POINTER(_vp), C.POINTER(_i), _i, _i, _i, _i, _vp]),
+    "lqcd_destroy": (_i, [_vp]),
+    "lqcd_last_error": (C.c_char_p, [_vp]),
+    "lqcd_set_option": (_i, [_vp, C.c_char_p, C.c_long]),
+    "lqcd_get_option": (C.c_long, [_vp, C.c_char_p]),
+    "lqcd_spinor_bytes": (_sz, [_vp]),
+    "lqcd_links_bytes": (_sz, [_vp]),
+    "lqcd_workspace_bytes": (_sz, [_vp, _i]),
+    "lqcd_set_workspace": (_i, [_vp, _vp, _sz]),
+    "lqcd_pack_links": (_i, [_vp, _vp, _vp]),
+    "lqcd_pack_spinor": (_i, [_vp, _i, _vp, _vp]),
+    "lqcd_unpack_spinor": (_i, [_vp, _i, _vp, _vp]),
+    "lqcd_dslash": (_i, [_vp, _i, _vp, _vp, _vp]),
+    "lqcd_mdagm": (_i, [_vp, _vp, _vp, _vp, _d, _d]),
+    "lqcd_cg": (_i, [_vp, _vp, _vp, _vp, _d, _d, _i, _pi, _pd]),
+    "lqcd_cg_multishift": (_i, [_vp, _i, _pd, _vp, C.POINTER(_vp), _vp, _d, _d, _i, _pi, _pi, _pd]),
+    "lqcd_solver_history": (_i, [_vp, _i, _pd, _pd, _pd]),
+    "lqcd_dslash_host": (_i, [_vp, _i, _vp, _vp, _vp]),
+    "lqcd_cg_multishift_host": (_i, [_vp, _i, _pd, _vp, _vp, _vp, _d, _d, _i, _pi, _pi, _pd]),
+}
+for _name, (_res, _args) in _sig.items():
+    _f = getattr(lib, _name)
+    _f.restype = _res
+    _f.argtypes = _args
+
+
+def version() -> str:
+    return lib.lqcd_version().decode()
+
+
+class Lattice:
+    """One lqcd context plus torch tensors as device memory.  Marshalling only.
+
+    All numpy arguments / results are complex128 arrays in the canonical layout
+    (include/lqcd.h).  Native device buffers are opaque uint8 torch tensors.
+    """
+
+    def __init__(self, dims, prec=F64, recon=RECON_18, antiperiodic_t=True, device=0, options=None):
+        import torch  # device memory and streams only
+
+        if not torch.cuda.is_available():
+            raise LqcdError(ERR_CUDA, "no CUDA device: the lqcd_b200 path has no CPU fallback")
+        self.torch = torch
+        self.dims = tuple(int(d) for d in dims)
+        self.prec, self.recon = prec, recon
+        self.device = torch.device("cuda", device)
+        torch.cuda.set_device(self.device)
+        self.stream = torch.cuda.current_stream(self.device)
+        self._ctx = _vp()
+        rc = lib.lqcd_create(C.byref(self._ctx), (C.c_int * 4)(*self.dims), prec, recon,
+                             int(bool(antiperiodic_t)), device, _vp(self.stream.cuda_stream))
+        if rc:
+            raise LqcdError(rc, lib.lqcd_last_error(None).decode())
+        for k, v in (options or {}).items():
+            self.set_option(k, v)
+        self.V = self.dims[0] * self.dims[1] * self.dims[2] * self.dims[3]
+        self.Vh = self.V // 2
+        self._ws = None
+        self._ws_shifts = 0
+
+    # -- plumbing ------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_ctx", None):
+            lib.lqcd_destroy(self._ctx)
+            self._ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, allow=()):
+        if rc and rc not in allow:
+            raise LqcdError(rc, lib.lqcd_last_error(self._ctx).decode())
+        return rc
+
+    def set_option(self, name, value):
+        self._check(lib.lqcd_set_option(self._ctx, name.encode(), int(value)))
+
+    def get_option(self, name):
+        return int(lib.lqcd_get_option(self._ctx, name.encode()))
+
+    @property
+    def launches(self):
+        return self.get_option("launches")
+
+    @property
+    def spinor_bytes(self):
+        return int(lib.lqcd_spinor_bytes(self._ctx))
+
+    @property
+    def links_bytes(self):
+        return int(lib.lqcd_links_bytes(self._ctx))
+
+    def _buf(self, nbytes):
+        return self.torch.empty(nbytes, dtype=self.torch.uint8, device=self.device)
+
+    def new_spinor(self):
+        return self._buf(self.spinor_bytes)
+
+    def ensure_workspace(self, nshift=1):
+        if self._ws is None or nshift > self._ws_shifts:
+            self._ws = self._buf(int(lib.lqcd_workspace_bytes(self._ctx, nshift)))
+            self._ws_shifts = nshift
+            self._check(lib.lqcd_set_workspace(self._ctx, _vp(self._ws.data_ptr()), self._ws.numel()))
+
+    def synchronize(self):
+        self.stream.synchronize()
+
+    # -- canonical <-> native ----------------------------------------------------------------
+    def _to_dev(self, arr):
+        import numpy as np
+        a = np.ascontiguousarray(arr, dtype=np.complex128)
+        return self.torch.from_numpy(a.view(np.float64).reshape(-1)).to(self.device)
+
+    def pack_links(self, U):
+        """U: complex128 [V][4][3][3] (numpy) -> native device buffer."""
+        assert U.shape == (self.V, 4, 3, 3)
+        canon = self._to_dev(U)
+        native = self._buf(self.links_bytes)
+        self._check(lib.lqcd_pack_links(self._ctx, _vp(native.data_ptr()), _vp(canon.data_ptr())))
+        self.synchronize()
+        return native
+
+    def pack_spinor(self, phi, parity):
+        assert phi.shape == (self.Vh, 3)
+        canon = self._to_dev(phi)
+        native = self.new_spinor()
+        self._check(lib.lqcd_pack_spinor(self._ctx, parity, _vp(native.data_ptr()), _vp(canon.data_ptr())))
+        self.synchronize()
+        return native
+
+    def unpack_spinor(self, native, parity):
+        import numpy as np
+        canon = self.torch.empty(self.Vh * 6, dtype=self.torch.float64, device=self.device)
+        self._check(lib.lqcd_unpack_spinor(self._ctx, parity, _vp(canon.data_ptr()), _vp(native.data_ptr())))
+        self.synchronize()
+        return canon.cpu().numpy().view(np.complex128).reshape(self.Vh, 3)
+
+    # -- the hot path (async unless stated) ---------------------------------------------------
+    def dslash(self, parity, out, inp, links):
+        self._check(lib.lqcd_dslash(self._ctx, parity, _vp(out.data_ptr()), _vp(inp.data_ptr()), _vp(links.data_ptr())))
+
+    def mdagm(self, out_e, in_e, links, mass, sigma=0.0):
+        self.ensure_workspace(1)
+        self._check(lib.lqcd_mdagm(self._ctx, _vp(out_e.data_ptr()), _vp(in_e.data_ptr()), _vp(links.data_ptr()), mass, sigma))
+
+    def cg(self, x_e, b_e, links, mass, tol, max_iter, raise_on_max_iter=True):
+        """blocking; returns dict(iters, rel_resid, converged)."""
+        self.ensure_workspace(1)
+        iters, res = C.c_int(0), C.c_double(0.0)
+        rc = self._check(lib.lqcd_cg(self._ctx, _vp(x_e.data_ptr()), _vp(b_e.data_ptr()), _vp(links.data_ptr()),
+                                     mass, tol, max_iter, C.byref(iters), C.byref(res)),
+                         allow=() if raise_on_max_iter else (ERR_NOT_CONVERGED,))
+        return dict(iters=iters.value, rel_resid=res.value, converged=(rc == OK))
+
+    def cg_multishift(self, xs, b_e, links, mass, shifts, tol, max_iter, raise_on_max_iter=True):
+        """blocking; xs: list of native even-site buffers (outputs)."""
+        import numpy as np
+        n = len(xs)
+        self.ensure_workspace(n)
+        sh = np.ascontiguousarray(shifts, dtype=np.float64)
+        assert sh.size == n
+        ptrs = (_vp * n)(*[x.data_ptr() for x in xs])
+        iters = C.c_int(0)
+        conv = (C.c_int * n)()
+        res = np.zeros(n)
+        rc = self._check(lib.lqcd_cg_multishift(self._ctx, n, sh.ctypes.data_as(_pd), _vp(b_e.data_ptr()), ptrs,
+                                                _vp(links.data_ptr()), mass, tol, max_iter, C.byref(iters), conv,
+                                                res.ctypes.data_as(_pd)),
+                         allow=() if raise_on_max_iter else (ERR_NOT_CONVERGED,))
+        return dict(iters=iters.value, conv_iter=np.array(list(conv)), rel_resid=res, converged=(rc == OK))
+
+    def solver_history(self):
+        import numpy as np
+        a, b, r = np.zeros(64), np.zeros(64), np.zeros(64)
+        n = lib.lqcd_solver_history(self._ctx, 64, a.ctypes.data_as(_pd), b.ctypes.data_as(_pd), r.ctypes.data_as(_pd))
+        n = max(0, min(n, 64))
+        return dict(alpha=a[:n], beta=b[:n], rnorm=r[:n])
+
+    # -- end-to-end on host buffers (blocking) --------------------------------------------------
+    def dslash_host(self, parity, out_host, in_host, links_host):
+        """numpy complex128 arrays (pinned or not); copies + pack + kernel + unpack inside the call."""
+        self._check(lib.lqcd_dslash_host(self._ctx, parity, _vp(out_host.ctypes.data), _vp(in_host.ctypes.data),
+                                         _vp(links_host.ctypes.data)))
+
+    def cg_multishift_host(self, sol_host, rhs_host, links_host, mass, shifts, tol, max_iter, raise_on_max_iter=True):
+        import numpy as np
+        sh = np.ascontiguousarray(shifts, dtype=np.float64)
+        n = sh.size
+        iters = C.c_int(0)
+        conv = (C.c_int * n)()
+        res = np.zeros(n)
+        rc = self._check(lib.lqcd_cg_multishift_host(self._ctx, n, sh.ctypes.data_as(_pd), _vp(rhs_host.ctypes.data),
+                                                     _vp(sol_host.ctypes.data), _vp(links_host.ctypes.data), mass, tol,
+                                                     max_iter, C.byref(iters), conv, res.ctypes.data_as(_pd)),
+                         allow=() if raise_on_max_iter else (ERR_NOT_CONVERGED,))
+        return dict(iters=iters.value, conv_iter=np.array(list(conv)), rel_resid=res, converged=(rc == OK))

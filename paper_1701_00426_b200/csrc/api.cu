@@ -1,0 +1,233 @@
+// api.cu -- context management, argument checking and the host-buffer entry points of the
+// C ABI declared in include/lqcd.h.  No arithmetic of the method lives here.
+#include <stdarg.h>
+#include <stdlib.h>
+
+#include "common.cuh"
+
+static thread_local char g_create_err[256] = "";
+
+extern "C" const char *lqcd_version(void) { return "lqcd_b200 0.1 (sm_100a)"; }
+
+int lqcd_fail(lqcd_ctx *ctx, int code, const char *fmt, ...)
+{
+    char *dst = ctx ? ctx->err : g_create_err;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 256, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int lqcd_check_cuda(lqcd_ctx *ctx, cudaError_t e, const char *what)
+{
+    if (e == cudaSuccess) return LQCD_OK;
+    return lqcd_fail(ctx, LQCD_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+size_t elem_size(const lqcd_ctx *ctx) { return ctx->prec == LQCD_F64 ? 8 : 4; }
+
+extern "C" const char *lqcd_last_error(const lqcd_ctx *ctx) { return ctx ? ctx->err : g_create_err; }
+
+extern "C" int lqcd_create(lqcd_ctx **out, const int dims[4], int prec, int recon,
+                           int antiperiodic_t, int device, void *cuda_stream)
+{
+    if (!out) return lqcd_fail(NULL, LQCD_ERR_ARG, "lqcd_create: ctx is NULL");
+    *out = NULL;
+    if (!dims) return lqcd_fail(NULL, LQCD_ERR_ARG, "lqcd_create: dims is NULL");
+    long long V = 1;
+    for (int i = 0; i < 4; ++i) {
+        if (dims[i] < 2 || (dims[i] & 1))
+            return lqcd_fail(NULL, LQCD_ERR_ARG, "lqcd_create: dims[%d] = %d must be even and >= 2", i, dims[i]);
+        V *= dims[i];
+        if (V >= (1LL << 31)) return lqcd_fail(NULL, LQCD_ERR_ARG, "lqcd_create: volume must be < 2^31");
+    }
+    if (prec != LQCD_F64 && prec != LQCD_F32) return lqcd_fail(NULL, LQCD_ERR_ARG, "lqcd_create: bad prec %d", prec);
+    if (recon != LQCD_RECON_18 && recon != LQCD_RECON_12)
+        return lqcd_fail(NULL, LQCD_ERR_ARG, "lqcd_create: bad recon %d", recon);
+    if (antiperiodic_t != 0 && antiperiodic_t != 1)
+        return lqcd_fail(NULL, LQCD_ERR_ARG, "lqcd_create: antiperiodic_t must be 0 or 1");
+    if (device < 0) return lqcd_fail(NULL, LQCD_ERR_ARG, "lqcd_create: bad device %d", device);
+
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0)
+        return lqcd_fail(NULL, LQCD_ERR_CUDA, "lqcd_create: no CUDA device (%s); there is no CPU fallback",
+                         cudaGetErrorString(e));
+    if (device >= ndev) return lqcd_fail(NULL, LQCD_ERR_ARG, "lqcd_create: device %d of %d", device, ndev);
+    if ((e = cudaSetDevice(device)) != cudaSuccess) return lqcd_check_cuda(NULL, e, "cudaSetDevice");
+
+    lqcd_ctx *c = (lqcd_ctx *)calloc(1, sizeof(lqcd_ctx));
+    if (!c) return lqcd_fail(NULL, LQCD_ERR_CUDA, "lqcd_create: out of host memory");
+    Geom &g = c->g;
+    g.N0 = dims[0]; g.N1 = dims[1]; g.N2 = dims[2]; g.N3 = dims[3];
+    g.Nh0 = g.N0 / 2;
+    g.Vh = (int)(V / 2);
+    g.s1 = g.Nh0; g.s2 = g.Nh0 * g.N1; g.s3 = g.Nh0 * g.N1 * g.N2;
+    g.ap = antiperiodic_t;
+    g.dNh0 = make_fastdiv((uint32_t)g.Nh0);
+    g.dN1 = make_fastdiv((uint32_t)g.N1);
+    g.dN2 = make_fastdiv((uint32_t)g.N2);
+    c->prec = prec; c->recon = recon; c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->layout = 0;
+    c->dslash_block = 128;
+    c->dslash_minblocks = 0;   // 0: the per-precision default of dslash.cu
+    c->blas_block = 256;
+    c->blas_ctas_per_sm = 8;
+    c->poll_chunk = 8;
+    cudaDeviceProp prop;
+    if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) { free(c); return lqcd_check_cuda(NULL, e, "cudaGetDeviceProperties"); }
+    c->num_sms = prop.multiProcessorCount;
+    c->max_partials = g.Vh / 32 + 1024;   // >= the largest grid any reducing kernel uses
+    if ((e = cudaMalloc(&c->d_state, sizeof(SolverState))) != cudaSuccess ||
+        (e = cudaMalloc(&c->d_partials, sizeof(double) * c->max_partials)) != cudaSuccess ||
+        (e = cudaMallocHost(&c->h_flag, 64)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&c->ev[0], cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaMemset(c->d_state, 0, sizeof(SolverState))) != cudaSuccess) {
+        int rc = lqcd_check_cuda(NULL, e, "lqcd_create: allocating solver state");
+        cudaFree(c->d_state); cudaFree(c->d_partials); if (c->h_flag) cudaFreeHost(c->h_flag);
+        free(c);
+        return rc;
+    }
+    *out = c;
+    return LQCD_OK;
+}
+
+extern "C" int lqcd_destroy(lqcd_ctx *ctx)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    cudaFree(ctx->d_state);
+    cudaFree(ctx->d_partials);
+    cudaFreeHost(ctx->h_flag);
+    cudaEventDestroy(ctx->ev[0]);
+    cudaEventDestroy(ctx->ev[1]);
+    cudaFree(ctx->stage);
+    free(ctx);
+    return LQCD_OK;
+}
+
+struct OptDesc { const char *name; size_t off; long lo, hi; };
+#define OPT(field, lo, hi) { #field, offsetof(lqcd_ctx, field), lo, hi }
+static const OptDesc g_opts[] = {
+    OPT(layout, 0, 1), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
+    OPT(blas_block, 64, 256), OPT(blas_ctas_per_sm, 1, 32), OPT(poll_chunk, 1, 1024),
+};
+
+extern "C" int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value)
+{
+    if (!ctx || !name) return LQCD_ERR_ARG;
+    for (const OptDesc &o : g_opts) {
+        if (strcmp(o.name, name)) continue;
+        if (value < o.lo || value > o.hi) return lqcd_fail(ctx, LQCD_ERR_ARG, "option %s: %ld out of [%ld,%ld]", name, value, o.lo, o.hi);
+        if (!strcmp(name, "layout") && ctx->layout_locked && value != ctx->layout)
+            return lqcd_fail(ctx, LQCD_ERR_ARG, "option layout: fields were already packed in layout %d", ctx->layout);
+        if ((!strcmp(name, "dslash_block") || !strcmp(name, "blas_block")) && (value % 32))
+            return lqcd_fail(ctx, LQCD_ERR_ARG, "option %s must be a multiple of 32", name);
+        *(int *)((char *)ctx + o.off) = (int)value;
+        return LQCD_OK;
+    }
+    return lqcd_fail(ctx, LQCD_ERR_ARG, "unknown option %s", name);
+}
+
+extern "C" long lqcd_get_option(const lqcd_ctx *ctx, const char *name)
+{
+    if (!ctx || !name) return -1;
+    if (!strcmp(name, "launches")) return ctx->launches;
+    if (!strcmp(name, "num_sms")) return ctx->num_sms;
+    for (const OptDesc &o : g_opts)
+        if (!strcmp(o.name, name)) return *(const int *)((const char *)ctx + o.off);
+    return -1;
+}
+
+extern "C" size_t lqcd_spinor_bytes(const lqcd_ctx *ctx)
+{
+    return ctx ? (size_t)ctx->g.Vh * 6 * elem_size(ctx) : 0;
+}
+
+extern "C" size_t lqcd_links_bytes(const lqcd_ctx *ctx)
+{
+    if (!ctx) return 0;
+    size_t rows = ctx->recon == LQCD_RECON_12 ? 2 : 3;
+    return (size_t)ctx->g.Vh * 2 * 4 * rows * 3 * 2 * elem_size(ctx);
+}
+
+// workspace = tmp_o, q, r, p  +  one p_i per shift (the base shift's is unused but keeps indexing
+// simple) ; each rounded up to 256 bytes.
+static size_t vec_stride(const lqcd_ctx *ctx) { return (lqcd_spinor_bytes(ctx) + 255) & ~(size_t)255; }
+
+extern "C" size_t lqcd_workspace_bytes(const lqcd_ctx *ctx, int nshift)
+{
+    if (!ctx || nshift < 1 || nshift > LQCD_MAX_SHIFTS) return 0;
+    return vec_stride(ctx) * (size_t)(4 + nshift);
+}
+
+extern "C" int lqcd_set_workspace(lqcd_ctx *ctx, void *dev_ptr, size_t bytes)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    if (!dev_ptr || ((uintptr_t)dev_ptr & 15)) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_set_workspace: null or unaligned pointer");
+    if (bytes < lqcd_workspace_bytes(ctx, 1)) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "lqcd_set_workspace: %zu bytes < minimum %zu", bytes, lqcd_workspace_bytes(ctx, 1));
+    ctx->ws = dev_ptr;
+    ctx->ws_bytes = bytes;
+    return LQCD_OK;
+}
+
+void *ws_vec(lqcd_ctx *ctx, int k) { return (char *)ctx->ws + vec_stride(ctx) * (size_t)k; }
+
+// ---- thin checked wrappers ------------------------------------------------------------------
+#define REQUIRE(cond, ...) do { if (!(cond)) return lqcd_fail(ctx, LQCD_ERR_ARG, __VA_ARGS__); } while (0)
+
+static int enter(lqcd_ctx *ctx)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    return lqcd_check_cuda(ctx, cudaSetDevice(ctx->device), "cudaSetDevice");
+}
+
+extern "C" int lqcd_pack_links(lqcd_ctx *ctx, void *native_dev, const void *canonical_dev)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(native_dev && canonical_dev, "lqcd_pack_links: null pointer");
+    ctx->layout_locked = 1;
+    return launch_pack_links(ctx, native_dev, canonical_dev);
+}
+
+extern "C" int lqcd_pack_spinor(lqcd_ctx *ctx, int parity, void *native_dev, const void *canonical_dev)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(native_dev && canonical_dev, "lqcd_pack_spinor: null pointer");
+    REQUIRE(parity == 0 || parity == 1, "lqcd_pack_spinor: parity %d", parity);
+    ctx->layout_locked = 1;
+    return launch_pack_spinor(ctx, parity, native_dev, canonical_dev);
+}
+
+extern "C" int lqcd_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical_dev, const void *native_dev)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(native_dev && canonical_dev, "lqcd_unpack_spinor: null pointer");
+    REQUIRE(parity == 0 || parity == 1, "lqcd_unpack_spinor: parity %d", parity);
+    return launch_unpack_spinor(ctx, parity, canonical_dev, native_dev);
+}
+
+extern "C" int lqcd_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(out && in && links, "lqcd_dslash: null pointer");
+    REQUIRE(parity == 0 || parity == 1, "lqcd_dslash: parity %d", parity);
+    REQUIRE(out != in, "lqcd_dslash: out and in alias");
+    return launch_dslash(ctx, parity, out, in, links, NULL, 0.0, 0, 0);
+}
+
+extern "C" int lqcd_mdagm(lqcd_ctx *ctx, void *out_e, const void *in_e, const void *links, double mass, double sigma)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(out_e && in_e && links, "lqcd_mdagm: null pointer");
+    REQUIRE(out_e != in_e, "lqcd_mdagm: out and in alias");
+    if (!ctx->ws) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "lqcd_mdagm: no workspace set");
+    void *tmp_o = ws_vec(ctx, 0);
+    rc = launch_dslash(ctx, LQCD_ODD, tmp_o, in_e, links, NULL, 0.0, 0, 0);
+    if (rc) return rc;
+    return launch_dslash(ctx, LQCD_EVEN, out_e, tmp_o, links, in_e, mass * mass + sigma, 0, 0);
+}

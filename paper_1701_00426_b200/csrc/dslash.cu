@@ -1,0 +1,205 @@
+// dslash.cu -- the even/odd staggered Dirac operator D_eo / D_oe (Eq. 7;
+// the paper's acc_Deo of Listing 2), hand-written for sm_100a.
+//
+//   (D psi)(x) = 1/2 sum_mu eta_mu(x) [ s+ U_mu(x) psi(x+mu) - s- U_mu(x-mu)^dagger psi(x-mu) ]
+//
+// Steps a2-a5 of SURVEY.md section 8(a); readings R1-R5, R8, R9 of DESIGN.md.
+//   a2  one thread per output site; coordinates, the 8 neighbour half-indices, eta_mu(x) and the
+//       antiperiodic sign come from integer arithmetic on the thread index (no neighbour tables,
+//       unlike the paper's nnp_openacc/nnm_openacc)
+//   a3  each link is read exactly once per application with streaming (evict-first) loads; with
+//       2-row storage the third row is rebuilt in registers, r2 = (r0 ^ r1)^*
+//   a4  8 SU(3) x colour-vector products accumulated in registers, one store per site
+//   a5  optional fused epilogue out = coef*x - D in (Eq. 8) and the partial sums of
+//       Re<x,out> for CG, reduced deterministically (reduce.cuh)
+// The kernel is bound by HBM bandwidth (1248 B/site fp64 18-real vs 570 flop/site): no tensor cores.
+#include "reduce.cuh"
+
+template <typename T> struct Su3 { Cx<T> e[3][3]; };
+
+template <typename T, int LAYOUT, int RECON12>
+__device__ __forceinline__ Su3<T> load_link(const T *__restrict__ links, int par, int mu, size_t Vh, size_t i)
+{
+    constexpr int R = RECON12 ? 2 : 3;
+    Su3<T> u;
+    size_t plane0 = (size_t)(par * 4 + mu) * (R * 3);
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) u.e[r][c] = ld_cx<T, LAYOUT, 1>(links, plane0 + r * 3 + c, Vh, i);
+    if (RECON12) {
+        // r2[k] = conj( eps_kij r0[i] r1[j] )   (reading R8)
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int a = (k + 1) % 3, b = (k + 2) % 3;
+            Cx<T> x = u.e[0][a], y = u.e[1][b], z = u.e[0][b], w = u.e[1][a];
+            T re = x.re * y.re - x.im * y.im - (z.re * w.re - z.im * w.im);
+            T im = x.re * y.im + x.im * y.re - (z.re * w.im + z.im * w.re);
+            u.e[2][k] = cx<T>(re, -im);
+        }
+    }
+    return u;
+}
+
+template <typename T, int LAYOUT>
+__device__ __forceinline__ void load_vec(const T *__restrict__ v, size_t Vh, size_t i, T coef, Cx<T> p[3])
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        Cx<T> z = ld_cx<T, LAYOUT, 0>(v, (size_t)c, Vh, i);
+        p[c] = cx<T>(coef * z.re, coef * z.im);
+    }
+}
+
+// acc += U p
+template <typename T> __device__ __forceinline__ void mv_acc(Cx<T> acc[3], const Su3<T> &u, const Cx<T> p[3])
+{
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            acc[a].re = fma(u.e[a][b].re, p[b].re, acc[a].re);
+            acc[a].re = fma(-u.e[a][b].im, p[b].im, acc[a].re);
+            acc[a].im = fma(u.e[a][b].re, p[b].im, acc[a].im);
+            acc[a].im = fma(u.e[a][b].im, p[b].re, acc[a].im);
+        }
+}
+// acc += U^dagger p,  (U^dagger)_{ab} = conj(U_{ba})
+template <typename T> __device__ __forceinline__ void mvdag_acc(Cx<T> acc[3], const Su3<T> &u, const Cx<T> p[3])
+{
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            acc[a].re = fma(u.e[b][a].re, p[b].re, acc[a].re);
+            acc[a].re = fma(u.e[b][a].im, p[b].im, acc[a].re);
+            acc[a].im = fma(u.e[b][a].re, p[b].im, acc[a].im);
+            acc[a].im = fma(-u.e[b][a].im, p[b].re, acc[a].im);
+        }
+}
+
+// MODE 0: out = D in;  1: out = coef*x - D in;  2: as 1, plus Re<x,out> -> solver_after_pq
+template <typename T, int LAYOUT, int RECON12, int MODE, int MINB>
+__global__ void __launch_bounds__(256, MINB)
+dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__restrict__ in,
+              const T *__restrict__ links, const T *__restrict__ xin, const double coef,
+              SolverState *__restrict__ st, double *__restrict__ partials, const int gate)
+{
+    if (gate) {
+        int d = *(volatile int *)&st->done;
+        if (d) {   // a converged solve: the rest of the enqueued iterations are no-ops
+            if (gate == 2 && d == 1 && blockIdx.x == 0 && threadIdx.x == 0) st->done = 2;
+            return;
+        }
+    }
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = i < g.Vh;
+    double dot = 0.0;
+    if (valid) {
+        const size_t Vh = (size_t)g.Vh;
+        // ---- a2: site decode (Eq. 9), neighbours, phases ---------------------------------
+        uint32_t t = fd_div((uint32_t)i, g.dNh0);
+        const int hx0 = i - (int)t * g.Nh0;
+        uint32_t t2 = fd_div(t, g.dN1);
+        const int x1 = (int)t - (int)t2 * g.N1;
+        const int x3 = (int)fd_div(t2, g.dN2);
+        const int x2 = (int)t2 - x3 * g.N2;
+        const int rp = (x1 + x2 + x3 + parity) & 1;            // x0 = 2*hx0 + rp
+        int nf[4], nb[4];
+        nf[0] = rp ? (hx0 + 1 == g.Nh0 ? i - (g.Nh0 - 1) : i + 1) : i;
+        nb[0] = rp ? i : (hx0 == 0 ? i + (g.Nh0 - 1) : i - 1);
+        nf[1] = x1 + 1 == g.N1 ? i - (g.N1 - 1) * g.s1 : i + g.s1;
+        nb[1] = x1 == 0 ? i + (g.N1 - 1) * g.s1 : i - g.s1;
+        nf[2] = x2 + 1 == g.N2 ? i - (g.N2 - 1) * g.s2 : i + g.s2;
+        nb[2] = x2 == 0 ? i + (g.N2 - 1) * g.s2 : i - g.s2;
+        nf[3] = x3 + 1 == g.N3 ? i - (g.N3 - 1) * g.s3 : i + g.s3;
+        nb[3] = x3 == 0 ? i + (g.N3 - 1) * g.s3 : i - g.s3;
+        // 1/2 * eta_mu(x) (readings R2, R3); boundary sign on the x3 hops (reading R4)
+        T cf[4], cb[4];
+        const T h = (T)0.5;
+        cf[0] = h;
+        cf[1] = rp ? -h : h;
+        cf[2] = ((rp + x1) & 1) ? -h : h;
+        cf[3] = ((rp + x1 + x2) & 1) ? -h : h;
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) cb[mu] = -cf[mu];
+        if (g.ap) {
+            if (x3 == g.N3 - 1) cf[3] = -cf[3];
+            if (x3 == 0) cb[3] = -cb[3];
+        }
+        // ---- a3, a4: 8 hops -----------------------------------------------------------------
+        Cx<T> acc[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) acc[c] = cx<T>((T)0, (T)0);
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) {
+            {
+                Su3<T> u = load_link<T, LAYOUT, RECON12>(links, parity, mu, Vh, (size_t)i);
+                Cx<T> p[3];
+                load_vec<T, LAYOUT>(in, Vh, (size_t)nf[mu], cf[mu], p);
+                mv_acc<T>(acc, u, p);
+            }
+            {
+                Su3<T> u = load_link<T, LAYOUT, RECON12>(links, 1 - parity, mu, Vh, (size_t)nb[mu]);
+                Cx<T> p[3];
+                load_vec<T, LAYOUT>(in, Vh, (size_t)nb[mu], cb[mu], p);
+                mvdag_acc<T>(acc, u, p);
+            }
+        }
+        // ---- a5: epilogue ------------------------------------------------------------------
+        if (MODE >= 1) {
+            const T cm = (T)coef;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                Cx<T> x = ld_cx<T, LAYOUT, 0>(xin, (size_t)c, Vh, (size_t)i);
+                acc[c] = cx<T>(fma(cm, x.re, -acc[c].re), fma(cm, x.im, -acc[c].im));
+                if (MODE == 2) dot += (double)x.re * (double)acc[c].re + (double)x.im * (double)acc[c].im;
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) st_cx<T, LAYOUT>(out, (size_t)c, Vh, (size_t)i, acc[c]);
+    }
+    if (MODE == 2) {
+        double total;
+        if (grid_sum_last(dot, partials, &st->ticket, &total)) solver_after_pq(st, total);
+    }
+}
+
+template <typename T, int LAYOUT, int RECON12, int MODE>
+static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
+                     const void *xin, double coef, int gate)
+{
+    int block = ctx->dslash_block > 256 ? 256 : ctx->dslash_block;
+    dim3 grid((ctx->g.Vh + block - 1) / block);
+    int minb = ctx->dslash_minblocks;
+    if (minb == 0) minb = sizeof(T) == 8 ? 2 : 3;
+#define GO(MB) dslash_kernel<T, LAYOUT, RECON12, MODE, MB><<<grid, block, 0, ctx->stream>>>( \
+        ctx->g, parity, (T *)out, (const T *)in, (const T *)links, (const T *)xin, coef, ctx->d_state, ctx->d_partials, gate)
+    if (minb <= 1) GO(1); else if (minb == 2) GO(2); else if (minb == 3) GO(3); else GO(4);
+#undef GO
+}
+
+template <typename T, int LAYOUT>
+static void launch_tl(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
+                      const void *xin, double coef, int mode, int gate)
+{
+#define GO(R, M) launch_t<T, LAYOUT, R, M>(ctx, parity, out, in, links, xin, coef, gate)
+    if (ctx->recon == LQCD_RECON_12) { if (mode == 0) GO(1, 0); else if (mode == 1) GO(1, 1); else GO(1, 2); }
+    else { if (mode == 0) GO(0, 0); else if (mode == 1) GO(0, 1); else GO(0, 2); }
+#undef GO
+}
+
+int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
+                  const void *xpay_in, double coef, int dot_mode, int gate)
+{
+    int mode = xpay_in ? (dot_mode ? 2 : 1) : 0;
+    if (ctx->prec == LQCD_F64) {
+        if (ctx->layout == 0) launch_tl<double, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
+        else launch_tl<double, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
+    } else {
+        if (ctx->layout == 0) launch_tl<float, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
+        else launch_tl<float, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
+    }
+    ctx->launches++;
+    return lqcd_check_cuda(ctx, cudaGetLastError(), "dslash");
+}

@@ -1,0 +1,97 @@
+// pack.cu -- canonical (AoS, lexicographic, complex128) <-> native (parity-split SoA) fields.
+// Step a1 of SURVEY.md section 8(a): PAPER.md:245-272 (SoA vec3_soa / su3_soa, Figs 1-2), the even-site
+// index of Eq. 9, and the 2-row link storage of PAPER.md:272 (row 2 dropped
+// here, rebuilt in registers by the Dslash kernel).  Setup cost, untimed.
+#include "common.cuh"
+
+// idxh, parity -> lexicographic site index
+__device__ __forceinline__ int lex_of_half(const Geom &g, int i, int parity)
+{
+    uint32_t t = fd_div((uint32_t)i, g.dNh0);
+    uint32_t t2 = fd_div(t, g.dN1);
+    int x1 = (int)t - (int)t2 * g.N1;
+    uint32_t x3 = fd_div(t2, g.dN2);
+    int x2 = (int)t2 - (int)x3 * g.N2;
+    int rp = (x1 + x2 + (int)x3 + parity) & 1;
+    return 2 * i + rp;     // lex = 2*idxh + (x0 & 1), and x0 = 2*hx0 + rp
+}
+
+template <typename T, int LAYOUT>
+__global__ void pack_links_kernel(Geom g, int rows, T *__restrict__ native, const double2 *__restrict__ canon)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int par = blockIdx.y;
+    if (i >= g.Vh) return;
+    size_t lex = (size_t)lex_of_half(g, i, par);
+    for (int mu = 0; mu < 4; ++mu)
+        for (int r = 0; r < rows; ++r)
+            for (int c = 0; c < 3; ++c) {
+                double2 z = canon[(lex * 4 + mu) * 9 + r * 3 + c];
+                size_t plane = ((size_t)(par * 4 + mu) * rows + r) * 3 + c;
+                st_cx<T, LAYOUT>(native, plane, (size_t)g.Vh, (size_t)i, cx<T>((T)z.x, (T)z.y));
+            }
+}
+
+template <typename T, int LAYOUT>
+__global__ void pack_spinor_kernel(Geom g, T *__restrict__ native, const double2 *__restrict__ canon)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.Vh) return;
+    for (int c = 0; c < 3; ++c) {
+        double2 z = canon[(size_t)i * 3 + c];
+        st_cx<T, LAYOUT>(native, (size_t)c, (size_t)g.Vh, (size_t)i, cx<T>((T)z.x, (T)z.y));
+    }
+}
+
+template <typename T, int LAYOUT>
+__global__ void unpack_spinor_kernel(Geom g, double2 *__restrict__ canon, const T *__restrict__ native)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.Vh) return;
+    for (int c = 0; c < 3; ++c) {
+        Cx<T> z = ld_cx<T, LAYOUT, 0>(native, (size_t)c, (size_t)g.Vh, (size_t)i);
+        canon[(size_t)i * 3 + c] = make_double2((double)z.re, (double)z.im);
+    }
+}
+
+#define DISPATCH_TL(ctx, CALL)                                             \
+    do {                                                                   \
+        if ((ctx)->prec == LQCD_F64) {                                     \
+            if ((ctx)->layout == 0) { CALL(double, 0); } else { CALL(double, 1); } \
+        } else {                                                           \
+            if ((ctx)->layout == 0) { CALL(float, 0); } else { CALL(float, 1); }   \
+        }                                                                  \
+    } while (0)
+
+int launch_pack_links(lqcd_ctx *ctx, void *native, const void *canonical)
+{
+    int rows = ctx->recon == LQCD_RECON_12 ? 2 : 3;
+    dim3 grid((ctx->g.Vh + 127) / 128, 2), block(128);
+#define CALL(T, L) pack_links_kernel<T, L><<<grid, block, 0, ctx->stream>>>(ctx->g, rows, (T *)native, (const double2 *)canonical)
+    DISPATCH_TL(ctx, CALL);
+#undef CALL
+    ctx->launches++;
+    return lqcd_check_cuda(ctx, cudaGetLastError(), "pack_links");
+}
+
+int launch_pack_spinor(lqcd_ctx *ctx, int parity, void *native, const void *canonical)
+{
+    (void)parity;  // the half-lattice order idxh = lex/2 is the same for both parities (Eq. 9)
+    dim3 grid((ctx->g.Vh + 127) / 128), block(128);
+#define CALL(T, L) pack_spinor_kernel<T, L><<<grid, block, 0, ctx->stream>>>(ctx->g, (T *)native, (const double2 *)canonical)
+    DISPATCH_TL(ctx, CALL);
+#undef CALL
+    ctx->launches++;
+    return lqcd_check_cuda(ctx, cudaGetLastError(), "pack_spinor");
+}
+
+int launch_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical, const void *native)
+{
+    (void)parity;
+    dim3 grid((ctx->g.Vh + 127) / 128), block(128);
+#define CALL(T, L) unpack_spinor_kernel<T, L><<<grid, block, 0, ctx->stream>>>(ctx->g, (double2 *)canonical, (const T *)native)
+    DISPATCH_TL(ctx, CALL);
+#undef CALL
+    ctx->launches++;
+    return lqcd_check_cuda(ctx, cudaGetLastError(), "unpack_spinor");
+}

@@ -1,0 +1,288 @@
+// solver.cu -- CG and multi-shift CG on A = m^2 - D_eo D_oe (Eq. 8; the
+// "multishift inverter routine" of PAPER.md:313 for Eq. 6), readings R10-R14, R16.
+//
+// Steps a5-a8 of SURVEY.md section 8(a).  Per iteration, on one stream, with no host round trip:
+//   K_A  tmp_o = D_oe p                                              (dslash.cu)
+//   K_B  q = (m^2 + sigma_min) p - D_eo tmp_o ;  Re<p,q>  -> alpha, zeta_i^new, alpha_i
+//   K1   r -= alpha q ;  <r,r>                             -> beta, beta_i, freeze flags
+//   K2   x_i += alpha_i p_i ;  p_i = zeta_i^new r + beta_i p_i ;  p = r + beta p   (one pass)
+// The paper's "zaxpy-like functions" and dot products are these two fused
+// kernels; the scalars live in a device struct and are produced by the last CTA of each
+// reduction.  The host only polls a `done` word every poll_chunk iterations.
+//
+// The vector kernels are layout-agnostic: every update is (real scalar) x (vector), so they run
+// over the 6*Vh reals of a half-lattice vector as a flat array with 16-byte loads.
+#include <stdlib.h>
+
+#include "reduce.cuh"
+
+void *ws_vec(lqcd_ctx *ctx, int k);   // api.cu
+
+template <typename T> struct Pack;            // 16-byte packet of reals
+template <> struct Pack<double> { typedef double2 type; enum { N = 2 }; };
+template <> struct Pack<float> { typedef float4 type; enum { N = 4 }; };
+
+template <typename T> __device__ __forceinline__ void unpack(const double2 &v, T *a) { a[0] = v.x; a[1] = v.y; }
+template <typename T> __device__ __forceinline__ void unpack(const float4 &v, T *a) { a[0] = v.x; a[1] = v.y; a[2] = v.z; a[3] = v.w; }
+__device__ __forceinline__ double2 repack(const double *a) { return make_double2(a[0], a[1]); }
+__device__ __forceinline__ float4 repack(const float *a) { return make_float4(a[0], a[1], a[2], a[3]); }
+
+struct ShiftPtrs {
+    void *x[LQCD_MAX_SHIFTS];
+    void *p[LQCD_MAX_SHIFTS];
+    int nshift, base;
+};
+
+// r = p = p_i = b, x_i = 0, rho = ||b||^2
+template <typename T>
+__global__ void __launch_bounds__(256) init_kernel(size_t npk, const T *__restrict__ b, T *__restrict__ r,
+                                                   T *__restrict__ p, ShiftPtrs sp, SolverState *st,
+                                                   double *partials)
+{
+    typedef typename Pack<T>::type P;
+    const int N = Pack<T>::N;
+    double acc = 0.0;
+    T zero[4] = {0, 0, 0, 0};
+    for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
+        P v = reinterpret_cast<const P *>(b)[k];
+        T a[4];
+        unpack<T>(v, a);
+        for (int j = 0; j < N; ++j) acc += (double)a[j] * (double)a[j];
+        reinterpret_cast<P *>(r)[k] = v;
+        reinterpret_cast<P *>(p)[k] = v;
+        for (int i = 0; i < sp.nshift; ++i) {
+            reinterpret_cast<P *>(sp.x[i])[k] = repack(zero);
+            if (i != sp.base) reinterpret_cast<P *>(sp.p[i])[k] = v;
+        }
+    }
+    double total;
+    if (grid_sum_last(acc, partials, &st->ticket, &total)) {
+        st->rho = total;
+        st->bnorm2 = total;
+        if (total == 0.0) st->done = 2;
+    }
+}
+
+// K1: r -= alpha q ; <r,r>
+template <typename T>
+__global__ void __launch_bounds__(256) k1_kernel(size_t npk, T *__restrict__ r, const T *__restrict__ q,
+                                                 SolverState *st, double *partials)
+{
+    if (*(volatile int *)&st->done) return;
+    typedef typename Pack<T>::type P;
+    const int N = Pack<T>::N;
+    const T alpha = (T)st->alpha;
+    double acc = 0.0;
+    for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
+        T a[4], c[4];
+        unpack<T>(reinterpret_cast<const P *>(r)[k], a);
+        unpack<T>(reinterpret_cast<const P *>(q)[k], c);
+        for (int j = 0; j < N; ++j) {
+            a[j] = fma(-alpha, c[j], a[j]);
+            acc += (double)a[j] * (double)a[j];
+        }
+        reinterpret_cast<P *>(r)[k] = repack(a);
+    }
+    double total;
+    if (grid_sum_last(acc, partials, &st->ticket, &total)) solver_after_rr(st, total);
+}
+
+// K2: x_i += alpha_i p_i ; p_i = zeta_i r + beta_i p_i ; p = r + beta p.  The base shift has
+// zeta = 1 and p_base == p, so its direction vector is not stored.
+template <typename T>
+__global__ void __launch_bounds__(256) k2_kernel(size_t npk, const T *__restrict__ r, T *__restrict__ p,
+                                                 ShiftPtrs sp, const SolverState *__restrict__ st)
+{
+    if (*(volatile const int *)&st->done == 2) return;
+    typedef typename Pack<T>::type P;
+    const int N = Pack<T>::N;
+    __shared__ T s_alpha[LQCD_MAX_SHIFTS], s_zeta[LQCD_MAX_SHIFTS], s_beta[LQCD_MAX_SHIFTS];
+    __shared__ int s_active[LQCD_MAX_SHIFTS];
+    if (threadIdx.x < sp.nshift) {
+        s_alpha[threadIdx.x] = (T)st->c_alpha[threadIdx.x];
+        s_zeta[threadIdx.x] = (T)st->c_zeta[threadIdx.x];
+        s_beta[threadIdx.x] = (T)st->c_beta[threadIdx.x];
+        s_active[threadIdx.x] = st->c_active[threadIdx.x];
+    }
+    __syncthreads();
+    const T beta = (T)st->beta;
+    for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
+        T rr[4], pp[4];
+        unpack<T>(reinterpret_cast<const P *>(r)[k], rr);
+        unpack<T>(reinterpret_cast<const P *>(p)[k], pp);
+        for (int i = 0; i < sp.nshift; ++i) {
+            if (!s_active[i]) continue;
+            T xx[4];
+            unpack<T>(reinterpret_cast<const P *>(sp.x[i])[k], xx);
+            if (i == sp.base) {
+                for (int j = 0; j < N; ++j) xx[j] = fma(s_alpha[i], pp[j], xx[j]);
+            } else {
+                T pi[4];
+                unpack<T>(reinterpret_cast<const P *>(sp.p[i])[k], pi);
+                for (int j = 0; j < N; ++j) {
+                    xx[j] = fma(s_alpha[i], pi[j], xx[j]);
+                    pi[j] = fma(s_beta[i], pi[j], s_zeta[i] * rr[j]);
+                }
+                reinterpret_cast<P *>(sp.p[i])[k] = repack(pi);
+            }
+            reinterpret_cast<P *>(sp.x[i])[k] = repack(xx);
+        }
+        for (int j = 0; j < N; ++j) pp[j] = fma(beta, pp[j], rr[j]);
+        reinterpret_cast<P *>(p)[k] = repack(pp);
+    }
+}
+
+// ||a - b||^2 -> *slot
+template <typename T>
+__global__ void __launch_bounds__(256) diffnorm_kernel(size_t npk, const T *__restrict__ a, const T *__restrict__ b,
+                                                       SolverState *st, double *partials, double *slot)
+{
+    typedef typename Pack<T>::type P;
+    const int N = Pack<T>::N;
+    double acc = 0.0;
+    for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
+        T x[4], y[4];
+        unpack<T>(reinterpret_cast<const P *>(a)[k], x);
+        unpack<T>(reinterpret_cast<const P *>(b)[k], y);
+        for (int j = 0; j < N; ++j) { double d = (double)x[j] - (double)y[j]; acc += d * d; }
+    }
+    double total;
+    if (grid_sum_last(acc, partials, &st->ticket, &total)) *slot = total;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Host driver
+// ---------------------------------------------------------------------------------------------
+static int blas_grid(const lqcd_ctx *ctx, size_t npk)
+{
+    size_t want = (npk + ctx->blas_block - 1) / ctx->blas_block;
+    size_t cap = (size_t)ctx->num_sms * ctx->blas_ctas_per_sm;
+    size_t g = want < cap ? want : cap;
+    if (g > (size_t)ctx->max_partials) g = ctx->max_partials;
+    return g < 1 ? 1 : (int)g;
+}
+
+template <typename T>
+static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *b, void *const *xs,
+                   const void *links, double mass, double tol, int max_iter,
+                   int *iters, int *conv_iter, double *rel_resid)
+{
+    const size_t npk = (size_t)ctx->g.Vh * 6 / Pack<T>::N;
+    const int grid = blas_grid(ctx, npk), block = ctx->blas_block;
+    cudaStream_t s = ctx->stream;
+    T *tmp_o = (T *)ws_vec(ctx, 0), *q = (T *)ws_vec(ctx, 1), *r = (T *)ws_vec(ctx, 2), *p = (T *)ws_vec(ctx, 3);
+
+    // base system = smallest shift (reading R11)
+    int base = 0;
+    for (int i = 1; i < nshift; ++i) if (shifts[i] < shifts[base]) base = i;
+    SolverState h;
+    memset(&h, 0, sizeof(h));
+    h.alpha_prev = 1.0; h.beta_prev = 0.0; h.tol = tol; h.nshift = nshift;
+    ShiftPtrs sp;
+    memset(&sp, 0, sizeof(sp));
+    sp.nshift = nshift; sp.base = base;
+    for (int i = 0; i < nshift; ++i) {
+        h.zeta[i] = h.zeta_old[i] = 1.0;
+        h.delta[i] = shifts[i] - shifts[base];
+        h.active[i] = 1;
+        sp.x[i] = xs[i];
+        sp.p[i] = ws_vec(ctx, 4 + i);
+    }
+    int rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(ctx->d_state, &h, sizeof(h), cudaMemcpyHostToDevice, s), "solver state upload");
+    if (rc) return rc;
+    init_kernel<T><<<grid, block, 0, s>>>(npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
+    ctx->launches++;
+
+    const double msq = mass * mass + shifts[base];
+    volatile int *flag = ctx->h_flag;
+    flag[0] = flag[16 / 4] = 0;
+    int enq = 0, chunk_id = 0, stop = 0;
+    while (!stop) {
+        int n = ctx->poll_chunk;
+        if (enq + n > max_iter) n = max_iter - enq;
+        for (int k = 0; k < n; ++k) {
+            if ((rc = launch_dslash(ctx, LQCD_ODD, tmp_o, p, links, NULL, 0.0, 0, 2))) return rc;
+            if ((rc = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, p, msq, 1, 1))) return rc;
+            k1_kernel<T><<<grid, block, 0, s>>>(npk, r, q, ctx->d_state, ctx->d_partials);
+            k2_kernel<T><<<grid, block, 0, s>>>(npk, r, p, sp, ctx->d_state);
+            ctx->launches += 2;
+        }
+        enq += n;
+        int slot = chunk_id & 1;
+        cudaMemcpyAsync((void *)(flag + slot * 4), &ctx->d_state->done, sizeof(int), cudaMemcpyDeviceToHost, s);
+        cudaEventRecord(ctx->ev[slot], s);
+        // look at the PREVIOUS chunk's flag, so that one chunk is always queued behind the GPU
+        if (chunk_id > 0) {
+            int prev = (chunk_id - 1) & 1;
+            if ((rc = lqcd_check_cuda(ctx, cudaEventSynchronize(ctx->ev[prev]), "cg poll"))) return rc;
+            if (flag[prev * 4]) stop = 1;
+        }
+        if (enq >= max_iter) stop = 1;
+        ++chunk_id;
+    }
+    // true residuals || b - (A + sigma_i) x_i || (reading R10), with the same kernels, ungated
+    for (int i = 0; i < nshift; ++i) {
+        if ((rc = launch_dslash(ctx, LQCD_ODD, tmp_o, xs[i], links, NULL, 0.0, 0, 0))) return rc;
+        if ((rc = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, xs[i], mass * mass + shifts[i], 0, 0))) return rc;
+        diffnorm_kernel<T><<<grid, block, 0, s>>>(npk, (const T *)b, q, ctx->d_state, ctx->d_partials, &ctx->d_state->resid[i]);
+        ctx->launches++;
+    }
+    if ((rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(&h, ctx->d_state, sizeof(h), cudaMemcpyDeviceToHost, s), "solver state download"))) return rc;
+    if ((rc = lqcd_check_cuda(ctx, cudaStreamSynchronize(s), "cg"))) return rc;
+
+    if (iters) *iters = h.iter;
+    int converged = (h.done != 0);
+    for (int i = 0; i < nshift; ++i) {
+        if (conv_iter) conv_iter[i] = h.active[i] ? h.iter : h.conv_iter[i];
+        if (rel_resid) rel_resid[i] = h.bnorm2 > 0.0 ? sqrt(h.resid[i] / h.bnorm2) : 0.0;
+    }
+    ctx->hist_n = h.iter < LQCD_HIST ? h.iter : LQCD_HIST;
+    memcpy(ctx->h_hist[0], h.hist_alpha, sizeof(h.hist_alpha));
+    memcpy(ctx->h_hist[1], h.hist_beta, sizeof(h.hist_beta));
+    memcpy(ctx->h_hist[2], h.hist_rnorm, sizeof(h.hist_rnorm));
+    if (!converged) return lqcd_fail(ctx, LQCD_ERR_NOT_CONVERGED, "not converged after %d iterations", h.iter);
+    return LQCD_OK;
+}
+
+extern "C" int lqcd_cg_multishift(lqcd_ctx *ctx, int nshift, const double *shifts, const void *rhs_e,
+                                  void *const *solutions_e, const void *links, double mass, double tol,
+                                  int max_iter, int *iters, int *conv_iter, double *rel_resid)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    int rc = lqcd_check_cuda(ctx, cudaSetDevice(ctx->device), "cudaSetDevice");
+    if (rc) return rc;
+    if (nshift < 1 || nshift > LQCD_MAX_SHIFTS) return lqcd_fail(ctx, LQCD_ERR_ARG, "nshift %d not in [1,%d]", nshift, LQCD_MAX_SHIFTS);
+    if (!shifts || !rhs_e || !solutions_e || !links) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_cg_multishift: null pointer");
+    if (!(tol > 0.0)) return lqcd_fail(ctx, LQCD_ERR_ARG, "tol must be > 0");
+    if (max_iter < 1) return lqcd_fail(ctx, LQCD_ERR_ARG, "max_iter must be >= 1");
+    for (int i = 0; i < nshift; ++i) {
+        if (!(shifts[i] >= 0.0)) return lqcd_fail(ctx, LQCD_ERR_ARG, "shift %d is negative or NaN", i);
+        if (!solutions_e[i] || solutions_e[i] == rhs_e) return lqcd_fail(ctx, LQCD_ERR_ARG, "solution %d is null or aliases rhs", i);
+    }
+    if (!ctx->ws) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "no workspace set");
+    if (ctx->ws_bytes < lqcd_workspace_bytes(ctx, nshift))
+        return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "workspace %zu bytes < %zu needed for %d shifts", ctx->ws_bytes, lqcd_workspace_bytes(ctx, nshift), nshift);
+    if (ctx->prec == LQCD_F64)
+        return solve_t<double>(ctx, nshift, shifts, rhs_e, solutions_e, links, mass, tol, max_iter, iters, conv_iter, rel_resid);
+    return solve_t<float>(ctx, nshift, shifts, rhs_e, solutions_e, links, mass, tol, max_iter, iters, conv_iter, rel_resid);
+}
+
+extern "C" int lqcd_cg(lqcd_ctx *ctx, void *x_e, const void *b_e, const void *links, double mass,
+                       double tol, int max_iter, int *iters, double *rel_resid)
+{
+    const double zero = 0.0;
+    void *xs[1] = { x_e };
+    if (ctx && !x_e) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_cg: null pointer");
+    return lqcd_cg_multishift(ctx, 1, &zero, b_e, xs, links, mass, tol, max_iter, iters, NULL, rel_resid);
+}
+
+extern "C" int lqcd_solver_history(lqcd_ctx *ctx, int n, double *alpha, double *beta, double *rnorm)
+{
+    if (!ctx) return -LQCD_ERR_ARG;
+    int m = n < ctx->hist_n ? n : ctx->hist_n;
+    if (m < 0) m = 0;
+    if (alpha) memcpy(alpha, ctx->h_hist[0], m * sizeof(double));
+    if (beta) memcpy(beta, ctx->h_hist[1], m * sizeof(double));
+    if (rnorm) memcpy(rnorm, ctx->h_hist[2], m * sizeof(double));
+    return ctx->hist_n;
+}

@@ -1,0 +1,273 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs (-m gpu).  Tolerances: 1e-12 relative L2 in fp64, 1e-5 in fp32 (BASELINE.json
+north_star); solver criteria are reading R16 of DESIGN.md.
+"""
+import numpy as np
+import pytest
+
+import lqcd_inputs as gen
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL = {0: 1e-12, 1: 1e-5}
+
+
+def rel(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+def round_inputs(prec, *arrs):
+    """fp32 contexts see the fp64 inputs rounded to nearest; the oracle runs in fp64 on the SAME
+    rounded numbers, so the 1e-5 bound measures arithmetic only (reading R14)."""
+    if prec == 0:
+        return arrs
+    return tuple(a.astype(np.complex64).astype(np.complex128) for a in arrs)
+
+
+def make_lattice(dims, prec=0, recon=0, ap=True, **opts):
+    import paper_1701_00426_b200 as L
+    return L.Lattice(dims, prec=prec, recon=recon, antiperiodic_t=ap, options=opts)
+
+
+def gpu_dslash(lat, U, phi_in, out_parity):
+    links = lat.pack_links(U)
+    inp = lat.pack_spinor(phi_in, 1 - out_parity)
+    out = lat.new_spinor()
+    lat.dslash(out_parity, out, inp, links)
+    return lat.unpack_spinor(out, out_parity)
+
+
+# ------------------------------------------------------------------------------------------------
+# Dslash
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("layout", [0, 1])
+@pytest.mark.parametrize("recon", [0, 1])
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (2, 2, 2, 2), (6, 4, 2, 8), (12, 10, 6, 4)])
+def test_dslash_both_parities(dims, prec, recon, layout):
+    """BASELINE.json config 1 (4^4, Haar-like links, seed 1, full-lattice Gaussian spinor, both
+    parities) plus 2^4 (N=2 wrap), a ragged lattice and one spanning several CTAs with a tail."""
+    rng = np.random.default_rng(1)
+    U = gen.haar_like_links(dims, rng)
+    psi = gen.gaussian_spinor(dims, rng)
+    U, psi = round_inputs(prec, U, psi)
+    if recon == 1 and prec == 1:
+        # rounding to fp32 breaks unitarity at 1e-7; the 12-real oracle input is the rebuilt field
+        U = oracle.reconstruct_row3(U)
+    lat = make_lattice(dims, prec, recon, True, layout=layout)
+    for out_parity in (0, 1):
+        phi_in = oracle.full_to_half(dims, 1 - out_parity, psi)
+        want = oracle.dslash_half(dims, U, out_parity, phi_in)
+        got = gpu_dslash(lat, U, phi_in, out_parity)
+        assert rel(got, want) < TOL[prec], (dims, prec, recon, layout, out_parity)
+    lat.close()
+
+
+@pytest.mark.parametrize("ap", [True, False])
+def test_dslash_boundary_conditions(ap):
+    dims = (4, 6, 4, 4)
+    rng = np.random.default_rng(17)
+    U = gen.smooth_links(dims, 0.5, rng)
+    phi = gen.gaussian_half_spinor(dims, rng)
+    lat = make_lattice(dims, ap=ap)
+    want = oracle.dslash_half(dims, U, 1, phi, antiperiodic_t=ap)
+    assert rel(gpu_dslash(lat, U, phi, 1), want) < 1e-12
+    lat.close()
+
+
+@pytest.mark.parametrize("block,minb", [(32, 1), (64, 2), (128, 3), (256, 4), (96, 2)])
+def test_dslash_launch_variants(block, minb):
+    """Every launch-bounds instantiation and odd CTA sizes give the same numbers."""
+    dims = (6, 6, 4, 10)     # Vh = 720: several CTAs and a ragged tail for every block size
+    rng = np.random.default_rng(3)
+    U = gen.smooth_links(dims, 0.3, rng)
+    phi = gen.gaussian_half_spinor(dims, rng)
+    want = oracle.dslash_half(dims, U, 0, phi)
+    lat = make_lattice(dims, dslash_block=block, dslash_minblocks=minb)
+    assert rel(gpu_dslash(lat, U, phi, 0), want) < 1e-12
+    lat.close()
+
+
+def test_dslash_16x4_config2_and_mdagm():
+    """BASELINE.json config 2 operator part: 16^4, eps = 0.3, seed 2, both parities and mdagm."""
+    dims = (16, 16, 16, 16)
+    rng = np.random.default_rng(2)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    for recon in (0, 1):
+        lat = make_lattice(dims, recon=recon)
+        links = lat.pack_links(U)
+        for par in (0, 1):
+            inp = lat.pack_spinor(b, 1 - par)
+            out = lat.new_spinor()
+            lat.dslash(par, out, inp, links)
+            assert rel(lat.unpack_spinor(out, par), oracle.dslash_half(dims, U, par, b)) < 1e-12
+        be = lat.pack_spinor(b, 0)
+        out = lat.new_spinor()
+        lat.mdagm(out, be, links, 0.01, 0.0)
+        assert rel(lat.unpack_spinor(out, 0), oracle.mdagm(dims, U, 0.01, b)) < 1e-12
+        lat.mdagm(out, be, links, 0.01, 0.37)
+        assert rel(lat.unpack_spinor(out, 0), oracle.mdagm(dims, U, 0.01, b, sigma=0.37)) < 1e-12
+        lat.close()
+
+
+def test_pack_unpack_roundtrip():
+    dims = (4, 8, 2, 6)
+    phi = gen.gaussian_half_spinor(dims, 5)
+    for prec in (0, 1):
+        for layout in (0, 1):
+            lat = make_lattice(dims, prec, layout=layout)
+            back = lat.unpack_spinor(lat.pack_spinor(phi, 0), 0)
+            if prec == 0:
+                assert np.array_equal(back, phi)
+            else:
+                assert np.array_equal(back, phi.astype(np.complex64).astype(np.complex128))
+            lat.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# CG and multi-shift CG (criteria: reading R16)
+# ------------------------------------------------------------------------------------------------
+def test_cg_lockstep_small():
+    """First iterates' alpha, beta, |r| agree with the oracle to 1e-10; solution parity."""
+    dims = (8, 8, 8, 8)
+    rng = np.random.default_rng(2)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m, tol = 0.05, 1e-10
+    ref = oracle.cg(dims, U, m, b, tol, 5000, hist_len=64)
+    lat = make_lattice(dims)
+    links, be, x = lat.pack_links(U), lat.pack_spinor(b, 0), lat.new_spinor()
+    res = lat.cg(x, be, links, m, tol, 5000)
+    h = lat.solver_history()
+    n = min(10, ref["iters"])
+    assert np.allclose(h["alpha"][:n], ref["alpha"][:n], rtol=1e-10)
+    assert np.allclose(h["beta"][:n], ref["beta"][:n], rtol=1e-10)
+    assert np.allclose(h["rnorm"][:n], ref["rnorm"][:n], rtol=1e-10)
+    assert abs(res["iters"] - ref["iters"]) <= max(1, ref["iters"] // 50)
+    xg = lat.unpack_spinor(x, 0)
+    # (i) true residual of the GPU solution evaluated with the ORACLE operator
+    true_res = np.linalg.norm(b - oracle.mdagm(dims, U, m, xg)) / np.linalg.norm(b)
+    assert true_res < 1.5 * tol
+    assert abs(res["rel_resid"] - true_res) < 1e-12
+    # (iii) || x_gpu - x_oracle || <= 10 kappa tol, kappa <= lambda_max / m^2, lambda_max ~ 7
+    assert rel(xg, ref["x"]) < 10 * (7.0 / m ** 2) * tol
+    lat.close()
+
+
+def test_cg_config2_16x4():
+    """BASELINE.json config 2: 16^4, m = 0.01, eps = 0.3, seed 2, tol 1e-10."""
+    dims = (16, 16, 16, 16)
+    rng = np.random.default_rng(2)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m, tol = 0.01, 1e-10
+    ref = oracle.cg(dims, U, m, b, tol, 20000, hist_len=64)
+    assert ref["converged"]
+    lat = make_lattice(dims)
+    links, be, x = lat.pack_links(U), lat.pack_spinor(b, 0), lat.new_spinor()
+    res = lat.cg(x, be, links, m, tol, 20000)
+    assert abs(res["iters"] - ref["iters"]) <= max(2, ref["iters"] // 50)
+    xg = lat.unpack_spinor(x, 0)
+    assert np.linalg.norm(b - oracle.mdagm(dims, U, m, xg)) / np.linalg.norm(b) < 1.5 * tol
+    assert rel(xg, ref["x"]) < 10 * (7.0 / m ** 2) * tol
+    h = lat.solver_history()
+    assert np.allclose(h["rnorm"][:10], ref["rnorm"][:10], rtol=1e-10)
+    lat.close()
+
+
+@pytest.mark.parametrize("recon", [0, 1])
+def test_multishift_small(recon):
+    dims = (8, 8, 8, 16)
+    rng = np.random.default_rng(4)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m, tol = 0.0025, 1e-10
+    shifts = gen.rhmc_shifts(8)[[3, 0, 7, 1, 2, 4, 6, 5]]     # unsorted: base is not index 0
+    ref = oracle.cg_multishift(dims, U, m, shifts, b, tol, 20000, hist_len=64)
+    assert ref["converged"]
+    lat = make_lattice(dims, recon=recon)
+    links, be = lat.pack_links(U), lat.pack_spinor(b, 0)
+    xs = [lat.new_spinor() for _ in shifts]
+    res = lat.cg_multishift(xs, be, links, m, shifts, tol, 20000)
+    assert abs(res["iters"] - ref["iters"]) <= max(2, ref["iters"] // 50)
+    assert np.all(np.abs(res["conv_iter"] - ref["conv_iter"]) <= np.maximum(2, ref["conv_iter"] // 50))
+    h = lat.solver_history()
+    assert np.allclose(h["alpha"][:10], ref["alpha"][:10], rtol=1e-10)
+    assert np.allclose(h["beta"][:10], ref["beta"][:10], rtol=1e-10)
+    bn = np.linalg.norm(b)
+    for i, s in enumerate(shifts):
+        xg = lat.unpack_spinor(xs[i], 0)
+        tr = np.linalg.norm(b - oracle.mdagm(dims, U, m, xg, sigma=s)) / bn
+        assert tr < 1.5 * tol, (i, s, tr)
+        assert abs(tr - res["rel_resid"][i]) < 1e-12
+        assert rel(xg, ref["x"][i]) < 10 * (7.0 / (m * m + s)) * tol
+    lat.close()
+
+
+def test_cg_fp32_and_max_iter():
+    dims = (8, 8, 8, 8)
+    rng = np.random.default_rng(5)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    U, b = round_inputs(1, U, b)
+    m, tol = 0.1, 1e-5
+    ref = oracle.cg(dims, U, m, b, tol, 5000)
+    lat = make_lattice(dims, prec=1)
+    links, be, x = lat.pack_links(U), lat.pack_spinor(b, 0), lat.new_spinor()
+    res = lat.cg(x, be, links, m, tol, 5000)
+    assert abs(res["iters"] - ref["iters"]) <= max(2, ref["iters"] // 20)
+    xg = lat.unpack_spinor(x, 0)
+    assert np.linalg.norm(b - oracle.mdagm(dims, U, m, xg)) / np.linalg.norm(b) < 5 * tol
+    assert rel(xg, ref["x"]) < 1e-3
+    # max_iter is reported, not hidden, and x is the last iterate
+    res = lat.cg(x, be, links, m, 1e-30, 7, raise_on_max_iter=False)
+    assert not res["converged"] and res["iters"] == 7
+    ref7 = oracle.cg(dims, U, m, b, 1e-30, 7)
+    assert rel(lat.unpack_spinor(x, 0), ref7["x"]) < 1e-4
+    lat.close()
+
+
+def test_cg_zero_rhs_and_errors():
+    import paper_1701_00426_b200 as L
+    dims = (4, 4, 4, 4)
+    U = gen.unit_links(dims)
+    lat = make_lattice(dims)
+    links = lat.pack_links(U)
+    b = lat.pack_spinor(np.zeros((lat.Vh, 3), dtype=np.complex128), 0)
+    x = lat.new_spinor()
+    res = lat.cg(x, b, links, 0.1, 1e-10, 100)
+    assert res["iters"] == 0 and np.abs(lat.unpack_spinor(x, 0)).max() == 0.0
+    with pytest.raises(L.LqcdError) as e:
+        lat.cg(x, b, links, 0.1, -1.0, 100)
+    assert e.value.code == L.ERR_ARG
+    with pytest.raises(L.LqcdError) as e:
+        lat.cg_multishift([x], b, links, 0.1, [-0.5], 1e-8, 10)
+    assert e.value.code == L.ERR_ARG
+    with pytest.raises(L.LqcdError) as e:
+        lat.dslash(0, x, x, links)
+    assert e.value.code == L.ERR_ARG
+    with pytest.raises(L.LqcdError) as e:
+        lat.dslash(3, x, b, links)
+    assert e.value.code == L.ERR_ARG
+    lat.close()
+
+
+def test_host_entry_points():
+    dims = (8, 4, 4, 6)
+    rng = np.random.default_rng(8)
+    U = gen.smooth_links(dims, 0.4, rng)
+    phi = gen.gaussian_half_spinor(dims, rng)
+    lat = make_lattice(dims)
+    out = np.empty_like(phi)
+    lat.dslash_host(1, out, phi, U)
+    assert rel(out, oracle.dslash_half(dims, U, 1, phi)) < 1e-12
+    shifts = np.array([0.5, 0.01])
+    sol = np.empty((2,) + phi.shape, dtype=np.complex128)
+    res = lat.cg_multishift_host(sol, phi, U, 0.05, shifts, 1e-10, 5000)
+    ref = oracle.cg_multishift(dims, U, 0.05, shifts, phi, 1e-10, 5000)
+    assert abs(res["iters"] - ref["iters"]) <= 2
+    for i in range(2):
+        assert rel(sol[i], ref["x"][i]) < 1e-6
+    lat.close()
