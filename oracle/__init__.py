@@ -7,6 +7,7 @@ See staggered_oracle.c for the arithmetic and its citations, oracle.py for the c
 from .oracle import (  # noqa: F401
     dirac_full,
     dirac_site,
+    dirac_range,
     dslash_half,
     mdagm,
     reconstruct_row3,

@@ -21,6 +21,8 @@ _pi = C.POINTER(C.c_int)
 
 _lib.oracle_dirac_full.argtypes = [_i4, C.c_int, _c128, _c128, _c128, C.c_int]
 _lib.oracle_dirac_full.restype = None
+_lib.oracle_dirac_range.argtypes = [_i4, C.c_int, _c128, _c128, _c128, C.c_longlong, C.c_longlong]
+_lib.oracle_dirac_range.restype = None
 _lib.oracle_dirac_site.argtypes = [_i4, C.c_int, _c128, _c128, _i4, _c128]
 _lib.oracle_dirac_site.restype = None
 _lib.oracle_half_to_full.argtypes = [_i4, C.c_int, _c128, _c128]
@@ -75,6 +77,14 @@ def dirac_full(dims, U, psi, antiperiodic_t=True, which=2):
     n4, V = _dims(dims)
     out = np.zeros((V, 3), dtype=np.complex128)
     _lib.oracle_dirac_full(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), _arr(psi, (V, 3)), out, which)
+    return out
+
+
+def dirac_range(dims, U, psi, out, lo, hi, antiperiodic_t=True):
+    """out[lo:hi] = (D psi)(lex) for lex in [lo, hi); `out` is a caller-provided (V,3) array."""
+    n4, V = _dims(dims)
+    assert out.shape == (V, 3) and out.dtype == np.complex128 and 0 <= lo <= hi <= V
+    _lib.oracle_dirac_range(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), _arr(psi, (V, 3)), out, lo, hi)
     return out
 
 

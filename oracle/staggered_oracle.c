@@ -121,6 +121,19 @@ void oracle_dirac_full(const int N[4], int antiperiodic_t, const cplx *U, const 
     }
 }
 
+/* Sites lex in [lo, hi) only (a bounded sample of a large lattice for bench.py's timed CPU
+ * baseline); other sites of `out` are left untouched. */
+void oracle_dirac_range(const int N[4], int antiperiodic_t, const cplx *U, const cplx *psi,
+                        cplx *out, long long lo, long long hi)
+{
+#pragma omp parallel for schedule(static)
+    for (long long s = lo; s < hi; ++s) {
+        int x[4];
+        coords_of(N, (size_t)s, x);
+        dirac_site(N, antiperiodic_t, U, psi, x, out + (size_t)s * 3);
+    }
+}
+
 /* One output site, for sampled parity checks at sizes where the full field is not wanted. */
 void oracle_dirac_site(const int N[4], int antiperiodic_t, const cplx *U, const cplx *psi,
                        const int x[4], cplx out[3])

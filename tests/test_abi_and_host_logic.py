@@ -1,0 +1,151 @@
+"""-m "not gpu": the C-ABI library loads and exports every symbol include/lqcd.h declares; argument
+checks that happen before any CUDA call; the product never routes through the oracle; the
+multi-process (replica) plumbing of bench.py under gloo with world_size 2."""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "lqcd.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(lqcd_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol():
+    import paper_1701_00426_b200 as L
+    names = declared_symbols()
+    assert len(names) >= 18 and "lqcd_dslash" in names and "lqcd_cg_multishift" in names
+    for n in names:
+        assert hasattr(L.lib, n), n
+    # and the binding gives every one of them a signature
+    from paper_1701_00426_b200 import binding
+    assert sorted(binding._sig) == names
+    assert b"sm_100a" in L.lib.lqcd_version()
+
+
+def test_library_contains_sm100a_code_only():
+    import paper_1701_00426_b200 as L
+    out = subprocess.run(["cuobjdump", "-lelf", L.lib_path], capture_output=True, text=True)
+    if out.returncode != 0:
+        pytest.skip("cuobjdump unavailable")
+    archs = set(re.findall(r"sm_\d+a?", out.stdout))
+    assert archs == {"sm_100a"}, archs
+
+
+def test_argument_errors_before_any_cuda_call():
+    import paper_1701_00426_b200 as L
+    ctx = C.c_void_p()
+    bad = [((4, 4, 4, 3), 0, 0, 1), ((4, 4, 0, 4), 0, 0, 1), ((4, 4, 4, 4), 7, 0, 1),
+           ((4, 4, 4, 4), 0, 5, 1), ((4, 4, 4, 4), 0, 0, 2), ((2048, 2048, 2048, 2), 0, 0, 1)]
+    for dims, prec, recon, ap in bad:
+        rc = L.lib.lqcd_create(C.byref(ctx), (C.c_int * 4)(*dims), prec, recon, ap, 0, None)
+        assert rc == L.ERR_ARG, (dims, prec, recon, ap, rc)
+        assert ctx.value is None
+        assert L.lib.lqcd_last_error(None) != b""
+    assert L.lib.lqcd_create(None, (C.c_int * 4)(4, 4, 4, 4), 0, 0, 1, 0, None) == L.ERR_ARG
+    # null contexts are rejected, sizes of a null context are 0
+    assert L.lib.lqcd_destroy(None) == L.ERR_ARG
+    assert L.lib.lqcd_spinor_bytes(None) == 0 and L.lib.lqcd_links_bytes(None) == 0
+    assert L.lib.lqcd_dslash(None, 0, None, None, None) == L.ERR_ARG
+    assert L.lib.lqcd_cg(None, None, None, None, 0.1, 1e-8, 10, None, None) == L.ERR_ARG
+
+
+def test_no_gpu_means_loud_failure_not_fallback():
+    import torch
+    import paper_1701_00426_b200 as L
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    ctx = C.c_void_p()
+    rc = L.lib.lqcd_create(C.byref(ctx), (C.c_int * 4)(4, 4, 4, 4), 0, 0, 1, 0, None)
+    assert rc == L.ERR_CUDA and b"no CPU fallback" in L.lib.lqcd_last_error(None)
+    with pytest.raises(L.LqcdError):
+        L.Lattice((4, 4, 4, 4))
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1701_00426_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert "staggered_oracle" not in txt and "liboracle" not in txt, f
+    for f in ("oracle/staggered_oracle.c", "oracle/oracle.py"):
+        txt = open(os.path.join(ROOT, f)).read()
+        assert "paper_1701_00426_b200" not in txt.replace("under paper_1701_00426_b200/", "") or f.endswith(".c")
+        assert "lqcd.h" not in txt and "liblqcd" not in txt
+
+
+def test_fastdiv_formula():
+    """The multiply-high division used for the site decode (common.cuh make_fastdiv), re-derived:
+    q = (n * ceil(2^(31+l)/d)) >> (31+l) for n < 2^31, l = ceil(log2 d)."""
+    rng = np.random.default_rng(0)
+    for d in [1, 2, 3, 4, 5, 6, 7, 8, 12, 16, 18, 24, 31, 32, 36, 48, 64, 96, 1000, 65535]:
+        if d == 1:
+            continue
+        l = int(np.ceil(np.log2(d)))
+        m = ((1 << (32 + l - 1)) + d - 1) // d
+        assert m < (1 << 32)
+        ns = np.concatenate([rng.integers(0, 2 ** 31 - 1, 2000), [0, 1, d - 1, d, d + 1, 2 ** 31 - 1]])
+        for n in ns:
+            n = int(n)
+            assert ((n * m) >> 32) >> (l - 1) == n // d
+
+
+def test_shift_recipe_and_generators_are_deterministic():
+    import lqcd_inputs as gen
+    s = gen.rhmc_shifts(8)
+    assert np.allclose(s, [1e-4, 3.72759372e-4, 1.38949549e-3, 5.17947468e-3, 1.93069773e-2, 7.19685673e-2, 2.68269580e-1, 1.0])
+    a = gen.smooth_links((4, 4, 2, 2), 0.3, 2)
+    b = gen.smooth_links((4, 4, 2, 2), 0.3, 2)
+    assert np.array_equal(a, b)
+    eye = np.einsum("nmab,nmcb->nmac", a, a.conj())
+    assert np.abs(eye - np.eye(3)).max() < 1e-14 and np.abs(np.linalg.det(a) - 1).max() < 1e-14
+    # eps = 0.3 links are "smoothed toward identity": Re tr U / 3 well above a Haar sample's ~0
+    assert np.mean(np.trace(a, axis1=-2, axis2=-1).real) / 3 > 0.8
+    with pytest.raises(ValueError):
+        gen.gaussian_spinor((4, 4, 3, 4), 1)
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, %r)
+from paper_1701_00426_b200 import dist as D
+rank, local_rank, world = D.init("gloo")
+assert world == 2 and rank in (0, 1)
+D.barrier(world)
+# device time differs per rank: the job time is the MAX
+t = D.max_over_ranks(10.0 + 5.0 * rank, world)
+assert t == 15.0, t
+seeds = (D.replica_seed(3, 0), D.replica_seed(3, 1))
+assert seeds[0] != seeds[1] and D.replica_seed(3, rank) == seeds[rank]
+ns = D.aggregate_ns_per_site(t, 5, 1000, world)     # 15 ms / (5 steps * 1000 sites * 2 ranks)
+assert abs(ns - 1500.0) < 1e-9, ns
+D.barrier(world)
+D.finalize(world)
+print("rank", rank, "ok")
+"""
+
+
+def test_replica_plumbing_gloo_world2(tmp_path):
+    script = tmp_path / "w.py"
+    script.write_text(_WORKER % ROOT)
+    port = 29600 + os.getpid() % 300
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE="2",
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.STDOUT, text=True))
+    outs = [p.communicate(timeout=180)[0] for p in procs]
+    for r, (p, o) in enumerate(zip(procs, outs)):
+        assert p.returncode == 0, o
+        assert f"rank {r} ok" in o
