@@ -6,8 +6,8 @@
 Workload = BASELINE.json configs[2] ("config 3" of SURVEY.md section 8(d)): 32^4 lattice, fp64,
 18-real links, U = exp(i*0.3*H) seed 3, fixed Gaussian inputs.  One STEP = D_oe (odd <- even)
 followed by D_eo (even <- odd) from FIXED inputs (no ping-pong: rho(D) > 1 would overflow),
-i.e. one pass over all V sites; --steps 500 is the config's "1000 applications, parities
-alternated".  metric = Dslash ns/site = step time / V (= time of one parity / (V/2)).
+i.e. one pass over all V sites; the default --steps 1000 is twice the config's "1000
+applications, parities alternated" (longer, so that the clock sampler sees the timed region).  metric = Dslash ns/site = step time / V (= time of one parity / (V/2)).
 
 The JSON line also carries: roofline (HBM, algorithmic 1248 B/site against MEASURED_PEAKS.json),
 e2e (same metric through lqcd_dslash_host with host buffers, copies inside the timed region),
@@ -59,7 +59,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -330,8 +330,8 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=500)
-    ap.add_argument("--warmup", type=int, default=25)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=10.0, dest="cpu_seconds")
     args = ap.parse_args()

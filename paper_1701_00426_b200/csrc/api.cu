@@ -113,7 +113,7 @@ extern "C" int lqcd_destroy(lqcd_ctx *ctx)
 struct OptDesc { const char *name; size_t off; long lo, hi; };
 #define OPT(field, lo, hi) { #field, offsetof(lqcd_ctx, field), lo, hi }
 static const OptDesc g_opts[] = {
-    OPT(layout, 0, 1), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
+    OPT(layout, 0, 1), OPT(l2_hints, 0, 1), OPT(l2_persist, 0, 4), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
     OPT(blas_block, 64, 256), OPT(blas_ctas_per_sm, 1, 32), OPT(poll_chunk, 1, 1024),
 };
 
@@ -138,6 +138,8 @@ extern "C" long lqcd_get_option(const lqcd_ctx *ctx, const char *name)
     if (!ctx || !name) return -1;
     if (!strcmp(name, "launches")) return ctx->launches;
     if (!strcmp(name, "num_sms")) return ctx->num_sms;
+    if (!strcmp(name, "l2_window_bytes")) return ctx->l2_window_bytes;
+    if (!strcmp(name, "l2_max_persist")) return ctx->l2_max_persist;
     for (const OptDesc &o : g_opts)
         if (!strcmp(o.name, name)) return *(const int *)((const char *)ctx + o.off);
     return -1;
@@ -165,6 +167,35 @@ extern "C" size_t lqcd_workspace_bytes(const lqcd_ctx *ctx, int nshift)
     return vec_stride(ctx) * (size_t)(4 + nshift);
 }
 
+// Optional (option l2_persist): ask the driver to keep the four vectors every CG iteration re-reads
+// (tmp_o, q, r, p: the head of the workspace) in the persisting part of L2 while links stream by.
+static void apply_l2_window(lqcd_ctx *ctx)
+{
+    ctx->l2_window_bytes = 0;
+    if (!ctx->l2_persist || !ctx->ws) return;
+    int max_persist = 0, max_window = 0;
+    cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, ctx->device);
+    cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, ctx->device);
+    // 1: 4 vectors, misses streaming; 2: 3 vectors (fits the carve-out), misses normal;
+    // 3: 4 vectors, misses normal; 4: 2 vectors, misses normal
+    int nvec = ctx->l2_persist == 2 ? 3 : (ctx->l2_persist == 4 ? 2 : 4);
+    size_t want = vec_stride(ctx) * nvec;
+    if (want > ctx->ws_bytes) want = ctx->ws_bytes;
+    size_t win = want < (size_t)max_window ? want : (size_t)max_window;
+    if (max_persist <= 0 || win == 0) return;
+    if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)max_persist) != cudaSuccess) { cudaGetLastError(); return; }
+    cudaStreamAttrValue v;
+    memset(&v, 0, sizeof(v));
+    v.accessPolicyWindow.base_ptr = ctx->ws;
+    v.accessPolicyWindow.num_bytes = win;
+    v.accessPolicyWindow.hitRatio = win <= (size_t)max_persist ? 1.0f : (float)max_persist / (float)win;
+    v.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+    v.accessPolicyWindow.missProp = ctx->l2_persist == 1 ? cudaAccessPropertyStreaming : cudaAccessPropertyNormal;
+    if (cudaStreamSetAttribute(ctx->stream, cudaStreamAttributeAccessPolicyWindow, &v) != cudaSuccess) { cudaGetLastError(); return; }
+    ctx->l2_window_bytes = (long)win;
+    ctx->l2_max_persist = max_persist;
+}
+
 extern "C" int lqcd_set_workspace(lqcd_ctx *ctx, void *dev_ptr, size_t bytes)
 {
     if (!ctx) return LQCD_ERR_ARG;
@@ -172,6 +203,7 @@ extern "C" int lqcd_set_workspace(lqcd_ctx *ctx, void *dev_ptr, size_t bytes)
     if (bytes < lqcd_workspace_bytes(ctx, 1)) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "lqcd_set_workspace: %zu bytes < minimum %zu", bytes, lqcd_workspace_bytes(ctx, 1));
     ctx->ws = dev_ptr;
     ctx->ws_bytes = bytes;
+    apply_l2_window(ctx);
     return LQCD_OK;
 }
 

@@ -59,35 +59,129 @@ template <typename T> struct Cx { T re, im; };
 
 template <typename T> __device__ __forceinline__ Cx<T> cx(T re, T im) { Cx<T> z; z.re = re; z.im = im; return z; }
 
-// ---- loads with cache policy -------------------------------------------------------------
-// STREAM = 1: links, read exactly once per Dslash -> ld.global.cs (evict-first in L1/L2), so the
-// 126 MB L2 keeps the input spinor, which every output site's 8 neighbours re-read.
-template <typename T, int LAYOUT, int STREAM>
-__device__ __forceinline__ Cx<T> ld_cx(const T *__restrict__ base, size_t plane, size_t Vh, size_t i)
+// ---- loads / stores with cache policy -----------------------------------------------------
+// Links are read exactly once per Dslash; half-lattice vectors are re-read (8 neighbours, and by
+// the next kernel of a CG iteration).  POLICY selects how that is told to the memory system:
+//   POLICY 0: links ld.global.cs (streaming, evict-first), vectors ld.global.nc / plain stores
+//   POLICY 1: explicit L2 cache hints (createpolicy): links L2::evict_first + L1::no_allocate,
+//             vectors L2::evict_last on loads AND stores, so that the 126 MB L2 keeps the
+//             25 MB vectors of a 32^4 lattice resident while 604 MB of links stream through.
+__device__ __forceinline__ uint64_t l2_policy_evict_first()
+{
+    uint64_t p;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_last()
+{
+    uint64_t p;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+struct L2Pol { uint64_t stream, keep; };
+__device__ __forceinline__ L2Pol make_l2pol() { L2Pol p; p.stream = l2_policy_evict_first(); p.keep = l2_policy_evict_last(); return p; }
+
+__device__ __forceinline__ double2 ld_hint_stream(const double2 *p, uint64_t pol)
+{
+    double2 v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ float2 ld_hint_stream(const float2 *p, uint64_t pol)
+{
+    float2 v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double ld_hint_stream(const double *p, uint64_t pol)
+{
+    double v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ float ld_hint_stream(const float *p, uint64_t pol)
+{
+    float v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double2 ld_hint_keep(const double2 *p, uint64_t pol)
+{
+    double2 v;
+    asm("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ float2 ld_hint_keep(const float2 *p, uint64_t pol)
+{
+    float2 v;
+    asm("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double ld_hint_keep(const double *p, uint64_t pol)
+{
+    double v;
+    asm("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ float ld_hint_keep(const float *p, uint64_t pol)
+{
+    float v;
+    asm("ld.global.nc.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ void st_hint_keep(double2 *p, double2 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_hint_keep(float2 *p, float2 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1,%2}, %3;" ::"l"(p), "f"(v.x), "f"(v.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_hint_keep(double *p, double v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_hint_keep(float *p, float v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(p), "f"(v), "l"(pol) : "memory");
+}
+
+// STREAM = 1: link load; 0: vector load.
+template <typename T, int LAYOUT, int STREAM, int POLICY>
+__device__ __forceinline__ Cx<T> ld_cx(const T *__restrict__ base, size_t plane, size_t Vh, size_t i, const L2Pol &pol)
 {
     Cx<T> z;
     if (LAYOUT == 0) {
         typedef typename Vec2<T>::type V2;
         const V2 *p = reinterpret_cast<const V2 *>(base) + plane * Vh + i;
-        V2 v = STREAM ? __ldcs(p) : __ldg(p);
+        V2 v;
+        if (POLICY == 0) v = STREAM ? __ldcs(p) : __ldg(p);
+        else v = STREAM ? ld_hint_stream(p, pol.stream) : ld_hint_keep(p, pol.keep);
         z.re = v.x; z.im = v.y;
     } else {
         const T *p = base + (2 * plane) * Vh + i;
-        z.re = STREAM ? __ldcs(p) : __ldg(p);
-        z.im = STREAM ? __ldcs(p + Vh) : __ldg(p + Vh);
+        if (POLICY == 0) {
+            z.re = STREAM ? __ldcs(p) : __ldg(p);
+            z.im = STREAM ? __ldcs(p + Vh) : __ldg(p + Vh);
+        } else {
+            z.re = STREAM ? ld_hint_stream(p, pol.stream) : ld_hint_keep(p, pol.keep);
+            z.im = STREAM ? ld_hint_stream(p + Vh, pol.stream) : ld_hint_keep(p + Vh, pol.keep);
+        }
     }
     return z;
 }
-template <typename T, int LAYOUT>
-__device__ __forceinline__ void st_cx(T *__restrict__ base, size_t plane, size_t Vh, size_t i, Cx<T> z)
+template <typename T, int LAYOUT, int POLICY>
+__device__ __forceinline__ void st_cx(T *__restrict__ base, size_t plane, size_t Vh, size_t i, Cx<T> z, const L2Pol &pol)
 {
     if (LAYOUT == 0) {
         typedef typename Vec2<T>::type V2;
         V2 v; v.x = z.re; v.y = z.im;
-        reinterpret_cast<V2 *>(base)[plane * Vh + i] = v;
+        V2 *p = reinterpret_cast<V2 *>(base) + plane * Vh + i;
+        if (POLICY == 0) *p = v; else st_hint_keep(p, v, pol.keep);
     } else {
-        base[(2 * plane) * Vh + i] = z.re;
-        base[(2 * plane + 1) * Vh + i] = z.im;
+        T *p = base + (2 * plane) * Vh + i;
+        if (POLICY == 0) { p[0] = z.re; p[Vh] = z.im; }
+        else { st_hint_keep(p, z.re, pol.keep); st_hint_keep(p + Vh, z.im, pol.keep); }
     }
 }
 
@@ -120,6 +214,9 @@ struct lqcd_ctx {
     cudaStream_t stream;
     int layout;            // 0 interleaved complex, 1 split re/im
     int layout_locked;
+    int l2_persist;        // 1: persisting-L2 access-policy window over the CG vectors
+    long l2_window_bytes, l2_max_persist;
+    int l2_hints;          // 0: ld.cs / plain, 1: explicit L2 evict_first / evict_last hints
     int dslash_block;      // threads per CTA of the Dslash kernel
     int dslash_minblocks;  // launch-bounds variant (occupancy target)
     int blas_block, blas_ctas_per_sm;

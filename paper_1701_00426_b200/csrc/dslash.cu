@@ -17,8 +17,8 @@
 
 template <typename T> struct Su3 { Cx<T> e[3][3]; };
 
-template <typename T, int LAYOUT, int RECON12>
-__device__ __forceinline__ Su3<T> load_link(const T *__restrict__ links, int par, int mu, size_t Vh, size_t i)
+template <typename T, int LAYOUT, int RECON12, int POLICY>
+__device__ __forceinline__ Su3<T> load_link(const T *__restrict__ links, int par, int mu, size_t Vh, size_t i, const L2Pol &pol)
 {
     constexpr int R = RECON12 ? 2 : 3;
     Su3<T> u;
@@ -26,7 +26,7 @@ __device__ __forceinline__ Su3<T> load_link(const T *__restrict__ links, int par
 #pragma unroll
     for (int r = 0; r < R; ++r)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) u.e[r][c] = ld_cx<T, LAYOUT, 1>(links, plane0 + r * 3 + c, Vh, i);
+        for (int c = 0; c < 3; ++c) u.e[r][c] = ld_cx<T, LAYOUT, 1, POLICY>(links, plane0 + r * 3 + c, Vh, i, pol);
     if (RECON12) {
         // r2[k] = conj( eps_kij r0[i] r1[j] )   (reading R8)
 #pragma unroll
@@ -41,12 +41,12 @@ __device__ __forceinline__ Su3<T> load_link(const T *__restrict__ links, int par
     return u;
 }
 
-template <typename T, int LAYOUT>
-__device__ __forceinline__ void load_vec(const T *__restrict__ v, size_t Vh, size_t i, T coef, Cx<T> p[3])
+template <typename T, int LAYOUT, int POLICY>
+__device__ __forceinline__ void load_vec(const T *__restrict__ v, size_t Vh, size_t i, T coef, Cx<T> p[3], const L2Pol &pol)
 {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        Cx<T> z = ld_cx<T, LAYOUT, 0>(v, (size_t)c, Vh, i);
+        Cx<T> z = ld_cx<T, LAYOUT, 0, POLICY>(v, (size_t)c, Vh, i, pol);
         p[c] = cx<T>(coef * z.re, coef * z.im);
     }
 }
@@ -79,7 +79,7 @@ template <typename T> __device__ __forceinline__ void mvdag_acc(Cx<T> acc[3], co
 }
 
 // MODE 0: out = D in;  1: out = coef*x - D in;  2: as 1, plus Re<x,out> -> solver_after_pq
-template <typename T, int LAYOUT, int RECON12, int MODE, int MINB>
+template <typename T, int LAYOUT, int RECON12, int MODE, int MINB, int POLICY>
 __global__ void __launch_bounds__(256, MINB)
 dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__restrict__ in,
               const T *__restrict__ links, const T *__restrict__ xin, const double coef,
@@ -95,6 +95,8 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < g.Vh;
     double dot = 0.0;
+    L2Pol pol = {0, 0};
+    if (POLICY) pol = make_l2pol();
     if (valid) {
         const size_t Vh = (size_t)g.Vh;
         // ---- a2: site decode (Eq. 9), neighbours, phases ---------------------------------
@@ -134,15 +136,15 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
             {
-                Su3<T> u = load_link<T, LAYOUT, RECON12>(links, parity, mu, Vh, (size_t)i);
+                Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, parity, mu, Vh, (size_t)i, pol);
                 Cx<T> p[3];
-                load_vec<T, LAYOUT>(in, Vh, (size_t)nf[mu], cf[mu], p);
+                load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], p, pol);
                 mv_acc<T>(acc, u, p);
             }
             {
-                Su3<T> u = load_link<T, LAYOUT, RECON12>(links, 1 - parity, mu, Vh, (size_t)nb[mu]);
+                Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, 1 - parity, mu, Vh, (size_t)nb[mu], pol);
                 Cx<T> p[3];
-                load_vec<T, LAYOUT>(in, Vh, (size_t)nb[mu], cb[mu], p);
+                load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], p, pol);
                 mvdag_acc<T>(acc, u, p);
             }
         }
@@ -151,13 +153,13 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
             const T cm = (T)coef;
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                Cx<T> x = ld_cx<T, LAYOUT, 0>(xin, (size_t)c, Vh, (size_t)i);
+                Cx<T> x = ld_cx<T, LAYOUT, 0, POLICY>(xin, (size_t)c, Vh, (size_t)i, pol);
                 acc[c] = cx<T>(fma(cm, x.re, -acc[c].re), fma(cm, x.im, -acc[c].im));
                 if (MODE == 2) dot += (double)x.re * (double)acc[c].re + (double)x.im * (double)acc[c].im;
             }
         }
 #pragma unroll
-        for (int c = 0; c < 3; ++c) st_cx<T, LAYOUT>(out, (size_t)c, Vh, (size_t)i, acc[c]);
+        for (int c = 0; c < 3; ++c) st_cx<T, LAYOUT, POLICY>(out, (size_t)c, Vh, (size_t)i, acc[c], pol);
     }
     if (MODE == 2) {
         double total;
@@ -173,10 +175,12 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
     dim3 grid((ctx->g.Vh + block - 1) / block);
     int minb = ctx->dslash_minblocks;
     if (minb == 0) minb = sizeof(T) == 8 ? 2 : 3;
-#define GO(MB) dslash_kernel<T, LAYOUT, RECON12, MODE, MB><<<grid, block, 0, ctx->stream>>>( \
+#define GO1(MB, P) dslash_kernel<T, LAYOUT, RECON12, MODE, MB, P><<<grid, block, 0, ctx->stream>>>( \
         ctx->g, parity, (T *)out, (const T *)in, (const T *)links, (const T *)xin, coef, ctx->d_state, ctx->d_partials, gate)
-    if (minb <= 1) GO(1); else if (minb == 2) GO(2); else if (minb == 3) GO(3); else GO(4);
+#define GO(MB) do { if (ctx->l2_hints) GO1(MB, 1); else GO1(MB, 0); } while (0)
+    if (minb <= 2) GO(2); else if (minb == 3) GO(3); else GO(4);
 #undef GO
+#undef GO1
 }
 
 template <typename T, int LAYOUT>

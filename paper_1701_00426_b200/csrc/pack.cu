@@ -28,7 +28,7 @@ __global__ void pack_links_kernel(Geom g, int rows, T *__restrict__ native, cons
             for (int c = 0; c < 3; ++c) {
                 double2 z = canon[(lex * 4 + mu) * 9 + r * 3 + c];
                 size_t plane = ((size_t)(par * 4 + mu) * rows + r) * 3 + c;
-                st_cx<T, LAYOUT>(native, plane, (size_t)g.Vh, (size_t)i, cx<T>((T)z.x, (T)z.y));
+                st_cx<T, LAYOUT, 0>(native, plane, (size_t)g.Vh, (size_t)i, cx<T>((T)z.x, (T)z.y), L2Pol());
             }
 }
 
@@ -39,7 +39,7 @@ __global__ void pack_spinor_kernel(Geom g, T *__restrict__ native, const double2
     if (i >= g.Vh) return;
     for (int c = 0; c < 3; ++c) {
         double2 z = canon[(size_t)i * 3 + c];
-        st_cx<T, LAYOUT>(native, (size_t)c, (size_t)g.Vh, (size_t)i, cx<T>((T)z.x, (T)z.y));
+        st_cx<T, LAYOUT, 0>(native, (size_t)c, (size_t)g.Vh, (size_t)i, cx<T>((T)z.x, (T)z.y), L2Pol());
     }
 }
 
@@ -49,7 +49,7 @@ __global__ void unpack_spinor_kernel(Geom g, double2 *__restrict__ canon, const 
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.Vh) return;
     for (int c = 0; c < 3; ++c) {
-        Cx<T> z = ld_cx<T, LAYOUT, 0>(native, (size_t)c, (size_t)g.Vh, (size_t)i);
+        Cx<T> z = ld_cx<T, LAYOUT, 0, 0>(native, (size_t)c, (size_t)g.Vh, (size_t)i, L2Pol());
         canon[(size_t)i * 3 + c] = make_double2((double)z.re, (double)z.im);
     }
 }

@@ -27,6 +27,34 @@ template <typename T> __device__ __forceinline__ void unpack(const float4 &v, T 
 __device__ __forceinline__ double2 repack(const double *a) { return make_double2(a[0], a[1]); }
 __device__ __forceinline__ float4 repack(const float *a) { return make_float4(a[0], a[1], a[2], a[3]); }
 
+// 16-byte vector loads / stores of the flat kernels; POLICY 1 adds L2::evict_last so that the
+// CG vectors stay L2-resident between kernels (common.cuh).  Plain (coherent) loads: these
+// kernels read and write the same buffers.
+template <int POLICY> __device__ __forceinline__ double2 ldv(const double2 *p, uint64_t pol)
+{
+    if (POLICY == 0) return *p;
+    double2 v;
+    asm volatile("ld.global.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+template <int POLICY> __device__ __forceinline__ float4 ldv(const float4 *p, uint64_t pol)
+{
+    if (POLICY == 0) return *p;
+    float4 v;
+    asm volatile("ld.global.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+template <int POLICY> __device__ __forceinline__ void stv(double2 *p, double2 v, uint64_t pol)
+{
+    if (POLICY == 0) { *p = v; return; }
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+template <int POLICY> __device__ __forceinline__ void stv(float4 *p, float4 v, uint64_t pol)
+{
+    if (POLICY == 0) { *p = v; return; }
+    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(pol) : "memory");
+}
+
 struct ShiftPtrs {
     void *x[LQCD_MAX_SHIFTS];
     void *p[LQCD_MAX_SHIFTS];
@@ -34,25 +62,27 @@ struct ShiftPtrs {
 };
 
 // r = p = p_i = b, x_i = 0, rho = ||b||^2
-template <typename T>
+template <typename T, int POLICY>
 __global__ void __launch_bounds__(256) init_kernel(size_t npk, const T *__restrict__ b, T *__restrict__ r,
                                                    T *__restrict__ p, ShiftPtrs sp, SolverState *st,
                                                    double *partials)
 {
     typedef typename Pack<T>::type P;
     const int N = Pack<T>::N;
+    const uint64_t keep = POLICY ? l2_policy_evict_last() : 0;
+    const uint64_t strm = POLICY ? l2_policy_evict_first() : 0;
     double acc = 0.0;
     T zero[4] = {0, 0, 0, 0};
     for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
-        P v = reinterpret_cast<const P *>(b)[k];
+        P v = ldv<POLICY>(reinterpret_cast<const P *>(b) + k, keep);
         T a[4];
         unpack<T>(v, a);
         for (int j = 0; j < N; ++j) acc += (double)a[j] * (double)a[j];
-        reinterpret_cast<P *>(r)[k] = v;
-        reinterpret_cast<P *>(p)[k] = v;
+        stv<POLICY>(reinterpret_cast<P *>(r) + k, v, keep);
+        stv<POLICY>(reinterpret_cast<P *>(p) + k, v, keep);
         for (int i = 0; i < sp.nshift; ++i) {
-            reinterpret_cast<P *>(sp.x[i])[k] = repack(zero);
-            if (i != sp.base) reinterpret_cast<P *>(sp.p[i])[k] = v;
+            stv<POLICY>(reinterpret_cast<P *>(sp.x[i]) + k, repack(zero), strm);
+            if (i != sp.base) stv<POLICY>(reinterpret_cast<P *>(sp.p[i]) + k, v, strm);
         }
     }
     double total;
@@ -64,24 +94,25 @@ __global__ void __launch_bounds__(256) init_kernel(size_t npk, const T *__restri
 }
 
 // K1: r -= alpha q ; <r,r>
-template <typename T>
+template <typename T, int POLICY>
 __global__ void __launch_bounds__(256) k1_kernel(size_t npk, T *__restrict__ r, const T *__restrict__ q,
                                                  SolverState *st, double *partials)
 {
     if (*(volatile int *)&st->done) return;
     typedef typename Pack<T>::type P;
     const int N = Pack<T>::N;
+    const uint64_t keep = POLICY ? l2_policy_evict_last() : 0;
     const T alpha = (T)st->alpha;
     double acc = 0.0;
     for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
         T a[4], c[4];
-        unpack<T>(reinterpret_cast<const P *>(r)[k], a);
-        unpack<T>(reinterpret_cast<const P *>(q)[k], c);
+        unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(r) + k, keep), a);
+        unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(q) + k, keep), c);
         for (int j = 0; j < N; ++j) {
             a[j] = fma(-alpha, c[j], a[j]);
             acc += (double)a[j] * (double)a[j];
         }
-        reinterpret_cast<P *>(r)[k] = repack(a);
+        stv<POLICY>(reinterpret_cast<P *>(r) + k, repack(a), keep);
     }
     double total;
     if (grid_sum_last(acc, partials, &st->ticket, &total)) solver_after_rr(st, total);
@@ -89,13 +120,17 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, T *__restrict__ r, 
 
 // K2: x_i += alpha_i p_i ; p_i = zeta_i r + beta_i p_i ; p = r + beta p.  The base shift has
 // zeta = 1 and p_base == p, so its direction vector is not stored.
-template <typename T>
+template <typename T, int POLICY>
 __global__ void __launch_bounds__(256) k2_kernel(size_t npk, const T *__restrict__ r, T *__restrict__ p,
                                                  ShiftPtrs sp, const SolverState *__restrict__ st)
 {
     if (*(volatile const int *)&st->done == 2) return;
     typedef typename Pack<T>::type P;
     const int N = Pack<T>::N;
+    // r and p are re-read by the next kernels: keep.  x_i, p_i are touched once per iteration and
+    // together exceed L2 for several shifts: stream them through.
+    const uint64_t keep = POLICY ? l2_policy_evict_last() : 0;
+    const uint64_t strm = POLICY ? l2_policy_evict_first() : 0;
     __shared__ T s_alpha[LQCD_MAX_SHIFTS], s_zeta[LQCD_MAX_SHIFTS], s_beta[LQCD_MAX_SHIFTS];
     __shared__ int s_active[LQCD_MAX_SHIFTS];
     if (threadIdx.x < sp.nshift) {
@@ -108,42 +143,43 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, const T *__restrict
     const T beta = (T)st->beta;
     for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
         T rr[4], pp[4];
-        unpack<T>(reinterpret_cast<const P *>(r)[k], rr);
-        unpack<T>(reinterpret_cast<const P *>(p)[k], pp);
+        unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(r) + k, keep), rr);
+        unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(p) + k, keep), pp);
         for (int i = 0; i < sp.nshift; ++i) {
             if (!s_active[i]) continue;
             T xx[4];
-            unpack<T>(reinterpret_cast<const P *>(sp.x[i])[k], xx);
+            unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(sp.x[i]) + k, strm), xx);
             if (i == sp.base) {
                 for (int j = 0; j < N; ++j) xx[j] = fma(s_alpha[i], pp[j], xx[j]);
             } else {
                 T pi[4];
-                unpack<T>(reinterpret_cast<const P *>(sp.p[i])[k], pi);
+                unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(sp.p[i]) + k, strm), pi);
                 for (int j = 0; j < N; ++j) {
                     xx[j] = fma(s_alpha[i], pi[j], xx[j]);
                     pi[j] = fma(s_beta[i], pi[j], s_zeta[i] * rr[j]);
                 }
-                reinterpret_cast<P *>(sp.p[i])[k] = repack(pi);
+                stv<POLICY>(reinterpret_cast<P *>(sp.p[i]) + k, repack(pi), strm);
             }
-            reinterpret_cast<P *>(sp.x[i])[k] = repack(xx);
+            stv<POLICY>(reinterpret_cast<P *>(sp.x[i]) + k, repack(xx), strm);
         }
         for (int j = 0; j < N; ++j) pp[j] = fma(beta, pp[j], rr[j]);
-        reinterpret_cast<P *>(p)[k] = repack(pp);
+        stv<POLICY>(reinterpret_cast<P *>(p) + k, repack(pp), keep);
     }
 }
 
 // ||a - b||^2 -> *slot
-template <typename T>
+template <typename T, int POLICY>
 __global__ void __launch_bounds__(256) diffnorm_kernel(size_t npk, const T *__restrict__ a, const T *__restrict__ b,
                                                        SolverState *st, double *partials, double *slot)
 {
     typedef typename Pack<T>::type P;
     const int N = Pack<T>::N;
+    const uint64_t keep = POLICY ? l2_policy_evict_last() : 0;
     double acc = 0.0;
     for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
         T x[4], y[4];
-        unpack<T>(reinterpret_cast<const P *>(a)[k], x);
-        unpack<T>(reinterpret_cast<const P *>(b)[k], y);
+        unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(a) + k, keep), x);
+        unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(b) + k, keep), y);
         for (int j = 0; j < N; ++j) { double d = (double)x[j] - (double)y[j]; acc += d * d; }
     }
     double total;
@@ -190,7 +226,8 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     }
     int rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(ctx->d_state, &h, sizeof(h), cudaMemcpyHostToDevice, s), "solver state upload");
     if (rc) return rc;
-    init_kernel<T><<<grid, block, 0, s>>>(npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
+    if (ctx->l2_hints) init_kernel<T, 1><<<grid, block, 0, s>>>(npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
+    else init_kernel<T, 0><<<grid, block, 0, s>>>(npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
     ctx->launches++;
 
     const double msq = mass * mass + shifts[base];
@@ -203,8 +240,13 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         for (int k = 0; k < n; ++k) {
             if ((rc = launch_dslash(ctx, LQCD_ODD, tmp_o, p, links, NULL, 0.0, 0, 2))) return rc;
             if ((rc = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, p, msq, 1, 1))) return rc;
-            k1_kernel<T><<<grid, block, 0, s>>>(npk, r, q, ctx->d_state, ctx->d_partials);
-            k2_kernel<T><<<grid, block, 0, s>>>(npk, r, p, sp, ctx->d_state);
+            if (ctx->l2_hints) {
+                k1_kernel<T, 1><<<grid, block, 0, s>>>(npk, r, q, ctx->d_state, ctx->d_partials);
+                k2_kernel<T, 1><<<grid, block, 0, s>>>(npk, r, p, sp, ctx->d_state);
+            } else {
+                k1_kernel<T, 0><<<grid, block, 0, s>>>(npk, r, q, ctx->d_state, ctx->d_partials);
+                k2_kernel<T, 0><<<grid, block, 0, s>>>(npk, r, p, sp, ctx->d_state);
+            }
             ctx->launches += 2;
         }
         enq += n;
@@ -224,7 +266,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     for (int i = 0; i < nshift; ++i) {
         if ((rc = launch_dslash(ctx, LQCD_ODD, tmp_o, xs[i], links, NULL, 0.0, 0, 0))) return rc;
         if ((rc = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, xs[i], mass * mass + shifts[i], 0, 0))) return rc;
-        diffnorm_kernel<T><<<grid, block, 0, s>>>(npk, (const T *)b, q, ctx->d_state, ctx->d_partials, &ctx->d_state->resid[i]);
+        diffnorm_kernel<T, 0><<<grid, block, 0, s>>>(npk, (const T *)b, q, ctx->d_state, ctx->d_partials, &ctx->d_state->resid[i]);
         ctx->launches++;
     }
     if ((rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(&h, ctx->d_state, sizeof(h), cudaMemcpyDeviceToHost, s), "solver state download"))) return rc;
