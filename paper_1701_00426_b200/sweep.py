@@ -1,0 +1,165 @@
+"""Volume sweep and solve-to-tolerance runs (BASELINE.json configs[3] and configs[4]).
+
+    python -m paper_1701_00426_b200.sweep --ladder            # config 5: ns/site, GB/s vs volume
+    python -m paper_1701_00426_b200.sweep --multishift        # config 4: 24^3x48 and 32^4 solves
+    python -m paper_1701_00426_b200.sweep --dims 16,16,16,16 --ladder
+
+Prints one JSON line per measurement and, with --md FILE, appends a Markdown table.  Timing is by
+CUDA events on the launching stream after warm-up.  Volumes whose links fit the 126 MB L2 are
+labelled "L2" (they are not HBM measurements).  Inputs are the seeded synthetic
+fields of lqcd_inputs; nothing here touches oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+L2_BYTES = 126e6
+BYTES = {(0, 0): 1248, (0, 1): 864, (1, 0): 624, (1, 1): 432}
+LADDER = [(8,) * 4, (12,) * 4, (16,) * 4, (20,) * 4, (24,) * 4, (32, 32, 8, 32), (32, 32, 32, 8), (32,) * 4,
+          (32, 32, 32, 36), (40,) * 4, (64, 64, 64, 16), (48,) * 4]
+
+
+def ev_time_us(torch, fn, n, warm):
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(n):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / n * 1e3
+
+
+def iter_time_us(torch, lat, links, b, shifts, mass, n_lo, n_hi):
+    """(multi-shift) CG time per iteration from two fixed-length solves (unreachable tol)."""
+    xs = [lat.new_spinor() for _ in shifts]
+
+    def solve(n):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        lat.cg_multishift(xs, b, links, mass, shifts, 1e-300, n, raise_on_max_iter=False)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    solve(n_lo)
+    t_lo = min(solve(n_lo) for _ in range(2))
+    t_hi = min(solve(n_hi) for _ in range(2))
+    return (t_hi - t_lo) / (n_hi - n_lo) * 1e3
+
+
+def ladder(dims_list, eps, seed, out):
+    import numpy as np
+    import torch
+    import lqcd_inputs as gen
+    import paper_1701_00426_b200 as L
+
+    for dims in dims_list:
+        V = gen.volume(dims)
+        Vh = V // 2
+        t0 = time.time()
+        rng = np.random.default_rng(seed)
+        U = gen.smooth_links(dims, eps, rng)
+        ie, io = gen.gaussian_half_spinor(dims, rng), gen.gaussian_half_spinor(dims, rng)
+        gen_s = time.time() - t0
+        for prec in (0, 1):
+            for recon in (0, 1):
+                lat = L.Lattice(dims, prec=prec, recon=recon)
+                links = lat.pack_links(U)
+                a, b = lat.pack_spinor(ie, 0), lat.pack_spinor(io, 1)
+                oo, oe = lat.new_spinor(), lat.new_spinor()
+
+                def step():
+                    lat.dslash(1, oo, a, links)
+                    lat.dslash(0, oe, b, links)
+                n = max(20, min(500, int(2e8 / V)))
+                us = ev_time_us(torch, step, n, 5) / 2
+                rec = dict(kind="dslash", dims="x".join(map(str, dims)), V=V, prec=("f64", "f32")[prec],
+                           links=(18, 12)[recon], us=round(us, 2), ns_per_site=round(us * 1e3 / Vh, 4),
+                           GBs=round(BYTES[(prec, recon)] * Vh / us / 1e3, 1),
+                           GFLOPs=round(570 * Vh / us / 1e3, 1),
+                           regime="L2" if lat.links_bytes < L2_BYTES else "HBM", gen_s=round(gen_s, 1))
+                out(rec)
+                if recon == 0:
+                    it_us = iter_time_us(torch, lat, links, a, [0.0], 0.01, 20, 220)   # config 5: 200 iterations
+                    es = 8 if prec == 0 else 4
+                    by = (2 * (18 * 8 + 12) + 6 + 18 + 30) * es
+                    out(dict(kind="cg", dims=rec["dims"], V=V, prec=rec["prec"], links=18, us_per_iter=round(it_us, 2),
+                             iter_per_s=round(1e6 / it_us, 1), GBs=round(by * Vh / it_us / 1e3, 1), regime=rec["regime"]))
+                lat.close()
+                del links, a, b, oo, oe
+        del U
+
+
+def multishift(dims_list, out):
+    import numpy as np
+    import torch
+    import lqcd_inputs as gen
+    import paper_1701_00426_b200 as L
+
+    for dims in dims_list:
+        rng = np.random.default_rng(4)
+        U = gen.smooth_links(dims, 0.3, rng)
+        b = gen.gaussian_half_spinor(dims, rng)
+        shifts = gen.rhmc_shifts(8)
+        lat = L.Lattice(dims)
+        links, be = lat.pack_links(U), lat.pack_spinor(b, 0)
+        xs = [lat.new_spinor() for _ in shifts]
+        lat.cg_multishift(xs, be, links, 0.0025, shifts, 1e-10, 50, raise_on_max_iter=False)   # warm-up
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        res = lat.cg_multishift(xs, be, links, 0.0025, shifts, 1e-10, 50000)
+        dt = time.perf_counter() - t0
+        out(dict(kind="multishift_solve", dims="x".join(map(str, dims)), mass=0.0025, tol=1e-10, iters=res["iters"],
+                 conv_iter=res["conv_iter"].tolist(), max_true_rel_resid=float(res["rel_resid"].max()),
+                 seconds=round(dt, 4), iter_per_s=round(res["iters"] / dt, 1)))
+        lat.close()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--ladder", action="store_true")
+    ap.add_argument("--multishift", action="store_true")
+    ap.add_argument("--dims", default=None, help="comma-separated N0,N1,N2,N3 (repeatable with ';')")
+    ap.add_argument("--eps", type=float, default=0.5)
+    ap.add_argument("--seed", type=int, default=5)
+    ap.add_argument("--md", default=None)
+    args = ap.parse_args()
+    dims_list = None
+    if args.dims:
+        dims_list = [tuple(int(x) for x in d.split(",")) for d in args.dims.split(";")]
+    rows = []
+
+    def out(rec):
+        rows.append(rec)
+        print(json.dumps(rec), flush=True)
+
+    if args.ladder:
+        ladder(dims_list or LADDER, args.eps, args.seed, out)
+    if args.multishift:
+        multishift(dims_list or [(24, 24, 24, 48), (32, 32, 32, 32)], out)
+    if args.md:
+        with open(args.md, "a") as f:
+            for kind in ("dslash", "cg", "multishift_solve"):
+                sel = [r for r in rows if r["kind"] == kind]
+                if not sel:
+                    continue
+                keys = [k for k in sel[0] if k != "kind"]
+                f.write(f"\n### {kind}\n\n| " + " | ".join(keys) + " |\n|" + "---|" * len(keys) + "\n")
+                for r in sel:
+                    f.write("| " + " | ".join(str(r[k]) for k in keys) + " |\n")
+
+
+if __name__ == "__main__":
+    main()
