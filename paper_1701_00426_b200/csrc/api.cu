@@ -63,6 +63,7 @@ extern "C" int lqcd_create(lqcd_ctx **out, const int dims[4], int prec, int reco
     g.N0 = dims[0]; g.N1 = dims[1]; g.N2 = dims[2]; g.N3 = dims[3];
     g.Nh0 = g.N0 / 2;
     g.Vh = (int)(V / 2);
+    g.Ls = g.Vh;
     g.s1 = g.Nh0; g.s2 = g.Nh0 * g.N1; g.s3 = g.Nh0 * g.N1 * g.N2;
     g.ap = antiperiodic_t;
     g.dNh0 = make_fastdiv((uint32_t)g.Nh0);
@@ -113,7 +114,7 @@ extern "C" int lqcd_destroy(lqcd_ctx *ctx)
 struct OptDesc { const char *name; size_t off; long lo, hi; };
 #define OPT(field, lo, hi) { #field, offsetof(lqcd_ctx, field), lo, hi }
 static const OptDesc g_opts[] = {
-    OPT(layout, 0, 1), OPT(l2_hints, 0, 1), OPT(l2_persist, 0, 4), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
+    OPT(layout, 0, 1), OPT(l2_hints, 0, 1), OPT(l2_persist, 0, 4), OPT(link_pad, 0, 1 << 20), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
     OPT(blas_block, 64, 256), OPT(blas_ctas_per_sm, 1, 32), OPT(poll_chunk, 1, 1024),
 };
 
@@ -127,6 +128,11 @@ extern "C" int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value)
             return lqcd_fail(ctx, LQCD_ERR_ARG, "option layout: fields were already packed in layout %d", ctx->layout);
         if ((!strcmp(name, "dslash_block") || !strcmp(name, "blas_block")) && (value % 32))
             return lqcd_fail(ctx, LQCD_ERR_ARG, "option %s must be a multiple of 32", name);
+        if (!strcmp(name, "link_pad")) {
+            if (ctx->layout_locked && value != ctx->link_pad) return lqcd_fail(ctx, LQCD_ERR_ARG, "option link_pad: fields were already packed");
+            if (value % 8) return lqcd_fail(ctx, LQCD_ERR_ARG, "option link_pad must be a multiple of 8 sites");
+            ctx->g.Ls = ctx->g.Vh + (int)value;
+        }
         *(int *)((char *)ctx + o.off) = (int)value;
         return LQCD_OK;
     }
@@ -154,7 +160,7 @@ extern "C" size_t lqcd_links_bytes(const lqcd_ctx *ctx)
 {
     if (!ctx) return 0;
     size_t rows = ctx->recon == LQCD_RECON_12 ? 2 : 3;
-    return (size_t)ctx->g.Vh * 2 * 4 * rows * 3 * 2 * elem_size(ctx);
+    return (size_t)ctx->g.Ls * 2 * 4 * rows * 3 * 2 * elem_size(ctx);
 }
 
 // workspace = tmp_o, q, r, p  +  one p_i per shift (the base shift's is unused but keeps indexing

@@ -38,6 +38,7 @@ struct Geom {
     int N0, N1, N2, N3;   // extents (all even)
     int Nh0;              // N0/2
     int Vh;               // sites per parity
+    int Ls;               // link plane stride in sites (Vh + link_pad): breaks the power-of-two plane spacing
     int s1, s2, s3;       // idxh strides of x1, x2, x3: Nh0, Nh0*N1, Nh0*N1*N2
     int ap;               // antiperiodic in x3
     FastDiv dNh0, dN1, dN2;
@@ -214,6 +215,7 @@ struct lqcd_ctx {
     cudaStream_t stream;
     int layout;            // 0 interleaved complex, 1 split re/im
     int layout_locked;
+    int link_pad;          // extra sites between link planes
     int l2_persist;        // 1: persisting-L2 access-policy window over the CG vectors
     long l2_window_bytes, l2_max_persist;
     int l2_hints;          // 0: ld.cs / plain, 1: explicit L2 evict_first / evict_last hints

@@ -136,13 +136,13 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
             {
-                Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, parity, mu, Vh, (size_t)i, pol);
+                Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, parity, mu, (size_t)g.Ls, (size_t)i, pol);
                 Cx<T> p[3];
                 load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], p, pol);
                 mv_acc<T>(acc, u, p);
             }
             {
-                Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, 1 - parity, mu, Vh, (size_t)nb[mu], pol);
+                Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, 1 - parity, mu, (size_t)g.Ls, (size_t)nb[mu], pol);
                 Cx<T> p[3];
                 load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], p, pol);
                 mvdag_acc<T>(acc, u, p);

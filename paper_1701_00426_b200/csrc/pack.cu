@@ -28,7 +28,7 @@ __global__ void pack_links_kernel(Geom g, int rows, T *__restrict__ native, cons
             for (int c = 0; c < 3; ++c) {
                 double2 z = canon[(lex * 4 + mu) * 9 + r * 3 + c];
                 size_t plane = ((size_t)(par * 4 + mu) * rows + r) * 3 + c;
-                st_cx<T, LAYOUT, 0>(native, plane, (size_t)g.Vh, (size_t)i, cx<T>((T)z.x, (T)z.y), L2Pol());
+                st_cx<T, LAYOUT, 0>(native, plane, (size_t)g.Ls, (size_t)i, cx<T>((T)z.x, (T)z.y), L2Pol());
             }
 }
 
