@@ -271,3 +271,90 @@ def test_host_entry_points():
     for i in range(2):
         assert rel(sol[i], ref["x"][i]) < 1e-6
     lat.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# Full size, in the launch configuration bench.py times (BASELINE.json configs[2]: 32^4)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec,recon", [(0, 0), (0, 1), (1, 0), (1, 1)])
+def test_dslash_32x4_bench_configuration(prec, recon):
+    """Same inputs (eps 0.3, seed 3), same default launch configuration as bench.py; every output
+    site of both parities against the oracle (the C oracle does 32^4 in well under a second)."""
+    dims = (32, 32, 32, 32)
+    rng = np.random.default_rng(3)
+    U = gen.smooth_links(dims, 0.3, rng)
+    in_e = gen.gaussian_half_spinor(dims, rng)
+    in_o = gen.gaussian_half_spinor(dims, rng)
+    U, in_e, in_o = round_inputs(prec, U, in_e, in_o)
+    lat = make_lattice(dims, prec, recon)
+    links = lat.pack_links(U)
+    for par, inp in ((1, in_e), (0, in_o)):
+        d_in, d_out = lat.pack_spinor(inp, 1 - par), lat.new_spinor()
+        lat.dslash(par, d_out, d_in, links)
+        got = lat.unpack_spinor(d_out, par)
+        want = oracle.dslash_half(dims, U, par, inp)
+        assert rel(got, want) < TOL[prec]
+        # element-wise, not only in norm: worst site
+        assert np.abs(got - want).max() < 50 * TOL[prec] * np.abs(want).max()
+    lat.close()
+
+
+def test_dslash_large_volume_sampled_sites():
+    """Maximum-size style check (64^3 x 16, V = 4.2 M, links 2.4 GB): sampled output sites computed
+    one by one by oracle_dirac_site, including corners and both x3 boundary slices."""
+    dims = (64, 64, 64, 16)
+    rng = np.random.default_rng(5)
+    U = gen.smooth_links(dims, 0.5, rng)
+    psi = gen.gaussian_spinor(dims, rng)
+    lat = make_lattice(dims)
+    links = lat.pack_links(U)
+    coords = gen.site_coords(dims)
+    samp = np.random.default_rng(99)
+    picks = [(0, 0, 0, 0), (63, 63, 63, 15), (1, 0, 0, 0), (0, 63, 0, 15), (62, 1, 63, 0), (63, 0, 0, 0)]
+    picks += [tuple(int(v) for v in coords[i]) for i in samp.integers(0, coords.shape[0], 200)]
+    got = {}
+    for par in (0, 1):
+        inp = oracle.full_to_half(dims, 1 - par, psi)
+        d_in, d_out = lat.pack_spinor(inp, 1 - par), lat.new_spinor()
+        lat.dslash(par, d_out, d_in, links)
+        got[par] = lat.unpack_spinor(d_out, par)
+    worst = 0.0
+    for x in picks:
+        par = sum(x) % 2
+        lex = x[0] + dims[0] * (x[1] + dims[1] * (x[2] + dims[2] * x[3]))
+        # the oracle reads the full-lattice psi; only opposite-parity neighbours enter D
+        want = oracle.dirac_site(dims, U, psi, x)
+        err = np.abs(got[par][lex // 2] - want).max() / np.abs(want).max()
+        worst = max(worst, err)
+    assert worst < 1e-12, worst
+    lat.close()
+
+
+def test_multishift_config4_24x24x24x48():
+    """BASELINE.json configs[3]: 24^3 x 48, 8 shifts, m = 0.0025, tol 1e-10 per shift, against the
+    oracle run to the same tolerance (reading R16)."""
+    dims = (24, 24, 24, 48)
+    rng = np.random.default_rng(4)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m, tol = 0.0025, 1e-10
+    shifts = gen.rhmc_shifts(8)
+    lat = make_lattice(dims)
+    links, be = lat.pack_links(U), lat.pack_spinor(b, 0)
+    xs = [lat.new_spinor() for _ in shifts]
+    res = lat.cg_multishift(xs, be, links, m, shifts, tol, 50000)
+    ref = oracle.cg_multishift(dims, U, m, shifts, b, tol, 50000, hist_len=16)
+    assert ref["converged"]
+    assert abs(res["iters"] - ref["iters"]) <= max(2, ref["iters"] // 50)
+    assert np.all(np.abs(res["conv_iter"] - ref["conv_iter"]) <= np.maximum(2, ref["conv_iter"] // 50))
+    h = lat.solver_history()
+    assert np.allclose(h["alpha"][:10], ref["alpha"][:10], rtol=1e-10)
+    assert np.allclose(h["rnorm"][:10], ref["rnorm"][:10], rtol=1e-10)
+    bn = np.linalg.norm(b)
+    for i in (0, 3, 7):                      # smallest, middle, largest shift
+        xg = lat.unpack_spinor(xs[i], 0)
+        tr = np.linalg.norm(b - oracle.mdagm(dims, U, m, xg, sigma=shifts[i])) / bn
+        assert tr < 1.5 * tol
+        assert rel(xg, ref["x"][i]) < 10 * (7.0 / (m * m + shifts[i])) * tol
+    assert res["rel_resid"].max() < 1.5 * tol
+    lat.close()

@@ -341,3 +341,23 @@ def test_multishift_rejects_bad_shifts():
     b = gen.gaussian_half_spinor(dims, 1)
     with pytest.raises(ValueError):
         oracle.cg_multishift(dims, U, 0.1, [0.1, -0.2], b, 1e-8, 10)
+
+
+def test_oracle_regression_fixture():
+    """tests/golden/oracle_regression.json (written by make_golden.py from oracle/ only) still
+    matches: guards against an unannounced change of the oracle's arithmetic.  The 8^4 CG count
+    (143) also equals the survey's independent scratch run."""
+    import json
+    import os
+    import sys
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    sys.path.insert(0, here)
+    import make_golden
+    want = json.load(open(os.path.join(here, "oracle_regression.json")))
+    got = make_golden.compute()
+    assert got["cg_8x4_m0.01_iters"] == want["cg_8x4_m0.01_iters"] == 143
+    assert got["multishift_8x4_iters"] == want["multishift_8x4_iters"]
+    assert got["multishift_8x4_conv_iter"] == want["multishift_8x4_conv_iter"]
+    assert abs(got["config1_4x4_dirac_norm2"] - want["config1_4x4_dirac_norm2"]) < 1e-9 * want["config1_4x4_dirac_norm2"]
+    assert np.allclose(got["config1_4x4_dirac_site0"], want["config1_4x4_dirac_site0"], rtol=1e-12)
+    assert abs(got["cg_8x4_alpha0"] - want["cg_8x4_alpha0"]) < 1e-12
