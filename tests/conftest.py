@@ -9,7 +9,16 @@ if ROOT not in sys.path:
 sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
 
 
+def _ensure_built():
+    """A fresh checkout has no .so (they are git-ignored): compile before the first import.
+    nvcc cross-compiles for sm_100a without a GPU.  This builds; it never substitutes a fallback."""
+    if not os.path.exists(os.path.join(ROOT, "paper_1701_00426_b200", "liblqcd_b200.so")):
+        import __graft_entry__
+        __graft_entry__.build()
+
+
 def pytest_configure(config):
+    _ensure_built()
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
 
 
