@@ -77,6 +77,11 @@ extern "C" int lqcd_create(lqcd_ctx **out, const int dims[4], int prec, int reco
     c->blas_block = 256;
     c->blas_ctas_per_sm = 8;
     c->poll_chunk = 8;
+    c->pdl = 1;
+    c->graph = 1;
+    c->dot_early = 1;
+    c->iter_mask = 15;
+    c->launch_stream = c->stream;
     cudaDeviceProp prop;
     if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) { free(c); return lqcd_check_cuda(NULL, e, "cudaGetDeviceProperties"); }
     c->num_sms = prop.multiProcessorCount;
@@ -86,6 +91,7 @@ extern "C" int lqcd_create(lqcd_ctx **out, const int dims[4], int prec, int reco
         (e = cudaMallocHost(&c->h_flag, 64)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&c->ev[0], cudaEventDisableTiming)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking)) != cudaSuccess ||
         (e = cudaMemset(c->d_state, 0, sizeof(SolverState))) != cudaSuccess) {
         int rc = lqcd_check_cuda(NULL, e, "lqcd_create: allocating solver state");
         cudaFree(c->d_state); cudaFree(c->d_partials); if (c->h_flag) cudaFreeHost(c->h_flag);
@@ -107,6 +113,8 @@ extern "C" int lqcd_destroy(lqcd_ctx *ctx)
     cudaEventDestroy(ctx->ev[0]);
     cudaEventDestroy(ctx->ev[1]);
     cudaFree(ctx->stage);
+    if (ctx->chunk_exec) cudaGraphExecDestroy(ctx->chunk_exec);
+    if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     free(ctx);
     return LQCD_OK;
 }
@@ -114,8 +122,9 @@ extern "C" int lqcd_destroy(lqcd_ctx *ctx)
 struct OptDesc { const char *name; size_t off; long lo, hi; };
 #define OPT(field, lo, hi) { #field, offsetof(lqcd_ctx, field), lo, hi }
 static const OptDesc g_opts[] = {
-    OPT(layout, 0, 1), OPT(l2_hints, 0, 1), OPT(l2_persist, 0, 4), OPT(link_pad, 0, 1 << 20), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
+    OPT(layout, 0, 2), OPT(l2_hints, 0, 1), OPT(l2_persist, 0, 4), OPT(link_pad, 0, 1 << 20), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
     OPT(blas_block, 64, 256), OPT(blas_ctas_per_sm, 1, 32), OPT(poll_chunk, 1, 1024),
+    OPT(pdl, 0, 1), OPT(graph, 0, 1), OPT(dot_early, 0, 1), OPT(iter_mask, 0, 15),
 };
 
 extern "C" int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value)
@@ -131,9 +140,11 @@ extern "C" int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value)
         if (!strcmp(name, "link_pad")) {
             if (ctx->layout_locked && value != ctx->link_pad) return lqcd_fail(ctx, LQCD_ERR_ARG, "option link_pad: fields were already packed");
             if (value % 8) return lqcd_fail(ctx, LQCD_ERR_ARG, "option link_pad must be a multiple of 8 sites");
-            ctx->g.Ls = ctx->g.Vh + (int)value;
         }
         *(int *)((char *)ctx + o.off) = (int)value;
+        // link plane stride in sites; the blocked layout needs whole 32-site blocks
+        ctx->g.Ls = ctx->g.Vh + ctx->link_pad;
+        if (ctx->layout == 2) ctx->g.Ls = (ctx->g.Ls + 31) & ~31;
         return LQCD_OK;
     }
     return lqcd_fail(ctx, LQCD_ERR_ARG, "unknown option %s", name);
@@ -144,6 +155,7 @@ extern "C" long lqcd_get_option(const lqcd_ctx *ctx, const char *name)
     if (!ctx || !name) return -1;
     if (!strcmp(name, "launches")) return ctx->launches;
     if (!strcmp(name, "num_sms")) return ctx->num_sms;
+    if (!strcmp(name, "graph_active")) return ctx->graph_active;
     if (!strcmp(name, "l2_window_bytes")) return ctx->l2_window_bytes;
     if (!strcmp(name, "l2_max_persist")) return ctx->l2_max_persist;
     for (const OptDesc &o : g_opts)

@@ -48,6 +48,11 @@ struct Geom {
 // Native layout (private).  A "plane" is one complex component for all Vh sites of one parity.
 //   layout 0 (interleaved): plane p, site i -> reals [ (p*Vh + i)*2 + {0:re,1:im} ]
 //   layout 1 (split)      : plane p, site i -> reals [ (2p + {0,1})*Vh + i ]
+//   layout 2 (blocked links): vectors as layout 0; links in blocks of 32 sites: within one parity
+//                           the PPP = 4*R*3 planes of a 32-site block are contiguous (PPP*512 B
+//                           in fp64 = 18 KB: the 4 forward links of a warp's sites are ONE
+//                           contiguous run instead of 36 runs of 512 B that lie 8 MB apart):
+//                           complex index = par*PPP*Ls + ((i>>5)*PPP + plane_in_parity)*32 + (i&31)
 // half spinor : 3 planes (colour c)
 // links       : plane ((par*4 + mu)*R + row)*3 + col, R = 3 (18-real) or 2 (12-real);
 //               U_mu(x) is stored at x's own parity and idxh.
@@ -152,7 +157,7 @@ template <typename T, int LAYOUT, int STREAM, int POLICY>
 __device__ __forceinline__ Cx<T> ld_cx(const T *__restrict__ base, size_t plane, size_t Vh, size_t i, const L2Pol &pol)
 {
     Cx<T> z;
-    if (LAYOUT == 0) {
+    if (LAYOUT != 1) {
         typedef typename Vec2<T>::type V2;
         const V2 *p = reinterpret_cast<const V2 *>(base) + plane * Vh + i;
         V2 v;
@@ -174,7 +179,7 @@ __device__ __forceinline__ Cx<T> ld_cx(const T *__restrict__ base, size_t plane,
 template <typename T, int LAYOUT, int POLICY>
 __device__ __forceinline__ void st_cx(T *__restrict__ base, size_t plane, size_t Vh, size_t i, Cx<T> z, const L2Pol &pol)
 {
-    if (LAYOUT == 0) {
+    if (LAYOUT != 1) {
         typedef typename Vec2<T>::type V2;
         V2 v; v.x = z.re; v.y = z.im;
         V2 *p = reinterpret_cast<V2 *>(base) + plane * Vh + i;
@@ -184,6 +189,14 @@ __device__ __forceinline__ void st_cx(T *__restrict__ base, size_t plane, size_t
         if (POLICY == 0) { p[0] = z.re; p[Vh] = z.im; }
         else { st_hint_keep(p, z.re, pol.keep); st_hint_keep(p + Vh, z.im, pol.keep); }
     }
+}
+
+// complex index of link component (par, local plane pl = (mu*R + row)*3 + col, site i)
+template <int LAYOUT, int PPP>
+__device__ __forceinline__ size_t link_cidx(int par, int pl, size_t Ls, size_t i)
+{
+    if (LAYOUT == 2) return (size_t)par * PPP * Ls + ((i >> 5) * PPP + pl) * 32 + (i & 31);
+    return ((size_t)par * PPP + pl) * Ls + i;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -223,6 +236,16 @@ struct lqcd_ctx {
     int dslash_minblocks;  // launch-bounds variant (occupancy target)
     int blas_block, blas_ctas_per_sm;
     int poll_chunk;        // CG iterations enqueued between convergence polls
+    int pdl;               // 1: programmatic dependent launch (kernel N+1 is scheduled while N drains)
+    int graph;             // 1: the solver replays one CUDA graph per chunk of poll_chunk iterations
+    int dot_early;         // 1: Dslash-with-dot reduces its partial BEFORE storing the output
+    int iter_mask;         // diagnostic: bit k set = kernel k of the CG iteration is launched (default 15)
+    int graph_active;      // read-only: the last solve ran from a graph
+    cudaStream_t cap_stream;      // private stream used only for graph capture
+    cudaStream_t launch_stream;   // where launch_k enqueues: ctx->stream, or cap_stream while capturing
+    cudaGraphExec_t chunk_exec;   // cached chunk graph and the key it was built for
+    unsigned long long chunk_key[48];
+    int chunk_key_n;
     int num_sms;
     void *ws; size_t ws_bytes;
     SolverState *d_state;  // device
@@ -236,6 +259,34 @@ struct lqcd_ctx {
     long launches;         // kernels launched through this context (bench.py's gpu_launches)
     char err[256];
 };
+
+// ------------------------------------------------------------------------------------------
+// Programmatic dependent launch (sm_90+).  Every kernel of the library starts with pdl_wait()
+// -- which returns once the preceding kernel in the stream has completed and its writes are
+// visible; a no-op without the launch attribute -- and calls pdl_trigger() right after, so that
+// the CTAs of the NEXT kernel become resident while the last wave of this one drains and are
+// parked in their own pdl_wait().  Nothing is read or written before pdl_wait(): the dependency
+// semantics are exactly those of plain stream order; only launch latency and ramp-up overlap.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_k(lqcd_ctx *ctx, void (*kern)(KArgs...), dim3 grid, dim3 block, Args... args)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.stream = ctx->launch_stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = ctx->pdl ? 1 : 0;
+    ctx->launches++;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
 
 int lqcd_fail(lqcd_ctx *ctx, int code, const char *fmt, ...);
 int lqcd_check_cuda(lqcd_ctx *ctx, cudaError_t e, const char *what);

@@ -67,6 +67,8 @@ __global__ void __launch_bounds__(256) init_kernel(size_t npk, const T *__restri
                                                    T *__restrict__ p, ShiftPtrs sp, SolverState *st,
                                                    double *partials)
 {
+    pdl_wait();
+    pdl_trigger();
     typedef typename Pack<T>::type P;
     const int N = Pack<T>::N;
     const uint64_t keep = POLICY ? l2_policy_evict_last() : 0;
@@ -98,6 +100,8 @@ template <typename T, int POLICY>
 __global__ void __launch_bounds__(256) k1_kernel(size_t npk, T *__restrict__ r, const T *__restrict__ q,
                                                  SolverState *st, double *partials)
 {
+    pdl_wait();
+    pdl_trigger();
     if (*(volatile int *)&st->done) return;
     typedef typename Pack<T>::type P;
     const int N = Pack<T>::N;
@@ -124,6 +128,8 @@ template <typename T, int POLICY>
 __global__ void __launch_bounds__(256) k2_kernel(size_t npk, const T *__restrict__ r, T *__restrict__ p,
                                                  ShiftPtrs sp, const SolverState *__restrict__ st)
 {
+    pdl_wait();
+    pdl_trigger();
     if (*(volatile const int *)&st->done == 2) return;
     typedef typename Pack<T>::type P;
     const int N = Pack<T>::N;
@@ -172,6 +178,8 @@ template <typename T, int POLICY>
 __global__ void __launch_bounds__(256) diffnorm_kernel(size_t npk, const T *__restrict__ a, const T *__restrict__ b,
                                                        SolverState *st, double *partials, double *slot)
 {
+    pdl_wait();
+    pdl_trigger();
     typedef typename Pack<T>::type P;
     const int N = Pack<T>::N;
     const uint64_t keep = POLICY ? l2_policy_evict_last() : 0;
@@ -226,28 +234,68 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     }
     int rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(ctx->d_state, &h, sizeof(h), cudaMemcpyHostToDevice, s), "solver state upload");
     if (rc) return rc;
-    if (ctx->l2_hints) init_kernel<T, 1><<<grid, block, 0, s>>>(npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
-    else init_kernel<T, 0><<<grid, block, 0, s>>>(npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
-    ctx->launches++;
+    if (ctx->l2_hints) launch_k(ctx, init_kernel<T, 1>, dim3(grid), dim3(block), npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
+    else launch_k(ctx, init_kernel<T, 0>, dim3(grid), dim3(block), npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
 
     const double msq = mass * mass + shifts[base];
     volatile int *flag = ctx->h_flag;
     flag[0] = flag[16 / 4] = 0;
     int enq = 0, chunk_id = 0, stop = 0;
+    // one CG iteration = 4 kernels; all arguments are the same in every iteration
+    auto enqueue_iteration = [&]() -> int {
+        int e;
+        const int m = ctx->iter_mask;   // diagnostic: which of the 4 kernels run (timing experiments only)
+        if ((m & 1) && (e = launch_dslash(ctx, LQCD_ODD, tmp_o, p, links, NULL, 0.0, 0, 2))) return e;
+        if ((m & 2) && (e = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, p, msq, 1, 1))) return e;
+        if (ctx->l2_hints) {
+            if (m & 4) launch_k(ctx, k1_kernel<T, 1>, dim3(grid), dim3(block), npk, r, (const T *)q, ctx->d_state, ctx->d_partials);
+            if (m & 8) launch_k(ctx, k2_kernel<T, 1>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+        } else {
+            if (m & 4) launch_k(ctx, k1_kernel<T, 0>, dim3(grid), dim3(block), npk, r, (const T *)q, ctx->d_state, ctx->d_partials);
+            if (m & 8) launch_k(ctx, k2_kernel<T, 0>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+        }
+        return lqcd_check_cuda(ctx, cudaGetLastError(), "cg iteration");
+    };
+    // Chunk graph (option `graph`): poll_chunk iterations captured once and replayed; the key is
+    // every value the captured launches depend on.
+    unsigned long long key[48];
+    int kn = 0;
+    key[kn++] = (unsigned long long)(uintptr_t)ctx->ws; key[kn++] = (unsigned long long)(uintptr_t)links;
+    memcpy(&key[kn++], &msq, sizeof(double));
+    key[kn++] = ((unsigned long long)nshift << 32) | (unsigned)base;
+    key[kn++] = ((unsigned long long)ctx->poll_chunk << 32) | (unsigned)grid;
+    key[kn++] = ((unsigned long long)block << 32) | (unsigned)(ctx->dslash_block * 64 + ctx->dslash_minblocks * 8 + ctx->l2_hints * 4 + ctx->pdl * 2 + ctx->dot_early);
+    key[kn++] = (unsigned long long)(uintptr_t)ctx->stream ^ ((unsigned long long)ctx->iter_mask << 56);
+    for (int i = 0; i < nshift; ++i) key[kn++] = (unsigned long long)(uintptr_t)xs[i];
+    ctx->graph_active = 0;
+    if (ctx->graph && max_iter >= ctx->poll_chunk) {
+        if (!ctx->chunk_exec || ctx->chunk_key_n != kn || memcmp(ctx->chunk_key, key, kn * sizeof(key[0]))) {
+            if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
+            const long launches0 = ctx->launches;
+            cudaGraph_t g = NULL;
+            int ok = cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+            if (ok) {
+                ctx->launch_stream = ctx->cap_stream;
+                for (int k = 0; k < ctx->poll_chunk && ok; ++k) ok = enqueue_iteration() == LQCD_OK;
+                ctx->launch_stream = ctx->stream;
+                ok = (cudaStreamEndCapture(ctx->cap_stream, &g) == cudaSuccess) && ok && g;
+            }
+            if (ok) ok = cudaGraphInstantiate(&ctx->chunk_exec, g, 0) == cudaSuccess;
+            if (g) cudaGraphDestroy(g);
+            ctx->launches = launches0;
+            if (!ok) { cudaGetLastError(); ctx->chunk_exec = NULL; ctx->graph = 0; }   // plain launches from now on
+            else { memcpy(ctx->chunk_key, key, kn * sizeof(key[0])); ctx->chunk_key_n = kn; }
+        }
+    }
     while (!stop) {
         int n = ctx->poll_chunk;
         if (enq + n > max_iter) n = max_iter - enq;
-        for (int k = 0; k < n; ++k) {
-            if ((rc = launch_dslash(ctx, LQCD_ODD, tmp_o, p, links, NULL, 0.0, 0, 2))) return rc;
-            if ((rc = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, p, msq, 1, 1))) return rc;
-            if (ctx->l2_hints) {
-                k1_kernel<T, 1><<<grid, block, 0, s>>>(npk, r, q, ctx->d_state, ctx->d_partials);
-                k2_kernel<T, 1><<<grid, block, 0, s>>>(npk, r, p, sp, ctx->d_state);
-            } else {
-                k1_kernel<T, 0><<<grid, block, 0, s>>>(npk, r, q, ctx->d_state, ctx->d_partials);
-                k2_kernel<T, 0><<<grid, block, 0, s>>>(npk, r, p, sp, ctx->d_state);
-            }
-            ctx->launches += 2;
+        if (ctx->graph && ctx->chunk_exec && n == ctx->poll_chunk) {
+            if ((rc = lqcd_check_cuda(ctx, cudaGraphLaunch(ctx->chunk_exec, s), "chunk graph launch"))) return rc;
+            ctx->launches += (long)__builtin_popcount(ctx->iter_mask) * n;
+            ctx->graph_active = 1;
+        } else {
+            for (int k = 0; k < n; ++k) if ((rc = enqueue_iteration())) return rc;
         }
         enq += n;
         int slot = chunk_id & 1;
@@ -266,8 +314,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     for (int i = 0; i < nshift; ++i) {
         if ((rc = launch_dslash(ctx, LQCD_ODD, tmp_o, xs[i], links, NULL, 0.0, 0, 0))) return rc;
         if ((rc = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, xs[i], mass * mass + shifts[i], 0, 0))) return rc;
-        diffnorm_kernel<T, 0><<<grid, block, 0, s>>>(npk, (const T *)b, q, ctx->d_state, ctx->d_partials, &ctx->d_state->resid[i]);
-        ctx->launches++;
+        launch_k(ctx, diffnorm_kernel<T, 0>, dim3(grid), dim3(block), npk, (const T *)b, (const T *)q, ctx->d_state, ctx->d_partials, &ctx->d_state->resid[i]);
     }
     if ((rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(&h, ctx->d_state, sizeof(h), cudaMemcpyDeviceToHost, s), "solver state download"))) return rc;
     if ((rc = lqcd_check_cuda(ctx, cudaStreamSynchronize(s), "cg"))) return rc;

@@ -41,7 +41,7 @@ def gpu_dslash(lat, U, phi_in, out_parity):
 # ------------------------------------------------------------------------------------------------
 # Dslash
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("layout", [0, 1])
+@pytest.mark.parametrize("layout", [0, 1, 2])
 @pytest.mark.parametrize("recon", [0, 1])
 @pytest.mark.parametrize("prec", [0, 1])
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (2, 2, 2, 2), (6, 4, 2, 8), (12, 10, 6, 4)])
@@ -116,7 +116,7 @@ def test_pack_unpack_roundtrip():
     dims = (4, 8, 2, 6)
     phi = gen.gaussian_half_spinor(dims, 5)
     for prec in (0, 1):
-        for layout in (0, 1):
+        for layout in (0, 1, 2):
             lat = make_lattice(dims, prec, layout=layout)
             back = lat.unpack_spinor(lat.pack_spinor(phi, 0), 0)
             if prec == 0:
