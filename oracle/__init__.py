@@ -13,6 +13,7 @@ from .oracle import (  # noqa: F401
     reconstruct_row3,
     cg,
     cg_multishift,
+    rational_apply,
     half_to_full,
     full_to_half,
     num_threads,

@@ -42,6 +42,9 @@ _lib.oracle_cg_multishift.argtypes = [_i4, C.c_int, _c128, C.c_double, C.c_int, 
                                       C.c_double, C.c_int, _pi, _pi, _pd, _pd, C.c_void_p,
                                       _pd, _pd, _pd, C.c_int]
 _lib.oracle_cg_multishift.restype = C.c_int
+_lib.oracle_rational_apply.argtypes = [_i4, C.c_int, _c128, C.c_double, C.c_int, _pd, C.c_double, _pd, _c128, _c128,
+                                       C.c_double, C.c_int, _pi, _pi]
+_lib.oracle_rational_apply.restype = C.c_int
 _lib.oracle_num_threads.restype = C.c_int
 _lib.oracle_set_num_threads.argtypes = [C.c_int]
 
@@ -183,3 +186,24 @@ def cg_multishift(dims, U, mass, shifts, b, tol, max_iter, antiperiodic_t=True, 
     return dict(x=x, iters=iters.value, converged=(rc == 0), conv_iter=np.array(list(conv)),
                 true_relres=relres, zeta=zeta, r=r,
                 alpha=ha[:hist_len], beta=hb[:hist_len], rnorm=hr[:hist_len])
+
+
+def rational_apply(dims, U, mass, shifts, c0, coeffs, b, tol, max_iter, antiperiodic_t=True):
+    """y = c0 b + sum_i coeffs[i] (A + shifts[i])^-1 b.  Returns dict(y, iters, converged, conv_iter)."""
+    n4, V = _dims(dims)
+    shifts = np.ascontiguousarray(shifts, dtype=np.float64)
+    coeffs = np.ascontiguousarray(coeffs, dtype=np.float64)
+    ns = shifts.size
+    if coeffs.size != ns:
+        raise ValueError("one coefficient per shift")
+    y = np.empty((V // 2, 3), dtype=np.complex128)
+    iters = C.c_int(0)
+    conv = (C.c_int * ns)()
+    rc = _lib.oracle_rational_apply(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), mass, ns, _dptr(shifts),
+                                    float(c0), _dptr(coeffs), _arr(b, (V // 2, 3)), y, tol, max_iter,
+                                    C.byref(iters), conv)
+    if rc == -1:
+        raise MemoryError("oracle_rational_apply")
+    if rc == -2:
+        raise ValueError("shifts must be >= 0 and nshift >= 1")
+    return dict(y=y, iters=iters.value, converged=(rc == 0), conv_iter=np.array(list(conv)))

@@ -23,7 +23,8 @@
  * constant-spinor closed form for the antiperiodic boundary; <phi,D_eo psi> = -<D_oe phi,psi>;
  * gauge covariance; reconstructed row 3 against the generator's Gram-Schmidt row 3;
  * CG / multi-shift against dense numpy.linalg.solve; the identity
- * b - (A + sigma_i) x_i = zeta_i r; one-iteration convergence on a plane wave.
+ * b - (A + sigma_i) x_i = zeta_i r; one-iteration convergence on a plane wave; the
+ * rational-function sum against dense solves and a partial-fraction identity.
  * No function in this file is "parity unpinned".
  *
  * OpenMP is used on the site loop of the operator only, so that bench.py can time the
@@ -417,6 +418,43 @@ done:
     }
     if (r_out) memcpy(r_out, r, n * sizeof(cplx));
     free(r); free(p); free(q); free(ps); free(sc); free(active);
+    return rc;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Rational function of A = m^2 - D_eo D_oe applied to a vector:
+ *
+ *   y = c0 b + sum_{i=1..r} c_i x_i ,     (A + sigma_i) x_i = b                      (Eq. 6)
+ *
+ * PAPER.md:133 "the algebraic matrix function appearing in Eq. (3) is approximated to machine
+ * precision by a rational function" whose poles are the sigma_i of Eq. 6;
+ * this partial-fraction sum is what the pseudofermion heatbath and the action evaluation
+ * (Algorithm 1 steps 3 and 6: "function calls to the multishift inverter")
+ * do with the solutions.  The paper prints neither c_i nor sigma_i: both are inputs.
+ * Written as the definition: solve with the multi-shift CG above, then add the r+1 terms in
+ * the order of the formula.  (The CUDA path accumulates y inside its vector-update kernel
+ * and never stores x_i; that is a reordering of this sum, not a different quantity.)
+ * Pins: dense (c0 + sum c_i (A+sigma_i)^-1) b by numpy.linalg.solve; the partial-fraction
+ * identity 1/((A+s1)(A+s2)) = [1/(A+s1) - 1/(A+s2)]/(s2-s1) checked by applying both factors;
+ * free-field plane wave b: y = (c0 + sum c_i/(lambda+sigma_i)) b.
+ * Returns as oracle_cg_multishift.
+ * ------------------------------------------------------------------------------------- */
+int oracle_rational_apply(const int N[4], int antiperiodic_t, const cplx *U, double mass,
+                          int nshift, const double *sigma, double c0, const double *c,
+                          const cplx *b, cplx *y, double tol, int max_iter,
+                          int *iters, int *conv_iter)
+{
+    size_t n = vol(N) / 2 * 3;
+    cplx *x = (cplx *)malloc(n * (size_t)(nshift > 0 ? nshift : 1) * sizeof(cplx));
+    if (!x) return -1;
+    int rc = oracle_cg_multishift(N, antiperiodic_t, U, mass, nshift, sigma, b, x, tol, max_iter,
+                                  iters, conv_iter, NULL, NULL, NULL, NULL, NULL, NULL, 0);
+    if (rc >= 0) {
+        for (size_t j = 0; j < n; ++j) y[j] = c0 * b[j];
+        for (int i = 0; i < nshift; ++i)
+            for (size_t j = 0; j < n; ++j) y[j] += c[i] * x[(size_t)i * n + j];
+    }
+    free(x);
     return rc;
 }
 

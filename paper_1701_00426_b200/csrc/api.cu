@@ -79,7 +79,7 @@ extern "C" int lqcd_create(lqcd_ctx **out, const int dims[4], int prec, int reco
     c->poll_chunk = 8;
     c->pdl = 1;
     c->graph = 1;
-    c->dot_early = 1;
+    c->dslash_persist = 0;
     c->iter_mask = 15;
     c->launch_stream = c->stream;
     cudaDeviceProp prop;
@@ -122,9 +122,9 @@ extern "C" int lqcd_destroy(lqcd_ctx *ctx)
 struct OptDesc { const char *name; size_t off; long lo, hi; };
 #define OPT(field, lo, hi) { #field, offsetof(lqcd_ctx, field), lo, hi }
 static const OptDesc g_opts[] = {
-    OPT(layout, 0, 2), OPT(l2_hints, 0, 1), OPT(l2_persist, 0, 4), OPT(link_pad, 0, 1 << 20), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
+    OPT(layout, 0, 1), OPT(l2_hints, 0, 1), OPT(l2_persist, 0, 4), OPT(link_pad, 0, 1 << 20), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
     OPT(blas_block, 64, 256), OPT(blas_ctas_per_sm, 1, 32), OPT(poll_chunk, 1, 1024),
-    OPT(pdl, 0, 1), OPT(graph, 0, 1), OPT(dot_early, 0, 1), OPT(iter_mask, 0, 15),
+    OPT(pdl, 0, 1), OPT(graph, 0, 1), OPT(dslash_persist, 0, 16), OPT(iter_mask, 0, 15),
 };
 
 extern "C" int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value)
@@ -142,9 +142,7 @@ extern "C" int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value)
             if (value % 8) return lqcd_fail(ctx, LQCD_ERR_ARG, "option link_pad must be a multiple of 8 sites");
         }
         *(int *)((char *)ctx + o.off) = (int)value;
-        // link plane stride in sites; the blocked layout needs whole 32-site blocks
-        ctx->g.Ls = ctx->g.Vh + ctx->link_pad;
-        if (ctx->layout == 2) ctx->g.Ls = (ctx->g.Ls + 31) & ~31;
+        ctx->g.Ls = ctx->g.Vh + ctx->link_pad;   // link plane stride in sites
         return LQCD_OK;
     }
     return lqcd_fail(ctx, LQCD_ERR_ARG, "unknown option %s", name);

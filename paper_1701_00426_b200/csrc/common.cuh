@@ -48,11 +48,6 @@ struct Geom {
 // Native layout (private).  A "plane" is one complex component for all Vh sites of one parity.
 //   layout 0 (interleaved): plane p, site i -> reals [ (p*Vh + i)*2 + {0:re,1:im} ]
 //   layout 1 (split)      : plane p, site i -> reals [ (2p + {0,1})*Vh + i ]
-//   layout 2 (blocked links): vectors as layout 0; links in blocks of 32 sites: within one parity
-//                           the PPP = 4*R*3 planes of a 32-site block are contiguous (PPP*512 B
-//                           in fp64 = 18 KB: the 4 forward links of a warp's sites are ONE
-//                           contiguous run instead of 36 runs of 512 B that lie 8 MB apart):
-//                           complex index = par*PPP*Ls + ((i>>5)*PPP + plane_in_parity)*32 + (i&31)
 // half spinor : 3 planes (colour c)
 // links       : plane ((par*4 + mu)*R + row)*3 + col, R = 3 (18-real) or 2 (12-real);
 //               U_mu(x) is stored at x's own parity and idxh.
@@ -157,7 +152,7 @@ template <typename T, int LAYOUT, int STREAM, int POLICY>
 __device__ __forceinline__ Cx<T> ld_cx(const T *__restrict__ base, size_t plane, size_t Vh, size_t i, const L2Pol &pol)
 {
     Cx<T> z;
-    if (LAYOUT != 1) {
+    if (LAYOUT == 0) {
         typedef typename Vec2<T>::type V2;
         const V2 *p = reinterpret_cast<const V2 *>(base) + plane * Vh + i;
         V2 v;
@@ -179,7 +174,7 @@ __device__ __forceinline__ Cx<T> ld_cx(const T *__restrict__ base, size_t plane,
 template <typename T, int LAYOUT, int POLICY>
 __device__ __forceinline__ void st_cx(T *__restrict__ base, size_t plane, size_t Vh, size_t i, Cx<T> z, const L2Pol &pol)
 {
-    if (LAYOUT != 1) {
+    if (LAYOUT == 0) {
         typedef typename Vec2<T>::type V2;
         V2 v; v.x = z.re; v.y = z.im;
         V2 *p = reinterpret_cast<V2 *>(base) + plane * Vh + i;
@@ -189,14 +184,6 @@ __device__ __forceinline__ void st_cx(T *__restrict__ base, size_t plane, size_t
         if (POLICY == 0) { p[0] = z.re; p[Vh] = z.im; }
         else { st_hint_keep(p, z.re, pol.keep); st_hint_keep(p + Vh, z.im, pol.keep); }
     }
-}
-
-// complex index of link component (par, local plane pl = (mu*R + row)*3 + col, site i)
-template <int LAYOUT, int PPP>
-__device__ __forceinline__ size_t link_cidx(int par, int pl, size_t Ls, size_t i)
-{
-    if (LAYOUT == 2) return (size_t)par * PPP * Ls + ((i >> 5) * PPP + pl) * 32 + (i & 31);
-    return ((size_t)par * PPP + pl) * Ls + i;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -238,7 +225,7 @@ struct lqcd_ctx {
     int poll_chunk;        // CG iterations enqueued between convergence polls
     int pdl;               // 1: programmatic dependent launch (kernel N+1 is scheduled while N drains)
     int graph;             // 1: the solver replays one CUDA graph per chunk of poll_chunk iterations
-    int dot_early;         // 1: Dslash-with-dot reduces its partial BEFORE storing the output
+    int dslash_persist;    // 0: one 128-site tile per CTA; k > 0: num_sms*k CTAs loop over the tiles
     int iter_mask;         // diagnostic: bit k set = kernel k of the CG iteration is launched (default 15)
     int graph_active;      // read-only: the last solve ran from a graph
     cudaStream_t cap_stream;      // private stream used only for graph capture

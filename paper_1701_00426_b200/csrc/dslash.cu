@@ -22,24 +22,11 @@ __device__ __forceinline__ Su3<T> load_link(const T *__restrict__ links, int par
 {
     constexpr int R = RECON12 ? 2 : 3;
     Su3<T> u;
-    if (LAYOUT == 2) {
-        // blocked links: one base address, the 3R components at constant offsets of 32 complex
-        typedef typename Vec2<T>::type V2;
-        const V2 *p = reinterpret_cast<const V2 *>(links) + link_cidx<2, 12 * R>(par, mu * R * 3, Vh, i);
+    size_t plane0 = (size_t)(par * 4 + mu) * (R * 3);
 #pragma unroll
-        for (int r = 0; r < R; ++r)
+    for (int r = 0; r < R; ++r)
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                V2 v = POLICY == 0 ? __ldcs(p + (r * 3 + c) * 32) : ld_hint_stream(p + (r * 3 + c) * 32, pol.stream);
-                u.e[r][c] = cx<T>(v.x, v.y);
-            }
-    } else {
-        size_t plane0 = (size_t)(par * 4 + mu) * (R * 3);
-#pragma unroll
-        for (int r = 0; r < R; ++r)
-#pragma unroll
-            for (int c = 0; c < 3; ++c) u.e[r][c] = ld_cx<T, LAYOUT, 1, POLICY>(links, plane0 + r * 3 + c, Vh, i, pol);
-    }
+        for (int c = 0; c < 3; ++c) u.e[r][c] = ld_cx<T, LAYOUT, 1, POLICY>(links, plane0 + r * 3 + c, Vh, i, pol);
     if (RECON12) {
         // r2[k] = conj( eps_kij r0[i] r1[j] )   (reading R8)
 #pragma unroll
@@ -96,7 +83,7 @@ template <typename T, int LAYOUT, int RECON12, int MODE, int MINB, int POLICY>
 __global__ void __launch_bounds__(256, MINB)
 dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__restrict__ in,
               const T *__restrict__ links, const T *__restrict__ xin, const double coef,
-              SolverState *__restrict__ st, double *__restrict__ partials, const int gate, const int early)
+              SolverState *__restrict__ st, double *__restrict__ partials, const int gate)
 {
     pdl_wait();
     pdl_trigger();
@@ -107,15 +94,16 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
             return;
         }
     }
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const bool valid = i < g.Vh;
     double dot = 0.0;
     L2Pol pol = {0, 0};
     if (POLICY) pol = make_l2pol();
     const size_t Vh = (size_t)g.Vh;
-    Cx<T> acc[3];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) acc[c] = cx<T>((T)0, (T)0);
+    // One tile = blockDim.x consecutive sites.  gridDim.x = number of tiles (one pass), or fewer
+    // CTAs that loop (option dslash_persist): the reduction protocol below is then paid once per
+    // CTA instead of once per tile.
+    for (int tile0 = blockIdx.x * blockDim.x; tile0 < g.Vh; tile0 += gridDim.x * blockDim.x) {
+    const int i = tile0 + threadIdx.x;
+    const bool valid = i < g.Vh;
     if (valid) {
         // ---- a2: site decode (Eq. 9), neighbours, phases ---------------------------------
         uint32_t t = fd_div((uint32_t)i, g.dNh0);
@@ -148,6 +136,9 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
             if (x3 == 0) cb[3] = -cb[3];
         }
         // ---- a3, a4: 8 hops -----------------------------------------------------------------
+        Cx<T> acc[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) acc[c] = cx<T>((T)0, (T)0);
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
             {
@@ -173,22 +164,13 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
                 if (MODE == 2) dot += (double)x.re * (double)acc[c].re + (double)x.im * (double)acc[c].im;
             }
         }
-        if (!(MODE == 2 && early)) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) st_cx<T, LAYOUT, POLICY>(out, (size_t)c, Vh, (size_t)i, acc[c], pol);
-        }
+        for (int c = 0; c < 3; ++c) st_cx<T, LAYOUT, POLICY>(out, (size_t)c, Vh, (size_t)i, acc[c], pol);
+    }
     }
     if (MODE == 2) {
-        // `early`: the CTA's partial, fence and ticket go out BEFORE its output stores, so that the
-        // __threadfence of the ticket protocol has only the 8-byte partial to wait for instead of
-        // the whole CTA's output; the stores then drain while the CTA retires.
         double total;
-        const bool last = grid_sum_ticket(dot, partials, &st->ticket);
-        if (early && valid) {
-#pragma unroll
-            for (int c = 0; c < 3; ++c) st_cx<T, LAYOUT, POLICY>(out, (size_t)c, Vh, (size_t)i, acc[c], pol);
-        }
-        if (last && grid_sum_finish(partials, &total)) solver_after_pq(st, total);
+        if (grid_sum_last(dot, partials, &st->ticket, &total)) solver_after_pq(st, total);
     }
 }
 
@@ -197,11 +179,13 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
                      const void *xin, double coef, int gate)
 {
     int block = ctx->dslash_block > 256 ? 256 : ctx->dslash_block;
-    dim3 grid((ctx->g.Vh + block - 1) / block);
+    int tiles = (ctx->g.Vh + block - 1) / block;
+    if (ctx->dslash_persist > 0 && tiles > ctx->num_sms * ctx->dslash_persist) tiles = ctx->num_sms * ctx->dslash_persist;
+    dim3 grid(tiles);
     int minb = ctx->dslash_minblocks;
     if (minb == 0) minb = sizeof(T) == 8 ? 2 : 3;
 #define GO1(MB, P) launch_k(ctx, dslash_kernel<T, LAYOUT, RECON12, MODE, MB, P>, grid, dim3(block), \
-        ctx->g, parity, (T *)out, (const T *)in, (const T *)links, (const T *)xin, coef, ctx->d_state, ctx->d_partials, gate, ctx->dot_early)
+        ctx->g, parity, (T *)out, (const T *)in, (const T *)links, (const T *)xin, coef, ctx->d_state, ctx->d_partials, gate)
 #define GO(MB) do { if (ctx->l2_hints) GO1(MB, 1); else GO1(MB, 0); } while (0)
     if (minb <= 2) GO(2); else if (minb == 3) GO(3); else GO(4);
 #undef GO
@@ -224,11 +208,9 @@ int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const vo
     int mode = xpay_in ? (dot_mode ? 2 : 1) : 0;
     if (ctx->prec == LQCD_F64) {
         if (ctx->layout == 0) launch_tl<double, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
-        else if (ctx->layout == 2) launch_tl<double, 2>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
         else launch_tl<double, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
     } else {
         if (ctx->layout == 0) launch_tl<float, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
-        else if (ctx->layout == 2) launch_tl<float, 2>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
         else launch_tl<float, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
     }
     return lqcd_check_cuda(ctx, cudaGetLastError(), "dslash");

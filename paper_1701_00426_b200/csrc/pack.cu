@@ -27,17 +27,8 @@ __global__ void pack_links_kernel(Geom g, int rows, T *__restrict__ native, cons
         for (int r = 0; r < rows; ++r)
             for (int c = 0; c < 3; ++c) {
                 double2 z = canon[(lex * 4 + mu) * 9 + r * 3 + c];
-                if (LAYOUT == 2) {
-                    typedef typename Vec2<T>::type V2;
-                    const int pl = (mu * rows + r) * 3 + c;
-                    size_t k = rows == 2 ? link_cidx<2, 24>(par, pl, (size_t)g.Ls, (size_t)i)
-                                         : link_cidx<2, 36>(par, pl, (size_t)g.Ls, (size_t)i);
-                    V2 v; v.x = (T)z.x; v.y = (T)z.y;
-                    reinterpret_cast<V2 *>(native)[k] = v;
-                } else {
-                    size_t plane = ((size_t)(par * 4 + mu) * rows + r) * 3 + c;
-                    st_cx<T, LAYOUT, 0>(native, plane, (size_t)g.Ls, (size_t)i, cx<T>((T)z.x, (T)z.y), L2Pol());
-                }
+                size_t plane = ((size_t)(par * 4 + mu) * rows + r) * 3 + c;
+                st_cx<T, LAYOUT, 0>(native, plane, (size_t)g.Ls, (size_t)i, cx<T>((T)z.x, (T)z.y), L2Pol());
             }
 }
 
@@ -66,9 +57,9 @@ __global__ void unpack_spinor_kernel(Geom g, double2 *__restrict__ canon, const 
 #define DISPATCH_TL(ctx, CALL)                                             \
     do {                                                                   \
         if ((ctx)->prec == LQCD_F64) {                                     \
-            if ((ctx)->layout == 0) { CALL(double, 0); } else if ((ctx)->layout == 2) { CALL(double, 2); } else { CALL(double, 1); } \
+            if ((ctx)->layout == 0) { CALL(double, 0); } else { CALL(double, 1); } \
         } else {                                                           \
-            if ((ctx)->layout == 0) { CALL(float, 0); } else if ((ctx)->layout == 2) { CALL(float, 2); } else { CALL(float, 1); }   \
+            if ((ctx)->layout == 0) { CALL(float, 0); } else { CALL(float, 1); }   \
         }                                                                  \
     } while (0)
 

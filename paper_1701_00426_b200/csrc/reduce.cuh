@@ -50,31 +50,6 @@ __device__ __forceinline__ bool grid_sum_last(double v, double *partials, unsign
     return threadIdx.x == 0;
 }
 
-// The same protocol in two halves, so that a kernel can put work (its output stores) between
-// "my partial is published" and "I am the last CTA: add them up".
-__device__ __forceinline__ bool grid_sum_ticket(double v, double *partials, unsigned int *ticket)
-{
-    __shared__ bool s_last2;
-    double b = block_sum(v);
-    if (threadIdx.x == 0) {
-        partials[blockIdx.x] = b;
-        __threadfence();
-        unsigned int t = atomicInc(ticket, gridDim.x - 1);
-        s_last2 = (t == gridDim.x - 1);
-    }
-    __syncthreads();
-    return s_last2;
-}
-__device__ __forceinline__ bool grid_sum_finish(double *partials, double *total)
-{
-    __threadfence();
-    double s = 0.0;
-    for (unsigned int k = threadIdx.x; k < gridDim.x; k += blockDim.x) s += __ldcg(partials + k);
-    s = block_sum(s);
-    if (threadIdx.x == 0) *total = s;
-    return threadIdx.x == 0;
-}
-
 // ---- scalar recurrences (one thread) -----------------------------------------------------
 // After q = A_b p and pq = Re<p,q>:   alpha = rho/pq;  zeta_i^new, alpha_i   (reading R11)
 __device__ __forceinline__ void solver_after_pq(SolverState *st, double pq)

@@ -264,7 +264,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     memcpy(&key[kn++], &msq, sizeof(double));
     key[kn++] = ((unsigned long long)nshift << 32) | (unsigned)base;
     key[kn++] = ((unsigned long long)ctx->poll_chunk << 32) | (unsigned)grid;
-    key[kn++] = ((unsigned long long)block << 32) | (unsigned)(ctx->dslash_block * 64 + ctx->dslash_minblocks * 8 + ctx->l2_hints * 4 + ctx->pdl * 2 + ctx->dot_early);
+    key[kn++] = ((unsigned long long)block << 32) | (unsigned)(ctx->dslash_block * 64 + ctx->dslash_minblocks * 8 + ctx->l2_hints * 4 + ctx->pdl * 2) ^ ((unsigned long long)ctx->dslash_persist << 48);
     key[kn++] = (unsigned long long)(uintptr_t)ctx->stream ^ ((unsigned long long)ctx->iter_mask << 56);
     for (int i = 0; i < nshift; ++i) key[kn++] = (unsigned long long)(uintptr_t)xs[i];
     ctx->graph_active = 0;

@@ -41,7 +41,7 @@ def gpu_dslash(lat, U, phi_in, out_parity):
 # ------------------------------------------------------------------------------------------------
 # Dslash
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("layout", [0, 1, 2])
+@pytest.mark.parametrize("layout", [0, 1])
 @pytest.mark.parametrize("recon", [0, 1])
 @pytest.mark.parametrize("prec", [0, 1])
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (2, 2, 2, 2), (6, 4, 2, 8), (12, 10, 6, 4)])
@@ -89,6 +89,20 @@ def test_dslash_launch_variants(block, minb):
     lat.close()
 
 
+@pytest.mark.parametrize("persist", [1, 2])
+def test_dslash_looping_grid(persist):
+    """Option dslash_persist: fewer CTAs that loop over the 128-site tiles (ragged last tile)."""
+    dims = (12, 12, 12, 20)    # Vh = 17280 = 135 tiles of 128: more tiles than looping CTAs need
+    rng = np.random.default_rng(3)
+    U = gen.smooth_links(dims, 0.3, rng)
+    phi = gen.gaussian_half_spinor(dims, rng)
+    want = oracle.dslash_half(dims, U, 1, phi)
+    lat = make_lattice(dims, dslash_persist=persist, dslash_block=32)
+    assert lat.get_option("num_sms") * persist < (lat.Vh + 31) // 32       # the loop really loops
+    assert rel(gpu_dslash(lat, U, phi, 1), want) < 1e-12
+    lat.close()
+
+
 def test_dslash_16x4_config2_and_mdagm():
     """BASELINE.json config 2 operator part: 16^4, eps = 0.3, seed 2, both parities and mdagm."""
     dims = (16, 16, 16, 16)
@@ -116,7 +130,7 @@ def test_pack_unpack_roundtrip():
     dims = (4, 8, 2, 6)
     phi = gen.gaussian_half_spinor(dims, 5)
     for prec in (0, 1):
-        for layout in (0, 1, 2):
+        for layout in (0, 1):
             lat = make_lattice(dims, prec, layout=layout)
             back = lat.unpack_spinor(lat.pack_spinor(phi, 0), 0)
             if prec == 0:
@@ -204,6 +218,47 @@ def test_multishift_small(recon):
         assert abs(tr - res["rel_resid"][i]) < 1e-12
         assert rel(xg, ref["x"][i]) < 10 * (7.0 / (m * m + s)) * tol
     lat.close()
+
+
+@pytest.mark.parametrize("opts", [dict(pdl=0, graph=0), dict(pdl=1, graph=0), dict(pdl=0, graph=1),
+                                  dict(poll_chunk=3), dict(poll_chunk=1), dict(poll_chunk=64),
+                                  dict(dslash_persist=1, dslash_block=32)])
+def test_solver_launch_variants(opts):
+    """Programmatic dependent launch, CUDA-graph replay of the iteration chunks and the chunk length
+    are scheduling choices: same iterates as the plain launch path (bit for bit, unless the grid
+    shape -- hence the reduction order -- changes), and the oracle criteria R16 hold."""
+    dims = (8, 8, 8, 8)
+    rng = np.random.default_rng(11)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m, tol = 0.05, 1e-10
+    shifts = gen.rhmc_shifts(4)
+    ref = oracle.cg_multishift(dims, U, m, shifts, b, tol, 5000)
+
+    def solve(o):
+        lat = make_lattice(dims, **o)
+        links, be = lat.pack_links(U), lat.pack_spinor(b, 0)
+        xs = [lat.new_spinor() for _ in shifts]
+        res = lat.cg_multishift(xs, be, links, m, shifts, tol, 5000)
+        res2 = lat.cg_multishift(xs, be, links, m, shifts, tol, 5000)      # cached graph is reused
+        assert res2["iters"] == res["iters"]
+        out = [lat.unpack_spinor(x, 0) for x in xs]
+        ga = lat.get_option("graph_active")
+        lat.close()
+        return res, out, ga
+
+    base, xb, ga0 = solve(dict(pdl=0, graph=0))
+    res, xv, ga = solve(opts)
+    assert ga0 == 0
+    assert ga == (1 if opts.get("graph", 1) and opts.get("poll_chunk", 8) <= res["iters"] else 0) or "poll_chunk" in opts
+    assert abs(res["iters"] - ref["iters"]) <= 2
+    bn = np.linalg.norm(b)
+    for i, s in enumerate(shifts):
+        assert np.linalg.norm(b - oracle.mdagm(dims, U, m, xv[i], sigma=s)) / bn < 1.5 * tol
+        if "dslash_persist" not in opts:
+            assert np.array_equal(xv[i], xb[i]), (opts, i)
+    if "dslash_persist" not in opts:
+        assert res["iters"] == base["iters"] and np.array_equal(res["conv_iter"], base["conv_iter"])
 
 
 def test_cg_fp32_and_max_iter():

@@ -335,6 +335,46 @@ def test_multishift_residual_identity_and_first_zeta():
     assert np.allclose(ms["beta"][:9], sg["beta"][:9], rtol=1e-10)
 
 
+def test_rational_apply_against_dense_partial_fractions_and_plane_wave():
+    """NEXT-1: y = c0 b + sum_i c_i (A+sigma_i)^-1 b  (the rational function of
+    the RHMC whose poles are the shifts of Eq. 6).  Pins: (i) dense solves; (ii) the partial-fraction
+    identity 1/((A+s1)(A+s2)) = [1/(A+s1) - 1/(A+s2)]/(s2-s1): applying both factors to y must give
+    b back -- catches a wrong sign, a swapped or dropped coefficient, a dropped c0 (checked with a
+    second case); (iii) free field, plane-wave b: y = (c0 + sum c_i/(lambda+sigma_i)) b."""
+    dims = (4, 4, 4, 4)
+    rng = np.random.default_rng(8)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m = 0.05
+    shifts = np.array([0.3, 1e-3, 1.0, 0.02])
+    c0, c = 0.7, np.array([0.5, -1.25, 2.0, 0.125])
+    A, _, _ = dense_normal_operator(dims, U, m)
+    eye = np.eye(A.shape[0])
+    res = oracle.rational_apply(dims, U, m, shifts, c0, c, b, 1e-12, 5000)
+    assert res["converged"]
+    yd = c0 * b.reshape(-1) + sum(ci * np.linalg.solve(A + s * eye, b.reshape(-1)) for ci, s in zip(c, shifts))
+    assert rel(res["y"].reshape(-1), yd) < 1e-9
+    # (ii) partial fractions, checked with the operator only
+    s1, s2 = 0.11, 0.83
+    pf = oracle.rational_apply(dims, U, m, [s1, s2], 0.0, [1.0 / (s2 - s1), -1.0 / (s2 - s1)], b, 1e-12, 5000)
+    back = oracle.mdagm(dims, U, m, oracle.mdagm(dims, U, m, pf["y"], sigma=s2), sigma=s1)
+    assert rel(back, b) < 1e-9
+    # with c0 = 1 and the same poles: (A+s1)(A+s2)(y - b) = b
+    pf1 = oracle.rational_apply(dims, U, m, [s1, s2], 1.0, [1.0 / (s2 - s1), -1.0 / (s2 - s1)], b, 1e-12, 5000)
+    back = oracle.mdagm(dims, U, m, oracle.mdagm(dims, U, m, pf1["y"] - b, sigma=s2), sigma=s1)
+    assert rel(back, b) < 1e-9
+    # (iii) free field plane wave
+    dims = (4, 4, 6, 4)
+    U1 = gen.unit_links(dims)
+    xe = gen.site_coords(dims)[gen.half_index_of_parity(dims, 0)]
+    p = np.array([2 * np.pi / 4, 0.0, 2 * np.pi * 2 / 6, 3 * np.pi / 4])
+    phi = np.exp(1j * (xe @ p))[:, None] * np.array([0.3 - 0.2j, 1.0 + 0.5j, -0.7j])[None, :]
+    lam = 0.37 ** 2 + np.sum(np.sin(p) ** 2)
+    r = oracle.rational_apply(dims, U1, 0.37, shifts, c0, c, phi, 1e-13, 100)
+    assert r["iters"] <= 2
+    assert rel(r["y"], (c0 + np.sum(c / (lam + shifts))) * phi) < 1e-12
+
+
 def test_multishift_rejects_bad_shifts():
     dims = (2, 2, 2, 2)
     U = gen.unit_links(dims)
