@@ -37,6 +37,9 @@ EPS, SEED = 0.3, 3
 FLOP_PER_SITE = 570          # 8*66 + 7*6, SURVEY.md section 8(a) a4
 BYTES_PER_SITE = {("f64", 18): 1248, ("f64", 12): 864, ("f32", 18): 624, ("f32", 12): 432}
 FALLBACK_HBM_GBS = 6650.0    # /opt/skills/guides/B200_PROFILING.md fallback
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the headline kernel, from the ncu --set full
+# capture summarised in profiles/ncu_dslash_r1.md (629.3 MB read + 5.6 MB written; algorithmic 654.3 MB)
+NCU_DRAM_TRAFFIC_BYTES = 634.9e6
 
 
 def measured_hbm_peak():
@@ -180,7 +183,7 @@ def workload_config():
             "l2": "inputs larger than L2 (links 604 MB vs 126 MB L2); no flush needed"}
 
 
-def solver_iter_rate(torch, lat, L, links, b_e, shifts, mass, n_lo=20, n_hi=120):
+def solver_iter_rate(torch, lat, L, links, b_e, shifts, mass, n_lo=24, n_hi=120, rational=False):
     """Time per (multi-shift) CG iteration by differencing two fixed-length solves (tol is
     unreachable, so every shift stays active: worst-case K2 traffic).  Setup, the true-residual
     epilogue and the final sync cancel in the difference."""
@@ -190,7 +193,11 @@ def solver_iter_rate(torch, lat, L, links, b_e, shifts, mass, n_lo=20, n_hi=120)
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        res = lat.cg_multishift(xs, b_e, links, mass, shifts, 1e-300, n, raise_on_max_iter=False)
+        if rational:   # lqcd_rational_apply: y accumulated in K2, the x_i are never stored
+            res = lat.rational_apply(xs[0], b_e, links, mass, shifts, 0.5, [1.0] * len(shifts), 1e-300, n,
+                                     raise_on_max_iter=False)
+        else:
+            res = lat.cg_multishift(xs, b_e, links, mass, shifts, 1e-300, n, raise_on_max_iter=False)
         e1.record()
         torch.cuda.synchronize()
         assert res["iters"] == n, res
@@ -296,6 +303,11 @@ def run_ours(args):
         extra["multishift8_f64"] = {"iter_per_s": 1e3 / ms_it, "us_per_iter": ms_it * 1e3, "bytes_per_site_iter": by,
                                     "GBs": by * Vh / (ms_it * 1e-3) / 1e9, "frac": by * Vh / (ms_it * 1e-3) / 1e9 / peak,
                                     "note": "all 8 shifts active (worst case)"}
+        ms_it = solver_iter_rate(torch, lat, L, links, d_in_e, shifts, 0.0025, rational=True)
+        by = 2544 + 144 + 144 + 96 + 7 * 96
+        extra["rational8_f64"] = {"iter_per_s": 1e3 / ms_it, "us_per_iter": ms_it * 1e3, "bytes_per_site_iter": by,
+                                  "GBs": by * Vh / (ms_it * 1e-3) / 1e9, "frac": by * Vh / (ms_it * 1e-3) / 1e9 / peak,
+                                  "note": "lqcd_rational_apply, 8 shifts all active: y += c_i alpha_i p_i fused, x_i never stored"}
         # ---- CPU oracle beside it -------------------------------------------------------------
         psi = np.zeros((V, 3), dtype=np.complex128)
         psi[gen.half_index_of_parity(DIMS, 0)] = in_e
@@ -308,7 +320,8 @@ def run_ours(args):
             "data": "synthetic", "config": dict(workload_config(), parallelism=f"replicas x{world} (no collective)"),
             "GFLOPs": FLOP_PER_SITE * V * world / (ms / args.steps * 1e-3) / 1e9,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": peak_src, "kernel": "dslash_kernel<double,0,0,0,3>",
+                         "traffic": NCU_DRAM_TRAFFIC_BYTES, "traffic_source": "profiles/ncu_dslash_r1.md (ncu --set full, per launch)",
+                         "peak_source": peak_src, "kernel": "dslash_kernel<double,0,0,0,2,0>",
                          "bytes_per_launch": BYTES_PER_SITE[("f64", 18)] * Vh, "us_per_launch": us_launch,
                          "frac_of_nominal_8TBs": achieved / 8000.0},
             "e2e": {"value": e2e_ms * 1e6 / (e2e_steps * V * world), "unit": "ns/site", "steps": e2e_steps,

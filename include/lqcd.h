@@ -10,6 +10,9 @@
  *   - lqcd_cg              : "the conjugate gradient" on Eq. 8
  *   - lqcd_cg_multishift   : the "multishift inverter routine" for Eq. 6
  *
+ *   - lqcd_rational_apply  : c0 b + sum_i c_i (A + sigma_i)^-1 b, the rational function whose
+ *                            poles are the shifts of Eq. 6, fused into the
+ *                            multi-shift solve
  *   - lqcd_pack_* / unpack : canonical <-> native SoA, parity-split fields (PAPER.md:245-272,
  *                            Figs 1-2, Eq. 9) with optional 2-row ("12-real") links whose third
  *                            row is rebuilt in registers as r2 = (r0 ^ r1)^*
@@ -142,6 +145,26 @@ int lqcd_cg(lqcd_ctx *ctx, void *x_e, const void *b_e, const void *links, double
 int lqcd_cg_multishift(lqcd_ctx *ctx, int nshift, const double *shifts, const void *rhs_e,
                        void *const *solutions_e, const void *links, double mass, double tol,
                        int max_iter, int *iters, int *conv_iter, double *rel_resid);
+
+/*
+ * Rational function of A = mass^2 - D_eo D_oe applied to a vector, fused into the multi-shift
+ * solve:
+ *     y_e = c0 * rhs_e + sum_i coeffs[i] * x_i ,   (A + shifts[i]) x_i = rhs_e        (Eq. 6)
+ * "the algebraic matrix function appearing in Eq. (3) is approximated ... by a
+ * rational function" with the poles sigma_i of Eq. 6; this sum is what the
+ * pseudofermion heatbath and the action evaluation (Algorithm 1 steps 3 and 6)
+ * take from "the multishift inverter routine".  The solutions x_i are never stored: every
+ * iteration adds coeffs[i]*alpha_i*p_i of the still-active shifts to y.  Same recurrences,
+ * stopping rule and freezing as lqcd_cg_multishift (readings R11, R12).
+ *   shifts, coeffs  host, nshift doubles each (shifts >= 0; coefficients any sign)
+ *   rhs_e, y_e      native even-site vectors (device); must not alias
+ *   iters, conv_iter  host outputs as in lqcd_cg_multishift (may be NULL)
+ * blocking.  Needs the workspace of lqcd_workspace_bytes(ctx, nshift).  Errors as lqcd_cg_multishift
+ * (LQCD_ERR_NOT_CONVERGED leaves y at the last iterate).
+ */
+int lqcd_rational_apply(lqcd_ctx *ctx, int nshift, const double *shifts, double c0,
+                        const double *coeffs, const void *rhs_e, void *y_e, const void *links,
+                        double mass, double tol, int max_iter, int *iters, int *conv_iter);
 
 /*
  * After lqcd_cg / lqcd_cg_multishift: copy up to `n` entries of the per-iteration history

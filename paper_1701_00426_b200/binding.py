@@ -28,7 +28,7 @@ class LqcdError(RuntimeError):
 def _load():
     if not os.path.exists(lib_path):
         raise ImportError(
-            f"{lib_path} is missing: build it with `python -m paper_1701_00426_b200.build` "
+            f"{lib_path} is missing: build it with `python paper_1701_00426_b200/build.py` "
             "(or __graft_entry__.build()).  There is no fallback path.")
     return C.CDLL(lib_path)
 
@@ -55,6 +55,7 @@ _sig = {
     "lqcd_mdagm": (_i, [_vp, _vp, _vp, _vp, _d, _d]),
     "lqcd_cg": (_i, [_vp, _vp, _vp, _vp, _d, _d, _i, _pi, _pd]),
     "lqcd_cg_multishift": (_i, [_vp, _i, _pd, _vp, C.POINTER(_vp), _vp, _d, _d, _i, _pi, _pi, _pd]),
+    "lqcd_rational_apply": (_i, [_vp, _i, _pd, _d, _pd, _vp, _vp, _vp, _d, _d, _i, _pi, _pi]),
     "lqcd_solver_history": (_i, [_vp, _i, _pd, _pd, _pd]),
     "lqcd_dslash_host": (_i, [_vp, _i, _vp, _vp, _vp]),
     "lqcd_cg_multishift_host": (_i, [_vp, _i, _pd, _vp, _vp, _vp, _d, _d, _i, _pi, _pi, _pd]),
@@ -212,6 +213,22 @@ class Lattice:
                                                 res.ctypes.data_as(_pd)),
                          allow=() if raise_on_max_iter else (ERR_NOT_CONVERGED,))
         return dict(iters=iters.value, conv_iter=np.array(list(conv)), rel_resid=res, converged=(rc == OK))
+
+    def rational_apply(self, y_e, b_e, links, mass, shifts, c0, coeffs, tol, max_iter, raise_on_max_iter=True):
+        """blocking; y = c0 b + sum_i coeffs[i] (A + shifts[i])^-1 b, accumulated inside the solve."""
+        import numpy as np
+        sh = np.ascontiguousarray(shifts, dtype=np.float64)
+        co = np.ascontiguousarray(coeffs, dtype=np.float64)
+        n = sh.size
+        assert co.size == n
+        self.ensure_workspace(n)
+        iters = C.c_int(0)
+        conv = (C.c_int * n)()
+        rc = self._check(lib.lqcd_rational_apply(self._ctx, n, sh.ctypes.data_as(_pd), float(c0), co.ctypes.data_as(_pd),
+                                                 _vp(b_e.data_ptr()), _vp(y_e.data_ptr()), _vp(links.data_ptr()),
+                                                 mass, tol, max_iter, C.byref(iters), conv),
+                         allow=() if raise_on_max_iter else (ERR_NOT_CONVERGED,))
+        return dict(iters=iters.value, conv_iter=np.array(list(conv)), converged=(rc == OK))
 
     def solver_history(self):
         import numpy as np

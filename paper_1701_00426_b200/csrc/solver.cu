@@ -59,6 +59,10 @@ struct ShiftPtrs {
     void *x[LQCD_MAX_SHIFTS];
     void *p[LQCD_MAX_SHIFTS];
     int nshift, base;
+    // rational mode (lqcd_rational_apply): y = c0 b + sum_i coef[i] x_i is accumulated instead of
+    // storing the x_i; x[] is unused then
+    void *y;
+    double c0, coef[LQCD_MAX_SHIFTS];
 };
 
 // r = p = p_i = b, x_i = 0, rho = ||b||^2
@@ -82,8 +86,13 @@ __global__ void __launch_bounds__(256) init_kernel(size_t npk, const T *__restri
         for (int j = 0; j < N; ++j) acc += (double)a[j] * (double)a[j];
         stv<POLICY>(reinterpret_cast<P *>(r) + k, v, keep);
         stv<POLICY>(reinterpret_cast<P *>(p) + k, v, keep);
+        if (sp.y) {
+            T yy[4];
+            for (int j = 0; j < N; ++j) yy[j] = (T)sp.c0 * a[j];
+            stv<POLICY>(reinterpret_cast<P *>(sp.y) + k, repack(yy), strm);
+        }
         for (int i = 0; i < sp.nshift; ++i) {
-            stv<POLICY>(reinterpret_cast<P *>(sp.x[i]) + k, repack(zero), strm);
+            if (!sp.y) stv<POLICY>(reinterpret_cast<P *>(sp.x[i]) + k, repack(zero), strm);
             if (i != sp.base) stv<POLICY>(reinterpret_cast<P *>(sp.p[i]) + k, v, strm);
         }
     }
@@ -124,7 +133,10 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, T *__restrict__ r, 
 
 // K2: x_i += alpha_i p_i ; p_i = zeta_i r + beta_i p_i ; p = r + beta p.  The base shift has
 // zeta = 1 and p_base == p, so its direction vector is not stored.
-template <typename T, int POLICY>
+// RAT = 1 (lqcd_rational_apply): the solutions are never stored;
+// y += (c_i alpha_i) p_i replaces x_i += alpha_i p_i, which removes 96 B/site/iteration of x_i
+// traffic per active shift in exchange for one read-modify-write of y.
+template <typename T, int POLICY, int RAT>
 __global__ void __launch_bounds__(256) k2_kernel(size_t npk, const T *__restrict__ r, T *__restrict__ p,
                                                  ShiftPtrs sp, const SolverState *__restrict__ st)
 {
@@ -140,7 +152,7 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, const T *__restrict
     __shared__ T s_alpha[LQCD_MAX_SHIFTS], s_zeta[LQCD_MAX_SHIFTS], s_beta[LQCD_MAX_SHIFTS];
     __shared__ int s_active[LQCD_MAX_SHIFTS];
     if (threadIdx.x < sp.nshift) {
-        s_alpha[threadIdx.x] = (T)st->c_alpha[threadIdx.x];
+        s_alpha[threadIdx.x] = RAT ? (T)(sp.coef[threadIdx.x] * st->c_alpha[threadIdx.x]) : (T)st->c_alpha[threadIdx.x];
         s_zeta[threadIdx.x] = (T)st->c_zeta[threadIdx.x];
         s_beta[threadIdx.x] = (T)st->c_beta[threadIdx.x];
         s_active[threadIdx.x] = st->c_active[threadIdx.x];
@@ -151,6 +163,25 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, const T *__restrict
         T rr[4], pp[4];
         unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(r) + k, keep), rr);
         unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(p) + k, keep), pp);
+        if (RAT) {
+            T yy[4];
+            unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(sp.y) + k, strm), yy);
+            for (int i = 0; i < sp.nshift; ++i) {
+                if (!s_active[i]) continue;
+                if (i == sp.base) {
+                    for (int j = 0; j < N; ++j) yy[j] = fma(s_alpha[i], pp[j], yy[j]);
+                } else {
+                    T pi[4];
+                    unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(sp.p[i]) + k, strm), pi);
+                    for (int j = 0; j < N; ++j) {
+                        yy[j] = fma(s_alpha[i], pi[j], yy[j]);
+                        pi[j] = fma(s_beta[i], pi[j], s_zeta[i] * rr[j]);
+                    }
+                    stv<POLICY>(reinterpret_cast<P *>(sp.p[i]) + k, repack(pi), strm);
+                }
+            }
+            stv<POLICY>(reinterpret_cast<P *>(sp.y) + k, repack(yy), strm);
+        } else
         for (int i = 0; i < sp.nshift; ++i) {
             if (!s_active[i]) continue;
             T xx[4];
@@ -209,7 +240,8 @@ static int blas_grid(const lqcd_ctx *ctx, size_t npk)
 template <typename T>
 static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *b, void *const *xs,
                    const void *links, double mass, double tol, int max_iter,
-                   int *iters, int *conv_iter, double *rel_resid)
+                   int *iters, int *conv_iter, double *rel_resid,
+                   void *y = NULL, double c0 = 0.0, const double *coef = NULL)
 {
     const size_t npk = (size_t)ctx->g.Vh * 6 / Pack<T>::N;
     const int grid = blas_grid(ctx, npk), block = ctx->blas_block;
@@ -229,9 +261,12 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         h.zeta[i] = h.zeta_old[i] = 1.0;
         h.delta[i] = shifts[i] - shifts[base];
         h.active[i] = 1;
-        sp.x[i] = xs[i];
+        sp.x[i] = y ? NULL : xs[i];
         sp.p[i] = ws_vec(ctx, 4 + i);
+        if (y) sp.coef[i] = coef[i];
     }
+    sp.y = y;
+    sp.c0 = c0;
     int rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(ctx->d_state, &h, sizeof(h), cudaMemcpyHostToDevice, s), "solver state upload");
     if (rc) return rc;
     if (ctx->l2_hints) launch_k(ctx, init_kernel<T, 1>, dim3(grid), dim3(block), npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
@@ -249,10 +284,16 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         if ((m & 2) && (e = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, p, msq, 1, 1))) return e;
         if (ctx->l2_hints) {
             if (m & 4) launch_k(ctx, k1_kernel<T, 1>, dim3(grid), dim3(block), npk, r, (const T *)q, ctx->d_state, ctx->d_partials);
-            if (m & 8) launch_k(ctx, k2_kernel<T, 1>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+            if (m & 8) {
+                if (sp.y) launch_k(ctx, k2_kernel<T, 1, 1>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+                else launch_k(ctx, k2_kernel<T, 1, 0>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+            }
         } else {
             if (m & 4) launch_k(ctx, k1_kernel<T, 0>, dim3(grid), dim3(block), npk, r, (const T *)q, ctx->d_state, ctx->d_partials);
-            if (m & 8) launch_k(ctx, k2_kernel<T, 0>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+            if (m & 8) {
+                if (sp.y) launch_k(ctx, k2_kernel<T, 0, 1>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+                else launch_k(ctx, k2_kernel<T, 0, 0>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+            }
         }
         return lqcd_check_cuda(ctx, cudaGetLastError(), "cg iteration");
     };
@@ -266,7 +307,12 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     key[kn++] = ((unsigned long long)ctx->poll_chunk << 32) | (unsigned)grid;
     key[kn++] = ((unsigned long long)block << 32) | (unsigned)(ctx->dslash_block * 64 + ctx->dslash_minblocks * 8 + ctx->l2_hints * 4 + ctx->pdl * 2) ^ ((unsigned long long)ctx->dslash_persist << 48);
     key[kn++] = (unsigned long long)(uintptr_t)ctx->stream ^ ((unsigned long long)ctx->iter_mask << 56);
-    for (int i = 0; i < nshift; ++i) key[kn++] = (unsigned long long)(uintptr_t)xs[i];
+    if (y) {
+        key[kn++] = (unsigned long long)(uintptr_t)y;
+        for (int i = 0; i < nshift; ++i) memcpy(&key[kn++], &coef[i], sizeof(double));
+    } else {
+        for (int i = 0; i < nshift; ++i) key[kn++] = (unsigned long long)(uintptr_t)xs[i];
+    }
     ctx->graph_active = 0;
     if (ctx->graph && max_iter >= ctx->poll_chunk) {
         if (!ctx->chunk_exec || ctx->chunk_key_n != kn || memcmp(ctx->chunk_key, key, kn * sizeof(key[0]))) {
@@ -311,7 +357,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         ++chunk_id;
     }
     // true residuals || b - (A + sigma_i) x_i || (reading R10), with the same kernels, ungated
-    for (int i = 0; i < nshift; ++i) {
+    for (int i = 0; i < nshift && !y; ++i) {
         if ((rc = launch_dslash(ctx, LQCD_ODD, tmp_o, xs[i], links, NULL, 0.0, 0, 0))) return rc;
         if ((rc = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, xs[i], mass * mass + shifts[i], 0, 0))) return rc;
         launch_k(ctx, diffnorm_kernel<T, 0>, dim3(grid), dim3(block), npk, (const T *)b, (const T *)q, ctx->d_state, ctx->d_partials, &ctx->d_state->resid[i]);
@@ -323,7 +369,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     int converged = (h.done != 0);
     for (int i = 0; i < nshift; ++i) {
         if (conv_iter) conv_iter[i] = h.active[i] ? h.iter : h.conv_iter[i];
-        if (rel_resid) rel_resid[i] = h.bnorm2 > 0.0 ? sqrt(h.resid[i] / h.bnorm2) : 0.0;
+        if (rel_resid && !y) rel_resid[i] = h.bnorm2 > 0.0 ? sqrt(h.resid[i] / h.bnorm2) : 0.0;
     }
     ctx->hist_n = h.iter < LQCD_HIST ? h.iter : LQCD_HIST;
     memcpy(ctx->h_hist[0], h.hist_alpha, sizeof(h.hist_alpha));
@@ -354,6 +400,31 @@ extern "C" int lqcd_cg_multishift(lqcd_ctx *ctx, int nshift, const double *shift
     if (ctx->prec == LQCD_F64)
         return solve_t<double>(ctx, nshift, shifts, rhs_e, solutions_e, links, mass, tol, max_iter, iters, conv_iter, rel_resid);
     return solve_t<float>(ctx, nshift, shifts, rhs_e, solutions_e, links, mass, tol, max_iter, iters, conv_iter, rel_resid);
+}
+
+extern "C" int lqcd_rational_apply(lqcd_ctx *ctx, int nshift, const double *shifts, double c0, const double *coeffs,
+                                   const void *rhs_e, void *y_e, const void *links, double mass, double tol,
+                                   int max_iter, int *iters, int *conv_iter)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    int rc = lqcd_check_cuda(ctx, cudaSetDevice(ctx->device), "cudaSetDevice");
+    if (rc) return rc;
+    if (nshift < 1 || nshift > LQCD_MAX_SHIFTS) return lqcd_fail(ctx, LQCD_ERR_ARG, "nshift %d not in [1,%d]", nshift, LQCD_MAX_SHIFTS);
+    if (!shifts || !coeffs || !rhs_e || !y_e || !links) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_rational_apply: null pointer");
+    if (y_e == rhs_e) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_rational_apply: y aliases rhs");
+    if (!(tol > 0.0)) return lqcd_fail(ctx, LQCD_ERR_ARG, "tol must be > 0");
+    if (max_iter < 1) return lqcd_fail(ctx, LQCD_ERR_ARG, "max_iter must be >= 1");
+    for (int i = 0; i < nshift; ++i) {
+        if (!(shifts[i] >= 0.0)) return lqcd_fail(ctx, LQCD_ERR_ARG, "shift %d is negative or NaN", i);
+        if (coeffs[i] != coeffs[i]) return lqcd_fail(ctx, LQCD_ERR_ARG, "coefficient %d is NaN", i);
+    }
+    if (c0 != c0) return lqcd_fail(ctx, LQCD_ERR_ARG, "c0 is NaN");
+    if (!ctx->ws) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "no workspace set");
+    if (ctx->ws_bytes < lqcd_workspace_bytes(ctx, nshift))
+        return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "workspace %zu bytes < %zu needed for %d shifts", ctx->ws_bytes, lqcd_workspace_bytes(ctx, nshift), nshift);
+    if (ctx->prec == LQCD_F64)
+        return solve_t<double>(ctx, nshift, shifts, rhs_e, NULL, links, mass, tol, max_iter, iters, conv_iter, NULL, y_e, c0, coeffs);
+    return solve_t<float>(ctx, nshift, shifts, rhs_e, NULL, links, mass, tol, max_iter, iters, conv_iter, NULL, y_e, c0, coeffs);
 }
 
 extern "C" int lqcd_cg(lqcd_ctx *ctx, void *x_e, const void *b_e, const void *links, double mass,

@@ -261,6 +261,61 @@ def test_solver_launch_variants(opts):
         assert res["iters"] == base["iters"] and np.array_equal(res["conv_iter"], base["conv_iter"])
 
 
+@pytest.mark.parametrize("prec", [0, 1])
+def test_rational_apply(prec):
+    """NEXT-1 (lqcd_rational_apply): y = c0 b + sum_i c_i (A+sigma_i)^-1 b accumulated inside the
+    multi-shift solve, against the oracle's definition.  Criteria as R16: same iteration counts;
+    ||y_gpu - y_oracle|| within the sum of the per-shift solution bounds; the partial-fraction
+    identity holds when checked with the ORACLE operator; and the fused y equals the sum formed
+    from the GPU's own stored solutions to rounding."""
+    dims = (8, 8, 8, 16)
+    rng = np.random.default_rng(4)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    U, b = round_inputs(prec, U, b)
+    m = 0.0025 if prec == 0 else 0.05
+    tol = 1e-10 if prec == 0 else 1e-5
+    shifts = gen.rhmc_shifts(8)[[3, 0, 7, 1, 2, 4, 6, 5]]
+    c0 = 0.35
+    c = np.array([0.5, -1.25, 2.0, 0.125, -0.3, 0.9, 1.5, -0.05])
+    ref = oracle.rational_apply(dims, U, m, shifts, c0, c, b, tol, 20000)
+    refx = oracle.cg_multishift(dims, U, m, shifts, b, tol, 20000)
+    assert ref["converged"]
+    lat = make_lattice(dims, prec=prec)
+    links, be = lat.pack_links(U), lat.pack_spinor(b, 0)
+    y = lat.new_spinor()
+    res = lat.rational_apply(y, be, links, m, shifts, c0, c, tol, 20000)
+    yg = lat.unpack_spinor(y, 0)
+    slack = 2 if prec == 0 else 10          # fp32 rounding moves the freeze iteration of a shift
+    assert abs(res["iters"] - ref["iters"]) <= max(slack, ref["iters"] // 50)
+    assert np.all(np.abs(res["conv_iter"] - ref["conv_iter"]) <= np.maximum(slack, ref["conv_iter"] // 50))
+    eps = tol if prec == 0 else 2e-5
+    bound = sum(abs(ci) * 10 * (7.0 / (m * m + s)) * eps * np.linalg.norm(xi)
+                for ci, s, xi in zip(c, shifts, refx["x"])) / np.linalg.norm(ref["y"])
+    assert rel(yg, ref["y"]) < bound, (rel(yg, ref["y"]), bound)
+    # the fused accumulation equals the sum over the GPU's own stored solutions
+    xs = [lat.new_spinor() for _ in shifts]
+    res2 = lat.cg_multishift(xs, be, links, m, shifts, tol, 20000)
+    assert res2["iters"] == res["iters"] and np.array_equal(res2["conv_iter"], res["conv_iter"])
+    y2 = c0 * b + sum(ci * lat.unpack_spinor(x, 0) for ci, x in zip(c, xs))
+    assert rel(yg, y2) < (1e-13 if prec == 0 else 2e-6)
+    # partial fractions: (A+s1)(A+s2) y = b for c = (+-1/(s2-s1)), evaluated with the oracle operator
+    s1, s2 = 0.11, 0.83
+    res = lat.rational_apply(y, be, links, m, [s1, s2], 0.0, [1.0 / (s2 - s1), -1.0 / (s2 - s1)], tol, 20000)
+    yg = lat.unpack_spinor(y, 0)
+    back = oracle.mdagm(dims, U, m, oracle.mdagm(dims, U, m, yg, sigma=s2), sigma=s1)
+    assert rel(back, b) < (30 * tol if prec == 0 else 1e-4)
+    # errors: aliasing, NaN coefficient, negative shift
+    import paper_1701_00426_b200 as L
+    with pytest.raises(L.LqcdError):
+        lat.rational_apply(be, be, links, m, [s1], 0.0, [1.0], tol, 10)
+    with pytest.raises(L.LqcdError):
+        lat.rational_apply(y, be, links, m, [s1], 0.0, [float("nan")], tol, 10)
+    with pytest.raises(L.LqcdError):
+        lat.rational_apply(y, be, links, m, [-1.0], 0.0, [1.0], tol, 10)
+    lat.close()
+
+
 def test_cg_fp32_and_max_iter():
     dims = (8, 8, 8, 8)
     rng = np.random.default_rng(5)
