@@ -149,56 +149,68 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, const T *__restrict
     // together exceed L2 for several shifts: stream them through.
     const uint64_t keep = POLICY ? l2_policy_evict_last() : 0;
     const uint64_t strm = POLICY ? l2_policy_evict_first() : 0;
+    // Coefficients of the ACTIVE non-base shifts, compacted, so that the loop below is branch-free
+    // and can issue the loads of K2_BATCH shifts before the first dependent FMA (the pointers may
+    // alias as far as the compiler knows, so it cannot hoist loads over stores by itself).
     __shared__ T s_alpha[LQCD_MAX_SHIFTS], s_zeta[LQCD_MAX_SHIFTS], s_beta[LQCD_MAX_SHIFTS];
-    __shared__ int s_active[LQCD_MAX_SHIFTS];
-    if (threadIdx.x < sp.nshift) {
-        s_alpha[threadIdx.x] = RAT ? (T)(sp.coef[threadIdx.x] * st->c_alpha[threadIdx.x]) : (T)st->c_alpha[threadIdx.x];
-        s_zeta[threadIdx.x] = (T)st->c_zeta[threadIdx.x];
-        s_beta[threadIdx.x] = (T)st->c_beta[threadIdx.x];
-        s_active[threadIdx.x] = st->c_active[threadIdx.x];
+    __shared__ P *s_x[LQCD_MAX_SHIFTS], *s_p[LQCD_MAX_SHIFTS];
+    __shared__ int s_n, s_base_active;
+    __shared__ T s_base_alpha;
+    if (threadIdx.x == 0) {
+        int n = 0, ba = 0;
+        for (int i = 0; i < sp.nshift; ++i) {
+            if (!st->c_active[i]) continue;
+            const T al = RAT ? (T)(sp.coef[i] * st->c_alpha[i]) : (T)st->c_alpha[i];
+            if (i == sp.base) { ba = 1; s_base_alpha = al; continue; }
+            s_alpha[n] = al;
+            s_zeta[n] = (T)st->c_zeta[i];
+            s_beta[n] = (T)st->c_beta[i];
+            s_x[n] = RAT ? (P *)0 : reinterpret_cast<P *>(sp.x[i]);
+            s_p[n] = reinterpret_cast<P *>(sp.p[i]);
+            ++n;
+        }
+        s_n = n;
+        s_base_active = ba;
     }
     __syncthreads();
-    const T beta = (T)st->beta;
+    const int n_act = s_n, base_active = s_base_active;
+    const T beta = (T)st->beta, base_alpha = base_active ? s_base_alpha : (T)0;
+    P *const xb = RAT ? reinterpret_cast<P *>(sp.y) : reinterpret_cast<P *>(sp.x[sp.base]);
+    constexpr int B = 4;     // shifts whose loads are in flight together
     for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
-        T rr[4], pp[4];
+        T rr[4], pp[4], acc[4];
         unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(r) + k, keep), rr);
         unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(p) + k, keep), pp);
-        if (RAT) {
-            T yy[4];
-            unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(sp.y) + k, strm), yy);
-            for (int i = 0; i < sp.nshift; ++i) {
-                if (!s_active[i]) continue;
-                if (i == sp.base) {
-                    for (int j = 0; j < N; ++j) yy[j] = fma(s_alpha[i], pp[j], yy[j]);
-                } else {
-                    T pi[4];
-                    unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(sp.p[i]) + k, strm), pi);
-                    for (int j = 0; j < N; ++j) {
-                        yy[j] = fma(s_alpha[i], pi[j], yy[j]);
-                        pi[j] = fma(s_beta[i], pi[j], s_zeta[i] * rr[j]);
-                    }
-                    stv<POLICY>(reinterpret_cast<P *>(sp.p[i]) + k, repack(pi), strm);
-                }
-            }
-            stv<POLICY>(reinterpret_cast<P *>(sp.y) + k, repack(yy), strm);
-        } else
-        for (int i = 0; i < sp.nshift; ++i) {
-            if (!s_active[i]) continue;
-            T xx[4];
-            unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(sp.x[i]) + k, strm), xx);
-            if (i == sp.base) {
-                for (int j = 0; j < N; ++j) xx[j] = fma(s_alpha[i], pp[j], xx[j]);
-            } else {
-                T pi[4];
-                unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(sp.p[i]) + k, strm), pi);
-                for (int j = 0; j < N; ++j) {
-                    xx[j] = fma(s_alpha[i], pi[j], xx[j]);
-                    pi[j] = fma(s_beta[i], pi[j], s_zeta[i] * rr[j]);
-                }
-                stv<POLICY>(reinterpret_cast<P *>(sp.p[i]) + k, repack(pi), strm);
-            }
-            stv<POLICY>(reinterpret_cast<P *>(sp.x[i]) + k, repack(xx), strm);
+        // the vector the base shift updates: x_base (or y, which also collects every other shift)
+        const bool touch = RAT ? true : (base_active != 0);
+        if (touch) {
+            unpack<T>(ldv<POLICY>(xb + k, strm), acc);
+            for (int j = 0; j < N; ++j) acc[j] = fma(base_alpha, pp[j], acc[j]);
         }
+        for (int a0 = 0; a0 < n_act; a0 += B) {
+            P vx[B], vp[B];
+#pragma unroll
+            for (int u = 0; u < B; ++u)
+                if (a0 + u < n_act) {
+                    vp[u] = ldv<POLICY>(s_p[a0 + u] + k, strm);
+                    if (!RAT) vx[u] = ldv<POLICY>(s_x[a0 + u] + k, strm);
+                }
+#pragma unroll
+            for (int u = 0; u < B; ++u)
+                if (a0 + u < n_act) {
+                    T pi[4], xx[4];
+                    unpack<T>(vp[u], pi);
+                    if (!RAT) unpack<T>(vx[u], xx);
+                    const T al = s_alpha[a0 + u], ze = s_zeta[a0 + u], be = s_beta[a0 + u];
+                    for (int j = 0; j < N; ++j) {
+                        if (RAT) acc[j] = fma(al, pi[j], acc[j]); else xx[j] = fma(al, pi[j], xx[j]);
+                        pi[j] = fma(be, pi[j], ze * rr[j]);
+                    }
+                    stv<POLICY>(s_p[a0 + u] + k, repack(pi), strm);
+                    if (!RAT) stv<POLICY>(s_x[a0 + u] + k, repack(xx), strm);
+                }
+        }
+        if (touch) stv<POLICY>(xb + k, repack(acc), strm);
         for (int j = 0; j < N; ++j) pp[j] = fma(beta, pp[j], rr[j]);
         stv<POLICY>(reinterpret_cast<P *>(p) + k, repack(pp), keep);
     }
@@ -228,10 +240,21 @@ __global__ void __launch_bounds__(256) diffnorm_kernel(size_t npk, const T *__re
 // ---------------------------------------------------------------------------------------------
 // Host driver
 // ---------------------------------------------------------------------------------------------
-static int blas_grid(const lqcd_ctx *ctx, size_t npk)
+// Grid of a grid-stride vector kernel: ONE resident wave.  The CTAs per SM come from the occupancy
+// calculator for that kernel (registers decide: k1 40 regs -> 6, k2 44 regs -> 5 CTAs of 256), capped
+// by option blas_ctas_per_sm.  (Round-1 bug found with ncu: a fixed 8 CTAs/SM gave 1.33-1.6 waves,
+// i.e. a second, mostly empty pass of every vector kernel.)
+template <typename K>
+static int blas_grid(const lqcd_ctx *ctx, K kern, size_t npk)
 {
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, ctx->blas_block, 0) != cudaSuccess || occ < 1) {
+        cudaGetLastError();
+        occ = 1;
+    }
+    if (occ > ctx->blas_ctas_per_sm) occ = ctx->blas_ctas_per_sm;
     size_t want = (npk + ctx->blas_block - 1) / ctx->blas_block;
-    size_t cap = (size_t)ctx->num_sms * ctx->blas_ctas_per_sm;
+    size_t cap = (size_t)ctx->num_sms * occ;
     size_t g = want < cap ? want : cap;
     if (g > (size_t)ctx->max_partials) g = ctx->max_partials;
     return g < 1 ? 1 : (int)g;
@@ -244,7 +267,12 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
                    void *y = NULL, double c0 = 0.0, const double *coef = NULL)
 {
     const size_t npk = (size_t)ctx->g.Vh * 6 / Pack<T>::N;
-    const int grid = blas_grid(ctx, npk), block = ctx->blas_block;
+    const int block = ctx->blas_block;
+    const int g_init = ctx->l2_hints ? blas_grid(ctx, init_kernel<T, 1>, npk) : blas_grid(ctx, init_kernel<T, 0>, npk);
+    const int g_k1 = ctx->l2_hints ? blas_grid(ctx, k1_kernel<T, 1>, npk) : blas_grid(ctx, k1_kernel<T, 0>, npk);
+    const int g_k2 = y ? (ctx->l2_hints ? blas_grid(ctx, k2_kernel<T, 1, 1>, npk) : blas_grid(ctx, k2_kernel<T, 0, 1>, npk))
+                       : (ctx->l2_hints ? blas_grid(ctx, k2_kernel<T, 1, 0>, npk) : blas_grid(ctx, k2_kernel<T, 0, 0>, npk));
+    const int g_diff = blas_grid(ctx, diffnorm_kernel<T, 0>, npk);
     cudaStream_t s = ctx->stream;
     T *tmp_o = (T *)ws_vec(ctx, 0), *q = (T *)ws_vec(ctx, 1), *r = (T *)ws_vec(ctx, 2), *p = (T *)ws_vec(ctx, 3);
 
@@ -269,8 +297,8 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     sp.c0 = c0;
     int rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(ctx->d_state, &h, sizeof(h), cudaMemcpyHostToDevice, s), "solver state upload");
     if (rc) return rc;
-    if (ctx->l2_hints) launch_k(ctx, init_kernel<T, 1>, dim3(grid), dim3(block), npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
-    else launch_k(ctx, init_kernel<T, 0>, dim3(grid), dim3(block), npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
+    if (ctx->l2_hints) launch_k(ctx, init_kernel<T, 1>, dim3(g_init), dim3(block), npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
+    else launch_k(ctx, init_kernel<T, 0>, dim3(g_init), dim3(block), npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
 
     const double msq = mass * mass + shifts[base];
     volatile int *flag = ctx->h_flag;
@@ -283,16 +311,16 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         if ((m & 1) && (e = launch_dslash(ctx, LQCD_ODD, tmp_o, p, links, NULL, 0.0, 0, 2))) return e;
         if ((m & 2) && (e = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, p, msq, 1, 1))) return e;
         if (ctx->l2_hints) {
-            if (m & 4) launch_k(ctx, k1_kernel<T, 1>, dim3(grid), dim3(block), npk, r, (const T *)q, ctx->d_state, ctx->d_partials);
+            if (m & 4) launch_k(ctx, k1_kernel<T, 1>, dim3(g_k1), dim3(block), npk, r, (const T *)q, ctx->d_state, ctx->d_partials);
             if (m & 8) {
-                if (sp.y) launch_k(ctx, k2_kernel<T, 1, 1>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
-                else launch_k(ctx, k2_kernel<T, 1, 0>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+                if (sp.y) launch_k(ctx, k2_kernel<T, 1, 1>, dim3(g_k2), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+                else launch_k(ctx, k2_kernel<T, 1, 0>, dim3(g_k2), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
             }
         } else {
-            if (m & 4) launch_k(ctx, k1_kernel<T, 0>, dim3(grid), dim3(block), npk, r, (const T *)q, ctx->d_state, ctx->d_partials);
+            if (m & 4) launch_k(ctx, k1_kernel<T, 0>, dim3(g_k1), dim3(block), npk, r, (const T *)q, ctx->d_state, ctx->d_partials);
             if (m & 8) {
-                if (sp.y) launch_k(ctx, k2_kernel<T, 0, 1>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
-                else launch_k(ctx, k2_kernel<T, 0, 0>, dim3(grid), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+                if (sp.y) launch_k(ctx, k2_kernel<T, 0, 1>, dim3(g_k2), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+                else launch_k(ctx, k2_kernel<T, 0, 0>, dim3(g_k2), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
             }
         }
         return lqcd_check_cuda(ctx, cudaGetLastError(), "cg iteration");
@@ -304,7 +332,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     key[kn++] = (unsigned long long)(uintptr_t)ctx->ws; key[kn++] = (unsigned long long)(uintptr_t)links;
     memcpy(&key[kn++], &msq, sizeof(double));
     key[kn++] = ((unsigned long long)nshift << 32) | (unsigned)base;
-    key[kn++] = ((unsigned long long)ctx->poll_chunk << 32) | (unsigned)grid;
+    key[kn++] = ((unsigned long long)ctx->poll_chunk << 32) | (unsigned)(g_k1 * 4096 + g_k2);
     key[kn++] = ((unsigned long long)block << 32) | (unsigned)(ctx->dslash_block * 64 + ctx->dslash_minblocks * 8 + ctx->l2_hints * 4 + ctx->pdl * 2) ^ ((unsigned long long)ctx->dslash_persist << 48);
     key[kn++] = (unsigned long long)(uintptr_t)ctx->stream ^ ((unsigned long long)ctx->iter_mask << 56);
     if (y) {
@@ -360,7 +388,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     for (int i = 0; i < nshift && !y; ++i) {
         if ((rc = launch_dslash(ctx, LQCD_ODD, tmp_o, xs[i], links, NULL, 0.0, 0, 0))) return rc;
         if ((rc = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, xs[i], mass * mass + shifts[i], 0, 0))) return rc;
-        launch_k(ctx, diffnorm_kernel<T, 0>, dim3(grid), dim3(block), npk, (const T *)b, (const T *)q, ctx->d_state, ctx->d_partials, &ctx->d_state->resid[i]);
+        launch_k(ctx, diffnorm_kernel<T, 0>, dim3(g_diff), dim3(block), npk, (const T *)b, (const T *)q, ctx->d_state, ctx->d_partials, &ctx->d_state->resid[i]);
     }
     if ((rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(&h, ctx->d_state, sizeof(h), cudaMemcpyDeviceToHost, s), "solver state download"))) return rc;
     if ((rc = lqcd_check_cuda(ctx, cudaStreamSynchronize(s), "cg"))) return rc;
