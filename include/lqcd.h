@@ -167,6 +167,52 @@ int lqcd_rational_apply(lqcd_ctx *ctx, int nshift, const double *shifts, double 
                         double mass, double tol, int max_iter, int *iters, int *conv_iter);
 
 /*
+ * ---- Slab mode: one x3 slab per GPU (the paper leaves the
+ * multi-device version as future work) --------------------------------------
+ * A rank that owns L3 = N3/P time slices creates its context with dims (N0,N1,N2,L3+2) and
+ * antiperiodic_t = 0: slices 1..L3 are owned, slices 0 and L3+1 are ghost copies of the neighbours'
+ * boundary slices (ghost depth 1, so the local parity is the opposite of the global one when
+ * r*L3 is even).  The staggered phases do not depend on x3 and the antiperiodic sign is applied to
+ * the ghost data when it crosses the global boundary (lqcd_halo_pack's `sign`), so the slab is an
+ * ordinary lattice on which only the owned slices are computed.
+ */
+
+/* out(x) = (D in)(x) for the sites of `parity` with x3 in [x3_lo, x3_hi) only; the other sites of
+ * `out` are not touched.  0 <= x3_lo < x3_hi <= N3.  async.  Lets the caller run the interior
+ * slices while the halo is in flight and the two boundary slices afterwards. */
+int lqcd_dslash_slices(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
+                       int x3_lo, int x3_hi);
+
+/* Bytes of one x3 slice of a native half vector (both parities have N0*N1*N2/2 sites per slice). */
+size_t lqcd_halo_bytes(const lqcd_ctx *ctx);
+/* buf = sign * (slice x3 of spinor), contiguous (device, lqcd_halo_bytes);  async. */
+int lqcd_halo_pack(lqcd_ctx *ctx, void *buf, const void *spinor, int x3, double sign);
+/* slice x3 of spinor = buf;  async. */
+int lqcd_halo_unpack(lqcd_ctx *ctx, void *spinor, const void *buf, int x3);
+
+/*
+ * Communication hooks for the solvers in slab mode.  The library does not link a communication
+ * library: the caller (torch.distributed / NCCL in paper_1701_00426_b200/slab.py) supplies
+ *   halo(user, vec, parity)       fill the ghost slices 0 and N3-1 of the native half vector `vec`
+ *                                 from the neighbours (work enqueued on / ordered with the context's
+ *                                 stream); returns 0 on success
+ *   allreduce(user, dev, count)   sum `count` device doubles at `dev` over all ranks, in place,
+ *                                 ordered with the context's stream; returns 0 on success
+ * With hooks set, lqcd_cg / lqcd_cg_multishift / lqcd_rational_apply / lqcd_mdagm restrict every
+ * vector operation and dot product to the owned slices [x3_lo, x3_hi), call `halo` before each
+ * Dslash, and complete each dot product with `allreduce` before the scalar recurrences (which then
+ * run in a one-thread kernel instead of the last CTA of the reduction).  Pass NULLs to clear.
+ * x3_lo/x3_hi: owned slices (1 and N3-1 for ghost depth 1).  solve_parity: LOCAL parity of the sites
+ * the solvers and lqcd_mdagm act on -- the paper's even sites (Eq. 8) are the local ODD sites of a slab
+ * whose first owned slice sits at an odd local x3 (ghost depth 1, even global offset); the solver then
+ * uses D(1-solve_parity <- solve_parity) first.  The "_e" buffers of those calls are vectors of that parity.
+ */
+typedef int (*lqcd_halo_fn)(void *user, void *vec, int parity);
+typedef int (*lqcd_allreduce_fn)(void *user, void *dev_doubles, int count);
+int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_parity, lqcd_halo_fn halo,
+                  lqcd_allreduce_fn allreduce, void *user);
+
+/*
  * After lqcd_cg / lqcd_cg_multishift: copy up to `n` entries of the per-iteration history
  * (alpha_k, beta_k, ||r_{k+1}||) of the last solve to host arrays (any may be NULL).
  * Returns the number of entries available (<= 64), or a negative status.

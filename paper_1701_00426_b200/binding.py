@@ -37,6 +37,8 @@ lib = _load()
 
 _vp, _i, _d, _sz = C.c_void_p, C.c_int, C.c_double, C.c_size_t
 _pi, _pd = C.POINTER(C.c_int), C.POINTER(C.c_double)
+HALO_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int)        # lqcd_halo_fn
+ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int)   # lqcd_allreduce_fn
 _sig = {
     "lqcd_version": (C.c_char_p, []),
     "lqcd_create": (_i, [C.POINTER(_vp), C.POINTER(_i), _i, _i, _i, _i, _vp]),
@@ -56,6 +58,11 @@ _sig = {
     "lqcd_cg": (_i, [_vp, _vp, _vp, _vp, _d, _d, _i, _pi, _pd]),
     "lqcd_cg_multishift": (_i, [_vp, _i, _pd, _vp, C.POINTER(_vp), _vp, _d, _d, _i, _pi, _pi, _pd]),
     "lqcd_rational_apply": (_i, [_vp, _i, _pd, _d, _pd, _vp, _vp, _vp, _d, _d, _i, _pi, _pi]),
+    "lqcd_dslash_slices": (_i, [_vp, _i, _vp, _vp, _vp, _i, _i]),
+    "lqcd_halo_bytes": (_sz, [_vp]),
+    "lqcd_halo_pack": (_i, [_vp, _vp, _vp, _i, _d]),
+    "lqcd_halo_unpack": (_i, [_vp, _vp, _vp, _i]),
+    "lqcd_set_slab": (_i, [_vp, _i, _i, _i, HALO_FN, ALLREDUCE_FN, _vp]),
     "lqcd_solver_history": (_i, [_vp, _i, _pd, _pd, _pd]),
     "lqcd_dslash_host": (_i, [_vp, _i, _vp, _vp, _vp]),
     "lqcd_cg_multishift_host": (_i, [_vp, _i, _pd, _vp, _vp, _vp, _d, _d, _i, _pi, _pi, _pd]),
@@ -183,6 +190,30 @@ class Lattice:
     # -- the hot path (async unless stated) ---------------------------------------------------
     def dslash(self, parity, out, inp, links):
         self._check(lib.lqcd_dslash(self._ctx, parity, _vp(out.data_ptr()), _vp(inp.data_ptr()), _vp(links.data_ptr())))
+
+    def dslash_slices(self, parity, out, inp, links, x3_lo, x3_hi):
+        self._check(lib.lqcd_dslash_slices(self._ctx, parity, _vp(out.data_ptr()), _vp(inp.data_ptr()),
+                                           _vp(links.data_ptr()), x3_lo, x3_hi))
+
+    @property
+    def halo_bytes(self):
+        return int(lib.lqcd_halo_bytes(self._ctx))
+
+    def halo_pack(self, buf, spinor_ptr, x3, sign=1.0):
+        """spinor_ptr: a native half vector as a tensor or a raw device address."""
+        ptr = spinor_ptr if isinstance(spinor_ptr, int) else spinor_ptr.data_ptr()
+        self._check(lib.lqcd_halo_pack(self._ctx, _vp(buf.data_ptr()), _vp(ptr), x3, float(sign)))
+
+    def halo_unpack(self, spinor_ptr, buf, x3):
+        ptr = spinor_ptr if isinstance(spinor_ptr, int) else spinor_ptr.data_ptr()
+        self._check(lib.lqcd_halo_unpack(self._ctx, _vp(ptr), _vp(buf.data_ptr()), x3))
+
+    def set_slab(self, x3_lo, x3_hi, solve_parity, halo_cb=None, allreduce_cb=None):
+        """halo_cb / allreduce_cb: HALO_FN / ALLREDUCE_FN instances (kept alive here) or None."""
+        self._slab_cbs = (halo_cb, allreduce_cb)
+        self._check(lib.lqcd_set_slab(self._ctx, x3_lo, x3_hi, solve_parity,
+                                      halo_cb if halo_cb is not None else HALO_FN(),
+                                      allreduce_cb if allreduce_cb is not None else ALLREDUCE_FN(), None))
 
     def mdagm(self, out_e, in_e, links, mass, sigma=0.0):
         self.ensure_workspace(1)

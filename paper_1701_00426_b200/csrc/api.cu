@@ -82,6 +82,8 @@ extern "C" int lqcd_create(lqcd_ctx **out, const int dims[4], int prec, int reco
     c->dslash_persist = 0;
     c->iter_mask = 15;
     c->launch_stream = c->stream;
+    c->x3_lo = 0;
+    c->x3_hi = g.N3;
     cudaDeviceProp prop;
     if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) { free(c); return lqcd_check_cuda(NULL, e, "cudaGetDeviceProperties"); }
     c->num_sms = prop.multiProcessorCount;
@@ -268,6 +270,52 @@ extern "C" int lqcd_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in,
     return launch_dslash(ctx, parity, out, in, links, NULL, 0.0, 0, 0);
 }
 
+extern "C" int lqcd_dslash_slices(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
+                                  int x3_lo, int x3_hi)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(out && in && links, "lqcd_dslash_slices: null pointer");
+    REQUIRE(parity == 0 || parity == 1, "lqcd_dslash_slices: parity %d", parity);
+    REQUIRE(out != in, "lqcd_dslash_slices: out and in alias");
+    REQUIRE(0 <= x3_lo && x3_lo < x3_hi && x3_hi <= ctx->g.N3, "lqcd_dslash_slices: bad slice range [%d,%d)", x3_lo, x3_hi);
+    return launch_dslash(ctx, parity, out, in, links, NULL, 0.0, 0, 0, x3_lo, x3_hi);
+}
+
+extern "C" size_t lqcd_halo_bytes(const lqcd_ctx *ctx)
+{
+    return ctx ? (size_t)ctx->g.s3 * 6 * elem_size(ctx) : 0;
+}
+
+extern "C" int lqcd_halo_pack(lqcd_ctx *ctx, void *buf, const void *spinor, int x3, double sign)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(buf && spinor, "lqcd_halo_pack: null pointer");
+    REQUIRE(0 <= x3 && x3 < ctx->g.N3, "lqcd_halo_pack: slice %d", x3);
+    return launch_halo(ctx, 1, buf, (void *)spinor, x3, sign);
+}
+
+extern "C" int lqcd_halo_unpack(lqcd_ctx *ctx, void *spinor, const void *buf, int x3)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(buf && spinor, "lqcd_halo_unpack: null pointer");
+    REQUIRE(0 <= x3 && x3 < ctx->g.N3, "lqcd_halo_unpack: slice %d", x3);
+    return launch_halo(ctx, 0, (void *)buf, spinor, x3, 1.0);
+}
+
+extern "C" int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_parity, lqcd_halo_fn halo,
+                             lqcd_allreduce_fn allreduce, void *user)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(solve_parity == 0 || solve_parity == 1, "lqcd_set_slab: solve_parity %d", solve_parity);
+    ctx->solve_parity = solve_parity;
+    REQUIRE(0 <= x3_lo && x3_lo < x3_hi && x3_hi <= ctx->g.N3, "lqcd_set_slab: bad slice range [%d,%d)", x3_lo, x3_hi);
+    REQUIRE((halo == NULL) == (allreduce == NULL), "lqcd_set_slab: give both hooks or neither");
+    ctx->x3_lo = x3_lo; ctx->x3_hi = x3_hi;
+    ctx->halo_fn = halo; ctx->allreduce_fn = allreduce; ctx->comm_user = user;
+    if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
+    return LQCD_OK;
+}
+
 extern "C" int lqcd_mdagm(lqcd_ctx *ctx, void *out_e, const void *in_e, const void *links, double mass, double sigma)
 {
     int rc = enter(ctx); if (rc) return rc;
@@ -275,7 +323,10 @@ extern "C" int lqcd_mdagm(lqcd_ctx *ctx, void *out_e, const void *in_e, const vo
     REQUIRE(out_e != in_e, "lqcd_mdagm: out and in alias");
     if (!ctx->ws) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "lqcd_mdagm: no workspace set");
     void *tmp_o = ws_vec(ctx, 0);
-    rc = launch_dslash(ctx, LQCD_ODD, tmp_o, in_e, links, NULL, 0.0, 0, 0);
+    const int par = ctx->solve_parity;     // LQCD_EVEN unless a slab says otherwise
+    if (ctx->halo_fn && ctx->halo_fn(ctx->comm_user, (void *)in_e, par)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "halo hook failed");
+    rc = launch_dslash(ctx, 1 - par, tmp_o, in_e, links, NULL, 0.0, 0, 0);
     if (rc) return rc;
-    return launch_dslash(ctx, LQCD_EVEN, out_e, tmp_o, links, in_e, mass * mass + sigma, 0, 0);
+    if (ctx->halo_fn && ctx->halo_fn(ctx->comm_user, tmp_o, 1 - par)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "halo hook failed");
+    return launch_dslash(ctx, par, out_e, tmp_o, links, in_e, mass * mass + sigma, 0, 0);
 }

@@ -202,6 +202,8 @@ struct SolverState {
     int nshift, iter;
     int done;              // 0 running; 1 converged in this iteration (K2 still to run); 2 finished
     unsigned int ticket;   // last-block-done counter of the reductions
+    int comm;              // slab mode: reductions leave LOCAL sums in sum[] (0: <p,q>, 1: <r,r>, 2: <b,b>); the
+    double sum[4];         // recurrences run in scalar_kernel after the caller's all-reduce
     double resid[LQCD_MAX_SHIFTS];  // ||b - (A+sigma_i) x_i||^2 recomputed at exit
     double hist_alpha[LQCD_HIST], hist_beta[LQCD_HIST], hist_rnorm[LQCD_HIST];
 };
@@ -226,6 +228,13 @@ struct lqcd_ctx {
     int pdl;               // 1: programmatic dependent launch (kernel N+1 is scheduled while N drains)
     int graph;             // 1: the solver replays one CUDA graph per chunk of poll_chunk iterations
     int dslash_persist;    // 0: one 128-site tile per CTA; k > 0: num_sms*k CTAs loop over the tiles
+    // slab mode (multi-GPU): the context describes the rank's x3 slab plus one
+    // ghost slice on each side; only the slices [x3_lo, x3_hi) are owned (default: all of them)
+    int x3_lo, x3_hi;
+    int solve_parity;      // local parity of the sites the solvers act on (default LQCD_EVEN)
+    lqcd_halo_fn halo_fn;            // fills the ghost slices of a half vector (NULL: nothing to do)
+    lqcd_allreduce_fn allreduce_fn;  // sums device doubles over the ranks (NULL: single rank)
+    void *comm_user;
     int iter_mask;         // diagnostic: bit k set = kernel k of the CG iteration is launched (default 15)
     int graph_active;      // read-only: the last solve ran from a graph
     cudaStream_t cap_stream;      // private stream used only for graph capture
@@ -286,4 +295,5 @@ int launch_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical, const void 
 // out = D in; if xpay_in != NULL: out = coef*xpay_in - D in and partial Re<xpay_in,out> is reduced
 // into the solver state (dot_mode 1: CG "pq" epilogue; 0: none).  `gate`: obey state->done.
 int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
-                  const void *xpay_in, double coef, int dot_mode, int gate);
+                  const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo = -1, int x3_hi = -1);
+int launch_halo(lqcd_ctx *ctx, int pack, void *buf, void *spinor, int x3, double sign);

@@ -83,7 +83,8 @@ template <typename T, int LAYOUT, int RECON12, int MODE, int MINB, int POLICY>
 __global__ void __launch_bounds__(256, MINB)
 dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__restrict__ in,
               const T *__restrict__ links, const T *__restrict__ xin, const double coef,
-              SolverState *__restrict__ st, double *__restrict__ partials, const int gate)
+              SolverState *__restrict__ st, double *__restrict__ partials, const int gate,
+              const int i_begin, const int i_end)
 {
     pdl_wait();
     pdl_trigger();
@@ -101,9 +102,10 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
     // One tile = blockDim.x consecutive sites.  gridDim.x = number of tiles (one pass), or fewer
     // CTAs that loop (option dslash_persist): the reduction protocol below is then paid once per
     // CTA instead of once per tile.
-    for (int tile0 = blockIdx.x * blockDim.x; tile0 < g.Vh; tile0 += gridDim.x * blockDim.x) {
+    // Sites [i_begin, i_end): the whole parity, or a range of x3 slices (lqcd_dslash_slices; slab mode).
+    for (int tile0 = i_begin + blockIdx.x * blockDim.x; tile0 < i_end; tile0 += gridDim.x * blockDim.x) {
     const int i = tile0 + threadIdx.x;
-    const bool valid = i < g.Vh;
+    const bool valid = i < i_end;
     if (valid) {
         // ---- a2: site decode (Eq. 9), neighbours, phases ---------------------------------
         uint32_t t = fd_div((uint32_t)i, g.dNh0);
@@ -170,22 +172,25 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
     }
     if (MODE == 2) {
         double total;
-        if (grid_sum_last(dot, partials, &st->ticket, &total)) solver_after_pq(st, total);
+        if (grid_sum_last(dot, partials, &st->ticket, &total)) {
+            if (st->comm) st->sum[0] = total; else solver_after_pq(st, total);
+        }
     }
 }
 
 template <typename T, int LAYOUT, int RECON12, int MODE>
 static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
-                     const void *xin, double coef, int gate)
+                     const void *xin, double coef, int gate, int i_begin, int i_end)
 {
     int block = ctx->dslash_block > 256 ? 256 : ctx->dslash_block;
-    int tiles = (ctx->g.Vh + block - 1) / block;
+    int tiles = (i_end - i_begin + block - 1) / block;
+    if (tiles < 1) tiles = 1;
     if (ctx->dslash_persist > 0 && tiles > ctx->num_sms * ctx->dslash_persist) tiles = ctx->num_sms * ctx->dslash_persist;
     dim3 grid(tiles);
     int minb = ctx->dslash_minblocks;
     if (minb == 0) minb = sizeof(T) == 8 ? 2 : 3;
 #define GO1(MB, P) launch_k(ctx, dslash_kernel<T, LAYOUT, RECON12, MODE, MB, P>, grid, dim3(block), \
-        ctx->g, parity, (T *)out, (const T *)in, (const T *)links, (const T *)xin, coef, ctx->d_state, ctx->d_partials, gate)
+        ctx->g, parity, (T *)out, (const T *)in, (const T *)links, (const T *)xin, coef, ctx->d_state, ctx->d_partials, gate, i_begin, i_end)
 #define GO(MB) do { if (ctx->l2_hints) GO1(MB, 1); else GO1(MB, 0); } while (0)
     if (minb <= 2) GO(2); else if (minb == 3) GO(3); else GO(4);
 #undef GO
@@ -194,24 +199,26 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
 
 template <typename T, int LAYOUT>
 static void launch_tl(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
-                      const void *xin, double coef, int mode, int gate)
+                      const void *xin, double coef, int mode, int gate, int i_begin, int i_end)
 {
-#define GO(R, M) launch_t<T, LAYOUT, R, M>(ctx, parity, out, in, links, xin, coef, gate)
+#define GO(R, M) launch_t<T, LAYOUT, R, M>(ctx, parity, out, in, links, xin, coef, gate, i_begin, i_end)
     if (ctx->recon == LQCD_RECON_12) { if (mode == 0) GO(1, 0); else if (mode == 1) GO(1, 1); else GO(1, 2); }
     else { if (mode == 0) GO(0, 0); else if (mode == 1) GO(0, 1); else GO(0, 2); }
 #undef GO
 }
 
 int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
-                  const void *xpay_in, double coef, int dot_mode, int gate)
+                  const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo, int x3_hi)
 {
     int mode = xpay_in ? (dot_mode ? 2 : 1) : 0;
+    if (x3_lo < 0) { x3_lo = ctx->x3_lo; x3_hi = ctx->x3_hi; }      // the context's interior slices
+    const int i_begin = x3_lo * ctx->g.s3, i_end = x3_hi * ctx->g.s3;
     if (ctx->prec == LQCD_F64) {
-        if (ctx->layout == 0) launch_tl<double, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
-        else launch_tl<double, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
+        if (ctx->layout == 0) launch_tl<double, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end);
+        else launch_tl<double, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end);
     } else {
-        if (ctx->layout == 0) launch_tl<float, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
-        else launch_tl<float, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate);
+        if (ctx->layout == 0) launch_tl<float, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end);
+        else launch_tl<float, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end);
     }
     return lqcd_check_cuda(ctx, cudaGetLastError(), "dslash");
 }

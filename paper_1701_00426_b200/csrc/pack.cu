@@ -54,6 +54,35 @@ __global__ void unpack_spinor_kernel(Geom g, double2 *__restrict__ canon, const 
     }
 }
 
+// One x3 slice (s3 = Nh0*N1*N2 sites) of a native half vector <-> a contiguous buffer laid out like a
+// half vector of s3 sites.  PACK: buf = sign * slice; else slice = buf.  (Slab mode halo, lqcd.h.)
+template <typename T, int LAYOUT, int PACK>
+__global__ void halo_kernel(Geom g, T *__restrict__ buf, T *__restrict__ spinor, int x3, T sign)
+{
+    pdl_wait();
+    pdl_trigger();
+    int f = blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= g.s3) return;
+    const size_t i = (size_t)x3 * g.s3 + f;
+    for (int c = 0; c < 3; ++c) {
+        if (PACK) {
+            Cx<T> z = ld_cx<T, LAYOUT, 0, 0>(spinor, (size_t)c, (size_t)g.Vh, i, L2Pol());
+            st_cx<T, LAYOUT, 0>(buf, (size_t)c, (size_t)g.s3, (size_t)f, cx<T>(sign * z.re, sign * z.im), L2Pol());
+        } else {
+            // plain (coherent) load: the buffer was just written by a copy / another rank
+            Cx<T> z;
+            if (LAYOUT == 0) {
+                typedef typename Vec2<T>::type V2;
+                V2 v = reinterpret_cast<const V2 *>(buf)[(size_t)c * g.s3 + f];
+                z = cx<T>(v.x, v.y);
+            } else {
+                z = cx<T>(buf[(size_t)(2 * c) * g.s3 + f], buf[(size_t)(2 * c + 1) * g.s3 + f]);
+            }
+            st_cx<T, LAYOUT, 0>(spinor, (size_t)c, (size_t)g.Vh, i, z, L2Pol());
+        }
+    }
+}
+
 #define DISPATCH_TL(ctx, CALL)                                             \
     do {                                                                   \
         if ((ctx)->prec == LQCD_F64) {                                     \
@@ -94,4 +123,14 @@ int launch_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical, const void 
 #undef CALL
     ctx->launches++;
     return lqcd_check_cuda(ctx, cudaGetLastError(), "unpack_spinor");
+}
+
+int launch_halo(lqcd_ctx *ctx, int pack, void *buf, void *spinor, int x3, double sign)
+{
+    dim3 grid((ctx->g.s3 + 127) / 128), block(128);
+#define CALL(T, L) do { if (pack) launch_k(ctx, halo_kernel<T, L, 1>, grid, block, ctx->g, (T *)buf, (T *)spinor, x3, (T)sign); \
+                        else launch_k(ctx, halo_kernel<T, L, 0>, grid, block, ctx->g, (T *)buf, (T *)spinor, x3, (T)sign); } while (0)
+    DISPATCH_TL(ctx, CALL);
+#undef CALL
+    return lqcd_check_cuda(ctx, cudaGetLastError(), "halo");
 }

@@ -55,6 +55,17 @@ template <int POLICY> __device__ __forceinline__ void stv(float4 *p, float4 v, u
     asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(pol) : "memory");
 }
 
+// Slab mode: the vector kernels touch only the owned x3 slices, i.e. `nseg` runs of `len` packets that
+// start `off` packets into planes `stride` packets apart (layout 0: 3 complex planes; layout 1: 6 real
+// planes).  len == 0: the whole vector, flat (single GPU).
+struct Seg { unsigned int len, stride, off; };
+__device__ __forceinline__ size_t seg_idx(size_t k, const Seg &sg)
+{
+    if (sg.len == 0) return k;
+    const unsigned int pl = (unsigned int)k / sg.len;
+    return (size_t)pl * sg.stride + sg.off + ((unsigned int)k - pl * sg.len);
+}
+
 struct ShiftPtrs {
     void *x[LQCD_MAX_SHIFTS];
     void *p[LQCD_MAX_SHIFTS];
@@ -67,7 +78,7 @@ struct ShiftPtrs {
 
 // r = p = p_i = b, x_i = 0, rho = ||b||^2
 template <typename T, int POLICY>
-__global__ void __launch_bounds__(256) init_kernel(size_t npk, const T *__restrict__ b, T *__restrict__ r,
+__global__ void __launch_bounds__(256) init_kernel(size_t npk, Seg sg, const T *__restrict__ b, T *__restrict__ r,
                                                    T *__restrict__ p, ShiftPtrs sp, SolverState *st,
                                                    double *partials)
 {
@@ -79,7 +90,8 @@ __global__ void __launch_bounds__(256) init_kernel(size_t npk, const T *__restri
     const uint64_t strm = POLICY ? l2_policy_evict_first() : 0;
     double acc = 0.0;
     T zero[4] = {0, 0, 0, 0};
-    for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
+    for (size_t k0 = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k0 < npk; k0 += (size_t)gridDim.x * blockDim.x) {
+        const size_t k = seg_idx(k0, sg);
         P v = ldv<POLICY>(reinterpret_cast<const P *>(b) + k, keep);
         T a[4];
         unpack<T>(v, a);
@@ -98,15 +110,18 @@ __global__ void __launch_bounds__(256) init_kernel(size_t npk, const T *__restri
     }
     double total;
     if (grid_sum_last(acc, partials, &st->ticket, &total)) {
-        st->rho = total;
-        st->bnorm2 = total;
-        if (total == 0.0) st->done = 2;
+        if (st->comm) st->sum[2] = total;
+        else {
+            st->rho = total;
+            st->bnorm2 = total;
+            if (total == 0.0) st->done = 2;
+        }
     }
 }
 
 // K1: r -= alpha q ; <r,r>
 template <typename T, int POLICY>
-__global__ void __launch_bounds__(256) k1_kernel(size_t npk, T *__restrict__ r, const T *__restrict__ q,
+__global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restrict__ r, const T *__restrict__ q,
                                                  SolverState *st, double *partials)
 {
     pdl_wait();
@@ -117,7 +132,8 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, T *__restrict__ r, 
     const uint64_t keep = POLICY ? l2_policy_evict_last() : 0;
     const T alpha = (T)st->alpha;
     double acc = 0.0;
-    for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
+    for (size_t k0 = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k0 < npk; k0 += (size_t)gridDim.x * blockDim.x) {
+        const size_t k = seg_idx(k0, sg);
         T a[4], c[4];
         unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(r) + k, keep), a);
         unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(q) + k, keep), c);
@@ -128,7 +144,9 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, T *__restrict__ r, 
         stv<POLICY>(reinterpret_cast<P *>(r) + k, repack(a), keep);
     }
     double total;
-    if (grid_sum_last(acc, partials, &st->ticket, &total)) solver_after_rr(st, total);
+    if (grid_sum_last(acc, partials, &st->ticket, &total)) {
+        if (st->comm) st->sum[1] = total; else solver_after_rr(st, total);
+    }
 }
 
 // K2: x_i += alpha_i p_i ; p_i = zeta_i r + beta_i p_i ; p = r + beta p.  The base shift has
@@ -137,7 +155,7 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, T *__restrict__ r, 
 // y += (c_i alpha_i) p_i replaces x_i += alpha_i p_i, which removes 96 B/site/iteration of x_i
 // traffic per active shift in exchange for one read-modify-write of y.
 template <typename T, int POLICY, int RAT>
-__global__ void __launch_bounds__(256) k2_kernel(size_t npk, const T *__restrict__ r, T *__restrict__ p,
+__global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__restrict__ r, T *__restrict__ p,
                                                  ShiftPtrs sp, const SolverState *__restrict__ st)
 {
     pdl_wait();
@@ -177,7 +195,8 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, const T *__restrict
     const T beta = (T)st->beta, base_alpha = base_active ? s_base_alpha : (T)0;
     P *const xb = RAT ? reinterpret_cast<P *>(sp.y) : reinterpret_cast<P *>(sp.x[sp.base]);
     constexpr int B = 4;     // shifts whose loads are in flight together
-    for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
+    for (size_t k0 = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k0 < npk; k0 += (size_t)gridDim.x * blockDim.x) {
+        const size_t k = seg_idx(k0, sg);
         T rr[4], pp[4], acc[4];
         unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(r) + k, keep), rr);
         unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(p) + k, keep), pp);
@@ -216,9 +235,27 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, const T *__restrict
     }
 }
 
+// Slab mode: the scalar step that the last CTA of a reduction performs on a single GPU, run after the
+// caller's all-reduce of st->sum[which] (0: after <p,q>; 1: after <r,r>; 2: after <b,b>).
+__global__ void scalar_kernel(SolverState *st, int which)
+{
+    pdl_wait();
+    pdl_trigger();
+    if (threadIdx.x || blockIdx.x) return;
+    if (which == 2) {
+        const double t = st->sum[2];
+        st->rho = t;
+        st->bnorm2 = t;
+        if (t == 0.0) st->done = 2;
+        return;
+    }
+    if (*(volatile int *)&st->done) return;
+    if (which == 0) solver_after_pq(st, st->sum[0]); else solver_after_rr(st, st->sum[1]);
+}
+
 // ||a - b||^2 -> *slot
 template <typename T, int POLICY>
-__global__ void __launch_bounds__(256) diffnorm_kernel(size_t npk, const T *__restrict__ a, const T *__restrict__ b,
+__global__ void __launch_bounds__(256) diffnorm_kernel(size_t npk, Seg sg, const T *__restrict__ a, const T *__restrict__ b,
                                                        SolverState *st, double *partials, double *slot)
 {
     pdl_wait();
@@ -227,7 +264,8 @@ __global__ void __launch_bounds__(256) diffnorm_kernel(size_t npk, const T *__re
     const int N = Pack<T>::N;
     const uint64_t keep = POLICY ? l2_policy_evict_last() : 0;
     double acc = 0.0;
-    for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < npk; k += (size_t)gridDim.x * blockDim.x) {
+    for (size_t k0 = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k0 < npk; k0 += (size_t)gridDim.x * blockDim.x) {
+        const size_t k = seg_idx(k0, sg);
         T x[4], y[4];
         unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(a) + k, keep), x);
         unpack<T>(ldv<POLICY>(reinterpret_cast<const P *>(b) + k, keep), y);
@@ -266,7 +304,32 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
                    int *iters, int *conv_iter, double *rel_resid,
                    void *y = NULL, double c0 = 0.0, const double *coef = NULL)
 {
-    const size_t npk = (size_t)ctx->g.Vh * 6 / Pack<T>::N;
+    // vector kernels: the whole half vector, or (slab mode) only the owned x3 slices of each plane
+    size_t npk = (size_t)ctx->g.Vh * 6 / Pack<T>::N;
+    Seg sg = {0, 0, 0};
+    if (ctx->x3_lo != 0 || ctx->x3_hi != ctx->g.N3) {
+        const unsigned per = ctx->layout == 0 ? 2 : 1;                 // reals per site in one plane
+        const unsigned nseg = ctx->layout == 0 ? 3 : 6;
+        sg.len = (unsigned)((size_t)(ctx->x3_hi - ctx->x3_lo) * ctx->g.s3 * per / Pack<T>::N);
+        sg.stride = (unsigned)((size_t)ctx->g.Vh * per / Pack<T>::N);
+        sg.off = (unsigned)((size_t)ctx->x3_lo * ctx->g.s3 * per / Pack<T>::N);
+        npk = (size_t)nseg * sg.len;
+    }
+    const int comm = ctx->allreduce_fn != NULL;
+    const int par = ctx->solve_parity;                                 // parity of x, b, p, r, q
+    SolverState *const dst = ctx->d_state;
+    // slab hooks: ghost slices of a vector before it is a Dslash input; global sum of a local dot product
+    auto halo = [&](void *v, int parity) -> int {
+        if (!ctx->halo_fn) return LQCD_OK;
+        if (ctx->halo_fn(ctx->comm_user, v, parity)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "halo hook failed");
+        return LQCD_OK;
+    };
+    auto reduce_then = [&](int which) -> int {
+        if (!comm) return LQCD_OK;
+        if (ctx->allreduce_fn(ctx->comm_user, &dst->sum[which], 1)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "allreduce hook failed");
+        launch_k(ctx, scalar_kernel, dim3(1), dim3(32), dst, which);
+        return lqcd_check_cuda(ctx, cudaGetLastError(), "scalar kernel");
+    };
     const int block = ctx->blas_block;
     const int g_init = ctx->l2_hints ? blas_grid(ctx, init_kernel<T, 1>, npk) : blas_grid(ctx, init_kernel<T, 0>, npk);
     const int g_k1 = ctx->l2_hints ? blas_grid(ctx, k1_kernel<T, 1>, npk) : blas_grid(ctx, k1_kernel<T, 0>, npk);
@@ -282,6 +345,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     SolverState h;
     memset(&h, 0, sizeof(h));
     h.alpha_prev = 1.0; h.beta_prev = 0.0; h.tol = tol; h.nshift = nshift;
+    h.comm = comm;
     ShiftPtrs sp;
     memset(&sp, 0, sizeof(sp));
     sp.nshift = nshift; sp.base = base;
@@ -297,8 +361,9 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     sp.c0 = c0;
     int rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(ctx->d_state, &h, sizeof(h), cudaMemcpyHostToDevice, s), "solver state upload");
     if (rc) return rc;
-    if (ctx->l2_hints) launch_k(ctx, init_kernel<T, 1>, dim3(g_init), dim3(block), npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
-    else launch_k(ctx, init_kernel<T, 0>, dim3(g_init), dim3(block), npk, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
+    if (ctx->l2_hints) launch_k(ctx, init_kernel<T, 1>, dim3(g_init), dim3(block), npk, sg, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
+    else launch_k(ctx, init_kernel<T, 0>, dim3(g_init), dim3(block), npk, sg, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
+    if ((rc = reduce_then(2))) return rc;
 
     const double msq = mass * mass + shifts[base];
     volatile int *flag = ctx->h_flag;
@@ -308,19 +373,29 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     auto enqueue_iteration = [&]() -> int {
         int e;
         const int m = ctx->iter_mask;   // diagnostic: which of the 4 kernels run (timing experiments only)
-        if ((m & 1) && (e = launch_dslash(ctx, LQCD_ODD, tmp_o, p, links, NULL, 0.0, 0, 2))) return e;
-        if ((m & 2) && (e = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, p, msq, 1, 1))) return e;
-        if (ctx->l2_hints) {
-            if (m & 4) launch_k(ctx, k1_kernel<T, 1>, dim3(g_k1), dim3(block), npk, r, (const T *)q, ctx->d_state, ctx->d_partials);
+        if ((e = halo(p, par))) return e;
+        if ((m & 1) && (e = launch_dslash(ctx, 1 - par, tmp_o, p, links, NULL, 0.0, 0, 2))) return e;
+        if ((e = halo(tmp_o, 1 - par))) return e;
+        if ((m & 2) && (e = launch_dslash(ctx, par, q, tmp_o, links, p, msq, 1, 1))) return e;
+        if ((e = reduce_then(0))) return e;
+        if (comm) {    // slab mode: the all-reduce of <r,r> sits between K1 and K2
+            if (m & 4) launch_k(ctx, k1_kernel<T, 0>, dim3(g_k1), dim3(block), npk, sg, r, (const T *)q, ctx->d_state, ctx->d_partials);
+            if ((e = reduce_then(1))) return e;
             if (m & 8) {
-                if (sp.y) launch_k(ctx, k2_kernel<T, 1, 1>, dim3(g_k2), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
-                else launch_k(ctx, k2_kernel<T, 1, 0>, dim3(g_k2), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+                if (sp.y) launch_k(ctx, k2_kernel<T, 0, 1>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+                else launch_k(ctx, k2_kernel<T, 0, 0>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+            }
+        } else if (ctx->l2_hints) {
+            if (m & 4) launch_k(ctx, k1_kernel<T, 1>, dim3(g_k1), dim3(block), npk, sg, r, (const T *)q, ctx->d_state, ctx->d_partials);
+            if (m & 8) {
+                if (sp.y) launch_k(ctx, k2_kernel<T, 1, 1>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+                else launch_k(ctx, k2_kernel<T, 1, 0>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
             }
         } else {
-            if (m & 4) launch_k(ctx, k1_kernel<T, 0>, dim3(g_k1), dim3(block), npk, r, (const T *)q, ctx->d_state, ctx->d_partials);
+            if (m & 4) launch_k(ctx, k1_kernel<T, 0>, dim3(g_k1), dim3(block), npk, sg, r, (const T *)q, ctx->d_state, ctx->d_partials);
             if (m & 8) {
-                if (sp.y) launch_k(ctx, k2_kernel<T, 0, 1>, dim3(g_k2), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
-                else launch_k(ctx, k2_kernel<T, 0, 0>, dim3(g_k2), dim3(block), npk, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+                if (sp.y) launch_k(ctx, k2_kernel<T, 0, 1>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
+                else launch_k(ctx, k2_kernel<T, 0, 0>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
             }
         }
         return lqcd_check_cuda(ctx, cudaGetLastError(), "cg iteration");
@@ -330,6 +405,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     unsigned long long key[48];
     int kn = 0;
     key[kn++] = (unsigned long long)(uintptr_t)ctx->ws; key[kn++] = (unsigned long long)(uintptr_t)links;
+    key[kn++] = ((unsigned long long)ctx->x3_lo << 40) | ((unsigned long long)ctx->x3_hi << 8) | (unsigned)par;
     memcpy(&key[kn++], &msq, sizeof(double));
     key[kn++] = ((unsigned long long)nshift << 32) | (unsigned)base;
     key[kn++] = ((unsigned long long)ctx->poll_chunk << 32) | (unsigned)(g_k1 * 4096 + g_k2);
@@ -342,7 +418,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         for (int i = 0; i < nshift; ++i) key[kn++] = (unsigned long long)(uintptr_t)xs[i];
     }
     ctx->graph_active = 0;
-    if (ctx->graph && max_iter >= ctx->poll_chunk) {
+    if (ctx->graph && max_iter >= ctx->poll_chunk && !comm && !ctx->halo_fn) {
         if (!ctx->chunk_exec || ctx->chunk_key_n != kn || memcmp(ctx->chunk_key, key, kn * sizeof(key[0]))) {
             if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
             const long launches0 = ctx->launches;
@@ -386,10 +462,13 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     }
     // true residuals || b - (A + sigma_i) x_i || (reading R10), with the same kernels, ungated
     for (int i = 0; i < nshift && !y; ++i) {
-        if ((rc = launch_dslash(ctx, LQCD_ODD, tmp_o, xs[i], links, NULL, 0.0, 0, 0))) return rc;
-        if ((rc = launch_dslash(ctx, LQCD_EVEN, q, tmp_o, links, xs[i], mass * mass + shifts[i], 0, 0))) return rc;
-        launch_k(ctx, diffnorm_kernel<T, 0>, dim3(g_diff), dim3(block), npk, (const T *)b, (const T *)q, ctx->d_state, ctx->d_partials, &ctx->d_state->resid[i]);
+        if ((rc = halo(xs[i], par))) return rc;
+        if ((rc = launch_dslash(ctx, 1 - par, tmp_o, xs[i], links, NULL, 0.0, 0, 0))) return rc;
+        if ((rc = halo(tmp_o, 1 - par))) return rc;
+        if ((rc = launch_dslash(ctx, par, q, tmp_o, links, xs[i], mass * mass + shifts[i], 0, 0))) return rc;
+        launch_k(ctx, diffnorm_kernel<T, 0>, dim3(g_diff), dim3(block), npk, sg, (const T *)b, (const T *)q, ctx->d_state, ctx->d_partials, &ctx->d_state->resid[i]);
     }
+    if (comm && !y && ctx->allreduce_fn(ctx->comm_user, &dst->resid[0], nshift)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "allreduce hook failed");
     if ((rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(&h, ctx->d_state, sizeof(h), cudaMemcpyDeviceToHost, s), "solver state download"))) return rc;
     if ((rc = lqcd_check_cuda(ctx, cudaStreamSynchronize(s), "cg"))) return rc;
 

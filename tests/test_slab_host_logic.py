@@ -1,0 +1,126 @@
+"""-m "not gpu": host logic of the x3-slab decomposition (paper_1701_00426_b200/slab.py, NEXT-2).
+
+The design claim -- a slab with one ghost slice per side is an ORDINARY lattice with antiperiodic_t = 0,
+the opposite local parity, and the boundary sign carried by the halo data -- is checked against the
+oracle on the CPU: the oracle applied to each rank's local fields reproduces, on the owned slices, the
+oracle applied to the global lattice.  The exchange itself runs under gloo with world_size 2."""
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+import lqcd_inputs as gen
+import oracle
+from paper_1701_00426_b200.slab import SlabGeometry
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def rel(a, b):
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+def signed_local_half(geo, phi, gp, ap):
+    """What a rank's local vector holds after a halo exchange: true neighbour slices, with the sender's
+    boundary sign on the ghosts."""
+    loc = geo.extract_half(phi, gp)
+    s3 = geo.slice_sites // 2
+    # bottom ghost came from `down`'s top slice (sender sign_send_up of that rank); top ghost from `up`
+    down = SlabGeometry(geo.dims, geo.world, geo.down, ap)
+    up = SlabGeometry(geo.dims, geo.world, geo.up, ap)
+    loc[:s3] *= down.sign_send_up
+    loc[-s3:] *= up.sign_send_down
+    return loc
+
+
+@pytest.mark.parametrize("ap", [True, False])
+@pytest.mark.parametrize("world", [1, 2, 4])
+def test_slab_is_an_ordinary_lattice_with_signed_ghosts(world, ap):
+    dims = (4, 6, 2, 8)
+    rng = np.random.default_rng(21)
+    U = gen.haar_like_links(dims, rng)
+    psi = gen.gaussian_spinor(dims, rng)
+    for gp_out in (0, 1):
+        phi_in = oracle.full_to_half(dims, 1 - gp_out, psi)
+        want = oracle.dslash_half(dims, U, gp_out, phi_in, antiperiodic_t=ap)
+        got = np.zeros_like(want)
+        for rank in range(world):
+            geo = SlabGeometry(dims, world, rank, ap)
+            assert geo.local_parity(gp_out) == 1 - gp_out
+            U_loc = np.ascontiguousarray(geo.extract_full(U))
+            in_loc = signed_local_half(geo, phi_in, 1 - gp_out, ap)
+            out_loc = oracle.dslash_half(geo.local_dims, U_loc, geo.local_parity(gp_out), in_loc,
+                                         antiperiodic_t=False)
+            geo.insert_half(out_loc, gp_out, got)
+        assert rel(got, want) < 1e-14, (world, ap, gp_out)
+
+
+def test_geometry_roundtrip_and_errors():
+    dims = (4, 4, 2, 8)
+    phi = gen.gaussian_half_spinor(dims, 3)
+    out = np.zeros_like(phi)
+    for rank in range(2):
+        geo = SlabGeometry(dims, 2, rank)
+        assert geo.local_dims == (4, 4, 2, 6) and (geo.x3_lo, geo.x3_hi) == (1, 5)
+        geo.insert_half(geo.extract_half(phi, 0), 0, out)
+    assert np.array_equal(out, phi)
+    g0, g1 = SlabGeometry(dims, 2, 0), SlabGeometry(dims, 2, 1)
+    assert g0.global_x3_of_local() == [7, 0, 1, 2, 3, 4] and g1.global_x3_of_local() == [3, 4, 5, 6, 7, 0]
+    assert (g0.sign_send_down, g0.sign_send_up, g1.sign_send_down, g1.sign_send_up) == (-1.0, 1.0, 1.0, -1.0)
+    assert SlabGeometry(dims, 1, 0).sign_send_up == -1.0 and SlabGeometry(dims, 1, 0, False).sign_send_up == 1.0
+    with pytest.raises(ValueError):
+        SlabGeometry(dims, 8, 0)        # slabs of thickness 1
+    with pytest.raises(ValueError):
+        SlabGeometry(dims, 3, 0)
+    with pytest.raises(ValueError):
+        SlabGeometry(dims, 2, 2)
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, %r)
+import numpy as np, torch
+import torch.distributed as dist
+import lqcd_inputs as gen
+from paper_1701_00426_b200.slab import SlabGeometry, SlabComm
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo", rank=rank, world_size=world)
+dims = (4, 4, 2, 8)
+phi = gen.gaussian_half_spinor(dims, 7)              # same global vector on both ranks
+geo = SlabGeometry(dims, world, rank)
+comm = SlabComm(world, rank)
+loc = geo.extract_half(phi, 0)                        # ghosts hold the TRUE neighbour values
+s3 = geo.slice_sites // 2
+top = torch.from_numpy(np.ascontiguousarray(loc[-2 * s3:-s3]) * geo.sign_send_up)
+bot = torch.from_numpy(np.ascontiguousarray(loc[s3:2 * s3]) * geo.sign_send_down)
+from_down, from_up = torch.empty_like(top), torch.empty_like(top)
+comm.exchange_wait(comm.exchange_start(top, bot, from_down, from_up))
+sign_b = -1.0 if rank == 0 else 1.0                   # my bottom ghost crossed the global boundary
+sign_t = -1.0 if rank == world - 1 else 1.0
+assert np.array_equal(from_down.numpy(), sign_b * loc[:s3]), "bottom ghost"
+assert np.array_equal(from_up.numpy(), sign_t * loc[-s3:]), "top ghost"
+t = torch.tensor([1.5 + rank, -2.0], dtype=torch.float64)
+comm.allreduce_sum(t)
+assert t.tolist() == [4.0, -4.0], t
+dist.barrier()
+dist.destroy_process_group()
+print("rank", rank, "ok")
+"""
+
+
+def test_slab_exchange_gloo_world2(tmp_path):
+    script = tmp_path / "w.py"
+    script.write_text(_WORKER % ROOT)
+    port = 29950 + os.getpid() % 40
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE="2",
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.STDOUT, text=True))
+    outs = [p.communicate(timeout=180)[0] for p in procs]
+    for r, (p, o) in enumerate(zip(procs, outs)):
+        assert p.returncode == 0, o
+        assert f"rank {r} ok" in o
