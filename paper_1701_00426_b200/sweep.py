@@ -3,6 +3,7 @@
     python -m paper_1701_00426_b200.sweep --ladder            # config 5: ns/site, GB/s vs volume
     python -m paper_1701_00426_b200.sweep --multishift        # config 4: 24^3x48 and 32^4 solves
     python -m paper_1701_00426_b200.sweep --dims 16,16,16,16 --ladder
+    python -m paper_1701_00426_b200.sweep --slab              # NEXT-2: slab path (torchrun for N > 1)
 
 Prints one JSON line per measurement and, with --md FILE, appends a Markdown table.  Timing is by
 CUDA events on the launching stream after warm-up.  Volumes whose links fit the 126 MB L2 are
@@ -127,10 +128,66 @@ def multishift(dims_list, out):
         lat.close()
 
 
+def slab(dims_list, out):
+    """Strong-scaling Dslash / multi-shift CG of ONE lattice split into x3 slabs, one per rank
+    (torchrun + NCCL for WORLD_SIZE > 1; alone it measures the slab path's own overhead: self-exchange
+    of the two faces and three launches per Dslash instead of one)."""
+    import numpy as np
+    import torch
+    import lqcd_inputs as gen
+    from paper_1701_00426_b200 import dist as D
+    from paper_1701_00426_b200.slab import SlabLattice
+
+    rank, local_rank, world = D.init("nccl")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    for dims in dims_list:
+        rng = np.random.default_rng(3)
+        U = gen.smooth_links(dims, 0.3, rng)
+        ie, io = gen.gaussian_half_spinor(dims, rng), gen.gaussian_half_spinor(dims, rng)
+        V = gen.volume(dims)
+        sl = SlabLattice(dims, world, rank, device=local_rank)
+        links = sl.pack_links(U)
+        a, b = sl.pack_spinor(ie, 0), sl.pack_spinor(io, 1)
+        oo, oe = sl.new_spinor(), sl.new_spinor()
+        for overlap in (True, False):
+            def step():
+                sl.dslash(1, oo, a, links, overlap=overlap)
+                sl.dslash(0, oe, b, links, overlap=overlap)
+            D.barrier(world)
+            us = D.max_over_ranks(ev_time_us(torch, step, 200, 10) / 2, world, device)
+            if rank == 0:
+                out(dict(kind="slab_dslash", dims="x".join(map(str, dims)), world=world, overlap=overlap,
+                         us=round(us, 2), ns_per_site=round(us * 1e3 / (V // 2), 4),
+                         GBs_aggregate=round(1248 * (V // 2) / us / 1e3, 1)))
+        shifts = gen.rhmc_shifts(8)
+        xs = [sl.new_spinor() for _ in shifts]
+
+        def solve(n):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            sl.cg_multishift(xs, a, links, 0.0025, shifts, 1e-300, n, raise_on_max_iter=False)
+            e1.record()
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1)
+        solve(16)
+        t_lo, t_hi = min(solve(16), solve(16)), min(solve(80), solve(80))
+        it_us = D.max_over_ranks((t_hi - t_lo) / 64 * 1e3, world, device)
+        if rank == 0:
+            out(dict(kind="slab_multishift8", dims="x".join(map(str, dims)), world=world,
+                     us_per_iter=round(it_us, 2), iter_per_s=round(1e6 / it_us, 1),
+                     note="host-driven hooks: 2 halo exchanges + 2 all-reduces per iteration"))
+        sl.close()
+    D.barrier(world)
+    D.finalize(world)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--ladder", action="store_true")
     ap.add_argument("--multishift", action="store_true")
+    ap.add_argument("--slab", action="store_true", help="x3-slab path (run under torchrun for more than one GPU)")
     ap.add_argument("--dims", default=None, help="comma-separated N0,N1,N2,N3 (repeatable with ';')")
     ap.add_argument("--eps", type=float, default=0.5)
     ap.add_argument("--seed", type=int, default=5)
@@ -149,9 +206,11 @@ def main():
         ladder(dims_list or LADDER, args.eps, args.seed, out)
     if args.multishift:
         multishift(dims_list or [(24, 24, 24, 48), (32, 32, 32, 32)], out)
+    if args.slab:
+        slab(dims_list or [(32, 32, 32, 32)], out)
     if args.md:
         with open(args.md, "a") as f:
-            for kind in ("dslash", "cg", "multishift_solve"):
+            for kind in ("dslash", "cg", "multishift_solve", "slab_dslash", "slab_multishift8"):
                 sel = [r for r in rows if r["kind"] == kind]
                 if not sel:
                     continue
