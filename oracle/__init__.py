@@ -14,6 +14,7 @@ from .oracle import (  # noqa: F401
     cg,
     cg_multishift,
     rational_apply,
+    fermion_force,
     half_to_full,
     full_to_half,
     num_threads,

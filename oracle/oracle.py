@@ -45,6 +45,8 @@ _lib.oracle_cg_multishift.restype = C.c_int
 _lib.oracle_rational_apply.argtypes = [_i4, C.c_int, _c128, C.c_double, C.c_int, _pd, C.c_double, _pd, _c128, _c128,
                                        C.c_double, C.c_int, _pi, _pi]
 _lib.oracle_rational_apply.restype = C.c_int
+_lib.oracle_fermion_force.argtypes = [_i4, C.c_int, _c128, C.c_int, _pd, _c128, _c128]
+_lib.oracle_fermion_force.restype = C.c_int
 _lib.oracle_num_threads.restype = C.c_int
 _lib.oracle_set_num_threads.argtypes = [C.c_int]
 
@@ -207,3 +209,18 @@ def rational_apply(dims, U, mass, shifts, c0, coeffs, b, tol, max_iter, antiperi
     if rc == -2:
         raise ValueError("shifts must be >= 0 and nshift >= 1")
     return dict(y=y, iters=iters.value, converged=(rc == 0), conv_iter=np.array(list(conv)))
+
+
+def fermion_force(dims, U, coeffs, xs, antiperiodic_t=True):
+    """F[V,4,3,3] = TA[U_mu(x) Q_mu(x)] from the solutions xs[nshift, V/2, 3] (even sites) and c_i."""
+    n4, V = _dims(dims)
+    coeffs = np.ascontiguousarray(coeffs, dtype=np.float64)
+    xs = np.ascontiguousarray(xs, dtype=np.complex128)
+    if xs.shape != (coeffs.size, V // 2, 3):
+        raise ValueError(f"xs must be ({coeffs.size}, {V // 2}, 3)")
+    F = np.empty((V, 4, 3, 3), dtype=np.complex128)
+    rc = _lib.oracle_fermion_force(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), coeffs.size, _dptr(coeffs),
+                                   xs.reshape(-1), F.reshape(-1))
+    if rc:
+        raise MemoryError("oracle_fermion_force")
+    return F

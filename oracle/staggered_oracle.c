@@ -24,7 +24,8 @@
  * gauge covariance; reconstructed row 3 against the generator's Gram-Schmidt row 3;
  * CG / multi-shift against dense numpy.linalg.solve; the identity
  * b - (A + sigma_i) x_i = zeta_i r; one-iteration convergence on a plane wave; the
- * rational-function sum against dense solves and a partial-fraction identity.
+ * rational-function sum against dense solves and a partial-fraction identity; the fermion-force
+ * outer products against finite differences of the action computed with dense solves.
  * No function in this file is "parity unpinned".
  *
  * OpenMP is used on the site loop of the operator only, so that bench.py can time the
@@ -456,6 +457,77 @@ int oracle_rational_apply(const int N[4], int antiperiodic_t, const cplx *U, dou
     }
     free(x);
     return rc;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Fermion-force outer products ("the fermion force
+ * calculation step ... a large fraction of the execution time is spent in ... deo and doe").
+ * The paper gives no formula (it follows its ref. 33); reading R21 of DESIGN.md derives it:
+ *
+ *   S = phi^dagger r(A) phi,  r(A) = c0 + sum_i c_i (A + sigma_i)^-1,  A = m^2 - D_eo D_oe  (Eq. 3, 6, 8)
+ *   x_i = (A + sigma_i)^-1 phi (even sites),  y_i = D_oe x_i (odd sites),
+ *   w_i = x_i on even sites, y_i on odd sites.
+ *   Under U_mu(x) -> exp(i eps T) U_mu(x)  (T Hermitian traceless):
+ *       dS/d eps = 2 Re Tr[ i T F_mu(x) ],
+ *   F_mu(x) = TA[ U_mu(x) Q_mu(x) ],
+ *   Q_mu(x) = 1/2 eta_mu(x) s+_mu(x) (-1)^{p(x)} sum_i c_i  w_i(x+mu) w_i(x)^dagger      (3x3 outer product)
+ *   TA[M]   = (M - M^dagger)/2 - Tr(M - M^dagger)/6                     (traceless anti-Hermitian part)
+ * (both places where U_mu(x) enters D -- the forward hop out of x and the backward hop out of
+ * x+mu -- are included; they are complex conjugates of each other, hence the "2 Re").
+ * Pin: central finite differences of S computed with DENSE numpy solves, for random links,
+ * directions and generators, both parities, across the antiperiodic boundary, and N_mu = 2.
+ *
+ * x: nshift even half vectors, contiguous.  F: [V][4][3][3], row-major.  Returns 0, or -1.
+ * ------------------------------------------------------------------------------------- */
+int oracle_fermion_force(const int N[4], int antiperiodic_t, const cplx *U, int nshift,
+                         const double *c, const cplx *x, cplx *F)
+{
+    size_t V = vol(N), nh = V / 2 * 3;
+    cplx *w = (cplx *)malloc(V * 3 * (size_t)nshift * sizeof(cplx));
+    cplx *y = (cplx *)malloc(nh * sizeof(cplx));
+    cplx *full = (cplx *)malloc(V * 3 * sizeof(cplx));
+    if (!w || !y || !full) { free(w); free(y); free(full); return -1; }
+    for (int i = 0; i < nshift; ++i) {
+        cplx *wi = w + (size_t)i * V * 3;
+        if (oracle_dslash_half(N, antiperiodic_t, U, 1, x + (size_t)i * nh, y)) { free(w); free(y); free(full); return -1; }
+        oracle_half_to_full(N, 0, x + (size_t)i * nh, wi);        /* even sites: x_i, odd: 0 */
+        oracle_half_to_full(N, 1, y, full);                        /* odd sites: y_i, even: 0 */
+        for (size_t j = 0; j < V * 3; ++j) wi[j] += full[j];
+    }
+    for (size_t lex = 0; lex < V; ++lex) {
+        int xc[4];
+        coords_of(N, lex, xc);
+        double sp = parity_of(xc) ? -1.0 : 1.0;
+        for (int mu = 0; mu < 4; ++mu) {
+            int xf[4] = { xc[0], xc[1], xc[2], xc[3] };
+            xf[mu] = (xc[mu] + 1) % N[mu];
+            size_t lf = lex_of(N, xf);
+            double e = 0.5 * eta(mu, xc) * sp;
+            if (antiperiodic_t && mu == 3 && xc[3] == N[3] - 1) e = -e;
+            cplx Q[3][3], M[3][3];
+            for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) Q[a][b] = 0.0;
+            for (int i = 0; i < nshift; ++i) {
+                const cplx *wi = w + (size_t)i * V * 3;
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b) Q[a][b] += c[i] * wi[lf * 3 + a] * conj(wi[lex * 3 + b]);
+            }
+            const cplx *u = U + (lex * 4 + (size_t)mu) * 9;
+            for (int a = 0; a < 3; ++a)
+                for (int b = 0; b < 3; ++b) {
+                    cplx t = 0.0;
+                    for (int k = 0; k < 3; ++k) t += u[a * 3 + k] * (e * Q[k][b]);
+                    M[a][b] = t;
+                }
+            cplx tr = 0.0;
+            for (int a = 0; a < 3; ++a) tr += M[a][a] - conj(M[a][a]);
+            cplx *f = F + (lex * 4 + (size_t)mu) * 9;
+            for (int a = 0; a < 3; ++a)
+                for (int b = 0; b < 3; ++b)
+                    f[a * 3 + b] = 0.5 * (M[a][b] - conj(M[b][a])) - (a == b ? tr / 6.0 : 0.0);
+        }
+    }
+    free(w); free(y); free(full);
+    return 0;
 }
 
 /* Number of OpenMP threads the site loop uses (for bench.py's "cores" field). */

@@ -375,6 +375,70 @@ def test_rational_apply_against_dense_partial_fractions_and_plane_wave():
     assert rel(r["y"], (c0 + np.sum(c / (lam + shifts))) * phi) < 1e-12
 
 
+def _gell_mann():
+    l = np.zeros((8, 3, 3), dtype=np.complex128)
+    l[0][0, 1] = l[0][1, 0] = 1
+    l[1][0, 1], l[1][1, 0] = -1j, 1j
+    l[2][0, 0], l[2][1, 1] = 1, -1
+    l[3][0, 2] = l[3][2, 0] = 1
+    l[4][0, 2], l[4][2, 0] = -1j, 1j
+    l[5][1, 2] = l[5][2, 1] = 1
+    l[6][1, 2], l[6][2, 1] = -1j, 1j
+    l[7] = np.diag([1, 1, -2]) / np.sqrt(3)
+    return l
+
+
+def _expm_herm(H, eps):
+    w, v = np.linalg.eigh(H)
+    return (v * np.exp(1j * eps * w)) @ v.conj().T
+
+
+@pytest.mark.parametrize("dims,ap", [((2, 2, 2, 4), True), ((4, 2, 2, 2), True), ((2, 4, 2, 2), False)])
+def test_fermion_force_against_finite_differences_of_the_action(dims, ap):
+    """NEXT-3 (reading R21): dS/d eps under U_mu(x) -> exp(i eps T_a) U_mu(x) equals 2 Re Tr[i T_a F_mu(x)],
+    with S = sum_i c_i Re phi^dag (A+sigma_i)^-1 phi evaluated by DENSE solves (no oracle code in S).
+    Links on both parities, all four directions, across the antiperiodic boundary and with N_mu = 2
+    (where x+mu = x-mu); catches a wrong sign, parity factor, conjugation, dropped 1/2 or eta."""
+    rng = np.random.default_rng(12)
+    U = gen.haar_like_links(dims, rng)
+    phi = gen.gaussian_half_spinor(dims, rng)
+    m = 0.4
+    shifts = np.array([0.05, 0.7, 0.2])
+    c = np.array([0.8, -0.45, 1.3])
+    V = gen.volume(dims)
+
+    def action(Uv):
+        A, _, _ = dense_normal_operator(dims, Uv, m, antiperiodic_t=ap)
+        eye = np.eye(A.shape[0])
+        b = phi.reshape(-1)
+        return sum(ci * np.real(np.vdot(b, np.linalg.solve(A + s * eye, b))) for ci, s in zip(c, shifts))
+
+    A, _, _ = dense_normal_operator(dims, U, m, antiperiodic_t=ap)
+    eye = np.eye(A.shape[0])
+    xs = np.stack([np.linalg.solve(A + s * eye, phi.reshape(-1)).reshape(-1, 3) for s in shifts])
+    F = oracle.fermion_force(dims, U, c, xs, antiperiodic_t=ap)
+    # F is traceless anti-Hermitian
+    assert np.abs(F + F.conj().transpose(0, 1, 3, 2)).max() < 1e-14
+    assert np.abs(np.trace(F, axis1=2, axis2=3)).max() < 1e-14
+    lam = _gell_mann()
+    coords = gen.site_coords(dims)
+    eps = 1e-5
+    # sites chosen to include both parities and the last x3 slice (boundary-crossing forward hop)
+    picks = [0, 1, V - 1, V - 2, V // 2 + 1]
+    worst = 0.0
+    for k, lex in enumerate(picks):
+        for mu in range(4):
+            a = (3 * k + mu) % 8
+            Up, Um = U.copy(), U.copy()
+            Up[lex, mu] = _expm_herm(lam[a], eps) @ U[lex, mu]
+            Um[lex, mu] = _expm_herm(lam[a], -eps) @ U[lex, mu]
+            fd = (action(Up) - action(Um)) / (2 * eps)
+            an = 2 * np.real(np.trace(1j * lam[a] @ F[lex, mu]))
+            worst = max(worst, abs(fd - an) / max(1e-3, abs(an)))
+    assert worst < 1e-6, worst
+    assert {int(coords[p].sum() % 2) for p in picks} == {0, 1}
+
+
 def test_multishift_rejects_bad_shifts():
     dims = (2, 2, 2, 2)
     U = gen.unit_links(dims)
