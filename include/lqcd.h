@@ -167,6 +167,28 @@ int lqcd_rational_apply(lqcd_ctx *ctx, int nshift, const double *shifts, double 
                         double mass, double tol, int max_iter, int *iters, int *conv_iter);
 
 /*
+ * Fermion-force outer products (the step after the
+ * multi-shift solve).  The paper prints no formula (it follows its ref. 33); reading R21 of DESIGN.md:
+ * for S = phi^dagger [c0 + sum_i c_i (A + sigma_i)^-1] phi, A = mass^2 - D_eo D_oe (Eq. 3, 6, 8), with
+ * x_i = (A + sigma_i)^-1 phi on even sites, y_i = D_oe x_i on odd sites and w_i = x_i | y_i by parity,
+ *     F_mu(x) = TA[ U_mu(x) Q_mu(x) ],
+ *     Q_mu(x) = 1/2 eta_mu(x) s+_mu(x) (-1)^{p(x)} sum_i c_i w_i(x+mu) w_i(x)^dagger,
+ *     TA[M]   = (M - M^dagger)/2 - Tr(M - M^dagger)/6,
+ * so that dS/d eps = 2 Re Tr[ i T F_mu(x) ] under U_mu(x) -> exp(i eps T) U_mu(x).
+ *   coeffs   host, nshift doubles (the c_i; c0 does not enter the force)
+ *   xs_e     host array of nshift device pointers: the solutions x_i (native even-site vectors, e.g.
+ *            from lqcd_cg_multishift); read only
+ *   force    native force field (device, lqcd_force_bytes; out): 3x3 complex per link, layout private
+ * The y_i are computed inside (nshift Dslash applications into the workspace of
+ * lqcd_workspace_bytes(ctx, nshift)).  async.  LQCD_ERR_UNSUPPORTED in slab mode.
+ */
+size_t lqcd_force_bytes(const lqcd_ctx *ctx);
+int lqcd_fermion_force(lqcd_ctx *ctx, int nshift, const double *coeffs, void *const *xs_e,
+                       const void *links, void *force);
+/* native force field -> canonical complex128 F[lex][mu][row][col] (device).  async. */
+int lqcd_unpack_force(lqcd_ctx *ctx, void *canonical_dev /* c128 [V][4][3][3] */, const void *native);
+
+/*
  * ---- Slab mode: one x3 slab per GPU (the paper leaves the
  * multi-device version as future work) --------------------------------------
  * A rank that owns L3 = N3/P time slices creates its context with dims (N0,N1,N2,L3+2) and

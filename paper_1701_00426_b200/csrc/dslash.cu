@@ -15,41 +15,7 @@
 // The kernel is bound by HBM bandwidth (1248 B/site fp64 18-real vs 570 flop/site): no tensor cores.
 #include "reduce.cuh"
 
-template <typename T> struct Su3 { Cx<T> e[3][3]; };
-
-template <typename T, int LAYOUT, int RECON12, int POLICY>
-__device__ __forceinline__ Su3<T> load_link(const T *__restrict__ links, int par, int mu, size_t Vh, size_t i, const L2Pol &pol)
-{
-    constexpr int R = RECON12 ? 2 : 3;
-    Su3<T> u;
-    size_t plane0 = (size_t)(par * 4 + mu) * (R * 3);
-#pragma unroll
-    for (int r = 0; r < R; ++r)
-#pragma unroll
-        for (int c = 0; c < 3; ++c) u.e[r][c] = ld_cx<T, LAYOUT, 1, POLICY>(links, plane0 + r * 3 + c, Vh, i, pol);
-    if (RECON12) {
-        // r2[k] = conj( eps_kij r0[i] r1[j] )   (reading R8)
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const int a = (k + 1) % 3, b = (k + 2) % 3;
-            Cx<T> x = u.e[0][a], y = u.e[1][b], z = u.e[0][b], w = u.e[1][a];
-            T re = x.re * y.re - x.im * y.im - (z.re * w.re - z.im * w.im);
-            T im = x.re * y.im + x.im * y.re - (z.re * w.im + z.im * w.re);
-            u.e[2][k] = cx<T>(re, -im);
-        }
-    }
-    return u;
-}
-
-template <typename T, int LAYOUT, int POLICY>
-__device__ __forceinline__ void load_vec(const T *__restrict__ v, size_t Vh, size_t i, T coef, Cx<T> p[3], const L2Pol &pol)
-{
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        Cx<T> z = ld_cx<T, LAYOUT, 0, POLICY>(v, (size_t)c, Vh, i, pol);
-        p[c] = cx<T>(coef * z.re, coef * z.im);
-    }
-}
+#include "su3.cuh"
 
 // acc += U p
 template <typename T> __device__ __forceinline__ void mv_acc(Cx<T> acc[3], const Su3<T> &u, const Cx<T> p[3])

@@ -1,0 +1,198 @@
+// force.cu -- fermion-force outer products (the step after
+// the multi-shift solve, "a large fraction of the execution time is spent in ... deo and doe").
+// The paper gives no formula (it follows its ref. 33); reading R21 of DESIGN.md:
+//
+//   S = phi^dagger r(A) phi,  r(A) = c0 + sum_i c_i (A + sigma_i)^-1,  A = m^2 - D_eo D_oe   (Eq. 3, 6, 8)
+//   x_i = (A + sigma_i)^-1 phi (even sites), y_i = D_oe x_i (odd sites), w_i = x_i | y_i by parity
+//   F_mu(x) = TA[ U_mu(x) Q_mu(x) ],   dS/d eps = 2 Re Tr[i T F_mu(x)]  for U_mu(x) -> exp(i eps T) U_mu(x)
+//   Q_mu(x) = 1/2 eta_mu(x) s+_mu(x) (-1)^{p(x)} sum_i c_i w_i(x+mu) w_i(x)^dagger
+//   TA[M]   = (M - M^dagger)/2 - Tr(M - M^dagger)/6
+//
+// One thread per site, the four directions in turn: per direction the n outer products are
+// accumulated in registers (the site's own n vectors are re-read from L1 for each direction), then
+// U_mu(x) is streamed in once, multiplied, projected and the 3x3 result stored.  HBM-bound like the
+// Dslash: per full-lattice site 576 B of links + 48 n B of vectors (each w_i once; the 4 neighbour
+// reads hit L1/L2) + 576 B of force written; the n Dslash applications that produce the y_i come on top.
+#include "su3.cuh"
+
+void *ws_vec(lqcd_ctx *ctx, int k);   // api.cu
+
+struct ForceVecs {
+    const void *self[LQCD_MAX_SHIFTS];   // w_i on the sites of the launch's parity
+    const void *nbr[LQCD_MAX_SHIFTS];    // w_i on the other parity
+    double coef[LQCD_MAX_SHIFTS];        // c_i (-1)^parity
+    int n;
+};
+
+template <typename T, int LAYOUT, int RECON12>
+__global__ void __launch_bounds__(128) force_kernel(const Geom g, const int parity, T *__restrict__ force,
+                                                    const T *__restrict__ links, const ForceVecs fv)
+{
+    pdl_wait();
+    pdl_trigger();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.Vh) return;
+    const size_t Vh = (size_t)g.Vh;
+    const L2Pol pol = {0, 0};
+    // site decode and forward neighbours as in dslash.cu (Eq. 9)
+    uint32_t t = fd_div((uint32_t)i, g.dNh0);
+    const int hx0 = i - (int)t * g.Nh0;
+    uint32_t t2 = fd_div(t, g.dN1);
+    const int x1 = (int)t - (int)t2 * g.N1;
+    const int x3 = (int)fd_div(t2, g.dN2);
+    const int x2 = (int)t2 - x3 * g.N2;
+    const int rp = (x1 + x2 + x3 + parity) & 1;
+    int nf[4];
+    nf[0] = rp ? (hx0 + 1 == g.Nh0 ? i - (g.Nh0 - 1) : i + 1) : i;
+    nf[1] = x1 + 1 == g.N1 ? i - (g.N1 - 1) * g.s1 : i + g.s1;
+    nf[2] = x2 + 1 == g.N2 ? i - (g.N2 - 1) * g.s2 : i + g.s2;
+    nf[3] = x3 + 1 == g.N3 ? i - (g.N3 - 1) * g.s3 : i + g.s3;
+    T e[4];
+    const T h = (T)0.5;
+    e[0] = h;
+    e[1] = rp ? -h : h;
+    e[2] = ((rp + x1) & 1) ? -h : h;
+    e[3] = ((rp + x1 + x2) & 1) ? -h : h;
+    if (g.ap && x3 == g.N3 - 1) e[3] = -e[3];
+
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        Cx<T> Q[3][3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) Q[a][b] = cx<T>((T)0, (T)0);
+        for (int s = 0; s < fv.n; ++s) {
+            Cx<T> ws[3], wn[3];
+            load_vec<T, LAYOUT, 0>((const T *)fv.self[s], Vh, (size_t)i, (T)1, ws, pol);
+            load_vec<T, LAYOUT, 0>((const T *)fv.nbr[s], Vh, (size_t)nf[mu], (T)fv.coef[s], wn, pol);
+            // Q[a][b] += c w(x+mu)[a] conj(w(x)[b])
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = 0; b < 3; ++b) {
+                    Q[a][b].re = fma(wn[a].re, ws[b].re, Q[a][b].re);
+                    Q[a][b].re = fma(wn[a].im, ws[b].im, Q[a][b].re);
+                    Q[a][b].im = fma(wn[a].im, ws[b].re, Q[a][b].im);
+                    Q[a][b].im = fma(-wn[a].re, ws[b].im, Q[a][b].im);
+                }
+        }
+        const Su3<T> u = load_link<T, LAYOUT, RECON12, 0>(links, parity, mu, (size_t)g.Ls, (size_t)i, pol);
+        Cx<T> M[3][3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                T re = 0, im = 0;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    re = fma(u.e[a][k].re, Q[k][b].re, re);
+                    re = fma(-u.e[a][k].im, Q[k][b].im, re);
+                    im = fma(u.e[a][k].re, Q[k][b].im, im);
+                    im = fma(u.e[a][k].im, Q[k][b].re, im);
+                }
+                M[a][b] = cx<T>(e[mu] * re, e[mu] * im);
+            }
+        // TA[M]: Tr(M - M^dagger) = 2 i sum_a Im M_aa
+        const T tr3 = (M[0][0].im + M[1][1].im + M[2][2].im) / (T)3;
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                Cx<T> f = cx<T>((T)0.5 * (M[a][b].re - M[b][a].re), (T)0.5 * (M[a][b].im + M[b][a].im));
+                if (a == b) f.im -= tr3;
+                st_cx<T, LAYOUT, 0>(force, (size_t)((parity * 4 + mu) * 9 + a * 3 + b), Vh, (size_t)i, f, pol);
+            }
+    }
+}
+
+// native force field (planes ((parity*4 + mu)*3 + row)*3 + col of Vh sites) -> canonical c128 [V][4][3][3]
+template <typename T, int LAYOUT>
+__global__ void unpack_force_kernel(Geom g, double2 *__restrict__ canon, const T *__restrict__ native)
+{
+    pdl_wait();
+    pdl_trigger();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int par = blockIdx.y;
+    if (i >= g.Vh) return;
+    uint32_t t = fd_div((uint32_t)i, g.dNh0);
+    uint32_t t2 = fd_div(t, g.dN1);
+    const int x1 = (int)t - (int)t2 * g.N1;
+    const int x3 = (int)fd_div(t2, g.dN2);
+    const int x2 = (int)t2 - x3 * g.N2;
+    const size_t lex = 2 * (size_t)i + ((x1 + x2 + x3 + par) & 1);
+    for (int mu = 0; mu < 4; ++mu)
+        for (int k = 0; k < 9; ++k) {
+            Cx<T> z = ld_cx<T, LAYOUT, 0, 0>(native, (size_t)((par * 4 + mu) * 9 + k), (size_t)g.Vh, (size_t)i, L2Pol());
+            canon[(lex * 4 + mu) * 9 + k] = make_double2((double)z.re, (double)z.im);
+        }
+}
+
+extern "C" size_t lqcd_force_bytes(const lqcd_ctx *ctx)
+{
+    return ctx ? (size_t)ctx->g.Vh * 2 * 4 * 9 * 2 * elem_size(ctx) : 0;
+}
+
+template <typename T, int LAYOUT>
+static void launch_force_tl(lqcd_ctx *ctx, int parity, void *force, const void *links, const ForceVecs &fv)
+{
+    dim3 grid((ctx->g.Vh + 127) / 128), block(128);
+    if (ctx->recon == LQCD_RECON_12) launch_k(ctx, force_kernel<T, LAYOUT, 1>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv);
+    else launch_k(ctx, force_kernel<T, LAYOUT, 0>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv);
+}
+
+extern "C" int lqcd_fermion_force(lqcd_ctx *ctx, int nshift, const double *coeffs, void *const *xs_e,
+                                  const void *links, void *force)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    int rc = lqcd_check_cuda(ctx, cudaSetDevice(ctx->device), "cudaSetDevice");
+    if (rc) return rc;
+    if (nshift < 1 || nshift > LQCD_MAX_SHIFTS) return lqcd_fail(ctx, LQCD_ERR_ARG, "nshift %d not in [1,%d]", nshift, LQCD_MAX_SHIFTS);
+    if (!coeffs || !xs_e || !links || !force) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_fermion_force: null pointer");
+    for (int i = 0; i < nshift; ++i) {
+        if (!xs_e[i]) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_fermion_force: solution %d is null", i);
+        if (coeffs[i] != coeffs[i]) return lqcd_fail(ctx, LQCD_ERR_ARG, "coefficient %d is NaN", i);
+    }
+    if (ctx->halo_fn || ctx->x3_lo != 0 || ctx->x3_hi != ctx->g.N3)
+        return lqcd_fail(ctx, LQCD_ERR_UNSUPPORTED, "lqcd_fermion_force: not available in slab mode");
+    if (!ctx->ws) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "no workspace set");
+    if (ctx->ws_bytes < lqcd_workspace_bytes(ctx, nshift))
+        return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "workspace %zu bytes < %zu needed for %d shifts", ctx->ws_bytes, lqcd_workspace_bytes(ctx, nshift), nshift);
+    // y_i = D_oe x_i into the workspace slots the solver uses for its p_i
+    ForceVecs ev, od;
+    memset(&ev, 0, sizeof(ev));
+    memset(&od, 0, sizeof(od));
+    ev.n = od.n = nshift;
+    for (int i = 0; i < nshift; ++i) {
+        void *y = ws_vec(ctx, 4 + i);
+        if ((rc = launch_dslash(ctx, LQCD_ODD, y, xs_e[i], links, NULL, 0.0, 0, 0))) return rc;
+        ev.self[i] = xs_e[i]; ev.nbr[i] = y; ev.coef[i] = coeffs[i];        // x even: + c_i y_i(x+mu) x_i(x)^dagger
+        od.self[i] = y; od.nbr[i] = xs_e[i]; od.coef[i] = -coeffs[i];       // x odd:  - c_i x_i(x+mu) y_i(x)^dagger
+    }
+    for (int par = 0; par < 2; ++par) {
+        const ForceVecs &fv = par ? od : ev;
+        if (ctx->prec == LQCD_F64) {
+            if (ctx->layout == 0) launch_force_tl<double, 0>(ctx, par, force, links, fv); else launch_force_tl<double, 1>(ctx, par, force, links, fv);
+        } else {
+            if (ctx->layout == 0) launch_force_tl<float, 0>(ctx, par, force, links, fv); else launch_force_tl<float, 1>(ctx, par, force, links, fv);
+        }
+    }
+    return lqcd_check_cuda(ctx, cudaGetLastError(), "fermion force");
+}
+
+extern "C" int lqcd_unpack_force(lqcd_ctx *ctx, void *canonical_dev, const void *native)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    int rc = lqcd_check_cuda(ctx, cudaSetDevice(ctx->device), "cudaSetDevice");
+    if (rc) return rc;
+    if (!canonical_dev || !native) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_unpack_force: null pointer");
+    dim3 grid((ctx->g.Vh + 127) / 128, 2), block(128);
+    if (ctx->prec == LQCD_F64) {
+        if (ctx->layout == 0) launch_k(ctx, unpack_force_kernel<double, 0>, grid, block, ctx->g, (double2 *)canonical_dev, (const double *)native);
+        else launch_k(ctx, unpack_force_kernel<double, 1>, grid, block, ctx->g, (double2 *)canonical_dev, (const double *)native);
+    } else {
+        if (ctx->layout == 0) launch_k(ctx, unpack_force_kernel<float, 0>, grid, block, ctx->g, (double2 *)canonical_dev, (const float *)native);
+        else launch_k(ctx, unpack_force_kernel<float, 1>, grid, block, ctx->g, (double2 *)canonical_dev, (const float *)native);
+    }
+    return lqcd_check_cuda(ctx, cudaGetLastError(), "unpack_force");
+}

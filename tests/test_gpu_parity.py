@@ -316,6 +316,56 @@ def test_rational_apply(prec):
     lat.close()
 
 
+@pytest.mark.parametrize("recon", [0, 1])
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (2, 2, 2, 4), (6, 4, 10, 8)])
+def test_fermion_force(dims, prec, recon):
+    """NEXT-3 (lqcd_fermion_force): F_mu(x) = TA[U_mu(x) Q_mu(x)] from given solutions x_i, element by
+    element against the oracle (whose formula is pinned by finite differences of the action).  The x_i
+    are arbitrary Gaussian vectors here: the map (x_i, c_i, U) -> F is what is under test."""
+    rng = np.random.default_rng(9)
+    U = gen.haar_like_links(dims, rng)
+    n = 3
+    xs = np.stack([gen.gaussian_half_spinor(dims, rng) for _ in range(n)])
+    U, xs = round_inputs(prec, U, xs)
+    if recon == 1 and prec == 1:
+        U = oracle.reconstruct_row3(U)
+    c = np.array([0.8, -0.45, 1.3])
+    want = oracle.fermion_force(dims, U, c, xs)
+    lat = make_lattice(dims, prec, recon)
+    links = lat.pack_links(U)
+    dx = [lat.pack_spinor(x, 0) for x in xs]
+    got = lat.unpack_force(lat.fermion_force(dx, links, c))
+    assert rel(got, want) < TOL[prec], (dims, prec, recon, rel(got, want))
+    # per-link check as well (a wrong sign on one parity or direction would hide in a global norm less
+    # than one would like): worst link relative to the typical link norm
+    link_err = np.linalg.norm((got - want).reshape(-1, 9), axis=1).max()
+    assert link_err / np.linalg.norm(want.reshape(-1, 9), axis=1).mean() < 10 * TOL[prec]
+    assert np.abs(got + got.conj().transpose(0, 1, 3, 2)).max() < (1e-12 if prec == 0 else 1e-4)
+    lat.close()
+
+
+def test_fermion_force_after_solve_periodic_bc():
+    """End to end: multi-shift solve on the GPU, force from its solutions; oracle force from the oracle's
+    solutions (periodic BC variant, 12x10x6x4 spans several CTAs with a ragged tail)."""
+    dims = (12, 10, 6, 4)
+    rng = np.random.default_rng(10)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m, tol = 0.1, 1e-11
+    shifts = gen.rhmc_shifts(4)
+    c = np.array([0.5, -1.25, 2.0, 0.125])
+    ref = oracle.cg_multishift(dims, U, m, shifts, b, tol, 5000, antiperiodic_t=False)
+    want = oracle.fermion_force(dims, U, c, ref["x"], antiperiodic_t=False)
+    lat = make_lattice(dims, ap=False)
+    links, be = lat.pack_links(U), lat.pack_spinor(b, 0)
+    xs = [lat.new_spinor() for _ in shifts]
+    lat.cg_multishift(xs, be, links, m, shifts, tol, 5000)
+    got = lat.unpack_force(lat.fermion_force(xs, links, c))
+    assert rel(got, want) < 1e-7          # solutions agree to O(kappa tol), the force is bilinear in them
+    lat.close()
+
+
 def test_cg_fp32_and_max_iter():
     dims = (8, 8, 8, 8)
     rng = np.random.default_rng(5)
