@@ -308,6 +308,16 @@ def run_ours(args):
         extra["rational8_f64"] = {"iter_per_s": 1e3 / ms_it, "us_per_iter": ms_it * 1e3, "bytes_per_site_iter": by,
                                   "GBs": by * Vh / (ms_it * 1e-3) / 1e9, "frac": by * Vh / (ms_it * 1e-3) / 1e9 / peak,
                                   "note": "lqcd_rational_apply, 8 shifts all active: y += c_i alpha_i p_i fused, x_i never stored"}
+        # ---- NEXT-3: fermion-force outer products from 8 solutions (n Dslash + 2 outer-product launches)
+        xs8 = [lat.new_spinor() for _ in shifts]
+        lat.cg_multishift(xs8, d_in_e, links, 0.0025, shifts, 1e-300, 8, raise_on_max_iter=False)
+        fbuf = lat.fermion_force(xs8, links, [1.0] * 8)
+        t_f = timed_loop(torch, lambda: lat.fermion_force(xs8, links, [1.0] * 8, force=fbuf), 20, 3, 1, D, device) / 20
+        by = 8 * 1248 * Vh + V * (576 + 48 * 8 + 576)
+        extra["fermion_force8_f64"] = {"ms": t_f, "ns_per_site": t_f * 1e6 / V, "bytes": by, "GBs": by / (t_f * 1e-3) / 1e9,
+                                       "frac": by / (t_f * 1e-3) / 1e9 / peak,
+                                       "note": "8 x D_oe (1248 B per odd site) + outer products (576 links + 48*8 vectors + 576 force B per site)"}
+        del xs8, fbuf
         # ---- CPU oracle beside it -------------------------------------------------------------
         psi = np.zeros((V, 3), dtype=np.complex128)
         psi[gen.half_index_of_parity(DIMS, 0)] = in_e

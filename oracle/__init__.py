@@ -15,6 +15,8 @@ from .oracle import (  # noqa: F401
     cg_multishift,
     rational_apply,
     fermion_force,
+    gauge_staples,
+    SYMANZIK_C0, SYMANZIK_C1,
     half_to_full,
     full_to_half,
     num_threads,

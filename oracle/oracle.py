@@ -47,6 +47,8 @@ _lib.oracle_rational_apply.argtypes = [_i4, C.c_int, _c128, C.c_double, C.c_int,
 _lib.oracle_rational_apply.restype = C.c_int
 _lib.oracle_fermion_force.argtypes = [_i4, C.c_int, _c128, C.c_int, _pd, _c128, _c128]
 _lib.oracle_fermion_force.restype = C.c_int
+_lib.oracle_gauge_staples.argtypes = [_i4, _c128, C.c_double, C.c_double, _c128]
+_lib.oracle_gauge_staples.restype = None
 _lib.oracle_num_threads.restype = C.c_int
 _lib.oracle_set_num_threads.argtypes = [C.c_int]
 
@@ -224,3 +226,14 @@ def fermion_force(dims, U, coeffs, xs, antiperiodic_t=True):
     if rc:
         raise MemoryError("oracle_fermion_force")
     return F
+
+
+SYMANZIK_C0, SYMANZIK_C1 = 5.0 / 3.0, -1.0 / 12.0
+
+
+def gauge_staples(dims, U, c0=SYMANZIK_C0, c1=SYMANZIK_C1):
+    """S[V,4,3,3]: staples of the tree-level Symanzik action (plaquette x c0 + 2x1 rectangles x c1)."""
+    n4, V = _dims(dims)
+    S = np.empty((V, 4, 3, 3), dtype=np.complex128)
+    _lib.oracle_gauge_staples(n4, _arr(U, (V, 4, 3, 3)), float(c0), float(c1), S.reshape(-1))
+    return S

@@ -25,7 +25,8 @@
  * CG / multi-shift against dense numpy.linalg.solve; the identity
  * b - (A + sigma_i) x_i = zeta_i r; one-iteration convergence on a plane wave; the
  * rational-function sum against dense solves and a partial-fraction identity; the fermion-force
- * outer products against finite differences of the action computed with dense solves.
+ * outer products against finite differences of the action computed with dense solves; the gauge
+ * staples against finite differences of the gauge action, a loop-counting sum rule and covariance.
  * No function in this file is "parity unpinned".
  *
  * OpenMP is used on the site loop of the operator only, so that bench.py can time the
@@ -528,6 +529,93 @@ int oracle_fermion_force(const int N[4], int antiperiodic_t, const cplx *U, int 
     }
     free(w); free(y); free(full);
     return 0;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Gauge staples of the tree-level Symanzik improved action.
+ * PAPER.md:105 names the action; PAPER.md:365 says the staples are "products of 3 and 5 SU(3)
+ * matrices representing links on C-shaped paths" (Listing 3, shows only the loop
+ * nest).  The paths and coefficients are not printed; reading R22 of DESIGN.md:
+ *
+ *   W[U] = sum_x sum_{mu<nu} { c0 Re Tr P_{mu nu}(x) + c1 [ Re Tr R_{mu nu}(x) + Re Tr R_{nu mu}(x) ] },
+ *   c0 = 5/3, c1 = -1/12   (S_g = -(beta/3) W; P the 1x1 plaquette, R_{mu nu} the 2x1 rectangle, 2 along mu)
+ *   staple S_mu(x) = sum over the loops of W through U_mu(x) of coefficient x (the remaining links,
+ *   ordered from x+mu back to x), so that  W = ... + Re Tr[ U_mu(x) S_mu(x) ] + (terms without U_mu(x)).
+ *
+ * Per nu != mu that is 2 three-link paths (plaquette, above and below) and 6 five-link paths
+ * (the link as first or second long side of a 2x1 rectangle, or as the short side of a 1x2 one;
+ * each above and below).  A path is walked from x+mu: a step +d from y multiplies by U_d(y),
+ * a step -d by U_d(y-d)^dagger.  Gauge links are periodic in all directions (no fermion phases).
+ * Pins: the finite-difference derivative of W (computed by an independent numpy routine),
+ * sum_{x,mu} Re Tr[U S] = 4 c0 sum P + 6 c1 sum R, unit links, gauge covariance.
+ * ------------------------------------------------------------------------------------- */
+static void mat_mul(const cplx *a, const cplx *b, cplx *o)
+{
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+            cplx t = 0.0;
+            for (int k = 0; k < 3; ++k) t += a[i * 3 + k] * b[k * 3 + j];
+            o[i * 3 + j] = t;
+        }
+}
+
+/* out += coef * (product of the links along `steps` starting at site y); step = +-(d+1) */
+static void add_path(const int N[4], const cplx *U, const int start[4], const int *steps, int nsteps,
+                     double coef, cplx *out)
+{
+    cplx M[9] = { 1, 0, 0, 0, 1, 0, 0, 0, 1 }, L[9], T[9];
+    int y[4] = { start[0], start[1], start[2], start[3] };
+    for (int s = 0; s < nsteps; ++s) {
+        int d = abs(steps[s]) - 1;
+        if (steps[s] > 0) {
+            const cplx *u = U + (lex_of(N, y) * 4 + (size_t)d) * 9;
+            for (int k = 0; k < 9; ++k) L[k] = u[k];
+            y[d] = (y[d] + 1) % N[d];
+        } else {
+            y[d] = (y[d] + N[d] - 1) % N[d];
+            const cplx *u = U + (lex_of(N, y) * 4 + (size_t)d) * 9;
+            for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) L[i * 3 + j] = conj(u[j * 3 + i]);
+        }
+        mat_mul(M, L, T);
+        memcpy(M, T, sizeof(M));
+    }
+    for (int k = 0; k < 9; ++k) out[k] += coef * M[k];
+}
+
+/* S: [V][4][3][3].  c0, c1 are arguments so that tests can look at the two families separately. */
+void oracle_gauge_staples(const int N[4], const cplx *U, double c0, double c1, cplx *S)
+{
+    size_t V = vol(N);
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (long long l = 0; l < (long long)V; ++l) {
+        int x[4];
+        coords_of(N, (size_t)l, x);
+        for (int mu = 0; mu < 4; ++mu) {
+            cplx *out = S + ((size_t)l * 4 + (size_t)mu) * 9;
+            for (int k = 0; k < 9; ++k) out[k] = 0.0;
+            int xm[4] = { x[0], x[1], x[2], x[3] };
+            xm[mu] = (x[mu] + 1) % N[mu];
+            int m = mu + 1;
+            for (int nu = 0; nu < 4; ++nu) {
+                if (nu == mu) continue;
+                int n = nu + 1;
+                const int pl_up[3] = { n, -m, -n }, pl_dn[3] = { -n, -m, n };
+                const int ra_up[5] = { m, n, -m, -m, -n }, ra_dn[5] = { m, -n, -m, -m, n };
+                const int rb_up[5] = { n, -m, -m, -n, m }, rb_dn[5] = { -n, -m, -m, n, m };
+                const int rc_up[5] = { n, n, -m, -n, -n }, rc_dn[5] = { -n, -n, -m, n, n };
+                add_path(N, U, xm, pl_up, 3, c0, out);
+                add_path(N, U, xm, pl_dn, 3, c0, out);
+                add_path(N, U, xm, ra_up, 5, c1, out);
+                add_path(N, U, xm, ra_dn, 5, c1, out);
+                add_path(N, U, xm, rb_up, 5, c1, out);
+                add_path(N, U, xm, rb_dn, 5, c1, out);
+                add_path(N, U, xm, rc_up, 5, c1, out);
+                add_path(N, U, xm, rc_dn, 5, c1, out);
+            }
+        }
+    }
 }
 
 /* Number of OpenMP threads the site loop uses (for bench.py's "cores" field). */

@@ -439,6 +439,84 @@ def test_fermion_force_against_finite_differences_of_the_action(dims, ap):
     assert {int(coords[p].sum() % 2) for p in picks} == {0, 1}
 
 
+def _gauge_W(dims, U, c0, c1):
+    """W = sum_x sum_{mu<nu} c0 ReTr P + c1 (ReTr R_{mu nu} + ReTr R_{nu mu}), with numpy rolls on the
+    [x3,x2,x1,x0] grid -- independent of the oracle's path walker.  Returns (W, sum ReTr P, sum ReTr R)."""
+    n0, n1, n2, n3 = dims
+    G = U.reshape(n3, n2, n1, n0, 4, 3, 3)
+
+    def sh(A, mu, k=1):                       # A(x + k mu)
+        return np.roll(A, -k, axis=3 - mu)
+
+    def dag(A):
+        return A.conj().swapaxes(-1, -2)
+
+    def retr(A):
+        return np.real(np.trace(A, axis1=-2, axis2=-1)).sum()
+
+    sp = sr = 0.0
+    for mu in range(4):
+        for nu in range(4):
+            if nu == mu:
+                continue
+            Um, Un = G[..., mu, :, :], G[..., nu, :, :]
+            if mu < nu:
+                sp += retr(Um @ sh(Un, mu) @ dag(sh(Um, nu)) @ dag(Un))
+            # R_{mu nu}: two steps along mu, one along nu (all ordered pairs mu != nu)
+            sr += retr(Um @ sh(Um, mu) @ sh(Un, mu, 2) @ dag(sh(sh(Um, mu), nu)) @ dag(sh(Um, nu)) @ dag(Un))
+    return c0 * sp + c1 * sr, sp, sr
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (2, 4, 6, 2)])
+def test_gauge_staples_finite_differences_sum_rule_unit_links_covariance(dims):
+    """NEXT-4 (reading R22).  (i) d/d eps of W under U_mu(x) -> exp(i eps T_a) U_mu(x) = Re Tr[i T_a U_mu(x) S_mu(x)]
+    -- any wrong path, ordering, dagger or coefficient fails it; (ii) sum_{x,mu} Re Tr[U S] = 4 c0 sum P +
+    6 c1 sum R (a plaquette has 4 links, a rectangle 6), for each family separately; (iii) unit links:
+    S = (6 c0 + 18 c1) 1; (iv) S'_mu(x) = g(x+mu) S_mu(x) g(x)^dagger under a gauge transformation."""
+    rng = np.random.default_rng(14)
+    U = gen.haar_like_links(dims, rng)
+    V = gen.volume(dims)
+    c0, c1 = oracle.SYMANZIK_C0, oracle.SYMANZIK_C1
+    assert (c0, c1) == (5.0 / 3.0, -1.0 / 12.0)
+    S = oracle.gauge_staples(dims, U)
+    lam = _gell_mann()
+    eps = 1e-5
+    worst = 0.0
+    for k, lex in enumerate([0, 3, V - 1, V // 2 + 1, V // 3]):
+        for mu in range(4):
+            a = (5 * k + mu) % 8
+            Up, Um = U.copy(), U.copy()
+            Up[lex, mu] = _expm_herm(lam[a], eps) @ U[lex, mu]
+            Um[lex, mu] = _expm_herm(lam[a], -eps) @ U[lex, mu]
+            fd = (_gauge_W(dims, Up, c0, c1)[0] - _gauge_W(dims, Um, c0, c1)[0]) / (2 * eps)
+            an = np.real(np.trace(1j * lam[a] @ U[lex, mu] @ S[lex, mu]))
+            worst = max(worst, abs(fd - an) / max(1e-2, abs(an)))
+    assert worst < 1e-6, worst
+    # (ii) loop counting, each family alone
+    _, sp, sr = _gauge_W(dims, U, 1.0, 1.0)
+    Sp = oracle.gauge_staples(dims, U, 1.0, 0.0)
+    Sr = oracle.gauge_staples(dims, U, 0.0, 1.0)
+    tot = lambda St: np.real(np.einsum("xmab,xmba->", U, St))
+    assert abs(tot(Sp) - 4 * sp) < 1e-9 * abs(sp) and abs(tot(Sr) - 6 * sr) < 1e-9 * abs(sr)
+    assert np.allclose(S, c0 * Sp + c1 * Sr, atol=1e-13)
+    # (iii) unit links
+    S1 = oracle.gauge_staples(dims, gen.unit_links(dims))
+    assert np.allclose(S1, (6 * c0 + 18 * c1) * np.eye(3), atol=1e-13)
+    # (iv) gauge covariance
+    g = gen.haar_like_links(dims, rng)[:, 0]
+    coords = gen.site_coords(dims)
+    Ug = np.empty_like(U)
+    fwd = np.empty((V, 4), dtype=np.int64)
+    for mu in range(4):
+        c = coords.copy()
+        c[:, mu] = (c[:, mu] + 1) % dims[mu]
+        fwd[:, mu] = c[:, 0] + dims[0] * (c[:, 1] + dims[1] * (c[:, 2] + dims[2] * c[:, 3]))
+        Ug[:, mu] = g @ U[:, mu] @ g[fwd[:, mu]].conj().swapaxes(-1, -2)
+    Sg = oracle.gauge_staples(dims, Ug)
+    for mu in range(4):
+        assert np.allclose(Sg[:, mu], g[fwd[:, mu]] @ S[:, mu] @ g.conj().swapaxes(-1, -2), atol=1e-12)
+
+
 def test_multishift_rejects_bad_shifts():
     dims = (2, 2, 2, 2)
     U = gen.unit_links(dims)
