@@ -189,6 +189,21 @@ int lqcd_fermion_force(lqcd_ctx *ctx, int nshift, const double *coeffs, void *co
 int lqcd_unpack_force(lqcd_ctx *ctx, void *canonical_dev /* c128 [V][4][3][3] */, const void *native);
 
 /*
+ * Gauge staples of the tree-level Symanzik improved action (PAPER.md:105,
+ * 365-393: "products of 3 and 5 SU(3) matrices representing links on C-shaped paths", Listing 3).
+ * The paper prints neither paths nor coefficients; reading R22 of DESIGN.md: with
+ *   W[U] = sum_x sum_{mu<nu} { c0 Re Tr P_{mu nu}(x) + c1 [Re Tr R_{mu nu}(x) + Re Tr R_{nu mu}(x)] }
+ * (P the 1x1 plaquette, R_{mu nu} the 2x1 rectangle; tree-level Symanzik: c0 = 5/3, c1 = -1/12),
+ *   staples[x][mu] = S_mu(x) = sum over the loops of W through U_mu(x) of coefficient x (remaining
+ *   links, ordered from x+mu back to x), i.e. W = Re Tr[U_mu(x) S_mu(x)] + (terms without U_mu(x)):
+ * per nu != mu two 3-link and six 5-link paths.  Links are periodic in all four directions.
+ *   links    native link field (device); staples: native 3x3-per-link field (device, lqcd_force_bytes;
+ *            same private layout as the force field: read it back with lqcd_unpack_force)
+ * async.  LQCD_ERR_UNSUPPORTED in slab mode.
+ */
+int lqcd_gauge_staples(lqcd_ctx *ctx, const void *links, void *staples, double c0, double c1);
+
+/*
  * ---- Slab mode: one x3 slab per GPU (the paper leaves the
  * multi-device version as future work) --------------------------------------
  * A rank that owns L3 = N3/P time slices creates its context with dims (N0,N1,N2,L3+2) and

@@ -61,6 +61,7 @@ _sig = {
     "lqcd_force_bytes": (_sz, [_vp]),
     "lqcd_fermion_force": (_i, [_vp, _i, _pd, C.POINTER(_vp), _vp, _vp]),
     "lqcd_unpack_force": (_i, [_vp, _vp, _vp]),
+    "lqcd_gauge_staples": (_i, [_vp, _vp, _vp, _d, _d]),
     "lqcd_dslash_slices": (_i, [_vp, _i, _vp, _vp, _vp, _i, _i]),
     "lqcd_halo_bytes": (_sz, [_vp]),
     "lqcd_halo_pack": (_i, [_vp, _vp, _vp, _i, _d]),
@@ -277,6 +278,13 @@ class Lattice:
         self._check(lib.lqcd_fermion_force(self._ctx, n, co.ctypes.data_as(_pd), ptrs, _vp(links.data_ptr()),
                                            _vp(force.data_ptr())))
         return force
+
+    def gauge_staples(self, links, c0=5.0 / 3.0, c1=-1.0 / 12.0, out=None):
+        """async; tree-level Symanzik staples (3x3 per link); read back with unpack_force."""
+        if out is None:
+            out = self._buf(int(lib.lqcd_force_bytes(self._ctx)))
+        self._check(lib.lqcd_gauge_staples(self._ctx, _vp(links.data_ptr()), _vp(out.data_ptr()), float(c0), float(c1)))
+        return out
 
     def unpack_force(self, native):
         """native force field -> numpy complex128 [V][4][3][3]."""

@@ -6,7 +6,9 @@
 
 template <typename T> struct Su3 { Cx<T> e[3][3]; };
 
-template <typename T, int LAYOUT, int RECON12, int POLICY>
+// STREAM = 1: evict-first loads (each link read once: Dslash, force); 0: cached loads (staples re-read
+// every link ~100 times from L1/L2).
+template <typename T, int LAYOUT, int RECON12, int POLICY, int STREAM = 1>
 __device__ __forceinline__ Su3<T> load_link(const T *__restrict__ links, int par, int mu, size_t Vh, size_t i, const L2Pol &pol)
 {
     constexpr int R = RECON12 ? 2 : 3;
@@ -15,7 +17,7 @@ __device__ __forceinline__ Su3<T> load_link(const T *__restrict__ links, int par
 #pragma unroll
     for (int r = 0; r < R; ++r)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) u.e[r][c] = ld_cx<T, LAYOUT, 1, POLICY>(links, plane0 + r * 3 + c, Vh, i, pol);
+        for (int c = 0; c < 3; ++c) u.e[r][c] = ld_cx<T, LAYOUT, STREAM, POLICY>(links, plane0 + r * 3 + c, Vh, i, pol);
     if (RECON12) {
         // r2[k] = conj( eps_kij r0[i] r1[j] )   (reading R8)
 #pragma unroll

@@ -366,6 +366,29 @@ def test_fermion_force_after_solve_periodic_bc():
     lat.close()
 
 
+@pytest.mark.parametrize("recon", [0, 1])
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (2, 2, 4, 2), (6, 4, 10, 8)])
+def test_gauge_staples(dims, prec, recon):
+    """NEXT-4 (lqcd_gauge_staples): tree-level Symanzik staples, element by element against the oracle
+    (pinned by finite differences of the gauge action).  2x2x4x2: every second-neighbour step wraps
+    onto the starting site; 6x4x10x8 spans several CTAs with a ragged tail."""
+    rng = np.random.default_rng(15)
+    U = gen.haar_like_links(dims, rng)
+    (U,) = round_inputs(prec, U)
+    if recon == 1 and prec == 1:
+        U = oracle.reconstruct_row3(U)
+    lat = make_lattice(dims, prec, recon)
+    links = lat.pack_links(U)
+    for c0, c1 in ((oracle.SYMANZIK_C0, oracle.SYMANZIK_C1), (1.0, 0.0), (0.0, 1.0)):
+        want = oracle.gauge_staples(dims, U, c0, c1)
+        got = lat.unpack_force(lat.gauge_staples(links, c0, c1))
+        assert rel(got, want) < TOL[prec], (dims, prec, recon, c0, c1, rel(got, want))
+        link_err = np.linalg.norm((got - want).reshape(-1, 9), axis=1).max()
+        assert link_err / np.linalg.norm(want.reshape(-1, 9), axis=1).mean() < 10 * TOL[prec]
+    lat.close()
+
+
 def test_cg_fp32_and_max_iter():
     dims = (8, 8, 8, 8)
     rng = np.random.default_rng(5)
