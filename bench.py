@@ -318,6 +318,21 @@ def run_ours(args):
                                        "frac": by / (t_f * 1e-3) / 1e9 / peak,
                                        "note": "8 x D_oe (1248 B per odd site) + outer products (576 links + 48*8 vectors + 576 force B per site)"}
         del xs8, fbuf
+        # ---- NEXT-4: tree-level Symanzik gauge staples (ALU / cache bound: 84 SU(3) products per link)
+        sbuf = lat.gauge_staples(links)
+        t_s = timed_loop(torch, lambda: lat.gauge_staples(links, out=sbuf), 10, 3, 1, D, device) / 10
+        flop_site = 4 * (84 * 198 + 24 * 36)
+        try:
+            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+                mhz = float(json.load(f)["sm_max_mhz"])
+        except Exception:
+            mhz = 1965.0
+        fp64_peak = 148 * 64 * 2 * mhz * 1e6 / 1e12          # 64 FP64 FMA lanes per SM
+        extra["gauge_staples_f64"] = {"ms": t_s, "ns_per_site": t_s * 1e6 / V, "flop_per_site": flop_site,
+                                      "TFLOPs": flop_site * V / (t_s * 1e-3) / 1e12, "bound": "alu",
+                                      "peak_TFLOPs": fp64_peak, "frac": flop_site * V / (t_s * 1e-3) / 1e12 / fp64_peak,
+                                      "note": "2 plaquette + 6 rectangle paths per nu, c0 = 5/3, c1 = -1/12"}
+        del sbuf
         # ---- CPU oracle beside it -------------------------------------------------------------
         psi = np.zeros((V, 3), dtype=np.complex128)
         psi[gen.half_index_of_parity(DIMS, 0)] = in_e

@@ -84,7 +84,7 @@ __device__ __forceinline__ void site_step(Site4 &s, const Geom &g, int d, int ne
 }
 
 template <typename T, int LAYOUT, int RECON12>
-__global__ void __launch_bounds__(128) staples_kernel(const Geom g, T *__restrict__ staples, const T *__restrict__ links,
+__global__ void __launch_bounds__(128, 3) staples_kernel(const Geom g, T *__restrict__ staples, const T *__restrict__ links,
                                                       const T c0, const T c1)
 {
     pdl_wait();
@@ -114,27 +114,37 @@ __global__ void __launch_bounds__(128) staples_kernel(const Geom g, T *__restric
         if (nu == mu) continue;
 #pragma unroll 1
         for (int p = 0; p < 8; ++p) {
+            // Addresses depend only on the path, not on the running product: resolve all steps first so
+            // that the link loads of a path are issued back to back, ahead of the dependent products.
+            const int nsteps = p < 2 ? 3 : 5;
             Site4 y = xm;
-            Su3<T> M;
-#pragma unroll 1
+            int spar[5], sdir[5], sneg[5];
+            size_t sidx[5];
+#pragma unroll
             for (int s = 0; s < 5; ++s) {
-                const int code = c_paths[p][s];
-                if (code == 0xF) break;
+                const int code = c_paths[p][s < nsteps ? s : 0];
                 const int d = (code & 2) ? nu : mu, neg = code & 1;
                 if (neg) site_step(y, g, d, 1);    // U_d(y-d)^dagger lives at y-d
-                const int par = (y.x0 + y.x1 + y.x2 + y.x3) & 1;
-                const size_t idx = (size_t)((y.x0 >> 1) + g.Nh0 * (y.x1 + g.N1 * (y.x2 + g.N2 * y.x3)));
-                const Su3<T> L = load_link<T, LAYOUT, RECON12, 0, 0>(links, par, d, (size_t)g.Ls, idx, pol);
+                spar[s] = (y.x0 + y.x1 + y.x2 + y.x3) & 1;
+                sidx[s] = (size_t)((y.x0 >> 1) + g.Nh0 * (y.x1 + g.N1 * (y.x2 + g.N2 * y.x3)));
+                sdir[s] = d; sneg[s] = neg;
                 if (!neg) site_step(y, g, d, 0);
-                if (s == 0) {
-                    if (neg) {
+            }
+            Su3<T> M = load_link<T, LAYOUT, RECON12, 0, 0>(links, spar[0], sdir[0], (size_t)g.Ls, sidx[0], pol);
+            if (sneg[0]) {
+                Su3<T> D;
 #pragma unroll
-                        for (int a = 0; a < 3; ++a)
+                for (int a = 0; a < 3; ++a)
 #pragma unroll
-                            for (int b = 0; b < 3; ++b) M.e[a][b] = cx<T>(L.e[b][a].re, -L.e[b][a].im);
-                    } else M = L;
-                } else if (neg) mat_mul_nd<T>(M, L);
-                else mat_mul_nn<T>(M, L);
+                    for (int b = 0; b < 3; ++b) D.e[a][b] = cx<T>(M.e[b][a].re, -M.e[b][a].im);
+                M = D;
+            }
+#pragma unroll
+            for (int s = 1; s < 5; ++s) {
+                if (s < nsteps) {
+                    const Su3<T> L = load_link<T, LAYOUT, RECON12, 0, 0>(links, spar[s], sdir[s], (size_t)g.Ls, sidx[s], pol);
+                    if (sneg[s]) mat_mul_nd<T>(M, L); else mat_mul_nn<T>(M, L);
+                }
             }
             const T c = p < 2 ? c0 : c1;
 #pragma unroll
