@@ -235,6 +235,8 @@ struct lqcd_ctx {
     lqcd_halo_fn halo_fn;            // fills the ghost slices of a half vector (NULL: nothing to do)
     lqcd_allreduce_fn allreduce_fn;  // sums device doubles over the ranks (NULL: single rank)
     void *comm_user;
+    int staples_x2block;   // x2 block size of the staples' CTA order (0: plain idxh order)
+    int staples_variant;   // 0: one product chain per path; 1: shared sub-products per (mu, nu)
     int iter_mask;         // diagnostic: bit k set = kernel k of the CG iteration is launched (default 15)
     int graph_active;      // read-only: the last solve ran from a graph
     cudaStream_t cap_stream;      // private stream used only for graph capture

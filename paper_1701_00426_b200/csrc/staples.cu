@@ -83,14 +83,39 @@ __device__ __forceinline__ void site_step(Site4 &s, const Geom &g, int d, int ne
     else s.x3 = neg ? (s.x3 == 0 ? g.N3 - 1 : s.x3 - 1) : (s.x3 + 1 == g.N3 ? 0 : s.x3 + 1);
 }
 
+// CTA -> (site tile, mu, parity).  A link is needed again by staples two x3 slices away; in plain idxh
+// order that reuse distance is 4-5 full time slices of links (94 MB at 32^4: ncu showed 8.6 GB of DRAM
+// reads per launch against 0.6 GB of links).  The swizzle (a) makes (mu, parity) the fastest index, so
+// that the 8 CTAs of one site tile run together, and (b) sweeps x3 inside blocks of `x2b` values of x2,
+// which cuts the x3 reuse distance to x2b/N2 of a slice.  tiles_row = tiles of 128 sites per (x2, x3)
+// row; sw.x2b == 0: identity order.
+struct StapleSwizzle { int x2b, tiles_row, N2, N3; };
+__device__ __forceinline__ void staple_cta(const StapleSwizzle &sw, int &tile, int &mu, int &parity)
+{
+    const int bid = blockIdx.x;
+    parity = bid & 1;
+    mu = (bid >> 1) & 3;
+    int t = bid >> 3;
+    if (sw.x2b > 0) {
+        // t enumerates (b, x3, j, tx) with x2 = b*x2b + j, tx the tile inside the row
+        const int tx = t % sw.tiles_row; t /= sw.tiles_row;
+        const int j = t % sw.x2b; t /= sw.x2b;
+        const int x3 = t % sw.N3;
+        const int b = t / sw.N3;
+        t = tx + sw.tiles_row * ((b * sw.x2b + j) + sw.N2 * x3);
+    }
+    tile = t;
+}
+
 template <typename T, int LAYOUT, int RECON12>
 __global__ void __launch_bounds__(128, 3) staples_kernel(const Geom g, T *__restrict__ staples, const T *__restrict__ links,
-                                                      const T c0, const T c1)
+                                                      const T c0, const T c1, const StapleSwizzle sw)
 {
     pdl_wait();
     pdl_trigger();
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int mu = blockIdx.y, parity = blockIdx.z;
+    int tile, mu, parity;
+    staple_cta(sw, tile, mu, parity);
+    const int i = tile * blockDim.x + threadIdx.x;
     if (i >= g.Vh) return;
     const L2Pol pol = {0, 0};
     uint32_t t = fd_div((uint32_t)i, g.dNh0);
@@ -163,6 +188,131 @@ __global__ void __launch_bounds__(128, 3) staples_kernel(const Geom g, T *__rest
             st_cx<T, LAYOUT, 0>(staples, (size_t)((parity * 4 + mu) * 9 + a * 3 + b), (size_t)g.Vh, (size_t)i, S.e[a][b], pol);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Variant 1 (option staples_variant = 1): the eight paths of one (mu, nu) share sub-products.
+// With m = mu^, n = nu^ and, above the link,
+//   A = U_nu(x+m), B = U_mu(x+n)^+, C = U_nu(x)^+,
+//   X = U_mu(x+m) U_nu(x+2m) U_mu(x+m+n)^+,  Y = U_mu(x-m+n)^+ U_nu(x-m)^+ U_mu(x-m),
+//   Z = U_nu(x+m+n) U_mu(x+2n)^+ U_nu(x+n)^+ :
+//   c0 ABC + c1 (XBC + ABY + AZC) = (c0 A + c1 X)(BC) + c1 A (BY + ZC)
+// and the mirror image below the link: 22 products and 28 link loads per nu instead of 28 and 36.
+// ---------------------------------------------------------------------------------------------
+template <typename T> __device__ __forceinline__ Su3<T> mm(const Su3<T> &a, const Su3<T> &b)
+{
+    Su3<T> o = a;
+    mat_mul_nn<T>(o, b);
+    return o;
+}
+template <typename T> __device__ __forceinline__ Su3<T> dagger(const Su3<T> &l)
+{
+    Su3<T> d;
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) d.e[a][b] = cx<T>(l.e[b][a].re, -l.e[b][a].im);
+    return d;
+}
+// lin = ca a + cb b
+template <typename T> __device__ __forceinline__ Su3<T> lin(T ca, const Su3<T> &a, T cb, const Su3<T> &b)
+{
+    Su3<T> o;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+            o.e[i][j] = cx<T>(fma(ca, a.e[i][j].re, cb * b.e[i][j].re), fma(ca, a.e[i][j].im, cb * b.e[i][j].im));
+    return o;
+}
+__device__ __forceinline__ int wrap_coord(int c, int N) { return c >= N ? c - N : (c < 0 ? c + N : c); }
+__device__ __forceinline__ int coord_of(const Site4 &s, int d) { return d == 0 ? s.x0 : d == 1 ? s.x1 : d == 2 ? s.x2 : s.x3; }
+__device__ __forceinline__ int extent_of(const Geom &g, int d) { return d == 0 ? g.N0 : d == 1 ? g.N1 : d == 2 ? g.N2 : g.N3; }
+__device__ __forceinline__ void set_coord(Site4 &s, int d, int v)
+{
+    if (d == 0) s.x0 = v; else if (d == 1) s.x1 = v; else if (d == 2) s.x2 = v; else s.x3 = v;
+}
+
+// U_dir(x + dm m + dn n), optionally daggered
+template <typename T, int LAYOUT, int RECON12>
+__device__ __forceinline__ Su3<T> link_at(const T *__restrict__ links, const Geom &g, const Site4 &x, int mu, int dm,
+                                          int nu, int dn, int dir, bool dag)
+{
+    Site4 y = x;
+    set_coord(y, mu, wrap_coord(coord_of(x, mu) + dm, extent_of(g, mu)));
+    set_coord(y, nu, wrap_coord(coord_of(x, nu) + dn, extent_of(g, nu)));
+    const int par = (y.x0 + y.x1 + y.x2 + y.x3) & 1;
+    const size_t idx = (size_t)((y.x0 >> 1) + g.Nh0 * (y.x1 + g.N1 * (y.x2 + g.N2 * y.x3)));
+    const L2Pol pol = {0, 0};
+    const Su3<T> L = load_link<T, LAYOUT, RECON12, 0, 0>(links, par, dir, (size_t)g.Ls, idx, pol);
+    return dag ? dagger<T>(L) : L;
+}
+
+template <typename T, int LAYOUT, int RECON12>
+__global__ void __launch_bounds__(128, 2) staples_kernel_shared(const Geom g, T *__restrict__ staples,
+                                                                const T *__restrict__ links, const T c0, const T c1, const StapleSwizzle sw)
+{
+    pdl_wait();
+    pdl_trigger();
+    int tile, mu, parity;
+    staple_cta(sw, tile, mu, parity);
+    const int i = tile * blockDim.x + threadIdx.x;
+    if (i >= g.Vh) return;
+    uint32_t t = fd_div((uint32_t)i, g.dNh0);
+    const int hx0 = i - (int)t * g.Nh0;
+    uint32_t t2 = fd_div(t, g.dN1);
+    Site4 x;
+    x.x1 = (int)t - (int)t2 * g.N1;
+    x.x3 = (int)fd_div(t2, g.dN2);
+    x.x2 = (int)t2 - x.x3 * g.N2;
+    x.x0 = 2 * hx0 + ((x.x1 + x.x2 + x.x3 + parity) & 1);
+#define LK(dm, dn, dir, dag) link_at<T, LAYOUT, RECON12>(links, g, x, mu, dm, nu, dn, dir, dag)
+    Su3<T> S;
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) S.e[a][b] = cx<T>((T)0, (T)0);
+#pragma unroll 1
+    for (int nu = 0; nu < 4; ++nu) {
+        if (nu == mu) continue;
+        // Order chosen for short live ranges (an fp64 SU(3) matrix is 36 registers): W = BY + ZC first,
+        // then A W, then (c0 A + c1 X)(BC); B and C are re-read from L1 rather than kept.
+        {   // above the link
+            Su3<T> W = mm<T>(LK(0, 1, mu, true),
+                             mm<T>(mm<T>(LK(-1, 1, mu, true), LK(-1, 0, nu, true)), LK(-1, 0, mu, false)));      // B Y
+            {
+                const Su3<T> ZC = mm<T>(mm<T>(mm<T>(LK(1, 1, nu, false), LK(0, 2, mu, true)), LK(0, 1, nu, true)),
+                                        LK(0, 0, nu, true));                                                  // Z C
+                W = lin<T>((T)1, W, (T)1, ZC);
+            }
+            const Su3<T> A = LK(1, 0, nu, false);
+            S = lin<T>((T)1, S, c1, mm<T>(A, W));
+            const Su3<T> X = lin<T>(c0, A, c1, mm<T>(mm<T>(LK(1, 0, mu, false), LK(2, 0, nu, false)), LK(1, 1, mu, true)));
+            const Su3<T> BC = mm<T>(LK(0, 1, mu, true), LK(0, 0, nu, true));
+            S = lin<T>((T)1, S, (T)1, mm<T>(X, BC));
+        }
+        {   // below the link
+            Su3<T> W = mm<T>(LK(0, -1, mu, true),
+                             mm<T>(mm<T>(LK(-1, -1, mu, true), LK(-1, -1, nu, false)), LK(-1, 0, mu, false)));    // B' Y'
+            {
+                const Su3<T> ZC = mm<T>(mm<T>(mm<T>(LK(1, -2, nu, true), LK(0, -2, mu, true)), LK(0, -2, nu, false)),
+                                        LK(0, -1, nu, false));                                                // Z' C'
+                W = lin<T>((T)1, W, (T)1, ZC);
+            }
+            const Su3<T> A = LK(1, -1, nu, true);
+            S = lin<T>((T)1, S, c1, mm<T>(A, W));
+            const Su3<T> X = lin<T>(c0, A, c1, mm<T>(mm<T>(LK(1, 0, mu, false), LK(2, -1, nu, true)), LK(1, -1, mu, true)));
+            const Su3<T> BC = mm<T>(LK(0, -1, mu, true), LK(0, -1, nu, false));
+            S = lin<T>((T)1, S, (T)1, mm<T>(X, BC));
+        }
+    }
+#undef LK
+    const L2Pol pol = {0, 0};
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+            st_cx<T, LAYOUT, 0>(staples, (size_t)((parity * 4 + mu) * 9 + a * 3 + b), (size_t)g.Vh, (size_t)i, S.e[a][b], pol);
+}
+
 extern "C" int lqcd_gauge_staples(lqcd_ctx *ctx, const void *links, void *staples, double c0, double c1)
 {
     if (!ctx) return LQCD_ERR_ARG;
@@ -173,10 +323,19 @@ extern "C" int lqcd_gauge_staples(lqcd_ctx *ctx, const void *links, void *staple
     if (c0 != c0 || c1 != c1) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_gauge_staples: NaN coefficient");
     if (ctx->halo_fn || ctx->x3_lo != 0 || ctx->x3_hi != ctx->g.N3)
         return lqcd_fail(ctx, LQCD_ERR_UNSUPPORTED, "lqcd_gauge_staples: not available in slab mode (second-neighbour halo)");
-    dim3 grid((ctx->g.Vh + 127) / 128, 4, 2), block(128);
+    dim3 grid(((ctx->g.Vh + 127) / 128) * 8), block(128);
+    StapleSwizzle sw = {0, 0, ctx->g.N2, ctx->g.N3};
+    const int row = ctx->g.Nh0 * ctx->g.N1;          // half-sites per (x2, x3) row
+    if (ctx->staples_x2block > 0 && row % 128 == 0 && ctx->g.N2 % ctx->staples_x2block == 0) {
+        sw.x2b = ctx->staples_x2block;
+        sw.tiles_row = row / 128;
+    }
 #define GO(T, L) do { \
-        if (ctx->recon == LQCD_RECON_12) launch_k(ctx, staples_kernel<T, L, 1>, grid, block, ctx->g, (T *)staples, (const T *)links, (T)c0, (T)c1); \
-        else launch_k(ctx, staples_kernel<T, L, 0>, grid, block, ctx->g, (T *)staples, (const T *)links, (T)c0, (T)c1); } while (0)
+        if (ctx->staples_variant == 1) { \
+            if (ctx->recon == LQCD_RECON_12) launch_k(ctx, staples_kernel_shared<T, L, 1>, grid, block, ctx->g, (T *)staples, (const T *)links, (T)c0, (T)c1, sw); \
+            else launch_k(ctx, staples_kernel_shared<T, L, 0>, grid, block, ctx->g, (T *)staples, (const T *)links, (T)c0, (T)c1, sw); \
+        } else if (ctx->recon == LQCD_RECON_12) launch_k(ctx, staples_kernel<T, L, 1>, grid, block, ctx->g, (T *)staples, (const T *)links, (T)c0, (T)c1, sw); \
+        else launch_k(ctx, staples_kernel<T, L, 0>, grid, block, ctx->g, (T *)staples, (const T *)links, (T)c0, (T)c1, sw); } while (0)
     if (ctx->prec == LQCD_F64) { if (ctx->layout == 0) GO(double, 0); else GO(double, 1); }
     else { if (ctx->layout == 0) GO(float, 0); else GO(float, 1); }
 #undef GO

@@ -183,10 +183,36 @@ def slab(dims_list, out):
     D.finalize(world)
 
 
+def staples(dims_list, out):
+    """NEXT-4: gauge staples, both kernel variants, fp64 / fp32, 18- / 12-real links."""
+    import numpy as np
+    import torch
+    import lqcd_inputs as gen
+    import paper_1701_00426_b200 as L
+
+    flop_site = 4 * (84 * 198 + 24 * 36)       # the definition's count: 84 SU(3) products per link
+    for dims in dims_list:
+        rng = np.random.default_rng(5)
+        U = gen.smooth_links(dims, 0.5, rng)
+        V = gen.volume(dims)
+        for prec in (0, 1):
+            for recon in (0, 1):
+                for variant in (0, 1):
+                    lat = L.Lattice(dims, prec=prec, recon=recon, options=dict(staples_variant=variant))
+                    links = lat.pack_links(U)
+                    buf = lat.gauge_staples(links)
+                    us = ev_time_us(torch, lambda: lat.gauge_staples(links, out=buf), 10, 2)
+                    out(dict(kind="staples", dims="x".join(map(str, dims)), prec=("f64", "f32")[prec], links=(18, 12)[recon],
+                             variant=variant, us=round(us, 1), ns_per_site=round(us * 1e3 / V, 3),
+                             TFLOPs=round(flop_site * V / us / 1e6, 2)))
+                    lat.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--ladder", action="store_true")
     ap.add_argument("--multishift", action="store_true")
+    ap.add_argument("--staples", action="store_true", help="NEXT-4 gauge staples timing")
     ap.add_argument("--slab", action="store_true", help="x3-slab path (run under torchrun for more than one GPU)")
     ap.add_argument("--dims", default=None, help="comma-separated N0,N1,N2,N3 (repeatable with ';')")
     ap.add_argument("--eps", type=float, default=0.5)
@@ -206,11 +232,13 @@ def main():
         ladder(dims_list or LADDER, args.eps, args.seed, out)
     if args.multishift:
         multishift(dims_list or [(24, 24, 24, 48), (32, 32, 32, 32)], out)
+    if args.staples:
+        staples(dims_list or [(16,) * 4, (32, 32, 32, 8), (32,) * 4], out)
     if args.slab:
         slab(dims_list or [(32, 32, 32, 32)], out)
     if args.md:
         with open(args.md, "a") as f:
-            for kind in ("dslash", "cg", "multishift_solve", "slab_dslash", "slab_multishift8"):
+            for kind in ("dslash", "cg", "multishift_solve", "slab_dslash", "slab_multishift8", "staples"):
                 sel = [r for r in rows if r["kind"] == kind]
                 if not sel:
                     continue
