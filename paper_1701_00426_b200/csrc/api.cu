@@ -91,7 +91,7 @@ extern "C" int lqcd_create(lqcd_ctx **out, const int dims[4], int prec, int reco
     c->num_sms = prop.multiProcessorCount;
     c->max_partials = g.Vh / 32 + 1024;   // >= the largest grid any reducing kernel uses
     if ((e = cudaMalloc(&c->d_state, sizeof(SolverState))) != cudaSuccess ||
-        (e = cudaMalloc(&c->d_partials, sizeof(double) * c->max_partials)) != cudaSuccess ||
+        (e = cudaMalloc(&c->d_partials, sizeof(double) * 2 * c->max_partials)) != cudaSuccess ||
         (e = cudaMallocHost(&c->h_flag, 64)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&c->ev[0], cudaEventDisableTiming)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming)) != cudaSuccess ||

@@ -192,13 +192,17 @@ __device__ __forceinline__ void st_cx(T *__restrict__ base, size_t plane, size_t
 #define LQCD_HIST 64
 struct SolverState {
     // recurrence state
-    double rho, alpha_prev, beta_prev, bnorm2, tol;
-    double zeta[LQCD_MAX_SHIFTS], zeta_old[LQCD_MAX_SHIFTS], zeta_new[LQCD_MAX_SHIFTS], delta[LQCD_MAX_SHIFTS];
+    // rho, zeta_i and the sticky active flags are DOUBLE-BUFFERED by iteration parity: the kernel that
+    // finishes iteration k (K2) reads cur[k&1] in every CTA while its CTA 0 writes cur[(k+1)&1], so the
+    // scalar step needs no grid-wide synchronisation (reduce.cuh).
+    struct Recur { double rho; double zeta[LQCD_MAX_SHIFTS]; int active[LQCD_MAX_SHIFTS]; } cur[2];
+    double alpha_prev, beta_prev, bnorm2, tol;
+    double zeta_old[LQCD_MAX_SHIFTS], zeta_new[LQCD_MAX_SHIFTS], delta[LQCD_MAX_SHIFTS];
     // coefficients of the current iteration, written by the reduction epilogues, read by K1/K2
     double alpha, beta;
     double c_alpha[LQCD_MAX_SHIFTS], c_zeta[LQCD_MAX_SHIFTS], c_beta[LQCD_MAX_SHIFTS];
     int c_active[LQCD_MAX_SHIFTS];
-    int active[LQCD_MAX_SHIFTS], conv_iter[LQCD_MAX_SHIFTS];
+    int conv_iter[LQCD_MAX_SHIFTS];
     int nshift, iter;
     int done;              // 0 running; 1 converged in this iteration (K2 still to run); 2 finished
     unsigned int ticket;   // last-block-done counter of the reductions
@@ -254,6 +258,7 @@ struct lqcd_ctx {
     void *stage; size_t stage_bytes;   // device staging of the *_host entry points (grow-only)
     int hist_n;
     double h_hist[3][LQCD_HIST];
+    int last_dslash_grid;  // CTAs of the most recent Dslash launch (= number of <p,q> partials)
     long launches;         // kernels launched through this context (bench.py's gpu_launches)
     char err[256];
 };

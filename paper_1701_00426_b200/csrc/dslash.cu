@@ -137,9 +137,12 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
     }
     }
     if (MODE == 2) {
-        double total;
-        if (grid_sum_last(dot, partials, &st->ticket, &total)) {
-            if (st->comm) st->sum[0] = total; else solver_after_pq(st, total);
+        if (st->comm) {   // slab mode: the caller all-reduces the LOCAL total (lqcd_set_slab)
+            double total;
+            if (grid_sum_last(dot, partials, &st->ticket, &total)) st->sum[0] = total;
+        } else {          // the next kernel (K1) adds the partials up itself: no fence, no ticket, no tail
+            const double b = block_sum(dot);
+            if (threadIdx.x == 0) partials[blockIdx.x] = b;
         }
     }
 }
@@ -153,6 +156,7 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
     if (tiles < 1) tiles = 1;
     if (ctx->dslash_persist > 0 && tiles > ctx->num_sms * ctx->dslash_persist) tiles = ctx->num_sms * ctx->dslash_persist;
     dim3 grid(tiles);
+    ctx->last_dslash_grid = tiles;
     int minb = ctx->dslash_minblocks;
     if (minb == 0) minb = sizeof(T) == 8 ? 2 : 3;
 #define GO1(MB, P) launch_k(ctx, dslash_kernel<T, LAYOUT, RECON12, MODE, MB, P>, grid, dim3(block), \

@@ -50,14 +50,31 @@ __device__ __forceinline__ bool grid_sum_last(double v, double *partials, unsign
     return threadIdx.x == 0;
 }
 
-// ---- scalar recurrences (one thread) -----------------------------------------------------
-// After q = A_b p and pq = Re<p,q>:   alpha = rho/pq;  zeta_i^new, alpha_i   (reading R11)
-__device__ __forceinline__ void solver_after_pq(SolverState *st, double pq)
+// Sum of `n` per-CTA partials written by the PREVIOUS kernel, computed by every CTA for itself in the
+// same fixed order (so every CTA gets the bit-identical total, run-to-run deterministic).  This replaces
+// fence + ticket + last-CTA sum in the producer: the producer only stores its partial, and the serial
+// tail of the reduction disappears (profiles/experiments_r1b.md section 3).  All threads get the result.
+__device__ __forceinline__ double sum_partials(const double *partials, int n)
 {
-    double alpha = st->rho / pq;
+    __shared__ double s_total;
+    double s = 0.0;
+    for (int k = threadIdx.x; k < n; k += blockDim.x) s += partials[k];
+    s = block_sum(s);
+    if (threadIdx.x == 0) s_total = s;
+    __syncthreads();
+    return s_total;
+}
+
+// ---- scalar recurrences (one thread) -------------------------------------------------------
+// ip = parity of the iteration number: the buffer of SolverState::cur that holds the current state.
+// After q = A_b p and pq = Re<p,q>:   alpha = rho/pq;  zeta_i^new, alpha_i   (reading R11)
+__device__ __forceinline__ void solver_after_pq(SolverState *st, double pq, int ip)
+{
+    const SolverState::Recur &c = st->cur[ip];
+    double alpha = c.rho / pq;
     st->alpha = alpha;
     for (int i = 0; i < st->nshift; ++i) {
-        double z = st->zeta[i], zo = st->zeta_old[i];
+        double z = c.zeta[i], zo = st->zeta_old[i];
         double zn = z * zo * st->alpha_prev /
                     (alpha * st->beta_prev * (zo - z) + zo * st->alpha_prev * (1.0 + st->delta[i] * alpha));
         st->zeta_new[i] = zn;
@@ -66,30 +83,35 @@ __device__ __forceinline__ void solver_after_pq(SolverState *st, double pq)
 }
 
 // After r -= alpha q and rho' = <r,r>:  beta, beta_i, history, convergence flags (sticky).
-__device__ __forceinline__ void solver_after_rr(SolverState *st, double rho_new)
+// Reads cur[ip], writes cur[ip^1].
+__device__ __forceinline__ void solver_after_rr(SolverState *st, double rho_new, int ip)
 {
-    double beta = rho_new / st->rho;
+    const SolverState::Recur &c = st->cur[ip];
+    SolverState::Recur &nx = st->cur[ip ^ 1];
+    double beta = rho_new / c.rho;
     st->beta = beta;
     int k = st->iter;
     if (k < LQCD_HIST) { st->hist_alpha[k] = st->alpha; st->hist_beta[k] = beta; st->hist_rnorm[k] = sqrt(rho_new); }
     double thresh = st->tol * sqrt(st->bnorm2);
     int n_active = 0;
     for (int i = 0; i < st->nshift; ++i) {
-        double zn = st->zeta_new[i], z = st->zeta[i];
+        double zn = st->zeta_new[i], z = c.zeta[i];
         double ratio = zn / z;
+        int act = c.active[i];
         st->c_zeta[i] = zn;
         st->c_beta[i] = beta * ratio * ratio;
-        st->c_active[i] = st->active[i];          // what K2 of THIS iteration must update
+        st->c_active[i] = act;                    // what K2 of THIS iteration must update
         st->zeta_old[i] = z;
-        st->zeta[i] = zn;
-        if (st->active[i]) {
+        nx.zeta[i] = zn;
+        if (act) {
             if (fabs(zn) * sqrt(rho_new) > thresh) ++n_active;
-            else { st->active[i] = 0; st->conv_iter[i] = k + 1; }
+            else { act = 0; st->conv_iter[i] = k + 1; }
         }
+        nx.active[i] = act;
     }
     st->alpha_prev = st->alpha;
     st->beta_prev = beta;
-    st->rho = rho_new;
+    nx.rho = rho_new;
     st->iter = k + 1;
     if (n_active == 0) st->done = 1;               // K2 of this iteration still runs
 }

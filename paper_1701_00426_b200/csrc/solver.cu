@@ -112,17 +112,20 @@ __global__ void __launch_bounds__(256) init_kernel(size_t npk, Seg sg, const T *
     if (grid_sum_last(acc, partials, &st->ticket, &total)) {
         if (st->comm) st->sum[2] = total;
         else {
-            st->rho = total;
+            st->cur[0].rho = total;
             st->bnorm2 = total;
             if (total == 0.0) st->done = 2;
         }
     }
 }
 
-// K1: r -= alpha q ; <r,r>
+// K1: r -= alpha q ; <r,r>.  Single GPU: every CTA first adds up the <p,q> partials the Dslash left
+// (`n_in` of them) and derives alpha; CTA 0 also runs the per-shift recurrence; the <r,r> partials go to
+// `part_out` for K2.  Slab mode (st->comm): alpha comes from scalar_kernel, the local <r,r> goes to sum[1].
 template <typename T, int POLICY>
 __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restrict__ r, const T *__restrict__ q,
-                                                 SolverState *st, double *partials)
+                                                 SolverState *st, const double *part_in, int n_in,
+                                                 double *part_out, int ip)
 {
     pdl_wait();
     pdl_trigger();
@@ -130,7 +133,15 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restri
     typedef typename Pack<T>::type P;
     const int N = Pack<T>::N;
     const uint64_t keep = POLICY ? l2_policy_evict_last() : 0;
-    const T alpha = (T)st->alpha;
+    const int comm = st->comm;
+    double alpha_d;
+    if (comm) alpha_d = st->alpha;
+    else {
+        const double pq = sum_partials(part_in, n_in);
+        alpha_d = st->cur[ip].rho / pq;
+        if (blockIdx.x == 0 && threadIdx.x == 0) solver_after_pq(st, pq, ip);
+    }
+    const T alpha = (T)alpha_d;
     double acc = 0.0;
     for (size_t k0 = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k0 < npk; k0 += (size_t)gridDim.x * blockDim.x) {
         const size_t k = seg_idx(k0, sg);
@@ -143,9 +154,12 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restri
         }
         stv<POLICY>(reinterpret_cast<P *>(r) + k, repack(a), keep);
     }
-    double total;
-    if (grid_sum_last(acc, partials, &st->ticket, &total)) {
-        if (st->comm) st->sum[1] = total; else solver_after_rr(st, total);
+    if (comm) {
+        double total;
+        if (grid_sum_last(acc, part_out, &st->ticket, &total)) st->sum[1] = total;
+    } else {
+        const double b = block_sum(acc);
+        if (threadIdx.x == 0) part_out[blockIdx.x] = b;
     }
 }
 
@@ -156,11 +170,21 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restri
 // traffic per active shift in exchange for one read-modify-write of y.
 template <typename T, int POLICY, int RAT>
 __global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__restrict__ r, T *__restrict__ p,
-                                                 ShiftPtrs sp, const SolverState *__restrict__ st)
+                                                 ShiftPtrs sp, SolverState *st, const double *part_in, int n_in, int ip)
 {
     pdl_wait();
     pdl_trigger();
     if (*(volatile const int *)&st->done == 2) return;
+    // Single GPU: every CTA adds up K1's <r,r> partials and derives beta and the per-shift coefficients
+    // from the state of iteration parity ip; CTA 0 also advances the state (into the other buffer).
+    // Slab mode: the coefficients were written by scalar_kernel after the all-reduce.
+    const int comm = st->comm;
+    double rho_new = 0.0, beta_d;
+    if (comm) beta_d = st->beta;
+    else {
+        rho_new = sum_partials(part_in, n_in);
+        beta_d = rho_new / st->cur[ip].rho;
+    }
     typedef typename Pack<T>::type P;
     const int N = Pack<T>::N;
     // r and p are re-read by the next kernels: keep.  x_i, p_i are touched once per iteration and
@@ -177,22 +201,33 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__
     if (threadIdx.x == 0) {
         int n = 0, ba = 0;
         for (int i = 0; i < sp.nshift; ++i) {
-            if (!st->c_active[i]) continue;
+            double c_zeta, c_beta;
+            int c_active;
+            if (comm) { c_active = st->c_active[i]; c_zeta = st->c_zeta[i]; c_beta = st->c_beta[i]; }
+            else {       // same expressions as solver_after_rr
+                const double zn = st->zeta_new[i], ratio = zn / st->cur[ip].zeta[i];
+                c_active = st->cur[ip].active[i];
+                c_zeta = zn;
+                c_beta = beta_d * ratio * ratio;
+            }
+            if (!c_active) continue;
             const T al = RAT ? (T)(sp.coef[i] * st->c_alpha[i]) : (T)st->c_alpha[i];
             if (i == sp.base) { ba = 1; s_base_alpha = al; continue; }
             s_alpha[n] = al;
-            s_zeta[n] = (T)st->c_zeta[i];
-            s_beta[n] = (T)st->c_beta[i];
+            s_zeta[n] = (T)c_zeta;
+            s_beta[n] = (T)c_beta;
             s_x[n] = RAT ? (P *)0 : reinterpret_cast<P *>(sp.x[i]);
             s_p[n] = reinterpret_cast<P *>(sp.p[i]);
             ++n;
         }
         s_n = n;
         s_base_active = ba;
+        // cur[ip] is not written by anyone in this kernel; the new state goes to cur[ip^1]
+        if (!comm && blockIdx.x == 0) solver_after_rr(st, rho_new, ip);
     }
     __syncthreads();
     const int n_act = s_n, base_active = s_base_active;
-    const T beta = (T)st->beta, base_alpha = base_active ? s_base_alpha : (T)0;
+    const T beta = (T)beta_d, base_alpha = base_active ? s_base_alpha : (T)0;
     P *const xb = RAT ? reinterpret_cast<P *>(sp.y) : reinterpret_cast<P *>(sp.x[sp.base]);
     constexpr int B = 4;     // shifts whose loads are in flight together
     for (size_t k0 = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k0 < npk; k0 += (size_t)gridDim.x * blockDim.x) {
@@ -237,20 +272,20 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__
 
 // Slab mode: the scalar step that the last CTA of a reduction performs on a single GPU, run after the
 // caller's all-reduce of st->sum[which] (0: after <p,q>; 1: after <r,r>; 2: after <b,b>).
-__global__ void scalar_kernel(SolverState *st, int which)
+__global__ void scalar_kernel(SolverState *st, int which, int ip)
 {
     pdl_wait();
     pdl_trigger();
     if (threadIdx.x || blockIdx.x) return;
     if (which == 2) {
         const double t = st->sum[2];
-        st->rho = t;
+        st->cur[0].rho = t;
         st->bnorm2 = t;
         if (t == 0.0) st->done = 2;
         return;
     }
     if (*(volatile int *)&st->done) return;
-    if (which == 0) solver_after_pq(st, st->sum[0]); else solver_after_rr(st, st->sum[1]);
+    if (which == 0) solver_after_pq(st, st->sum[0], ip); else solver_after_rr(st, st->sum[1], ip);
 }
 
 // ||a - b||^2 -> *slot
@@ -324,10 +359,10 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         if (ctx->halo_fn(ctx->comm_user, v, parity)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "halo hook failed");
         return LQCD_OK;
     };
-    auto reduce_then = [&](int which) -> int {
+    auto reduce_then = [&](int which, int ip) -> int {
         if (!comm) return LQCD_OK;
         if (ctx->allreduce_fn(ctx->comm_user, &dst->sum[which], 1)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "allreduce hook failed");
-        launch_k(ctx, scalar_kernel, dim3(1), dim3(32), dst, which);
+        launch_k(ctx, scalar_kernel, dim3(1), dim3(32), dst, which, ip);
         return lqcd_check_cuda(ctx, cudaGetLastError(), "scalar kernel");
     };
     const int block = ctx->blas_block;
@@ -350,9 +385,9 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     memset(&sp, 0, sizeof(sp));
     sp.nshift = nshift; sp.base = base;
     for (int i = 0; i < nshift; ++i) {
-        h.zeta[i] = h.zeta_old[i] = 1.0;
+        h.cur[0].zeta[i] = h.cur[1].zeta[i] = h.zeta_old[i] = 1.0;
         h.delta[i] = shifts[i] - shifts[base];
-        h.active[i] = 1;
+        h.cur[0].active[i] = h.cur[1].active[i] = 1;
         sp.x[i] = y ? NULL : xs[i];
         sp.p[i] = ws_vec(ctx, 4 + i);
         if (y) sp.coef[i] = coef[i];
@@ -363,41 +398,39 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     if (rc) return rc;
     if (ctx->l2_hints) launch_k(ctx, init_kernel<T, 1>, dim3(g_init), dim3(block), npk, sg, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
     else launch_k(ctx, init_kernel<T, 0>, dim3(g_init), dim3(block), npk, sg, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
-    if ((rc = reduce_then(2))) return rc;
+    if ((rc = reduce_then(2, 0))) return rc;
 
     const double msq = mass * mass + shifts[base];
     volatile int *flag = ctx->h_flag;
     flag[0] = flag[16 / 4] = 0;
     int enq = 0, chunk_id = 0, stop = 0;
     // one CG iteration = 4 kernels; all arguments are the same in every iteration
-    auto enqueue_iteration = [&]() -> int {
+    // <p,q> partials (one per Dslash CTA) and <r,r> partials (one per K1 CTA) live in separate halves of
+    // d_partials: K1 reads the first while it writes the second.
+    double *const part_pq = ctx->d_partials, *const part_rr = ctx->d_partials + ctx->max_partials;
+    auto enqueue_iteration = [&](int ip) -> int {      // ip = parity of the iteration number
         int e;
         const int m = ctx->iter_mask;   // diagnostic: which of the 4 kernels run (timing experiments only)
         if ((e = halo(p, par))) return e;
         if ((m & 1) && (e = launch_dslash(ctx, 1 - par, tmp_o, p, links, NULL, 0.0, 0, 2))) return e;
         if ((e = halo(tmp_o, 1 - par))) return e;
         if ((m & 2) && (e = launch_dslash(ctx, par, q, tmp_o, links, p, msq, 1, 1))) return e;
-        if ((e = reduce_then(0))) return e;
-        if (comm) {    // slab mode: the all-reduce of <r,r> sits between K1 and K2
-            if (m & 4) launch_k(ctx, k1_kernel<T, 0>, dim3(g_k1), dim3(block), npk, sg, r, (const T *)q, ctx->d_state, ctx->d_partials);
-            if ((e = reduce_then(1))) return e;
-            if (m & 8) {
-                if (sp.y) launch_k(ctx, k2_kernel<T, 0, 1>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
-                else launch_k(ctx, k2_kernel<T, 0, 0>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
-            }
-        } else if (ctx->l2_hints) {
-            if (m & 4) launch_k(ctx, k1_kernel<T, 1>, dim3(g_k1), dim3(block), npk, sg, r, (const T *)q, ctx->d_state, ctx->d_partials);
-            if (m & 8) {
-                if (sp.y) launch_k(ctx, k2_kernel<T, 1, 1>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
-                else launch_k(ctx, k2_kernel<T, 1, 0>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
-            }
+        const int n_pq = ctx->last_dslash_grid;
+        if ((e = reduce_then(0, ip))) return e;
+#define K1(POL) launch_k(ctx, k1_kernel<T, POL>, dim3(g_k1), dim3(block), npk, sg, r, (const T *)q, dst, \
+                         (const double *)part_pq, n_pq, part_rr, ip)
+#define K2(POL, RAT) launch_k(ctx, k2_kernel<T, POL, RAT>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, dst, \
+                              (const double *)part_rr, g_k1, ip)
+        if (ctx->l2_hints && !comm) {
+            if (m & 4) K1(1);
+            if (m & 8) { if (sp.y) K2(1, 1); else K2(1, 0); }
         } else {
-            if (m & 4) launch_k(ctx, k1_kernel<T, 0>, dim3(g_k1), dim3(block), npk, sg, r, (const T *)q, ctx->d_state, ctx->d_partials);
-            if (m & 8) {
-                if (sp.y) launch_k(ctx, k2_kernel<T, 0, 1>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
-                else launch_k(ctx, k2_kernel<T, 0, 0>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, (const SolverState *)ctx->d_state);
-            }
+            if (m & 4) K1(0);
+            if ((e = reduce_then(1, ip))) return e;    // slab mode: the all-reduce of <r,r> sits between K1 and K2
+            if (m & 8) { if (sp.y) K2(0, 1); else K2(0, 0); }
         }
+#undef K1
+#undef K2
         return lqcd_check_cuda(ctx, cudaGetLastError(), "cg iteration");
     };
     // Chunk graph (option `graph`): poll_chunk iterations captured once and replayed; the key is
@@ -418,7 +451,9 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         for (int i = 0; i < nshift; ++i) key[kn++] = (unsigned long long)(uintptr_t)xs[i];
     }
     ctx->graph_active = 0;
-    if (ctx->graph && max_iter >= ctx->poll_chunk && !comm && !ctx->halo_fn) {
+    // (even chunk length: the iteration parity `ip` of every captured launch is then the same in every replay)
+    const bool use_graph = ctx->graph && max_iter >= ctx->poll_chunk && !comm && !ctx->halo_fn && ctx->poll_chunk % 2 == 0;
+    if (use_graph) {
         if (!ctx->chunk_exec || ctx->chunk_key_n != kn || memcmp(ctx->chunk_key, key, kn * sizeof(key[0]))) {
             if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
             const long launches0 = ctx->launches;
@@ -426,7 +461,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
             int ok = cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
             if (ok) {
                 ctx->launch_stream = ctx->cap_stream;
-                for (int k = 0; k < ctx->poll_chunk && ok; ++k) ok = enqueue_iteration() == LQCD_OK;
+                for (int k = 0; k < ctx->poll_chunk && ok; ++k) ok = enqueue_iteration(k & 1) == LQCD_OK;
                 ctx->launch_stream = ctx->stream;
                 ok = (cudaStreamEndCapture(ctx->cap_stream, &g) == cudaSuccess) && ok && g;
             }
@@ -440,12 +475,12 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     while (!stop) {
         int n = ctx->poll_chunk;
         if (enq + n > max_iter) n = max_iter - enq;
-        if (ctx->graph && ctx->chunk_exec && n == ctx->poll_chunk) {
+        if (use_graph && ctx->graph && ctx->chunk_exec && n == ctx->poll_chunk) {
             if ((rc = lqcd_check_cuda(ctx, cudaGraphLaunch(ctx->chunk_exec, s), "chunk graph launch"))) return rc;
             ctx->launches += (long)__builtin_popcount(ctx->iter_mask) * n;
             ctx->graph_active = 1;
         } else {
-            for (int k = 0; k < n; ++k) if ((rc = enqueue_iteration())) return rc;
+            for (int k = 0; k < n; ++k) if ((rc = enqueue_iteration((enq + k) & 1))) return rc;
         }
         enq += n;
         int slot = chunk_id & 1;
@@ -475,7 +510,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     if (iters) *iters = h.iter;
     int converged = (h.done != 0);
     for (int i = 0; i < nshift; ++i) {
-        if (conv_iter) conv_iter[i] = h.active[i] ? h.iter : h.conv_iter[i];
+        if (conv_iter) conv_iter[i] = h.cur[h.iter & 1].active[i] ? h.iter : h.conv_iter[i];
         if (rel_resid && !y) rel_resid[i] = h.bnorm2 > 0.0 ? sqrt(h.resid[i] / h.bnorm2) : 0.0;
     }
     ctx->hist_n = h.iter < LQCD_HIST ? h.iter : LQCD_HIST;
