@@ -239,6 +239,7 @@ struct lqcd_ctx {
     lqcd_halo_fn halo_fn;            // fills the ghost slices of a half vector (NULL: nothing to do)
     lqcd_allreduce_fn allreduce_fn;  // sums device doubles over the ranks (NULL: single rank)
     void *comm_user;
+    int force_stage;       // 1: force_kernel stages the site's own vectors in shared memory when they fit
     int staples_x2block;   // x2 block size of the staples' CTA order (0: plain idxh order)
     int staples_variant;   // 0: one product chain per path; 1: shared sub-products per (mu, nu)
     int iter_mask;         // diagnostic: bit k set = kernel k of the CG iteration is launched (default 15)
@@ -275,12 +276,14 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 template <typename... KArgs, typename... Args>
-static inline cudaError_t launch_k(lqcd_ctx *ctx, void (*kern)(KArgs...), dim3 grid, dim3 block, Args... args)
+static inline cudaError_t launch_k_smem(lqcd_ctx *ctx, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                                        Args... args)
 {
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = grid;
     cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
     cfg.stream = ctx->launch_stream;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -289,6 +292,11 @@ static inline cudaError_t launch_k(lqcd_ctx *ctx, void (*kern)(KArgs...), dim3 g
     cfg.numAttrs = ctx->pdl ? 1 : 0;
     ctx->launches++;
     return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_k(lqcd_ctx *ctx, void (*kern)(KArgs...), dim3 grid, dim3 block, Args... args)
+{
+    return launch_k_smem(ctx, kern, grid, block, 0, args...);
 }
 
 int lqcd_fail(lqcd_ctx *ctx, int code, const char *fmt, ...);

@@ -24,10 +24,15 @@ struct ForceVecs {
     int n;
 };
 
-template <typename T, int LAYOUT, int RECON12>
+// STAGE = 1: the site's own n vectors are read from global memory ONCE into the thread's private
+// column of dynamic shared memory (n * 6 reals * 128 threads <= 48 KB) and re-read from there for each
+// direction; ncu had shown the four re-reads missing L1 (hit rate 0.8 %) and costing +33 % DRAM reads.
+template <typename T, int LAYOUT, int RECON12, int STAGE>
 __global__ void __launch_bounds__(128) force_kernel(const Geom g, const int parity, T *__restrict__ force,
                                                     const T *__restrict__ links, const ForceVecs fv)
 {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T *const own = reinterpret_cast<T *>(smem_raw);      // own[(s*6 + k)*128 + tid]
     pdl_wait();
     pdl_trigger();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -55,6 +60,17 @@ __global__ void __launch_bounds__(128) force_kernel(const Geom g, const int pari
     e[3] = ((rp + x1 + x2) & 1) ? -h : h;
     if (g.ap && x3 == g.N3 - 1) e[3] = -e[3];
 
+    if (STAGE) {
+        for (int s = 0; s < fv.n; ++s) {
+            Cx<T> ws[3];
+            load_vec<T, LAYOUT, 0>((const T *)fv.self[s], Vh, (size_t)i, (T)1, ws, pol);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                own[(s * 6 + 2 * c) * 128 + threadIdx.x] = ws[c].re;
+                own[(s * 6 + 2 * c + 1) * 128 + threadIdx.x] = ws[c].im;
+            }
+        }
+    }
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) {
         Cx<T> Q[3][3];
@@ -64,7 +80,11 @@ __global__ void __launch_bounds__(128) force_kernel(const Geom g, const int pari
             for (int b = 0; b < 3; ++b) Q[a][b] = cx<T>((T)0, (T)0);
         for (int s = 0; s < fv.n; ++s) {
             Cx<T> ws[3], wn[3];
-            load_vec<T, LAYOUT, 0>((const T *)fv.self[s], Vh, (size_t)i, (T)1, ws, pol);
+            if (STAGE) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    ws[c] = cx<T>(own[(s * 6 + 2 * c) * 128 + threadIdx.x], own[(s * 6 + 2 * c + 1) * 128 + threadIdx.x]);
+            } else load_vec<T, LAYOUT, 0>((const T *)fv.self[s], Vh, (size_t)i, (T)1, ws, pol);
             load_vec<T, LAYOUT, 0>((const T *)fv.nbr[s], Vh, (size_t)nf[mu], (T)fv.coef[s], wn, pol);
             // Q[a][b] += c w(x+mu)[a] conj(w(x)[b])
 #pragma unroll
@@ -137,8 +157,15 @@ template <typename T, int LAYOUT>
 static void launch_force_tl(lqcd_ctx *ctx, int parity, void *force, const void *links, const ForceVecs &fv)
 {
     dim3 grid((ctx->g.Vh + 127) / 128), block(128);
-    if (ctx->recon == LQCD_RECON_12) launch_k(ctx, force_kernel<T, LAYOUT, 1>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv);
-    else launch_k(ctx, force_kernel<T, LAYOUT, 0>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv);
+    const size_t smem = (size_t)fv.n * 6 * 128 * sizeof(T);
+    // measured at 32^4 (profiles/experiments_r1b.md section 7): fp64 -3 %, fp32 +20 % (the carve-out costs L1)
+    if (smem <= 48 * 1024 && ctx->force_stage && sizeof(T) == 8) {
+        if (ctx->recon == LQCD_RECON_12) launch_k_smem(ctx, force_kernel<T, LAYOUT, 1, 1>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv);
+        else launch_k_smem(ctx, force_kernel<T, LAYOUT, 0, 1>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv);
+    } else {
+        if (ctx->recon == LQCD_RECON_12) launch_k(ctx, force_kernel<T, LAYOUT, 1, 0>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv);
+        else launch_k(ctx, force_kernel<T, LAYOUT, 0, 0>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv);
+    }
 }
 
 extern "C" int lqcd_fermion_force(lqcd_ctx *ctx, int nshift, const double *coeffs, void *const *xs_e,
