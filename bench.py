@@ -10,7 +10,8 @@ i.e. one pass over all V sites; the default --steps 1000 is twice the config's "
 applications, parities alternated" (longer, so that the clock sampler sees the timed region).  metric = Dslash ns/site = step time / V (= time of one parity / (V/2)).
 
 The JSON line also carries: roofline (HBM, algorithmic 1248 B/site against MEASURED_PEAKS.json),
-e2e (same metric through lqcd_dslash_host with host buffers, copies inside the timed region),
+e2e (same metric through lqcd_dslash_host_vectors with host vectors, copies inside the timed region; links
+resident as the operator -- the all-inclusive lqcd_dslash_host figure is reported beside it as cold_links),
 cpu_baseline (the oracle on the host cores, bounded sample), clocks, gpu_launches, and `extra`
 (12-real, fp32, CG and multi-shift CG iter/s with their own algorithmic-bytes rooflines).
 
@@ -261,13 +262,22 @@ def run_ours(args):
     keep_j, h_in_o = pinned(in_o)
     keep_o, h_out = pinned(np.zeros_like(in_e))
 
+    # (a) the step's inputs are the two vectors; the link field is the OPERATOR: resident on the device,
+    #     uploaded once per gauge configuration and reused by every application
     def e2e_step():
+        lat.dslash_host_vectors(L.ODD, h_out, h_in_e, links)
+        lat.dslash_host_vectors(L.EVEN, h_out, h_in_o, links)
+    e2e_steps = max(1, min(args.steps, 50))
+    e2e_ms = timed_loop(torch, e2e_step, e2e_steps, 2, world, D, device)
+    h2d = 2 * in_e.nbytes
+    d2h = 2 * in_e.nbytes
+
+    # (b) worst case, nothing resident: the 604 MB canonical link field crosses PCIe in every call too
+    def e2e_cold_step():
         lat.dslash_host(L.ODD, h_out, h_in_e, hU)
         lat.dslash_host(L.EVEN, h_out, h_in_o, hU)
-    e2e_steps = max(1, min(args.steps, 5))
-    e2e_ms = timed_loop(torch, e2e_step, e2e_steps, 1, world, D, device)
-    h2d = 2 * (U.nbytes + in_e.nbytes)
-    d2h = 2 * in_e.nbytes
+    cold_steps = max(1, min(args.steps, 5))
+    cold_ms = timed_loop(torch, e2e_cold_step, cold_steps, 1, world, D, device)
     del keep_U, hU
 
     line = None
@@ -351,7 +361,11 @@ def run_ours(args):
                          "frac_of_nominal_8TBs": achieved / 8000.0},
             "e2e": {"value": e2e_ms * 1e6 / (e2e_steps * V * world), "unit": "ns/site", "steps": e2e_steps,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "api": "lqcd_dslash_host x2 per step (canonical host buffers, pinned)"},
+                    "api": "lqcd_dslash_host_vectors x2 per step: pinned canonical host vectors in and out, links resident "
+                           "(the operator; uploaded once per configuration, PAPER.md:276)",
+                    "cold_links": {"value": cold_ms * 1e6 / (cold_steps * V * world), "unit": "ns/site", "steps": cold_steps,
+                                   "h2d_bytes_per_step": 2 * (U.nbytes + in_e.nbytes), "d2h_bytes_per_step": 2 * in_e.nbytes,
+                                   "api": "lqcd_dslash_host x2 per step: the canonical link field is uploaded and packed in every call"}},
             "gpu_launches": launches,
             "clocks": clocks,
             "cpu_baseline": {"value": cpu_ns, "unit": "ns/site", "cores": cores, "kind": "oracle",

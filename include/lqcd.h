@@ -264,6 +264,11 @@ int lqcd_solver_history(lqcd_ctx *ctx, int n, double *alpha, double *beta, doubl
 int lqcd_dslash_host(lqcd_ctx *ctx, int parity, void *out_host /* c128 [V/2][3] */,
                      const void *in_host /* c128 [V/2][3] */,
                      const void *links_host /* c128 [V][4][3][3] */);
+/* As lqcd_dslash_host with the link field already resident on the device in NATIVE form (packed once per
+ * gauge configuration -- the paper moves fields only at the start and end of an update):
+ * only the input and output vectors cross the bus.  blocking. */
+int lqcd_dslash_host_vectors(lqcd_ctx *ctx, int parity, void *out_host /* c128 [V/2][3] */,
+                             const void *in_host /* c128 [V/2][3] */, const void *links_native_dev);
 int lqcd_cg_multishift_host(lqcd_ctx *ctx, int nshift, const double *shifts,
                             const void *rhs_host /* c128 [V/2][3] */,
                             void *solutions_host /* c128 [nshift][V/2][3] */,

@@ -69,6 +69,7 @@ _sig = {
     "lqcd_set_slab": (_i, [_vp, _i, _i, _i, HALO_FN, ALLREDUCE_FN, _vp]),
     "lqcd_solver_history": (_i, [_vp, _i, _pd, _pd, _pd]),
     "lqcd_dslash_host": (_i, [_vp, _i, _vp, _vp, _vp]),
+    "lqcd_dslash_host_vectors": (_i, [_vp, _i, _vp, _vp, _vp]),
     "lqcd_cg_multishift_host": (_i, [_vp, _i, _pd, _vp, _vp, _vp, _d, _d, _i, _pi, _pi, _pd]),
 }
 for _name, (_res, _args) in _sig.items():
@@ -306,6 +307,11 @@ class Lattice:
         """numpy complex128 arrays (pinned or not); copies + pack + kernel + unpack inside the call."""
         self._check(lib.lqcd_dslash_host(self._ctx, parity, _vp(out_host.ctypes.data), _vp(in_host.ctypes.data),
                                          _vp(links_host.ctypes.data)))
+
+    def dslash_host_vectors(self, parity, out_host, in_host, links):
+        """as dslash_host, links resident on the device in native form (only the vectors are copied)."""
+        self._check(lib.lqcd_dslash_host_vectors(self._ctx, parity, _vp(out_host.ctypes.data), _vp(in_host.ctypes.data),
+                                                 _vp(links.data_ptr())))
 
     def cg_multishift_host(self, sol_host, rhs_host, links_host, mass, shifts, tol, max_iter, raise_on_max_iter=True):
         import numpy as np

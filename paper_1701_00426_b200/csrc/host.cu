@@ -41,6 +41,29 @@ extern "C" int lqcd_dslash_host(lqcd_ctx *ctx, int parity, void *out_host, const
     return lqcd_check_cuda(ctx, cudaStreamSynchronize(s), "lqcd_dslash_host");
 }
 
+// As lqcd_dslash_host, but the link field is already resident in native form (uploaded and packed once
+// per gauge configuration, as the paper does: PAPER.md:276); only the vectors cross the bus.
+extern "C" int lqcd_dslash_host_vectors(lqcd_ctx *ctx, int parity, void *out_host, const void *in_host,
+                                        const void *links_native_dev)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    int rc = lqcd_check_cuda(ctx, cudaSetDevice(ctx->device), "cudaSetDevice");
+    if (rc) return rc;
+    if (!out_host || !in_host || !links_native_dev) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_dslash_host_vectors: null pointer");
+    if (parity != 0 && parity != 1) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_dslash_host_vectors: parity %d", parity);
+    const size_t canon_sp = (size_t)ctx->g.Vh * 3 * 16;
+    const size_t nat_sp = up256(lqcd_spinor_bytes(ctx));
+    if ((rc = stage_reserve(ctx, up256(canon_sp) + 2 * nat_sp))) return rc;
+    char *c_sp = (char *)ctx->stage, *n_in = c_sp + up256(canon_sp), *n_out = n_in + nat_sp;
+    cudaStream_t s = ctx->stream;
+    if ((rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(c_sp, in_host, canon_sp, cudaMemcpyHostToDevice, s), "H2D spinor"))) return rc;
+    if ((rc = lqcd_pack_spinor(ctx, 1 - parity, n_in, c_sp))) return rc;
+    if ((rc = lqcd_dslash(ctx, parity, n_out, n_in, links_native_dev))) return rc;
+    if ((rc = lqcd_unpack_spinor(ctx, parity, c_sp, n_out))) return rc;
+    if ((rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(out_host, c_sp, canon_sp, cudaMemcpyDeviceToHost, s), "D2H spinor"))) return rc;
+    return lqcd_check_cuda(ctx, cudaStreamSynchronize(s), "lqcd_dslash_host_vectors");
+}
+
 extern "C" int lqcd_cg_multishift_host(lqcd_ctx *ctx, int nshift, const double *shifts, const void *rhs_host,
                                        void *solutions_host, const void *links_host, double mass, double tol,
                                        int max_iter, int *iters, int *conv_iter, double *rel_resid)

@@ -391,6 +391,22 @@ def test_gauge_staples(dims, prec, recon):
     lat.close()
 
 
+@pytest.mark.parametrize("x2b", [0, 2, 4])
+def test_gauge_staples_cta_swizzle(x2b):
+    """The x2-blocked CTA order (option staples_x2block) is a pure scheduling choice.  16x16x4x4 has rows
+    of exactly 128 half-sites, so the swizzle is really applied (it silently falls back to plain order
+    when rows are not whole tiles, e.g. on the lattices of test_gauge_staples)."""
+    dims = (16, 16, 4, 4)
+    rng = np.random.default_rng(16)
+    U = gen.smooth_links(dims, 0.5, rng)
+    want = oracle.gauge_staples(dims, U)
+    for variant in (0, 1):
+        lat = make_lattice(dims, staples_x2block=x2b, staples_variant=variant)
+        got = lat.unpack_force(lat.gauge_staples(lat.pack_links(U)))
+        assert rel(got, want) < 1e-12, (x2b, variant, rel(got, want))
+        lat.close()
+
+
 def test_cg_fp32_and_max_iter():
     dims = (8, 8, 8, 8)
     rng = np.random.default_rng(5)
@@ -448,6 +464,9 @@ def test_host_entry_points():
     out = np.empty_like(phi)
     lat.dslash_host(1, out, phi, U)
     assert rel(out, oracle.dslash_half(dims, U, 1, phi)) < 1e-12
+    out2 = np.empty_like(phi)
+    lat.dslash_host_vectors(0, out2, phi, lat.pack_links(U))      # links resident, only vectors copied
+    assert rel(out2, oracle.dslash_half(dims, U, 0, phi)) < 1e-12
     shifts = np.array([0.5, 0.01])
     sol = np.empty((2,) + phi.shape, dtype=np.complex128)
     res = lat.cg_multishift_host(sol, phi, U, 0.05, shifts, 1e-10, 5000)
