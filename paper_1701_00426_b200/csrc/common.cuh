@@ -230,6 +230,8 @@ struct lqcd_ctx {
     int blas_block, blas_ctas_per_sm;
     int poll_chunk;        // CG iterations enqueued between convergence polls
     int pdl;               // 1: programmatic dependent launch (kernel N+1 is scheduled while N drains)
+    int capturing;         // (internal) launches are being captured into the chunk graph: plain edges there --
+                           // inside a graph PDL gains nothing and costs 4 us per iteration at 16^4 (experiments_r1b.md section 8)
     int graph;             // 1: the solver replays one CUDA graph per chunk of poll_chunk iterations
     int dslash_persist;    // 0: one 128-site tile per CTA; k > 0: num_sms*k CTAs loop over the tiles
     // slab mode (multi-GPU): the context describes the rank's x3 slab plus one
@@ -289,7 +291,7 @@ static inline cudaError_t launch_k_smem(lqcd_ctx *ctx, void (*kern)(KArgs...), d
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
-    cfg.numAttrs = ctx->pdl ? 1 : 0;
+    cfg.numAttrs = (ctx->pdl && !ctx->capturing) ? 1 : 0;
     ctx->launches++;
     return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }

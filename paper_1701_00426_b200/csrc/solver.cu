@@ -461,8 +461,10 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
             int ok = cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
             if (ok) {
                 ctx->launch_stream = ctx->cap_stream;
+                ctx->capturing = 1;
                 for (int k = 0; k < ctx->poll_chunk && ok; ++k) ok = enqueue_iteration(k & 1) == LQCD_OK;
                 ctx->launch_stream = ctx->stream;
+                ctx->capturing = 0;
                 ok = (cudaStreamEndCapture(ctx->cap_stream, &g) == cudaSuccess) && ok && g;
             }
             if (ok) ok = cudaGraphInstantiate(&ctx->chunk_exec, g, 0) == cudaSuccess;
