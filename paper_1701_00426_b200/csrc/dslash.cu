@@ -158,7 +158,7 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
     dim3 grid(tiles);
     ctx->last_dslash_grid = tiles;
     int minb = ctx->dslash_minblocks;
-    if (minb == 0) minb = sizeof(T) == 8 ? 2 : 3;
+    if (minb == 0) minb = sizeof(T) == 8 ? 2 : 4;   // profiles/experiments_r1b.md section 9
 #define GO1(MB, P) launch_k(ctx, dslash_kernel<T, LAYOUT, RECON12, MODE, MB, P>, grid, dim3(block), \
         ctx->g, parity, (T *)out, (const T *)in, (const T *)links, (const T *)xin, coef, ctx->d_state, ctx->d_partials, gate, i_begin, i_end)
 #define GO(MB) do { if (ctx->l2_hints) GO1(MB, 1); else GO1(MB, 0); } while (0)
