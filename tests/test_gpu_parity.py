@@ -407,6 +407,29 @@ def test_gauge_staples_cta_swizzle(x2b):
         lat.close()
 
 
+def test_next_rows_on_a_paper_lattice_shape():
+    """NEXT-3 / NEXT-4 at one of the paper's Table 3 / 4 shapes, 32^2 x 8 x 32, in the
+    default launch configuration (shared sub-products, x2-blocked CTA order really applied: rows are 4
+    tiles; 8 shifts staged in shared memory): every link against the oracle."""
+    dims = (32, 32, 8, 32)
+    rng = np.random.default_rng(5)
+    U = gen.smooth_links(dims, 0.5, rng)
+    lat = make_lattice(dims)
+    links = lat.pack_links(U)
+    got = lat.unpack_force(lat.gauge_staples(links))
+    want = oracle.gauge_staples(dims, U)
+    assert rel(got, want) < 1e-12
+    assert np.abs(got - want).max() < 1e-11
+    n = 8
+    xs = np.stack([gen.gaussian_half_spinor(dims, rng) for _ in range(n)])
+    c = np.linspace(-1.0, 1.5, n)
+    dx = [lat.pack_spinor(x, 0) for x in xs]
+    gotf = lat.unpack_force(lat.fermion_force(dx, links, c))
+    wantf = oracle.fermion_force(dims, U, c, xs)
+    assert rel(gotf, wantf) < 1e-12
+    lat.close()
+
+
 def test_cg_fp32_and_max_iter():
     dims = (8, 8, 8, 8)
     rng = np.random.default_rng(5)
