@@ -227,6 +227,13 @@ int lqcd_halo_pack(lqcd_ctx *ctx, void *buf, const void *spinor, int x3, double 
 /* slice x3 of spinor = buf;  async. */
 int lqcd_halo_unpack(lqcd_ctx *ctx, void *spinor, const void *buf, int x3);
 
+/* Both faces in one launch each way, for a context whose owned slices were set with lqcd_set_slab:
+ * buf_top = sign_top * (slice x3_hi-1), buf_bottom = sign_bottom * (slice x3_lo); and ghost slice
+ * x3_lo-1 = buf_from_down, ghost slice x3_hi = buf_from_up.  async. */
+int lqcd_halo_pack_faces(lqcd_ctx *ctx, void *buf_top, void *buf_bottom, const void *spinor,
+                         double sign_top, double sign_bottom);
+int lqcd_halo_unpack_ghosts(lqcd_ctx *ctx, void *spinor, const void *buf_from_down, const void *buf_from_up);
+
 /*
  * Communication hooks for the solvers in slab mode.  The library does not link a communication
  * library: the caller (torch.distributed / NCCL in paper_1701_00426_b200/slab.py) supplies

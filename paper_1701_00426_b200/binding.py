@@ -66,6 +66,8 @@ _sig = {
     "lqcd_halo_bytes": (_sz, [_vp]),
     "lqcd_halo_pack": (_i, [_vp, _vp, _vp, _i, _d]),
     "lqcd_halo_unpack": (_i, [_vp, _vp, _vp, _i]),
+    "lqcd_halo_pack_faces": (_i, [_vp, _vp, _vp, _vp, _d, _d]),
+    "lqcd_halo_unpack_ghosts": (_i, [_vp, _vp, _vp, _vp]),
     "lqcd_set_slab": (_i, [_vp, _i, _i, _i, HALO_FN, ALLREDUCE_FN, _vp]),
     "lqcd_solver_history": (_i, [_vp, _i, _pd, _pd, _pd]),
     "lqcd_dslash_host": (_i, [_vp, _i, _vp, _vp, _vp]),
@@ -212,6 +214,16 @@ class Lattice:
     def halo_unpack(self, spinor_ptr, buf, x3):
         ptr = spinor_ptr if isinstance(spinor_ptr, int) else spinor_ptr.data_ptr()
         self._check(lib.lqcd_halo_unpack(self._ctx, _vp(ptr), _vp(buf.data_ptr()), x3))
+
+    def halo_pack_faces(self, buf_top, buf_bottom, spinor_ptr, sign_top, sign_bottom):
+        ptr = spinor_ptr if isinstance(spinor_ptr, int) else spinor_ptr.data_ptr()
+        self._check(lib.lqcd_halo_pack_faces(self._ctx, _vp(buf_top.data_ptr()), _vp(buf_bottom.data_ptr()), _vp(ptr),
+                                             float(sign_top), float(sign_bottom)))
+
+    def halo_unpack_ghosts(self, spinor_ptr, buf_from_down, buf_from_up):
+        ptr = spinor_ptr if isinstance(spinor_ptr, int) else spinor_ptr.data_ptr()
+        self._check(lib.lqcd_halo_unpack_ghosts(self._ctx, _vp(ptr), _vp(buf_from_down.data_ptr()),
+                                                _vp(buf_from_up.data_ptr())))
 
     def set_slab(self, x3_lo, x3_hi, solve_parity, halo_cb=None, allreduce_cb=None):
         """halo_cb / allreduce_cb: HALO_FN / ALLREDUCE_FN instances (kept alive here) or None."""

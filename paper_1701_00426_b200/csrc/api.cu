@@ -305,6 +305,22 @@ extern "C" int lqcd_halo_unpack(lqcd_ctx *ctx, void *spinor, const void *buf, in
     return launch_halo(ctx, 0, (void *)buf, spinor, x3, 1.0);
 }
 
+extern "C" int lqcd_halo_pack_faces(lqcd_ctx *ctx, void *buf_top, void *buf_bottom, const void *spinor,
+                                    double sign_top, double sign_bottom)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(buf_top && buf_bottom && spinor, "lqcd_halo_pack_faces: null pointer");
+    return launch_halo2(ctx, 1, buf_top, buf_bottom, (void *)spinor, ctx->x3_hi - 1, ctx->x3_lo, sign_top, sign_bottom);
+}
+
+extern "C" int lqcd_halo_unpack_ghosts(lqcd_ctx *ctx, void *spinor, const void *buf_from_down, const void *buf_from_up)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(buf_from_down && buf_from_up && spinor, "lqcd_halo_unpack_ghosts: null pointer");
+    REQUIRE(ctx->x3_lo >= 1 && ctx->x3_hi < ctx->g.N3, "lqcd_halo_unpack_ghosts: the context has no ghost slices");
+    return launch_halo2(ctx, 0, (void *)buf_from_down, (void *)buf_from_up, spinor, ctx->x3_lo - 1, ctx->x3_hi, 1.0, 1.0);
+}
+
 extern "C" int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_parity, lqcd_halo_fn halo,
                              lqcd_allreduce_fn allreduce, void *user)
 {

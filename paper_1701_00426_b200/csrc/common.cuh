@@ -314,3 +314,4 @@ int launch_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical, const void 
 int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
                   const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo = -1, int x3_hi = -1);
 int launch_halo(lqcd_ctx *ctx, int pack, void *buf, void *spinor, int x3, double sign);
+int launch_halo2(lqcd_ctx *ctx, int pack, void *buf0, void *buf1, void *spinor, int x3_0, int x3_1, double sign0, double sign1);

@@ -56,11 +56,16 @@ __global__ void unpack_spinor_kernel(Geom g, double2 *__restrict__ canon, const 
 
 // One x3 slice (s3 = Nh0*N1*N2 sites) of a native half vector <-> a contiguous buffer laid out like a
 // half vector of s3 sites.  PACK: buf = sign * slice; else slice = buf.  (Slab mode halo, lqcd.h.)
+// blockIdx.y selects one of up to two faces handled by the same launch (buf / x3 / sign of face 0 or 1).
 template <typename T, int LAYOUT, int PACK>
-__global__ void halo_kernel(Geom g, T *__restrict__ buf, T *__restrict__ spinor, int x3, T sign)
+__global__ void halo_kernel(Geom g, T *__restrict__ buf0, T *__restrict__ buf1, T *__restrict__ spinor, int x3_0, int x3_1,
+                            T sign0, T sign1)
 {
     pdl_wait();
     pdl_trigger();
+    T *__restrict__ buf = blockIdx.y ? buf1 : buf0;
+    const int x3 = blockIdx.y ? x3_1 : x3_0;
+    const T sign = blockIdx.y ? sign1 : sign0;
     int f = blockIdx.x * blockDim.x + threadIdx.x;
     if (f >= g.s3) return;
     const size_t i = (size_t)x3 * g.s3 + f;
@@ -127,9 +132,15 @@ int launch_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical, const void 
 
 int launch_halo(lqcd_ctx *ctx, int pack, void *buf, void *spinor, int x3, double sign)
 {
-    dim3 grid((ctx->g.s3 + 127) / 128), block(128);
-#define CALL(T, L) do { if (pack) launch_k(ctx, halo_kernel<T, L, 1>, grid, block, ctx->g, (T *)buf, (T *)spinor, x3, (T)sign); \
-                        else launch_k(ctx, halo_kernel<T, L, 0>, grid, block, ctx->g, (T *)buf, (T *)spinor, x3, (T)sign); } while (0)
+    return launch_halo2(ctx, pack, buf, NULL, spinor, x3, 0, sign, 1.0);
+}
+
+// one launch for both faces (buf1 == NULL: one face only)
+int launch_halo2(lqcd_ctx *ctx, int pack, void *buf0, void *buf1, void *spinor, int x3_0, int x3_1, double sign0, double sign1)
+{
+    dim3 grid((ctx->g.s3 + 127) / 128, buf1 ? 2 : 1), block(128);
+#define CALL(T, L) do { if (pack) launch_k(ctx, halo_kernel<T, L, 1>, grid, block, ctx->g, (T *)buf0, (T *)buf1, (T *)spinor, x3_0, x3_1, (T)sign0, (T)sign1); \
+                        else launch_k(ctx, halo_kernel<T, L, 0>, grid, block, ctx->g, (T *)buf0, (T *)buf1, (T *)spinor, x3_0, x3_1, (T)sign0, (T)sign1); } while (0)
     DISPATCH_TL(ctx, CALL);
 #undef CALL
     return lqcd_check_cuda(ctx, cudaGetLastError(), "halo");

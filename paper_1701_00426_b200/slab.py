@@ -195,15 +195,13 @@ class SlabLattice:
     # -- hooks called from inside liblqcd_b200.so (lqcd_set_slab) ---------------------------------
     def _halo_start(self, vec_ptr):
         g, lat = self.geo, self.lat
-        lat.halo_pack(self._send_up, vec_ptr, g.x3_hi - 1, g.sign_send_up)
-        lat.halo_pack(self._send_down, vec_ptr, g.x3_lo, g.sign_send_down)
+        lat.halo_pack_faces(self._send_up, self._send_down, vec_ptr, g.sign_send_up, g.sign_send_down)
         return self.comm.exchange_start(self._send_up, self._send_down, self._from_down, self._from_up)
 
     def _halo_finish(self, vec_ptr, handle):
         g, lat = self.geo, self.lat
         self.comm.exchange_wait(handle)
-        lat.halo_unpack(vec_ptr, self._from_down, g.x3_lo - 1)
-        lat.halo_unpack(vec_ptr, self._from_up, g.x3_hi)
+        lat.halo_unpack_ghosts(vec_ptr, self._from_down, self._from_up)
 
     def _halo_hook(self, user, vec_ptr, parity):
         try:

@@ -174,3 +174,29 @@ def test_slab_mdagm_and_multishift_cg(world):
     bound = sum(abs(ci) * 10 * (7.0 / (m * m + s)) * tol * np.linalg.norm(xi)
                 for ci, s, xi in zip(c, shifts, ref["x"])) / np.linalg.norm(y_ref)
     assert rel(got_y, y_ref) < bound
+
+
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("layout", [0, 1])
+def test_single_face_halo_calls(prec, layout):
+    """lqcd_halo_pack / lqcd_halo_unpack (one face per call): slice 2 of a vector, sign -1, lands in
+    slice 0 of another; everything else of the target is untouched."""
+    import paper_1701_00426_b200 as L
+    dims = (4, 6, 2, 6)
+    phi = gen.gaussian_half_spinor(dims, 41)
+    if prec == 1:
+        phi = phi.astype(np.complex64).astype(np.complex128)
+    lat = L.Lattice(dims, prec=prec, options=dict(layout=layout))
+    src = lat.pack_spinor(phi, 0)
+    dst = lat.pack_spinor(2.0 * phi, 0)
+    buf = lat._buf(lat.halo_bytes)
+    lat.halo_pack(buf, src, 2, -1.0)
+    lat.halo_unpack(dst, buf, 0)
+    got = lat.unpack_spinor(dst, 0)
+    s3 = dims[0] * dims[1] * dims[2] // 2
+    want = 2.0 * phi
+    want[:s3] = -phi[2 * s3:3 * s3]
+    assert np.array_equal(got, want)
+    with pytest.raises(L.LqcdError):
+        lat.halo_pack(buf, src, 6, 1.0)
+    lat.close()
