@@ -39,8 +39,8 @@ FLOP_PER_SITE = 570          # 8*66 + 7*6, SURVEY.md section 8(a) a4
 BYTES_PER_SITE = {("f64", 18): 1248, ("f64", 12): 864, ("f32", 18): 624, ("f32", 12): 432}
 FALLBACK_HBM_GBS = 6650.0    # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the headline kernel, from the ncu --set full
-# capture summarised in profiles/ncu_dslash_r1.md (629.3 MB read + 5.6 MB written; algorithmic 654.3 MB)
-NCU_DRAM_TRAFFIC_BYTES = 634.9e6
+# capture summarised in profiles/ncu_dslash_r1d.md (629.3 MB read + 5.3 MB written; algorithmic 654.3 MB)
+NCU_DRAM_TRAFFIC_BYTES = 634.6e6
 
 
 def measured_hbm_peak():
@@ -355,7 +355,7 @@ def run_ours(args):
             "data": "synthetic", "config": dict(workload_config(), parallelism=f"replicas x{world} (no collective)"),
             "GFLOPs": FLOP_PER_SITE * V * world / (ms / args.steps * 1e-3) / 1e9,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_DRAM_TRAFFIC_BYTES, "traffic_source": "profiles/ncu_dslash_r1.md (ncu --set full, per launch)",
+                         "traffic": NCU_DRAM_TRAFFIC_BYTES, "traffic_source": "profiles/ncu_dslash_r1d.md (ncu --set full, per launch)",
                          "peak_source": peak_src, "kernel": "dslash_kernel<double,0,0,0,2,0>",
                          "bytes_per_launch": BYTES_PER_SITE[("f64", 18)] * Vh, "us_per_launch": us_launch,
                          "frac_of_nominal_8TBs": achieved / 8000.0},
