@@ -543,3 +543,7 @@ def test_oracle_regression_fixture():
     assert abs(got["config1_4x4_dirac_norm2"] - want["config1_4x4_dirac_norm2"]) < 1e-9 * want["config1_4x4_dirac_norm2"]
     assert np.allclose(got["config1_4x4_dirac_site0"], want["config1_4x4_dirac_site0"], rtol=1e-12)
     assert abs(got["cg_8x4_alpha0"] - want["cg_8x4_alpha0"]) < 1e-12
+    assert got["rational_4x4_iters"] == want["rational_4x4_iters"]
+    for k in ("rational_4x4_norm2", "force_4x4_norm2", "staples_4x4_norm2", "staples_4x4_retr_US"):
+        assert abs(got[k] - want[k]) < 1e-9 * abs(want[k]), k
+    assert np.allclose(got["force_4x4_link0"], want["force_4x4_link0"], rtol=1e-10, atol=1e-12)
