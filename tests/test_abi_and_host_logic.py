@@ -100,6 +100,37 @@ def test_fastdiv_formula():
             assert ((n * m) >> 32) >> (l - 1) == n // d
 
 
+def test_staple_cta_swizzle_is_a_permutation():
+    """The CTA order of the staples kernel (staples.cu staple_cta), re-derived: t enumerates (b, x3, j, tx)
+    and lands on tile tx + tiles_row*((b*x2b + j) + N2*x3): every tile exactly once."""
+    for N2, N3, tiles_row, x2b in [(32, 32, 4, 8), (8, 32, 4, 2), (4, 4, 1, 4), (12, 6, 3, 4), (32, 8, 4, 16)]:
+        n = tiles_row * N2 * N3
+        seen = np.zeros(n, dtype=int)
+        for t0 in range(n):
+            t = t0
+            tx = t % tiles_row; t //= tiles_row
+            j = t % x2b; t //= x2b
+            x3 = t % N3
+            b = t // N3
+            seen[tx + tiles_row * ((b * x2b + j) + N2 * x3)] += 1
+        assert (seen == 1).all(), (N2, N3, tiles_row, x2b)
+
+
+def test_slab_segment_map_covers_exactly_the_owned_packets():
+    """solver.cu seg_idx, re-derived: flat packet k of the owned slices -> plane*stride + off + (k mod len).
+    Layout 0: 3 complex planes of Vh sites (2 reals per site), packets of N reals."""
+    N0, N1, N2, N3 = 8, 4, 2, 6
+    s3, Vh = (N0 // 2) * N1 * N2, (N0 // 2) * N1 * N2 * N3
+    for N in (2, 4):                      # double2 / float4 packets
+        for x3_lo, x3_hi in ((1, 5), (0, 6), (2, 3)):
+            ln = (x3_hi - x3_lo) * s3 * 2 // N
+            stride, off = Vh * 2 // N, x3_lo * s3 * 2 // N
+            got = sorted((k // ln) * stride + off + k % ln for k in range(3 * ln))
+            want = sorted(p * stride + (x3 * s3 * 2 // N) + q for p in range(3) for x3 in range(x3_lo, x3_hi)
+                          for q in range(s3 * 2 // N))
+            assert got == want
+
+
 def test_shift_recipe_and_generators_are_deterministic():
     import lqcd_inputs as gen
     s = gen.rhmc_shifts(8)
