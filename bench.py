@@ -224,6 +224,10 @@ def run_ours(args):
     import lqcd_inputs as gen
     if int(os.environ.get("RANK", "0")) == 0:
         ensure_built()
+    else:                                    # other ranks wait for rank 0's build
+        t0 = time.time()
+        while not os.path.exists(os.path.join(ROOT, "paper_1701_00426_b200", "liblqcd_b200.so")) and time.time() - t0 < 600:
+            time.sleep(1.0)
     import paper_1701_00426_b200 as L
     from paper_1701_00426_b200 import dist as D
 
