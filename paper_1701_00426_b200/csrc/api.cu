@@ -83,7 +83,7 @@ extern "C" int lqcd_create(lqcd_ctx **out, const int dims[4], int prec, int reco
     c->iter_mask = 15;
     c->staples_variant = 1;
     c->force_stage = 1;
-    c->staples_x2block = 8;
+    c->staples_x2block = 4;
     c->launch_stream = c->stream;
     c->x3_lo = 0;
     c->x3_hi = g.N3;

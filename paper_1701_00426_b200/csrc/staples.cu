@@ -246,6 +246,27 @@ __device__ __forceinline__ Su3<T> link_at(const T *__restrict__ links, const Geo
     return dag ? dagger<T>(L) : L;
 }
 
+// idxh displacement of the site x + k d^ relative to x (periodic wrap included).  Direction 0 moves the
+// half-index by (x0' >> 1) - (x0 >> 1); the others by whole strides.  The parity of the displaced site is
+// parity ^ (k & 1) (all extents are even).  With these per-thread tables a link address is
+// i + dmu[dm] + dnu[dn]: two adds instead of a coordinate walk per load.
+__device__ __forceinline__ int idxh_disp(const Geom &g, const Site4 &x, int d, int k)
+{
+    const int c = coord_of(x, d), N = extent_of(g, d);
+    const int c2 = wrap_coord(c + k, N);
+    if (d == 0) return (c2 >> 1) - (c >> 1);
+    const int stride = d == 1 ? g.s1 : d == 2 ? g.s2 : g.s3;
+    return (c2 - c) * stride;
+}
+
+template <typename T, int LAYOUT, int RECON12>
+__device__ __forceinline__ Su3<T> link_rel(const T *__restrict__ links, const Geom &g, int i, int par, int disp, int dir, bool dag)
+{
+    const L2Pol pol = {0, 0};
+    const Su3<T> L = load_link<T, LAYOUT, RECON12, 0, 0>(links, par, dir, (size_t)g.Ls, (size_t)(i + disp), pol);
+    return dag ? dagger<T>(L) : L;
+}
+
 template <typename T, int LAYOUT, int RECON12>
 __global__ void __launch_bounds__(128, 2) staples_kernel_shared(const Geom g, T *__restrict__ staples,
                                                                 const T *__restrict__ links, const T c0, const T c1, const StapleSwizzle sw)
@@ -264,15 +285,21 @@ __global__ void __launch_bounds__(128, 2) staples_kernel_shared(const Geom g, T 
     x.x3 = (int)fd_div(t2, g.dN2);
     x.x2 = (int)t2 - x.x3 * g.N2;
     x.x0 = 2 * hx0 + ((x.x1 + x.x2 + x.x3 + parity) & 1);
-#define LK(dm, dn, dir, dag) link_at<T, LAYOUT, RECON12>(links, g, x, mu, dm, nu, dn, dir, dag)
+#define LK(dm, dn, dir, dag) link_rel<T, LAYOUT, RECON12>(links, g, i, parity ^ (((dm) + (dn)) & 1), dmu[(dm) + 1] + dnu[(dn) + 2], dir, dag)
     Su3<T> S;
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
         for (int b = 0; b < 3; ++b) S.e[a][b] = cx<T>((T)0, (T)0);
+    int dmu[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) dmu[k] = idxh_disp(g, x, mu, k - 1);
 #pragma unroll 1
     for (int nu = 0; nu < 4; ++nu) {
         if (nu == mu) continue;
+        int dnu[5];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) dnu[k] = idxh_disp(g, x, nu, k - 2);
         // Order chosen for short live ranges (an fp64 SU(3) matrix is 36 registers): W = BY + ZC first,
         // then A W, then (c0 A + c1 X)(BC); B and C are re-read from L1 rather than kept.
         {   // above the link
