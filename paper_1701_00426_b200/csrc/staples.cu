@@ -285,7 +285,12 @@ __global__ void __launch_bounds__(128, 2) staples_kernel_shared(const Geom g, T 
     x.x3 = (int)fd_div(t2, g.dN2);
     x.x2 = (int)t2 - x.x3 * g.N2;
     x.x0 = 2 * hx0 + ((x.x1 + x.x2 + x.x3 + parity) & 1);
-#define LK(dm, dn, dir, dag) link_rel<T, LAYOUT, RECON12>(links, g, i, parity ^ (((dm) + (dn)) & 1), dmu[(dm) + 1] + dnu[(dn) + 2], dir, dag)
+    // base pointers of the four link blocks this thread reads: (own / other parity) x (mu / nu)
+    constexpr int R3 = (RECON12 ? 2 : 3) * 3;
+    const T *const bm0 = links + 2 * (size_t)((parity * 4 + mu) * R3) * g.Ls;
+    const T *const bm1 = links + 2 * (size_t)(((parity ^ 1) * 4 + mu) * R3) * g.Ls;
+#define LKM(dm, dn, dag) link_rel<T, LAYOUT, RECON12>((((dm) + (dn)) & 1) ? bm1 : bm0, g, i, 0, dmu[(dm) + 1] + dnu[(dn) + 2], 0, dag)
+#define LKN(dm, dn, dag) link_rel<T, LAYOUT, RECON12>((((dm) + (dn)) & 1) ? bn1 : bn0, g, i, 0, dmu[(dm) + 1] + dnu[(dn) + 2], 0, dag)
     Su3<T> S;
 #pragma unroll
     for (int a = 0; a < 3; ++a)
@@ -300,38 +305,41 @@ __global__ void __launch_bounds__(128, 2) staples_kernel_shared(const Geom g, T 
         int dnu[5];
 #pragma unroll
         for (int k = 0; k < 5; ++k) dnu[k] = idxh_disp(g, x, nu, k - 2);
+        const T *const bn0 = links + 2 * (size_t)((parity * 4 + nu) * R3) * g.Ls;
+        const T *const bn1 = links + 2 * (size_t)(((parity ^ 1) * 4 + nu) * R3) * g.Ls;
         // Order chosen for short live ranges (an fp64 SU(3) matrix is 36 registers): W = BY + ZC first,
         // then A W, then (c0 A + c1 X)(BC); B and C are re-read from L1 rather than kept.
         {   // above the link
-            Su3<T> W = mm<T>(LK(0, 1, mu, true),
-                             mm<T>(mm<T>(LK(-1, 1, mu, true), LK(-1, 0, nu, true)), LK(-1, 0, mu, false)));      // B Y
+            Su3<T> W = mm<T>(LKM(0, 1, true),
+                             mm<T>(mm<T>(LKM(-1, 1, true), LKN(-1, 0, true)), LKM(-1, 0, false)));      // B Y
             {
-                const Su3<T> ZC = mm<T>(mm<T>(mm<T>(LK(1, 1, nu, false), LK(0, 2, mu, true)), LK(0, 1, nu, true)),
-                                        LK(0, 0, nu, true));                                                  // Z C
+                const Su3<T> ZC = mm<T>(mm<T>(mm<T>(LKN(1, 1, false), LKM(0, 2, true)), LKN(0, 1, true)),
+                                        LKN(0, 0, true));                                                  // Z C
                 W = lin<T>((T)1, W, (T)1, ZC);
             }
-            const Su3<T> A = LK(1, 0, nu, false);
+            const Su3<T> A = LKN(1, 0, false);
             S = lin<T>((T)1, S, c1, mm<T>(A, W));
-            const Su3<T> X = lin<T>(c0, A, c1, mm<T>(mm<T>(LK(1, 0, mu, false), LK(2, 0, nu, false)), LK(1, 1, mu, true)));
-            const Su3<T> BC = mm<T>(LK(0, 1, mu, true), LK(0, 0, nu, true));
+            const Su3<T> X = lin<T>(c0, A, c1, mm<T>(mm<T>(LKM(1, 0, false), LKN(2, 0, false)), LKM(1, 1, true)));
+            const Su3<T> BC = mm<T>(LKM(0, 1, true), LKN(0, 0, true));
             S = lin<T>((T)1, S, (T)1, mm<T>(X, BC));
         }
         {   // below the link
-            Su3<T> W = mm<T>(LK(0, -1, mu, true),
-                             mm<T>(mm<T>(LK(-1, -1, mu, true), LK(-1, -1, nu, false)), LK(-1, 0, mu, false)));    // B' Y'
+            Su3<T> W = mm<T>(LKM(0, -1, true),
+                             mm<T>(mm<T>(LKM(-1, -1, true), LKN(-1, -1, false)), LKM(-1, 0, false)));    // B' Y'
             {
-                const Su3<T> ZC = mm<T>(mm<T>(mm<T>(LK(1, -2, nu, true), LK(0, -2, mu, true)), LK(0, -2, nu, false)),
-                                        LK(0, -1, nu, false));                                                // Z' C'
+                const Su3<T> ZC = mm<T>(mm<T>(mm<T>(LKN(1, -2, true), LKM(0, -2, true)), LKN(0, -2, false)),
+                                        LKN(0, -1, false));                                                // Z' C'
                 W = lin<T>((T)1, W, (T)1, ZC);
             }
-            const Su3<T> A = LK(1, -1, nu, true);
+            const Su3<T> A = LKN(1, -1, true);
             S = lin<T>((T)1, S, c1, mm<T>(A, W));
-            const Su3<T> X = lin<T>(c0, A, c1, mm<T>(mm<T>(LK(1, 0, mu, false), LK(2, -1, nu, true)), LK(1, -1, mu, true)));
-            const Su3<T> BC = mm<T>(LK(0, -1, mu, true), LK(0, -1, nu, false));
+            const Su3<T> X = lin<T>(c0, A, c1, mm<T>(mm<T>(LKM(1, 0, false), LKN(2, -1, true)), LKM(1, -1, true)));
+            const Su3<T> BC = mm<T>(LKM(0, -1, true), LKN(0, -1, false));
             S = lin<T>((T)1, S, (T)1, mm<T>(X, BC));
         }
     }
-#undef LK
+#undef LKM
+#undef LKN
     const L2Pol pol = {0, 0};
 #pragma unroll
     for (int a = 0; a < 3; ++a)
