@@ -28,7 +28,7 @@ struct ForceVecs {
 // column of dynamic shared memory (n * 6 reals * 128 threads <= 48 KB) and re-read from there for each
 // direction; ncu had shown the four re-reads missing L1 (hit rate 0.8 %) and costing +33 % DRAM reads.
 template <typename T, int LAYOUT, int RECON12, int STAGE>
-__global__ void __launch_bounds__(128) force_kernel(const Geom g, const int parity, T *__restrict__ force,
+__global__ void __launch_bounds__(128, 5) force_kernel(const Geom g, const int parity, T *__restrict__ force,
                                                     const T *__restrict__ links, const ForceVecs fv)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
