@@ -585,3 +585,35 @@ def test_multishift_config4_24x24x24x48():
         assert rel(xg, ref["x"][i]) < 10 * (7.0 / (m * m + shifts[i])) * tol
     assert res["rel_resid"].max() < 1.5 * tol
     lat.close()
+
+
+def test_multishift_config4_32x4_properties_at_full_size():
+    """BASELINE.json configs[3], second lattice (32^4, the bench configuration): the full GPU solve is
+    checked by what holds at any size -- every shift's TRUE residual evaluated with the ORACLE operator
+    (reading R16 (i)) -- and the first 12 iterations in lock step with the oracle (R16 (iv)); the oracle
+    is not run to convergence here (the 24^3 x 48 test above does that)."""
+    dims = (32, 32, 32, 32)
+    rng = np.random.default_rng(4)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m, tol = 0.0025, 1e-10
+    shifts = gen.rhmc_shifts(8)
+    lat = make_lattice(dims)
+    links, be = lat.pack_links(U), lat.pack_spinor(b, 0)
+    xs = [lat.new_spinor() for _ in shifts]
+    res = lat.cg_multishift(xs, be, links, m, shifts, tol, 50000)
+    assert lat.get_option("graph_active") == 1
+    h = lat.solver_history()
+    ref = oracle.cg_multishift(dims, U, m, shifts, b, tol, 12, hist_len=12)
+    assert np.allclose(h["alpha"][:12], ref["alpha"], rtol=1e-10)
+    assert np.allclose(h["beta"][:12], ref["beta"], rtol=1e-10)
+    assert np.allclose(h["rnorm"][:12], ref["rnorm"], rtol=1e-10)
+    bn = np.linalg.norm(b)
+    for i, s in enumerate(shifts):
+        xg = lat.unpack_spinor(xs[i], 0)
+        tr = np.linalg.norm(b - oracle.mdagm(dims, U, m, xg, sigma=s)) / bn
+        assert tr < 1.5 * tol, (i, tr)
+        assert abs(tr - res["rel_resid"][i]) < 1e-12
+    assert np.all(np.diff(res["conv_iter"]) <= 0)          # larger shifts freeze earlier
+    assert res["conv_iter"][0] == res["iters"]
+    lat.close()
