@@ -29,6 +29,8 @@
  *   - All device work is enqueued on the CUDA stream given to lqcd_create.  Functions marked
  *     "async" return after enqueueing; functions marked "blocking" synchronise that stream.
  *   - out/in buffers of one call must not alias unless stated.
+ *   - A context is not thread-safe: one context per host thread (several contexts may share a
+ *     device and a stream).
  *   - Errors: bad arguments are detected before any launch (LQCD_ERR_ARG / _WORKSPACE);
  *     CUDA failures give LQCD_ERR_CUDA; lqcd_last_error() returns a message.
  *
