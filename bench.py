@@ -337,10 +337,10 @@ def run_ours(args):
         lat.cg_multishift(xs8, d_in_e, links, 0.0025, shifts, 1e-300, 8, raise_on_max_iter=False)
         fbuf = lat.fermion_force(xs8, links, [1.0] * 8)
         t_f = timed_loop(torch, lambda: lat.fermion_force(xs8, links, [1.0] * 8, force=fbuf), 20, 3, 1, D, device) / 20
-        by = 8 * 1248 * Vh + V * (576 + 48 * 8 + 576)
+        by = 8 * 1248 * Vh + V * (576 + 48 * 8 + 256)
         extra["fermion_force8_f64"] = {"ms": t_f, "ns_per_site": t_f * 1e6 / V, "bytes": by, "GBs": by / (t_f * 1e-3) / 1e9,
                                        "frac": by / (t_f * 1e-3) / 1e9 / peak,
-                                       "note": "8 x D_oe (1248 B per odd site) + outer products (576 links + 48*8 vectors + 576 force B per site)"}
+                                       "note": "8 x D_oe (1248 B per odd site) + outer products (576 links + 48*8 vectors + 256 B of 8-real force per site)"}
         del xs8, fbuf
         # ---- NEXT-4: tree-level Symanzik gauge staples (ALU / cache bound: 84 SU(3) products per link)
         sbuf = lat.gauge_staples(links)

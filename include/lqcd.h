@@ -180,14 +180,19 @@ int lqcd_rational_apply(lqcd_ctx *ctx, int nshift, const double *shifts, double 
  *   coeffs   host, nshift doubles (the c_i; c0 does not enter the force)
  *   xs_e     host array of nshift device pointers: the solutions x_i (native even-site vectors, e.g.
  *            from lqcd_cg_multishift); read only
- *   force    native force field (device, lqcd_force_bytes; out): 3x3 complex per link, layout private
+ *   force    native force field (device, lqcd_tamat_bytes; out).  F is traceless anti-Hermitian, so it is
+ *            stored as 8 reals per link -- the paper's tamat_soa: F01, F02, F12 and
+ *            (Im F00, Im F11); layout private, read it back with lqcd_unpack_tamat
  * The y_i are computed inside (nshift Dslash applications into the workspace of
  * lqcd_workspace_bytes(ctx, nshift)).  async.  LQCD_ERR_UNSUPPORTED in slab mode.
  */
-size_t lqcd_force_bytes(const lqcd_ctx *ctx);
+size_t lqcd_tamat_bytes(const lqcd_ctx *ctx); /* 8-real traceless anti-Hermitian field (fermion force)  */
+size_t lqcd_force_bytes(const lqcd_ctx *ctx); /* generic 3x3-complex-per-link field (gauge staples)          */
 int lqcd_fermion_force(lqcd_ctx *ctx, int nshift, const double *coeffs, void *const *xs_e,
                        const void *links, void *force);
-/* native force field -> canonical complex128 F[lex][mu][row][col] (device).  async. */
+/* native 8-real (tamat) field -> canonical complex128 F[lex][mu][row][col] (device).  async. */
+int lqcd_unpack_tamat(lqcd_ctx *ctx, void *canonical_dev /* c128 [V][4][3][3] */, const void *native);
+/* native 3x3-per-link field (staples) -> canonical complex128 [lex][mu][row][col] (device).  async. */
 int lqcd_unpack_force(lqcd_ctx *ctx, void *canonical_dev /* c128 [V][4][3][3] */, const void *native);
 
 /*
@@ -200,7 +205,7 @@ int lqcd_unpack_force(lqcd_ctx *ctx, void *canonical_dev /* c128 [V][4][3][3] */
  *   links, ordered from x+mu back to x), i.e. W = Re Tr[U_mu(x) S_mu(x)] + (terms without U_mu(x)):
  * per nu != mu two 3-link and six 5-link paths.  Links are periodic in all four directions.
  *   links    native link field (device); staples: native 3x3-per-link field (device, lqcd_force_bytes;
- *            same private layout as the force field: read it back with lqcd_unpack_force)
+ *            layout private: read it back with lqcd_unpack_force)
  * async.  LQCD_ERR_UNSUPPORTED in slab mode.
  */
 int lqcd_gauge_staples(lqcd_ctx *ctx, const void *links, void *staples, double c0, double c1);

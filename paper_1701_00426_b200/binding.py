@@ -59,6 +59,8 @@ _sig = {
     "lqcd_cg_multishift": (_i, [_vp, _i, _pd, _vp, C.POINTER(_vp), _vp, _d, _d, _i, _pi, _pi, _pd]),
     "lqcd_rational_apply": (_i, [_vp, _i, _pd, _d, _pd, _vp, _vp, _vp, _d, _d, _i, _pi, _pi]),
     "lqcd_force_bytes": (_sz, [_vp]),
+    "lqcd_tamat_bytes": (_sz, [_vp]),
+    "lqcd_unpack_tamat": (_i, [_vp, _vp, _vp]),
     "lqcd_fermion_force": (_i, [_vp, _i, _pd, C.POINTER(_vp), _vp, _vp]),
     "lqcd_unpack_force": (_i, [_vp, _vp, _vp]),
     "lqcd_gauge_staples": (_i, [_vp, _vp, _vp, _d, _d]),
@@ -279,14 +281,14 @@ class Lattice:
         return dict(iters=iters.value, conv_iter=np.array(list(conv)), converged=(rc == OK))
 
     def fermion_force(self, xs, links, coeffs, force=None):
-        """async; xs: the solutions x_i (native even-site buffers); returns the native force buffer."""
+        """async; xs: the solutions x_i (native even-site buffers); returns the native (tamat) force buffer."""
         import numpy as np
         n = len(xs)
         co = np.ascontiguousarray(coeffs, dtype=np.float64)
         assert co.size == n
         self.ensure_workspace(n)
         if force is None:
-            force = self._buf(int(lib.lqcd_force_bytes(self._ctx)))
+            force = self._buf(int(lib.lqcd_tamat_bytes(self._ctx)))
         ptrs = (_vp * n)(*[x.data_ptr() for x in xs])
         self._check(lib.lqcd_fermion_force(self._ctx, n, co.ctypes.data_as(_pd), ptrs, _vp(links.data_ptr()),
                                            _vp(force.data_ptr())))
@@ -299,8 +301,16 @@ class Lattice:
         self._check(lib.lqcd_gauge_staples(self._ctx, _vp(links.data_ptr()), _vp(out.data_ptr()), float(c0), float(c1)))
         return out
 
+    def unpack_tamat(self, native):
+        """native 8-real (tamat) field, e.g. the fermion force -> numpy complex128 [V][4][3][3]."""
+        import numpy as np
+        canon = self.torch.empty(self.V * 4 * 9 * 2, dtype=self.torch.float64, device=self.device)
+        self._check(lib.lqcd_unpack_tamat(self._ctx, _vp(canon.data_ptr()), _vp(native.data_ptr())))
+        self.synchronize()
+        return canon.cpu().numpy().view(np.complex128).reshape(self.V, 4, 3, 3)
+
     def unpack_force(self, native):
-        """native force field -> numpy complex128 [V][4][3][3]."""
+        """native 3x3-per-link field (gauge staples) -> numpy complex128 [V][4][3][3]."""
         import numpy as np
         canon = self.torch.empty(self.V * 4 * 9 * 2, dtype=self.torch.float64, device=self.device)
         self._check(lib.lqcd_unpack_force(self._ctx, _vp(canon.data_ptr()), _vp(native.data_ptr())))

@@ -115,14 +115,13 @@ __global__ void __launch_bounds__(128, 5) force_kernel(const Geom g, const int p
             }
         // TA[M]: Tr(M - M^dagger) = 2 i sum_a Im M_aa
         const T tr3 = (M[0][0].im + M[1][1].im + M[2][2].im) / (T)3;
-#pragma unroll
-        for (int a = 0; a < 3; ++a)
-#pragma unroll
-            for (int b = 0; b < 3; ++b) {
-                Cx<T> f = cx<T>((T)0.5 * (M[a][b].re - M[b][a].re), (T)0.5 * (M[a][b].im + M[b][a].im));
-                if (a == b) f.im -= tr3;
-                st_cx<T, LAYOUT, 0>(force, (size_t)((parity * 4 + mu) * 9 + a * 3 + b), Vh, (size_t)i, f, pol);
-            }
+        // F is traceless anti-Hermitian: 8 reals (the paper's tamat_soa).  Planes per
+        // (parity, mu): F01, F02, F12 and (Im F00, Im F11); lqcd_unpack_tamat rebuilds the 3x3 matrix.
+        const size_t pl = (size_t)(parity * 4 + mu) * 4;
+        st_cx<T, LAYOUT, 0>(force, pl + 0, Vh, (size_t)i, cx<T>((T)0.5 * (M[0][1].re - M[1][0].re), (T)0.5 * (M[0][1].im + M[1][0].im)), pol);
+        st_cx<T, LAYOUT, 0>(force, pl + 1, Vh, (size_t)i, cx<T>((T)0.5 * (M[0][2].re - M[2][0].re), (T)0.5 * (M[0][2].im + M[2][0].im)), pol);
+        st_cx<T, LAYOUT, 0>(force, pl + 2, Vh, (size_t)i, cx<T>((T)0.5 * (M[1][2].re - M[2][1].re), (T)0.5 * (M[1][2].im + M[2][1].im)), pol);
+        st_cx<T, LAYOUT, 0>(force, pl + 3, Vh, (size_t)i, cx<T>(M[0][0].im - tr3, M[1][1].im - tr3), pol);
     }
 }
 
@@ -146,6 +145,60 @@ __global__ void unpack_force_kernel(Geom g, double2 *__restrict__ canon, const T
             Cx<T> z = ld_cx<T, LAYOUT, 0, 0>(native, (size_t)((par * 4 + mu) * 9 + k), (size_t)g.Vh, (size_t)i, L2Pol());
             canon[(lex * 4 + mu) * 9 + k] = make_double2((double)z.re, (double)z.im);
         }
+}
+
+// native tamat field (4 complex planes per (parity, mu)) -> canonical c128 [V][4][3][3]
+template <typename T, int LAYOUT>
+__global__ void unpack_tamat_kernel(Geom g, double2 *__restrict__ canon, const T *__restrict__ native)
+{
+    pdl_wait();
+    pdl_trigger();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int par = blockIdx.y;
+    if (i >= g.Vh) return;
+    uint32_t t = fd_div((uint32_t)i, g.dNh0);
+    uint32_t t2 = fd_div(t, g.dN1);
+    const int x1 = (int)t - (int)t2 * g.N1;
+    const int x3 = (int)fd_div(t2, g.dN2);
+    const int x2 = (int)t2 - x3 * g.N2;
+    const size_t lex = 2 * (size_t)i + ((x1 + x2 + x3 + par) & 1);
+    for (int mu = 0; mu < 4; ++mu) {
+        Cx<T> z[4];
+        for (int k = 0; k < 4; ++k) z[k] = ld_cx<T, LAYOUT, 0, 0>(native, (size_t)((par * 4 + mu) * 4 + k), (size_t)g.Vh, (size_t)i, L2Pol());
+        double2 *f = canon + (lex * 4 + mu) * 9;
+        const double a = (double)z[3].re, b = (double)z[3].im;
+        f[0] = make_double2(0.0, a);
+        f[1] = make_double2((double)z[0].re, (double)z[0].im);
+        f[2] = make_double2((double)z[1].re, (double)z[1].im);
+        f[3] = make_double2(-(double)z[0].re, (double)z[0].im);      // F10 = -conj(F01)
+        f[4] = make_double2(0.0, b);
+        f[5] = make_double2((double)z[2].re, (double)z[2].im);
+        f[6] = make_double2(-(double)z[1].re, (double)z[1].im);
+        f[7] = make_double2(-(double)z[2].re, (double)z[2].im);
+        f[8] = make_double2(0.0, -(a + b));
+    }
+}
+
+extern "C" size_t lqcd_tamat_bytes(const lqcd_ctx *ctx)
+{
+    return ctx ? (size_t)ctx->g.Vh * 2 * 4 * 4 * 2 * elem_size(ctx) : 0;
+}
+
+extern "C" int lqcd_unpack_tamat(lqcd_ctx *ctx, void *canonical_dev, const void *native)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    int rc = lqcd_check_cuda(ctx, cudaSetDevice(ctx->device), "cudaSetDevice");
+    if (rc) return rc;
+    if (!canonical_dev || !native) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_unpack_tamat: null pointer");
+    dim3 grid((ctx->g.Vh + 127) / 128, 2), block(128);
+    if (ctx->prec == LQCD_F64) {
+        if (ctx->layout == 0) launch_k(ctx, unpack_tamat_kernel<double, 0>, grid, block, ctx->g, (double2 *)canonical_dev, (const double *)native);
+        else launch_k(ctx, unpack_tamat_kernel<double, 1>, grid, block, ctx->g, (double2 *)canonical_dev, (const double *)native);
+    } else {
+        if (ctx->layout == 0) launch_k(ctx, unpack_tamat_kernel<float, 0>, grid, block, ctx->g, (double2 *)canonical_dev, (const float *)native);
+        else launch_k(ctx, unpack_tamat_kernel<float, 1>, grid, block, ctx->g, (double2 *)canonical_dev, (const float *)native);
+    }
+    return lqcd_check_cuda(ctx, cudaGetLastError(), "unpack_tamat");
 }
 
 extern "C" size_t lqcd_force_bytes(const lqcd_ctx *ctx)

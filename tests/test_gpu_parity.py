@@ -335,7 +335,7 @@ def test_fermion_force(dims, prec, recon):
     lat = make_lattice(dims, prec, recon)
     links = lat.pack_links(U)
     dx = [lat.pack_spinor(x, 0) for x in xs]
-    got = lat.unpack_force(lat.fermion_force(dx, links, c))
+    got = lat.unpack_tamat(lat.fermion_force(dx, links, c))
     assert rel(got, want) < TOL[prec], (dims, prec, recon, rel(got, want))
     # per-link check as well (a wrong sign on one parity or direction would hide in a global norm less
     # than one would like): worst link relative to the typical link norm
@@ -361,7 +361,7 @@ def test_fermion_force_after_solve_periodic_bc():
     links, be = lat.pack_links(U), lat.pack_spinor(b, 0)
     xs = [lat.new_spinor() for _ in shifts]
     lat.cg_multishift(xs, be, links, m, shifts, tol, 5000)
-    got = lat.unpack_force(lat.fermion_force(xs, links, c))
+    got = lat.unpack_tamat(lat.fermion_force(xs, links, c))
     assert rel(got, want) < 1e-7          # solutions agree to O(kappa tol), the force is bilinear in them
     lat.close()
 
@@ -424,7 +424,7 @@ def test_next_rows_on_a_paper_lattice_shape():
     xs = np.stack([gen.gaussian_half_spinor(dims, rng) for _ in range(n)])
     c = np.linspace(-1.0, 1.5, n)
     dx = [lat.pack_spinor(x, 0) for x in xs]
-    gotf = lat.unpack_force(lat.fermion_force(dx, links, c))
+    gotf = lat.unpack_tamat(lat.fermion_force(dx, links, c))
     wantf = oracle.fermion_force(dims, U, c, xs)
     assert rel(gotf, wantf) < 1e-12
     lat.close()
