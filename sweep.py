@@ -1,9 +1,9 @@
 """Volume sweep and solve-to-tolerance runs (BASELINE.json configs[3] and configs[4]).
 
-    python -m paper_1701_00426_b200.sweep --ladder            # config 5: ns/site, GB/s vs volume
-    python -m paper_1701_00426_b200.sweep --multishift        # config 4: 24^3x48 and 32^4 solves
-    python -m paper_1701_00426_b200.sweep --dims 16,16,16,16 --ladder
-    python -m paper_1701_00426_b200.sweep --slab              # NEXT-2: slab path (torchrun for N > 1)
+    python sweep.py --ladder            # config 5: ns/site, GB/s vs volume
+    python sweep.py --multishift        # config 4: 24^3x48 and 32^4 solves
+    python sweep.py --dims 16,16,16,16 --ladder
+    python sweep.py --slab              # NEXT-2: slab path (torchrun for N > 1)
 
 Prints one JSON line per measurement and, with --md FILE, appends a Markdown table.  Timing is by
 CUDA events on the launching stream after warm-up.  Volumes whose links fit the 126 MB L2 are
@@ -18,7 +18,7 @@ import os
 import sys
 import time
 
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 

@@ -526,35 +526,53 @@ def test_dslash_32x4_bench_configuration(prec, recon):
     lat.close()
 
 
-def test_dslash_large_volume_sampled_sites():
-    """Maximum-size style check (64^3 x 16, V = 4.2 M, links 2.4 GB): sampled output sites computed
-    one by one by oracle_dirac_site, including corners and both x3 boundary slices."""
-    dims = (64, 64, 64, 16)
+@pytest.mark.parametrize("dims", [(64, 64, 64, 16), (48, 48, 48, 48)])
+def test_dslash_large_volume_sampled_sites(dims):
+    """BASELINE.json configs[4]: 64^3 x 16 (V = 4.2 M, links 2.4 GB) and 48^4 (V = 5.3 M, links 3.06 GB: the
+    largest index range the kernels see), in fp64 AND fp32, 18- and 12-real: sampled output sites computed one
+    by one by oracle_dirac_site (pinned to the dense matrix in tests/test_oracle_pins.py), including the
+    corners and both x3 boundary slices; in fp64 18-real also the FULL field of both parities."""
     rng = np.random.default_rng(5)
-    U = gen.smooth_links(dims, 0.5, rng)
-    psi = gen.gaussian_spinor(dims, rng)
-    lat = make_lattice(dims)
-    links = lat.pack_links(U)
+    U64 = gen.smooth_links(dims, 0.5, rng)
+    psi64 = gen.gaussian_spinor(dims, rng)
     coords = gen.site_coords(dims)
+    n0, n1, n2, n3 = dims
     samp = np.random.default_rng(99)
-    picks = [(0, 0, 0, 0), (63, 63, 63, 15), (1, 0, 0, 0), (0, 63, 0, 15), (62, 1, 63, 0), (63, 0, 0, 0)]
+    picks = [(0, 0, 0, 0), (n0 - 1, n1 - 1, n2 - 1, n3 - 1), (1, 0, 0, 0), (0, n1 - 1, 0, n3 - 1),
+             (n0 - 2, 1, n2 - 1, 0), (n0 - 1, 0, 0, 0), (0, 0, 0, n3 - 1), (n0 - 1, n1 - 1, n2 - 1, 0)]
     picks += [tuple(int(v) for v in coords[i]) for i in samp.integers(0, coords.shape[0], 200)]
-    got = {}
-    for par in (0, 1):
-        inp = oracle.full_to_half(dims, 1 - par, psi)
-        d_in, d_out = lat.pack_spinor(inp, 1 - par), lat.new_spinor()
-        lat.dslash(par, d_out, d_in, links)
-        got[par] = lat.unpack_spinor(d_out, par)
-    worst = 0.0
-    for x in picks:
-        par = sum(x) % 2
-        lex = x[0] + dims[0] * (x[1] + dims[1] * (x[2] + dims[2] * x[3]))
-        # the oracle reads the full-lattice psi; only opposite-parity neighbours enter D
-        want = oracle.dirac_site(dims, U, psi, x)
-        err = np.abs(got[par][lex // 2] - want).max() / np.abs(want).max()
-        worst = max(worst, err)
-    assert worst < 1e-12, worst
-    lat.close()
+    # both x3 boundary slices, random positions inside them
+    for x3 in (0, n3 - 1):
+        picks += [(int(samp.integers(n0)), int(samp.integers(n1)), int(samp.integers(n2)), x3) for _ in range(20)]
+    del coords
+    for prec in (0, 1):
+        U, psi = round_inputs(prec, U64, psi64)
+        halves = {p: oracle.full_to_half(dims, p, psi) for p in (0, 1)}
+        for recon in (0, 1):
+            lat = make_lattice(dims, prec, recon)
+            links = lat.pack_links(U)
+            got = {}
+            for par in (0, 1):
+                d_in, d_out = lat.pack_spinor(halves[1 - par], 1 - par), lat.new_spinor()
+                lat.dslash(par, d_out, d_in, links)
+                got[par] = lat.unpack_spinor(d_out, par)
+                del d_in, d_out
+            worst = 0.0
+            for x in picks:
+                par = sum(x) % 2
+                lex = x[0] + n0 * (x[1] + n1 * (x[2] + n2 * x[3]))
+                # the oracle reads the full-lattice psi; only opposite-parity neighbours enter D
+                want = oracle.dirac_site(dims, U, psi, x)
+                worst = max(worst, np.abs(got[par][lex // 2] - want).max() / np.abs(want).max())
+            assert worst < TOL[prec], (dims, prec, recon, worst)
+            if prec == 0 and recon == 0:
+                for par in (0, 1):
+                    want = oracle.dslash_half(dims, U, par, halves[1 - par])
+                    assert rel(got[par], want) < TOL[0], (dims, par)
+                    assert np.abs(got[par] - want).max() < 50 * TOL[0] * np.abs(want).max()
+                    del want
+            lat.close()
+            del links, got
 
 
 def test_multishift_config4_24x24x24x48():

@@ -50,6 +50,46 @@ def test_dirac_columns_at_2x4():
         assert np.abs(col - D[:, j]).max() < 1e-15
 
 
+@pytest.mark.parametrize("ap", [True, False])
+def test_dirac_site_is_the_dense_row_at_every_site(ap):
+    """oracle.dirac_site(x) (the checker of the large-volume sampled GPU parity tests) = rows
+    3*lex(x)..3*lex(x)+2 of the dense matrix applied to psi, for EVERY site of 4x2x6x2 (N_mu = 2 wraps in
+    two directions), both boundary conditions.  Catches a coordinate-order slip in the wrapper."""
+    dims = (4, 2, 6, 2)
+    rng = np.random.default_rng(21)
+    U = gen.haar_like_links(dims, rng)
+    psi = gen.gaussian_spinor(dims, rng)
+    want = (dense_dirac(dims, U, ap) @ psi.reshape(-1)).reshape(-1, 3)
+    coords = gen.site_coords(dims)
+    for lex in range(gen.volume(dims)):
+        got = oracle.dirac_site(dims, U, psi, coords[lex], antiperiodic_t=ap)
+        assert np.abs(got - want[lex]).max() < 1e-14, (lex, coords[lex])
+
+
+@pytest.mark.parametrize("ap", [True, False])
+def test_dirac_range_fills_exactly_lo_hi(ap):
+    """oracle.dirac_range(lo, hi) (what bench.py's CPU legs time) writes the dense-matrix values to
+    exactly [lo, hi) and leaves a NaN-prefilled remainder untouched: an off-by-one at either end, or a
+    loop over the wrong range, fails here."""
+    dims = (4, 2, 6, 2)
+    rng = np.random.default_rng(22)
+    U = gen.haar_like_links(dims, rng)
+    psi = gen.gaussian_spinor(dims, rng)
+    V = gen.volume(dims)
+    want = (dense_dirac(dims, U, ap) @ psi.reshape(-1)).reshape(-1, 3)
+    for lo, hi in [(0, V), (0, 1), (V - 1, V), (5, 5), (7, 40), (1, V - 1), (48, 49)]:
+        out = np.full((V, 3), np.nan + 1j * np.nan)
+        oracle.dirac_range(dims, U, psi, out, lo, hi, antiperiodic_t=ap)
+        assert np.isnan(out[:lo]).all() and np.isnan(out[hi:]).all(), (lo, hi)
+        if hi > lo:
+            assert np.abs(out[lo:hi] - want[lo:hi]).max() < 1e-14, (lo, hi)
+    # and the three entry points agree bit for bit (same static function underneath)
+    full = oracle.dirac_full(dims, U, psi, antiperiodic_t=ap)
+    out = np.zeros((V, 3), dtype=np.complex128)
+    oracle.dirac_range(dims, U, psi, out, 0, V, antiperiodic_t=ap)
+    assert np.array_equal(out, full)
+
+
 def test_half_lattice_views_and_parity_naming():
     """dslash_half(out_parity) = the (out, in) block of the dense matrix (reading R5)."""
     dims = (4, 4, 2, 4)
