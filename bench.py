@@ -1,21 +1,27 @@
 #!/usr/bin/env python
 """bench.py -- staggered Dslash / CG throughput on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--quick]
 
 Workload = BASELINE.json configs[2] ("config 3" of SURVEY.md section 8(d)): 32^4 lattice, fp64,
-18-real links, U = exp(i*0.3*H) seed 3, fixed Gaussian inputs.  One STEP = D_oe (odd <- even)
-followed by D_eo (even <- odd) from FIXED inputs (no ping-pong: rho(D) > 1 would overflow),
-i.e. one pass over all V sites; the default --steps 1000 is twice the config's "1000
-applications, parities alternated" (longer, so that the clock sampler sees the timed region).  metric = Dslash ns/site = step time / V (= time of one parity / (V/2)).
+18-real links, U = exp(i*0.3*H) seed 3, fixed Gaussian inputs.  One STEP = k x (D_oe then D_eo) from
+FIXED inputs (no ping-pong: rho(D) > 1 would overflow), k chosen so that the K timed steps hold at least
+MIN_APPLICATIONS single-parity applications whatever --steps is (config 3: "time 1000 applications, even
+and odd parity alternated"; more here, so that the clock sampler sees the timed region).
+metric = Dslash ns/site = time of one single-parity application / (V/2) = time of (D_oe + D_eo) / V.
 
-The JSON line also carries: roofline (HBM, algorithmic 1248 B/site against MEASURED_PEAKS.json),
-e2e (same metric through lqcd_dslash_host_vectors with host vectors, copies inside the timed region; links
-resident as the operator -- the all-inclusive lqcd_dslash_host figure is reported beside it as cold_links),
-cpu_baseline (the oracle on the host cores, bounded sample), clocks, gpu_launches, and `extra`
-(12-real, fp32, CG and multi-shift CG iter/s with their own algorithmic-bytes rooflines).
+The JSON line also carries: roofline (HBM, algorithmic 1248 B/site against MEASURED_PEAKS.json; DRAM traffic
+from profiles/traffic.json, the ncu capture of the SAME kernel), e2e (same metric through
+lqcd_dslash_host_vectors_batch with pinned host vectors, copies inside the timed region; links resident as the
+operator -- the all-inclusive lqcd_dslash_host figure is reported beside it as cold_links), cpu_baseline (the
+oracle on the host cores: Dslash, CG at 16^4, multi-shift CG at 24^3 x 48; bounded samples), clocks,
+gpu_launches, and `extra`: 12-real / fp32 Dslash, CG / multi-shift / rational iteration rates at 32^4,
+BASELINE.json configs[1], [3], [4] (16^4 CG and 24^3 x 48 / 32^4 multi-shift solves to tolerance, 48^4 and
+64^3 x 16 Dslash in fp64 and fp32), the fermion force, the gauge staples against the FP64 peak measured in
+this run, and the end-to-end multi-shift solve on host vectors.
 
---impl reference times the CPU oracle (this tier has no reference implementation).
+--impl reference times the CPU oracle (this tier has no reference implementation); that arm
+imports nothing of the product.
 Links (604 MB) exceed the 126 MB L2, so successive applications cannot reuse them from cache
 ("inputs larger than L2" rule); stated in config.l2.
 """
@@ -38,9 +44,9 @@ EPS, SEED = 0.3, 3
 FLOP_PER_SITE = 570          # 8*66 + 7*6, SURVEY.md section 8(a) a4
 BYTES_PER_SITE = {("f64", 18): 1248, ("f64", 12): 864, ("f32", 18): 624, ("f32", 12): 432}
 FALLBACK_HBM_GBS = 6650.0    # /opt/skills/guides/B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the headline kernel, from the ncu --set full
-# capture summarised in profiles/ncu_dslash_r1d.md (629.3 MB read + 5.3 MB written; algorithmic 654.3 MB)
-NCU_DRAM_TRAFFIC_BYTES = 634.6e6
+MIN_APPLICATIONS = 4000      # single-parity Dslash applications in the timed region (config 3 asks >= 1000)
+CG_BYTES = 2928              # per even site and CG iteration
+MS8_BYTES = 2544 + 144 + 144 + 96 + 7 * 192      # 8 shifts, all active
 
 
 def measured_hbm_peak():
@@ -49,6 +55,20 @@ def measured_hbm_peak():
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     except Exception:
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(kernel_name):
+    """DRAM bytes per launch of the headline kernel from profiles/traffic.json (written by
+    `python sweep.py --traffic-from-ncu` from an `ncu --set full` capture).  The entry must be for the kernel
+    this run launches: a stale file (kernel renamed or re-templated) is an error, not a silent constant."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    with open(path) as f:
+        t = json.load(f)
+    ent = t.get(kernel_name)
+    if ent is None:
+        raise SystemExit(f"bench.py: profiles/traffic.json has no entry for the kernel this run launches "
+                         f"({kernel_name}); re-capture it (python sweep.py --traffic-from-ncu)")
+    return ent
 
 
 class ClockSampler:
@@ -77,7 +97,6 @@ class ClockSampler:
     def stop(self):
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
         self.proc.terminate()
         try:
             self.proc.wait(timeout=2)
@@ -132,14 +151,46 @@ def cpu_oracle_dslash(U, psi, min_seconds=10.0, max_reps=50):
     return dt / reps * 1e9 / V, reps, oracle.num_threads()
 
 
+def cpu_oracle_solvers(gen, cfg2, cfg4, ms_sample_iters):
+    """The solver half of the metric on the host cores: the oracle's CG at 16^4 to
+    tolerance (config 2) and its multi-shift CG at 24^3 x 48 (config 4) for a bounded number of iterations."""
+    import numpy as np
+    import oracle
+    out = {}
+    dims, U, b, mass, tol = cfg2
+    t0 = time.perf_counter()
+    r = oracle.cg(dims, U, mass, b, tol, 20000)
+    dt = time.perf_counter() - t0
+    out["cg_16x4"] = {"value": r["iters"] / dt, "unit": "iter/s", "iters": r["iters"], "seconds": dt,
+                      "converged": bool(r["converged"]), "rel_resid": float(r["true_relres"]),
+                      "sample": "oracle_cg at 16^4 to tol 1e-10 (BASELINE.json configs[1]), whole solve"}
+    dims, U, b, mass, tol, shifts = cfg4
+    t0 = time.perf_counter()
+    r = oracle.cg_multishift(dims, U, mass, shifts, b, tol, ms_sample_iters)
+    dt = time.perf_counter() - t0
+    out["multishift_24x24x24x48"] = {"value": r["iters"] / dt, "unit": "iter/s", "iters": r["iters"], "seconds": dt,
+                                     "sample": f"first {ms_sample_iters} iterations of oracle_cg_multishift at 24^3 x 48, "
+                                               "8 shifts all active (BASELINE.json configs[3]); includes the oracle's "
+                                               "true-residual evaluation at exit"}
+    return out
+
+
+def workload_config(n_gpus):
+    return {"workload": "BASELINE.json configs[2]: Dslash on 32^4, fp64, 18-real links; one step = k x (D_oe then D_eo) "
+                        "from fixed inputs; value = time per single-parity application / (V/2)",
+            "dims": list(DIMS), "links": "U = exp(i*0.3*H) re-unitarised, seed 3", "spinors": "Gaussian, fixed",
+            "bc": "periodic x0-x2, antiperiodic x3",
+            "l2": "inputs larger than L2 (links 604 MB vs 126 MB L2); no flush needed",
+            "parallelism": f"replicas x{n_gpus} (no collective)"}
+
+
 def run_reference(args):
     """--impl reference: this tier has no reference implementation, so the arm times the CPU oracle
     (oracle/staggered_oracle.c, as it stands) on the same config and metric.  Each step is a
     bounded sample of the workload: a contiguous range of S lattice sites of the 32^4 problem,
-    S chosen from one calibration pass so that W+K steps end within ~2 minutes.  Rank 0 only."""
-    from paper_1701_00426_b200 import dist as D
-    rank, _, _ = D.env_world()
-    if rank != 0:
+    S chosen from one calibration pass so that W+K steps end within ~2 minutes.  Rank 0 only.
+    Nothing of the product (paper_1701_00426_b200) is imported or loaded here."""
+    if int(os.environ.get("RANK", "0")) != 0:
         return
     import numpy as np
     import lqcd_inputs as gen
@@ -168,7 +219,7 @@ def run_reference(args):
         "impl": "reference", "metric": "dslash_ns_per_site", "value": ns, "unit": "ns/site",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": workload_config(),
+        "data": "synthetic", "config": workload_config(args.gpus),
         "cpu_baseline": {"value": ns, "unit": "ns/site", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": ns, "unit": "ns/site", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -176,12 +227,14 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def workload_config():
-    return {"workload": "BASELINE.json configs[2]: Dslash on 32^4, fp64, 18-real links; one step = D_oe then D_eo "
-                        "from fixed inputs (V sites)",
-            "dims": list(DIMS), "links": "U = exp(i*0.3*H) re-unitarised, seed 3", "spinors": "Gaussian, fixed",
-            "bc": "periodic x0-x2, antiperiodic x3",
-            "l2": "inputs larger than L2 (links 604 MB vs 126 MB L2); no flush needed"}
+def ev_ms(torch, fn):
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    r = fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1), r
 
 
 def solver_iter_rate(torch, lat, L, links, b_e, shifts, mass, n_lo=24, n_hi=120, rational=False):
@@ -191,23 +244,34 @@ def solver_iter_rate(torch, lat, L, links, b_e, shifts, mass, n_lo=24, n_hi=120,
     xs = [lat.new_spinor() for _ in shifts]
 
     def solve(n):
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        if rational:   # lqcd_rational_apply: y accumulated in K2, the x_i are never stored
-            res = lat.rational_apply(xs[0], b_e, links, mass, shifts, 0.5, [1.0] * len(shifts), 1e-300, n,
-                                     raise_on_max_iter=False)
-        else:
-            res = lat.cg_multishift(xs, b_e, links, mass, shifts, 1e-300, n, raise_on_max_iter=False)
-        e1.record()
-        torch.cuda.synchronize()
+        def go():
+            if rational:   # lqcd_rational_apply: y accumulated in K2, the x_i are never stored
+                return lat.rational_apply(xs[0], b_e, links, mass, shifts, 0.5, [1.0] * len(shifts), 1e-300, n,
+                                          raise_on_max_iter=False)
+            return lat.cg_multishift(xs, b_e, links, mass, shifts, 1e-300, n, raise_on_max_iter=False)
+        ms, res = ev_ms(torch, go)
         assert res["iters"] == n, res
-        return e0.elapsed_time(e1)
+        return ms
 
     solve(n_lo)                                   # warm-up
     t_lo = min(solve(n_lo) for _ in range(2))
     t_hi = min(solve(n_hi) for _ in range(2))
     return (t_hi - t_lo) / (n_hi - n_lo)          # ms per iteration
+
+
+def solve_to_tolerance(torch, lat, links, b_e, shifts, mass, tol, peak, bytes_all_active=None):
+    """A (multi-shift) CG solve to tolerance: iterations, device time (CUDA events around the blocking call),
+    iter/s, worst true residual.  Second of two runs (the first builds the chunk graph)."""
+    xs = [lat.new_spinor() for _ in shifts]
+    go = lambda: lat.cg_multishift(xs, b_e, links, mass, shifts, tol, 100000)   # noqa: E731
+    ev_ms(torch, go)
+    ms, res = ev_ms(torch, go)
+    out = {"iters": int(res["iters"]), "ms": ms, "iter_per_s": res["iters"] / (ms * 1e-3),
+           "us_per_iter": ms * 1e3 / res["iters"], "max_true_rel_resid": float(res["rel_resid"].max()),
+           "conv_iter": [int(c) for c in res["conv_iter"]], "tol": tol, "mass": mass, "nshift": len(shifts)}
+    if bytes_all_active:
+        out["frac_if_all_active"] = bytes_all_active * lat.Vh / (out["us_per_iter"] * 1e-6) / 1e9 / peak
+    return out
 
 
 def ensure_built():
@@ -216,6 +280,14 @@ def ensure_built():
     if not os.path.exists(os.path.join(ROOT, "paper_1701_00426_b200", "liblqcd_b200.so")):
         import __graft_entry__
         __graft_entry__.build()
+
+
+def dslash_kernel_name(lat, L, prec, recon):
+    """Name of the Dslash instantiation the default options launch (template arguments of
+    dslash_kernel<T, LAYOUT, RECON12, MODE, MINB, POLICY> in csrc/dslash.cu)."""
+    minb = lat.get_option("dslash_minblocks") or (2 if prec == L.F64 else 4)
+    return (f"dslash_kernel<{'double' if prec == L.F64 else 'float'},{lat.get_option('layout')},"
+            f"{1 if recon == L.RECON_12 else 0},0,{minb},{lat.get_option('l2_hints')}>")
 
 
 def run_ours(args):
@@ -250,47 +322,75 @@ def run_ours(args):
     links = lat.pack_links(U)
     d_in_e, d_in_o = lat.pack_spinor(in_e, L.EVEN), lat.pack_spinor(in_o, L.ODD)
     d_out_e, d_out_o = lat.new_spinor(), lat.new_spinor()
+    kernel = dslash_kernel_name(lat, L, L.F64, L.RECON_18)
+    traffic = ncu_traffic(kernel)
+
+    # one step = k pairs, so that the timed region holds >= MIN_APPLICATIONS applications for any --steps
+    k = max(1, -(-MIN_APPLICATIONS // (2 * args.steps)))
 
     def step():
-        lat.dslash(L.ODD, d_out_o, d_in_e, links)     # D_oe
-        lat.dslash(L.EVEN, d_out_e, d_in_o, links)    # D_eo
+        for _ in range(k):
+            lat.dslash(L.ODD, d_out_o, d_in_e, links)     # D_oe
+            lat.dslash(L.EVEN, d_out_e, d_in_o, links)    # D_eo
 
     # ---- headline: K steps, inputs resident in HBM -------------------------------------------
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    for _ in range(args.warmup):
+        step()
+    if sampler is not None:
+        # the clock sampler starts AFTER the warm-up and the GPU is kept busy (untimed) until nvidia-smi has
+        # delivered its first row, so that every sample is taken under load; it stops right after the timed region
         sampler.start()
+        t0 = time.time()
+        while sampler.proc and not sampler.rows and time.time() - t0 < 3.0:
+            step()
+            torch.cuda.synchronize()
     n0 = lat.launches
-    ms = timed_loop(torch, step, args.steps, args.warmup, world, D, device)
-    launches = lat.launches - n0 - 2 * args.warmup
+    ms = timed_loop(torch, step, args.steps, 0, world, D, device)
+    launches = lat.launches - n0
     clocks = sampler.stop() if rank == 0 else None
-    ns_site = D.aggregate_ns_per_site(ms, args.steps, V, world)
-    us_launch = ms * 1e3 / (2 * args.steps)
+    apps = 2 * k * args.steps
+    ns_site = D.aggregate_ns_per_site(ms, k * args.steps, V, world)
+    us_launch = ms * 1e3 / apps
     achieved = BYTES_PER_SITE[("f64", 18)] * Vh / (us_launch * 1e-6) / 1e9
 
-    # ---- e2e: lqcd_dslash_host, pinned host buffers, copies inside the timed region ----------
+    # ---- e2e: pinned host buffers, copies inside the timed region ----------------------------
     def pinned(a):
         t = torch.from_numpy(np.ascontiguousarray(a).view(np.float64).reshape(-1)).pin_memory()
         return t, t.numpy().view(np.complex128).reshape(a.shape)
     keep_U, hU = pinned(U)
     keep_i, h_in_e = pinned(in_e)
     keep_j, h_in_o = pinned(in_o)
-    keep_o, h_out = pinned(np.zeros_like(in_e))
+    E2E_PAIRS = 4
+    keep_o = [pinned(np.zeros_like(in_e)) for _ in range(2 * E2E_PAIRS)]
+    h_outs = [o[1] for o in keep_o]
 
-    # (a) the step's inputs are the two vectors; the link field is the OPERATOR: resident on the device,
-    #     uploaded once per gauge configuration and reused by every application
+    # (a) the step's inputs are the vectors; the link field is the OPERATOR: resident on the device,
+    #     uploaded once per gauge configuration and reused by every application.  One step =
+    #     one lqcd_dslash_host_vectors_batch call of E2E_PAIRS x (D_oe, D_eo): every vector goes up and every
+    #     result comes down inside the call; uploads, kernels and downloads of successive applications overlap.
+    pars = [L.ODD, L.EVEN] * E2E_PAIRS
+    h_ins = [h_in_e, h_in_o] * E2E_PAIRS
+
     def e2e_step():
-        lat.dslash_host_vectors(L.ODD, h_out, h_in_e, links)
-        lat.dslash_host_vectors(L.EVEN, h_out, h_in_o, links)
-    e2e_steps = max(1, min(args.steps, 50))
+        lat.dslash_host_vectors_batch(pars, h_outs, h_ins, links)
+    e2e_steps = max(2, min(args.steps, 25))
     e2e_ms = timed_loop(torch, e2e_step, e2e_steps, 2, world, D, device)
-    h2d = 2 * in_e.nbytes
-    d2h = 2 * in_e.nbytes
+    h2d = 2 * E2E_PAIRS * in_e.nbytes
+    d2h = 2 * E2E_PAIRS * in_e.nbytes
+
+    # (a') one blocking call per application (round 1's figure): upload -> compute -> download in sequence
+    def e2e_serial_step():
+        lat.dslash_host_vectors(L.ODD, h_outs[0], h_in_e, links)
+        lat.dslash_host_vectors(L.EVEN, h_outs[1], h_in_o, links)
+    ser_steps = max(2, min(args.steps, 20))
+    ser_ms = timed_loop(torch, e2e_serial_step, ser_steps, 2, world, D, device)
 
     # (b) worst case, nothing resident: the 604 MB canonical link field crosses PCIe in every call too
     def e2e_cold_step():
-        lat.dslash_host(L.ODD, h_out, h_in_e, hU)
-        lat.dslash_host(L.EVEN, h_out, h_in_o, hU)
-    cold_steps = max(1, min(args.steps, 5))
+        lat.dslash_host(L.ODD, h_outs[0], h_in_e, hU)
+        lat.dslash_host(L.EVEN, h_outs[1], h_in_o, hU)
+    cold_steps = max(1, min(args.steps, 3))
     cold_ms = timed_loop(torch, e2e_cold_step, cold_steps, 1, world, D, device)
     del keep_U, hU
 
@@ -302,28 +402,14 @@ def run_ours(args):
             for recon, rn in ((L.RECON_18, 18), (L.RECON_12, 12)):
                 if prec == L.F64 and recon == L.RECON_18:
                     continue
-                lt = L.Lattice(DIMS, prec=prec, recon=recon, device=local_rank)
-                lk = lt.pack_links(U)
-                a, b_, o1, o2 = lt.pack_spinor(in_e, 0), lt.pack_spinor(in_o, 1), lt.new_spinor(), lt.new_spinor()
-
-                def st():
-                    lt.dslash(L.ODD, o1, a, lk)
-                    lt.dslash(L.EVEN, o2, b_, lk)
-                t = timed_loop(torch, st, 100, 5, 1, D, device)
-                us = t * 1e3 / 200
-                gbs = BYTES_PER_SITE[(pname, rn)] * Vh / (us * 1e-6) / 1e9
-                extra[f"dslash_{pname}_{rn}real"] = {"ns_per_site": us * 1e3 / Vh, "GBs": gbs, "frac": gbs / peak,
-                                                     "GFLOPs": FLOP_PER_SITE * Vh / (us * 1e-6) / 1e9}
-                lt.close()
-                del lk, a, b_, o1, o2
+                extra[f"dslash_{pname}_{rn}real"] = dslash_rate(torch, L, D, gen, DIMS, U, in_e, in_o, prec, recon, peak, device)
         # ---- CG and multi-shift CG iteration rates (configs 2/4 shaped, on 32^4) --------------
         ms_it = solver_iter_rate(torch, lat, L, links, d_in_e, [0.0], 0.01)
-        by = 2928
-        extra["cg_f64"] = {"iter_per_s": 1e3 / ms_it, "us_per_iter": ms_it * 1e3, "bytes_per_site_iter": by,
-                           "GBs": by * Vh / (ms_it * 1e-3) / 1e9, "frac": by * Vh / (ms_it * 1e-3) / 1e9 / peak}
+        extra["cg_f64"] = {"iter_per_s": 1e3 / ms_it, "us_per_iter": ms_it * 1e3, "bytes_per_site_iter": CG_BYTES,
+                           "GBs": CG_BYTES * Vh / (ms_it * 1e-3) / 1e9, "frac": CG_BYTES * Vh / (ms_it * 1e-3) / 1e9 / peak}
         shifts = gen.rhmc_shifts(8)
         ms_it = solver_iter_rate(torch, lat, L, links, d_in_e, shifts, 0.0025)
-        by = 2544 + 144 + 144 + 96 + 7 * 192
+        by = MS8_BYTES
         extra["multishift8_f64"] = {"iter_per_s": 1e3 / ms_it, "us_per_iter": ms_it * 1e3, "bytes_per_site_iter": by,
                                     "GBs": by * Vh / (ms_it * 1e-3) / 1e9, "frac": by * Vh / (ms_it * 1e-3) / 1e9 / peak,
                                     "note": "all 8 shifts active (worst case)"}
@@ -332,6 +418,22 @@ def run_ours(args):
         extra["rational8_f64"] = {"iter_per_s": 1e3 / ms_it, "us_per_iter": ms_it * 1e3, "bytes_per_site_iter": by,
                                   "GBs": by * Vh / (ms_it * 1e-3) / 1e9, "frac": by * Vh / (ms_it * 1e-3) / 1e9 / peak,
                                   "note": "lqcd_rational_apply, 8 shifts all active: y += c_i alpha_i p_i fused, x_i never stored"}
+        # ---- BASELINE.json configs[3], second lattice: the 8-shift solve to tolerance at 32^4 -------
+        extra["multishift_32x32x32x32"] = dict(
+            solve_to_tolerance(torch, lat, links, d_in_e, shifts, 0.0025, 1e-10, peak, MS8_BYTES),
+            note="BASELINE.json configs[3] at 32^4: 8 shifts 1e-4..1, m = 0.0025, tol 1e-10 per shift; the bench's "
+                 "resident links (eps 0.3, seed 3) and rhs in_e; traffic falls as shifts freeze")
+        # ---- e2e of the method: rhs up, 8 solutions down, hundreds of applications in between ------
+        sol_keep, h_sol = pinned(np.zeros((8,) + in_e.shape, dtype=np.complex128))
+        go = lambda: lat.cg_multishift_host_vectors(h_sol, h_in_e, links, 0.0025, shifts, 1e-10, 100000)   # noqa: E731
+        ev_ms(torch, go)
+        t_e2e, r_e2e = ev_ms(torch, go)
+        dev = extra["multishift_32x32x32x32"]
+        extra["e2e_multishift"] = {"ms": t_e2e, "iters": int(r_e2e["iters"]), "iter_per_s": r_e2e["iters"] / (t_e2e * 1e-3),
+                                   "device_only_ms": dev["ms"], "overhead_frac": t_e2e / dev["ms"] - 1.0,
+                                   "h2d_bytes": in_e.nbytes, "d2h_bytes": 8 * in_e.nbytes,
+                                   "api": "lqcd_cg_multishift_host_vectors: pinned rhs in, 8 solutions out, links resident"}
+        del sol_keep, h_sol
         # ---- NEXT-3: fermion-force outer products from 8 solutions (n Dslash + 2 outer-product launches)
         xs8 = [lat.new_spinor() for _ in shifts]
         lat.cg_multishift(xs8, d_in_e, links, 0.0025, shifts, 1e-300, 8, raise_on_max_iter=False)
@@ -342,48 +444,104 @@ def run_ours(args):
                                        "frac": by / (t_f * 1e-3) / 1e9 / peak,
                                        "note": "8 x D_oe (1248 B per odd site) + outer products (576 links + 48*8 vectors + 256 B of 8-real force per site)"}
         del xs8, fbuf
-        # ---- NEXT-4: tree-level Symanzik gauge staples (ALU / cache bound: 84 SU(3) products per link)
+        # ---- NEXT-4: tree-level Symanzik gauge staples (ALU bound) against the FP64 rate measured here
+        fp64_peak = lat.measure_fp64_peak()
+        extra["fp64_peak_tflops"] = {"value": fp64_peak, "how": "lqcd_measure_fp64_peak: independent DFMA chains, "
+                                     "num_SMs x 8 CTAs of 256 threads, best of 4 after 2 warm-up launches"}
         sbuf = lat.gauge_staples(links)
         t_s = timed_loop(torch, lambda: lat.gauge_staples(links, out=sbuf), 10, 3, 1, D, device) / 10
-        flop_site = 4 * (84 * 198 + 24 * 36)
-        try:
-            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-                mhz = float(json.load(f)["sm_max_mhz"])
-        except Exception:
-            mhz = 1965.0
-        fp64_peak = 148 * 64 * 2 * mhz * 1e6 / 1e12          # 64 FP64 FMA lanes per SM
-        extra["gauge_staples_f64"] = {"ms": t_s, "ns_per_site": t_s * 1e6 / V, "flop_per_site": flop_site,
-                                      "TFLOPs": flop_site * V / (t_s * 1e-3) / 1e12, "bound": "alu",
-                                      "peak_TFLOPs": fp64_peak, "frac": flop_site * V / (t_s * 1e-3) / 1e12 / fp64_peak,
-                                      "note": "2 plaquette + 6 rectangle paths per nu, c0 = 5/3, c1 = -1/12"}
+        variant = lat.get_option("staples_variant")
+        flop_def = 4 * (84 * 198 + 24 * 36)                     # the definition: 84 products + 24 scaled adds per link
+        flop_exec = 4 * STAPLES_EXEC_FLOP_PER_LINK[variant]      # what the default variant executes
+        extra["gauge_staples_f64"] = {"ms": t_s, "ns_per_site": t_s * 1e6 / V, "bound": "alu", "peak_TFLOPs": fp64_peak,
+                                      "flop_per_site_definition": flop_def, "flop_per_site_executed": flop_exec,
+                                      "TFLOPs_definition": flop_def * V / (t_s * 1e-3) / 1e12,
+                                      "TFLOPs_executed": flop_exec * V / (t_s * 1e-3) / 1e12,
+                                      "frac": flop_exec * V / (t_s * 1e-3) / 1e12 / fp64_peak,
+                                      "frac_by_definition_count": flop_def * V / (t_s * 1e-3) / 1e12 / fp64_peak,
+                                      "variant": variant,
+                                      "note": "2 plaquette + 6 rectangle paths per nu, c0 = 5/3, c1 = -1/12; frac = EXECUTED "
+                                              "flops / measured FP64 peak"}
         del sbuf
+        cfg2 = cfg4 = None
+        if not args.quick:
+            # ---- BASELINE.json configs[1]: CG at 16^4 to tolerance (L2-resident: launch-latency bound) ----
+            d2 = (16, 16, 16, 16)
+            r2 = np.random.default_rng(2)
+            U2 = gen.smooth_links(d2, 0.3, r2)
+            b2 = gen.gaussian_half_spinor(d2, r2)
+            l2 = L.Lattice(d2, device=local_rank)
+            extra["cg_16x16x16x16"] = dict(
+                solve_to_tolerance(torch, l2, l2.pack_links(U2), l2.pack_spinor(b2, L.EVEN), [0.0], 0.01, 1e-10, peak),
+                note="BASELINE.json configs[1]: m = 0.01, eps 0.3, seed 2, tol 1e-10; links 37.7 MB fit L2: not an HBM figure")
+            l2.close()
+            cfg2 = (d2, U2, b2, 0.01, 1e-10)
+            # ---- BASELINE.json configs[3], first lattice: 24^3 x 48 to tolerance ---------------------------
+            d4 = (24, 24, 24, 48)
+            r4 = np.random.default_rng(4)
+            U4 = gen.smooth_links(d4, 0.3, r4)
+            b4 = gen.gaussian_half_spinor(d4, r4)
+            l4 = L.Lattice(d4, device=local_rank)
+            extra["multishift_24x24x24x48"] = dict(
+                solve_to_tolerance(torch, l4, l4.pack_links(U4), l4.pack_spinor(b4, L.EVEN), shifts, 0.0025, 1e-10, peak, MS8_BYTES),
+                note="BASELINE.json configs[3]: 8 shifts 1e-4..1, m = 0.0025, eps 0.3, seed 4, tol 1e-10 per shift")
+            l4.close()
+            cfg4 = (d4, U4, b4, 0.0025, 1e-10, shifts)
+            # ---- BASELINE.json configs[4]: large-volume Dslash, fp64 and fp32 (eps 0.5, seed 5) ------------
+            d48, d64 = (48, 48, 48, 48), (64, 64, 64, 16)
+            r5 = np.random.default_rng(5)
+            U48 = gen.smooth_links(d48, 0.5, r5)
+            for dims_l, name in ((d48, "48x48x48x48"), (d64, "64x64x64x16")):
+                Vl = gen.volume(dims_l)
+                # the generator draws link by link in canonical order, so the first Vl sites of the 48^4 field ARE
+                # the field smooth_links(dims_l, 0.5, seed 5) would produce (bit for bit)
+                Ul = U48[:Vl]
+                rs = np.random.default_rng(55)
+                ie, io = gen.gaussian_half_spinor(dims_l, rs), gen.gaussian_half_spinor(dims_l, rs)
+                for prec, pname in ((L.F64, "f64"), (L.F32, "f32")):
+                    for recon, rn in ((L.RECON_18, 18), (L.RECON_12, 12)):
+                        extra[f"dslash_{name}_{pname}_{rn}real"] = dslash_rate(torch, L, D, gen, dims_l, Ul, ie, io, prec, recon,
+                                                                             peak, device, n=60)
+            del U48
         # ---- CPU oracle beside it -------------------------------------------------------------
         psi = np.zeros((V, 3), dtype=np.complex128)
         psi[gen.half_index_of_parity(DIMS, 0)] = in_e
         psi[gen.half_index_of_parity(DIMS, 1)] = in_o
         cpu_ns, reps, cores = cpu_oracle_dslash(U, psi, min_seconds=args.cpu_seconds)
+        cpu = {"value": cpu_ns, "unit": "ns/site", "cores": cores, "kind": "oracle",
+               "sample": f"{reps} full-lattice applications of oracle_dirac_full at 32^4"}
+        if cfg2 is not None:
+            cpu["solver"] = cpu_oracle_solvers(gen, cfg2, cfg4, 40)
+            cpu["solver"]["note"] = (f"same oracle, same inputs as extra.cg_16x16x16x16 / extra.multishift_24x24x24x48, {cores} threads "
+                                     "on the site loop of the operator (reductions and vector updates are the oracle's plain serial loops)")
         line = {
             "metric": "dslash_ns_per_site", "value": ns_site, "unit": "ns/site", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": dict(workload_config(), parallelism=f"replicas x{world} (no collective)"),
-            "GFLOPs": FLOP_PER_SITE * V * world / (ms / args.steps * 1e-3) / 1e9,
+            "data": "synthetic", "config": workload_config(world),
+            "applications_timed": apps, "pairs_per_step": k,
+            "GFLOPs": FLOP_PER_SITE * Vh * world / (us_launch * 1e-6) / 1e9,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_DRAM_TRAFFIC_BYTES, "traffic_source": "profiles/ncu_dslash_r1d.md (ncu --set full, per launch)",
-                         "peak_source": peak_src, "kernel": "dslash_kernel<double,0,0,0,2,0>",
+                         "traffic": traffic["dram_bytes"], "traffic_source": traffic.get("source"),
+                         "traffic_commit": traffic.get("commit"),
+                         "frac_by_ncu_traffic": traffic["dram_bytes"] / (us_launch * 1e-6) / 1e9 / peak,
+                         "peak_source": peak_src, "kernel": kernel,
+                         "peak_note": "the peak is a 50 %-write copy; this kernel is 96 % reads, so frac may exceed 1",
                          "bytes_per_launch": BYTES_PER_SITE[("f64", 18)] * Vh, "us_per_launch": us_launch,
                          "frac_of_nominal_8TBs": achieved / 8000.0},
-            "e2e": {"value": e2e_ms * 1e6 / (e2e_steps * V * world), "unit": "ns/site", "steps": e2e_steps,
+            "e2e": {"value": e2e_ms * 1e6 / (e2e_steps * E2E_PAIRS * V * world), "unit": "ns/site", "steps": e2e_steps,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "api": "lqcd_dslash_host_vectors x2 per step: pinned canonical host vectors in and out, links resident "
+                    "api": f"lqcd_dslash_host_vectors_batch, one call of {2 * E2E_PAIRS} applications per step: pinned canonical "
+                           "host vectors in and out, uploads / kernels / downloads pipelined on three streams, links resident "
                            "(the operator; uploaded once per configuration, PAPER.md:276)",
+                    "one_call_per_application": {"value": ser_ms * 1e6 / (ser_steps * V * world), "unit": "ns/site", "steps": ser_steps,
+                                                 "api": "lqcd_dslash_host_vectors x2 per step (upload, compute, download in sequence)"},
                     "cold_links": {"value": cold_ms * 1e6 / (cold_steps * V * world), "unit": "ns/site", "steps": cold_steps,
                                    "h2d_bytes_per_step": 2 * (U.nbytes + in_e.nbytes), "d2h_bytes_per_step": 2 * in_e.nbytes,
                                    "api": "lqcd_dslash_host x2 per step: the canonical link field is uploaded and packed in every call"}},
             "gpu_launches": launches,
             "clocks": clocks,
-            "cpu_baseline": {"value": cpu_ns, "unit": "ns/site", "cores": cores, "kind": "oracle",
-                             "sample": f"{reps} full-lattice applications of oracle_dirac_full at 32^4"},
+            "cpu_baseline": cpu,
             "extra": extra,
         }
     lat.close()
@@ -393,13 +551,38 @@ def run_ours(args):
         print(json.dumps(line), flush=True)
 
 
+# flops per LINK each staples variant executes: SU(3) product = 198, scaled add = 36
+STAPLES_EXEC_FLOP_PER_LINK = {0: 84 * 198 + 24 * 36, 1: 3 * (22 * 198 + 10 * 36)}
+
+
+def dslash_rate(torch, L, D, gen, dims, U, in_e, in_o, prec, recon, peak, device, n=100):
+    """ns/site, GB/s, fraction of the copy peak of one Dslash variant (alternating parities, fixed inputs)."""
+    pname, rn = ("f64" if prec == L.F64 else "f32"), (18 if recon == L.RECON_18 else 12)
+    Vh = gen.volume(dims) // 2
+    lt = L.Lattice(dims, prec=prec, recon=recon, device=device.index)
+    lk = lt.pack_links(U)
+    a, b_, o1, o2 = lt.pack_spinor(in_e, 0), lt.pack_spinor(in_o, 1), lt.new_spinor(), lt.new_spinor()
+
+    def st():
+        lt.dslash(L.ODD, o1, a, lk)
+        lt.dslash(L.EVEN, o2, b_, lk)
+    t = timed_loop(torch, st, n, 5, 1, D, device)
+    us = t * 1e3 / (2 * n)
+    gbs = BYTES_PER_SITE[(pname, rn)] * Vh / (us * 1e-6) / 1e9
+    lt.close()
+    return {"ns_per_site": us * 1e3 / Vh, "us_per_launch": us, "GBs": gbs, "frac": gbs / peak,
+            "GFLOPs": FLOP_PER_SITE * Vh / (us * 1e-6) / 1e9, "dims": list(dims)}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=1000)
-    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=10.0, dest="cpu_seconds")
+    ap.add_argument("--quick", action="store_true",
+                    help="skip the extras that need other lattices (configs[1], [3] at 24^3 x 48, [4]) and their CPU legs")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

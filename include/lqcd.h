@@ -87,6 +87,9 @@ const char *lqcd_last_error(const lqcd_ctx *ctx);
 /*
  * Private tuning knobs (block sizes, layout variant, cache policy); see DESIGN.md "Tuning".
  * Unknown names -> LQCD_ERR_ARG.  "layout" may only be changed before any field is packed.
+ * Side effect of "l2_persist" > 0: the device-wide persisting-L2 limit is raised and an access-policy window
+ * is set on the context's stream; both are restored to the values found when the option is cleared, the
+ * workspace changes or the context is destroyed.
  */
 int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value);
 long lqcd_get_option(const lqcd_ctx *ctx, const char *name); /* -1 if unknown */
@@ -142,7 +145,9 @@ int lqcd_cg(lqcd_ctx *ctx, void *x_e, const void *b_e, const void *links, double
  *   iters         host, out: total iterations (may be NULL)
  *   conv_iter     host, out [nshift]: iteration at which each shift froze (may be NULL)
  *   rel_resid     host, out [nshift]: TRUE residuals at exit (may be NULL)
- * blocking.  Error behaviour as lqcd_cg; a negative shift is LQCD_ERR_ARG.
+ * blocking.  Error behaviour as lqcd_cg; a negative shift is LQCD_ERR_ARG.  Also LQCD_ERR_ARG (before any
+ * launch): a solution vector that is null, not 16-byte aligned, or overlaps rhs, another solution, the
+ * workspace or the link field (the kernels assume distinct 16-byte aligned operands).
  */
 int lqcd_cg_multishift(lqcd_ctx *ctx, int nshift, const double *shifts, const void *rhs_e,
                        void *const *solutions_e, const void *links, double mass, double tol,
@@ -283,11 +288,34 @@ int lqcd_dslash_host(lqcd_ctx *ctx, int parity, void *out_host /* c128 [V/2][3] 
  * only the input and output vectors cross the bus.  blocking. */
 int lqcd_dslash_host_vectors(lqcd_ctx *ctx, int parity, void *out_host /* c128 [V/2][3] */,
                              const void *in_host /* c128 [V/2][3] */, const void *links_native_dev);
+/* n applications outs_host[j] = D ins_host[j] (output parity parities[j]) in ONE pipelined call: uploads,
+ * pack -> Dslash -> unpack, and downloads run on three streams chained by events with double-buffered
+ * staging, so the download of application j overlaps the upload of application j+1 (PCIe is full duplex).
+ * Host buffers should be pinned (pageable memory works but serialises the copies).  outs/ins: host arrays
+ * of n host pointers (c128 [V/2][3] each); an output may not alias any input.  blocking. */
+int lqcd_dslash_host_vectors_batch(lqcd_ctx *ctx, int n, const int *parities, void *const *outs_host,
+                                   const void *const *ins_host, const void *links_native_dev);
+/* lqcd_cg_multishift on host vectors with the link field resident in native form (the operator is uploaded
+ * once per gauge configuration): rhs up, nshift solutions down, the 10^2-10^3 operator
+ * applications in between (PAPER.md:173 fn. c) never leave the device.  Needs the workspace of
+ * lqcd_workspace_bytes(ctx, nshift).  blocking; errors as lqcd_cg_multishift. */
+int lqcd_cg_multishift_host_vectors(lqcd_ctx *ctx, int nshift, const double *shifts,
+                                    const void *rhs_host /* c128 [V/2][3] */,
+                                    void *solutions_host /* c128 [nshift][V/2][3] */,
+                                    const void *links_native_dev, double mass, double tol, int max_iter,
+                                    int *iters, int *conv_iter, double *rel_resid);
 int lqcd_cg_multishift_host(lqcd_ctx *ctx, int nshift, const double *shifts,
                             const void *rhs_host /* c128 [V/2][3] */,
                             void *solutions_host /* c128 [nshift][V/2][3] */,
                             const void *links_host, double mass, double tol, int max_iter,
                             int *iters, int *conv_iter, double *rel_resid);
+
+/*
+ * Measurement helper (no arithmetic of the method): attainable FP64 FMA rate of the device in TFLOP/s, from a
+ * kernel of independent DFMA chains on the context's stream -- the roofline denominator of the ALU-bound
+ * gauge-staples kernel (bench.py extra.fp64_peak_tflops).  tflops: host, out.  blocking.
+ */
+int lqcd_measure_fp64_peak(lqcd_ctx *ctx, double *tflops);
 
 #ifdef __cplusplus
 }

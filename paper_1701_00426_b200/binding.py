@@ -75,6 +75,9 @@ _sig = {
     "lqcd_dslash_host": (_i, [_vp, _i, _vp, _vp, _vp]),
     "lqcd_dslash_host_vectors": (_i, [_vp, _i, _vp, _vp, _vp]),
     "lqcd_cg_multishift_host": (_i, [_vp, _i, _pd, _vp, _vp, _vp, _d, _d, _i, _pi, _pi, _pd]),
+    "lqcd_dslash_host_vectors_batch": (_i, [_vp, _i, _pi, C.POINTER(_vp), C.POINTER(_vp), _vp]),
+    "lqcd_cg_multishift_host_vectors": (_i, [_vp, _i, _pd, _vp, _vp, _vp, _d, _d, _i, _pi, _pi, _pd]),
+    "lqcd_measure_fp64_peak": (_i, [_vp, _pd]),
 }
 for _name, (_res, _args) in _sig.items():
     _f = getattr(lib, _name)
@@ -170,7 +173,8 @@ class Lattice:
     def _to_dev(self, arr):
         import numpy as np
         a = np.ascontiguousarray(arr, dtype=np.complex128)
-        return self.torch.from_numpy(a.view(np.float64).reshape(-1)).to(self.device)
+        with self.torch.cuda.stream(self.stream):      # the upload is ordered with the context's kernels
+            return self.torch.from_numpy(a.view(np.float64).reshape(-1)).to(self.device)
 
     def pack_links(self, U):
         """U: complex128 [V][4][3][3] (numpy) -> native device buffer."""
@@ -347,3 +351,33 @@ class Lattice:
                                                      max_iter, C.byref(iters), conv, res.ctypes.data_as(_pd)),
                          allow=() if raise_on_max_iter else (ERR_NOT_CONVERGED,))
         return dict(iters=iters.value, conv_iter=np.array(list(conv)), rel_resid=res, converged=(rc == OK))
+
+    def dslash_host_vectors_batch(self, parities, outs_host, ins_host, links):
+        """n applications on host vectors in one pipelined call (uploads, compute and downloads overlap)."""
+        n = len(parities)
+        assert len(outs_host) == n and len(ins_host) == n
+        par = (C.c_int * n)(*[int(p) for p in parities])
+        outs = (_vp * n)(*[o.ctypes.data for o in outs_host])
+        ins = (_vp * n)(*[i.ctypes.data for i in ins_host])
+        self._check(lib.lqcd_dslash_host_vectors_batch(self._ctx, n, par, outs, ins, _vp(links.data_ptr())))
+
+    def cg_multishift_host_vectors(self, sol_host, rhs_host, links, mass, shifts, tol, max_iter, raise_on_max_iter=True):
+        """as cg_multishift_host with the links resident on the device in native form."""
+        import numpy as np
+        sh = np.ascontiguousarray(shifts, dtype=np.float64)
+        n = sh.size
+        self.ensure_workspace(n)
+        iters = C.c_int(0)
+        conv = (C.c_int * n)()
+        res = np.zeros(n)
+        rc = self._check(lib.lqcd_cg_multishift_host_vectors(self._ctx, n, sh.ctypes.data_as(_pd), _vp(rhs_host.ctypes.data),
+                                                             _vp(sol_host.ctypes.data), _vp(links.data_ptr()), mass, tol,
+                                                             max_iter, C.byref(iters), conv, res.ctypes.data_as(_pd)),
+                         allow=() if raise_on_max_iter else (ERR_NOT_CONVERGED,))
+        return dict(iters=iters.value, conv_iter=np.array(list(conv)), rel_resid=res, converged=(rc == OK))
+
+    def measure_fp64_peak(self):
+        """attainable FP64 FMA rate in TFLOP/s (measurement helper; blocking)."""
+        v = C.c_double(0.0)
+        self._check(lib.lqcd_measure_fp64_peak(self._ctx, C.byref(v)))
+        return v.value

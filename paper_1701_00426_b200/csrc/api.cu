@@ -102,6 +102,9 @@ extern "C" int lqcd_create(lqcd_ctx **out, const int dims[4], int prec, int reco
         (e = cudaMemset(c->d_state, 0, sizeof(SolverState))) != cudaSuccess) {
         int rc = lqcd_check_cuda(NULL, e, "lqcd_create: allocating solver state");
         cudaFree(c->d_state); cudaFree(c->d_partials); if (c->h_flag) cudaFreeHost(c->h_flag);
+        if (c->ev[0]) cudaEventDestroy(c->ev[0]);
+        if (c->ev[1]) cudaEventDestroy(c->ev[1]);
+        if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
         free(c);
         return rc;
     }
@@ -121,6 +124,9 @@ extern "C" int lqcd_destroy(lqcd_ctx *ctx)
     cudaEventDestroy(ctx->ev[0]);
     cudaEventDestroy(ctx->ev[1]);
     cudaFree(ctx->stage);
+    if (ctx->h2d_stream) cudaStreamDestroy(ctx->h2d_stream);
+    if (ctx->d2h_stream) cudaStreamDestroy(ctx->d2h_stream);
+    for (int k = 0; k < 3; ++k) for (int j = 0; j < 2; ++j) if (ctx->pipe_ev[k][j]) cudaEventDestroy(ctx->pipe_ev[k][j]);
     if (ctx->chunk_exec) cudaGraphExecDestroy(ctx->chunk_exec);
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     free(ctx);
@@ -205,11 +211,17 @@ static void clear_l2_window(lqcd_ctx *ctx)
     v.accessPolicyWindow.num_bytes = 0;
     v.accessPolicyWindow.hitProp = cudaAccessPropertyNormal;
     v.accessPolicyWindow.missProp = cudaAccessPropertyNormal;
+    // put back what apply_l2_window found (the stream may be shared and the carve-out is device-wide: other
+    // contexts or frameworks may have set their own)
+    if (ctx->l2_saved) v = ctx->l2_prev_attr;
     if (cudaStreamSetAttribute(ctx->stream, cudaStreamAttributeAccessPolicyWindow, &v) != cudaSuccess) cudaGetLastError();
-    if (cudaCtxResetPersistingL2Cache() != cudaSuccess) cudaGetLastError();
-    // give the carve-out back: a persisting-L2 limit left at its maximum keeps 2/3 of the L2 away from
-    // every later kernel of the process (measured: CG at 32^3 x 8 89.8 instead of 64 us per iteration)
-    if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, 0) != cudaSuccess) cudaGetLastError();
+    // a persisting-L2 limit left at its maximum keeps 2/3 of the L2 away from every later kernel of the
+    // process (measured: CG at 32^3 x 8 89.8 instead of 64 us per iteration): restore the previous limit.
+    // Lines of OUR window that are still marked persisting are demoted only when nobody else had a
+    // carve-out (previous limit 0); otherwise they age out by themselves.
+    if (ctx->l2_saved && ctx->l2_prev_limit == 0 && cudaCtxResetPersistingL2Cache() != cudaSuccess) cudaGetLastError();
+    if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, ctx->l2_saved ? ctx->l2_prev_limit : 0) != cudaSuccess) cudaGetLastError();
+    ctx->l2_saved = 0;
     ctx->l2_window_bytes = 0;
 }
 
@@ -227,7 +239,16 @@ static void apply_l2_window(lqcd_ctx *ctx)
     if (want > ctx->ws_bytes) want = ctx->ws_bytes;
     size_t win = want < (size_t)max_window ? want : (size_t)max_window;
     if (max_persist <= 0 || win == 0) return;
-    if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)max_persist) != cudaSuccess) { cudaGetLastError(); return; }
+    // remember the device limit and the stream's window as we found them (restored by clear_l2_window)
+    ctx->l2_prev_limit = 0;
+    memset(&ctx->l2_prev_attr, 0, sizeof(ctx->l2_prev_attr));
+    if (cudaDeviceGetLimit(&ctx->l2_prev_limit, cudaLimitPersistingL2CacheSize) != cudaSuccess) { cudaGetLastError(); ctx->l2_prev_limit = 0; }
+    if (cudaStreamGetAttribute(ctx->stream, cudaStreamAttributeAccessPolicyWindow, &ctx->l2_prev_attr) != cudaSuccess) {
+        cudaGetLastError();
+        memset(&ctx->l2_prev_attr, 0, sizeof(ctx->l2_prev_attr));
+    }
+    ctx->l2_saved = 1;
+    if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)max_persist) != cudaSuccess) { cudaGetLastError(); ctx->l2_saved = 0; return; }
     cudaStreamAttrValue v;
     memset(&v, 0, sizeof(v));
     v.accessPolicyWindow.base_ptr = ctx->ws;
@@ -235,7 +256,12 @@ static void apply_l2_window(lqcd_ctx *ctx)
     v.accessPolicyWindow.hitRatio = win <= (size_t)max_persist ? 1.0f : (float)max_persist / (float)win;
     v.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
     v.accessPolicyWindow.missProp = ctx->l2_persist == 1 ? cudaAccessPropertyStreaming : cudaAccessPropertyNormal;
-    if (cudaStreamSetAttribute(ctx->stream, cudaStreamAttributeAccessPolicyWindow, &v) != cudaSuccess) { cudaGetLastError(); return; }
+    if (cudaStreamSetAttribute(ctx->stream, cudaStreamAttributeAccessPolicyWindow, &v) != cudaSuccess) {
+        cudaGetLastError();
+        if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, ctx->l2_prev_limit) != cudaSuccess) cudaGetLastError();
+        ctx->l2_saved = 0;
+        return;
+    }
     ctx->l2_window_bytes = (long)win;
     ctx->l2_max_persist = max_persist;
 }
@@ -348,10 +374,11 @@ extern "C" int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_pari
                              lqcd_allreduce_fn allreduce, void *user)
 {
     int rc = enter(ctx); if (rc) return rc;
+    // every argument is validated before any field of the context changes
     REQUIRE(solve_parity == 0 || solve_parity == 1, "lqcd_set_slab: solve_parity %d", solve_parity);
-    ctx->solve_parity = solve_parity;
     REQUIRE(0 <= x3_lo && x3_lo < x3_hi && x3_hi <= ctx->g.N3, "lqcd_set_slab: bad slice range [%d,%d)", x3_lo, x3_hi);
     REQUIRE((halo == NULL) == (allreduce == NULL), "lqcd_set_slab: give both hooks or neither");
+    ctx->solve_parity = solve_parity;
     ctx->x3_lo = x3_lo; ctx->x3_hi = x3_hi;
     ctx->halo_fn = halo; ctx->allreduce_fn = allreduce; ctx->comm_user = user;
     if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }

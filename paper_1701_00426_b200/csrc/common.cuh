@@ -224,6 +224,9 @@ struct lqcd_ctx {
     int link_pad;          // extra sites between link planes
     int l2_persist;        // 1: persisting-L2 access-policy window over the CG vectors
     long l2_window_bytes, l2_max_persist;
+    int l2_saved;          // apply_l2_window saved the device limit / stream window it found:
+    size_t l2_prev_limit;
+    cudaStreamAttrValue l2_prev_attr;
     int l2_hints;          // 0: ld.cs / plain, 1: explicit L2 evict_first / evict_last hints
     int dslash_block;      // threads per CTA of the Dslash kernel
     int dslash_minblocks;  // launch-bounds variant (occupancy target)
@@ -259,6 +262,10 @@ struct lqcd_ctx {
     int *h_flag;           // pinned host words (two poll slots)
     cudaEvent_t ev[2];
     void *stage; size_t stage_bytes;   // device staging of the *_host entry points (grow-only)
+    // copy pipeline of lqcd_dslash_host_vectors_batch (created on first use): uploads and downloads run on
+    // their own streams so that the D2H of application n overlaps the H2D of application n+1
+    cudaStream_t h2d_stream, d2h_stream;
+    cudaEvent_t pipe_ev[3][2];         // [0: upload done, 1: compute done, 2: download done][slot]
     int hist_n;
     double h_hist[3][LQCD_HIST];
     int last_dslash_grid;  // CTAs of the most recent Dslash launch (= number of <p,q> partials)

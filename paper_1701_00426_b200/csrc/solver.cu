@@ -523,6 +523,32 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     return LQCD_OK;
 }
 
+// Argument hygiene shared by the solver entry points (before any launch): the vector kernels declare their
+// operands __restrict__ and use 16-byte loads, so a buffer that aliases another operand, the workspace or
+// the link field would corrupt the solve silently and a misaligned one would fault asynchronously.
+static int check_solver_buffers(lqcd_ctx *ctx, const char *who, int n_out, void *const *outs, const void *rhs, const void *links)
+{
+    const uintptr_t vb = (uintptr_t)lqcd_spinor_bytes(ctx), lb = (uintptr_t)lqcd_links_bytes(ctx);
+    const uintptr_t ws0 = (uintptr_t)ctx->ws, ws1 = ws0 + ctx->ws_bytes;
+    const uintptr_t r0 = (uintptr_t)rhs, l0 = (uintptr_t)links;
+    if ((r0 & 15) || (l0 & 15)) return lqcd_fail(ctx, LQCD_ERR_ARG, "%s: rhs / links not 16-byte aligned", who);
+    if (r0 < ws1 && r0 + vb > ws0) return lqcd_fail(ctx, LQCD_ERR_ARG, "%s: rhs lies inside the workspace", who);
+    if (l0 < ws1 && l0 + lb > ws0) return lqcd_fail(ctx, LQCD_ERR_ARG, "%s: links overlap the workspace", who);
+    for (int i = 0; i < n_out; ++i) {
+        const uintptr_t a = (uintptr_t)outs[i];
+        if (!a) return lqcd_fail(ctx, LQCD_ERR_ARG, "%s: output vector %d is null", who, i);
+        if (a & 15) return lqcd_fail(ctx, LQCD_ERR_ARG, "%s: output vector %d is not 16-byte aligned", who, i);
+        if (a < r0 + vb && a + vb > r0) return lqcd_fail(ctx, LQCD_ERR_ARG, "%s: output vector %d aliases rhs", who, i);
+        if (a < ws1 && a + vb > ws0) return lqcd_fail(ctx, LQCD_ERR_ARG, "%s: output vector %d lies inside the workspace", who, i);
+        if (a < l0 + lb && a + vb > l0) return lqcd_fail(ctx, LQCD_ERR_ARG, "%s: output vector %d overlaps the link field", who, i);
+        for (int j = 0; j < i; ++j) {
+            const uintptr_t b = (uintptr_t)outs[j];
+            if (a < b + vb && a + vb > b) return lqcd_fail(ctx, LQCD_ERR_ARG, "%s: output vectors %d and %d overlap", who, j, i);
+        }
+    }
+    return LQCD_OK;
+}
+
 extern "C" int lqcd_cg_multishift(lqcd_ctx *ctx, int nshift, const double *shifts, const void *rhs_e,
                                   void *const *solutions_e, const void *links, double mass, double tol,
                                   int max_iter, int *iters, int *conv_iter, double *rel_resid)
@@ -541,6 +567,7 @@ extern "C" int lqcd_cg_multishift(lqcd_ctx *ctx, int nshift, const double *shift
     if (!ctx->ws) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "no workspace set");
     if (ctx->ws_bytes < lqcd_workspace_bytes(ctx, nshift))
         return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "workspace %zu bytes < %zu needed for %d shifts", ctx->ws_bytes, lqcd_workspace_bytes(ctx, nshift), nshift);
+    if ((rc = check_solver_buffers(ctx, "lqcd_cg_multishift", nshift, solutions_e, rhs_e, links))) return rc;
     if (ctx->prec == LQCD_F64)
         return solve_t<double>(ctx, nshift, shifts, rhs_e, solutions_e, links, mass, tol, max_iter, iters, conv_iter, rel_resid);
     return solve_t<float>(ctx, nshift, shifts, rhs_e, solutions_e, links, mass, tol, max_iter, iters, conv_iter, rel_resid);
@@ -566,6 +593,7 @@ extern "C" int lqcd_rational_apply(lqcd_ctx *ctx, int nshift, const double *shif
     if (!ctx->ws) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "no workspace set");
     if (ctx->ws_bytes < lqcd_workspace_bytes(ctx, nshift))
         return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "workspace %zu bytes < %zu needed for %d shifts", ctx->ws_bytes, lqcd_workspace_bytes(ctx, nshift), nshift);
+    { void *ys[1] = { y_e }; if ((rc = check_solver_buffers(ctx, "lqcd_rational_apply", 1, ys, rhs_e, links))) return rc; }
     if (ctx->prec == LQCD_F64)
         return solve_t<double>(ctx, nshift, shifts, rhs_e, NULL, links, mass, tol, max_iter, iters, conv_iter, NULL, y_e, c0, coeffs);
     return solve_t<float>(ctx, nshift, shifts, rhs_e, NULL, links, mass, tol, max_iter, iters, conv_iter, NULL, y_e, c0, coeffs);

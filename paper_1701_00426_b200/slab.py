@@ -193,14 +193,20 @@ class SlabLattice:
         return t
 
     # -- hooks called from inside liblqcd_b200.so (lqcd_set_slab) ---------------------------------
+    # The library's kernels run on the stream captured when the Lattice was created; torch copies and
+    # collectives run on torch's CURRENT stream.  Every piece of communication is therefore issued under
+    # `with torch.cuda.stream(lat.stream)`, so that it stays ordered with the kernels even when the caller
+    # has entered another stream context.
     def _halo_start(self, vec_ptr):
         g, lat = self.geo, self.lat
         lat.halo_pack_faces(self._send_up, self._send_down, vec_ptr, g.sign_send_up, g.sign_send_down)
-        return self.comm.exchange_start(self._send_up, self._send_down, self._from_down, self._from_up)
+        with self.torch.cuda.stream(lat.stream):
+            return self.comm.exchange_start(self._send_up, self._send_down, self._from_down, self._from_up)
 
     def _halo_finish(self, vec_ptr, handle):
         g, lat = self.geo, self.lat
-        self.comm.exchange_wait(handle)
+        with self.torch.cuda.stream(lat.stream):
+            self.comm.exchange_wait(handle)
         lat.halo_unpack_ghosts(vec_ptr, self._from_down, self._from_up)
 
     def _halo_hook(self, user, vec_ptr, parity):
@@ -213,8 +219,9 @@ class SlabLattice:
 
     def _allreduce_hook(self, user, dev_ptr, count):
         try:
-            t = self.torch.as_tensor(_RawDeviceDoubles(dev_ptr, count), device=self.lat.device)
-            self.comm.allreduce_sum(t)
+            with self.torch.cuda.stream(self.lat.stream):
+                t = self.torch.as_tensor(_RawDeviceDoubles(dev_ptr, count), device=self.lat.device)
+                self.comm.allreduce_sum(t)
             return 0
         except Exception as e:
             self.hook_error = e

@@ -208,8 +208,51 @@ def staples(dims_list, out):
                     lat.close()
 
 
+_UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+
+
+def traffic_from_ncu(csv_path, commit, source):
+    """Write profiles/traffic.json from `ncu -i X.ncu-rep --page raw --csv > csv_path` (an `ncu --set full`
+    capture): per kernel (demangled name, template arguments without spaces), the mean over the captured
+    launches of dram__bytes_read.sum + dram__bytes_write.sum, with the commit the capture was taken at.
+    bench.py reads the entry of the kernel it launches and refuses a file that lacks it."""
+    import csv
+    import re
+    rows = list(csv.reader(open(csv_path)))
+    hdr, units = rows[0], rows[1]
+    col = {n: hdr.index(n) for n in ("Kernel Name", "dram__bytes_read.sum", "dram__bytes_write.sum", "gpu__time_duration.sum")}
+    acc = {}
+    for r in rows[2:]:
+        m = re.match(r"(?:void )?([A-Za-z_0-9]+<[^(]*>|[A-Za-z_0-9]+)\(", r[col["Kernel Name"]])
+        if not m:
+            continue
+        name = m.group(1).replace(" ", "")
+        rd = float(r[col["dram__bytes_read.sum"]]) * _UNIT[units[col["dram__bytes_read.sum"]]]
+        wr = float(r[col["dram__bytes_write.sum"]]) * _UNIT[units[col["dram__bytes_write.sum"]]]
+        acc.setdefault(name, []).append((rd, wr, float(r[col["gpu__time_duration.sum"]])))
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(path) as f:
+            table = json.load(f)
+    except Exception:
+        table = {}
+    for name, v in acc.items():
+        n = len(v)
+        table[name] = {"dram_bytes": sum(a + b for a, b, _ in v) / n, "dram_read_bytes": sum(a for a, _, _ in v) / n,
+                       "dram_write_bytes": sum(b for _, b, _ in v) / n, "launches_captured": n,
+                       "ncu_duration_us": sum(t for _, _, t in v) / n, "commit": commit, "source": source}
+    with open(path, "w") as f:
+        json.dump(table, f, indent=1, sort_keys=True)
+        f.write("\n")
+    print(json.dumps({k: table[k] for k in acc}, indent=1))
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--traffic-from-ncu", default=None, metavar="RAW.csv",
+                    help="write profiles/traffic.json from an `ncu --page raw --csv` export (no GPU needed)")
+    ap.add_argument("--commit", default="", help="with --traffic-from-ncu: the commit the capture was taken at")
+    ap.add_argument("--source", default="", help="with --traffic-from-ncu: the profiles/*.md that describes the capture")
     ap.add_argument("--ladder", action="store_true")
     ap.add_argument("--multishift", action="store_true")
     ap.add_argument("--staples", action="store_true", help="NEXT-4 gauge staples timing")
@@ -219,6 +262,9 @@ def main():
     ap.add_argument("--seed", type=int, default=5)
     ap.add_argument("--md", default=None)
     args = ap.parse_args()
+    if args.traffic_from_ncu:
+        traffic_from_ncu(args.traffic_from_ncu, args.commit, args.source)
+        return
     dims_list = None
     if args.dims:
         dims_list = [tuple(int(x) for x in d.split(",")) for d in args.dims.split(";")]

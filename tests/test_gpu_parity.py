@@ -497,6 +497,76 @@ def test_host_entry_points():
     assert abs(res["iters"] - ref["iters"]) <= 2
     for i in range(2):
         assert rel(sol[i], ref["x"][i]) < 1e-6
+    # links resident: rhs up, solutions down
+    sol2 = np.empty_like(sol)
+    res2 = lat.cg_multishift_host_vectors(sol2, phi, lat.pack_links(U), 0.05, shifts, 1e-10, 5000)
+    assert res2["iters"] == res["iters"] and np.array_equal(sol2, sol)
+    lat.close()
+
+
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("n", [1, 2, 5])
+def test_host_batch_pipeline(prec, n):
+    """lqcd_dslash_host_vectors_batch: n applications through the three-stream copy pipeline (double-buffered
+    staging: n = 5 re-uses every slot) = the oracle applied to each input, and bit-identical to one blocking
+    lqcd_dslash_host_vectors call per application."""
+    import torch
+    dims = (8, 6, 4, 10)
+    rng = np.random.default_rng(18)
+    U = gen.smooth_links(dims, 0.4, rng)
+    ins = [gen.gaussian_half_spinor(dims, rng) for _ in range(n)]
+    U, *ins = round_inputs(prec, U, *ins)
+    pars = [(j + 1) % 2 for j in range(n)]
+    lat = make_lattice(dims, prec)
+    links = lat.pack_links(U)
+
+    def pinned(a):
+        t = torch.from_numpy(np.ascontiguousarray(a).view(np.float64).reshape(-1)).pin_memory()
+        return t, t.numpy().view(np.complex128).reshape(a.shape)
+    keep = [pinned(a) for a in ins] + [pinned(np.zeros_like(ins[0])) for _ in range(n)]
+    h_ins, h_outs = [k[1] for k in keep[:n]], [k[1] for k in keep[n:]]
+    for _ in range(2):                                   # second call: slots and events are re-used
+        lat.dslash_host_vectors_batch(pars, h_outs, h_ins, links)
+    for j in range(n):
+        assert rel(h_outs[j], oracle.dslash_half(dims, U, pars[j], ins[j])) < TOL[prec], j
+        one = np.empty_like(ins[j])
+        lat.dslash_host_vectors(pars[j], one, ins[j], links)
+        assert np.array_equal(one, h_outs[j])
+    lat.close()
+
+
+def test_solver_rejects_aliased_and_misaligned_buffers():
+    """Before any launch: outputs that overlap each other, rhs, the workspace or the links, or that are not
+    16-byte aligned, are LQCD_ERR_ARG (the vector kernels assume distinct, aligned operands)."""
+    import paper_1701_00426_b200 as L
+    dims = (4, 4, 4, 4)
+    lat = make_lattice(dims)
+    links = lat.pack_links(gen.unit_links(dims))
+    b = lat.pack_spinor(gen.gaussian_half_spinor(dims, 3), 0)
+    x = lat.new_spinor()
+    lat.ensure_workspace(2)
+    big = lat._buf(2 * lat.spinor_bytes + 64)
+    cases = [([x, x], b), ([x, b], b), ([x, lat._ws[:lat.spinor_bytes]], b), ([x, links[:lat.spinor_bytes]], b),
+             ([x, big[8:8 + lat.spinor_bytes]], b), ([big[:lat.spinor_bytes], big[16:16 + lat.spinor_bytes]], b)]
+    for xs, rhs in cases:
+        with pytest.raises(L.LqcdError) as e:
+            lat.cg_multishift(xs, rhs, links, 0.1, [0.0, 0.5], 1e-8, 10)
+        assert e.value.code == L.ERR_ARG
+    with pytest.raises(L.LqcdError) as e:
+        lat.rational_apply(big[8:8 + lat.spinor_bytes], b, links, 0.1, [0.0, 0.5], 1.0, [1.0, 1.0], 1e-8, 10)
+    assert e.value.code == L.ERR_ARG
+    # a well-formed call still works afterwards
+    res = lat.cg_multishift([x, big[:lat.spinor_bytes]], b, links, 0.1, [0.0, 0.5], 1e-8, 100)
+    assert res["converged"]
+    lat.close()
+
+
+def test_fp64_peak_measurement_is_plausible():
+    """lqcd_measure_fp64_peak (bench.py's denominator for the ALU-bound staples): a B200 does some tens of
+    TFLOP/s in FP64; anything outside 5..100 means the kernel or its flop count is broken."""
+    lat = make_lattice((4, 4, 4, 4))
+    v = lat.measure_fp64_peak()
+    assert 5.0 < v < 100.0, v
     lat.close()
 
 
