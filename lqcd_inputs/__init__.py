@@ -13,6 +13,7 @@ from .fields import (  # noqa: F401
     gaussian_spinor,
     gaussian_half_spinor,
     rhmc_shifts,
+    uniform_backfield,
     site_coords,
     half_index_of_parity,
 )

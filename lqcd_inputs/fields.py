@@ -148,6 +148,15 @@ def gaussian_half_spinor(dims, seed_or_rng) -> np.ndarray:
     return np.ascontiguousarray(g[..., 0] + 1j * g[..., 1])
 
 
+def uniform_backfield(dims, seed_or_rng) -> np.ndarray:
+    """Backfield theta[lex][mu] (the paper's unexplained `backfield` argument of acc_Deo, PAPER.md:320-326;
+    reading R6 of DESIGN.md: a U(1) phase per link): theta ~ U(-pi, pi) independently -- the phase
+    equivalent of Haar-like links; every value of e^{i theta} occurs."""
+    dims = _check_dims(dims)
+    rng = _as_rng(seed_or_rng)
+    return rng.uniform(-np.pi, np.pi, size=(volume(dims), 4))
+
+
 def rhmc_shifts(n: int = 8, lo_exp: float = -4.0, hi_exp: float = 0.0) -> np.ndarray:
     """BASELINE.json config 4: n shifts log-spaced in [10^lo_exp, 10^hi_exp]."""
     if n == 1:

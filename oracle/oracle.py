@@ -49,6 +49,22 @@ _lib.oracle_fermion_force.argtypes = [_i4, C.c_int, _c128, C.c_int, _pd, _c128, 
 _lib.oracle_fermion_force.restype = C.c_int
 _lib.oracle_gauge_staples.argtypes = [_i4, _c128, C.c_double, C.c_double, _c128]
 _lib.oracle_gauge_staples.restype = None
+# *_bf: the same functions with the optional backfield theta[V][4] (float64; NULL = none) after U
+_lib.oracle_dirac_full_bf.argtypes = [_i4, C.c_int, _c128, C.c_void_p, _c128, _c128, C.c_int]
+_lib.oracle_dirac_full_bf.restype = None
+_lib.oracle_dirac_site_bf.argtypes = [_i4, C.c_int, _c128, C.c_void_p, _c128, _i4, _c128]
+_lib.oracle_dirac_site_bf.restype = None
+_lib.oracle_dslash_half_bf.argtypes = [_i4, C.c_int, _c128, C.c_void_p, C.c_int, _c128, _c128]
+_lib.oracle_dslash_half_bf.restype = C.c_int
+_lib.oracle_mdagm_bf.argtypes = [_i4, C.c_int, _c128, C.c_void_p, C.c_double, C.c_double, _c128, _c128]
+_lib.oracle_mdagm_bf.restype = C.c_int
+_lib.oracle_cg_bf.argtypes = [_i4, C.c_int, _c128, C.c_void_p, C.c_double, _c128, _c128, C.c_double, C.c_int,
+                              _pi, _pd, _pd, _pd, _pd, C.c_int]
+_lib.oracle_cg_bf.restype = C.c_int
+_lib.oracle_cg_multishift_bf.argtypes = [_i4, C.c_int, _c128, C.c_void_p, C.c_double, C.c_int, _pd, _c128, _c128,
+                                         C.c_double, C.c_int, _pi, _pi, _pd, _pd, C.c_void_p,
+                                         _pd, _pd, _pd, C.c_int]
+_lib.oracle_cg_multishift_bf.restype = C.c_int
 _lib.oracle_num_threads.restype = C.c_int
 _lib.oracle_set_num_threads.argtypes = [C.c_int]
 
@@ -71,6 +87,21 @@ def _dptr(a):
     return a.ctypes.data_as(_pd)
 
 
+class _Theta:
+    """The optional backfield theta[V][4] (float64) as a void* argument; keeps the array alive."""
+
+    def __init__(self, theta, V):
+        self.a = None
+        if theta is not None:
+            self.a = np.ascontiguousarray(theta, dtype=np.float64)
+            if self.a.shape != (V, 4):
+                raise ValueError(f"backfield must have shape ({V}, 4), got {self.a.shape}")
+
+    @property
+    def ptr(self):
+        return None if self.a is None else C.c_void_p(self.a.ctypes.data)
+
+
 def num_threads() -> int:
     return int(_lib.oracle_num_threads())
 
@@ -79,11 +110,16 @@ def set_num_threads(n: int) -> None:
     _lib.oracle_set_num_threads(int(n))
 
 
-def dirac_full(dims, U, psi, antiperiodic_t=True, which=2):
-    """(D psi)(x) on the whole lattice (which=2) or on one parity (0 even, 1 odd; rest zero)."""
+def dirac_full(dims, U, psi, antiperiodic_t=True, which=2, theta=None):
+    """(D psi)(x) on the whole lattice (which=2) or on one parity (0 even, 1 odd; rest zero).
+    theta: optional backfield [V][4] (every link enters as e^{i theta} U); None calls the plain entry point."""
     n4, V = _dims(dims)
     out = np.zeros((V, 3), dtype=np.complex128)
-    _lib.oracle_dirac_full(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), _arr(psi, (V, 3)), out, which)
+    if theta is None:
+        _lib.oracle_dirac_full(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), _arr(psi, (V, 3)), out, which)
+    else:
+        th = _Theta(theta, V)
+        _lib.oracle_dirac_full_bf(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), th.ptr, _arr(psi, (V, 3)), out, which)
     return out
 
 
@@ -95,11 +131,16 @@ def dirac_range(dims, U, psi, out, lo, hi, antiperiodic_t=True):
     return out
 
 
-def dirac_site(dims, U, psi, x, antiperiodic_t=True):
+def dirac_site(dims, U, psi, x, antiperiodic_t=True, theta=None):
     n4, V = _dims(dims)
     out = np.zeros(3, dtype=np.complex128)
-    _lib.oracle_dirac_site(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), _arr(psi, (V, 3)),
-                           _i4(*[int(c) for c in x]), out)
+    if theta is None:
+        _lib.oracle_dirac_site(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), _arr(psi, (V, 3)),
+                               _i4(*[int(c) for c in x]), out)
+    else:
+        th = _Theta(theta, V)
+        _lib.oracle_dirac_site_bf(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), th.ptr, _arr(psi, (V, 3)),
+                                  _i4(*[int(c) for c in x]), out)
     return out
 
 
@@ -117,23 +158,33 @@ def full_to_half(dims, parity, full):
     return half
 
 
-def dslash_half(dims, U, out_parity, in_half, antiperiodic_t=True):
+def dslash_half(dims, U, out_parity, in_half, antiperiodic_t=True, theta=None):
     """out_parity=0: D_eo in_o (even output); out_parity=1: D_oe in_e (odd output)."""
     n4, V = _dims(dims)
     out = np.empty((V // 2, 3), dtype=np.complex128)
-    rc = _lib.oracle_dslash_half(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), out_parity,
-                                 _arr(in_half, (V // 2, 3)), out)
+    if theta is None:
+        rc = _lib.oracle_dslash_half(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), out_parity,
+                                     _arr(in_half, (V // 2, 3)), out)
+    else:
+        th = _Theta(theta, V)
+        rc = _lib.oracle_dslash_half_bf(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), th.ptr, out_parity,
+                                        _arr(in_half, (V // 2, 3)), out)
     if rc:
         raise MemoryError("oracle_dslash_half")
     return out
 
 
-def mdagm(dims, U, mass, in_e, sigma=0.0, antiperiodic_t=True):
+def mdagm(dims, U, mass, in_e, sigma=0.0, antiperiodic_t=True, theta=None):
     """(m^2 + sigma) in_e - D_eo D_oe in_e."""
     n4, V = _dims(dims)
     out = np.empty((V // 2, 3), dtype=np.complex128)
-    rc = _lib.oracle_mdagm(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), mass, sigma,
-                           _arr(in_e, (V // 2, 3)), out)
+    if theta is None:
+        rc = _lib.oracle_mdagm(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), mass, sigma,
+                               _arr(in_e, (V // 2, 3)), out)
+    else:
+        th = _Theta(theta, V)
+        rc = _lib.oracle_mdagm_bf(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), th.ptr, mass, sigma,
+                                  _arr(in_e, (V // 2, 3)), out)
     if rc:
         raise MemoryError("oracle_mdagm")
     return out
@@ -146,7 +197,7 @@ def reconstruct_row3(U):
     return out
 
 
-def cg(dims, U, mass, b, tol, max_iter, antiperiodic_t=True, hist_len=0):
+def cg(dims, U, mass, b, tol, max_iter, antiperiodic_t=True, hist_len=0, theta=None):
     """Returns dict(x, iters, converged, true_relres, alpha, beta, rnorm)."""
     n4, V = _dims(dims)
     x = np.empty((V // 2, 3), dtype=np.complex128)
@@ -155,16 +206,22 @@ def cg(dims, U, mass, b, tol, max_iter, antiperiodic_t=True, hist_len=0):
     ha = np.zeros(max(hist_len, 1))
     hb = np.zeros(max(hist_len, 1))
     hr = np.zeros(max(hist_len, 1))
-    rc = _lib.oracle_cg(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), mass, _arr(b, (V // 2, 3)), x,
-                        tol, max_iter, C.byref(iters), C.byref(relres),
-                        _dptr(ha), _dptr(hb), _dptr(hr), hist_len)
+    if theta is None:
+        rc = _lib.oracle_cg(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), mass, _arr(b, (V // 2, 3)), x,
+                            tol, max_iter, C.byref(iters), C.byref(relres),
+                            _dptr(ha), _dptr(hb), _dptr(hr), hist_len)
+    else:
+        th = _Theta(theta, V)
+        rc = _lib.oracle_cg_bf(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), th.ptr, mass, _arr(b, (V // 2, 3)), x,
+                               tol, max_iter, C.byref(iters), C.byref(relres),
+                               _dptr(ha), _dptr(hb), _dptr(hr), hist_len)
     if rc < 0:
         raise MemoryError("oracle_cg")
     return dict(x=x, iters=iters.value, converged=(rc == 0), true_relres=relres.value,
                 alpha=ha[:hist_len], beta=hb[:hist_len], rnorm=hr[:hist_len])
 
 
-def cg_multishift(dims, U, mass, shifts, b, tol, max_iter, antiperiodic_t=True, hist_len=0):
+def cg_multishift(dims, U, mass, shifts, b, tol, max_iter, antiperiodic_t=True, hist_len=0, theta=None):
     """Returns dict(x[nshift], iters, converged, conv_iter, true_relres, zeta, r, alpha, beta, rnorm)."""
     n4, V = _dims(dims)
     shifts = np.ascontiguousarray(shifts, dtype=np.float64)
@@ -178,11 +235,19 @@ def cg_multishift(dims, U, mass, shifts, b, tol, max_iter, antiperiodic_t=True, 
     ha = np.zeros(max(hist_len, 1))
     hb = np.zeros(max(hist_len, 1))
     hr = np.zeros(max(hist_len, 1))
-    rc = _lib.oracle_cg_multishift(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), mass, ns, _dptr(shifts),
-                                   _arr(b, (V // 2, 3)), x.reshape(-1), tol, max_iter,
-                                   C.byref(iters), conv, _dptr(relres), _dptr(zeta),
-                                   r.ctypes.data_as(C.c_void_p),
-                                   _dptr(ha), _dptr(hb), _dptr(hr), hist_len)
+    if theta is None:
+        rc = _lib.oracle_cg_multishift(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), mass, ns, _dptr(shifts),
+                                       _arr(b, (V // 2, 3)), x.reshape(-1), tol, max_iter,
+                                       C.byref(iters), conv, _dptr(relres), _dptr(zeta),
+                                       r.ctypes.data_as(C.c_void_p),
+                                       _dptr(ha), _dptr(hb), _dptr(hr), hist_len)
+    else:
+        th = _Theta(theta, V)
+        rc = _lib.oracle_cg_multishift_bf(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), th.ptr, mass, ns, _dptr(shifts),
+                                          _arr(b, (V // 2, 3)), x.reshape(-1), tol, max_iter,
+                                          C.byref(iters), conv, _dptr(relres), _dptr(zeta),
+                                          r.ctypes.data_as(C.c_void_p),
+                                          _dptr(ha), _dptr(hb), _dptr(hr), hist_len)
     if rc == -1:
         raise MemoryError("oracle_cg_multishift")
     if rc == -2:

@@ -27,6 +27,11 @@
  * rational-function sum against dense solves and a partial-fraction identity; the fermion-force
  * outer products against finite differences of the action computed with dense solves; the gauge
  * staples against finite differences of the gauge action, a loop-counting sum rule and covariance.
+ * The optional backfield (U(1) phase per link, the paper's unexplained fourth argument of acc_Deo; *_bf
+ * entry points) is pinned by: theta = 0 reproduces D; the dense matrix built with phased links; the
+ * phases absorbed into the links give the same D through the plain entry points; a constant theta_mu
+ * shifts the free-field momenta, p_mu -> p_mu + theta_mu; a pure-gauge theta is removed by a U(1) gauge
+ * transformation.
  * No function in this file is "parity unpinned".
  *
  * OpenMP is used on the site loop of the operator only, so that bench.py can time the
@@ -78,7 +83,15 @@ static double eta(int mu, const int x[4])
  * x3 = N3-1 and s-_3 = -1 when x3 = 0.  The two hops are separate terms, so N_mu = 2 needs
  * no special case.
  */
-static void dirac_site(const int N[4], int antiperiodic_t, const cplx *U, const cplx *psi,
+/*
+ * Optional `backfield` theta[lex][mu] (NULL: none): the fourth argument of the paper's
+ * acc_Deo(u, out, in, backfield) (Listing 2), a per-link real field ("double_soa") the
+ * paper never explains.  Reading R6 of DESIGN.md: an external U(1) phase -- every link enters D as
+ * e^{i theta_mu(x)} U_mu(x), i.e. the forward hop out of x carries e^{+i theta_mu(x)} and the backward hop
+ * carries (e^{i theta_mu(x-mu)} U_mu(x-mu))^dagger = e^{-i theta_mu(x-mu)} U_mu(x-mu)^dagger.  The phase
+ * multiplies the full 3x3 link (after any third-row reconstruction), never the stored rows.
+ */
+static void dirac_site(const int N[4], int antiperiodic_t, const cplx *U, const double *theta, const cplx *psi,
                        const int x[4], cplx out[3])
 {
     cplx acc[3] = {0.0, 0.0, 0.0};
@@ -103,6 +116,10 @@ static void dirac_site(const int N[4], int antiperiodic_t, const cplx *U, const 
                 fwd += Ufwd[a * 3 + b] * pf[b];
                 bwd += conj(Ubwd[b * 3 + a]) * pb[b];   /* (U^dagger)_{ab} = conj(U_{ba}) */
             }
+            if (theta) {
+                fwd *= cexp(I * theta[lex_of(N, x) * 4 + (size_t)mu]);
+                bwd *= cexp(-I * theta[lex_of(N, xm) * 4 + (size_t)mu]);
+            }
             acc[a] += e * (sp * fwd - sm * bwd);
         }
     }
@@ -111,8 +128,8 @@ static void dirac_site(const int N[4], int antiperiodic_t, const cplx *U, const 
 
 /* Full-lattice D: out(x) = (D psi)(x) on the sites whose parity matches `which`
  * (0 = even only, 1 = odd only, 2 = all); other sites of `out` are left untouched. */
-void oracle_dirac_full(const int N[4], int antiperiodic_t, const cplx *U, const cplx *psi,
-                       cplx *out, int which)
+void oracle_dirac_full_bf(const int N[4], int antiperiodic_t, const cplx *U, const double *theta,
+                          const cplx *psi, cplx *out, int which)
 {
     long long V = (long long)vol(N);
 #pragma omp parallel for schedule(static)
@@ -120,8 +137,14 @@ void oracle_dirac_full(const int N[4], int antiperiodic_t, const cplx *U, const 
         int x[4];
         coords_of(N, (size_t)s, x);
         if (which != 2 && parity_of(x) != which) continue;
-        dirac_site(N, antiperiodic_t, U, psi, x, out + (size_t)s * 3);
+        dirac_site(N, antiperiodic_t, U, theta, psi, x, out + (size_t)s * 3);
     }
+}
+
+void oracle_dirac_full(const int N[4], int antiperiodic_t, const cplx *U, const cplx *psi,
+                       cplx *out, int which)
+{
+    oracle_dirac_full_bf(N, antiperiodic_t, U, NULL, psi, out, which);
 }
 
 /* Sites lex in [lo, hi) only (a bounded sample of a large lattice for bench.py's timed CPU
@@ -133,15 +156,21 @@ void oracle_dirac_range(const int N[4], int antiperiodic_t, const cplx *U, const
     for (long long s = lo; s < hi; ++s) {
         int x[4];
         coords_of(N, (size_t)s, x);
-        dirac_site(N, antiperiodic_t, U, psi, x, out + (size_t)s * 3);
+        dirac_site(N, antiperiodic_t, U, NULL, psi, x, out + (size_t)s * 3);
     }
 }
 
 /* One output site, for sampled parity checks at sizes where the full field is not wanted. */
+void oracle_dirac_site_bf(const int N[4], int antiperiodic_t, const cplx *U, const double *theta,
+                          const cplx *psi, const int x[4], cplx out[3])
+{
+    dirac_site(N, antiperiodic_t, U, theta, psi, x, out);
+}
+
 void oracle_dirac_site(const int N[4], int antiperiodic_t, const cplx *U, const cplx *psi,
                        const int x[4], cplx out[3])
 {
-    dirac_site(N, antiperiodic_t, U, psi, x, out);
+    dirac_site(N, antiperiodic_t, U, NULL, psi, x, out);
 }
 
 /* ---------------------------------------------------------------------------------------
@@ -177,37 +206,49 @@ void oracle_full_to_half(const int N[4], int parity, const cplx *full, cplx *hal
  *   out_parity = 0 (even):  out_e = D_eo in_o      out_parity = 1 (odd):  out_o = D_oe in_e
  * Returns 0, or -1 if scratch memory cannot be allocated.
  */
-int oracle_dslash_half(const int N[4], int antiperiodic_t, const cplx *U, int out_parity,
-                       const cplx *in_half, cplx *out_half)
+int oracle_dslash_half_bf(const int N[4], int antiperiodic_t, const cplx *U, const double *theta, int out_parity,
+                          const cplx *in_half, cplx *out_half)
 {
     size_t V = vol(N);
     cplx *full_in = (cplx *)malloc(V * 3 * sizeof(cplx));
     cplx *full_out = (cplx *)malloc(V * 3 * sizeof(cplx));
     if (!full_in || !full_out) { free(full_in); free(full_out); return -1; }
     oracle_half_to_full(N, 1 - out_parity, in_half, full_in);
-    oracle_dirac_full(N, antiperiodic_t, U, full_in, full_out, out_parity);
+    oracle_dirac_full_bf(N, antiperiodic_t, U, theta, full_in, full_out, out_parity);
     oracle_full_to_half(N, out_parity, full_out, out_half);
     free(full_in);
     free(full_out);
     return 0;
 }
 
+int oracle_dslash_half(const int N[4], int antiperiodic_t, const cplx *U, int out_parity,
+                       const cplx *in_half, cplx *out_half)
+{
+    return oracle_dslash_half_bf(N, antiperiodic_t, U, NULL, out_parity, in_half, out_half);
+}
+
 /*
  * Eq. 8 with an optional shift (Eq. 6):
  *   out_e = (m^2 + sigma) in_e - D_eo ( D_oe in_e )
  */
-int oracle_mdagm(const int N[4], int antiperiodic_t, const cplx *U, double mass, double sigma,
-                 const cplx *in_e, cplx *out_e)
+int oracle_mdagm_bf(const int N[4], int antiperiodic_t, const cplx *U, const double *theta, double mass,
+                    double sigma, const cplx *in_e, cplx *out_e)
 {
     size_t Vh = vol(N) / 2;
     cplx *tmp_o = (cplx *)malloc(Vh * 3 * sizeof(cplx));
     if (!tmp_o) return -1;
-    int rc = oracle_dslash_half(N, antiperiodic_t, U, 1, in_e, tmp_o);      /* D_oe in_e   */
-    if (!rc) rc = oracle_dslash_half(N, antiperiodic_t, U, 0, tmp_o, out_e); /* D_eo (...) */
+    int rc = oracle_dslash_half_bf(N, antiperiodic_t, U, theta, 1, in_e, tmp_o);      /* D_oe in_e   */
+    if (!rc) rc = oracle_dslash_half_bf(N, antiperiodic_t, U, theta, 0, tmp_o, out_e); /* D_eo (...) */
     if (!rc)
         for (size_t i = 0; i < Vh * 3; ++i) out_e[i] = (mass * mass + sigma) * in_e[i] - out_e[i];
     free(tmp_o);
     return rc;
+}
+
+int oracle_mdagm(const int N[4], int antiperiodic_t, const cplx *U, double mass, double sigma,
+                 const cplx *in_e, cplx *out_e)
+{
+    return oracle_mdagm_bf(N, antiperiodic_t, U, NULL, mass, sigma, in_e, out_e);
 }
 
 /*
@@ -251,10 +292,10 @@ static double re_dot(const cplx *a, const cplx *b, size_t n)
  * true_relres = || b - A x || / || b || recomputed at exit.
  * Returns 0 converged, 1 hit max_iter, -1 allocation failure.
  * ------------------------------------------------------------------------------------- */
-int oracle_cg(const int N[4], int antiperiodic_t, const cplx *U, double mass,
-              const cplx *b, cplx *x, double tol, int max_iter,
-              int *iters, double *true_relres,
-              double *hist_alpha, double *hist_beta, double *hist_rnorm, int hist_len)
+int oracle_cg_bf(const int N[4], int antiperiodic_t, const cplx *U, const double *theta, double mass,
+                 const cplx *b, cplx *x, double tol, int max_iter,
+                 int *iters, double *true_relres,
+                 double *hist_alpha, double *hist_beta, double *hist_rnorm, int hist_len)
 {
     size_t n = vol(N) / 2 * 3;
     cplx *r = (cplx *)malloc(n * sizeof(cplx));
@@ -267,7 +308,7 @@ int oracle_cg(const int N[4], int antiperiodic_t, const cplx *U, double mass,
     double bnorm = sqrt(rho);
     if (bnorm == 0.0) { rc = 0; goto done; }
     for (k = 0; k < max_iter; ++k) {
-        if (oracle_mdagm(N, antiperiodic_t, U, mass, 0.0, p, q)) { rc = -1; goto done; }
+        if (oracle_mdagm_bf(N, antiperiodic_t, U, theta, mass, 0.0, p, q)) { rc = -1; goto done; }
         double alpha = rho / re_dot(p, q, n);
         for (size_t i = 0; i < n; ++i) x[i] += alpha * p[i];
         for (size_t i = 0; i < n; ++i) r[i] -= alpha * q[i];
@@ -287,13 +328,22 @@ done:
     if (true_relres) {
         if (bnorm == 0.0 || rc < 0) *true_relres = 0.0;
         else {
-            oracle_mdagm(N, antiperiodic_t, U, mass, 0.0, x, q);
+            oracle_mdagm_bf(N, antiperiodic_t, U, theta, mass, 0.0, x, q);
             for (size_t i = 0; i < n; ++i) q[i] = b[i] - q[i];
             *true_relres = sqrt(re_dot(q, q, n)) / bnorm;
         }
     }
     free(r); free(p); free(q);
     return rc;
+}
+
+int oracle_cg(const int N[4], int antiperiodic_t, const cplx *U, double mass,
+              const cplx *b, cplx *x, double tol, int max_iter,
+              int *iters, double *true_relres,
+              double *hist_alpha, double *hist_beta, double *hist_rnorm, int hist_len)
+{
+    return oracle_cg_bf(N, antiperiodic_t, U, NULL, mass, b, x, tol, max_iter, iters, true_relres,
+                        hist_alpha, hist_beta, hist_rnorm, hist_len);
 }
 
 /* ---------------------------------------------------------------------------------------
@@ -324,12 +374,12 @@ done:
  * zeta_out[i]:  zeta_i at exit;  r_out: r at exit (either may be NULL)
  * Returns 0 all converged, 1 hit max_iter, -1 allocation failure, -2 bad shifts.
  * ------------------------------------------------------------------------------------- */
-int oracle_cg_multishift(const int N[4], int antiperiodic_t, const cplx *U, double mass,
-                         int nshift, const double *sigma, const cplx *b, cplx *x,
-                         double tol, int max_iter,
-                         int *iters, int *conv_iter, double *true_relres,
-                         double *zeta_out, cplx *r_out,
-                         double *hist_alpha, double *hist_beta, double *hist_rnorm, int hist_len)
+int oracle_cg_multishift_bf(const int N[4], int antiperiodic_t, const cplx *U, const double *theta, double mass,
+                            int nshift, const double *sigma, const cplx *b, cplx *x,
+                            double tol, int max_iter,
+                            int *iters, int *conv_iter, double *true_relres,
+                            double *zeta_out, cplx *r_out,
+                            double *hist_alpha, double *hist_beta, double *hist_rnorm, int hist_len)
 {
     if (nshift < 1) return -2;
     size_t n = vol(N) / 2 * 3;
@@ -366,7 +416,7 @@ int oracle_cg_multishift(const int N[4], int antiperiodic_t, const cplx *U, doub
     if (bnorm == 0.0) { rc = 0; goto done; }
 
     for (k = 0; k < max_iter; ++k) {
-        if (oracle_mdagm(N, antiperiodic_t, U, mass, sigma_min, p, q)) { rc = -1; goto done; }
+        if (oracle_mdagm_bf(N, antiperiodic_t, U, theta, mass, sigma_min, p, q)) { rc = -1; goto done; }
         double alpha = rho / re_dot(p, q, n);
         for (int i = 0; i < nshift; ++i) {
             zeta_new[i] = zeta[i] * zeta_old[i] * alpha_prev /
@@ -412,7 +462,7 @@ done:
         if (true_relres) {
             if (bnorm == 0.0 || rc < 0) true_relres[i] = 0.0;
             else {
-                oracle_mdagm(N, antiperiodic_t, U, mass, sigma[i], x + (size_t)i * n, q);
+                oracle_mdagm_bf(N, antiperiodic_t, U, theta, mass, sigma[i], x + (size_t)i * n, q);
                 for (size_t j = 0; j < n; ++j) q[j] = b[j] - q[j];
                 true_relres[i] = sqrt(re_dot(q, q, n)) / bnorm;
             }
@@ -421,6 +471,17 @@ done:
     if (r_out) memcpy(r_out, r, n * sizeof(cplx));
     free(r); free(p); free(q); free(ps); free(sc); free(active);
     return rc;
+}
+
+int oracle_cg_multishift(const int N[4], int antiperiodic_t, const cplx *U, double mass,
+                         int nshift, const double *sigma, const cplx *b, cplx *x,
+                         double tol, int max_iter,
+                         int *iters, int *conv_iter, double *true_relres,
+                         double *zeta_out, cplx *r_out,
+                         double *hist_alpha, double *hist_beta, double *hist_rnorm, int hist_len)
+{
+    return oracle_cg_multishift_bf(N, antiperiodic_t, U, NULL, mass, nshift, sigma, b, x, tol, max_iter, iters,
+                                   conv_iter, true_relres, zeta_out, r_out, hist_alpha, hist_beta, hist_rnorm, hist_len);
 }
 
 /* ---------------------------------------------------------------------------------------

@@ -15,7 +15,14 @@ import itertools
 import numpy as np
 
 
-def dense_dirac(dims, U, antiperiodic_t=True):
+def dense_dirac(dims, U, antiperiodic_t=True, theta=None):
+    """theta[V][4] (optional): every link enters as exp(i theta_mu(x)) U_mu(x) (the backfield)."""
+    if theta is not None:
+        U = U * np.exp(1j * np.asarray(theta))[:, :, None, None]
+    return _dense_dirac(dims, U, antiperiodic_t)
+
+
+def _dense_dirac(dims, U, antiperiodic_t):
     n0, n1, n2, n3 = dims
     V = n0 * n1 * n2 * n3
     D = np.zeros((3 * V, 3 * V), dtype=np.complex128)
@@ -50,9 +57,9 @@ def parity_mask(dims):
     return par.transpose(3, 2, 1, 0).reshape(-1)
 
 
-def dense_normal_operator(dims, U, mass, antiperiodic_t=True):
+def dense_normal_operator(dims, U, mass, antiperiodic_t=True, theta=None):
     """A = m^2 - D_eo D_oe on even sites, as a (3 Vh) x (3 Vh) matrix in idxh order."""
-    D = dense_dirac(dims, U, antiperiodic_t)
+    D = dense_dirac(dims, U, antiperiodic_t, theta)
     par = np.repeat(parity_mask(dims), 3)
     even = np.nonzero(par == 0)[0]
     odd = np.nonzero(par == 1)[0]

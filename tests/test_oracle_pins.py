@@ -90,6 +90,110 @@ def test_dirac_range_fills_exactly_lo_hi(ap):
     assert np.array_equal(out, full)
 
 
+# ----------------------------------------------------------------------------------------------
+# Backfield (the fourth argument of the paper's acc_Deo; reading R6: a U(1) phase
+# per link, every link enters D as e^{i theta_mu(x)} U_mu(x))
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (4, 2, 6, 2), (4, 4, 4, 4)])
+@pytest.mark.parametrize("ap", [True, False])
+def test_backfield_dense_matrix_zero_field_and_absorbed_phases(dims, ap):
+    """(i) theta = 0 reproduces D bit for bit; (ii) random theta = the dense matrix built from phased links
+    (wrong sign of the backward phase, phase taken at x instead of x-mu, or a phase on psi instead of on the
+    link all fail here; N_mu = 2 included); (iii) the phases absorbed into the links, U -> e^{i theta} U, give
+    the same result through the PLAIN (already pinned) entry point; (iv) D stays anti-Hermitian."""
+    rng = np.random.default_rng(31)
+    U = gen.haar_like_links(dims, rng)
+    psi = gen.gaussian_spinor(dims, rng)
+    theta = gen.uniform_backfield(dims, rng)
+    V = gen.volume(dims)
+    plain = oracle.dirac_full(dims, U, psi, antiperiodic_t=ap)
+    assert np.array_equal(oracle.dirac_full(dims, U, psi, antiperiodic_t=ap, theta=np.zeros((V, 4))), plain)
+    D = dense_dirac(dims, U, ap, theta)
+    assert np.abs(D + D.conj().T).max() < 1e-16
+    got = oracle.dirac_full(dims, U, psi, antiperiodic_t=ap, theta=theta)
+    assert rel(got, (D @ psi.reshape(-1)).reshape(-1, 3)) < 1e-14
+    assert rel(got, plain) > 0.1                                   # the field does something
+    absorbed = U * np.exp(1j * theta)[:, :, None, None]
+    assert rel(got, oracle.dirac_full(dims, absorbed, psi, antiperiodic_t=ap)) < 1e-14
+    # the single-site and half-lattice entry points see the same field
+    coords = gen.site_coords(dims)
+    for lex in (0, 1, V // 2 + 1, V - 1):
+        assert np.abs(oracle.dirac_site(dims, U, psi, coords[lex], antiperiodic_t=ap, theta=theta) - got[lex]).max() < 1e-15
+    for par in (0, 1):
+        half_in = oracle.full_to_half(dims, 1 - par, psi)
+        want = oracle.full_to_half(dims, par, got)
+        assert rel(oracle.dslash_half(dims, U, par, half_in, antiperiodic_t=ap, theta=theta), want) < 1e-14
+
+
+def test_backfield_constant_phase_shifts_the_free_momenta():
+    """U = 1, theta_mu(x) = t_mu constant: plane waves on even sites are eigenvectors of A with eigenvalue
+    m^2 + sum_mu sin^2(p_mu + t_mu) -- a momentum shift p -> p + t.  Catches a phase applied with the same
+    sign to both hops (which would give sin^2 p scaled, not shifted) and a factor 2 in the phase."""
+    dims = (4, 4, 6, 4)
+    U = gen.unit_links(dims)
+    m = 0.37
+    t = np.array([0.3, -0.45, 1.1, 0.2])
+    theta = np.tile(t, (gen.volume(dims), 1))
+    xe = gen.site_coords(dims)[gen.half_index_of_parity(dims, 0)]
+    colour = np.array([0.3 - 0.2j, 1.0 + 0.5j, -0.7j])
+    for n in [(0, 0, 0, 0), (1, 0, 0, 0), (0, 1, 2, 1), (3, 2, 5, 3)]:
+        p = np.array([2 * np.pi * n[0] / dims[0], 2 * np.pi * n[1] / dims[1],
+                      2 * np.pi * n[2] / dims[2], (2 * n[3] + 1) * np.pi / dims[3]])
+        phi = np.exp(1j * (xe @ p))[:, None] * colour[None, :]
+        lam = m * m + np.sum(np.sin(p + t) ** 2)
+        assert rel(oracle.mdagm(dims, U, m, phi, theta=theta), lam * phi) < 1e-13
+
+
+def test_backfield_pure_gauge_is_removed_by_a_u1_transformation():
+    """theta_mu(x) = a(x) - a(x+mu) (periodic a): D[U, theta] (g psi) = g D[U, 0] psi with g(x) = e^{i a(x)}.
+    Catches a phase attached to the wrong end of the link."""
+    dims = (4, 6, 2, 4)
+    rng = np.random.default_rng(33)
+    U = gen.smooth_links(dims, 0.5, rng)
+    psi = gen.gaussian_spinor(dims, rng)
+    V = gen.volume(dims)
+    a = rng.uniform(-np.pi, np.pi, size=V)
+    coords = gen.site_coords(dims)
+    theta = np.empty((V, 4))
+    for mu in range(4):
+        c = coords.copy()
+        c[:, mu] = (c[:, mu] + 1) % dims[mu]
+        fwd = c[:, 0] + dims[0] * (c[:, 1] + dims[1] * (c[:, 2] + dims[2] * c[:, 3]))
+        theta[:, mu] = a - a[fwd]
+    g = np.exp(1j * a)[:, None]
+    for ap in (True, False):
+        lhs = oracle.dirac_full(dims, U, g * psi, antiperiodic_t=ap, theta=theta)
+        assert rel(lhs, g * oracle.dirac_full(dims, U, psi, antiperiodic_t=ap)) < 1e-14
+
+
+def test_backfield_normal_operator_and_solvers():
+    """mdagm / CG / multi-shift CG with a backfield: the dense A built from phased links (Hermitian, spectrum
+    >= m^2), dense solves, and the absorbed-phase equivalence with the plain (pinned) solvers iteration by
+    iteration."""
+    dims = (4, 4, 2, 4)
+    rng = np.random.default_rng(34)
+    U = gen.smooth_links(dims, 0.4, rng)
+    theta = gen.uniform_backfield(dims, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    m = 0.2
+    A, _, _ = dense_normal_operator(dims, U, m, True, theta)
+    assert np.abs(A - A.conj().T).max() < 1e-15 and np.linalg.eigvalsh(A).min() >= m * m - 1e-12
+    assert rel(oracle.mdagm(dims, U, m, b, sigma=0.3, theta=theta).reshape(-1),
+               (A + 0.3 * np.eye(A.shape[0])) @ b.reshape(-1)) < 1e-13
+    r = oracle.cg(dims, U, m, b, 1e-12, 2000, theta=theta, hist_len=8)
+    assert r["converged"] and rel(r["x"].reshape(-1), np.linalg.solve(A, b.reshape(-1))) < 1e-10
+    absorbed = U * np.exp(1j * theta)[:, :, None, None]
+    r0 = oracle.cg(dims, absorbed, m, b, 1e-12, 2000, hist_len=8)
+    assert abs(r0["iters"] - r["iters"]) <= 2 and np.allclose(r0["alpha"], r["alpha"], rtol=1e-11)
+    assert np.allclose(r0["rnorm"], r["rnorm"], rtol=1e-11) and rel(r0["x"], r["x"]) < 1e-9
+    shifts = np.array([0.7, 0.0, 0.05])
+    ms = oracle.cg_multishift(dims, U, m, shifts, b, 1e-12, 2000, theta=theta)
+    assert ms["converged"]
+    for i, s in enumerate(shifts):
+        assert rel(ms["x"][i].reshape(-1), np.linalg.solve(A + s * np.eye(A.shape[0]), b.reshape(-1))) < 1e-10
+    assert rel(oracle.cg(dims, U, m, b, 1e-12, 2000).get("x"), r["x"]) > 1e-2       # and it is not the plain solve
+
+
 def test_half_lattice_views_and_parity_naming():
     """dslash_half(out_parity) = the (out, in) block of the dense matrix (reading R5)."""
     dims = (4, 4, 2, 4)
