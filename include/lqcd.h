@@ -118,6 +118,29 @@ int lqcd_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical_dev, const voi
 int lqcd_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links);
 
 /*
+ * The `backfield` argument of the paper's acc_Deo(u, out, in, backfield) (Listing 2): one
+ * real per link (the paper's double_soa), never explained in the text.  Reading R6 of DESIGN.md: an external
+ * U(1) phase theta_mu(x); every link enters D as e^{i theta_mu(x)} U_mu(x), i.e. the forward hop out of x is
+ * multiplied by e^{+i theta_mu(x)} and the backward hop by e^{-i theta_mu(x-mu)}.  The SU(3) link itself is
+ * untouched, so 2-row storage still works: the third row is rebuilt first, the phase is applied after
+ * (PAPER.md:272); eta and the boundary sign stay computed in-kernel.
+ *   canonical: float64 theta[lex][mu] (radians, any range);  native: one real of the context's precision per
+ *   link, layout private, lqcd_backfield_bytes bytes.
+ * lqcd_dslash_backfield is lqcd_dslash with the phases of that one call (the paper's four-argument form).
+ * lqcd_set_backfield attaches a native phase field to the context (NULL detaches): every later lqcd_dslash,
+ * lqcd_dslash_slices, lqcd_mdagm, lqcd_cg, lqcd_cg_multishift, lqcd_rational_apply and *_host* call of this
+ * context then uses it, at 8 (4) extra bytes per link and application: 1248 + 64 B per site in fp64.  The
+ * buffer must stay valid while attached.  lqcd_fermion_force returns LQCD_ERR_UNSUPPORTED while a backfield is
+ * attached; the gauge staples do not depend on it.  With a backfield the Dslash tuning options
+ * dslash_minblocks and l2_hints have no effect.  async.
+ */
+size_t lqcd_backfield_bytes(const lqcd_ctx *ctx);
+int lqcd_pack_backfield(lqcd_ctx *ctx, void *native_dev, const void *canonical_dev /* f64 [V][4] */);
+int lqcd_set_backfield(lqcd_ctx *ctx, const void *backfield_native_dev /* or NULL */);
+int lqcd_dslash_backfield(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
+                          const void *backfield_native_dev);
+
+/*
  * out_e = (mass^2 + sigma) in_e - D_eo (D_oe in_e)   (Eq. 8, shifted as in Eq. 6).
  * Needs a workspace (one odd-site temporary).  async.
  */

@@ -54,6 +54,10 @@ _sig = {
     "lqcd_pack_spinor": (_i, [_vp, _i, _vp, _vp]),
     "lqcd_unpack_spinor": (_i, [_vp, _i, _vp, _vp]),
     "lqcd_dslash": (_i, [_vp, _i, _vp, _vp, _vp]),
+    "lqcd_backfield_bytes": (_sz, [_vp]),
+    "lqcd_pack_backfield": (_i, [_vp, _vp, _vp]),
+    "lqcd_set_backfield": (_i, [_vp, _vp]),
+    "lqcd_dslash_backfield": (_i, [_vp, _i, _vp, _vp, _vp, _vp]),
     "lqcd_mdagm": (_i, [_vp, _vp, _vp, _vp, _d, _d]),
     "lqcd_cg": (_i, [_vp, _vp, _vp, _vp, _d, _d, _i, _pi, _pd]),
     "lqcd_cg_multishift": (_i, [_vp, _i, _pd, _vp, C.POINTER(_vp), _vp, _d, _d, _i, _pi, _pi, _pd]),
@@ -203,6 +207,27 @@ class Lattice:
     # -- the hot path (async unless stated) ---------------------------------------------------
     def dslash(self, parity, out, inp, links):
         self._check(lib.lqcd_dslash(self._ctx, parity, _vp(out.data_ptr()), _vp(inp.data_ptr()), _vp(links.data_ptr())))
+
+    def pack_backfield(self, theta):
+        """theta: float64 [V][4] (numpy), the per-link U(1) phases -> native device buffer."""
+        import numpy as np
+        assert theta.shape == (self.V, 4)
+        a = np.ascontiguousarray(theta, dtype=np.float64)
+        with self.torch.cuda.stream(self.stream):
+            canon = self.torch.from_numpy(a.reshape(-1)).to(self.device)
+        native = self._buf(int(lib.lqcd_backfield_bytes(self._ctx)))
+        self._check(lib.lqcd_pack_backfield(self._ctx, _vp(native.data_ptr()), _vp(canon.data_ptr())))
+        self.synchronize()
+        return native
+
+    def set_backfield(self, native=None):
+        """attach a native phase field to every later Dslash of this context (None detaches)."""
+        self._backfield = native            # keeps the buffer alive while attached
+        self._check(lib.lqcd_set_backfield(self._ctx, _vp(native.data_ptr()) if native is not None else None))
+
+    def dslash_backfield(self, parity, out, inp, links, backfield):
+        self._check(lib.lqcd_dslash_backfield(self._ctx, parity, _vp(out.data_ptr()), _vp(inp.data_ptr()),
+                                              _vp(links.data_ptr()), _vp(backfield.data_ptr())))
 
     def dslash_slices(self, parity, out, inp, links, x3_lo, x3_hi):
         self._check(lib.lqcd_dslash_slices(self._ctx, parity, _vp(out.data_ptr()), _vp(inp.data_ptr()),

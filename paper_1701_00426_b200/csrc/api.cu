@@ -322,6 +322,40 @@ extern "C" int lqcd_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in,
     return launch_dslash(ctx, parity, out, in, links, NULL, 0.0, 0, 0);
 }
 
+extern "C" size_t lqcd_backfield_bytes(const lqcd_ctx *ctx)
+{
+    return ctx ? (size_t)ctx->g.Vh * 2 * 4 * elem_size(ctx) : 0;
+}
+
+extern "C" int lqcd_pack_backfield(lqcd_ctx *ctx, void *native_dev, const void *canonical_dev)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(native_dev && canonical_dev, "lqcd_pack_backfield: null pointer");
+    return launch_pack_backfield(ctx, native_dev, canonical_dev);
+}
+
+extern "C" int lqcd_set_backfield(lqcd_ctx *ctx, const void *backfield_native_dev)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    REQUIRE(!((uintptr_t)backfield_native_dev & 15), "lqcd_set_backfield: pointer not 16-byte aligned");
+    ctx->backfield = backfield_native_dev;
+    return LQCD_OK;
+}
+
+extern "C" int lqcd_dslash_backfield(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
+                                     const void *backfield)
+{
+    int rc = enter(ctx); if (rc) return rc;
+    REQUIRE(out && in && links && backfield, "lqcd_dslash_backfield: null pointer");
+    REQUIRE(parity == 0 || parity == 1, "lqcd_dslash_backfield: parity %d", parity);
+    REQUIRE(out != in, "lqcd_dslash_backfield: out and in alias");
+    const void *saved = ctx->backfield;
+    ctx->backfield = backfield;
+    rc = launch_dslash(ctx, parity, out, in, links, NULL, 0.0, 0, 0);
+    ctx->backfield = saved;
+    return rc;
+}
+
 extern "C" int lqcd_dslash_slices(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
                                   int x3_lo, int x3_hi)
 {

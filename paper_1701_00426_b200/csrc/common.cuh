@@ -244,6 +244,7 @@ struct lqcd_ctx {
     lqcd_halo_fn halo_fn;            // fills the ghost slices of a half vector (NULL: nothing to do)
     lqcd_allreduce_fn allreduce_fn;  // sums device doubles over the ranks (NULL: single rank)
     void *comm_user;
+    const void *backfield; // native U(1) phase field applied by every Dslash of this context (NULL: none; lqcd_set_backfield)
     int force_stage;       // 1: force_kernel stages the site's own vectors in shared memory when they fit
     int staples_x2block;   // x2 block size of the staples' CTA order (0: plain idxh order)
     int staples_variant;   // 0: one product chain per path; 1: shared sub-products per (mu, nu)
@@ -315,6 +316,7 @@ size_t elem_size(const lqcd_ctx *ctx);
 // launchers implemented in the .cu files (all enqueue on ctx->stream)
 int launch_pack_links(lqcd_ctx *ctx, void *native, const void *canonical);
 int launch_pack_spinor(lqcd_ctx *ctx, int parity, void *native, const void *canonical);
+int launch_pack_backfield(lqcd_ctx *ctx, void *native, const void *canonical);
 int launch_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical, const void *native);
 // out = D in; if xpay_in != NULL: out = coef*xpay_in - D in and partial Re<xpay_in,out> is reduced
 // into the solver state (dot_mode 1: CG "pq" epilogue; 0: none).  `gate`: obey state->done.

@@ -45,12 +45,15 @@ template <typename T> __device__ __forceinline__ void mvdag_acc(Cx<T> acc[3], co
 }
 
 // MODE 0: out = D in;  1: out = coef*x - D in;  2: as 1, plus Re<x,out> -> solver_after_pq
-template <typename T, int LAYOUT, int RECON12, int MODE, int MINB, int POLICY>
+// BF 1: every link enters as e^{i theta_mu(x)} U_mu(x) (the `backfield` argument of the paper's acc_Deo, Listing 2,
+// PAPER.md:320-326; reading R6): theta is one real per link, [parity][mu][idxh]; the phase multiplies the
+// neighbour vector together with eta / the boundary sign, AFTER the third row was rebuilt from the SU(3) link.
+template <typename T, int LAYOUT, int RECON12, int MODE, int MINB, int POLICY, int BF>
 __global__ void __launch_bounds__(256, MINB)
 dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__restrict__ in,
               const T *__restrict__ links, const T *__restrict__ xin, const double coef,
               SolverState *__restrict__ st, double *__restrict__ partials, const int gate,
-              const int i_begin, const int i_end)
+              const int i_begin, const int i_end, const T *__restrict__ bf)
 {
     pdl_wait();
     pdl_trigger();
@@ -112,13 +115,15 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
             {
                 Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, parity, mu, (size_t)g.Ls, (size_t)i, pol);
                 Cx<T> p[3];
-                load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], p, pol);
+                if (BF) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], __ldcs(bf + (size_t)(parity * 4 + mu) * Vh + i), p, pol);
+                else load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], p, pol);
                 mv_acc<T>(acc, u, p);
             }
             {
                 Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, 1 - parity, mu, (size_t)g.Ls, (size_t)nb[mu], pol);
                 Cx<T> p[3];
-                load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], p, pol);
+                if (BF) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], -__ldcs(bf + (size_t)((1 - parity) * 4 + mu) * Vh + nb[mu]), p, pol);
+                else load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], p, pol);
                 mvdag_acc<T>(acc, u, p);
             }
         }
@@ -159,10 +164,14 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
     ctx->last_dslash_grid = tiles;
     int minb = ctx->dslash_minblocks;
     if (minb == 0) minb = sizeof(T) == 8 ? 2 : 4;   // profiles/experiments_r1b.md section 9
-#define GO1(MB, P) launch_k(ctx, dslash_kernel<T, LAYOUT, RECON12, MODE, MB, P>, grid, dim3(block), \
-        ctx->g, parity, (T *)out, (const T *)in, (const T *)links, (const T *)xin, coef, ctx->d_state, ctx->d_partials, gate, i_begin, i_end)
-#define GO(MB) do { if (ctx->l2_hints) GO1(MB, 1); else GO1(MB, 0); } while (0)
-    if (minb <= 2) GO(2); else if (minb == 3) GO(3); else GO(4);
+#define GO1(MB, P, B) launch_k(ctx, dslash_kernel<T, LAYOUT, RECON12, MODE, MB, P, B>, grid, dim3(block), \
+        ctx->g, parity, (T *)out, (const T *)in, (const T *)links, (const T *)xin, coef, ctx->d_state, ctx->d_partials, gate, i_begin, i_end, \
+        (const T *)ctx->backfield)
+#define GO(MB) do { if (ctx->l2_hints) GO1(MB, 1, 0); else GO1(MB, 0, 0); } while (0)
+    // with a backfield: the per-precision default variant only (the tuning options dslash_minblocks and
+    // l2_hints select nothing there)
+    if (ctx->backfield) { if (sizeof(T) == 8) GO1(2, 0, 1); else GO1(4, 0, 1); }
+    else if (minb <= 2) GO(2); else if (minb == 3) GO(3); else GO(4);
 #undef GO
 #undef GO1
 }

@@ -235,6 +235,7 @@ extern "C" int lqcd_fermion_force(lqcd_ctx *ctx, int nshift, const double *coeff
     }
     if (ctx->halo_fn || ctx->x3_lo != 0 || ctx->x3_hi != ctx->g.N3)
         return lqcd_fail(ctx, LQCD_ERR_UNSUPPORTED, "lqcd_fermion_force: not available in slab mode");
+    if (ctx->backfield) return lqcd_fail(ctx, LQCD_ERR_UNSUPPORTED, "lqcd_fermion_force: not available with a backfield attached");
     if (!ctx->ws) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "no workspace set");
     if (ctx->ws_bytes < lqcd_workspace_bytes(ctx, nshift))
         return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "workspace %zu bytes < %zu needed for %d shifts", ctx->ws_bytes, lqcd_workspace_bytes(ctx, nshift), nshift);

@@ -32,6 +32,18 @@ __global__ void pack_links_kernel(Geom g, int rows, T *__restrict__ native, cons
             }
 }
 
+// backfield theta[lex][mu] (one real per link, the paper's double_soa argument of acc_Deo)
+// -> native [parity][mu][idxh]
+template <typename T>
+__global__ void pack_backfield_kernel(Geom g, T *__restrict__ native, const double *__restrict__ canon)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int par = blockIdx.y;
+    if (i >= g.Vh) return;
+    size_t lex = (size_t)lex_of_half(g, i, par);
+    for (int mu = 0; mu < 4; ++mu) native[(size_t)(par * 4 + mu) * g.Vh + i] = (T)canon[lex * 4 + mu];
+}
+
 template <typename T, int LAYOUT>
 __global__ void pack_spinor_kernel(Geom g, T *__restrict__ native, const double2 *__restrict__ canon)
 {
@@ -106,6 +118,15 @@ int launch_pack_links(lqcd_ctx *ctx, void *native, const void *canonical)
 #undef CALL
     ctx->launches++;
     return lqcd_check_cuda(ctx, cudaGetLastError(), "pack_links");
+}
+
+int launch_pack_backfield(lqcd_ctx *ctx, void *native, const void *canonical)
+{
+    dim3 grid((ctx->g.Vh + 127) / 128, 2), block(128);
+    if (ctx->prec == LQCD_F64) pack_backfield_kernel<double><<<grid, block, 0, ctx->stream>>>(ctx->g, (double *)native, (const double *)canonical);
+    else pack_backfield_kernel<float><<<grid, block, 0, ctx->stream>>>(ctx->g, (float *)native, (const double *)canonical);
+    ctx->launches++;
+    return lqcd_check_cuda(ctx, cudaGetLastError(), "pack_backfield");
 }
 
 int launch_pack_spinor(lqcd_ctx *ctx, int parity, void *native, const void *canonical)

@@ -444,6 +444,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     key[kn++] = ((unsigned long long)ctx->poll_chunk << 32) | (unsigned)(g_k1 * 4096 + g_k2);
     key[kn++] = ((unsigned long long)block << 32) | (unsigned)(ctx->dslash_block * 64 + ctx->dslash_minblocks * 8 + ctx->l2_hints * 4 + ctx->pdl * 2) ^ ((unsigned long long)ctx->dslash_persist << 48);
     key[kn++] = (unsigned long long)(uintptr_t)ctx->stream ^ ((unsigned long long)ctx->iter_mask << 56);
+    key[kn++] = (unsigned long long)(uintptr_t)ctx->backfield;
     if (y) {
         key[kn++] = (unsigned long long)(uintptr_t)y;
         for (int i = 0; i < nshift; ++i) memcpy(&key[kn++], &coef[i], sizeof(double));

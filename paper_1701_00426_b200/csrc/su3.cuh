@@ -42,3 +42,19 @@ __device__ __forceinline__ void load_vec(const T *__restrict__ v, size_t Vh, siz
     }
 }
 
+// p = coef * e^{i theta} * v(i): the backfield phase of a hop (reading R6) folded into the
+// neighbour vector together with eta / the boundary sign.
+__device__ __forceinline__ void sincos_t(double x, double *s, double *c) { sincos(x, s, c); }
+__device__ __forceinline__ void sincos_t(float x, float *s, float *c) { sincosf(x, s, c); }
+template <typename T, int LAYOUT, int POLICY>
+__device__ __forceinline__ void load_vec_phase(const T *__restrict__ v, size_t Vh, size_t i, T coef, T theta, Cx<T> p[3], const L2Pol &pol)
+{
+    T sn, cs;
+    sincos_t(theta, &sn, &cs);
+    const T cr = coef * cs, ci = coef * sn;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        Cx<T> z = ld_cx<T, LAYOUT, 0, POLICY>(v, (size_t)c, Vh, i, pol);
+        p[c] = cx<T>(cr * z.re - ci * z.im, cr * z.im + ci * z.re);
+    }
+}
