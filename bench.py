@@ -403,6 +403,14 @@ def run_ours(args):
                 if prec == L.F64 and recon == L.RECON_18:
                     continue
                 extra[f"dslash_{pname}_{rn}real"] = dslash_rate(torch, L, D, gen, DIMS, U, in_e, in_o, prec, recon, peak, device)
+        # ---- Dslash with the backfield (the paper's fourth acc_Deo argument): theta stored (+64 B per site) and
+        #      (cos, sin) stored (+128 B per site)
+        theta = gen.uniform_backfield(DIMS, np.random.default_rng(33))
+        for fmt, add in ((0, 64), (1, 128)):
+            extra[f"dslash_backfield_f64_18real_fmt{fmt}"] = dslash_rate(
+                torch, L, D, gen, DIMS, U, in_e, in_o, L.F64, L.RECON_18, peak, device, theta=theta, bf_format=fmt,
+                bytes_per_site=BYTES_PER_SITE[("f64", 18)] + add)
+        del theta
         # ---- CG and multi-shift CG iteration rates (configs 2/4 shaped, on 32^4) --------------
         ms_it = solver_iter_rate(torch, lat, L, links, d_in_e, [0.0], 0.01)
         extra["cg_f64"] = {"iter_per_s": 1e3 / ms_it, "us_per_iter": ms_it * 1e3, "bytes_per_site_iter": CG_BYTES,
@@ -555,12 +563,15 @@ def run_ours(args):
 STAPLES_EXEC_FLOP_PER_LINK = {0: 84 * 198 + 24 * 36, 1: 3 * (22 * 198 + 10 * 36)}
 
 
-def dslash_rate(torch, L, D, gen, dims, U, in_e, in_o, prec, recon, peak, device, n=100):
+def dslash_rate(torch, L, D, gen, dims, U, in_e, in_o, prec, recon, peak, device, n=100, theta=None, bf_format=0,
+                bytes_per_site=None):
     """ns/site, GB/s, fraction of the copy peak of one Dslash variant (alternating parities, fixed inputs)."""
     pname, rn = ("f64" if prec == L.F64 else "f32"), (18 if recon == L.RECON_18 else 12)
     Vh = gen.volume(dims) // 2
-    lt = L.Lattice(dims, prec=prec, recon=recon, device=device.index)
+    lt = L.Lattice(dims, prec=prec, recon=recon, device=device.index, options={"backfield_format": bf_format})
     lk = lt.pack_links(U)
+    if theta is not None:
+        lt.set_backfield(lt.pack_backfield(theta))
     a, b_, o1, o2 = lt.pack_spinor(in_e, 0), lt.pack_spinor(in_o, 1), lt.new_spinor(), lt.new_spinor()
 
     def st():
@@ -568,7 +579,7 @@ def dslash_rate(torch, L, D, gen, dims, U, in_e, in_o, prec, recon, peak, device
         lt.dslash(L.EVEN, o2, b_, lk)
     t = timed_loop(torch, st, n, 5, 1, D, device)
     us = t * 1e3 / (2 * n)
-    gbs = BYTES_PER_SITE[(pname, rn)] * Vh / (us * 1e-6) / 1e9
+    gbs = (bytes_per_site or BYTES_PER_SITE[(pname, rn)]) * Vh / (us * 1e-6) / 1e9
     lt.close()
     return {"ns_per_site": us * 1e3 / Vh, "us_per_launch": us, "GBs": gbs, "frac": gbs / peak,
             "GFLOPs": FLOP_PER_SITE * Vh / (us * 1e-6) / 1e9, "dims": list(dims)}

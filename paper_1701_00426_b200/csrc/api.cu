@@ -138,7 +138,7 @@ struct OptDesc { const char *name; size_t off; long lo, hi; };
 static const OptDesc g_opts[] = {
     OPT(layout, 0, 1), OPT(l2_hints, 0, 1), OPT(l2_persist, 0, 4), OPT(link_pad, 0, 1 << 20), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
     OPT(blas_block, 64, 256), OPT(blas_ctas_per_sm, 1, 32), OPT(poll_chunk, 1, 1024),
-    OPT(pdl, 0, 1), OPT(graph, 0, 1), OPT(dslash_persist, 0, 16), OPT(iter_mask, 0, 15), OPT(staples_variant, 0, 1), OPT(force_stage, 0, 1), OPT(staples_x2block, 0, 64),
+    OPT(pdl, 0, 1), OPT(graph, 0, 1), OPT(dslash_persist, 0, 16), OPT(iter_mask, 0, 15), OPT(staples_variant, 0, 1), OPT(force_stage, 0, 1), OPT(staples_x2block, 0, 64), OPT(backfield_format, 0, 1),
 };
 
 extern "C" int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value)
@@ -151,6 +151,8 @@ extern "C" int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value)
             return lqcd_fail(ctx, LQCD_ERR_ARG, "option layout: fields were already packed in layout %d", ctx->layout);
         if ((!strcmp(name, "dslash_block") || !strcmp(name, "blas_block")) && (value % 32))
             return lqcd_fail(ctx, LQCD_ERR_ARG, "option %s must be a multiple of 32", name);
+        if (!strcmp(name, "backfield_format") && ctx->backfield_locked && value != ctx->backfield_format)
+            return lqcd_fail(ctx, LQCD_ERR_ARG, "option backfield_format: a backfield was already packed in format %d", ctx->backfield_format);
         if (!strcmp(name, "link_pad")) {
             if (ctx->layout_locked && value != ctx->link_pad) return lqcd_fail(ctx, LQCD_ERR_ARG, "option link_pad: fields were already packed");
             if (value % 8) return lqcd_fail(ctx, LQCD_ERR_ARG, "option link_pad must be a multiple of 8 sites");
@@ -324,13 +326,14 @@ extern "C" int lqcd_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in,
 
 extern "C" size_t lqcd_backfield_bytes(const lqcd_ctx *ctx)
 {
-    return ctx ? (size_t)ctx->g.Vh * 2 * 4 * elem_size(ctx) : 0;
+    return ctx ? (size_t)ctx->g.Vh * 2 * 4 * elem_size(ctx) * (ctx->backfield_format ? 2 : 1) : 0;
 }
 
 extern "C" int lqcd_pack_backfield(lqcd_ctx *ctx, void *native_dev, const void *canonical_dev)
 {
     int rc = enter(ctx); if (rc) return rc;
     REQUIRE(native_dev && canonical_dev, "lqcd_pack_backfield: null pointer");
+    ctx->backfield_locked = 1;
     return launch_pack_backfield(ctx, native_dev, canonical_dev);
 }
 

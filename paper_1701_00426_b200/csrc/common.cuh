@@ -244,6 +244,8 @@ struct lqcd_ctx {
     lqcd_halo_fn halo_fn;            // fills the ghost slices of a half vector (NULL: nothing to do)
     lqcd_allreduce_fn allreduce_fn;  // sums device doubles over the ranks (NULL: single rank)
     void *comm_user;
+    int backfield_format;  // 0: theta stored (one real per link, sincos in-kernel); 1: (cos theta, sin theta) stored
+    int backfield_locked;  // a backfield was packed: the format can no longer change
     const void *backfield; // native U(1) phase field applied by every Dslash of this context (NULL: none; lqcd_set_backfield)
     int force_stage;       // 1: force_kernel stages the site's own vectors in shared memory when they fit
     int staples_x2block;   // x2 block size of the staples' CTA order (0: plain idxh order)

@@ -45,9 +45,10 @@ template <typename T> __device__ __forceinline__ void mvdag_acc(Cx<T> acc[3], co
 }
 
 // MODE 0: out = D in;  1: out = coef*x - D in;  2: as 1, plus Re<x,out> -> solver_after_pq
-// BF 1: every link enters as e^{i theta_mu(x)} U_mu(x) (the `backfield` argument of the paper's acc_Deo, Listing 2,
-// PAPER.md:320-326; reading R6): theta is one real per link, [parity][mu][idxh]; the phase multiplies the
-// neighbour vector together with eta / the boundary sign, AFTER the third row was rebuilt from the SU(3) link.
+// BF != 0: every link enters as e^{i theta_mu(x)} U_mu(x) (the `backfield` argument of the paper's acc_Deo, Listing 2,
+// PAPER.md:320-326; reading R6), [parity][mu][idxh]; the phase multiplies the neighbour vector together with
+// eta / the boundary sign, AFTER the third row was rebuilt from the SU(3) link.  BF 1: theta stored, one real per
+// link, sincos in-kernel; BF 2: (cos theta, sin theta) stored (option backfield_format).
 template <typename T, int LAYOUT, int RECON12, int MODE, int MINB, int POLICY, int BF>
 __global__ void __launch_bounds__(256, MINB)
 dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__restrict__ in,
@@ -115,14 +116,16 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
             {
                 Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, parity, mu, (size_t)g.Ls, (size_t)i, pol);
                 Cx<T> p[3];
-                if (BF) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], __ldcs(bf + (size_t)(parity * 4 + mu) * Vh + i), p, pol);
+                if (BF == 1) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], __ldcs(bf + (size_t)(parity * 4 + mu) * Vh + i), p, pol);
+                else if (BF == 2) load_vec_unit<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], (T)1, bf, (size_t)(parity * 4 + mu) * Vh + i, p, pol);
                 else load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], p, pol);
                 mv_acc<T>(acc, u, p);
             }
             {
                 Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, 1 - parity, mu, (size_t)g.Ls, (size_t)nb[mu], pol);
                 Cx<T> p[3];
-                if (BF) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], -__ldcs(bf + (size_t)((1 - parity) * 4 + mu) * Vh + nb[mu]), p, pol);
+                if (BF == 1) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], -__ldcs(bf + (size_t)((1 - parity) * 4 + mu) * Vh + nb[mu]), p, pol);
+                else if (BF == 2) load_vec_unit<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], (T)-1, bf, (size_t)((1 - parity) * 4 + mu) * Vh + nb[mu], p, pol);
                 else load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], p, pol);
                 mvdag_acc<T>(acc, u, p);
             }
@@ -170,7 +173,8 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
 #define GO(MB) do { if (ctx->l2_hints) GO1(MB, 1, 0); else GO1(MB, 0, 0); } while (0)
     // with a backfield: the per-precision default variant only (the tuning options dslash_minblocks and
     // l2_hints select nothing there)
-    if (ctx->backfield) { if (sizeof(T) == 8) GO1(2, 0, 1); else GO1(4, 0, 1); }
+    if (ctx->backfield && ctx->backfield_format == 0) { if (sizeof(T) == 8) GO1(2, 0, 1); else GO1(4, 0, 1); }
+    else if (ctx->backfield) { if (sizeof(T) == 8) GO1(2, 0, 2); else GO1(4, 0, 2); }
     else if (minb <= 2) GO(2); else if (minb == 3) GO(3); else GO(4);
 #undef GO
 #undef GO1

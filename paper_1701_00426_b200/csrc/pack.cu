@@ -34,14 +34,20 @@ __global__ void pack_links_kernel(Geom g, int rows, T *__restrict__ native, cons
 
 // backfield theta[lex][mu] (one real per link, the paper's double_soa argument of acc_Deo)
 // -> native [parity][mu][idxh]
+// format 0: theta itself; format 1: (cos theta, sin theta), evaluated here in fp64 and rounded once
 template <typename T>
-__global__ void pack_backfield_kernel(Geom g, T *__restrict__ native, const double *__restrict__ canon)
+__global__ void pack_backfield_kernel(Geom g, int format, T *__restrict__ native, const double *__restrict__ canon)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     int par = blockIdx.y;
     if (i >= g.Vh) return;
     size_t lex = (size_t)lex_of_half(g, i, par);
-    for (int mu = 0; mu < 4; ++mu) native[(size_t)(par * 4 + mu) * g.Vh + i] = (T)canon[lex * 4 + mu];
+    for (int mu = 0; mu < 4; ++mu) {
+        const double th = canon[lex * 4 + mu];
+        const size_t k = (size_t)(par * 4 + mu) * g.Vh + i;
+        if (format == 0) native[k] = (T)th;
+        else { double sn, cs; sincos(th, &sn, &cs); native[2 * k] = (T)cs; native[2 * k + 1] = (T)sn; }
+    }
 }
 
 template <typename T, int LAYOUT>
@@ -123,8 +129,8 @@ int launch_pack_links(lqcd_ctx *ctx, void *native, const void *canonical)
 int launch_pack_backfield(lqcd_ctx *ctx, void *native, const void *canonical)
 {
     dim3 grid((ctx->g.Vh + 127) / 128, 2), block(128);
-    if (ctx->prec == LQCD_F64) pack_backfield_kernel<double><<<grid, block, 0, ctx->stream>>>(ctx->g, (double *)native, (const double *)canonical);
-    else pack_backfield_kernel<float><<<grid, block, 0, ctx->stream>>>(ctx->g, (float *)native, (const double *)canonical);
+    if (ctx->prec == LQCD_F64) pack_backfield_kernel<double><<<grid, block, 0, ctx->stream>>>(ctx->g, ctx->backfield_format, (double *)native, (const double *)canonical);
+    else pack_backfield_kernel<float><<<grid, block, 0, ctx->stream>>>(ctx->g, ctx->backfield_format, (float *)native, (const double *)canonical);
     ctx->launches++;
     return lqcd_check_cuda(ctx, cudaGetLastError(), "pack_backfield");
 }

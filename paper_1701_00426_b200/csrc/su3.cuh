@@ -58,3 +58,17 @@ __device__ __forceinline__ void load_vec_phase(const T *__restrict__ v, size_t V
         p[c] = cx<T>(cr * z.re - ci * z.im, cr * z.im + ci * z.re);
     }
 }
+// as load_vec_phase with the unit complex number (cos theta, sin theta) stored: conj = -1 takes e^{-i theta}
+template <typename T, int LAYOUT, int POLICY>
+__device__ __forceinline__ void load_vec_unit(const T *__restrict__ v, size_t Vh, size_t i, T coef, T conj, const T *__restrict__ bf,
+                                              size_t k, Cx<T> p[3], const L2Pol &pol)
+{
+    typedef typename Vec2<T>::type V2;
+    const V2 e = __ldcs(reinterpret_cast<const V2 *>(bf) + k);
+    const T cr = coef * e.x, ci = coef * conj * e.y;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        Cx<T> z = ld_cx<T, LAYOUT, 0, POLICY>(v, (size_t)c, Vh, i, pol);
+        p[c] = cx<T>(cr * z.re - ci * z.im, cr * z.im + ci * z.re);
+    }
+}

@@ -31,12 +31,14 @@ def make_lattice(dims, prec=0, recon=0, ap=True, **opts):
     return L.Lattice(dims, prec=prec, recon=recon, antiperiodic_t=ap, options=opts)
 
 
+@pytest.mark.parametrize("fmt", [0, 1])
 @pytest.mark.parametrize("layout", [0, 1])
 @pytest.mark.parametrize("recon", [0, 1])
 @pytest.mark.parametrize("prec", [0, 1])
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (2, 2, 2, 2), (6, 4, 2, 8), (12, 10, 6, 4)])
-def test_dslash_backfield_both_parities(dims, prec, recon, layout):
-    """Haar-like links, phases uniform in (-pi, pi): both parities, 2^4 (every hop wraps), ragged sizes."""
+def test_dslash_backfield_both_parities(dims, prec, recon, layout, fmt):
+    """Haar-like links, phases uniform in (-pi, pi): both parities, 2^4 (every hop wraps), ragged sizes; both
+    native formats (theta stored / (cos, sin) stored)."""
     rng = np.random.default_rng(61)
     U = gen.haar_like_links(dims, rng)
     psi = gen.gaussian_spinor(dims, rng)
@@ -44,7 +46,7 @@ def test_dslash_backfield_both_parities(dims, prec, recon, layout):
     U, psi, theta = round_inputs(prec, U, psi, theta)
     if recon == 1 and prec == 1:
         U = oracle.reconstruct_row3(U)
-    lat = make_lattice(dims, prec, recon, True, layout=layout)
+    lat = make_lattice(dims, prec, recon, True, layout=layout, backfield_format=fmt)
     links = lat.pack_links(U)
     bf = lat.pack_backfield(theta)
     for out_parity in (0, 1):
@@ -106,8 +108,9 @@ def test_backfield_absorbed_into_links_18real(ap):
     lat.close()
 
 
+@pytest.mark.parametrize("fmt", [0, 1])
 @pytest.mark.parametrize("prec", [0, 1])
-def test_mdagm_and_multishift_with_backfield(prec):
+def test_mdagm_and_multishift_with_backfield(prec, fmt):
     """The normal operator and the multi-shift solve with a backfield attached to the context: mdagm element by
     element; the solve by reading R16 (true residuals with the ORACLE operator, iteration counts, lock-step
     scalars) and with the chunk graph on (the graph key holds the backfield pointer)."""
@@ -119,7 +122,7 @@ def test_mdagm_and_multishift_with_backfield(prec):
     U, b, theta = round_inputs(prec, U, b, theta)
     mass, tol = 0.1, (1e-10 if prec == 0 else 1e-5)
     shifts = gen.rhmc_shifts(4)
-    lat = make_lattice(dims, prec)
+    lat = make_lattice(dims, prec, backfield_format=fmt)
     links = lat.pack_links(U)
     bf = lat.pack_backfield(theta)
     be = lat.pack_spinor(b, 0)
@@ -154,7 +157,8 @@ def test_mdagm_and_multishift_with_backfield(prec):
     lat.close()
 
 
-def test_backfield_large_volume_sampled_sites():
+@pytest.mark.parametrize("fmt", [0, 1])
+def test_backfield_large_volume_sampled_sites(fmt):
     """32^4 (the bench configuration), fp64 12-real: sampled sites incl. corners and both x3 boundary slices
     against oracle.dirac_site with the phase field."""
     dims = (32, 32, 32, 32)
@@ -162,7 +166,7 @@ def test_backfield_large_volume_sampled_sites():
     U = gen.smooth_links(dims, 0.3, rng)
     psi = gen.gaussian_spinor(dims, rng)
     theta = gen.uniform_backfield(dims, rng)
-    lat = make_lattice(dims, 0, 1)
+    lat = make_lattice(dims, 0, 1, backfield_format=fmt)
     links = lat.pack_links(U)
     bf = lat.pack_backfield(theta)
     coords = [(0, 0, 0, 0), (31, 31, 31, 31), (0, 31, 0, 31), (31, 0, 31, 0), (1, 0, 0, 0), (0, 0, 0, 31), (5, 7, 11, 0)]
@@ -200,4 +204,6 @@ def test_backfield_errors():
     lat.set_backfield(None)
     lat.fermion_force([x], links, [1.0])
     lat.synchronize()
+    with pytest.raises(L.LqcdError):            # the format is fixed once a backfield was packed
+        lat.set_option("backfield_format", 1)
     lat.close()
