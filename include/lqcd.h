@@ -236,8 +236,14 @@ int lqcd_unpack_force(lqcd_ctx *ctx, void *canonical_dev /* c128 [V][4][3][3] */
  * per nu != mu two 3-link and six 5-link paths.  Links are periodic in all four directions.
  *   links    native link field (device); staples: native 3x3-per-link field (device, lqcd_force_bytes;
  *            layout private: read it back with lqcd_unpack_force)
+ * Algorithm (option "staples_variant"): 2 (default) runs two passes through the 24 stored 3-link staples per
+ * site, 39 SU(3) products per link; it needs lqcd_staples_workspace_bytes(ctx) bytes in the workspace given to
+ * lqcd_set_workspace (contents destroyed) -- with no or a smaller workspace, and for variant 1, the one-pass
+ * kernel with shared sub-products runs (66 products per link, no workspace); 0 walks every path on its own
+ * (84 products).  All three agree to rounding.  Read-only option "staples_ran": the variant the last call used.
  * async.  LQCD_ERR_UNSUPPORTED in slab mode.
  */
+size_t lqcd_staples_workspace_bytes(const lqcd_ctx *ctx);
 int lqcd_gauge_staples(lqcd_ctx *ctx, const void *links, void *staples, double c0, double c1);
 
 /*

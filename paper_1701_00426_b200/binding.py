@@ -67,6 +67,7 @@ _sig = {
     "lqcd_unpack_tamat": (_i, [_vp, _vp, _vp]),
     "lqcd_fermion_force": (_i, [_vp, _i, _pd, C.POINTER(_vp), _vp, _vp]),
     "lqcd_unpack_force": (_i, [_vp, _vp, _vp]),
+    "lqcd_staples_workspace_bytes": (_sz, [_vp]),
     "lqcd_gauge_staples": (_i, [_vp, _vp, _vp, _d, _d]),
     "lqcd_dslash_slices": (_i, [_vp, _i, _vp, _vp, _vp, _i, _i]),
     "lqcd_halo_bytes": (_sz, [_vp]),
@@ -164,10 +165,10 @@ class Lattice:
     def new_spinor(self):
         return self._buf(self.spinor_bytes)
 
-    def ensure_workspace(self, nshift=1):
-        if self._ws is None or nshift > self._ws_shifts:
-            self._ws = self._buf(int(lib.lqcd_workspace_bytes(self._ctx, nshift)))
-            self._ws_shifts = nshift
+    def ensure_workspace(self, nshift=1, min_bytes=0):
+        need = max(int(lib.lqcd_workspace_bytes(self._ctx, nshift)), int(min_bytes))
+        if self._ws is None or need > self._ws.numel():
+            self._ws = self._buf(need)
             self._check(lib.lqcd_set_workspace(self._ctx, _vp(self._ws.data_ptr()), self._ws.numel()))
 
     def synchronize(self):
@@ -327,6 +328,8 @@ class Lattice:
         """async; tree-level Symanzik staples (3x3 per link); read back with unpack_force."""
         if out is None:
             out = self._buf(int(lib.lqcd_force_bytes(self._ctx)))
+        if self.get_option("staples_variant") == 2:     # the two-pass algorithm keeps its 3-link staples in the workspace
+            self.ensure_workspace(1, int(lib.lqcd_staples_workspace_bytes(self._ctx)))
         self._check(lib.lqcd_gauge_staples(self._ctx, _vp(links.data_ptr()), _vp(out.data_ptr()), float(c0), float(c1)))
         return out
 

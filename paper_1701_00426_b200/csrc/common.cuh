@@ -249,7 +249,10 @@ struct lqcd_ctx {
     const void *backfield; // native U(1) phase field applied by every Dslash of this context (NULL: none; lqcd_set_backfield)
     int force_stage;       // 1: force_kernel stages the site's own vectors in shared memory when they fit
     int staples_x2block;   // x2 block size of the staples' CTA order (0: plain idxh order)
-    int staples_variant;   // 0: one product chain per path; 1: shared sub-products per (mu, nu)
+    int staples_variant;   // 0: one product chain per path; 1: shared sub-products per (mu, nu); 2: two passes through
+                           // stored 3-link staples (needs lqcd_staples_workspace_bytes of workspace, else 1 runs)
+    int staples_minblocks; // launch-bounds variant (2, 3, 4 CTAs of 128 per SM) of the two-pass algorithm's second kernel; 0: default
+    int staples_ran;       // read-only: the variant the last lqcd_gauge_staples call used
     int iter_mask;         // diagnostic: bit k set = kernel k of the CG iteration is launched (default 15)
     int graph_active;      // read-only: the last solve ran from a graph
     cudaStream_t cap_stream;      // private stream used only for graph capture

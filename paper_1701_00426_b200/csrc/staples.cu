@@ -348,6 +348,224 @@ __global__ void __launch_bounds__(128, 2) staples_kernel_shared(const Geom g, T 
             st_cx<T, LAYOUT, 0>(staples, (size_t)((parity * 4 + mu) * 9 + a * 3 + b), (size_t)g.Vh, (size_t)i, S.e[a][b], pol);
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Variant 2 (option staples_variant = 2, the default when the workspace is large enough): two passes
+// through 24 intermediate fields per site, the 3-link staples of every ordered pair (m, n), m != n,
+//   Tu_mn(x) = U_n(x+m) U_m(x+n)^+ U_n(x)^+          (above the link U_m(x); the plaquette staple itself)
+//   Tl_mn(x) = U_n(x+m-n)^+ U_m(x-n)^+ U_n(x-n)       (below)
+// Every 5-link rectangle path through U_mu(x) is a 3-link staple of a NEIGHBOURING link times two links
+// (no unitarity is used: these are regroupings of the same ordered products):
+//   above:  U_mu(x+mu) U_nu(x+2mu) U_mu(x+mu+nu)^+ . B C  = Tu_numu(x+mu)^+ B C        B = U_mu(x+nu)^+
+//           A B . U_mu(x-mu+nu)^+ U_nu(x-mu)^+ U_mu(x-mu) = A B Tl_numu(x)             A = U_nu(x+mu)
+//           A . U_nu(x+mu+nu) U_mu(x+2nu)^+ U_nu(x+nu)^+ . C = A Tu_munu(x+nu) C      C = U_nu(x)^+
+//   below:  Tu_numu(x+mu-nu) B' C',  A' B' Tl_numu(x-nu)^+,  A' Tl_munu(x-nu) C'
+//           A' = U_nu(x+mu-nu)^+, B' = U_mu(x-nu)^+, C' = U_nu(x-nu)
+//   S_mu(x) = sum_nu  c0 [Tu_munu(x) + Tl_munu(x)]
+//                   + c1 { [Tu_numu(x+mu)^+ B + A Tu_munu(x+nu)] C + (A B) Tl_numu(x) }
+//                   + c1 { [Tu_numu(x+mu-nu) B' + A' Tl_munu(x-nu)] C' + (A' B') Tl_numu(x-nu)^+ }
+// Pass 1 (staples_produce_kernel, one thread per site and ordered pair): Q = U_m(y) U_n(y+m), then
+//   Tl_mn(y+n) = Q^+ U_n(y) and Tu_nm(y) = U_m(y+n) Q^+ : 3 products for 2 fields, 36 per site.
+// Pass 2 (staples_final_kernel, one thread per link): 10 products and 14 matrix loads per nu.
+// 39 products per link instead of 66 (variant 1) / 84 (the definition); the price is 24 x 144 B per site of
+// intermediate fields written and read once (fp64): the work moves from the FP64 pipe to HBM.
+// ---------------------------------------------------------------------------------------------
+__host__ __device__ __forceinline__ int pair_idx(int m, int n) { return m * 3 + (n < m ? n : n - 1); }
+// first plane of the field of `kind` (0: Tu, 1: Tl) of the ordered pair q on the sites of parity par
+__device__ __forceinline__ size_t tfield_plane(int par, int q, int kind) { return (size_t)(((par * 12 + q) * 2 + kind) * 9); }
+
+// op(a) op(b), op = dagger when the flag is set
+template <typename T, int DA, int DB> __device__ __forceinline__ Su3<T> mul_op(const Su3<T> &a, const Su3<T> &b)
+{
+    Su3<T> o;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            T re = 0, im = 0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const T ar = DA ? a.e[k][i].re : a.e[i][k].re, ai = DA ? -a.e[k][i].im : a.e[i][k].im;
+                const T br = DB ? b.e[j][k].re : b.e[k][j].re, bi = DB ? -b.e[j][k].im : b.e[k][j].im;
+                re = fma(ar, br, re);
+                re = fma(-ai, bi, re);
+                im = fma(ar, bi, im);
+                im = fma(ai, br, im);
+            }
+            o.e[i][j] = cx<T>(re, im);
+        }
+    return o;
+}
+// s += c * op(m)
+template <typename T, int DM> __device__ __forceinline__ void acc_op(Su3<T> &s, T c, const Su3<T> &m)
+{
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            s.e[i][j].re = fma(c, DM ? m.e[j][i].re : m.e[i][j].re, s.e[i][j].re);
+            s.e[i][j].im = fma(DM ? -c : c, DM ? m.e[j][i].im : m.e[i][j].im, s.e[i][j].im);
+        }
+}
+template <typename T, int LAYOUT>
+__device__ __forceinline__ Su3<T> load_mat(const T *__restrict__ f, size_t plane0, size_t Vh, size_t i)
+{
+    Su3<T> m;
+    const L2Pol pol = {0, 0};
+#pragma unroll
+    for (int k = 0; k < 9; ++k) m.e[k / 3][k % 3] = ld_cx<T, LAYOUT, 0, 0>(f, plane0 + k, Vh, i, pol);
+    return m;
+}
+template <typename T, int LAYOUT>
+__device__ __forceinline__ void store_mat(T *__restrict__ f, size_t plane0, size_t Vh, size_t i, const Su3<T> &m)
+{
+    const L2Pol pol = {0, 0};
+#pragma unroll
+    for (int k = 0; k < 9; ++k) st_cx<T, LAYOUT, 0>(f, plane0 + k, Vh, i, m.e[k / 3][k % 3], pol);
+}
+// the staple field is written once and not read again by this library: streaming stores keep the link
+// neighbourhood in L2 (ncu on variant 1: 855 MB written to DRAM against 604 MB of output)
+template <typename T, int LAYOUT>
+__device__ __forceinline__ void store_mat_stream(T *__restrict__ f, size_t plane0, size_t Vh, size_t i, const Su3<T> &m)
+{
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        const Cx<T> z = m.e[k / 3][k % 3];
+        if (LAYOUT == 0) {
+            typedef typename Vec2<T>::type V2;
+            V2 v; v.x = z.re; v.y = z.im;
+            __stcs(reinterpret_cast<V2 *>(f) + (plane0 + k) * Vh + i, v);
+        } else {
+            __stcs(f + (2 * (plane0 + k)) * Vh + i, z.re);
+            __stcs(f + (2 * (plane0 + k) + 1) * Vh + i, z.im);
+        }
+    }
+}
+
+__device__ __forceinline__ Site4 decode_site(const Geom &g, int i, int parity)
+{
+    uint32_t t = fd_div((uint32_t)i, g.dNh0);
+    const int hx0 = i - (int)t * g.Nh0;
+    uint32_t t2 = fd_div(t, g.dN1);
+    Site4 x;
+    x.x1 = (int)t - (int)t2 * g.N1;
+    x.x3 = (int)fd_div(t2, g.dN2);
+    x.x2 = (int)t2 - x.x3 * g.N2;
+    x.x0 = 2 * hx0 + ((x.x1 + x.x2 + x.x3 + parity) & 1);
+    return x;
+}
+
+// Pass 1.  CTA = 128 consecutive sites of one parity; blockIdx.x = (tile * 2 + parity) * 12 + ordered pair, so
+// that the 24 CTAs that read the links of one tile run together.
+template <typename T, int LAYOUT, int RECON12>
+__global__ void __launch_bounds__(128, 3) staples_produce_kernel(const Geom g, T *__restrict__ tf, const T *__restrict__ links)
+{
+    pdl_wait();
+    pdl_trigger();
+    const int bid = blockIdx.x;
+    const int q = bid % 12, parity = (bid / 12) & 1, tile = bid / 24;
+    const int i = tile * blockDim.x + threadIdx.x;
+    if (i >= g.Vh) return;
+    const int m = q / 3, n = (q % 3) + ((q % 3) >= m ? 1 : 0);
+    const Site4 x = decode_site(g, i, parity);
+    const size_t Vh = (size_t)g.Vh, Ls = (size_t)g.Ls;
+    const size_t im = (size_t)(i + idxh_disp(g, x, m, 1)), in = (size_t)(i + idxh_disp(g, x, n, 1));
+    const L2Pol pol = {0, 0};
+    Su3<T> Q;
+    {
+        const Su3<T> a = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity, m, Ls, (size_t)i, pol);
+        const Su3<T> d = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity ^ 1, n, Ls, im, pol);
+        Q = mul_op<T, 0, 0>(a, d);                                      // U_m(y) U_n(y+m)
+    }
+    {
+        const Su3<T> b = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity, n, Ls, (size_t)i, pol);
+        store_mat<T, LAYOUT>(tf, tfield_plane(parity ^ 1, pair_idx(m, n), 1), Vh, in, mul_op<T, 1, 0>(Q, b));   // Tl_mn(y+n)
+    }
+    {
+        const Su3<T> c = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity ^ 1, m, Ls, in, pol);
+        store_mat<T, LAYOUT>(tf, tfield_plane(parity, pair_idx(n, m), 0), Vh, (size_t)i, mul_op<T, 0, 1>(c, Q)); // Tu_nm(y)
+    }
+}
+
+// Pass 2.  One thread per link (x, mu); CTA order as in the one-pass kernels (staple_cta).
+template <typename T, int LAYOUT, int RECON12, int MINB>
+__global__ void __launch_bounds__(128, MINB) staples_final_kernel(const Geom g, T *__restrict__ staples, const T *__restrict__ links,
+                                                             const T *__restrict__ tf, const T c0, const T c1, const StapleSwizzle sw)
+{
+    pdl_wait();
+    pdl_trigger();
+    int tile, mu, parity;
+    staple_cta(sw, tile, mu, parity);
+    const int i = tile * blockDim.x + threadIdx.x;
+    if (i >= g.Vh) return;
+    const Site4 x = decode_site(g, i, parity);
+    const size_t Vh = (size_t)g.Vh, Ls = (size_t)g.Ls;
+    const L2Pol pol = {0, 0};
+    const int po = parity ^ 1;
+    const size_t i_m = (size_t)(i + idxh_disp(g, x, mu, 1));           // x + mu
+    Su3<T> S;
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) S.e[a][b] = cx<T>((T)0, (T)0);
+#pragma unroll 1
+    for (int nu = 0; nu < 4; ++nu) {
+        if (nu == mu) continue;
+        const int dn_p = idxh_disp(g, x, nu, 1), dn_m = idxh_disp(g, x, nu, -1);
+        const size_t i_n = (size_t)(i + dn_p), i_l = (size_t)(i + dn_m);                       // x + nu, x - nu
+        const size_t i_ml = (size_t)((int)i_m + dn_m);                                           // x + mu - nu
+        const int qmn = pair_idx(mu, nu), qnm = pair_idx(nu, mu);
+        {   // above the link
+            Su3<T> W;
+            {
+                const Su3<T> Ub = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, mu, Ls, i_n, pol);       // U_mu(x+nu)
+                {
+                    const Su3<T> T1 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qnm, 0), Vh, i_m);         // Tu_numu(x+mu)
+                    W = mul_op<T, 1, 1>(T1, Ub);                                                            // T1^+ B
+                }
+                const Su3<T> A = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, nu, Ls, i_m, pol);        // U_nu(x+mu)
+                {
+                    const Su3<T> T2 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qmn, 0), Vh, i_n);         // Tu_munu(x+nu)
+                    acc_op<T, 0>(W, (T)1, mul_op<T, 0, 0>(A, T2));
+                }
+                const Su3<T> AB = mul_op<T, 0, 1>(A, Ub);
+                const Su3<T> T3 = load_mat<T, LAYOUT>(tf, tfield_plane(parity, qnm, 1), Vh, (size_t)i);   // Tl_numu(x)
+                acc_op<T, 0>(S, c1, mul_op<T, 0, 0>(AB, T3));
+            }
+            const Su3<T> Uc = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity, nu, Ls, (size_t)i, pol); // U_nu(x)
+            acc_op<T, 0>(S, c1, mul_op<T, 0, 1>(W, Uc));
+            acc_op<T, 0>(S, c0, load_mat<T, LAYOUT>(tf, tfield_plane(parity, qmn, 0), Vh, (size_t)i));    // Tu_munu(x)
+        }
+        {   // below the link
+            Su3<T> W;
+            {
+                const Su3<T> Ub = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, mu, Ls, i_l, pol);       // U_mu(x-nu)
+                {
+                    const Su3<T> T1 = load_mat<T, LAYOUT>(tf, tfield_plane(parity, qnm, 0), Vh, i_ml);    // Tu_numu(x+mu-nu)
+                    W = mul_op<T, 0, 1>(T1, Ub);
+                }
+                const Su3<T> Ua = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity, nu, Ls, i_ml, pol);  // U_nu(x+mu-nu)
+                {
+                    const Su3<T> T2 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qmn, 1), Vh, i_l);         // Tl_munu(x-nu)
+                    acc_op<T, 0>(W, (T)1, mul_op<T, 1, 0>(Ua, T2));
+                }
+                const Su3<T> AB = mul_op<T, 1, 1>(Ua, Ub);
+                const Su3<T> T3 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qnm, 1), Vh, i_l);             // Tl_numu(x-nu)
+                acc_op<T, 0>(S, c1, mul_op<T, 0, 1>(AB, T3));
+            }
+            const Su3<T> Uc = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, nu, Ls, i_l, pol);           // U_nu(x-nu)
+            acc_op<T, 0>(S, c1, mul_op<T, 0, 0>(W, Uc));
+            acc_op<T, 0>(S, c0, load_mat<T, LAYOUT>(tf, tfield_plane(parity, qmn, 1), Vh, (size_t)i));    // Tl_munu(x)
+        }
+    }
+    store_mat_stream<T, LAYOUT>(staples, (size_t)((parity * 4 + mu) * 9), Vh, (size_t)i, S);
+}
+
+extern "C" size_t lqcd_staples_workspace_bytes(const lqcd_ctx *ctx)
+{
+    return ctx ? (size_t)ctx->g.Vh * 2 * 24 * 9 * 2 * elem_size(ctx) : 0;
+}
+
 extern "C" int lqcd_gauge_staples(lqcd_ctx *ctx, const void *links, void *staples, double c0, double c1)
 {
     if (!ctx) return LQCD_ERR_ARG;
@@ -365,8 +583,28 @@ extern "C" int lqcd_gauge_staples(lqcd_ctx *ctx, const void *links, void *staple
         sw.x2b = ctx->staples_x2block;
         sw.tiles_row = row / 128;
     }
+    // variant 2 needs the intermediate fields in the context's workspace; without one that is large enough the
+    // one-pass kernel with shared sub-products runs instead (same result to rounding)
+    const bool two_pass = ctx->staples_variant == 2 && ctx->ws && ctx->ws_bytes >= lqcd_staples_workspace_bytes(ctx);
+    ctx->staples_ran = two_pass ? 2 : (ctx->staples_variant == 0 ? 0 : 1);
+    if (two_pass) {
+        dim3 gridp(((ctx->g.Vh + 127) / 128) * 24);
+        int minb = ctx->staples_minblocks;           // launch-bounds variant of pass 2 (0: default per precision)
+        if (minb == 0) minb = ctx->prec == LQCD_F64 ? 3 : 3;
+#define GO2(T, L, R) do { \
+        launch_k(ctx, staples_produce_kernel<T, L, R>, gridp, block, ctx->g, (T *)ctx->ws, (const T *)links); \
+        if (minb == 2) launch_k(ctx, staples_final_kernel<T, L, R, 2>, grid, block, ctx->g, (T *)staples, (const T *)links, (const T *)ctx->ws, (T)c0, (T)c1, sw); \
+        else if (minb == 3) launch_k(ctx, staples_final_kernel<T, L, R, 3>, grid, block, ctx->g, (T *)staples, (const T *)links, (const T *)ctx->ws, (T)c0, (T)c1, sw); \
+        else launch_k(ctx, staples_final_kernel<T, L, R, 4>, grid, block, ctx->g, (T *)staples, (const T *)links, (const T *)ctx->ws, (T)c0, (T)c1, sw); } while (0)
+#define GO2R(T, L) do { if (ctx->recon == LQCD_RECON_12) GO2(T, L, 1); else GO2(T, L, 0); } while (0)
+        if (ctx->prec == LQCD_F64) { if (ctx->layout == 0) GO2R(double, 0); else GO2R(double, 1); }
+        else { if (ctx->layout == 0) GO2R(float, 0); else GO2R(float, 1); }
+#undef GO2R
+#undef GO2
+        return lqcd_check_cuda(ctx, cudaGetLastError(), "gauge staples (two passes)");
+    }
 #define GO(T, L) do { \
-        if (ctx->staples_variant == 1) { \
+        if (ctx->staples_variant >= 1) { \
             if (ctx->recon == LQCD_RECON_12) launch_k(ctx, staples_kernel_shared<T, L, 1>, grid, block, ctx->g, (T *)staples, (const T *)links, (T)c0, (T)c1, sw); \
             else launch_k(ctx, staples_kernel_shared<T, L, 0>, grid, block, ctx->g, (T *)staples, (const T *)links, (T)c0, (T)c1, sw); \
         } else if (ctx->recon == LQCD_RECON_12) launch_k(ctx, staples_kernel<T, L, 1>, grid, block, ctx->g, (T *)staples, (const T *)links, (T)c0, (T)c1, sw); \

@@ -183,8 +183,8 @@ def slab(dims_list, out):
     D.finalize(world)
 
 
-def staples(dims_list, out):
-    """NEXT-4: gauge staples, both kernel variants, fp64 / fp32, 18- / 12-real links."""
+def staples(dims_list, out, variants=(0, 1, 2), precs=(0, 1), recons=(0, 1)):
+    """NEXT-4: gauge staples, the three algorithm variants, fp64 / fp32, 18- / 12-real links."""
     import numpy as np
     import torch
     import lqcd_inputs as gen
@@ -195,15 +195,15 @@ def staples(dims_list, out):
         rng = np.random.default_rng(5)
         U = gen.smooth_links(dims, 0.5, rng)
         V = gen.volume(dims)
-        for prec in (0, 1):
-            for recon in (0, 1):
-                for variant in (0, 1):
+        for prec in precs:
+            for recon in recons:
+                for variant in variants:
                     lat = L.Lattice(dims, prec=prec, recon=recon, options=dict(staples_variant=variant))
                     links = lat.pack_links(U)
                     buf = lat.gauge_staples(links)
                     us = ev_time_us(torch, lambda: lat.gauge_staples(links, out=buf), 10, 2)
                     out(dict(kind="staples", dims="x".join(map(str, dims)), prec=("f64", "f32")[prec], links=(18, 12)[recon],
-                             variant=variant, us=round(us, 1), ns_per_site=round(us * 1e3 / V, 3),
+                             variant=variant, ran=lat.get_option("staples_ran"), us=round(us, 1), ns_per_site=round(us * 1e3 / V, 3),
                              TFLOPs=round(flop_site * V / us / 1e6, 2)))
                     lat.close()
 
@@ -258,6 +258,9 @@ def main():
     ap.add_argument("--staples", action="store_true", help="NEXT-4 gauge staples timing")
     ap.add_argument("--slab", action="store_true", help="x3-slab path (run under torchrun for more than one GPU)")
     ap.add_argument("--dims", default=None, help="comma-separated N0,N1,N2,N3 (repeatable with ';')")
+    ap.add_argument("--variants", default="0,1,2", help="with --staples: algorithm variants to time")
+    ap.add_argument("--precs", default="0,1", help="with --staples: 0 = fp64, 1 = fp32")
+    ap.add_argument("--recons", default="0,1", help="with --staples: 0 = 18-real, 1 = 12-real links")
     ap.add_argument("--eps", type=float, default=0.5)
     ap.add_argument("--seed", type=int, default=5)
     ap.add_argument("--md", default=None)
@@ -279,7 +282,8 @@ def main():
     if args.multishift:
         multishift(dims_list or [(24, 24, 24, 48), (32, 32, 32, 32)], out)
     if args.staples:
-        staples(dims_list or [(16,) * 4, (32, 32, 32, 8), (32,) * 4], out)
+        ints = lambda t: tuple(int(v) for v in t.split(","))   # noqa: E731
+        staples(dims_list or [(16,) * 4, (32, 32, 32, 8), (32,) * 4], out, ints(args.variants), ints(args.precs), ints(args.recons))
     if args.slab:
         slab(dims_list or [(32, 32, 32, 32)], out)
     if args.md:
