@@ -458,7 +458,7 @@ def run_ours(args):
                                      "num_SMs x 8 CTAs of 256 threads, best of 4 after 2 warm-up launches"}
         sbuf = lat.gauge_staples(links)
         t_s = timed_loop(torch, lambda: lat.gauge_staples(links, out=sbuf), 10, 3, 1, D, device) / 10
-        variant = lat.get_option("staples_variant")
+        variant = lat.get_option("staples_ran")
         flop_def = 4 * (84 * 198 + 24 * 36)                     # the definition: 84 products + 24 scaled adds per link
         flop_exec = 4 * STAPLES_EXEC_FLOP_PER_LINK[variant]      # what the default variant executes
         extra["gauge_staples_f64"] = {"ms": t_s, "ns_per_site": t_s * 1e6 / V, "bound": "alu", "peak_TFLOPs": fp64_peak,
@@ -470,6 +470,12 @@ def run_ours(args):
                                       "variant": variant,
                                       "note": "2 plaquette + 6 rectangle paths per nu, c0 = 5/3, c1 = -1/12; frac = EXECUTED "
                                               "flops / measured FP64 peak"}
+        if variant == 2:
+            gbs = STAPLES2_BYTES_PER_SITE * V / (t_s * 1e-3) / 1e9
+            extra["gauge_staples_f64"].update({
+                "hbm_bytes_per_site_two_pass": STAPLES2_BYTES_PER_SITE, "hbm_GBs": gbs, "hbm_frac": gbs / peak,
+                "note2": "variant 2 trades FP64 work for HBM traffic (39 instead of 66 / 84 products per link, 24 stored "
+                         "3-link staples per site): both fractions are reported; time per site is the figure of merit"})
         del sbuf
         cfg2 = cfg4 = None
         if not args.quick:
@@ -560,7 +566,12 @@ def run_ours(args):
 
 
 # flops per LINK each staples variant executes: SU(3) product = 198, scaled add = 36
-STAPLES_EXEC_FLOP_PER_LINK = {0: 84 * 198 + 24 * 36, 1: 3 * (22 * 198 + 10 * 36)}
+# executed flops per link: variant 2 = 30 products in pass 2 + 9 (36 per site) in pass 1, and per nu 2 W-sums,
+# 2 (c1 T3 + c0 C) combinations of 54 flops and 4 accumulations into S
+STAPLES_EXEC_FLOP_PER_LINK = {0: 84 * 198 + 24 * 36, 1: 3 * (22 * 198 + 10 * 36), 2: 39 * 198 + 3 * (6 * 36 + 2 * 54)}
+# two-pass staples: HBM bytes per site that the algorithm must move (fp64): pass 1 reads the links (576) and writes 24
+# fields (3456); pass 2 reads them and the links and writes the staples (576)
+STAPLES2_BYTES_PER_SITE = 576 + 3456 + 3456 + 576 + 576
 
 
 def dslash_rate(torch, L, D, gen, dims, U, in_e, in_o, prec, recon, peak, device, n=100, theta=None, bf_format=0,

@@ -407,6 +407,17 @@ template <typename T, int DM> __device__ __forceinline__ void acc_op(Su3<T> &s, 
             s.e[i][j].im = fma(DM ? -c : c, DM ? m.e[j][i].im : m.e[i][j].im, s.e[i][j].im);
         }
 }
+// x = cx * x + cm * op(m)
+template <typename T, int DM> __device__ __forceinline__ void scale_acc_op(Su3<T> &x, T cx_, T cm, const Su3<T> &m)
+{
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            x.e[i][j].re = fma(cx_, x.e[i][j].re, cm * (DM ? m.e[j][i].re : m.e[i][j].re));
+            x.e[i][j].im = fma(cx_, x.e[i][j].im, (DM ? -cm : cm) * (DM ? m.e[j][i].im : m.e[i][j].im));
+        }
+}
 template <typename T, int LAYOUT>
 __device__ __forceinline__ Su3<T> load_mat(const T *__restrict__ f, size_t plane0, size_t Vh, size_t i)
 {
@@ -515,47 +526,54 @@ __global__ void __launch_bounds__(128, MINB) staples_final_kernel(const Geom g, 
         const size_t i_n = (size_t)(i + dn_p), i_l = (size_t)(i + dn_m);                       // x + nu, x - nu
         const size_t i_ml = (size_t)((int)i_m + dn_m);                                           // x + mu - nu
         const int qmn = pair_idx(mu, nu), qnm = pair_idx(nu, mu);
+        // c0 Tu_munu(x) = c0 (A B) C and c0 Tl_munu(x) = c0 (A' B') C' are folded into the (A B) products, so the
+        // link's own two staple fields are not loaded: 6 matrix loads and 5 products per half.
         {   // above the link
+            const Su3<T> Ub = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, mu, Ls, i_n, pol);           // U_mu(x+nu)
+            const Su3<T> A = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, nu, Ls, i_m, pol);            // U_nu(x+mu)
             Su3<T> W;
             {
-                const Su3<T> Ub = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, mu, Ls, i_n, pol);       // U_mu(x+nu)
-                {
-                    const Su3<T> T1 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qnm, 0), Vh, i_m);         // Tu_numu(x+mu)
-                    W = mul_op<T, 1, 1>(T1, Ub);                                                            // T1^+ B
-                }
-                const Su3<T> A = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, nu, Ls, i_m, pol);        // U_nu(x+mu)
-                {
-                    const Su3<T> T2 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qmn, 0), Vh, i_n);         // Tu_munu(x+nu)
-                    acc_op<T, 0>(W, (T)1, mul_op<T, 0, 0>(A, T2));
-                }
-                const Su3<T> AB = mul_op<T, 0, 1>(A, Ub);
-                const Su3<T> T3 = load_mat<T, LAYOUT>(tf, tfield_plane(parity, qnm, 1), Vh, (size_t)i);   // Tl_numu(x)
-                acc_op<T, 0>(S, c1, mul_op<T, 0, 0>(AB, T3));
+                const Su3<T> T1 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qnm, 0), Vh, i_m);             // Tu_numu(x+mu)
+                W = mul_op<T, 1, 1>(T1, Ub);                                                                // T1^+ B
             }
+            {
+                const Su3<T> T2 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qmn, 0), Vh, i_n);             // Tu_munu(x+nu)
+                acc_op<T, 0>(W, (T)1, mul_op<T, 0, 0>(A, T2));
+            }
+            const Su3<T> AB = mul_op<T, 0, 1>(A, Ub);
             const Su3<T> Uc = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity, nu, Ls, (size_t)i, pol); // U_nu(x)
+            {
+                Su3<T> X = load_mat<T, LAYOUT>(tf, tfield_plane(parity, qnm, 1), Vh, (size_t)i);          // Tl_numu(x)
+                scale_acc_op<T, 1>(X, c1, c0, Uc);                                                          // c1 T3 + c0 C
+                acc_op<T, 0>(S, (T)1, mul_op<T, 0, 0>(AB, X));
+            }
             acc_op<T, 0>(S, c1, mul_op<T, 0, 1>(W, Uc));
-            acc_op<T, 0>(S, c0, load_mat<T, LAYOUT>(tf, tfield_plane(parity, qmn, 0), Vh, (size_t)i));    // Tu_munu(x)
         }
         {   // below the link
+            const Su3<T> Ub = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, mu, Ls, i_l, pol);           // U_mu(x-nu)
+            const Su3<T> Ua = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity, nu, Ls, i_ml, pol);      // U_nu(x+mu-nu)
             Su3<T> W;
             {
-                const Su3<T> Ub = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, mu, Ls, i_l, pol);       // U_mu(x-nu)
-                {
-                    const Su3<T> T1 = load_mat<T, LAYOUT>(tf, tfield_plane(parity, qnm, 0), Vh, i_ml);    // Tu_numu(x+mu-nu)
-                    W = mul_op<T, 0, 1>(T1, Ub);
-                }
-                const Su3<T> Ua = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity, nu, Ls, i_ml, pol);  // U_nu(x+mu-nu)
-                {
-                    const Su3<T> T2 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qmn, 1), Vh, i_l);         // Tl_munu(x-nu)
-                    acc_op<T, 0>(W, (T)1, mul_op<T, 1, 0>(Ua, T2));
-                }
-                const Su3<T> AB = mul_op<T, 1, 1>(Ua, Ub);
-                const Su3<T> T3 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qnm, 1), Vh, i_l);             // Tl_numu(x-nu)
-                acc_op<T, 0>(S, c1, mul_op<T, 0, 1>(AB, T3));
+                const Su3<T> T1 = load_mat<T, LAYOUT>(tf, tfield_plane(parity, qnm, 0), Vh, i_ml);        // Tu_numu(x+mu-nu)
+                W = mul_op<T, 0, 1>(T1, Ub);
             }
+            {
+                const Su3<T> T2 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qmn, 1), Vh, i_l);             // Tl_munu(x-nu)
+                acc_op<T, 0>(W, (T)1, mul_op<T, 1, 0>(Ua, T2));
+            }
+            const Su3<T> AB = mul_op<T, 1, 1>(Ua, Ub);
             const Su3<T> Uc = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, nu, Ls, i_l, pol);           // U_nu(x-nu)
+            {
+                const Su3<T> T3 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qnm, 1), Vh, i_l);             // Tl_numu(x-nu)
+                Su3<T> X;                                                                                   // c1 T3^+ + c0 C'
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+#pragma unroll
+                    for (int b = 0; b < 3; ++b)
+                        X.e[a][b] = cx<T>(fma(c1, T3.e[b][a].re, c0 * Uc.e[a][b].re), fma(-c1, T3.e[b][a].im, c0 * Uc.e[a][b].im));
+                acc_op<T, 0>(S, (T)1, mul_op<T, 0, 0>(AB, X));
+            }
             acc_op<T, 0>(S, c1, mul_op<T, 0, 0>(W, Uc));
-            acc_op<T, 0>(S, c0, load_mat<T, LAYOUT>(tf, tfield_plane(parity, qmn, 1), Vh, (size_t)i));    // Tl_munu(x)
         }
     }
     store_mat_stream<T, LAYOUT>(staples, (size_t)((parity * 4 + mu) * 9), Vh, (size_t)i, S);
@@ -590,7 +608,7 @@ extern "C" int lqcd_gauge_staples(lqcd_ctx *ctx, const void *links, void *staple
     if (two_pass) {
         dim3 gridp(((ctx->g.Vh + 127) / 128) * 24);
         int minb = ctx->staples_minblocks;           // launch-bounds variant of pass 2 (0: default per precision)
-        if (minb == 0) minb = ctx->prec == LQCD_F64 ? 3 : 3;
+        if (minb == 0) minb = ctx->prec == LQCD_F64 ? 2 : 3;
 #define GO2(T, L, R) do { \
         launch_k(ctx, staples_produce_kernel<T, L, R>, gridp, block, ctx->g, (T *)ctx->ws, (const T *)links); \
         if (minb == 2) launch_k(ctx, staples_final_kernel<T, L, R, 2>, grid, block, ctx->g, (T *)staples, (const T *)links, (const T *)ctx->ws, (T)c0, (T)c1, sw); \

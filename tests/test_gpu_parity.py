@@ -382,9 +382,11 @@ def test_gauge_staples(dims, prec, recon):
     links = lat.pack_links(U)
     for c0, c1 in ((oracle.SYMANZIK_C0, oracle.SYMANZIK_C1), (1.0, 0.0), (0.0, 1.0)):
         want = oracle.gauge_staples(dims, U, c0, c1)
-        for variant in (0, 1):       # one product chain per path / shared sub-products per (mu, nu)
+        # one product chain per path / shared sub-products per (mu, nu) / two passes through stored 3-link staples
+        for variant in (0, 1, 2):
             lat.set_option("staples_variant", variant)
             got = lat.unpack_force(lat.gauge_staples(links, c0, c1))
+            assert lat.get_option("staples_ran") == variant
             assert rel(got, want) < TOL[prec], (dims, prec, recon, c0, c1, variant, rel(got, want))
             link_err = np.linalg.norm((got - want).reshape(-1, 9), axis=1).max()
             assert link_err / np.linalg.norm(want.reshape(-1, 9), axis=1).mean() < 10 * TOL[prec]
@@ -400,16 +402,49 @@ def test_gauge_staples_cta_swizzle(x2b):
     rng = np.random.default_rng(16)
     U = gen.smooth_links(dims, 0.5, rng)
     want = oracle.gauge_staples(dims, U)
-    for variant in (0, 1):
+    for variant in (0, 1, 2):
         lat = make_lattice(dims, staples_x2block=x2b, staples_variant=variant)
         got = lat.unpack_force(lat.gauge_staples(lat.pack_links(U)))
         assert rel(got, want) < 1e-12, (x2b, variant, rel(got, want))
         lat.close()
 
 
+@pytest.mark.parametrize("layout", [0, 1])
+@pytest.mark.parametrize("minb", [2, 3, 4])
+def test_gauge_staples_two_pass_variants_and_workspace(minb, layout):
+    """Variant 2 (two passes through the 24 stored 3-link staples per site): every launch-bounds instantiation
+    of its second kernel, both layouts; without a large enough workspace the one-pass kernel runs instead and
+    gives the same field (through the raw C call: the binding would allocate the workspace)."""
+    import ctypes as C
+    import paper_1701_00426_b200 as L
+    dims = (6, 4, 10, 8)
+    rng = np.random.default_rng(18)
+    U = gen.smooth_links(dims, 0.5, rng)
+    want = oracle.gauge_staples(dims, U)
+    lat = make_lattice(dims, staples_minblocks=minb, layout=layout)
+    links = lat.pack_links(U)
+    out = lat._buf(int(L.lib.lqcd_force_bytes(lat._ctx)))
+    rc = L.lib.lqcd_gauge_staples(lat._ctx, C.c_void_p(links.data_ptr()), C.c_void_p(out.data_ptr()), 5.0 / 3.0, -1.0 / 12.0)
+    assert rc == 0 and lat.get_option("staples_ran") == 1          # no workspace yet
+    assert rel(lat.unpack_force(out), want) < 1e-12
+    lat.ensure_workspace(1)                                          # a solver-sized workspace is too small
+    assert lat._ws.numel() < int(L.lib.lqcd_staples_workspace_bytes(lat._ctx))
+    rc = L.lib.lqcd_gauge_staples(lat._ctx, C.c_void_p(links.data_ptr()), C.c_void_p(out.data_ptr()), 5.0 / 3.0, -1.0 / 12.0)
+    assert rc == 0 and lat.get_option("staples_ran") == 1
+    got = lat.unpack_force(lat.gauge_staples(links))                 # the binding sizes the workspace
+    assert lat.get_option("staples_ran") == 2
+    assert rel(got, want) < 1e-12
+    # the workspace is shared with the solvers: a solve afterwards still works
+    b = gen.gaussian_half_spinor(dims, rng)
+    x = lat.new_spinor()
+    r = lat.cg(x, lat.pack_spinor(b, 0), links, 0.2, 1e-10, 2000)
+    assert r["rel_resid"] < 1.5e-10
+    lat.close()
+
+
 def test_next_rows_on_a_paper_lattice_shape():
     """NEXT-3 / NEXT-4 at one of the paper's Table 3 / 4 shapes, 32^2 x 8 x 32, in the
-    default launch configuration (shared sub-products, x2-blocked CTA order really applied: rows are 4
+    default launch configuration (two-pass staples, x2-blocked CTA order really applied: rows are 4
     tiles; 8 shifts staged in shared memory): every link against the oracle."""
     dims = (32, 32, 8, 32)
     rng = np.random.default_rng(5)
@@ -417,6 +452,7 @@ def test_next_rows_on_a_paper_lattice_shape():
     lat = make_lattice(dims)
     links = lat.pack_links(U)
     got = lat.unpack_force(lat.gauge_staples(links))
+    assert lat.get_option("staples_ran") == 2
     want = oracle.gauge_staples(dims, U)
     assert rel(got, want) < 1e-12
     assert np.abs(got - want).max() < 1e-11
