@@ -300,6 +300,50 @@ int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_parity, lqcd_ha
                   lqcd_allreduce_fn allreduce, void *user);
 
 /*
+ * ---- Slab mode over peer-to-peer memory inside one node (the native transport; "direct
+ * P2P stores into the neighbour's ghost slice", two all-reduces of one double per CG iteration) --------------------
+ * No communication library and no host code between the kernels: every rank owns one block of device memory
+ * (flags, P slots per reduction, four landing buffers for halo faces) that all ranks of the node map -- through
+ * CUDA IPC with one process per GPU, or as plain pointers when the ranks share a process.  Per Dslash one small
+ * kernel stores the two boundary slices of the input vector (times the boundary sign) straight into the
+ * neighbours' landing buffers and raises their flags; the Dslash kernel waits for its two flags at its start and
+ * reads the x3 hops that leave the slab from the landing buffers.  Dot products: the last CTA of the producing
+ * kernel stores the local sum into every rank's slot and raises a flag; the consumer kernel (K1 after <p,q>, K2
+ * after <r,r>) waits for the P flags and adds the P slots in rank order, so every rank gets the bit-identical
+ * total and takes the same decisions.  The waits are inside the kernels: the CG loop stays one CUDA graph per
+ * chunk of iterations.  Flags are monotone counters; re-use of slots and landing buffers is ordered by the two
+ * all-reduces of every iteration.
+ *   lqcd_peer_init      allocate the block; the context must have local extents (N0,N1,N2,L3+2) and antiperiodic_t
+ *                       = 0 as described above; x3_lo/x3_hi/solve_parity as in lqcd_set_slab; sign_up / sign_down:
+ *                       factor applied to the face sent to the rank above / below (-1 where the hop crosses an
+ *                       antiperiodic global boundary, reading R4).  *block (may be NULL): the block's device
+ *                       address.  1 <= nranks <= 16.  blocking.
+ *   lqcd_peer_export    CUDA IPC handle (64 bytes) of the block, for the other processes
+ *   lqcd_peer_import    map another rank's block from its handle -> device pointer valid in this process
+ *   lqcd_peer_connect   blocks[r] = device pointer to rank r's block for every r (blocks[rank] is ignored);
+ *                       from now on lqcd_dslash, lqcd_mdagm, lqcd_cg, lqcd_cg_multishift and
+ *                       lqcd_rational_apply of this context exchange faces and sums through the blocks.
+ *                       lqcd_dslash_slices stays raw (reads the vector's own ghost slices).
+ *   lqcd_peer_disconnect  back to a single-rank context (frees the block, closes imported mappings).  blocking.
+ * All ranks must issue the same sequence of calls (as with any collective).  With nranks = 1 the rank is its own
+ * neighbour.  A backfield, lqcd_fermion_force and lqcd_gauge_staples are LQCD_ERR_UNSUPPORTED in this mode.
+ * The kernels of different ranks wait for one another: run each rank on its own GPU.  For validation on ONE GPU
+ * lqcd_set_phase_hook installs a host callback that the library calls after every launch that publishes to the
+ * peers (what = 0: face push, 1: generic all-reduce, 2: dot product); a test harness that synchronises its stream
+ * there and then meets the other ranks at a host barrier runs the ranks in lock step, so that no kernel ever
+ * waits (the chunk graph is off while a hook is set).  Pass NULL to clear.
+ */
+typedef int (*lqcd_phase_fn)(void *user, int what);
+size_t lqcd_peer_block_bytes(const lqcd_ctx *ctx);
+int lqcd_peer_init(lqcd_ctx *ctx, int nranks, int rank, int x3_lo, int x3_hi, int solve_parity,
+                   double sign_up, double sign_down, void **block);
+int lqcd_peer_export(lqcd_ctx *ctx, void *handle64);
+int lqcd_peer_import(lqcd_ctx *ctx, int rank, const void *handle64, void **block);
+int lqcd_peer_connect(lqcd_ctx *ctx, void *const *blocks);
+int lqcd_peer_disconnect(lqcd_ctx *ctx);
+int lqcd_set_phase_hook(lqcd_ctx *ctx, lqcd_phase_fn fn, void *user);
+
+/*
  * After lqcd_cg / lqcd_cg_multishift: copy up to `n` entries of the per-iteration history
  * (alpha_k, beta_k, ||r_{k+1}||) of the last solve to host arrays (any may be NULL).
  * Returns the number of entries available (<= 64), or a negative status.

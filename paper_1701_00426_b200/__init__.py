@@ -14,5 +14,5 @@ from .binding import (  # noqa: F401
     OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOT_CONVERGED, ERR_WORKSPACE,
     MAX_SHIFTS,
     version,
-    HALO_FN, ALLREDUCE_FN,
+    HALO_FN, ALLREDUCE_FN, PHASE_FN,
 )

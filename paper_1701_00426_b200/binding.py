@@ -39,6 +39,7 @@ _vp, _i, _d, _sz = C.c_void_p, C.c_int, C.c_double, C.c_size_t
 _pi, _pd = C.POINTER(C.c_int), C.POINTER(C.c_double)
 HALO_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int)        # lqcd_halo_fn
 ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int)   # lqcd_allreduce_fn
+PHASE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int)                   # lqcd_phase_fn
 _sig = {
     "lqcd_version": (C.c_char_p, []),
     "lqcd_create": (_i, [C.POINTER(_vp), C.POINTER(_i), _i, _i, _i, _i, _vp]),
@@ -76,6 +77,13 @@ _sig = {
     "lqcd_halo_pack_faces": (_i, [_vp, _vp, _vp, _vp, _d, _d]),
     "lqcd_halo_unpack_ghosts": (_i, [_vp, _vp, _vp, _vp]),
     "lqcd_set_slab": (_i, [_vp, _i, _i, _i, HALO_FN, ALLREDUCE_FN, _vp]),
+    "lqcd_peer_block_bytes": (_sz, [_vp]),
+    "lqcd_peer_init": (_i, [_vp, _i, _i, _i, _i, _i, _d, _d, C.POINTER(_vp)]),
+    "lqcd_peer_export": (_i, [_vp, _vp]),
+    "lqcd_peer_import": (_i, [_vp, _i, _vp, C.POINTER(_vp)]),
+    "lqcd_peer_connect": (_i, [_vp, C.POINTER(_vp)]),
+    "lqcd_peer_disconnect": (_i, [_vp]),
+    "lqcd_set_phase_hook": (_i, [_vp, PHASE_FN, _vp]),
     "lqcd_solver_history": (_i, [_vp, _i, _pd, _pd, _pd]),
     "lqcd_dslash_host": (_i, [_vp, _i, _vp, _vp, _vp]),
     "lqcd_dslash_host_vectors": (_i, [_vp, _i, _vp, _vp, _vp]),
@@ -263,6 +271,37 @@ class Lattice:
         self._check(lib.lqcd_set_slab(self._ctx, x3_lo, x3_hi, solve_parity,
                                       halo_cb if halo_cb is not None else HALO_FN(),
                                       allreduce_cb if allreduce_cb is not None else ALLREDUCE_FN(), None))
+
+    # -- slab mode over the peer transport (lqcd_peer_*) ------------------------------------------------
+    def peer_init(self, nranks, rank, x3_lo, x3_hi, solve_parity, sign_up, sign_down):
+        """allocate this rank's block; returns its device address."""
+        blk = _vp()
+        self._check(lib.lqcd_peer_init(self._ctx, nranks, rank, x3_lo, x3_hi, solve_parity, float(sign_up),
+                                       float(sign_down), C.byref(blk)))
+        return int(blk.value)
+
+    def peer_export(self):
+        """64-byte CUDA IPC handle of this rank's block."""
+        h = C.create_string_buffer(64)
+        self._check(lib.lqcd_peer_export(self._ctx, h))
+        return h.raw
+
+    def peer_import(self, rank, handle):
+        blk = _vp()
+        self._check(lib.lqcd_peer_import(self._ctx, rank, C.create_string_buffer(bytes(handle), 64), C.byref(blk)))
+        return int(blk.value)
+
+    def peer_connect(self, blocks):
+        arr = (_vp * len(blocks))(*[int(b) if b else None for b in blocks])
+        self._check(lib.lqcd_peer_connect(self._ctx, arr))
+
+    def peer_disconnect(self):
+        self._check(lib.lqcd_peer_disconnect(self._ctx))
+
+    def set_phase_hook(self, cb=None):
+        """cb: a PHASE_FN instance (kept alive here) or None."""
+        self._phase_cb = cb
+        self._check(lib.lqcd_set_phase_hook(self._ctx, cb if cb is not None else PHASE_FN(), None))
 
     def mdagm(self, out_e, in_e, links, mass, sigma=0.0):
         self.ensure_workspace(1)

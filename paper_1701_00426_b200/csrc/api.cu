@@ -118,6 +118,7 @@ extern "C" int lqcd_destroy(lqcd_ctx *ctx)
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     clear_l2_window(ctx);
+    lqcd_peer_destroy(ctx);
     cudaFree(ctx->d_state);
     cudaFree(ctx->d_partials);
     cudaFreeHost(ctx->h_flag);
@@ -322,6 +323,7 @@ extern "C" int lqcd_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in,
     REQUIRE(out && in && links, "lqcd_dslash: null pointer");
     REQUIRE(parity == 0 || parity == 1, "lqcd_dslash: parity %d", parity);
     REQUIRE(out != in, "lqcd_dslash: out and in alias");
+    if (ctx->peer_on && (rc = launch_peer_push(ctx, in, 1 - parity, 0))) return rc;     // faces of `in` to the neighbours
     return launch_dslash(ctx, parity, out, in, links, NULL, 0.0, 0, 0);
 }
 
@@ -416,6 +418,7 @@ extern "C" int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_pari
     REQUIRE(solve_parity == 0 || solve_parity == 1, "lqcd_set_slab: solve_parity %d", solve_parity);
     REQUIRE(0 <= x3_lo && x3_lo < x3_hi && x3_hi <= ctx->g.N3, "lqcd_set_slab: bad slice range [%d,%d)", x3_lo, x3_hi);
     REQUIRE((halo == NULL) == (allreduce == NULL), "lqcd_set_slab: give both hooks or neither");
+    REQUIRE(!ctx->peer_mem, "lqcd_set_slab: the context uses the peer transport (lqcd_peer_init); call lqcd_peer_disconnect first");
     ctx->solve_parity = solve_parity;
     ctx->x3_lo = x3_lo; ctx->x3_hi = x3_hi;
     ctx->halo_fn = halo; ctx->allreduce_fn = allreduce; ctx->comm_user = user;
@@ -431,9 +434,11 @@ extern "C" int lqcd_mdagm(lqcd_ctx *ctx, void *out_e, const void *in_e, const vo
     if (!ctx->ws) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "lqcd_mdagm: no workspace set");
     void *tmp_o = ws_vec(ctx, 0);
     const int par = ctx->solve_parity;     // LQCD_EVEN unless a slab says otherwise
-    if (ctx->halo_fn && ctx->halo_fn(ctx->comm_user, (void *)in_e, par)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "halo hook failed");
+    if (ctx->peer_on) { if ((rc = launch_peer_push(ctx, in_e, par, 0))) return rc; }
+    else if (ctx->halo_fn && ctx->halo_fn(ctx->comm_user, (void *)in_e, par)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "halo hook failed");
     rc = launch_dslash(ctx, 1 - par, tmp_o, in_e, links, NULL, 0.0, 0, 0);
     if (rc) return rc;
-    if (ctx->halo_fn && ctx->halo_fn(ctx->comm_user, tmp_o, 1 - par)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "halo hook failed");
+    if (ctx->peer_on) { if ((rc = launch_peer_push(ctx, tmp_o, 1 - par, 0))) return rc; }
+    else if (ctx->halo_fn && ctx->halo_fn(ctx->comm_user, tmp_o, 1 - par)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "halo hook failed");
     return launch_dslash(ctx, par, out_e, tmp_o, links, in_e, mass * mass + sigma, 0, 0);
 }

@@ -206,10 +206,33 @@ struct SolverState {
     int nshift, iter;
     int done;              // 0 running; 1 converged in this iteration (K2 still to run); 2 finished
     unsigned int ticket;   // last-block-done counter of the reductions
-    int comm;              // slab mode: reductions leave LOCAL sums in sum[] (0: <p,q>, 1: <r,r>, 2: <b,b>); the
-    double sum[4];         // recurrences run in scalar_kernel after the caller's all-reduce
+    int comm;              // slab mode.  1 (hooks): reductions leave LOCAL sums in sum[] (0: <p,q>, 1: <r,r>, 2: <b,b>); the
+    double sum[4];         // recurrences run in scalar_kernel after the caller's all-reduce.  2 (peer transport):
+                           // the last CTA publishes the local sum to every rank, the consumer kernel gathers (peer.cuh)
     double resid[LQCD_MAX_SHIFTS];  // ||b - (A+sigma_i) x_i||^2 recomputed at exit
     double hist_alpha[LQCD_HIST], hist_beta[LQCD_HIST], hist_rnorm[LQCD_HIST];
+};
+
+// ------------------------------------------------------------------------------------------
+// Slab mode, peer-to-peer transport (peer.cuh; lqcd_peer_* in lqcd.h).  One PeerBlock per rank, in that rank's
+// device memory, written by the other ranks of the node through peer / IPC mappings; the landing buffers of the
+// halo faces follow it in the same allocation.
+// ------------------------------------------------------------------------------------------
+#define LQCD_MAX_RANKS 16
+struct PeerBlock {
+    unsigned int flag_halo[2][2];                 // [exchange kind = parity of the pushed vector][0: from down, 1: from up]
+    unsigned int flag_red[3][LQCD_MAX_RANKS];     // [0: <p,q>, 1: <r,r>, 2: generic][sender]: the sender's counter
+    unsigned int cnt_halo[2], cnt_red[3];         // LOCAL counters (only this rank writes them)
+    unsigned int ticket, pad_[2];
+    double slot[3][2][LQCD_MAX_RANKS][LQCD_MAX_SHIFTS];   // [kind][counter parity][sender][value]
+};
+struct PeerDev {                                  // lives in device memory (ctx->d_peer); kernels get a pointer
+    int nranks, rank;
+    PeerBlock *self;
+    PeerBlock *peer[LQCD_MAX_RANKS];              // peer[rank] == self
+    void *land_self[2][2];                        // my landing buffers [kind][0: from down, 1: from up]
+    void *land_up[2], *land_down[2];              // [kind]: up neighbour's "from down" buffer, down neighbour's "from up" buffer
+    PeerBlock *up, *down;
 };
 
 // ------------------------------------------------------------------------------------------
@@ -241,6 +264,14 @@ struct lqcd_ctx {
     // ghost slice on each side; only the slices [x3_lo, x3_hi) are owned (default: all of them)
     int x3_lo, x3_hi;
     int solve_parity;      // local parity of the sites the solvers act on (default LQCD_EVEN)
+    // peer-to-peer transport (lqcd_peer_init / lqcd_peer_connect): library-owned block + landing buffers
+    int peer_on;                     // 1 after lqcd_peer_connect: solvers, lqcd_dslash and lqcd_mdagm use it
+    int peer_nranks, peer_rank;
+    double peer_sign_up, peer_sign_down;   // boundary sign applied by the SENDER to the face sent up / down
+    void *peer_mem; size_t peer_mem_bytes; // cudaMalloc: PeerBlock + 4 landing buffers
+    PeerDev h_peer, *d_peer;
+    void *peer_opened[LQCD_MAX_RANKS];     // IPC mappings to close (NULL: not ours)
+    lqcd_phase_fn phase_fn; void *phase_user;   // validation hook: called after every launch that publishes to peers
     lqcd_halo_fn halo_fn;            // fills the ghost slices of a half vector (NULL: nothing to do)
     lqcd_allreduce_fn allreduce_fn;  // sums device doubles over the ranks (NULL: single rank)
     void *comm_user;
@@ -328,4 +359,9 @@ int launch_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical, const void 
 int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
                   const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo = -1, int x3_hi = -1);
 int launch_halo(lqcd_ctx *ctx, int pack, void *buf, void *spinor, int x3, double sign);
+// peer transport (peer.cu): push both faces of `spinor` (a vector of local parity `parity`) to the neighbours
+int launch_peer_push(lqcd_ctx *ctx, const void *spinor, int parity, int gate);
+int peer_phase(lqcd_ctx *ctx, int what);     // lock-step validation hook (no-op unless set)
+int launch_peer_allreduce(lqcd_ctx *ctx, double *vals, int nv, int which);
+void lqcd_peer_destroy(lqcd_ctx *ctx);
 int launch_halo2(lqcd_ctx *ctx, int pack, void *buf0, void *buf1, void *spinor, int x3_0, int x3_1, double sign0, double sign1);

@@ -15,6 +15,7 @@
 // The kernel is bound by HBM bandwidth (1248 B/site fp64 18-real vs 570 flop/site): no tensor cores.
 #include "reduce.cuh"
 
+#include "peer.cuh"
 #include "su3.cuh"
 
 // acc += U p
@@ -49,12 +50,15 @@ template <typename T> __device__ __forceinline__ void mvdag_acc(Cx<T> acc[3], co
 // PAPER.md:320-326; reading R6), [parity][mu][idxh]; the phase multiplies the neighbour vector together with
 // eta / the boundary sign, AFTER the third row was rebuilt from the SU(3) link.  BF 1: theta stored, one real per
 // link, sincos in-kernel; BF 2: (cos theta, sin theta) stored (option backfield_format).
-template <typename T, int LAYOUT, int RECON12, int MODE, int MINB, int POLICY, int BF>
+// HALO 1 (slab mode over the peer transport, peer.cuh): [i_begin, i_end) are the owned slices; the kernel first
+// waits for the two faces of `in` pushed by the neighbours and takes the x3 hops that leave the slab from the
+// landing buffers instead of the vector's ghost slices; MODE 2 publishes the local <x,out> to every rank.
+template <typename T, int LAYOUT, int RECON12, int MODE, int MINB, int POLICY, int BF, int HALO>
 __global__ void __launch_bounds__(256, MINB)
 dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__restrict__ in,
               const T *__restrict__ links, const T *__restrict__ xin, const double coef,
               SolverState *__restrict__ st, double *__restrict__ partials, const int gate,
-              const int i_begin, const int i_end, const T *__restrict__ bf)
+              const int i_begin, const int i_end, const T *__restrict__ bf, const PeerDev *__restrict__ pdp)
 {
     pdl_wait();
     pdl_trigger();
@@ -65,6 +69,7 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
             return;
         }
     }
+    if (HALO) peer_wait_halo(*pdp, 1 - parity);
     double dot = 0.0;
     L2Pol pol = {0, 0};
     if (POLICY) pol = make_l2pol();
@@ -116,7 +121,9 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
             {
                 Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, parity, mu, (size_t)g.Ls, (size_t)i, pol);
                 Cx<T> p[3];
-                if (BF == 1) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], __ldcs(bf + (size_t)(parity * 4 + mu) * Vh + i), p, pol);
+                if (HALO && mu == 3 && nf[3] >= i_end)
+                    load_vec_cg<T, LAYOUT>((const T *)pdp->land_self[1 - parity][1], (size_t)g.s3, (size_t)(nf[3] - i_end), cf[3], p);
+                else if (BF == 1) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], __ldcs(bf + (size_t)(parity * 4 + mu) * Vh + i), p, pol);
                 else if (BF == 2) load_vec_unit<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], (T)1, bf, (size_t)(parity * 4 + mu) * Vh + i, p, pol);
                 else load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], p, pol);
                 mv_acc<T>(acc, u, p);
@@ -124,7 +131,9 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
             {
                 Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, 1 - parity, mu, (size_t)g.Ls, (size_t)nb[mu], pol);
                 Cx<T> p[3];
-                if (BF == 1) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], -__ldcs(bf + (size_t)((1 - parity) * 4 + mu) * Vh + nb[mu]), p, pol);
+                if (HALO && mu == 3 && nb[3] < i_begin)
+                    load_vec_cg<T, LAYOUT>((const T *)pdp->land_self[1 - parity][0], (size_t)g.s3, (size_t)(nb[3] - (i_begin - g.s3)), cb[3], p);
+                else if (BF == 1) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], -__ldcs(bf + (size_t)((1 - parity) * 4 + mu) * Vh + nb[mu]), p, pol);
                 else if (BF == 2) load_vec_unit<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], (T)-1, bf, (size_t)((1 - parity) * 4 + mu) * Vh + nb[mu], p, pol);
                 else load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], p, pol);
                 mvdag_acc<T>(acc, u, p);
@@ -145,7 +154,10 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
     }
     }
     if (MODE == 2) {
-        if (st->comm) {   // slab mode: the caller all-reduces the LOCAL total (lqcd_set_slab)
+        if (HALO) {       // slab mode, peer transport: the last CTA publishes the LOCAL total to every rank
+            double total;
+            if (grid_sum_last(dot, partials, &st->ticket, &total)) peer_publish(*pdp, 0, &total, 1);
+        } else if (st->comm) {   // slab mode: the caller all-reduces the LOCAL total (lqcd_set_slab)
             double total;
             if (grid_sum_last(dot, partials, &st->ticket, &total)) st->sum[0] = total;
         } else {          // the next kernel (K1) adds the partials up itself: no fence, no ticket, no tail
@@ -157,7 +169,7 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
 
 template <typename T, int LAYOUT, int RECON12, int MODE>
 static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
-                     const void *xin, double coef, int gate, int i_begin, int i_end)
+                     const void *xin, double coef, int gate, int i_begin, int i_end, int halo_in)
 {
     int block = ctx->dslash_block > 256 ? 256 : ctx->dslash_block;
     int tiles = (i_end - i_begin + block - 1) / block;
@@ -167,10 +179,13 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
     ctx->last_dslash_grid = tiles;
     int minb = ctx->dslash_minblocks;
     if (minb == 0) minb = sizeof(T) == 8 ? 2 : 4;   // profiles/experiments_r1b.md section 9
-#define GO1(MB, P, B) launch_k(ctx, dslash_kernel<T, LAYOUT, RECON12, MODE, MB, P, B>, grid, dim3(block), \
+#define GO1(MB, P, B) GO2(MB, P, B, 0)
+#define GO2(MB, P, B, H) launch_k(ctx, dslash_kernel<T, LAYOUT, RECON12, MODE, MB, P, B, H>, grid, dim3(block), \
         ctx->g, parity, (T *)out, (const T *)in, (const T *)links, (const T *)xin, coef, ctx->d_state, ctx->d_partials, gate, i_begin, i_end, \
-        (const T *)ctx->backfield)
+        (const T *)ctx->backfield, (const PeerDev *)ctx->d_peer)
 #define GO(MB) do { if (ctx->l2_hints) GO1(MB, 1, 0); else GO1(MB, 0, 0); } while (0)
+    // peer transport: the per-precision default variant, faces read from the landing buffers (halo_in)
+    if (halo_in) { if (sizeof(T) == 8) GO2(2, 0, 0, 1); else GO2(4, 0, 0, 1); } else
     // with a backfield: the per-precision default variant only (the tuning options dslash_minblocks and
     // l2_hints select nothing there)
     if (ctx->backfield && ctx->backfield_format == 0) { if (sizeof(T) == 8) GO1(2, 0, 1); else GO1(4, 0, 1); }
@@ -178,13 +193,14 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
     else if (minb <= 2) GO(2); else if (minb == 3) GO(3); else GO(4);
 #undef GO
 #undef GO1
+#undef GO2
 }
 
 template <typename T, int LAYOUT>
 static void launch_tl(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
-                      const void *xin, double coef, int mode, int gate, int i_begin, int i_end)
+                      const void *xin, double coef, int mode, int gate, int i_begin, int i_end, int halo_in)
 {
-#define GO(R, M) launch_t<T, LAYOUT, R, M>(ctx, parity, out, in, links, xin, coef, gate, i_begin, i_end)
+#define GO(R, M) launch_t<T, LAYOUT, R, M>(ctx, parity, out, in, links, xin, coef, gate, i_begin, i_end, halo_in)
     if (ctx->recon == LQCD_RECON_12) { if (mode == 0) GO(1, 0); else if (mode == 1) GO(1, 1); else GO(1, 2); }
     else { if (mode == 0) GO(0, 0); else if (mode == 1) GO(0, 1); else GO(0, 2); }
 #undef GO
@@ -194,14 +210,18 @@ int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const vo
                   const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo, int x3_hi)
 {
     int mode = xpay_in ? (dot_mode ? 2 : 1) : 0;
+    // peer transport: a Dslash over the context's owned slices reads the faces the neighbours pushed; an explicit
+    // slice range (lqcd_dslash_slices) reads the vector's own ghost slices as before
+    const int halo_in = ctx->peer_on && x3_lo < 0;
+    if (halo_in && ctx->backfield) return lqcd_fail(ctx, LQCD_ERR_UNSUPPORTED, "a backfield is not available over the peer transport");
     if (x3_lo < 0) { x3_lo = ctx->x3_lo; x3_hi = ctx->x3_hi; }      // the context's interior slices
     const int i_begin = x3_lo * ctx->g.s3, i_end = x3_hi * ctx->g.s3;
     if (ctx->prec == LQCD_F64) {
-        if (ctx->layout == 0) launch_tl<double, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end);
-        else launch_tl<double, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end);
+        if (ctx->layout == 0) launch_tl<double, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in);
+        else launch_tl<double, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in);
     } else {
-        if (ctx->layout == 0) launch_tl<float, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end);
-        else launch_tl<float, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end);
+        if (ctx->layout == 0) launch_tl<float, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in);
+        else launch_tl<float, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in);
     }
     return lqcd_check_cuda(ctx, cudaGetLastError(), "dslash");
 }

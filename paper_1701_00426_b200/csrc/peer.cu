@@ -1,0 +1,232 @@
+// peer.cu -- slab mode over peer-to-peer memory inside one node (the paper
+// leaves the multi-device version as future work): set-up of the per-rank PeerBlock, CUDA IPC
+// plumbing, the face-push kernel and the two generic publish / gather kernels.  Protocol: peer.cuh.
+#include <stdlib.h>
+
+#include "peer.cuh"
+#include "reduce.cuh"
+
+static size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
+static size_t land_bytes(const lqcd_ctx *ctx) { return align256(lqcd_halo_bytes(ctx)); }
+static size_t peer_block_bytes(const lqcd_ctx *ctx) { return align256(sizeof(PeerBlock)) + 4 * land_bytes(ctx); }
+static void *land_ptr(const lqcd_ctx *ctx, void *block, int kind, int dir)
+{
+    return (char *)block + align256(sizeof(PeerBlock)) + (size_t)(kind * 2 + dir) * land_bytes(ctx);
+}
+
+extern "C" size_t lqcd_peer_block_bytes(const lqcd_ctx *ctx) { return ctx ? peer_block_bytes(ctx) : 0; }
+
+static void peer_release(lqcd_ctx *ctx)
+{
+    for (int r = 0; r < LQCD_MAX_RANKS; ++r)
+        if (ctx->peer_opened[r]) { cudaIpcCloseMemHandle(ctx->peer_opened[r]); ctx->peer_opened[r] = NULL; }
+    if (ctx->peer_mem) cudaFree(ctx->peer_mem);
+    if (ctx->d_peer) cudaFree(ctx->d_peer);
+    ctx->peer_mem = NULL; ctx->d_peer = NULL; ctx->peer_on = 0; ctx->peer_nranks = 0;
+}
+void lqcd_peer_destroy(lqcd_ctx *ctx) { peer_release(ctx); }
+
+extern "C" int lqcd_peer_init(lqcd_ctx *ctx, int nranks, int rank, int x3_lo, int x3_hi, int solve_parity,
+                              double sign_up, double sign_down, void **block)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    int rc = lqcd_check_cuda(ctx, cudaSetDevice(ctx->device), "cudaSetDevice");
+    if (rc) return rc;
+    if (nranks < 1 || nranks > LQCD_MAX_RANKS || rank < 0 || rank >= nranks)
+        return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_peer_init: rank %d of %d (at most %d ranks)", rank, nranks, LQCD_MAX_RANKS);
+    if (solve_parity != 0 && solve_parity != 1) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_peer_init: solve_parity %d", solve_parity);
+    if (!(1 <= x3_lo && x3_lo < x3_hi && x3_hi <= ctx->g.N3 - 1))
+        return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_peer_init: owned slices [%d,%d) need a ghost slice on each side of [0,%d)", x3_lo, x3_hi, ctx->g.N3);
+    if (ctx->halo_fn) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_peer_init: the context already uses communication hooks (lqcd_set_slab)");
+    peer_release(ctx);
+    cudaError_t e;
+    ctx->peer_mem_bytes = peer_block_bytes(ctx);
+    if ((e = cudaMalloc(&ctx->peer_mem, ctx->peer_mem_bytes)) != cudaSuccess ||
+        (e = cudaMalloc(&ctx->d_peer, sizeof(PeerDev))) != cudaSuccess ||
+        (e = cudaMemset(ctx->peer_mem, 0, ctx->peer_mem_bytes)) != cudaSuccess ||
+        (e = cudaDeviceSynchronize()) != cudaSuccess) {
+        peer_release(ctx);
+        return lqcd_check_cuda(ctx, e, "lqcd_peer_init");
+    }
+    ctx->peer_nranks = nranks; ctx->peer_rank = rank;
+    ctx->peer_sign_up = sign_up; ctx->peer_sign_down = sign_down;
+    ctx->x3_lo = x3_lo; ctx->x3_hi = x3_hi; ctx->solve_parity = solve_parity;
+    if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
+    if (block) *block = ctx->peer_mem;
+    return LQCD_OK;
+}
+
+extern "C" int lqcd_peer_connect(lqcd_ctx *ctx, void *const *blocks)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    int rc = lqcd_check_cuda(ctx, cudaSetDevice(ctx->device), "cudaSetDevice");
+    if (rc) return rc;
+    if (!ctx->peer_mem) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_peer_connect: call lqcd_peer_init first");
+    if (!blocks) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_peer_connect: null pointer");
+    const int P = ctx->peer_nranks, me = ctx->peer_rank;
+    PeerDev &h = ctx->h_peer;
+    memset(&h, 0, sizeof(h));
+    h.nranks = P; h.rank = me;
+    h.self = (PeerBlock *)ctx->peer_mem;
+    for (int r = 0; r < P; ++r) {
+        void *b = r == me ? ctx->peer_mem : blocks[r];
+        if (!b) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_peer_connect: block of rank %d is null", r);
+        h.peer[r] = (PeerBlock *)b;
+    }
+    const int up = (me + 1) % P, down = (me + P - 1) % P;
+    h.up = h.peer[up]; h.down = h.peer[down];
+    for (int k = 0; k < 2; ++k) {
+        for (int d = 0; d < 2; ++d) h.land_self[k][d] = land_ptr(ctx, ctx->peer_mem, k, d);
+        h.land_up[k] = land_ptr(ctx, h.up, k, 0);       // my top slice is what the rank above receives "from down"
+        h.land_down[k] = land_ptr(ctx, h.down, k, 1);
+    }
+    if ((rc = lqcd_check_cuda(ctx, cudaMemcpy(ctx->d_peer, &h, sizeof(h), cudaMemcpyHostToDevice), "lqcd_peer_connect"))) return rc;
+    ctx->peer_on = 1;
+    if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
+    return LQCD_OK;
+}
+
+extern "C" int lqcd_peer_disconnect(lqcd_ctx *ctx)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    peer_release(ctx);
+    ctx->x3_lo = 0; ctx->x3_hi = ctx->g.N3; ctx->solve_parity = LQCD_EVEN;
+    if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
+    return LQCD_OK;
+}
+
+// ---- CUDA IPC plumbing for one process per GPU -------------------------------------------------------------------
+extern "C" int lqcd_peer_export(lqcd_ctx *ctx, void *handle64)
+{
+    if (!ctx || !handle64) return LQCD_ERR_ARG;
+    if (!ctx->peer_mem) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_peer_export: call lqcd_peer_init first");
+    cudaSetDevice(ctx->device);
+    cudaIpcMemHandle_t h;
+    static_assert(sizeof(h) == 64, "cudaIpcMemHandle_t is 64 bytes");
+    int rc = lqcd_check_cuda(ctx, cudaIpcGetMemHandle(&h, ctx->peer_mem), "cudaIpcGetMemHandle");
+    if (rc) return rc;
+    memcpy(handle64, &h, 64);
+    return LQCD_OK;
+}
+
+extern "C" int lqcd_peer_import(lqcd_ctx *ctx, int rank, const void *handle64, void **block)
+{
+    if (!ctx || !handle64 || !block) return LQCD_ERR_ARG;
+    if (rank < 0 || rank >= ctx->peer_nranks || rank == ctx->peer_rank) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_peer_import: rank %d", rank);
+    cudaSetDevice(ctx->device);
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle64, 64);
+    void *p = NULL;
+    int rc = lqcd_check_cuda(ctx, cudaIpcOpenMemHandle(&p, h, cudaIpcMemLazyEnablePeerAccess), "cudaIpcOpenMemHandle");
+    if (rc) return rc;
+    if (ctx->peer_opened[rank]) cudaIpcCloseMemHandle(ctx->peer_opened[rank]);
+    ctx->peer_opened[rank] = p;
+    *block = p;
+    return LQCD_OK;
+}
+
+extern "C" int lqcd_set_phase_hook(lqcd_ctx *ctx, lqcd_phase_fn fn, void *user)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    ctx->phase_fn = fn; ctx->phase_user = user;
+    if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
+    return LQCD_OK;
+}
+
+int peer_phase(lqcd_ctx *ctx, int what)
+{
+    if (!ctx->phase_fn) return LQCD_OK;
+    if (ctx->phase_fn(ctx->phase_user, what)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "phase hook failed");
+    return LQCD_OK;
+}
+
+// ---- face push ---------------------------------------------------------------------------------------------------
+// blockIdx.y = 0: my top owned slice (x3_hi - 1), times sign_up, -> the up neighbour's "from down" landing buffer;
+// blockIdx.y = 1: my bottom owned slice (x3_lo), times sign_down, -> the down neighbour's "from up" buffer.
+// The last CTA raises the neighbours' flags (every CTA has fenced its remote stores before taking a ticket).
+template <typename T, int LAYOUT>
+__global__ void __launch_bounds__(128) peer_push_kernel(const Geom g, const PeerDev *__restrict__ pdp, const int kind,
+                                                        const T *__restrict__ spinor, const int x3_lo, const int x3_hi,
+                                                        const T sign_up, const T sign_down, const SolverState *__restrict__ st,
+                                                        const int gate)
+{
+    pdl_wait();
+    pdl_trigger();
+    if (gate && *(volatile const int *)&st->done) return;     // a converged solve: every rank skips the same exchanges
+    const PeerDev &pd = *pdp;
+    const int up = blockIdx.y == 0;
+    T *__restrict__ buf = reinterpret_cast<T *>(up ? pd.land_up[kind] : pd.land_down[kind]);
+    const int x3 = up ? x3_hi - 1 : x3_lo;
+    const T sign = up ? sign_up : sign_down;
+    const int f = blockIdx.x * blockDim.x + threadIdx.x;
+    if (f < g.s3) {
+        const size_t i = (size_t)x3 * g.s3 + f;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const Cx<T> z = ld_cx<T, LAYOUT, 0, 0>(spinor, (size_t)c, (size_t)g.Vh, i, L2Pol());
+            st_cx<T, LAYOUT, 0>(buf, (size_t)c, (size_t)g.s3, (size_t)f, cx<T>(sign * z.re, sign * z.im), L2Pol());
+        }
+    }
+    __shared__ bool s_last;
+    __threadfence_system();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned int total = gridDim.x * gridDim.y;
+        const unsigned int t = atomicInc(&pd.self->ticket, total - 1);
+        s_last = (t == total - 1);
+    }
+    __syncthreads();
+    if (s_last && threadIdx.x == 0) {
+        __threadfence_system();
+        const unsigned int n = pd.self->cnt_halo[kind] + 1;
+        pd.self->cnt_halo[kind] = n;
+        st_flag(&pd.up->flag_halo[kind][0], n);        // the rank above sees its "from down" face
+        st_flag(&pd.down->flag_halo[kind][1], n);
+    }
+}
+
+int launch_peer_push(lqcd_ctx *ctx, const void *spinor, int parity, int gate)
+{
+    dim3 grid((ctx->g.s3 + 127) / 128, 2), block(128);
+#define CALL(T, L) launch_k(ctx, peer_push_kernel<T, L>, grid, block, ctx->g, (const PeerDev *)ctx->d_peer, parity, (const T *)spinor, \
+                            ctx->x3_lo, ctx->x3_hi, (T)ctx->peer_sign_up, (T)ctx->peer_sign_down, (const SolverState *)ctx->d_state, gate)
+    if (ctx->prec == LQCD_F64) { if (ctx->layout == 0) CALL(double, 0); else CALL(double, 1); }
+    else { if (ctx->layout == 0) CALL(float, 0); else CALL(float, 1); }
+#undef CALL
+    int rc = lqcd_check_cuda(ctx, cudaGetLastError(), "peer push");
+    return rc ? rc : peer_phase(ctx, 0);
+}
+
+// ---- generic all-reduce of up to LQCD_MAX_SHIFTS doubles, as two one-CTA kernels (publish, then gather) ----------
+__global__ void peer_publish_kernel(const PeerDev *pdp, const double *vals, int nv)
+{
+    pdl_wait();
+    pdl_trigger();
+    if (threadIdx.x == 0 && blockIdx.x == 0) peer_publish(*pdp, 2, vals, nv);
+}
+// out[v] = sum over ranks; which = 1: the sum is <b,b>: initialise the solver state like init_kernel's last CTA does
+__global__ void peer_gather_kernel(const PeerDev *pdp, double *out, int nv, SolverState *st, int which)
+{
+    pdl_wait();
+    pdl_trigger();
+    const unsigned int n = peer_wait_red(*pdp, 2);
+    if (threadIdx.x < nv) out[threadIdx.x] = peer_sum(*pdp, 2, n, threadIdx.x);
+    if (which == 1 && threadIdx.x == 0) {
+        const double t = peer_sum(*pdp, 2, n, 0);
+        st->cur[0].rho = t;
+        st->bnorm2 = t;
+        if (t == 0.0) st->done = 2;
+    }
+}
+
+// all-reduce nv device doubles at `vals` over the ranks, in place (nv <= LQCD_MAX_SHIFTS); which as above
+int launch_peer_allreduce(lqcd_ctx *ctx, double *vals, int nv, int which)
+{
+    launch_k(ctx, peer_publish_kernel, dim3(1), dim3(32), (const PeerDev *)ctx->d_peer, (const double *)vals, nv);
+    int rc = lqcd_check_cuda(ctx, cudaGetLastError(), "peer publish");
+    if (rc || (rc = peer_phase(ctx, 1))) return rc;
+    launch_k(ctx, peer_gather_kernel, dim3(1), dim3(32), (const PeerDev *)ctx->d_peer, vals, nv, ctx->d_state, which);
+    return lqcd_check_cuda(ctx, cudaGetLastError(), "peer gather");
+}

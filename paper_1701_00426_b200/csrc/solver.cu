@@ -14,6 +14,7 @@
 // over the 6*Vh reals of a half-lattice vector as a flat array with 16-byte loads.
 #include <stdlib.h>
 
+#include "peer.cuh"
 #include "reduce.cuh"
 
 void *ws_vec(lqcd_ctx *ctx, int k);   // api.cu
@@ -125,7 +126,7 @@ __global__ void __launch_bounds__(256) init_kernel(size_t npk, Seg sg, const T *
 template <typename T, int POLICY>
 __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restrict__ r, const T *__restrict__ q,
                                                  SolverState *st, const double *part_in, int n_in,
-                                                 double *part_out, int ip)
+                                                 double *part_out, int ip, const PeerDev *pdp)
 {
     pdl_wait();
     pdl_trigger();
@@ -135,9 +136,13 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restri
     const uint64_t keep = POLICY ? l2_policy_evict_last() : 0;
     const int comm = st->comm;
     double alpha_d;
-    if (comm) alpha_d = st->alpha;
+    if (comm == 1) alpha_d = st->alpha;
     else {
-        const double pq = sum_partials(part_in, n_in);
+        double pq;
+        if (comm == 2) {     // peer transport: the P local sums the Dslash kernels of all ranks published
+            const unsigned int n = peer_wait_red(*pdp, 0);
+            pq = peer_sum(*pdp, 0, n, 0);
+        } else pq = sum_partials(part_in, n_in);
         alpha_d = st->cur[ip].rho / pq;
         if (blockIdx.x == 0 && threadIdx.x == 0) solver_after_pq(st, pq, ip);
     }
@@ -156,7 +161,9 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restri
     }
     if (comm) {
         double total;
-        if (grid_sum_last(acc, part_out, &st->ticket, &total)) st->sum[1] = total;
+        if (grid_sum_last(acc, part_out, &st->ticket, &total)) {
+            if (comm == 2) peer_publish(*pdp, 1, &total, 1); else st->sum[1] = total;
+        }
     } else {
         const double b = block_sum(acc);
         if (threadIdx.x == 0) part_out[blockIdx.x] = b;
@@ -170,7 +177,8 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restri
 // traffic per active shift in exchange for one read-modify-write of y.
 template <typename T, int POLICY, int RAT>
 __global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__restrict__ r, T *__restrict__ p,
-                                                 ShiftPtrs sp, SolverState *st, const double *part_in, int n_in, int ip)
+                                                 ShiftPtrs sp, SolverState *st, const double *part_in, int n_in, int ip,
+                                                 const PeerDev *pdp)
 {
     pdl_wait();
     pdl_trigger();
@@ -180,9 +188,12 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__
     // Slab mode: the coefficients were written by scalar_kernel after the all-reduce.
     const int comm = st->comm;
     double rho_new = 0.0, beta_d;
-    if (comm) beta_d = st->beta;
+    if (comm == 1) beta_d = st->beta;
     else {
-        rho_new = sum_partials(part_in, n_in);
+        if (comm == 2) {     // peer transport: the P local <r,r> the K1 kernels of all ranks published
+            const unsigned int n = peer_wait_red(*pdp, 1);
+            rho_new = peer_sum(*pdp, 1, n, 0);
+        } else rho_new = sum_partials(part_in, n_in);
         beta_d = rho_new / st->cur[ip].rho;
     }
     typedef typename Pack<T>::type P;
@@ -203,7 +214,7 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__
         for (int i = 0; i < sp.nshift; ++i) {
             double c_zeta, c_beta;
             int c_active;
-            if (comm) { c_active = st->c_active[i]; c_zeta = st->c_zeta[i]; c_beta = st->c_beta[i]; }
+            if (comm == 1) { c_active = st->c_active[i]; c_zeta = st->c_zeta[i]; c_beta = st->c_beta[i]; }
             else {       // same expressions as solver_after_rr
                 const double zn = st->zeta_new[i], ratio = zn / st->cur[ip].zeta[i];
                 c_active = st->cur[ip].active[i];
@@ -223,7 +234,7 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__
         s_n = n;
         s_base_active = ba;
         // cur[ip] is not written by anyone in this kernel; the new state goes to cur[ip^1]
-        if (!comm && blockIdx.x == 0) solver_after_rr(st, rho_new, ip);
+        if (comm != 1 && blockIdx.x == 0) solver_after_rr(st, rho_new, ip);
     }
     __syncthreads();
     const int n_act = s_n, base_active = s_base_active;
@@ -350,17 +361,23 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         sg.off = (unsigned)((size_t)ctx->x3_lo * ctx->g.s3 * per / Pack<T>::N);
         npk = (size_t)nseg * sg.len;
     }
-    const int comm = ctx->allreduce_fn != NULL;
+    const int peer = ctx->peer_on;
+    const int comm = peer ? 2 : (ctx->allreduce_fn != NULL);      // SolverState::comm
     const int par = ctx->solve_parity;                                 // parity of x, b, p, r, q
     SolverState *const dst = ctx->d_state;
     // slab hooks: ghost slices of a vector before it is a Dslash input; global sum of a local dot product
-    auto halo = [&](void *v, int parity) -> int {
+    auto halo = [&](void *v, int parity, int gate) -> int {
+        if (peer) return launch_peer_push(ctx, v, parity, gate);
         if (!ctx->halo_fn) return LQCD_OK;
         if (ctx->halo_fn(ctx->comm_user, v, parity)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "halo hook failed");
         return LQCD_OK;
     };
     auto reduce_then = [&](int which, int ip) -> int {
         if (!comm) return LQCD_OK;
+        if (peer) {          // <p,q> and <r,r> are gathered by the consumer kernels; <b,b> by a pair of one-CTA kernels
+            if (which == 2) return launch_peer_allreduce(ctx, &dst->sum[2], 1, 1);
+            return peer_phase(ctx, 2);
+        }
         if (ctx->allreduce_fn(ctx->comm_user, &dst->sum[which], 1)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "allreduce hook failed");
         launch_k(ctx, scalar_kernel, dim3(1), dim3(32), dst, which, ip);
         return lqcd_check_cuda(ctx, cudaGetLastError(), "scalar kernel");
@@ -411,16 +428,16 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     auto enqueue_iteration = [&](int ip) -> int {      // ip = parity of the iteration number
         int e;
         const int m = ctx->iter_mask;   // diagnostic: which of the 4 kernels run (timing experiments only)
-        if ((e = halo(p, par))) return e;
+        if ((e = halo(p, par, 1))) return e;
         if ((m & 1) && (e = launch_dslash(ctx, 1 - par, tmp_o, p, links, NULL, 0.0, 0, 2))) return e;
-        if ((e = halo(tmp_o, 1 - par))) return e;
+        if ((e = halo(tmp_o, 1 - par, 1))) return e;
         if ((m & 2) && (e = launch_dslash(ctx, par, q, tmp_o, links, p, msq, 1, 1))) return e;
         const int n_pq = ctx->last_dslash_grid;
         if ((e = reduce_then(0, ip))) return e;
 #define K1(POL) launch_k(ctx, k1_kernel<T, POL>, dim3(g_k1), dim3(block), npk, sg, r, (const T *)q, dst, \
-                         (const double *)part_pq, n_pq, part_rr, ip)
+                         (const double *)part_pq, n_pq, part_rr, ip, (const PeerDev *)ctx->d_peer)
 #define K2(POL, RAT) launch_k(ctx, k2_kernel<T, POL, RAT>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, dst, \
-                              (const double *)part_rr, g_k1, ip)
+                              (const double *)part_rr, g_k1, ip, (const PeerDev *)ctx->d_peer)
         if (ctx->l2_hints && !comm) {
             if (m & 4) K1(1);
             if (m & 8) { if (sp.y) K2(1, 1); else K2(1, 0); }
@@ -445,6 +462,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     key[kn++] = ((unsigned long long)block << 32) | (unsigned)(ctx->dslash_block * 64 + ctx->dslash_minblocks * 8 + ctx->l2_hints * 4 + ctx->pdl * 2) ^ ((unsigned long long)ctx->dslash_persist << 48);
     key[kn++] = (unsigned long long)(uintptr_t)ctx->stream ^ ((unsigned long long)ctx->iter_mask << 56);
     key[kn++] = (unsigned long long)(uintptr_t)ctx->backfield;
+    key[kn++] = (unsigned long long)(uintptr_t)ctx->d_peer ^ (unsigned long long)peer;
     if (y) {
         key[kn++] = (unsigned long long)(uintptr_t)y;
         for (int i = 0; i < nshift; ++i) memcpy(&key[kn++], &coef[i], sizeof(double));
@@ -453,7 +471,10 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     }
     ctx->graph_active = 0;
     // (even chunk length: the iteration parity `ip` of every captured launch is then the same in every replay)
-    const bool use_graph = ctx->graph && max_iter >= ctx->poll_chunk && !comm && !ctx->halo_fn && ctx->poll_chunk % 2 == 0;
+    // (peer transport: the waits are inside the kernels, so the chunk graph stays on -- unless the lock-step
+    // validation hook wants the host between the kernels)
+    const bool use_graph = ctx->graph && max_iter >= ctx->poll_chunk && (comm == 0 || (peer && !ctx->phase_fn)) && !ctx->halo_fn &&
+                           ctx->poll_chunk % 2 == 0;
     if (use_graph) {
         if (!ctx->chunk_exec || ctx->chunk_key_n != kn || memcmp(ctx->chunk_key, key, kn * sizeof(key[0]))) {
             if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
@@ -480,7 +501,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         if (enq + n > max_iter) n = max_iter - enq;
         if (use_graph && ctx->graph && ctx->chunk_exec && n == ctx->poll_chunk) {
             if ((rc = lqcd_check_cuda(ctx, cudaGraphLaunch(ctx->chunk_exec, s), "chunk graph launch"))) return rc;
-            ctx->launches += (long)__builtin_popcount(ctx->iter_mask) * n;
+            ctx->launches += (long)(__builtin_popcount(ctx->iter_mask) + (peer ? 2 : 0)) * n;
             ctx->graph_active = 1;
         } else {
             for (int k = 0; k < n; ++k) if ((rc = enqueue_iteration((enq + k) & 1))) return rc;
@@ -500,13 +521,14 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     }
     // true residuals || b - (A + sigma_i) x_i || (reading R10), with the same kernels, ungated
     for (int i = 0; i < nshift && !y; ++i) {
-        if ((rc = halo(xs[i], par))) return rc;
+        if ((rc = halo(xs[i], par, 0))) return rc;
         if ((rc = launch_dslash(ctx, 1 - par, tmp_o, xs[i], links, NULL, 0.0, 0, 0))) return rc;
-        if ((rc = halo(tmp_o, 1 - par))) return rc;
+        if ((rc = halo(tmp_o, 1 - par, 0))) return rc;
         if ((rc = launch_dslash(ctx, par, q, tmp_o, links, xs[i], mass * mass + shifts[i], 0, 0))) return rc;
         launch_k(ctx, diffnorm_kernel<T, 0>, dim3(g_diff), dim3(block), npk, sg, (const T *)b, (const T *)q, ctx->d_state, ctx->d_partials, &ctx->d_state->resid[i]);
     }
-    if (comm && !y && ctx->allreduce_fn(ctx->comm_user, &dst->resid[0], nshift)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "allreduce hook failed");
+    if (peer && !y) { if ((rc = launch_peer_allreduce(ctx, &dst->resid[0], nshift, 0))) return rc; }
+    else if (comm && !y && ctx->allreduce_fn(ctx->comm_user, &dst->resid[0], nshift)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "allreduce hook failed");
     if ((rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(&h, ctx->d_state, sizeof(h), cudaMemcpyDeviceToHost, s), "solver state download"))) return rc;
     if ((rc = lqcd_check_cuda(ctx, cudaStreamSynchronize(s), "cg"))) return rc;
 

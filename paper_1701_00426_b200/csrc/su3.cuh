@@ -72,3 +72,19 @@ __device__ __forceinline__ void load_vec_unit(const T *__restrict__ v, size_t Vh
         p[c] = cx<T>(cr * z.re - ci * z.im, cr * z.im + ci * z.re);
     }
 }
+// a face vector from a landing buffer of the peer transport (peer.cuh): written by another GPU during this kernel's
+// lifetime (before its flag), so it is read through L2 (ld.global.cg), never through the non-coherent path
+template <typename T, int LAYOUT>
+__device__ __forceinline__ void load_vec_cg(const T *__restrict__ buf, size_t stride, size_t f, T coef, Cx<T> p[3])
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        if (LAYOUT == 0) {
+            typedef typename Vec2<T>::type V2;
+            const V2 v = __ldcg(reinterpret_cast<const V2 *>(buf) + (size_t)c * stride + f);
+            p[c] = cx<T>(coef * v.x, coef * v.y);
+        } else {
+            p[c] = cx<T>(coef * __ldcg(buf + (size_t)(2 * c) * stride + f), coef * __ldcg(buf + (size_t)(2 * c + 1) * stride + f));
+        }
+    }
+}

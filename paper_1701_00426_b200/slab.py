@@ -16,6 +16,15 @@ SURVEY.md section 8(e) gives the natural sharding of THIS path, built here (NEXT
     flight, the two boundary slices after it arrived;
   * per CG iteration two all-reduces of one double (<p,q>, <r,r>), through the hooks of lqcd_set_slab.
 
+Two transports:
+  * "peer" (the native one, lqcd_peer_* in lqcd.h): faces and partial sums move through peer-to-peer device
+    memory inside the library's own kernels -- no Python, no communication library and no host code between the
+    kernels of a solve; this module only creates the per-rank blocks and hands every rank the others' addresses
+    (CUDA IPC handles gathered with torch.distributed for one process per GPU; plain pointers for ranks that
+    share a process);
+  * "hooks" (lqcd_set_slab): the library calls back into this module for every halo exchange and all-reduce
+    (SlabComm: torch.distributed, NCCL on GPUs, gloo in the CPU tests) -- the portable fallback.
+
 Everything here is plumbing: index bookkeeping in numpy (SlabGeometry, covered by CPU tests), the
 exchange through torch.distributed (SlabComm: NCCL on GPUs, gloo in the CPU tests), and argument
 marshalling (SlabLattice).  Every arithmetic step runs in the CUDA kernels of liblqcd_b200.so.
@@ -149,22 +158,67 @@ class SlabLattice:
     `comm` (a SlabComm, or any object with exchange_start / exchange_wait / allreduce_sum).
     Parities in this API are GLOBAL (the paper's even sites); the local flip is handled here."""
 
-    def __init__(self, dims, world, rank, comm=None, prec=0, recon=0, antiperiodic_t=True, device=0, options=None):
+    def __init__(self, dims, world, rank, comm=None, prec=0, recon=0, antiperiodic_t=True, device=0, options=None,
+                 transport="hooks"):
         from .binding import Lattice, HALO_FN, ALLREDUCE_FN
+        if transport not in ("hooks", "peer"):
+            raise ValueError("transport must be 'hooks' or 'peer'")
+        self.transport = transport
         self.geo = SlabGeometry(dims, world, rank, antiperiodic_t)
         self.comm = comm if comm is not None else SlabComm(world, rank)
         self.lat = Lattice(self.geo.local_dims, prec=prec, recon=recon, antiperiodic_t=False, device=device,
                            options=options)
         self.torch = self.lat.torch
+        self.hook_error = None
+        if transport == "peer":
+            g = self.geo
+            self.peer_block = self.lat.peer_init(world, rank, g.x3_lo, g.x3_hi, g.local_parity(0),
+                                                 g.sign_send_up, g.sign_send_down)
+            if world == 1:
+                self.lat.peer_connect([self.peer_block])
+            return
         hb = self.lat.halo_bytes
         self._send_up, self._send_down, self._from_down, self._from_up = (self.lat._buf(hb) for _ in range(4))
         self._halo_cb = HALO_FN(self._halo_hook)
         self._allreduce_cb = ALLREDUCE_FN(self._allreduce_hook)
         self.lat.set_slab(self.geo.x3_lo, self.geo.x3_hi, self.geo.local_parity(0), self._halo_cb, self._allreduce_cb)
-        self.hook_error = None
 
     def close(self):
         self.lat.close()
+
+    # -- peer transport: hand every rank the other ranks' blocks ------------------------------------------
+    @staticmethod
+    def connect_local(slabs):
+        """Ranks that share a process (one context each, e.g. the single-GPU validation harness): plain pointers."""
+        blocks = [s.peer_block for s in sorted(slabs, key=lambda s: s.geo.rank)]
+        for s in slabs:
+            s.lat.peer_connect(blocks)
+
+    def connect_ipc(self):
+        """One process per GPU (torchrun): gather the CUDA IPC handles of all blocks with torch.distributed, map
+        the other ranks' blocks, connect.  Collective over the default process group."""
+        import torch.distributed as dist
+        g = self.geo
+        handles = [None] * g.world
+        dist.all_gather_object(handles, self.lat.peer_export())
+        blocks = [self.peer_block if r == g.rank else self.lat.peer_import(r, handles[r]) for r in range(g.world)]
+        self.lat.peer_connect(blocks)
+        dist.barrier()
+
+    def set_lockstep(self, barrier):
+        """Validation on ONE GPU: after every launch that publishes to the peers, finish this rank's stream and
+        meet the other ranks (host threads) at `barrier` -- no kernel ever waits for another rank's kernel."""
+        from .binding import PHASE_FN
+
+        def phase(user, what):
+            try:
+                self.lat.synchronize()
+                barrier.wait()
+                return 0
+            except Exception as e:        # an exception must not unwind through the C frames
+                self.hook_error = e
+                return 1
+        self.lat.set_phase_hook(PHASE_FN(phase) if barrier is not None else None)
 
     # -- fields ------------------------------------------------------------------------------
     def pack_links(self, U_global):
@@ -233,6 +287,10 @@ class SlabLattice:
         slices are computed while the two faces are in flight, the boundary slices afterwards."""
         g, lat = self.geo, self.lat
         lp = g.local_parity(out_global_parity)
+        if self.transport == "peer":          # the library pushes the faces and the kernel waits for them
+            lat.dslash(lp, out, inp, links)
+            self._raise_hook_error()
+            return
         handle = self._halo_start(inp.data_ptr())
         lo, hi = g.x3_lo, g.x3_hi
         if overlap and hi - lo > 2:
