@@ -233,6 +233,7 @@ struct PeerDev {                                  // lives in device memory (ctx
     void *land_self[2][2];                        // my landing buffers [kind][0: from down, 1: from up]
     void *land_up[2], *land_down[2];              // [kind]: up neighbour's "from down" buffer, down neighbour's "from up" buffer
     PeerBlock *up, *down;
+    double sign_up, sign_down;                    // boundary sign applied by the SENDER to the face sent up / down
 };
 
 // ------------------------------------------------------------------------------------------
@@ -356,12 +357,16 @@ int launch_pack_backfield(lqcd_ctx *ctx, void *native, const void *canonical);
 int launch_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical, const void *native);
 // out = D in; if xpay_in != NULL: out = coef*xpay_in - D in and partial Re<xpay_in,out> is reduced
 // into the solver state (dot_mode 1: CG "pq" epilogue; 0: none).  `gate`: obey state->done.
+// push_out (peer transport only): the kernel also stores the two boundary slices of `out` into the neighbours'
+// landing buffers (the face push fused into the producer)
 int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
-                  const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo = -1, int x3_hi = -1);
+                  const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo = -1, int x3_hi = -1, int push_out = 0);
+int peer_after_producer(lqcd_ctx *ctx, int kind, int gate);    // lock-step validation: signal kernel + host hook
 int launch_halo(lqcd_ctx *ctx, int pack, void *buf, void *spinor, int x3, double sign);
 // peer transport (peer.cu): push both faces of `spinor` (a vector of local parity `parity`) to the neighbours
 int launch_peer_push(lqcd_ctx *ctx, const void *spinor, int parity, int gate);
 int peer_phase(lqcd_ctx *ctx, int what);     // lock-step validation hook (no-op unless set)
 int launch_peer_allreduce(lqcd_ctx *ctx, double *vals, int nv, int which);
+int launch_peer_early_publish(lqcd_ctx *ctx, int kind, const double *partials, int n);   // lock-step validation only
 void lqcd_peer_destroy(lqcd_ctx *ctx);
 int launch_halo2(lqcd_ctx *ctx, int pack, void *buf0, void *buf1, void *spinor, int x3_0, int x3_1, double sign0, double sign1);

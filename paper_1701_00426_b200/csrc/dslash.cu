@@ -58,7 +58,8 @@ __global__ void __launch_bounds__(256, MINB)
 dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__restrict__ in,
               const T *__restrict__ links, const T *__restrict__ xin, const double coef,
               SolverState *__restrict__ st, double *__restrict__ partials, const int gate,
-              const int i_begin, const int i_end, const T *__restrict__ bf, const PeerDev *__restrict__ pdp)
+              const int i_begin, const int i_end, const T *__restrict__ bf, const PeerDev *__restrict__ pdp,
+              const int push_out)
 {
     pdl_wait();
     pdl_trigger();
@@ -69,7 +70,17 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
             return;
         }
     }
-    if (HALO) peer_wait_halo(*pdp, 1 - parity);
+    bool waited = false;
+    int rot = 0;
+    if (HALO) {
+        // the push of `in` is the previous kernel of the stream: its stores have landed, tell the neighbours
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            peer_signal_halo(*pdp, 1 - parity);
+            if (push_out) peer_bump_halo(*pdp, parity);      // this kernel pushes the faces of `out` itself (below)
+        }
+        // tiles start one slice in, so that the two boundary slices (the only tiles that wait) come last
+        if (g.s3 % (int)blockDim.x == 0 && (int)(gridDim.x * blockDim.x) >= i_end - i_begin) rot = g.s3 / (int)blockDim.x;
+    }
     double dot = 0.0;
     L2Pol pol = {0, 0};
     if (POLICY) pol = make_l2pol();
@@ -78,7 +89,14 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
     // CTAs that loop (option dslash_persist): the reduction protocol below is then paid once per
     // CTA instead of once per tile.
     // Sites [i_begin, i_end): the whole parity, or a range of x3 slices (lqcd_dslash_slices; slab mode).
-    for (int tile0 = i_begin + blockIdx.x * blockDim.x; tile0 < i_end; tile0 += gridDim.x * blockDim.x) {
+    int bx = blockIdx.x + rot;
+    if (bx >= (int)gridDim.x) bx -= gridDim.x;
+    for (int tile0 = i_begin + bx * blockDim.x; tile0 < i_end; tile0 += gridDim.x * blockDim.x) {
+    if (HALO && !waited && (tile0 < i_begin + g.s3 || tile0 + (int)blockDim.x > i_end - g.s3)) {
+        // only tiles that touch a boundary slice read the faces: the interior computes while they arrive
+        peer_wait_halo(*pdp, 1 - parity);
+        waited = true;
+    }
     const int i = tile0 + threadIdx.x;
     const bool valid = i < i_end;
     if (valid) {
@@ -151,12 +169,29 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
         }
 #pragma unroll
         for (int c = 0; c < 3; ++c) st_cx<T, LAYOUT, POLICY>(out, (size_t)c, Vh, (size_t)i, acc[c], pol);
+        if (HALO && push_out) {
+            // the face push fused into the producer: the owned boundary slices of `out` (times the boundary sign)
+            // go straight into the neighbours' landing buffers; the next Dslash raises the flags
+            if (i < i_begin + g.s3) {
+                const T sg = (T)pdp->sign_down;
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    st_cx<T, LAYOUT, 0>((T *)pdp->land_down[parity], (size_t)c, (size_t)g.s3, (size_t)(i - i_begin), cx<T>(sg * acc[c].re, sg * acc[c].im), pol);
+            }
+            if (i >= i_end - g.s3) {
+                const T sg = (T)pdp->sign_up;
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    st_cx<T, LAYOUT, 0>((T *)pdp->land_up[parity], (size_t)c, (size_t)g.s3, (size_t)(i - (i_end - g.s3)), cx<T>(sg * acc[c].re, sg * acc[c].im), pol);
+            }
+        }
     }
     }
     if (MODE == 2) {
-        if (HALO) {       // slab mode, peer transport: the last CTA publishes the LOCAL total to every rank
-            double total;
-            if (grid_sum_last(dot, partials, &st->ticket, &total)) peer_publish(*pdp, 0, &total, 1);
+        if (HALO) {       // slab mode, peer transport: per-CTA partials as on one GPU; K1's CTA 0 adds them up and publishes
+            const double b = block_sum(dot);
+            if (threadIdx.x == 0) partials[bx] = b;
+            if (blockIdx.x == 0 && threadIdx.x == 0) peer_bump_red(*pdp, 0);
         } else if (st->comm) {   // slab mode: the caller all-reduces the LOCAL total (lqcd_set_slab)
             double total;
             if (grid_sum_last(dot, partials, &st->ticket, &total)) st->sum[0] = total;
@@ -169,7 +204,7 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
 
 template <typename T, int LAYOUT, int RECON12, int MODE>
 static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
-                     const void *xin, double coef, int gate, int i_begin, int i_end, int halo_in)
+                     const void *xin, double coef, int gate, int i_begin, int i_end, int halo_in, int push_out)
 {
     int block = ctx->dslash_block > 256 ? 256 : ctx->dslash_block;
     int tiles = (i_end - i_begin + block - 1) / block;
@@ -182,7 +217,7 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
 #define GO1(MB, P, B) GO2(MB, P, B, 0)
 #define GO2(MB, P, B, H) launch_k(ctx, dslash_kernel<T, LAYOUT, RECON12, MODE, MB, P, B, H>, grid, dim3(block), \
         ctx->g, parity, (T *)out, (const T *)in, (const T *)links, (const T *)xin, coef, ctx->d_state, ctx->d_partials, gate, i_begin, i_end, \
-        (const T *)ctx->backfield, (const PeerDev *)ctx->d_peer)
+        (const T *)ctx->backfield, (const PeerDev *)ctx->d_peer, push_out)
 #define GO(MB) do { if (ctx->l2_hints) GO1(MB, 1, 0); else GO1(MB, 0, 0); } while (0)
     // peer transport: the per-precision default variant, faces read from the landing buffers (halo_in)
     if (halo_in) { if (sizeof(T) == 8) GO2(2, 0, 0, 1); else GO2(4, 0, 0, 1); } else
@@ -198,16 +233,16 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
 
 template <typename T, int LAYOUT>
 static void launch_tl(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
-                      const void *xin, double coef, int mode, int gate, int i_begin, int i_end, int halo_in)
+                      const void *xin, double coef, int mode, int gate, int i_begin, int i_end, int halo_in, int push_out)
 {
-#define GO(R, M) launch_t<T, LAYOUT, R, M>(ctx, parity, out, in, links, xin, coef, gate, i_begin, i_end, halo_in)
+#define GO(R, M) launch_t<T, LAYOUT, R, M>(ctx, parity, out, in, links, xin, coef, gate, i_begin, i_end, halo_in, push_out)
     if (ctx->recon == LQCD_RECON_12) { if (mode == 0) GO(1, 0); else if (mode == 1) GO(1, 1); else GO(1, 2); }
     else { if (mode == 0) GO(0, 0); else if (mode == 1) GO(0, 1); else GO(0, 2); }
 #undef GO
 }
 
 int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
-                  const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo, int x3_hi)
+                  const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo, int x3_hi, int push_out)
 {
     int mode = xpay_in ? (dot_mode ? 2 : 1) : 0;
     // peer transport: a Dslash over the context's owned slices reads the faces the neighbours pushed; an explicit
@@ -217,11 +252,11 @@ int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const vo
     if (x3_lo < 0) { x3_lo = ctx->x3_lo; x3_hi = ctx->x3_hi; }      // the context's interior slices
     const int i_begin = x3_lo * ctx->g.s3, i_end = x3_hi * ctx->g.s3;
     if (ctx->prec == LQCD_F64) {
-        if (ctx->layout == 0) launch_tl<double, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in);
-        else launch_tl<double, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in);
+        if (ctx->layout == 0) launch_tl<double, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in, halo_in ? push_out : 0);
+        else launch_tl<double, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in, halo_in ? push_out : 0);
     } else {
-        if (ctx->layout == 0) launch_tl<float, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in);
-        else launch_tl<float, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in);
+        if (ctx->layout == 0) launch_tl<float, 0>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in, halo_in ? push_out : 0);
+        else launch_tl<float, 1>(ctx, parity, out, in, links, xpay_in, coef, mode, gate, i_begin, i_end, halo_in, halo_in ? push_out : 0);
     }
     return lqcd_check_cuda(ctx, cudaGetLastError(), "dslash");
 }

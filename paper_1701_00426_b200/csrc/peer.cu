@@ -75,6 +75,7 @@ extern "C" int lqcd_peer_connect(lqcd_ctx *ctx, void *const *blocks)
     }
     const int up = (me + 1) % P, down = (me + P - 1) % P;
     h.up = h.peer[up]; h.down = h.peer[down];
+    h.sign_up = ctx->peer_sign_up; h.sign_down = ctx->peer_sign_down;
     for (int k = 0; k < 2; ++k) {
         for (int d = 0; d < 2; ++d) h.land_self[k][d] = land_ptr(ctx, ctx->peer_mem, k, d);
         h.land_up[k] = land_ptr(ctx, h.up, k, 0);       // my top slice is what the rank above receives "from down"
@@ -145,7 +146,7 @@ int peer_phase(lqcd_ctx *ctx, int what)
 // ---- face push ---------------------------------------------------------------------------------------------------
 // blockIdx.y = 0: my top owned slice (x3_hi - 1), times sign_up, -> the up neighbour's "from down" landing buffer;
 // blockIdx.y = 1: my bottom owned slice (x3_lo), times sign_down, -> the down neighbour's "from up" buffer.
-// The last CTA raises the neighbours' flags (every CTA has fenced its remote stores before taking a ticket).
+// One thread counts the exchange; the flags are raised by the Dslash that follows (kernel boundary).
 template <typename T, int LAYOUT>
 __global__ void __launch_bounds__(128) peer_push_kernel(const Geom g, const PeerDev *__restrict__ pdp, const int kind,
                                                         const T *__restrict__ spinor, const int x3_lo, const int x3_hi,
@@ -169,22 +170,43 @@ __global__ void __launch_bounds__(128) peer_push_kernel(const Geom g, const Peer
             st_cx<T, LAYOUT, 0>(buf, (size_t)c, (size_t)g.s3, (size_t)f, cx<T>(sign * z.re, sign * z.im), L2Pol());
         }
     }
-    __shared__ bool s_last;
-    __threadfence_system();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const unsigned int total = gridDim.x * gridDim.y;
-        const unsigned int t = atomicInc(&pd.self->ticket, total - 1);
-        s_last = (t == total - 1);
-    }
-    __syncthreads();
-    if (s_last && threadIdx.x == 0) {
-        __threadfence_system();
-        const unsigned int n = pd.self->cnt_halo[kind] + 1;
-        pd.self->cnt_halo[kind] = n;
-        st_flag(&pd.up->flag_halo[kind][0], n);        // the rank above sees its "from down" face
-        st_flag(&pd.down->flag_halo[kind][1], n);
-    }
+    // no fence, no ticket: the Dslash that follows in the stream raises the flags (peer.cuh)
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) peer_bump_halo(pd, kind);
+}
+
+// Lock-step validation only (lqcd_set_phase_hook): with every rank on ONE GPU no kernel may wait for another rank's
+// kernel, so what CTA 0 of the consumer does in production -- raise the halo flags, publish the rank's partial sum --
+// is done by these one-CTA kernels BEFORE the host barrier; the consumer then repeats the same stores (same
+// values, same counter) and finds every flag it waits for already raised.
+__global__ void peer_signal_kernel(const PeerDev *pdp, int kind, const SolverState *st, int gate)
+{
+    pdl_wait();
+    pdl_trigger();
+    if (gate && *(volatile const int *)&st->done) return;
+    if (threadIdx.x == 0) peer_signal_halo(*pdp, kind);
+}
+__global__ void peer_early_publish_kernel(const PeerDev *pdp, int kind, const double *partials, int n, const SolverState *st)
+{
+    pdl_wait();
+    pdl_trigger();
+    if (*(volatile const int *)&st->done) return;
+    const double local = sum_partials(partials, n);
+    if (threadIdx.x == 0) peer_publish(*pdp, kind, &local, 1);
+}
+int launch_peer_early_publish(lqcd_ctx *ctx, int kind, const double *partials, int n)
+{
+    if (!ctx->phase_fn) return LQCD_OK;
+    launch_k(ctx, peer_early_publish_kernel, dim3(1), dim3(256), (const PeerDev *)ctx->d_peer, kind, partials, n, (const SolverState *)ctx->d_state);
+    int rc = lqcd_check_cuda(ctx, cudaGetLastError(), "peer early publish");
+    return rc ? rc : peer_phase(ctx, 2);
+}
+
+int peer_after_producer(lqcd_ctx *ctx, int kind, int gate)
+{
+    if (!ctx->phase_fn) return LQCD_OK;
+    launch_k(ctx, peer_signal_kernel, dim3(1), dim3(32), (const PeerDev *)ctx->d_peer, kind, (const SolverState *)ctx->d_state, gate);
+    int rc = lqcd_check_cuda(ctx, cudaGetLastError(), "peer signal");
+    return rc ? rc : peer_phase(ctx, 0);
 }
 
 int launch_peer_push(lqcd_ctx *ctx, const void *spinor, int parity, int gate)
@@ -196,7 +218,7 @@ int launch_peer_push(lqcd_ctx *ctx, const void *spinor, int parity, int gate)
     else { if (ctx->layout == 0) CALL(float, 0); else CALL(float, 1); }
 #undef CALL
     int rc = lqcd_check_cuda(ctx, cudaGetLastError(), "peer push");
-    return rc ? rc : peer_phase(ctx, 0);
+    return rc ? rc : peer_after_producer(ctx, parity, gate);
 }
 
 // ---- generic all-reduce of up to LQCD_MAX_SHIFTS doubles, as two one-CTA kernels (publish, then gather) ----------
@@ -204,7 +226,7 @@ __global__ void peer_publish_kernel(const PeerDev *pdp, const double *vals, int 
 {
     pdl_wait();
     pdl_trigger();
-    if (threadIdx.x == 0 && blockIdx.x == 0) peer_publish(*pdp, 2, vals, nv);
+    if (threadIdx.x == 0 && blockIdx.x == 0) { peer_bump_red(*pdp, 2); __threadfence(); peer_publish(*pdp, 2, vals, nv); }
 }
 // out[v] = sum over ranks; which = 1: the sum is <b,b>: initialise the solver state like init_kernel's last CTA does
 __global__ void peer_gather_kernel(const PeerDev *pdp, double *out, int nv, SolverState *st, int which)

@@ -4,16 +4,22 @@
 //
 // Every rank owns one PeerBlock in its own device memory, mapped by all ranks of the node (cudaMalloc +
 // CUDA IPC, or plain pointers when the ranks share a process).  Nothing here launches a kernel of its own in
-// the CG loop except the face push: the PRODUCER of a partial sum publishes it to every rank's block from its
-// last CTA, the CONSUMER kernel waits for the P flags at its start and adds the P slots in rank order (every
-// rank gets the bit-identical total, so every rank takes the same decisions).  Halo: the push kernel stores the
-// two boundary slices of a vector straight into the neighbours' landing buffers and raises their flag; the
-// Dslash that reads the vector waits for its two flags and takes the x3 hops that leave the slab from the
-// landing buffers (no unpack kernel, no ghost slices in the vectors are read).
+// the CG loop except the face push, and no kernel of the loop uses a fence-and-ticket protocol: what orders a
+// rank's own writes is the KERNEL BOUNDARY (every kernel starts with griddepcontrol.wait), what orders them for
+// the peers is one release store per flag.
+//   dot products: the producer (Dslash with <p,q>, K1 with <r,r>) leaves per-CTA partials as on a single GPU;
+//     CTA 0 of the CONSUMER (K1, K2) adds them up and stores the rank's sum into every rank's slot, then raises
+//     the flags; every CTA of the consumer waits for the P flags and adds the P slots in rank order (every rank
+//     gets the bit-identical total, so every rank takes the same decisions);
+//   halo: the push kernel stores the two boundary slices of a vector straight into the neighbours' landing
+//     buffers; CTA 0 of the Dslash that follows it in the stream raises the neighbours' flags; only the tiles
+//     of that Dslash that touch a boundary slice wait for the rank's own two flags, and they take the x3 hops
+//     that leave the slab from the landing buffers (no unpack kernel; the vectors' ghost slices are not read).
 //
-// Flags carry monotone counters, never reset.  A rank's own counter of a sync point is, by construction, the
-// value it must see from its peers: all ranks run the same sequence of sync points.  Re-use of a slot or a
-// landing buffer is ordered by the all-reduces in between (solver.cu, "peer mode").
+// Flags carry monotone counters, never reset.  The counter of a sync point is bumped by one thread of the
+// PRODUCING kernel (visible to the consumer through the kernel boundary); a rank's own counter is, by
+// construction, the value it must see from its peers: all ranks run the same sequence of sync points.  Re-use of
+// a slot or a landing buffer is ordered by the all-reduces in between (solver.cu, "peer mode").
 #pragma once
 #include "common.cuh"
 
@@ -38,15 +44,18 @@ __device__ __forceinline__ double ld_slot(const double *p)
     return v;
 }
 
-// Called by ONE thread after the grid-wide local sum is complete (the last CTA of grid_sum_last, or a
-// one-thread kernel): vals[0..nv) go to slot[kind][n & 1][rank][*] of every rank, then the flags.
+// One thread of the producing kernel: this rank has one more reduction / exchange of `kind` under way.
+__device__ __forceinline__ void peer_bump_red(const PeerDev &pd, int kind) { pd.self->cnt_red[kind] += 1; }
+__device__ __forceinline__ void peer_bump_halo(const PeerDev &pd, int kind) { pd.self->cnt_halo[kind] += 1; }
+
+// Called by ONE thread once the rank's local sum is complete: vals[0..nv) go to slot[kind][n & 1][rank][*] of
+// every rank, then the flags (n = the rank's own counter of `kind`, bumped by the producing kernel).
 __device__ __forceinline__ void peer_publish(const PeerDev &pd, int kind, const double *vals, int nv)
 {
-    const unsigned int n = pd.self->cnt_red[kind] + 1;
-    pd.self->cnt_red[kind] = n;
+    const unsigned int n = *(volatile unsigned int *)&pd.self->cnt_red[kind];
     for (int r = 0; r < pd.nranks; ++r)
         for (int v = 0; v < nv; ++v) st_remote(&pd.peer[r]->slot[kind][n & 1][pd.rank][v], vals[v]);
-    __threadfence_system();
+    // (the release stores order the slots before the flags)
     for (int r = 0; r < pd.nranks; ++r) st_flag(&pd.peer[r]->flag_red[kind][pd.rank], n);
 }
 
@@ -70,7 +79,15 @@ __device__ __forceinline__ double peer_sum(const PeerDev &pd, int kind, unsigned
     return s;
 }
 
-// Start of a Dslash that reads a vector whose faces were pushed as exchange `kind`: wait for both neighbours.
+// One thread of the Dslash that follows the push in the stream: the faces are in the neighbours' landing buffers
+// (kernel boundary), tell them.
+__device__ __forceinline__ void peer_signal_halo(const PeerDev &pd, int kind)
+{
+    const unsigned int n = *(volatile unsigned int *)&pd.self->cnt_halo[kind];
+    st_flag(&pd.up->flag_halo[kind][0], n);        // the rank above sees its "from down" face
+    st_flag(&pd.down->flag_halo[kind][1], n);
+}
+// A tile of that Dslash that reads a face: wait for both neighbours.
 __device__ __forceinline__ void peer_wait_halo(const PeerDev &pd, int kind)
 {
     const unsigned int n = *(volatile unsigned int *)&pd.self->cnt_halo[kind];

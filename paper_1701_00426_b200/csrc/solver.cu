@@ -59,12 +59,35 @@ template <int POLICY> __device__ __forceinline__ void stv(float4 *p, float4 v, u
 // Slab mode: the vector kernels touch only the owned x3 slices, i.e. `nseg` runs of `len` packets that
 // start `off` packets into planes `stride` packets apart (layout 0: 3 complex planes; layout 1: 6 real
 // planes).  len == 0: the whole vector, flat (single GPU).
-struct Seg { unsigned int len, stride, off; };
+struct Seg { unsigned int len, stride, off, slice; };   // slice: packets of one x3 slice of one plane
 __device__ __forceinline__ size_t seg_idx(size_t k, const Seg &sg)
 {
     if (sg.len == 0) return k;
     const unsigned int pl = (unsigned int)k / sg.len;
     return (size_t)pl * sg.stride + sg.off + ((unsigned int)k - pl * sg.len);
+}
+
+// Peer transport: the face push fused into the kernel that PRODUCES a vector (p in init / K2): packet k0 of the owned
+// range, if it lies in the first / last owned slice, also goes (times the boundary sign) into the landing buffer of
+// the rank below / above, which is laid out like a half vector of one slice.
+template <typename T>
+__device__ __forceinline__ void peer_store_faces(const PeerDev &pd, int kind, const Seg &sg, size_t k0, const T *v)
+{
+    typedef typename Pack<T>::type P;
+    const int N = Pack<T>::N;
+    const unsigned int pl = (unsigned int)k0 / sg.len, off = (unsigned int)k0 - pl * sg.len;
+    if (off < sg.slice) {
+        T w[4];
+        const T s = (T)pd.sign_down;
+        for (int j = 0; j < N; ++j) w[j] = s * v[j];
+        reinterpret_cast<P *>(pd.land_down[kind])[(size_t)pl * sg.slice + off] = repack(w);
+    }
+    if (off >= sg.len - sg.slice) {
+        T w[4];
+        const T s = (T)pd.sign_up;
+        for (int j = 0; j < N; ++j) w[j] = s * v[j];
+        reinterpret_cast<P *>(pd.land_up[kind])[(size_t)pl * sg.slice + (off - (sg.len - sg.slice))] = repack(w);
+    }
 }
 
 struct ShiftPtrs {
@@ -81,7 +104,7 @@ struct ShiftPtrs {
 template <typename T, int POLICY>
 __global__ void __launch_bounds__(256) init_kernel(size_t npk, Seg sg, const T *__restrict__ b, T *__restrict__ r,
                                                    T *__restrict__ p, ShiftPtrs sp, SolverState *st,
-                                                   double *partials)
+                                                   double *partials, const PeerDev *pdp, int push_kind)
 {
     pdl_wait();
     pdl_trigger();
@@ -99,6 +122,7 @@ __global__ void __launch_bounds__(256) init_kernel(size_t npk, Seg sg, const T *
         for (int j = 0; j < N; ++j) acc += (double)a[j] * (double)a[j];
         stv<POLICY>(reinterpret_cast<P *>(r) + k, v, keep);
         stv<POLICY>(reinterpret_cast<P *>(p) + k, v, keep);
+        if (push_kind >= 0) peer_store_faces<T>(*pdp, push_kind, sg, k0, a);      // the faces of p = b
         if (sp.y) {
             T yy[4];
             for (int j = 0; j < N; ++j) yy[j] = (T)sp.c0 * a[j];
@@ -109,6 +133,7 @@ __global__ void __launch_bounds__(256) init_kernel(size_t npk, Seg sg, const T *
             if (i != sp.base) stv<POLICY>(reinterpret_cast<P *>(sp.p[i]) + k, v, strm);
         }
     }
+    if (push_kind >= 0 && blockIdx.x == 0 && threadIdx.x == 0) peer_bump_halo(*pdp, push_kind);
     double total;
     if (grid_sum_last(acc, partials, &st->ticket, &total)) {
         if (st->comm) st->sum[2] = total;
@@ -139,7 +164,11 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restri
     if (comm == 1) alpha_d = st->alpha;
     else {
         double pq;
-        if (comm == 2) {     // peer transport: the P local sums the Dslash kernels of all ranks published
+        if (comm == 2) {     // peer transport: CTA 0 publishes this rank's sum of the Dslash partials, every CTA gathers
+            if (blockIdx.x == 0) {
+                const double local = sum_partials(part_in, n_in);
+                if (threadIdx.x == 0) peer_publish(*pdp, 0, &local, 1);
+            }
             const unsigned int n = peer_wait_red(*pdp, 0);
             pq = peer_sum(*pdp, 0, n, 0);
         } else pq = sum_partials(part_in, n_in);
@@ -159,14 +188,13 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restri
         }
         stv<POLICY>(reinterpret_cast<P *>(r) + k, repack(a), keep);
     }
-    if (comm) {
+    if (comm == 1) {
         double total;
-        if (grid_sum_last(acc, part_out, &st->ticket, &total)) {
-            if (comm == 2) peer_publish(*pdp, 1, &total, 1); else st->sum[1] = total;
-        }
+        if (grid_sum_last(acc, part_out, &st->ticket, &total)) st->sum[1] = total;
     } else {
         const double b = block_sum(acc);
         if (threadIdx.x == 0) part_out[blockIdx.x] = b;
+        if (comm == 2 && blockIdx.x == 0 && threadIdx.x == 0) peer_bump_red(*pdp, 1);
     }
 }
 
@@ -178,7 +206,7 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restri
 template <typename T, int POLICY, int RAT>
 __global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__restrict__ r, T *__restrict__ p,
                                                  ShiftPtrs sp, SolverState *st, const double *part_in, int n_in, int ip,
-                                                 const PeerDev *pdp)
+                                                 const PeerDev *pdp, int push_kind)
 {
     pdl_wait();
     pdl_trigger();
@@ -190,7 +218,11 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__
     double rho_new = 0.0, beta_d;
     if (comm == 1) beta_d = st->beta;
     else {
-        if (comm == 2) {     // peer transport: the P local <r,r> the K1 kernels of all ranks published
+        if (comm == 2) {     // peer transport: CTA 0 publishes this rank's sum of K1's partials, every CTA gathers
+            if (blockIdx.x == 0) {
+                const double local = sum_partials(part_in, n_in);
+                if (threadIdx.x == 0) peer_publish(*pdp, 1, &local, 1);
+            }
             const unsigned int n = peer_wait_red(*pdp, 1);
             rho_new = peer_sum(*pdp, 1, n, 0);
         } else rho_new = sum_partials(part_in, n_in);
@@ -278,7 +310,9 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__
         if (touch) stv<POLICY>(xb + k, repack(acc), strm);
         for (int j = 0; j < N; ++j) pp[j] = fma(beta, pp[j], rr[j]);
         stv<POLICY>(reinterpret_cast<P *>(p) + k, repack(pp), keep);
+        if (push_kind >= 0) peer_store_faces<T>(*pdp, push_kind, sg, k0, pp);     // the faces of the new p
     }
+    if (push_kind >= 0 && blockIdx.x == 0 && threadIdx.x == 0) peer_bump_halo(*pdp, push_kind);
 }
 
 // Slab mode: the scalar step that the last CTA of a reduction performs on a single GPU, run after the
@@ -352,19 +386,26 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
 {
     // vector kernels: the whole half vector, or (slab mode) only the owned x3 slices of each plane
     size_t npk = (size_t)ctx->g.Vh * 6 / Pack<T>::N;
-    Seg sg = {0, 0, 0};
+    Seg sg = {0, 0, 0, 0};
     if (ctx->x3_lo != 0 || ctx->x3_hi != ctx->g.N3) {
         const unsigned per = ctx->layout == 0 ? 2 : 1;                 // reals per site in one plane
         const unsigned nseg = ctx->layout == 0 ? 3 : 6;
         sg.len = (unsigned)((size_t)(ctx->x3_hi - ctx->x3_lo) * ctx->g.s3 * per / Pack<T>::N);
         sg.stride = (unsigned)((size_t)ctx->g.Vh * per / Pack<T>::N);
         sg.off = (unsigned)((size_t)ctx->x3_lo * ctx->g.s3 * per / Pack<T>::N);
+        sg.slice = (unsigned)((size_t)ctx->g.s3 * per / Pack<T>::N);
         npk = (size_t)nseg * sg.len;
     }
     const int peer = ctx->peer_on;
     const int comm = peer ? 2 : (ctx->allreduce_fn != NULL);      // SolverState::comm
     const int par = ctx->solve_parity;                                 // parity of x, b, p, r, q
     SolverState *const dst = ctx->d_state;
+    const int block = ctx->blas_block;
+    const int g_init = ctx->l2_hints ? blas_grid(ctx, init_kernel<T, 1>, npk) : blas_grid(ctx, init_kernel<T, 0>, npk);
+    const int g_k1 = ctx->l2_hints ? blas_grid(ctx, k1_kernel<T, 1>, npk) : blas_grid(ctx, k1_kernel<T, 0>, npk);
+    const int g_k2 = y ? (ctx->l2_hints ? blas_grid(ctx, k2_kernel<T, 1, 1>, npk) : blas_grid(ctx, k2_kernel<T, 0, 1>, npk))
+                       : (ctx->l2_hints ? blas_grid(ctx, k2_kernel<T, 1, 0>, npk) : blas_grid(ctx, k2_kernel<T, 0, 0>, npk));
+    const int g_diff = blas_grid(ctx, diffnorm_kernel<T, 0>, npk);
     // slab hooks: ghost slices of a vector before it is a Dslash input; global sum of a local dot product
     auto halo = [&](void *v, int parity, int gate) -> int {
         if (peer) return launch_peer_push(ctx, v, parity, gate);
@@ -376,18 +417,15 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         if (!comm) return LQCD_OK;
         if (peer) {          // <p,q> and <r,r> are gathered by the consumer kernels; <b,b> by a pair of one-CTA kernels
             if (which == 2) return launch_peer_allreduce(ctx, &dst->sum[2], 1, 1);
-            return peer_phase(ctx, 2);
+            // lock-step validation: the rank's sum is published before the host barrier (peer.cu); in production
+            // CTA 0 of the consumer kernel does it
+            return which == 0 ? launch_peer_early_publish(ctx, 0, ctx->d_partials, ctx->last_dslash_grid)
+                              : launch_peer_early_publish(ctx, 1, ctx->d_partials + ctx->max_partials, g_k1);
         }
         if (ctx->allreduce_fn(ctx->comm_user, &dst->sum[which], 1)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "allreduce hook failed");
         launch_k(ctx, scalar_kernel, dim3(1), dim3(32), dst, which, ip);
         return lqcd_check_cuda(ctx, cudaGetLastError(), "scalar kernel");
     };
-    const int block = ctx->blas_block;
-    const int g_init = ctx->l2_hints ? blas_grid(ctx, init_kernel<T, 1>, npk) : blas_grid(ctx, init_kernel<T, 0>, npk);
-    const int g_k1 = ctx->l2_hints ? blas_grid(ctx, k1_kernel<T, 1>, npk) : blas_grid(ctx, k1_kernel<T, 0>, npk);
-    const int g_k2 = y ? (ctx->l2_hints ? blas_grid(ctx, k2_kernel<T, 1, 1>, npk) : blas_grid(ctx, k2_kernel<T, 0, 1>, npk))
-                       : (ctx->l2_hints ? blas_grid(ctx, k2_kernel<T, 1, 0>, npk) : blas_grid(ctx, k2_kernel<T, 0, 0>, npk));
-    const int g_diff = blas_grid(ctx, diffnorm_kernel<T, 0>, npk);
     cudaStream_t s = ctx->stream;
     T *tmp_o = (T *)ws_vec(ctx, 0), *q = (T *)ws_vec(ctx, 1), *r = (T *)ws_vec(ctx, 2), *p = (T *)ws_vec(ctx, 3);
 
@@ -413,8 +451,10 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     sp.c0 = c0;
     int rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(ctx->d_state, &h, sizeof(h), cudaMemcpyHostToDevice, s), "solver state upload");
     if (rc) return rc;
-    if (ctx->l2_hints) launch_k(ctx, init_kernel<T, 1>, dim3(g_init), dim3(block), npk, sg, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
-    else launch_k(ctx, init_kernel<T, 0>, dim3(g_init), dim3(block), npk, sg, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials);
+    const int push_kind = peer ? par : -1;     // peer transport: init and K2 push the faces of p themselves
+    if (ctx->l2_hints) launch_k(ctx, init_kernel<T, 1>, dim3(g_init), dim3(block), npk, sg, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials, (const PeerDev *)ctx->d_peer, push_kind);
+    else launch_k(ctx, init_kernel<T, 0>, dim3(g_init), dim3(block), npk, sg, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials, (const PeerDev *)ctx->d_peer, push_kind);
+    if (peer && (rc = peer_after_producer(ctx, par, 0))) return rc;
     if ((rc = reduce_then(2, 0))) return rc;
 
     const double msq = mass * mass + shifts[base];
@@ -428,16 +468,18 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     auto enqueue_iteration = [&](int ip) -> int {      // ip = parity of the iteration number
         int e;
         const int m = ctx->iter_mask;   // diagnostic: which of the 4 kernels run (timing experiments only)
-        if ((e = halo(p, par, 1))) return e;
-        if ((m & 1) && (e = launch_dslash(ctx, 1 - par, tmp_o, p, links, NULL, 0.0, 0, 2))) return e;
-        if ((e = halo(tmp_o, 1 - par, 1))) return e;
+        // peer transport: the faces of p were pushed by its producer (init / K2), K_A pushes those of tmp_o
+        if (!peer && (e = halo(p, par, 1))) return e;
+        if ((m & 1) && (e = launch_dslash(ctx, 1 - par, tmp_o, p, links, NULL, 0.0, 0, 2, -1, -1, peer))) return e;
+        if (peer) { if ((e = peer_after_producer(ctx, 1 - par, 1))) return e; }
+        else if ((e = halo(tmp_o, 1 - par, 1))) return e;
         if ((m & 2) && (e = launch_dslash(ctx, par, q, tmp_o, links, p, msq, 1, 1))) return e;
         const int n_pq = ctx->last_dslash_grid;
         if ((e = reduce_then(0, ip))) return e;
 #define K1(POL) launch_k(ctx, k1_kernel<T, POL>, dim3(g_k1), dim3(block), npk, sg, r, (const T *)q, dst, \
                          (const double *)part_pq, n_pq, part_rr, ip, (const PeerDev *)ctx->d_peer)
 #define K2(POL, RAT) launch_k(ctx, k2_kernel<T, POL, RAT>, dim3(g_k2), dim3(block), npk, sg, (const T *)r, p, sp, dst, \
-                              (const double *)part_rr, g_k1, ip, (const PeerDev *)ctx->d_peer)
+                              (const double *)part_rr, g_k1, ip, (const PeerDev *)ctx->d_peer, push_kind)
         if (ctx->l2_hints && !comm) {
             if (m & 4) K1(1);
             if (m & 8) { if (sp.y) K2(1, 1); else K2(1, 0); }
@@ -448,6 +490,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         }
 #undef K1
 #undef K2
+        if (peer && (e = peer_after_producer(ctx, par, 1))) return e;
         return lqcd_check_cuda(ctx, cudaGetLastError(), "cg iteration");
     };
     // Chunk graph (option `graph`): poll_chunk iterations captured once and replayed; the key is
@@ -501,7 +544,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         if (enq + n > max_iter) n = max_iter - enq;
         if (use_graph && ctx->graph && ctx->chunk_exec && n == ctx->poll_chunk) {
             if ((rc = lqcd_check_cuda(ctx, cudaGraphLaunch(ctx->chunk_exec, s), "chunk graph launch"))) return rc;
-            ctx->launches += (long)(__builtin_popcount(ctx->iter_mask) + (peer ? 2 : 0)) * n;
+            ctx->launches += (long)__builtin_popcount(ctx->iter_mask) * n;
             ctx->graph_active = 1;
         } else {
             for (int k = 0; k < n; ++k) if ((rc = enqueue_iteration((enq + k) & 1))) return rc;

@@ -128,57 +128,85 @@ def multishift(dims_list, out):
         lat.close()
 
 
-def slab(dims_list, out):
-    """Strong-scaling Dslash / multi-shift CG of ONE lattice split into x3 slabs, one per rank
-    (torchrun + NCCL for WORLD_SIZE > 1; alone it measures the slab path's own overhead: self-exchange
-    of the two faces and three launches per Dslash instead of one)."""
+def slab(dims_list, out, transports=("peer", "hooks")):
+    """Strong-scaling Dslash / multi-shift CG of ONE lattice split into x3 slabs, one per rank (torchrun for
+    WORLD_SIZE > 1; alone it measures the slab path's own overhead against the plain single-context run).
+    Transports: "peer" = the library's own peer-to-peer transport (CUDA IPC between the processes), "hooks" =
+    torch.distributed (NCCL) called back from inside the solver."""
     import numpy as np
     import torch
     import lqcd_inputs as gen
+    import paper_1701_00426_b200 as L
     from paper_1701_00426_b200 import dist as D
     from paper_1701_00426_b200.slab import SlabLattice
 
     rank, local_rank, world = D.init("nccl")
     torch.cuda.set_device(local_rank)
     device = torch.device("cuda", local_rank)
-    for dims in dims_list:
-        rng = np.random.default_rng(3)
-        U = gen.smooth_links(dims, 0.3, rng)
-        ie, io = gen.gaussian_half_spinor(dims, rng), gen.gaussian_half_spinor(dims, rng)
-        V = gen.volume(dims)
-        sl = SlabLattice(dims, world, rank, device=local_rank)
-        links = sl.pack_links(U)
-        a, b = sl.pack_spinor(ie, 0), sl.pack_spinor(io, 1)
-        oo, oe = sl.new_spinor(), sl.new_spinor()
-        for overlap in (True, False):
-            def step():
-                sl.dslash(1, oo, a, links, overlap=overlap)
-                sl.dslash(0, oe, b, links, overlap=overlap)
-            D.barrier(world)
-            us = D.max_over_ranks(ev_time_us(torch, step, 200, 10) / 2, world, device)
-            if rank == 0:
-                out(dict(kind="slab_dslash", dims="x".join(map(str, dims)), world=world, overlap=overlap,
-                         us=round(us, 2), ns_per_site=round(us * 1e3 / (V // 2), 4),
-                         GBs_aggregate=round(1248 * (V // 2) / us / 1e3, 1)))
-        shifts = gen.rhmc_shifts(8)
-        xs = [sl.new_spinor() for _ in shifts]
+    shifts = gen.rhmc_shifts(8)
 
+    def iter_us(solver, xs, a, links):
         def solve(n):
             torch.cuda.synchronize()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            sl.cg_multishift(xs, a, links, 0.0025, shifts, 1e-300, n, raise_on_max_iter=False)
+            solver(xs, a, links, 0.0025, shifts, 1e-300, n, raise_on_max_iter=False)
             e1.record()
             torch.cuda.synchronize()
             return e0.elapsed_time(e1)
         solve(16)
         t_lo, t_hi = min(solve(16), solve(16)), min(solve(80), solve(80))
-        it_us = D.max_over_ranks((t_hi - t_lo) / 64 * 1e3, world, device)
-        if rank == 0:
-            out(dict(kind="slab_multishift8", dims="x".join(map(str, dims)), world=world,
-                     us_per_iter=round(it_us, 2), iter_per_s=round(1e6 / it_us, 1),
-                     note="host-driven hooks: 2 halo exchanges + 2 all-reduces per iteration"))
-        sl.close()
+        return D.max_over_ranks((t_hi - t_lo) / 64 * 1e3, world, device)
+
+    for dims in dims_list:
+        rng = np.random.default_rng(3)
+        U = gen.smooth_links(dims, 0.3, rng)
+        ie, io = gen.gaussian_half_spinor(dims, rng), gen.gaussian_half_spinor(dims, rng)
+        V = gen.volume(dims)
+        name = "x".join(map(str, dims))
+        if world == 1:       # the plain single-context path on the same inputs: what the slab path's overhead is measured against
+            lat = L.Lattice(dims, device=local_rank)
+            links = lat.pack_links(U)
+            a, b = lat.pack_spinor(ie, 0), lat.pack_spinor(io, 1)
+            oo, oe = lat.new_spinor(), lat.new_spinor()
+
+            def step0():
+                lat.dslash(1, oo, a, links)
+                lat.dslash(0, oe, b, links)
+            us = ev_time_us(torch, step0, 200, 10) / 2
+            out(dict(kind="slab_dslash", dims=name, world=1, transport="none (plain context)", overlap=False, us=round(us, 2),
+                     ns_per_site=round(us * 1e3 / (V // 2), 4), GBs_aggregate=round(1248 * (V // 2) / us / 1e3, 1)))
+            xs = [lat.new_spinor() for _ in shifts]
+            it = iter_us(lat.cg_multishift, xs, a, links)
+            out(dict(kind="slab_multishift8", dims=name, world=1, transport="none (plain context)", us_per_iter=round(it, 2),
+                     iter_per_s=round(1e6 / it, 1), graph=lat.get_option("graph_active")))
+            lat.close()
+            del links, a, b, oo, oe, xs
+        for transport in transports:
+            sl = SlabLattice(dims, world, rank, device=local_rank, transport=transport)
+            if transport == "peer" and world > 1:
+                sl.connect_ipc()
+            links = sl.pack_links(U)
+            a, b = sl.pack_spinor(ie, 0), sl.pack_spinor(io, 1)
+            oo, oe = sl.new_spinor(), sl.new_spinor()
+            for overlap in ((False,) if transport == "peer" else (True, False)):
+                def step():
+                    sl.dslash(1, oo, a, links, overlap=overlap)
+                    sl.dslash(0, oe, b, links, overlap=overlap)
+                D.barrier(world)
+                us = D.max_over_ranks(ev_time_us(torch, step, 200, 10) / 2, world, device)
+                if rank == 0:
+                    out(dict(kind="slab_dslash", dims=name, world=world, transport=transport, overlap=overlap,
+                             us=round(us, 2), ns_per_site=round(us * 1e3 / (V // 2), 4),
+                             GBs_aggregate=round(1248 * (V // 2) / us / 1e3, 1)))
+            xs = [sl.new_spinor() for _ in shifts]
+            D.barrier(world)
+            it = iter_us(sl.cg_multishift, xs, a, links)
+            if rank == 0:
+                out(dict(kind="slab_multishift8", dims=name, world=world, transport=transport, us_per_iter=round(it, 2),
+                         iter_per_s=round(1e6 / it, 1), graph=sl.lat.get_option("graph_active")))
+            sl.close()
+            del links, a, b, oo, oe, xs
     D.barrier(world)
     D.finalize(world)
 
