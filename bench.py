@@ -394,9 +394,19 @@ def run_ours(args):
     cold_ms = timed_loop(torch, e2e_cold_step, cold_steps, 1, world, D, device)
     del keep_U, hU
 
+    # ---- strong scaling of ONE 32^4 lattice over the N ranks: x3 slabs over the library's
+    #      peer-to-peer transport; collective, every rank takes part.  At N = 1 it measures the slab path's own
+    #      overhead against the plain context.  `value` above stays the replica (weak-scaling) figure.
+    slab_strong = None
+    if DIMS[3] % world == 0 and (DIMS[3] // world) % 2 == 0 and world <= 16:
+        slab_strong = slab_strong_leg(torch, L, D, gen, U if world == 1 else None, rank, local_rank, world, device,
+                                      us_launch if world == 1 else None)
+
     line = None
     if rank == 0:
         extra = {}
+        if slab_strong is not None:
+            extra["slab_strong"] = slab_strong
         # ---- other Dslash variants (config 3's 12-real arm, config 5's fp32) -------------------
         for prec, pname in ((L.F64, "f64"), (L.F32, "f32")):
             for recon, rn in ((L.RECON_18, 18), (L.RECON_12, 12)):
@@ -572,6 +582,51 @@ STAPLES_EXEC_FLOP_PER_LINK = {0: 84 * 198 + 24 * 36, 1: 3 * (22 * 198 + 10 * 36)
 # two-pass staples: HBM bytes per site that the algorithm must move (fp64): pass 1 reads the links (576) and writes 24
 # fields (3456); pass 2 reads them and the links and writes the staples (576)
 STAPLES2_BYTES_PER_SITE = 576 + 3456 + 3456 + 576 + 576
+
+
+def slab_strong_leg(torch, L, D, gen, U, rank, local_rank, world, device, plain_us):
+    """One 32^4 lattice (the same on every rank: seed SEED) split into `world` x3 slabs, one per GPU, over the
+    peer transport (CUDA IPC between the processes): Dslash time per application and 8-shift CG time per iteration,
+    max over ranks.  No number here was ever taken on more than one GPU in this project's environment."""
+    import numpy as np
+    from paper_1701_00426_b200.slab import SlabLattice
+    if U is None:
+        U = gen.smooth_links(DIMS, EPS, np.random.default_rng(SEED))
+    r2 = np.random.default_rng(SEED + 7)
+    ie, io = gen.gaussian_half_spinor(DIMS, r2), gen.gaussian_half_spinor(DIMS, r2)
+    V = gen.volume(DIMS)
+    sl = SlabLattice(DIMS, world, rank, device=local_rank, transport="peer")
+    if world > 1:
+        sl.connect_ipc()
+    links = sl.pack_links(U)
+    a, b = sl.pack_spinor(ie, 0), sl.pack_spinor(io, 1)
+    oo, oe = sl.new_spinor(), sl.new_spinor()
+
+    def step():
+        sl.dslash(1, oo, a, links)
+        sl.dslash(0, oe, b, links)
+    n = 200
+    us = timed_loop(torch, step, n, 10, world, D, device) * 1e3 / (2 * n)
+    shifts = gen.rhmc_shifts(8)
+    xs = [sl.new_spinor() for _ in shifts]
+
+    def solve(m):
+        return ev_ms(torch, lambda: sl.cg_multishift(xs, a, links, 0.0025, shifts, 1e-300, m, raise_on_max_iter=False))[0]
+    solve(16)
+    D.barrier(world)
+    t_lo, t_hi = min(solve(16), solve(16)), min(solve(80), solve(80))
+    it_us = D.max_over_ranks((t_hi - t_lo) / 64 * 1e3, world, device)
+    graph = sl.lat.get_option("graph_active")
+    halo = sl.lat.halo_bytes
+    sl.close()
+    out = {"dims": list(DIMS), "ranks": world, "transport": "peer (lqcd_peer_*: P2P stores into the neighbours' landing "
+           "buffers, in-kernel flag waits, dot products gathered by the consumer kernels)",
+           "dslash_us": us, "dslash_ns_per_site": us * 1e3 / (V // 2), "dslash_GBs_aggregate": 1248 * (V // 2) / us / 1e3,
+           "multishift8_us_per_iter": it_us, "multishift8_iter_per_s": 1e6 / it_us, "chunk_graph": graph,
+           "halo_bytes_per_face": halo, "faces_per_dslash": 2, "allreduces_per_iteration": 2, "scaling": "strong"}
+    if plain_us is not None:
+        out["dslash_overhead_us_vs_plain_context"] = us - plain_us
+    return out
 
 
 def dslash_rate(torch, L, D, gen, dims, U, in_e, in_o, prec, recon, peak, device, n=100, theta=None, bf_format=0,

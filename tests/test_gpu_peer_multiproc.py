@@ -1,0 +1,74 @@
+"""-m gpu, needs >= 2 GPUs (skipped otherwise -- this project's GPU boxes have one): the peer transport with ONE
+PROCESS PER GPU, the blocks mapped through CUDA IPC (SlabLattice.connect_ipc), the kernels of the two ranks really
+waiting for one another.  Dslash and a multi-shift solve on a lattice split in two x3 slabs against the oracle on the
+global lattice."""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def _worker(rank, world, port, ret):
+    import torch
+    import torch.distributed as dist
+    import lqcd_inputs as gen
+    import oracle
+    from paper_1701_00426_b200.slab import SlabLattice
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    torch.cuda.set_device(rank)
+    dist.init_process_group("nccl", rank=rank, world_size=world)
+    dims = (8, 8, 4, 8)
+    rng = np.random.default_rng(81)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    shifts = gen.rhmc_shifts(4)
+    sl = SlabLattice(dims, world, rank, device=rank, transport="peer")
+    sl.connect_ipc()
+    links = sl.pack_links(U)
+    be = sl.pack_spinor(b, 0)
+    out = sl.new_spinor()
+    sl.dslash(1, out, be, links)
+    xs = [sl.new_spinor() for _ in shifts]
+    res = sl.cg_multishift(xs, be, links, 0.05, shifts, 1e-10, 5000)
+    got = np.zeros_like(b)
+    sl.unpack_spinor(out, 1, got)
+    sols = []
+    for x in xs:
+        g = np.zeros_like(b)
+        sl.unpack_spinor(x, 0, g)
+        sols.append(g)
+    # every rank holds its own slices; sum the disjoint pieces on rank 0
+    pieces = [None] * world
+    dist.all_gather_object(pieces, (got, sols, res["iters"], sl.lat.get_option("graph_active")))
+    if rank == 0:
+        want = oracle.dslash_half(dims, U, 1, b)
+        ref = oracle.cg_multishift(dims, U, 0.05, shifts, b, 1e-10, 5000)
+        d = sum(p[0] for p in pieces)
+        ok = np.linalg.norm(d - want) / np.linalg.norm(want) < 1e-12
+        ok = ok and all(p[2] == pieces[0][2] for p in pieces) and abs(pieces[0][2] - ref["iters"]) <= 2
+        ok = ok and all(p[3] == 1 for p in pieces)              # the chunk graph stayed on
+        for i, s in enumerate(shifts):
+            x = sum(p[1][i] for p in pieces)
+            tr = np.linalg.norm(b - oracle.mdagm(dims, U, 0.05, x, sigma=s)) / np.linalg.norm(b)
+            ok = ok and tr < 1.5e-10
+        ret["ok"] = bool(ok)
+    sl.close()
+    dist.destroy_process_group()
+
+
+def test_peer_transport_two_processes_two_gpus():
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    ret = ctx.Manager().dict()
+    procs = [ctx.Process(target=_worker, args=(r, 2, 29533, ret)) for r in range(2)]
+    for p in procs:
+        p.start()
+    for p in procs:
+        p.join(300)
+    assert all(p.exitcode == 0 for p in procs)
+    assert ret.get("ok") is True
