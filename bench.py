@@ -284,10 +284,10 @@ def ensure_built():
 
 def dslash_kernel_name(lat, L, prec, recon):
     """Name of the Dslash instantiation the default options launch (template arguments of
-    dslash_kernel<T, LAYOUT, RECON12, MODE, MINB, POLICY> in csrc/dslash.cu)."""
+    dslash_kernel<T, LAYOUT, RECON12, MODE, MINB, POLICY, BF, HALO> in csrc/dslash.cu; no backfield, no peer transport)."""
     minb = lat.get_option("dslash_minblocks") or (2 if prec == L.F64 else 4)
     return (f"dslash_kernel<{'double' if prec == L.F64 else 'float'},{lat.get_option('layout')},"
-            f"{1 if recon == L.RECON_12 else 0},0,{minb},{lat.get_option('l2_hints')}>")
+            f"{1 if recon == L.RECON_12 else 0},0,{minb},{lat.get_option('l2_hints')},0,0>")
 
 
 def run_ours(args):
