@@ -65,6 +65,8 @@ _lib.oracle_cg_multishift_bf.argtypes = [_i4, C.c_int, _c128, C.c_void_p, C.c_do
                                          C.c_double, C.c_int, _pi, _pi, _pd, _pd, C.c_void_p,
                                          _pd, _pd, _pd, C.c_int]
 _lib.oracle_cg_multishift_bf.restype = C.c_int
+_lib.oracle_fermion_force_bf.argtypes = [_i4, C.c_int, _c128, C.c_void_p, C.c_int, _pd, _c128, _c128]
+_lib.oracle_fermion_force_bf.restype = C.c_int
 _lib.oracle_num_threads.restype = C.c_int
 _lib.oracle_set_num_threads.argtypes = [C.c_int]
 
@@ -278,16 +280,22 @@ def rational_apply(dims, U, mass, shifts, c0, coeffs, b, tol, max_iter, antiperi
     return dict(y=y, iters=iters.value, converged=(rc == 0), conv_iter=np.array(list(conv)))
 
 
-def fermion_force(dims, U, coeffs, xs, antiperiodic_t=True):
-    """F[V,4,3,3] = TA[U_mu(x) Q_mu(x)] from the solutions xs[nshift, V/2, 3] (even sites) and c_i."""
+def fermion_force(dims, U, coeffs, xs, antiperiodic_t=True, theta=None):
+    """F[V,4,3,3] = TA[U_mu(x) Q_mu(x)] from the solutions xs[nshift, V/2, 3] (even sites) and c_i.
+    theta: optional backfield [V][4] (links e^{i theta} U in D and in the force)."""
     n4, V = _dims(dims)
     coeffs = np.ascontiguousarray(coeffs, dtype=np.float64)
     xs = np.ascontiguousarray(xs, dtype=np.complex128)
     if xs.shape != (coeffs.size, V // 2, 3):
         raise ValueError(f"xs must be ({coeffs.size}, {V // 2}, 3)")
     F = np.empty((V, 4, 3, 3), dtype=np.complex128)
-    rc = _lib.oracle_fermion_force(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), coeffs.size, _dptr(coeffs),
-                                   xs.reshape(-1), F.reshape(-1))
+    if theta is None:
+        rc = _lib.oracle_fermion_force(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), coeffs.size, _dptr(coeffs),
+                                       xs.reshape(-1), F.reshape(-1))
+    else:
+        th = _Theta(theta, V)
+        rc = _lib.oracle_fermion_force_bf(n4, int(antiperiodic_t), _arr(U, (V, 4, 3, 3)), th.ptr, coeffs.size,
+                                          _dptr(coeffs), xs.reshape(-1), F.reshape(-1))
     if rc:
         raise MemoryError("oracle_fermion_force")
     return F

@@ -31,7 +31,7 @@
  * entry points) is pinned by: theta = 0 reproduces D; the dense matrix built with phased links; the
  * phases absorbed into the links give the same D through the plain entry points; a constant theta_mu
  * shifts the free-field momenta, p_mu -> p_mu + theta_mu; a pure-gauge theta is removed by a U(1) gauge
- * transformation.
+ * transformation; the fermion force with a backfield by finite differences of the action with phased dense solves.
  * No function in this file is "parity unpinned".
  *
  * OpenMP is used on the site loop of the operator only, so that bench.py can time the
@@ -541,8 +541,11 @@ int oracle_rational_apply(const int N[4], int antiperiodic_t, const cplx *U, dou
  *
  * x: nshift even half vectors, contiguous.  F: [V][4][3][3], row-major.  Returns 0, or -1.
  * ------------------------------------------------------------------------------------- */
-int oracle_fermion_force(const int N[4], int antiperiodic_t, const cplx *U, int nshift,
-                         const double *c, const cplx *x, cplx *F)
+/* With the optional backfield theta (NULL: none; reading R6): the links of D are e^{i theta} U, a left
+ * multiplication exp(i eps T) U commutes with the phase, so F_mu(x) = TA[ e^{i theta_mu(x)} U_mu(x) Q_mu(x) ] with the
+ * y_i = D_oe x_i of the phased operator. */
+int oracle_fermion_force_bf(const int N[4], int antiperiodic_t, const cplx *U, const double *theta, int nshift,
+                            const double *c, const cplx *x, cplx *F)
 {
     size_t V = vol(N), nh = V / 2 * 3;
     cplx *w = (cplx *)malloc(V * 3 * (size_t)nshift * sizeof(cplx));
@@ -551,7 +554,7 @@ int oracle_fermion_force(const int N[4], int antiperiodic_t, const cplx *U, int 
     if (!w || !y || !full) { free(w); free(y); free(full); return -1; }
     for (int i = 0; i < nshift; ++i) {
         cplx *wi = w + (size_t)i * V * 3;
-        if (oracle_dslash_half(N, antiperiodic_t, U, 1, x + (size_t)i * nh, y)) { free(w); free(y); free(full); return -1; }
+        if (oracle_dslash_half_bf(N, antiperiodic_t, U, theta, 1, x + (size_t)i * nh, y)) { free(w); free(y); free(full); return -1; }
         oracle_half_to_full(N, 0, x + (size_t)i * nh, wi);        /* even sites: x_i, odd: 0 */
         oracle_half_to_full(N, 1, y, full);                        /* odd sites: y_i, even: 0 */
         for (size_t j = 0; j < V * 3; ++j) wi[j] += full[j];
@@ -574,11 +577,12 @@ int oracle_fermion_force(const int N[4], int antiperiodic_t, const cplx *U, int 
                     for (int b = 0; b < 3; ++b) Q[a][b] += c[i] * wi[lf * 3 + a] * conj(wi[lex * 3 + b]);
             }
             const cplx *u = U + (lex * 4 + (size_t)mu) * 9;
+            const cplx ph = theta ? cexp(I * theta[lex * 4 + (size_t)mu]) : 1.0;
             for (int a = 0; a < 3; ++a)
                 for (int b = 0; b < 3; ++b) {
                     cplx t = 0.0;
                     for (int k = 0; k < 3; ++k) t += u[a * 3 + k] * (e * Q[k][b]);
-                    M[a][b] = t;
+                    M[a][b] = theta ? ph * t : t;
                 }
             cplx tr = 0.0;
             for (int a = 0; a < 3; ++a) tr += M[a][a] - conj(M[a][a]);
@@ -590,6 +594,12 @@ int oracle_fermion_force(const int N[4], int antiperiodic_t, const cplx *U, int 
     }
     free(w); free(y); free(full);
     return 0;
+}
+
+int oracle_fermion_force(const int N[4], int antiperiodic_t, const cplx *U, int nshift,
+                         const double *c, const cplx *x, cplx *F)
+{
+    return oracle_fermion_force_bf(N, antiperiodic_t, U, NULL, nshift, c, x, F);
 }
 
 /* ---------------------------------------------------------------------------------------

@@ -583,6 +583,53 @@ def test_fermion_force_against_finite_differences_of_the_action(dims, ap):
     assert {int(coords[p].sum() % 2) for p in picks} == {0, 1}
 
 
+@pytest.mark.parametrize("dims,ap", [((2, 2, 2, 4), True), ((2, 4, 2, 2), False)])
+def test_fermion_force_with_backfield_against_finite_differences(dims, ap):
+    """oracle_fermion_force_bf (reading R6 + R21): with links e^{i theta} U in D, dS/d eps under U_mu(x) -> exp(i eps
+    T_a) U_mu(x) equals 2 Re Tr[i T_a F_mu(x)]; S by DENSE solves with the phased dense operator (no oracle code in S).
+    Also: theta = 0 reproduces the plain force, and the phases absorbed into the links give the same force through
+    the plain entry point (the force of a left multiplication does not care which factor carries the phase)."""
+    rng = np.random.default_rng(19)
+    U = gen.haar_like_links(dims, rng)
+    phi = gen.gaussian_half_spinor(dims, rng)
+    theta = gen.uniform_backfield(dims, rng)
+    m = 0.4
+    shifts = np.array([0.05, 0.7])
+    c = np.array([0.8, -0.45])
+    V = gen.volume(dims)
+
+    def action(Uv):
+        A, _, _ = dense_normal_operator(dims, Uv, m, antiperiodic_t=ap, theta=theta)
+        b = phi.reshape(-1)
+        return sum(ci * np.real(np.vdot(b, np.linalg.solve(A + s * np.eye(A.shape[0]), b))) for ci, s in zip(c, shifts))
+
+    A, _, _ = dense_normal_operator(dims, U, m, antiperiodic_t=ap, theta=theta)
+    xs = np.stack([np.linalg.solve(A + s * np.eye(A.shape[0]), phi.reshape(-1)).reshape(-1, 3) for s in shifts])
+    F = oracle.fermion_force(dims, U, c, xs, antiperiodic_t=ap, theta=theta)
+    assert np.abs(F + F.conj().transpose(0, 1, 3, 2)).max() < 1e-14
+    assert np.abs(np.trace(F, axis1=2, axis2=3)).max() < 1e-14
+    lam = _gell_mann()
+    eps = 1e-5
+    worst = 0.0
+    for k, lex in enumerate([0, 1, V - 1, V // 2 + 1]):
+        for mu in range(4):
+            a = (3 * k + mu + 2) % 8
+            Up, Um = U.copy(), U.copy()
+            Up[lex, mu] = _expm_herm(lam[a], eps) @ U[lex, mu]
+            Um[lex, mu] = _expm_herm(lam[a], -eps) @ U[lex, mu]
+            fd = (action(Up) - action(Um)) / (2 * eps)
+            an = 2 * np.real(np.trace(1j * lam[a] @ F[lex, mu]))
+            worst = max(worst, abs(fd - an) / max(1e-3, abs(an)))
+    assert worst < 1e-6, worst
+    # phases absorbed into the links, plain entry point
+    Uph = U * np.exp(1j * theta)[:, :, None, None]
+    assert rel(oracle.fermion_force(dims, Uph, c, xs, antiperiodic_t=ap), F) < 1e-13
+    # theta = 0 is the plain force; the phases matter
+    F0 = oracle.fermion_force(dims, U, c, xs, antiperiodic_t=ap)
+    assert np.array_equal(oracle.fermion_force(dims, U, c, xs, antiperiodic_t=ap, theta=np.zeros((V, 4))), F0)
+    assert rel(F0, F) > 0.1
+
+
 def _gauge_W(dims, U, c0, c1):
     """W = sum_x sum_{mu<nu} c0 ReTr P + c1 (ReTr R_{mu nu} + ReTr R_{nu mu}), with numpy rolls on the
     [x3,x2,x1,x0] grid -- independent of the oracle's path walker.  Returns (W, sum ReTr P, sum ReTr R)."""
