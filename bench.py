@@ -486,6 +486,15 @@ def run_ours(args):
                 "hbm_bytes_per_site_two_pass": STAPLES2_BYTES_PER_SITE, "hbm_GBs": gbs, "hbm_frac": gbs / peak,
                 "note2": "variant 2 trades FP64 work for HBM traffic (39 instead of 66 / 84 products per link, 24 stored "
                          "3-link staples per site): both fractions are reported; time per site is the figure of merit"})
+        # the one-pass kernel (variant 1: 66 products per link, no workspace) beside it: the FP64-bound alternative
+        lat.set_option("staples_variant", 1)
+        t_1 = timed_loop(torch, lambda: lat.gauge_staples(links, out=sbuf), 10, 3, 1, D, device) / 10
+        lat.set_option("staples_variant", 2)
+        f1 = 4 * STAPLES_EXEC_FLOP_PER_LINK[1]
+        extra["gauge_staples_f64_one_pass"] = {"ms": t_1, "ns_per_site": t_1 * 1e6 / V, "bound": "alu", "variant": 1,
+                                               "flop_per_site_executed": f1, "TFLOPs_executed": f1 * V / (t_1 * 1e-3) / 1e12,
+                                               "frac": f1 * V / (t_1 * 1e-3) / 1e12 / fp64_peak,
+                                               "frac_by_definition_count": flop_def * V / (t_1 * 1e-3) / 1e12 / fp64_peak}
         del sbuf
         cfg2 = cfg4 = None
         if not args.quick:

@@ -130,8 +130,8 @@ int lqcd_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void
  * lqcd_set_backfield attaches a native phase field to the context (NULL detaches): every later lqcd_dslash,
  * lqcd_dslash_slices, lqcd_mdagm, lqcd_cg, lqcd_cg_multishift, lqcd_rational_apply and *_host* call of this
  * context then uses it, at 8 (4) extra bytes per link and application: 1248 + 64 B per site in fp64.  The
- * buffer must stay valid while attached.  lqcd_fermion_force returns LQCD_ERR_UNSUPPORTED while a backfield is
- * attached; the gauge staples do not depend on it.  With a backfield the Dslash tuning options
+ * buffer must stay valid while attached.  lqcd_fermion_force uses it too (the y_i = D_oe x_i of the phased operator
+ * and F = TA[e^{i theta} U Q]); the gauge staples do not depend on it.  With a backfield the Dslash tuning options
  * dslash_minblocks and l2_hints have no effect.  Option "backfield_format" (before the first pack): 0 (default)
  * stores theta and evaluates sincos in the kernel; 1 stores (cos theta, sin theta), twice the bytes and no
  * sincos -- measured at 32^4: 104 vs 105 us (fp64 18-real), 90 vs 82 us (fp64 12-real).  async.

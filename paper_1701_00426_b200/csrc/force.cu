@@ -29,7 +29,8 @@ struct ForceVecs {
 // direction; ncu had shown the four re-reads missing L1 (hit rate 0.8 %) and costing +33 % DRAM reads.
 template <typename T, int LAYOUT, int RECON12, int STAGE, int FB, int MINB>
 __global__ void __launch_bounds__(128, MINB) force_kernel(const Geom g, const int parity, T *__restrict__ force,
-                                                    const T *__restrict__ links, const ForceVecs fv)
+                                                    const T *__restrict__ links, const ForceVecs fv,
+                                                    const T *__restrict__ bf, const int bf_fmt)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T *const own = reinterpret_cast<T *>(smem_raw);      // own[(s*6 + k)*128 + tid]
@@ -108,6 +109,15 @@ __global__ void __launch_bounds__(128, MINB) force_kernel(const Geom g, const in
             }
         }
         const Su3<T> u = load_link<T, LAYOUT, RECON12, 0>(links, parity, mu, (size_t)g.Ls, (size_t)i, pol);
+        // backfield (reading R6): the link of D is e^{i theta} U, and so is the link of the force
+        T pr = e[mu], pi = (T)0;
+        if (bf) {
+            T sn, cs;
+            const size_t k = (size_t)(parity * 4 + mu) * Vh + i;
+            if (bf_fmt == 0) sincos_t(__ldcs(bf + k), &sn, &cs);
+            else { cs = __ldcs(bf + 2 * k); sn = __ldcs(bf + 2 * k + 1); }
+            pr = e[mu] * cs; pi = e[mu] * sn;
+        }
         Cx<T> M[3][3];
 #pragma unroll
         for (int a = 0; a < 3; ++a)
@@ -121,7 +131,7 @@ __global__ void __launch_bounds__(128, MINB) force_kernel(const Geom g, const in
                     im = fma(u.e[a][k].re, Q[k][b].im, im);
                     im = fma(u.e[a][k].im, Q[k][b].re, im);
                 }
-                M[a][b] = cx<T>(e[mu] * re, e[mu] * im);
+                M[a][b] = cx<T>(pr * re - pi * im, pr * im + pi * re);
             }
         // TA[M]: Tr(M - M^dagger) = 2 i sum_a Im M_aa
         const T tr3 = (M[0][0].im + M[1][1].im + M[2][2].im) / (T)3;
@@ -223,11 +233,11 @@ static void launch_force_tlb(lqcd_ctx *ctx, int parity, void *force, const void 
     const size_t smem = (size_t)fv.n * 6 * 128 * sizeof(T);
     // measured at 32^4 (profiles/experiments_r1b.md section 7): fp64 -3 %, fp32 +20 % (the carve-out costs L1)
     if (smem <= 48 * 1024 && ctx->force_stage && sizeof(T) == 8) {
-        if (ctx->recon == LQCD_RECON_12) launch_k_smem(ctx, force_kernel<T, LAYOUT, 1, 1, FB, MINB>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv);
-        else launch_k_smem(ctx, force_kernel<T, LAYOUT, 0, 1, FB, MINB>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv);
+        if (ctx->recon == LQCD_RECON_12) launch_k_smem(ctx, force_kernel<T, LAYOUT, 1, 1, FB, MINB>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
+        else launch_k_smem(ctx, force_kernel<T, LAYOUT, 0, 1, FB, MINB>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
     } else {
-        if (ctx->recon == LQCD_RECON_12) launch_k(ctx, force_kernel<T, LAYOUT, 1, 0, FB, MINB>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv);
-        else launch_k(ctx, force_kernel<T, LAYOUT, 0, 0, FB, MINB>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv);
+        if (ctx->recon == LQCD_RECON_12) launch_k(ctx, force_kernel<T, LAYOUT, 1, 0, FB, MINB>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
+        else launch_k(ctx, force_kernel<T, LAYOUT, 0, 0, FB, MINB>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
     }
 }
 
@@ -259,7 +269,6 @@ extern "C" int lqcd_fermion_force(lqcd_ctx *ctx, int nshift, const double *coeff
     }
     if (ctx->halo_fn || ctx->x3_lo != 0 || ctx->x3_hi != ctx->g.N3)
         return lqcd_fail(ctx, LQCD_ERR_UNSUPPORTED, "lqcd_fermion_force: not available in slab mode");
-    if (ctx->backfield) return lqcd_fail(ctx, LQCD_ERR_UNSUPPORTED, "lqcd_fermion_force: not available with a backfield attached");
     if (!ctx->ws) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "no workspace set");
     if (ctx->ws_bytes < lqcd_workspace_bytes(ctx, nshift))
         return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "workspace %zu bytes < %zu needed for %d shifts", ctx->ws_bytes, lqcd_workspace_bytes(ctx, nshift), nshift);

@@ -267,6 +267,9 @@ __device__ __forceinline__ Su3<T> link_rel(const T *__restrict__ links, const Ge
     return dag ? dagger<T>(L) : L;
 }
 
+template <typename T, int LAYOUT>
+__device__ __forceinline__ void store_mat_stream(T *__restrict__ f, size_t plane0, size_t Vh, size_t i, const Su3<T> &m);
+
 template <typename T, int LAYOUT, int RECON12>
 __global__ void __launch_bounds__(128, 2) staples_kernel_shared(const Geom g, T *__restrict__ staples,
                                                                 const T *__restrict__ links, const T c0, const T c1, const StapleSwizzle sw)
@@ -340,12 +343,9 @@ __global__ void __launch_bounds__(128, 2) staples_kernel_shared(const Geom g, T 
     }
 #undef LKM
 #undef LKN
-    const L2Pol pol = {0, 0};
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b)
-            st_cx<T, LAYOUT, 0>(staples, (size_t)((parity * 4 + mu) * 9 + a * 3 + b), (size_t)g.Vh, (size_t)i, S.e[a][b], pol);
+    // streaming stores: the output must not evict the link neighbourhood from L2 (round 1: 855 MB written to DRAM
+    // against 604 MB of output)
+    store_mat_stream<T, LAYOUT>(staples, (size_t)((parity * 4 + mu) * 9), (size_t)g.Vh, (size_t)i, S);
 }
 
 

@@ -188,22 +188,45 @@ def test_backfield_large_volume_sampled_sites(fmt):
     lat.close()
 
 
+@pytest.mark.parametrize("fmt", [0, 1])
+@pytest.mark.parametrize("recon", [0, 1])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_fermion_force_with_backfield(prec, recon, fmt):
+    """lqcd_fermion_force with a backfield attached: F = TA[e^{i theta} U Q] with the y_i of the phased operator,
+    element by element against oracle_fermion_force_bf (pinned by finite differences on the CPU)."""
+    dims = (6, 4, 10, 8)
+    rng = np.random.default_rng(67)
+    U = gen.haar_like_links(dims, rng)
+    theta = gen.uniform_backfield(dims, rng)
+    n = 3
+    xs = np.stack([gen.gaussian_half_spinor(dims, rng) for _ in range(n)])
+    if prec == 1:
+        U = U.astype(np.complex64).astype(np.complex128)
+        xs = xs.astype(np.complex64).astype(np.complex128)
+        theta = theta.astype(np.float32).astype(np.float64)
+        if recon == 1:
+            U = oracle.reconstruct_row3(U)
+    c = np.array([0.7, -1.1, 0.4])
+    lat = make_lattice(dims, prec, recon, backfield_format=fmt)
+    links = lat.pack_links(U)
+    lat.set_backfield(lat.pack_backfield(theta))
+    got = lat.unpack_tamat(lat.fermion_force([lat.pack_spinor(x, 0) for x in xs], links, c))
+    want = oracle.fermion_force(dims, U, c, xs, theta=theta)
+    assert rel(got, want) < TOL[prec], (prec, recon, fmt, rel(got, want))
+    assert rel(oracle.fermion_force(dims, U, c, xs), want) > 0.1          # the phases matter
+    lat.close()
+
+
 def test_backfield_errors():
     import paper_1701_00426_b200 as L
     dims = (4, 4, 4, 4)
     rng = np.random.default_rng(66)
     U = gen.smooth_links(dims, 0.3, rng)
     lat = make_lattice(dims)
-    links = lat.pack_links(U)
-    bf = lat.pack_backfield(gen.uniform_backfield(dims, rng))
-    x = lat.pack_spinor(gen.gaussian_half_spinor(dims, rng), 0)
-    lat.set_backfield(bf)
-    with pytest.raises(L.LqcdError) as e:
-        lat.fermion_force([x], links, [1.0])
-    assert e.value.code == L.ERR_UNSUPPORTED
-    lat.set_backfield(None)
-    lat.fermion_force([x], links, [1.0])
-    lat.synchronize()
+    lat.pack_links(U)
+    lat.pack_backfield(gen.uniform_backfield(dims, rng))
     with pytest.raises(L.LqcdError):            # the format is fixed once a backfield was packed
         lat.set_option("backfield_format", 1)
+    with pytest.raises(L.LqcdError):
+        lat.set_option("backfield_format", 2)       # out of range
     lat.close()

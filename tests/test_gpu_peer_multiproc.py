@@ -1,6 +1,6 @@
-"""-m gpu, needs >= 2 GPUs (skipped otherwise -- this project's GPU boxes have one): the peer transport with ONE
-PROCESS PER GPU, the blocks mapped through CUDA IPC (SlabLattice.connect_ipc), the kernels of the two ranks really
-waiting for one another.  Dslash and a multi-shift solve on a lattice split in two x3 slabs against the oracle on the
+"""-m gpu, needs >= 2 GPUs (skipped otherwise -- this project's GPU boxes have one): both slab transports with ONE
+PROCESS PER GPU: the peer transport with the blocks mapped through CUDA IPC (SlabLattice.connect_ipc), the kernels of
+the two ranks really waiting for one another, and the hook transport over NCCL.  Dslash and a multi-shift solve on a lattice split in two x3 slabs against the oracle on the
 global lattice."""
 import os
 
@@ -10,7 +10,7 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 
-def _worker(rank, world, port, ret):
+def _worker(rank, world, port, ret, transport="peer"):
     import torch
     import torch.distributed as dist
     import lqcd_inputs as gen
@@ -24,8 +24,9 @@ def _worker(rank, world, port, ret):
     U = gen.smooth_links(dims, 0.3, rng)
     b = gen.gaussian_half_spinor(dims, rng)
     shifts = gen.rhmc_shifts(4)
-    sl = SlabLattice(dims, world, rank, device=rank, transport="peer")
-    sl.connect_ipc()
+    sl = SlabLattice(dims, world, rank, device=rank, transport=transport)
+    if transport == "peer":
+        sl.connect_ipc()
     links = sl.pack_links(U)
     be = sl.pack_spinor(b, 0)
     out = sl.new_spinor()
@@ -48,7 +49,7 @@ def _worker(rank, world, port, ret):
         d = sum(p[0] for p in pieces)
         ok = np.linalg.norm(d - want) / np.linalg.norm(want) < 1e-12
         ok = ok and all(p[2] == pieces[0][2] for p in pieces) and abs(pieces[0][2] - ref["iters"]) <= 2
-        ok = ok and all(p[3] == 1 for p in pieces)              # the chunk graph stayed on
+        ok = ok and all(p[3] == (1 if transport == "peer" else 0) for p in pieces)    # peer: the chunk graph stayed on
         for i, s in enumerate(shifts):
             x = sum(p[1][i] for p in pieces)
             tr = np.linalg.norm(b - oracle.mdagm(dims, U, 0.05, x, sigma=s)) / np.linalg.norm(b)
@@ -58,14 +59,17 @@ def _worker(rank, world, port, ret):
     dist.destroy_process_group()
 
 
-def test_peer_transport_two_processes_two_gpus():
+@pytest.mark.parametrize("transport,port", [("peer", 29533), ("hooks", 29534)])
+def test_slab_transports_two_processes_two_gpus(transport, port):
+    """peer: CUDA IPC blocks, in-kernel waits.  hooks: SlabComm over NCCL (isend / irecv of CUDA tensors, all-reduce of
+    a raw device address) -- the path ADVICE round 1 noted had only ever run under gloo."""
     import torch
     if torch.cuda.device_count() < 2:
         pytest.skip("needs two GPUs")
     import torch.multiprocessing as mp
     ctx = mp.get_context("spawn")
     ret = ctx.Manager().dict()
-    procs = [ctx.Process(target=_worker, args=(r, 2, 29533, ret)) for r in range(2)]
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, ret, transport)) for r in range(2)]
     for p in procs:
         p.start()
     for p in procs:
