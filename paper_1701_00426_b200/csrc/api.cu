@@ -139,7 +139,7 @@ struct OptDesc { const char *name; size_t off; long lo, hi; };
 static const OptDesc g_opts[] = {
     OPT(layout, 0, 1), OPT(l2_hints, 0, 1), OPT(l2_persist, 0, 4), OPT(link_pad, 0, 1 << 20), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
     OPT(blas_block, 64, 256), OPT(blas_ctas_per_sm, 1, 32), OPT(poll_chunk, 1, 1024),
-    OPT(pdl, 0, 1), OPT(graph, 0, 1), OPT(dslash_persist, 0, 16), OPT(iter_mask, 0, 15), OPT(staples_variant, 0, 2), OPT(staples_minblocks, 0, 4), OPT(force_stage, 0, 1), OPT(force_batch, 0, 8), OPT(staples_x2block, 0, 64), OPT(backfield_format, 0, 1),
+    OPT(pdl, 0, 1), OPT(graph, 0, 1), OPT(dslash_persist, 0, 16), OPT(iter_mask, 0, 15), OPT(staples_variant, 0, 2), OPT(staples_minblocks, 0, 4), OPT(force_stage, 0, 1), OPT(staples_x2block, 0, 64), OPT(backfield_format, 0, 1),
 };
 
 extern "C" int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value)

@@ -279,7 +279,6 @@ struct lqcd_ctx {
     int backfield_format;  // 0: theta stored (one real per link, sincos in-kernel); 1: (cos theta, sin theta) stored
     int backfield_locked;  // a backfield was packed: the format can no longer change
     const void *backfield; // native U(1) phase field applied by every Dslash of this context (NULL: none; lqcd_set_backfield)
-    int force_batch;       // neighbour vectors requested together by force_kernel (1, 2, 4, 8; 0: default)
     int force_stage;       // 1: force_kernel stages the site's own vectors in shared memory when they fit
     int staples_x2block;   // x2 block size of the staples' CTA order (0: plain idxh order)
     int staples_variant;   // 0: one product chain per path; 1: shared sub-products per (mu, nu); 2: two passes through

@@ -27,8 +27,8 @@ struct ForceVecs {
 // STAGE = 1: the site's own n vectors are read from global memory ONCE into the thread's private
 // column of dynamic shared memory (n * 6 reals * 128 threads <= 48 KB) and re-read from there for each
 // direction; ncu had shown the four re-reads missing L1 (hit rate 0.8 %) and costing +33 % DRAM reads.
-template <typename T, int LAYOUT, int RECON12, int STAGE, int FB, int MINB>
-__global__ void __launch_bounds__(128, MINB) force_kernel(const Geom g, const int parity, T *__restrict__ force,
+template <typename T, int LAYOUT, int RECON12, int STAGE>
+__global__ void __launch_bounds__(128, 5) force_kernel(const Geom g, const int parity, T *__restrict__ force,
                                                     const T *__restrict__ links, const ForceVecs fv,
                                                     const T *__restrict__ bf, const int bf_fmt)
 {
@@ -79,34 +79,26 @@ __global__ void __launch_bounds__(128, MINB) force_kernel(const Geom g, const in
         for (int a = 0; a < 3; ++a)
 #pragma unroll
             for (int b = 0; b < 3; ++b) Q[a][b] = cx<T>((T)0, (T)0);
-        // the neighbour vectors of FB shifts are requested before the first outer product (option force_batch)
-        for (int s0 = 0; s0 < fv.n; s0 += FB) {
-            Cx<T> wnb[FB][3];
+        for (int s = 0; s < fv.n; ++s) {
+            Cx<T> ws[3], wn[3];
+            if (STAGE) {
 #pragma unroll
-            for (int b = 0; b < FB; ++b)
-                if (s0 + b < fv.n) load_vec<T, LAYOUT, 0>((const T *)fv.nbr[s0 + b], Vh, (size_t)nf[mu], (T)fv.coef[s0 + b], wnb[b], pol);
+                for (int c = 0; c < 3; ++c)
+                    ws[c] = cx<T>(own[(s * 6 + 2 * c) * 128 + threadIdx.x], own[(s * 6 + 2 * c + 1) * 128 + threadIdx.x]);
+            } else load_vec<T, LAYOUT, 0>((const T *)fv.self[s], Vh, (size_t)i, (T)1, ws, pol);
+            load_vec<T, LAYOUT, 0>((const T *)fv.nbr[s], Vh, (size_t)nf[mu], (T)fv.coef[s], wn, pol);
+            // Q[a][b] += c w(x+mu)[a] conj(w(x)[b])
+            // (requesting the neighbour vectors of 2 / 4 / 8 shifts together was tried in round 2 and is slower at
+            // every batch size: profiles/sweep_r2.md section 5)
 #pragma unroll
-            for (int b = 0; b < FB; ++b) {
-                const int s = s0 + b;
-                if (s < fv.n) {
-                Cx<T> ws[3];
-                if (STAGE) {
+            for (int a = 0; a < 3; ++a)
 #pragma unroll
-                    for (int c = 0; c < 3; ++c)
-                        ws[c] = cx<T>(own[(s * 6 + 2 * c) * 128 + threadIdx.x], own[(s * 6 + 2 * c + 1) * 128 + threadIdx.x]);
-                } else load_vec<T, LAYOUT, 0>((const T *)fv.self[s], Vh, (size_t)i, (T)1, ws, pol);
-                // Q[a][b] += c w(x+mu)[a] conj(w(x)[b])
-#pragma unroll
-                for (int a = 0; a < 3; ++a)
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        Q[a][c].re = fma(wnb[b][a].re, ws[c].re, Q[a][c].re);
-                        Q[a][c].re = fma(wnb[b][a].im, ws[c].im, Q[a][c].re);
-                        Q[a][c].im = fma(wnb[b][a].im, ws[c].re, Q[a][c].im);
-                        Q[a][c].im = fma(-wnb[b][a].re, ws[c].im, Q[a][c].im);
-                    }
+                for (int b = 0; b < 3; ++b) {
+                    Q[a][b].re = fma(wn[a].re, ws[b].re, Q[a][b].re);
+                    Q[a][b].re = fma(wn[a].im, ws[b].im, Q[a][b].re);
+                    Q[a][b].im = fma(wn[a].im, ws[b].re, Q[a][b].im);
+                    Q[a][b].im = fma(-wn[a].re, ws[b].im, Q[a][b].im);
                 }
-            }
         }
         const Su3<T> u = load_link<T, LAYOUT, RECON12, 0>(links, parity, mu, (size_t)g.Ls, (size_t)i, pol);
         // backfield (reading R6): the link of D is e^{i theta} U, and so is the link of the force
@@ -226,33 +218,19 @@ extern "C" size_t lqcd_force_bytes(const lqcd_ctx *ctx)
     return ctx ? (size_t)ctx->g.Vh * 2 * 4 * 9 * 2 * elem_size(ctx) : 0;
 }
 
-template <typename T, int LAYOUT, int FB, int MINB>
-static void launch_force_tlb(lqcd_ctx *ctx, int parity, void *force, const void *links, const ForceVecs &fv)
+template <typename T, int LAYOUT>
+static void launch_force_tl(lqcd_ctx *ctx, int parity, void *force, const void *links, const ForceVecs &fv)
 {
     dim3 grid((ctx->g.Vh + 127) / 128), block(128);
     const size_t smem = (size_t)fv.n * 6 * 128 * sizeof(T);
     // measured at 32^4 (profiles/experiments_r1b.md section 7): fp64 -3 %, fp32 +20 % (the carve-out costs L1)
     if (smem <= 48 * 1024 && ctx->force_stage && sizeof(T) == 8) {
-        if (ctx->recon == LQCD_RECON_12) launch_k_smem(ctx, force_kernel<T, LAYOUT, 1, 1, FB, MINB>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
-        else launch_k_smem(ctx, force_kernel<T, LAYOUT, 0, 1, FB, MINB>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
+        if (ctx->recon == LQCD_RECON_12) launch_k_smem(ctx, force_kernel<T, LAYOUT, 1, 1>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
+        else launch_k_smem(ctx, force_kernel<T, LAYOUT, 0, 1>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
     } else {
-        if (ctx->recon == LQCD_RECON_12) launch_k(ctx, force_kernel<T, LAYOUT, 1, 0, FB, MINB>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
-        else launch_k(ctx, force_kernel<T, LAYOUT, 0, 0, FB, MINB>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
+        if (ctx->recon == LQCD_RECON_12) launch_k(ctx, force_kernel<T, LAYOUT, 1, 0>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
+        else launch_k(ctx, force_kernel<T, LAYOUT, 0, 0>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
     }
-}
-
-template <typename T, int LAYOUT>
-static void launch_force_tl(lqcd_ctx *ctx, int parity, void *force, const void *links, const ForceVecs &fv)
-{
-    // option force_batch: neighbour vectors in flight per thread (and the matching launch bounds); 0 = default = 1.
-    // Measured at 32^4, 8 shifts (round 2): 1.179 / 1.218 / 1.190 / 1.260 ms for 1 / 2 / 4 / 8 in fp64 and
-    // 0.615 / 0.646 / 0.677 / 0.760 ms in fp32 -- the registers the batch costs lose more occupancy than the
-    // extra loads in flight gain, so one vector per trip stays the default.
-    const int fb = ctx->force_batch ? ctx->force_batch : 1;
-    if (fb == 1) launch_force_tlb<T, LAYOUT, 1, 5>(ctx, parity, force, links, fv);
-    else if (fb == 2) launch_force_tlb<T, LAYOUT, 2, 5>(ctx, parity, force, links, fv);
-    else if (fb == 4) launch_force_tlb<T, LAYOUT, 4, 4>(ctx, parity, force, links, fv);
-    else launch_force_tlb<T, LAYOUT, 8, 3>(ctx, parity, force, links, fv);
 }
 
 extern "C" int lqcd_fermion_force(lqcd_ctx *ctx, int nshift, const double *coeffs, void *const *xs_e,

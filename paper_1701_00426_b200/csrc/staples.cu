@@ -526,6 +526,8 @@ __global__ void __launch_bounds__(128, MINB) staples_final_kernel(const Geom g, 
         const size_t i_n = (size_t)(i + dn_p), i_l = (size_t)(i + dn_m);                       // x + nu, x - nu
         const size_t i_ml = (size_t)((int)i_m + dn_m);                                           // x + mu - nu
         const int qmn = pair_idx(mu, nu), qnm = pair_idx(nu, mu);
+        // (prefetching the next nu's stored staples / links into L2 from here was tried: 2.63 -> 2.68 / 2.83 ns/site at 32^4
+        // fp64 -- the kernel is not waiting for DRAM alone; profiles/sweep_r2.md section 3)
         // c0 Tu_munu(x) = c0 (A B) C and c0 Tl_munu(x) = c0 (A' B') C' are folded into the (A B) products, so the
         // link's own two staple fields are not loaded: 6 matrix loads and 5 products per half.
         {   // above the link
@@ -608,7 +610,7 @@ extern "C" int lqcd_gauge_staples(lqcd_ctx *ctx, const void *links, void *staple
     if (two_pass) {
         dim3 gridp(((ctx->g.Vh + 127) / 128) * 24);
         int minb = ctx->staples_minblocks;           // launch-bounds variant of pass 2 (0: default per precision)
-        if (minb == 0) minb = ctx->prec == LQCD_F64 ? 2 : 3;
+        if (minb == 0) minb = ctx->prec == LQCD_F64 ? 2 : 4;      // measured best: profiles/sweep_r2.md section 3
 #define GO2(T, L, R) do { \
         launch_k(ctx, staples_produce_kernel<T, L, R>, gridp, block, ctx->g, (T *)ctx->ws, (const T *)links); \
         if (minb == 2) launch_k(ctx, staples_final_kernel<T, L, R, 2>, grid, block, ctx->g, (T *)staples, (const T *)links, (const T *)ctx->ws, (T)c0, (T)c1, sw); \
