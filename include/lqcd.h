@@ -391,6 +391,10 @@ int lqcd_cg_multishift_host(lqcd_ctx *ctx, int nshift, const double *shifts,
  * gauge-staples kernel (bench.py extra.fp64_peak_tflops).  tflops: host, out.  blocking.
  */
 int lqcd_measure_fp64_peak(lqcd_ctx *ctx, double *tflops);
+/* Measurement helper: attainable READ bandwidth in GB/s over the caller's device buffer (use one larger than L2, e.g.
+ * the link field): 16-byte streaming loads, nothing written.  MEASURED_PEAKS.json's HBM figure is a copy (half
+ * writes); the Dslash is 96 % reads (bench.py roofline.frac_of_read_rate).  buf: 16-byte aligned, >= 1 MiB.  blocking. */
+int lqcd_measure_hbm_read(lqcd_ctx *ctx, const void *buf_dev, size_t bytes, double *gbs);
 
 #ifdef __cplusplus
 }

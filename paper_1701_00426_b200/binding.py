@@ -91,6 +91,7 @@ _sig = {
     "lqcd_dslash_host_vectors_batch": (_i, [_vp, _i, _pi, C.POINTER(_vp), C.POINTER(_vp), _vp]),
     "lqcd_cg_multishift_host_vectors": (_i, [_vp, _i, _pd, _vp, _vp, _vp, _d, _d, _i, _pi, _pi, _pd]),
     "lqcd_measure_fp64_peak": (_i, [_vp, _pd]),
+    "lqcd_measure_hbm_read": (_i, [_vp, _vp, _sz, _pd]),
 }
 for _name, (_res, _args) in _sig.items():
     _f = getattr(lib, _name)
@@ -442,6 +443,12 @@ class Lattice:
                                                              max_iter, C.byref(iters), conv, res.ctypes.data_as(_pd)),
                          allow=() if raise_on_max_iter else (ERR_NOT_CONVERGED,))
         return dict(iters=iters.value, conv_iter=np.array(list(conv)), rel_resid=res, converged=(rc == OK))
+
+    def measure_hbm_read(self, buf):
+        """attainable read bandwidth in GB/s over a device buffer larger than L2 (measurement helper; blocking)."""
+        v = C.c_double(0.0)
+        self._check(lib.lqcd_measure_hbm_read(self._ctx, _vp(buf.data_ptr()), buf.numel() * buf.element_size(), C.byref(v)))
+        return v.value
 
     def measure_fp64_peak(self):
         """attainable FP64 FMA rate in TFLOP/s (measurement helper; blocking)."""
