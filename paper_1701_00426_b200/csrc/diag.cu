@@ -58,8 +58,19 @@ extern "C" int lqcd_measure_fp64_peak(lqcd_ctx *ctx, double *tflops)
 // copy peak exceeds 1 -- bench.py reports the fraction of this read rate beside it.
 __global__ void __launch_bounds__(256) hbm_read_kernel(const double2 *__restrict__ p, size_t n, double *sink)
 {
+    // 8 independent 16-byte loads in flight per thread (one per trip left the kernel latency-bound below the Dslash's
+    // own rate)
     double s = 0.0;
-    for (size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x; k < n; k += (size_t)gridDim.x * blockDim.x) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    size_t k = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    for (; k + 7 * stride < n; k += 8 * stride) {
+        double2 v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = __ldcs(p + k + u * stride);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) s += v[u].x + v[u].y;
+    }
+    for (; k < n; k += stride) {
         const double2 v = __ldcs(p + k);
         s += v.x + v.y;
     }
