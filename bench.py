@@ -538,6 +538,15 @@ def run_ours(args):
                     for recon, rn in ((L.RECON_18, 18), (L.RECON_12, 12)):
                         extra[f"dslash_{name}_{pname}_{rn}real"] = dslash_rate(torch, L, D, gen, dims_l, Ul, ie, io, prec, recon,
                                                                              peak, device, n=60)
+                    # config 5's CG leg: time per iteration at a fixed iteration count (m = 0.01; eps 0.5 needs thousands
+                    # of iterations to converge), 18-real links
+                    lc = L.Lattice(dims_l, prec=prec, device=local_rank)
+                    ms_it = solver_iter_rate(torch, lc, L, lc.pack_links(Ul), lc.pack_spinor(ie, L.EVEN), [0.0], 0.01, n_lo=12, n_hi=60)
+                    by = CG_BYTES if prec == L.F64 else CG_BYTES // 2
+                    extra[f"cg_{name}_{pname}"] = {"us_per_iter": ms_it * 1e3, "iter_per_s": 1e3 / ms_it, "bytes_per_site_iter": by,
+                                                   "GBs": by * (Vl // 2) / (ms_it * 1e-3) / 1e9,
+                                                   "frac": by * (Vl // 2) / (ms_it * 1e-3) / 1e9 / peak}
+                    lc.close()
             del U48
         # ---- CPU oracle beside it -------------------------------------------------------------
         psi = np.zeros((V, 3), dtype=np.complex128)

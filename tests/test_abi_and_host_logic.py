@@ -180,3 +180,72 @@ def test_replica_plumbing_gloo_world2(tmp_path):
     for r, (p, o) in enumerate(zip(procs, outs)):
         assert p.returncode == 0, o
         assert f"rank {r} ok" in o
+
+
+def test_peer_face_map_matches_the_landing_buffer_layout():
+    """Host re-derivation of peer_store_faces (csrc/solver.cu): packet k0 of the owned range [x3_lo, x3_hi) of plane pl,
+    if it lies in the first / last owned slice, lands at packet pl * slice + (offset inside the slice) of the landing
+    buffer -- which is laid out like a half vector of ONE slice.  Checked against the site indices: every face site
+    of every plane is hit exactly once, and the landing index equals the face index f = idxh - x3 * s3 that the
+    Dslash reads (csrc/dslash.cu, HALO)."""
+    for dims, per in (((4, 4, 2, 6), 2), ((8, 4, 4, 8), 2), ((4, 2, 2, 4), 1)):      # per = reals per site and plane
+        for N in (2, 4):                                                            # reals per packet (fp64 / fp32)
+            n0, n1, n2, n3 = dims
+            s3 = n0 // 2 * n1 * n2
+            if (s3 * per) % N:
+                continue
+            x3_lo, x3_hi = 1, n3 - 1
+            nplanes = 3 if per == 2 else 6
+            length = (x3_hi - x3_lo) * s3 * per // N
+            slice_ = s3 * per // N
+            hit_down, hit_up = set(), set()
+            for k0 in range(nplanes * length):
+                pl, off = divmod(k0, length)
+                real0 = (x3_lo * s3 * per) + off * N                 # first real of the packet inside plane pl
+                site, x3 = real0 // per, (real0 // per) // s3
+                if off < slice_:
+                    assert x3 == x3_lo
+                    land = pl * slice_ + off
+                    assert land * N == pl * s3 * per + (site - x3_lo * s3) * per + real0 % per
+                    hit_down.add(land)
+                if off >= length - slice_:
+                    assert x3 == x3_hi - 1
+                    land = pl * slice_ + (off - (length - slice_))
+                    assert land * N == pl * s3 * per + (site - (x3_hi - 1) * s3) * per + real0 % per
+                    hit_up.add(land)
+            assert hit_down == hit_up == set(range(nplanes * slice_))
+
+
+def test_traffic_json_matches_the_kernel_bench_launches(tmp_path, monkeypatch):
+    """profiles/traffic.json must hold the entry bench.py looks up for the default options (a re-templated kernel
+    without a fresh ncu capture would make bench.py fail on the GPU box), and sweep.traffic_from_ncu must parse an
+    `ncu --page raw --csv` export into that key format."""
+    import json
+    import bench
+    import sweep
+
+    class FakeLat:
+        def get_option(self, name):
+            return {"dslash_minblocks": 0, "layout": 0, "l2_hints": 0}[name]
+
+    class FakeL:
+        F64, F32, RECON_18, RECON_12 = 0, 1, 0, 1
+    name = bench.dslash_kernel_name(FakeLat(), FakeL, FakeL.F64, FakeL.RECON_18)
+    table = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+    assert name in table and table[name]["dram_bytes"] > 6e8
+    assert bench.ncu_traffic(name)["dram_bytes"] == table[name]["dram_bytes"]
+    with pytest.raises(SystemExit):
+        bench.ncu_traffic("dslash_kernel<double,9,9>")
+    # the parser, on a fabricated export, writing into a scratch root
+    (tmp_path / "profiles").mkdir()
+    monkeypatch.setattr(sweep, "ROOT", str(tmp_path))
+    csvp = tmp_path / "raw.csv"
+    csvp.write_text('"ID","Kernel Name","dram__bytes_read.sum","dram__bytes_write.sum","gpu__time_duration.sum"\n'
+                    '"","","Mbyte","Kbyte","us"\n'
+                    '"0","void dslash_kernel<double, 0, 0, 0, 2, 0, 0, 0>(Geom, int, T1 *)","600.5","5000","94.0"\n'
+                    '"1","void dslash_kernel<double, 0, 0, 0, 2, 0, 0, 0>(Geom, int, T1 *)","601.5","7000","96.0"\n')
+    sweep.traffic_from_ncu(str(csvp), "abc1234", "test")
+    got = json.load(open(tmp_path / "profiles" / "traffic.json"))
+    ent = got[name]
+    assert ent["launches_captured"] == 2 and ent["commit"] == "abc1234"
+    assert abs(ent["dram_bytes"] - (601.0e6 + 6.0e6)) < 1 and abs(ent["ncu_duration_us"] - 95.0) < 1e-9
