@@ -312,7 +312,9 @@ int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_parity, lqcd_ha
  * after <r,r>) waits for the P flags and adds the P slots in rank order, so every rank gets the bit-identical
  * total and takes the same decisions.  The waits are inside the kernels: the CG loop stays one CUDA graph per
  * chunk of iterations.  Flags are monotone counters; re-use of slots and landing buffers is ordered by the two
- * all-reduces of every iteration.
+ * all-reduces of every iteration and by the alternation of the two exchange kinds (even / odd input vector); where a
+ * caller exchanges the same kind twice in a row (lqcd_dslash twice for one parity, a solve right after it) the
+ * library puts a device-side barrier (a dummy all-reduce) in between by itself.
  *   lqcd_peer_init      allocate the block; the context must have local extents (N0,N1,N2,L3+2) and antiperiodic_t
  *                       = 0 as described above; x3_lo/x3_hi/solve_parity as in lqcd_set_slab; sign_up / sign_down:
  *                       factor applied to the face sent to the rank above / below (-1 where the hop crosses an

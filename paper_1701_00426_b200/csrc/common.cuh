@@ -268,6 +268,7 @@ struct lqcd_ctx {
     // peer-to-peer transport (lqcd_peer_init / lqcd_peer_connect): library-owned block + landing buffers
     int peer_on;                     // 1 after lqcd_peer_connect: solvers, lqcd_dslash and lqcd_mdagm use it
     int peer_nranks, peer_rank;
+    int peer_last_kind;              // kind of the most recent halo exchange whose reader may still run (-1: none); peer_guard
     double peer_sign_up, peer_sign_down;   // boundary sign applied by the SENDER to the face sent up / down
     void *peer_mem; size_t peer_mem_bytes; // cudaMalloc: PeerBlock + 4 landing buffers
     PeerDev h_peer, *d_peer;
@@ -361,7 +362,8 @@ int launch_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical, const void 
 // landing buffers (the face push fused into the producer)
 int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
                   const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo = -1, int x3_hi = -1, int push_out = 0);
-int peer_after_producer(lqcd_ctx *ctx, int kind, int gate);    // lock-step validation: signal kernel + host hook
+int peer_after_producer(lqcd_ctx *ctx, int kind, int gate);
+int peer_guard(lqcd_ctx *ctx, int kind);     // barrier before two exchanges of the same kind in a row (peer.cu)    // lock-step validation: signal kernel + host hook
 int launch_halo(lqcd_ctx *ctx, int pack, void *buf, void *spinor, int x3, double sign);
 // peer transport (peer.cu): push both faces of `spinor` (a vector of local parity `parity`) to the neighbours
 int launch_peer_push(lqcd_ctx *ctx, const void *spinor, int parity, int gate);

@@ -49,6 +49,7 @@ extern "C" int lqcd_peer_init(lqcd_ctx *ctx, int nranks, int rank, int x3_lo, in
         return lqcd_check_cuda(ctx, e, "lqcd_peer_init");
     }
     ctx->peer_nranks = nranks; ctx->peer_rank = rank;
+    ctx->peer_last_kind = -1;
     ctx->peer_sign_up = sign_up; ctx->peer_sign_down = sign_down;
     ctx->x3_lo = x3_lo; ctx->x3_hi = x3_hi; ctx->solve_parity = solve_parity;
     if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
@@ -209,8 +210,23 @@ int peer_after_producer(lqcd_ctx *ctx, int kind, int gate)
     return rc ? rc : peer_phase(ctx, 0);
 }
 
+// A landing buffer may be rewritten only after the neighbour's Dslash that read its previous content has finished.
+// Inside a solve the two all-reduces of every iteration guarantee that, and exchanges of the two kinds alternate
+// (a rank raises the flag of exchange n+1 of the OTHER kind only after its reader of exchange n has completed).  Two
+// exchanges of the SAME kind in a row with nothing in between -- lqcd_dslash called twice for the same parity, a
+// solve right after such a call -- get a device-side barrier first: one generic all-reduce of a dummy value.
+int peer_guard(lqcd_ctx *ctx, int kind)
+{
+    int rc = LQCD_OK;
+    if (ctx->peer_last_kind == kind) rc = launch_peer_allreduce(ctx, &ctx->d_state->sum[3], 1, 0);
+    ctx->peer_last_kind = kind;
+    return rc;
+}
+
 int launch_peer_push(lqcd_ctx *ctx, const void *spinor, int parity, int gate)
 {
+    int rcg = peer_guard(ctx, parity);
+    if (rcg) return rcg;
     dim3 grid((ctx->g.s3 + 127) / 128, 2), block(128);
 #define CALL(T, L) launch_k(ctx, peer_push_kernel<T, L>, grid, block, ctx->g, (const PeerDev *)ctx->d_peer, parity, (const T *)spinor, \
                             ctx->x3_lo, ctx->x3_hi, (T)ctx->peer_sign_up, (T)ctx->peer_sign_down, (const SolverState *)ctx->d_state, gate)

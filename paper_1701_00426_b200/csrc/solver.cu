@@ -452,6 +452,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     int rc = lqcd_check_cuda(ctx, cudaMemcpyAsync(ctx->d_state, &h, sizeof(h), cudaMemcpyHostToDevice, s), "solver state upload");
     if (rc) return rc;
     const int push_kind = peer ? par : -1;     // peer transport: init and K2 push the faces of p themselves
+    if (peer && (rc = peer_guard(ctx, par))) return rc;
     if (ctx->l2_hints) launch_k(ctx, init_kernel<T, 1>, dim3(g_init), dim3(block), npk, sg, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials, (const PeerDev *)ctx->d_peer, push_kind);
     else launch_k(ctx, init_kernel<T, 0>, dim3(g_init), dim3(block), npk, sg, (const T *)b, r, p, sp, ctx->d_state, ctx->d_partials, (const PeerDev *)ctx->d_peer, push_kind);
     if (peer && (rc = peer_after_producer(ctx, par, 0))) return rc;
@@ -562,6 +563,9 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         if (enq >= max_iter) stop = 1;
         ++chunk_id;
     }
+    // (peer transport: the loop's last exchange -- K2's faces of p -- has no reader: the next K_A is gated off or was
+    // never enqueued; inside the loop the kinds alternate, p / D p / p / ...)
+    if (peer) ctx->peer_last_kind = -1;
     // true residuals || b - (A + sigma_i) x_i || (reading R10), with the same kernels, ungated
     for (int i = 0; i < nshift && !y; ++i) {
         if ((rc = halo(xs[i], par, 0))) return rc;
