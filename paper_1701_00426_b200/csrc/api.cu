@@ -86,6 +86,7 @@ extern "C" int lqcd_create(lqcd_ctx **out, const int dims[4], int prec, int reco
     c->staples_variant = 2;
     c->force_stage = 1;
     c->staples_x2block = 4;
+    c->peer_wait_ms = 3000;
     c->launch_stream = c->stream;
     c->x3_lo = 0;
     c->x3_hi = g.N3;
@@ -139,7 +140,7 @@ struct OptDesc { const char *name; size_t off; long lo, hi; };
 static const OptDesc g_opts[] = {
     OPT(layout, 0, 1), OPT(l2_hints, 0, 1), OPT(l2_persist, 0, 4), OPT(link_pad, 0, 1 << 20), OPT(dslash_block, 32, 256), OPT(dslash_minblocks, 0, 4),
     OPT(blas_block, 64, 256), OPT(blas_ctas_per_sm, 1, 32), OPT(poll_chunk, 1, 1024),
-    OPT(pdl, 0, 1), OPT(graph, 0, 1), OPT(dslash_persist, 0, 16), OPT(iter_mask, 0, 15), OPT(staples_variant, 0, 2), OPT(staples_minblocks, 0, 4), OPT(force_stage, 0, 1), OPT(staples_x2block, 0, 64), OPT(backfield_format, 0, 1),
+    OPT(pdl, 0, 1), OPT(graph, 0, 1), OPT(dslash_persist, 0, 16), OPT(iter_mask, 0, 15), OPT(staples_variant, 0, 2), OPT(staples_minblocks, 0, 4), OPT(peer_wait_ms, 0, 600000), OPT(force_stage, 0, 1), OPT(staples_x2block, 0, 64), OPT(backfield_format, 0, 1),
 };
 
 extern "C" int lqcd_set_option(lqcd_ctx *ctx, const char *name, long value)
@@ -172,6 +173,7 @@ extern "C" long lqcd_get_option(const lqcd_ctx *ctx, const char *name)
     if (!strcmp(name, "launches")) return ctx->launches;
     if (!strcmp(name, "num_sms")) return ctx->num_sms;
     if (!strcmp(name, "graph_active")) return ctx->graph_active;
+    if (!strcmp(name, "peer_timeouts")) return peer_timeouts((lqcd_ctx *)ctx);
     if (!strcmp(name, "staples_ran")) return ctx->staples_ran;
     if (!strcmp(name, "l2_window_bytes")) return ctx->l2_window_bytes;
     if (!strcmp(name, "l2_max_persist")) return ctx->l2_max_persist;

@@ -223,7 +223,9 @@ struct PeerBlock {
     unsigned int flag_halo[2][2];                 // [exchange kind = parity of the pushed vector][0: from down, 1: from up]
     unsigned int flag_red[3][LQCD_MAX_RANKS];     // [0: <p,q>, 1: <r,r>, 2: generic][sender]: the sender's counter
     unsigned int cnt_halo[2], cnt_red[3];         // LOCAL counters (only this rank writes them)
-    unsigned int ticket, pad_[2];
+    unsigned int ticket;
+    unsigned int timeouts;                        // waits of THIS rank that gave up (peer.cuh: a dead or desynchronised peer must not hang the GPU)
+    unsigned int pad_[1];
     double slot[3][2][LQCD_MAX_RANKS][LQCD_MAX_SHIFTS];   // [kind][counter parity][sender][value]
 };
 struct PeerDev {                                  // lives in device memory (ctx->d_peer); kernels get a pointer
@@ -234,6 +236,7 @@ struct PeerDev {                                  // lives in device memory (ctx
     void *land_up[2], *land_down[2];              // [kind]: up neighbour's "from down" buffer, down neighbour's "from up" buffer
     PeerBlock *up, *down;
     double sign_up, sign_down;                    // boundary sign applied by the SENDER to the face sent up / down
+    long long wait_cycles;                        // longest wait for a peer, in SM clock cycles (option peer_wait_ms)
 };
 
 // ------------------------------------------------------------------------------------------
@@ -268,6 +271,8 @@ struct lqcd_ctx {
     // peer-to-peer transport (lqcd_peer_init / lqcd_peer_connect): library-owned block + landing buffers
     int peer_on;                     // 1 after lqcd_peer_connect: solvers, lqcd_dslash and lqcd_mdagm use it
     int peer_nranks, peer_rank;
+    int peer_wait_ms;                // longest wait for a peer (default 3000 ms); takes effect at lqcd_peer_connect
+    long peer_timeouts_seen;         // value of the block's timeout counter the host has already reported
     int peer_last_kind;              // kind of the most recent halo exchange whose reader may still run (-1: none); peer_guard
     double peer_sign_up, peer_sign_down;   // boundary sign applied by the SENDER to the face sent up / down
     void *peer_mem; size_t peer_mem_bytes; // cudaMalloc: PeerBlock + 4 landing buffers
@@ -363,6 +368,7 @@ int launch_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical, const void 
 int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
                   const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo = -1, int x3_hi = -1, int push_out = 0);
 int peer_after_producer(lqcd_ctx *ctx, int kind, int gate);
+long peer_timeouts(lqcd_ctx *ctx);           // waits that gave up (blocking read of the rank's block)
 int peer_guard(lqcd_ctx *ctx, int kind);     // barrier before two exchanges of the same kind in a row (peer.cu)    // lock-step validation: signal kernel + host hook
 int launch_halo(lqcd_ctx *ctx, int pack, void *buf, void *spinor, int x3, double sign);
 // peer transport (peer.cu): push both faces of `spinor` (a vector of local parity `parity`) to the neighbours

@@ -50,6 +50,7 @@ extern "C" int lqcd_peer_init(lqcd_ctx *ctx, int nranks, int rank, int x3_lo, in
     }
     ctx->peer_nranks = nranks; ctx->peer_rank = rank;
     ctx->peer_last_kind = -1;
+    ctx->peer_timeouts_seen = 0;
     ctx->peer_sign_up = sign_up; ctx->peer_sign_down = sign_down;
     ctx->x3_lo = x3_lo; ctx->x3_hi = x3_hi; ctx->solve_parity = solve_parity;
     if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
@@ -77,6 +78,11 @@ extern "C" int lqcd_peer_connect(lqcd_ctx *ctx, void *const *blocks)
     const int up = (me + 1) % P, down = (me + P - 1) % P;
     h.up = h.peer[up]; h.down = h.peer[down];
     h.sign_up = ctx->peer_sign_up; h.sign_down = ctx->peer_sign_down;
+    {
+        int khz = 0;
+        cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, ctx->device);
+        h.wait_cycles = (long long)(ctx->peer_wait_ms > 0 ? ctx->peer_wait_ms : 3000) * (long long)(khz > 0 ? khz : 1900000);
+    }
     for (int k = 0; k < 2; ++k) {
         for (int d = 0; d < 2; ++d) h.land_self[k][d] = land_ptr(ctx, ctx->peer_mem, k, d);
         h.land_up[k] = land_ptr(ctx, h.up, k, 0);       // my top slice is what the rank above receives "from down"
@@ -135,6 +141,19 @@ extern "C" int lqcd_set_phase_hook(lqcd_ctx *ctx, lqcd_phase_fn fn, void *user)
     ctx->phase_fn = fn; ctx->phase_user = user;
     if (ctx->chunk_exec) { cudaGraphExecDestroy(ctx->chunk_exec); ctx->chunk_exec = NULL; }
     return LQCD_OK;
+}
+
+// number of waits of this rank that gave up since lqcd_peer_init (blocking: finishes the stream first); < 0 on error
+long peer_timeouts(lqcd_ctx *ctx)
+{
+    if (!ctx->peer_mem) return 0;
+    unsigned int n = 0;
+    if (cudaStreamSynchronize(ctx->stream) != cudaSuccess ||
+        cudaMemcpy(&n, &((PeerBlock *)ctx->peer_mem)->timeouts, sizeof(n), cudaMemcpyDeviceToHost) != cudaSuccess) {
+        cudaGetLastError();
+        return -1;
+    }
+    return (long)n;
 }
 
 int peer_phase(lqcd_ctx *ctx, int what)

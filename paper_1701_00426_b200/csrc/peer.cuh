@@ -44,6 +44,18 @@ __device__ __forceinline__ double ld_slot(const double *p)
     return v;
 }
 
+// Spin until *f >= n (wrap-safe), but never for more than pd.wait_cycles (option peer_wait_ms, default 3 s): a peer that died or
+// ran a different sequence of calls must not hang this GPU.  A wait that gives up counts itself in the rank's block;
+// the host turns a non-zero count into LQCD_ERR_CUDA at the end of the solve (the results are then meaningless).
+__device__ __forceinline__ void peer_spin(const PeerDev &pd, const unsigned int *f, unsigned int n)
+{
+    if ((int)(ld_flag(f) - n) >= 0) return;
+    const long long t0 = clock64();
+    while ((int)(ld_flag(f) - n) < 0) {
+        if (clock64() - t0 > pd.wait_cycles) { atomicAdd(&pd.self->timeouts, 1u); return; }
+    }
+}
+
 // One thread of the producing kernel: this rank has one more reduction / exchange of `kind` under way.
 __device__ __forceinline__ void peer_bump_red(const PeerDev &pd, int kind) { pd.self->cnt_red[kind] += 1; }
 __device__ __forceinline__ void peer_bump_halo(const PeerDev &pd, int kind) { pd.self->cnt_halo[kind] += 1; }
@@ -65,8 +77,7 @@ __device__ __forceinline__ unsigned int peer_wait_red(const PeerDev &pd, int kin
 {
     const unsigned int n = *(volatile unsigned int *)&pd.self->cnt_red[kind];
     if (threadIdx.x < pd.nranks) {
-        const unsigned int *f = &pd.self->flag_red[kind][threadIdx.x];
-        while ((int)(ld_flag(f) - n) < 0) { }
+        peer_spin(pd, &pd.self->flag_red[kind][threadIdx.x], n);
     }
     __syncthreads();
     return n;
@@ -92,8 +103,7 @@ __device__ __forceinline__ void peer_wait_halo(const PeerDev &pd, int kind)
 {
     const unsigned int n = *(volatile unsigned int *)&pd.self->cnt_halo[kind];
     if (threadIdx.x < 2) {
-        const unsigned int *f = &pd.self->flag_halo[kind][threadIdx.x];
-        while ((int)(ld_flag(f) - n) < 0) { }
+        peer_spin(pd, &pd.self->flag_halo[kind][threadIdx.x], n);
     }
     __syncthreads();
 }

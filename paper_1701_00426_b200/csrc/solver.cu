@@ -589,6 +589,13 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     memcpy(ctx->h_hist[0], h.hist_alpha, sizeof(h.hist_alpha));
     memcpy(ctx->h_hist[1], h.hist_beta, sizeof(h.hist_beta));
     memcpy(ctx->h_hist[2], h.hist_rnorm, sizeof(h.hist_rnorm));
+    if (peer) {      // a wait for a peer gave up (dead or desynchronised rank): the results are meaningless
+        const long nt = peer_timeouts(ctx);
+        if (nt != ctx->peer_timeouts_seen) {
+            ctx->peer_timeouts_seen = nt;
+            return lqcd_fail(ctx, LQCD_ERR_CUDA, "peer transport: %ld waits for other ranks timed out", nt);
+        }
+    }
     if (!converged) return lqcd_fail(ctx, LQCD_ERR_NOT_CONVERGED, "not converged after %d iterations", h.iter);
     return LQCD_OK;
 }

@@ -184,6 +184,29 @@ def test_peer_fp32_cg_max_iter_and_zero_rhs():
     assert np.linalg.norm(b - oracle.mdagm(dims, U, 0.2, got)) / np.linalg.norm(b) < 2e-5
 
 
+def test_peer_wait_gives_up_instead_of_hanging():
+    """A rank whose neighbour never shows up (here: rank 0 of 2 runs alone, with a 50 ms limit) must not hang the GPU:
+    the boundary tiles of its Dslash give up, the count is readable, and a solve returns LQCD_ERR_CUDA."""
+    import paper_1701_00426_b200 as L
+    from paper_1701_00426_b200.slab import SlabLattice
+    dims = (4, 4, 4, 8)
+    rng = np.random.default_rng(75)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    slabs = [SlabLattice(dims, 2, r, transport="peer", options=dict(peer_wait_ms=50)) for r in range(2)]
+    SlabLattice.connect_local(slabs)
+    sl = slabs[0]
+    links, be, out = sl.pack_links(U), sl.pack_spinor(b, 0), sl.new_spinor()
+    assert sl.lat.get_option("peer_timeouts") == 0
+    sl.dslash(1, out, be, links)                      # rank 1 never pushes its faces
+    assert sl.lat.get_option("peer_timeouts") > 0
+    with pytest.raises(L.LqcdError) as e:
+        sl.cg_multishift([sl.new_spinor()], be, links, 0.2, [0.0], 1e-8, 8, raise_on_max_iter=False)
+    assert e.value.code == L.ERR_CUDA and "timed out" in str(e.value)
+    for s in slabs:
+        s.close()
+
+
 def test_peer_errors_and_disconnect():
     import paper_1701_00426_b200 as L
     from paper_1701_00426_b200.slab import SlabLattice
