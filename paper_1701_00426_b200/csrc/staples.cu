@@ -466,6 +466,52 @@ __device__ __forceinline__ Site4 decode_site(const Geom &g, int i, int parity)
     return x;
 }
 
+// Storage of the 48 intermediate fields (24 per parity).  TF_TILED 1: [field][tile of 128 sites][k = 0..8][site in tile] --
+// the nine entries of a matrix of one tile are contiguous (18 KB in fp64), so that a CTA's accesses to one matrix fall
+// into one DRAM page region and the entry offsets are compile-time constants; 0: nine planes of Vh sites per field,
+// like the links.
+#ifndef TF_TILED
+#define TF_TILED 1
+#endif
+__host__ __device__ __forceinline__ size_t tf_sites(size_t Vh) { return TF_TILED ? (Vh + 127) / 128 * 128 : Vh; }
+template <typename T, int LAYOUT>
+__device__ __forceinline__ Su3<T> load_tmat(const T *__restrict__ f, size_t plane0, size_t Vh, size_t i)
+{
+    if (!TF_TILED) return load_mat<T, LAYOUT>(f, plane0, Vh, i);
+    typedef typename Vec2<T>::type V2;
+    const size_t base = ((plane0 / 9) * (tf_sites(Vh) / 128) + (i >> 7)) * (9 * 128) + (i & 127);    // in complex numbers
+    Su3<T> m;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        if (LAYOUT == 0) {
+            const V2 v = __ldg(reinterpret_cast<const V2 *>(f) + base + k * 128);
+            m.e[k / 3][k % 3] = cx<T>(v.x, v.y);
+        } else {
+            const T *p = f + 2 * (base - (i & 127)) + (2 * k) * 128 + (i & 127);
+            m.e[k / 3][k % 3] = cx<T>(__ldg(p), __ldg(p + 128));
+        }
+    }
+    return m;
+}
+template <typename T, int LAYOUT>
+__device__ __forceinline__ void store_tmat(T *__restrict__ f, size_t plane0, size_t Vh, size_t i, const Su3<T> &m)
+{
+    if (!TF_TILED) { store_mat<T, LAYOUT>(f, plane0, Vh, i, m); return; }
+    typedef typename Vec2<T>::type V2;
+    const size_t base = ((plane0 / 9) * (tf_sites(Vh) / 128) + (i >> 7)) * (9 * 128) + (i & 127);
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        const Cx<T> z = m.e[k / 3][k % 3];
+        if (LAYOUT == 0) {
+            V2 v; v.x = z.re; v.y = z.im;
+            reinterpret_cast<V2 *>(f)[base + k * 128] = v;
+        } else {
+            T *p = f + 2 * (base - (i & 127)) + (2 * k) * 128 + (i & 127);
+            p[0] = z.re; p[128] = z.im;
+        }
+    }
+}
+
 // Pass 1.  CTA = 128 consecutive sites of one parity; blockIdx.x = (tile * 2 + parity) * 12 + ordered pair, so
 // that the 24 CTAs that read the links of one tile run together.
 template <typename T, int LAYOUT, int RECON12>
@@ -490,11 +536,11 @@ __global__ void __launch_bounds__(128, 3) staples_produce_kernel(const Geom g, T
     }
     {
         const Su3<T> b = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity, n, Ls, (size_t)i, pol);
-        store_mat<T, LAYOUT>(tf, tfield_plane(parity ^ 1, pair_idx(m, n), 1), Vh, in, mul_op<T, 1, 0>(Q, b));   // Tl_mn(y+n)
+        store_tmat<T, LAYOUT>(tf, tfield_plane(parity ^ 1, pair_idx(m, n), 1), Vh, in, mul_op<T, 1, 0>(Q, b));   // Tl_mn(y+n)
     }
     {
         const Su3<T> c = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity ^ 1, m, Ls, in, pol);
-        store_mat<T, LAYOUT>(tf, tfield_plane(parity, pair_idx(n, m), 0), Vh, (size_t)i, mul_op<T, 0, 1>(c, Q)); // Tu_nm(y)
+        store_tmat<T, LAYOUT>(tf, tfield_plane(parity, pair_idx(n, m), 0), Vh, (size_t)i, mul_op<T, 0, 1>(c, Q)); // Tu_nm(y)
     }
 }
 
@@ -535,17 +581,17 @@ __global__ void __launch_bounds__(128, MINB) staples_final_kernel(const Geom g, 
             const Su3<T> A = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, nu, Ls, i_m, pol);            // U_nu(x+mu)
             Su3<T> W;
             {
-                const Su3<T> T1 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qnm, 0), Vh, i_m);             // Tu_numu(x+mu)
+                const Su3<T> T1 = load_tmat<T, LAYOUT>(tf, tfield_plane(po, qnm, 0), Vh, i_m);             // Tu_numu(x+mu)
                 W = mul_op<T, 1, 1>(T1, Ub);                                                                // T1^+ B
             }
             {
-                const Su3<T> T2 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qmn, 0), Vh, i_n);             // Tu_munu(x+nu)
+                const Su3<T> T2 = load_tmat<T, LAYOUT>(tf, tfield_plane(po, qmn, 0), Vh, i_n);             // Tu_munu(x+nu)
                 acc_op<T, 0>(W, (T)1, mul_op<T, 0, 0>(A, T2));
             }
             const Su3<T> AB = mul_op<T, 0, 1>(A, Ub);
             const Su3<T> Uc = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity, nu, Ls, (size_t)i, pol); // U_nu(x)
             {
-                Su3<T> X = load_mat<T, LAYOUT>(tf, tfield_plane(parity, qnm, 1), Vh, (size_t)i);          // Tl_numu(x)
+                Su3<T> X = load_tmat<T, LAYOUT>(tf, tfield_plane(parity, qnm, 1), Vh, (size_t)i);          // Tl_numu(x)
                 scale_acc_op<T, 1>(X, c1, c0, Uc);                                                          // c1 T3 + c0 C
                 acc_op<T, 0>(S, (T)1, mul_op<T, 0, 0>(AB, X));
             }
@@ -556,17 +602,17 @@ __global__ void __launch_bounds__(128, MINB) staples_final_kernel(const Geom g, 
             const Su3<T> Ua = load_link<T, LAYOUT, RECON12, 0, 0>(links, parity, nu, Ls, i_ml, pol);      // U_nu(x+mu-nu)
             Su3<T> W;
             {
-                const Su3<T> T1 = load_mat<T, LAYOUT>(tf, tfield_plane(parity, qnm, 0), Vh, i_ml);        // Tu_numu(x+mu-nu)
+                const Su3<T> T1 = load_tmat<T, LAYOUT>(tf, tfield_plane(parity, qnm, 0), Vh, i_ml);        // Tu_numu(x+mu-nu)
                 W = mul_op<T, 0, 1>(T1, Ub);
             }
             {
-                const Su3<T> T2 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qmn, 1), Vh, i_l);             // Tl_munu(x-nu)
+                const Su3<T> T2 = load_tmat<T, LAYOUT>(tf, tfield_plane(po, qmn, 1), Vh, i_l);             // Tl_munu(x-nu)
                 acc_op<T, 0>(W, (T)1, mul_op<T, 1, 0>(Ua, T2));
             }
             const Su3<T> AB = mul_op<T, 1, 1>(Ua, Ub);
             const Su3<T> Uc = load_link<T, LAYOUT, RECON12, 0, 0>(links, po, nu, Ls, i_l, pol);           // U_nu(x-nu)
             {
-                const Su3<T> T3 = load_mat<T, LAYOUT>(tf, tfield_plane(po, qnm, 1), Vh, i_l);             // Tl_numu(x-nu)
+                const Su3<T> T3 = load_tmat<T, LAYOUT>(tf, tfield_plane(po, qnm, 1), Vh, i_l);             // Tl_numu(x-nu)
                 Su3<T> X;                                                                                   // c1 T3^+ + c0 C'
 #pragma unroll
                 for (int a = 0; a < 3; ++a)
@@ -583,7 +629,7 @@ __global__ void __launch_bounds__(128, MINB) staples_final_kernel(const Geom g, 
 
 extern "C" size_t lqcd_staples_workspace_bytes(const lqcd_ctx *ctx)
 {
-    return ctx ? (size_t)ctx->g.Vh * 2 * 24 * 9 * 2 * elem_size(ctx) : 0;
+    return ctx ? tf_sites((size_t)ctx->g.Vh) * 2 * 24 * 9 * 2 * elem_size(ctx) : 0;
 }
 
 extern "C" int lqcd_gauge_staples(lqcd_ctx *ctx, const void *links, void *staples, double c0, double c1)
