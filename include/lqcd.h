@@ -328,7 +328,8 @@ int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_parity, lqcd_ha
  *                       lqcd_dslash_slices stays raw (reads the vector's own ghost slices).
  *   lqcd_peer_disconnect  back to a single-rank context (frees the block, closes imported mappings).  blocking.
  * All ranks must issue the same sequence of calls (as with any collective).  With nranks = 1 the rank is its own
- * neighbour.  A backfield, lqcd_fermion_force and lqcd_gauge_staples are LQCD_ERR_UNSUPPORTED in this mode.
+ * neighbour.  A backfield works as on one GPU (the slab's phases include the ghost slices, like its links);
+ * lqcd_fermion_force and lqcd_gauge_staples are LQCD_ERR_UNSUPPORTED in this mode.
  * A wait for another rank never lasts longer than a few seconds of SM clock: a wait that gives up is counted in the
  * rank's block, the solver calls then return LQCD_ERR_CUDA ("... waits for other ranks timed out"; the results are
  * meaningless), and lqcd_get_option(ctx, "peer_timeouts") reads the count (blocking) after lqcd_dslash / lqcd_mdagm.

@@ -139,8 +139,11 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
             {
                 Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, parity, mu, (size_t)g.Ls, (size_t)i, pol);
                 Cx<T> p[3];
-                if (HALO && mu == 3 && nf[3] >= i_end)
-                    load_vec_cg<T, LAYOUT>((const T *)pdp->land_self[1 - parity][1], (size_t)g.s3, (size_t)(nf[3] - i_end), cf[3], p);
+                if (HALO && mu == 3 && nf[3] >= i_end) {
+                    T cr, ci;
+                    phase_coef<T, BF>(bf, (size_t)(parity * 4 + 3) * Vh + i, cf[3], (T)1, &cr, &ci);
+                    load_vec_cg<T, LAYOUT>((const T *)pdp->land_self[1 - parity][1], (size_t)g.s3, (size_t)(nf[3] - i_end), cr, ci, p);
+                }
                 else if (BF == 1) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], __ldcs(bf + (size_t)(parity * 4 + mu) * Vh + i), p, pol);
                 else if (BF == 2) load_vec_unit<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], (T)1, bf, (size_t)(parity * 4 + mu) * Vh + i, p, pol);
                 else load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nf[mu], cf[mu], p, pol);
@@ -149,8 +152,11 @@ dslash_kernel(const Geom g, const int parity, T *__restrict__ out, const T *__re
             {
                 Su3<T> u = load_link<T, LAYOUT, RECON12, POLICY>(links, 1 - parity, mu, (size_t)g.Ls, (size_t)nb[mu], pol);
                 Cx<T> p[3];
-                if (HALO && mu == 3 && nb[3] < i_begin)
-                    load_vec_cg<T, LAYOUT>((const T *)pdp->land_self[1 - parity][0], (size_t)g.s3, (size_t)(nb[3] - (i_begin - g.s3)), cb[3], p);
+                if (HALO && mu == 3 && nb[3] < i_begin) {
+                    T cr, ci;
+                    phase_coef<T, BF>(bf, (size_t)((1 - parity) * 4 + 3) * Vh + nb[3], cb[3], (T)-1, &cr, &ci);
+                    load_vec_cg<T, LAYOUT>((const T *)pdp->land_self[1 - parity][0], (size_t)g.s3, (size_t)(nb[3] - (i_begin - g.s3)), cr, ci, p);
+                }
                 else if (BF == 1) load_vec_phase<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], -__ldcs(bf + (size_t)((1 - parity) * 4 + mu) * Vh + nb[mu]), p, pol);
                 else if (BF == 2) load_vec_unit<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], (T)-1, bf, (size_t)((1 - parity) * 4 + mu) * Vh + nb[mu], p, pol);
                 else load_vec<T, LAYOUT, POLICY>(in, Vh, (size_t)nb[mu], cb[mu], p, pol);
@@ -220,7 +226,11 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
         (const T *)ctx->backfield, (const PeerDev *)ctx->d_peer, push_out)
 #define GO(MB) do { if (ctx->l2_hints) GO1(MB, 1, 0); else GO1(MB, 0, 0); } while (0)
     // peer transport: the per-precision default variant, faces read from the landing buffers (halo_in)
-    if (halo_in) { if (sizeof(T) == 8) GO2(2, 0, 0, 1); else GO2(4, 0, 0, 1); } else
+    if (halo_in) {
+        const int b = ctx->backfield ? 1 + ctx->backfield_format : 0;
+        if (sizeof(T) == 8) { if (b == 0) GO2(2, 0, 0, 1); else if (b == 1) GO2(2, 0, 1, 1); else GO2(2, 0, 2, 1); }
+        else { if (b == 0) GO2(4, 0, 0, 1); else if (b == 1) GO2(4, 0, 1, 1); else GO2(4, 0, 2, 1); }
+    } else
     // with a backfield: the per-precision default variant only (the tuning options dslash_minblocks and
     // l2_hints select nothing there)
     if (ctx->backfield && ctx->backfield_format == 0) { if (sizeof(T) == 8) GO1(2, 0, 1); else GO1(4, 0, 1); }
@@ -248,7 +258,6 @@ int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const vo
     // peer transport: a Dslash over the context's owned slices reads the faces the neighbours pushed; an explicit
     // slice range (lqcd_dslash_slices) reads the vector's own ghost slices as before
     const int halo_in = ctx->peer_on && x3_lo < 0;
-    if (halo_in && ctx->backfield) return lqcd_fail(ctx, LQCD_ERR_UNSUPPORTED, "a backfield is not available over the peer transport");
     if (x3_lo < 0) { x3_lo = ctx->x3_lo; x3_hi = ctx->x3_hi; }      // the context's interior slices
     const int i_begin = x3_lo * ctx->g.s3, i_end = x3_hi * ctx->g.s3;
     if (ctx->prec == LQCD_F64) {

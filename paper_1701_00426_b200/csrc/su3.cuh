@@ -74,17 +74,30 @@ __device__ __forceinline__ void load_vec_unit(const T *__restrict__ v, size_t Vh
 }
 // a face vector from a landing buffer of the peer transport (peer.cuh): written by another GPU during this kernel's
 // lifetime (before its flag), so it is read through L2 (ld.global.cg), never through the non-coherent path
+// (cr, ci): the hop's coefficient times the backfield phase (ci = 0 without a backfield)
 template <typename T, int LAYOUT>
-__device__ __forceinline__ void load_vec_cg(const T *__restrict__ buf, size_t stride, size_t f, T coef, Cx<T> p[3])
+__device__ __forceinline__ void load_vec_cg(const T *__restrict__ buf, size_t stride, size_t f, T cr, T ci, Cx<T> p[3])
 {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
+        T re, im;
         if (LAYOUT == 0) {
             typedef typename Vec2<T>::type V2;
             const V2 v = __ldcg(reinterpret_cast<const V2 *>(buf) + (size_t)c * stride + f);
-            p[c] = cx<T>(coef * v.x, coef * v.y);
+            re = v.x; im = v.y;
         } else {
-            p[c] = cx<T>(coef * __ldcg(buf + (size_t)(2 * c) * stride + f), coef * __ldcg(buf + (size_t)(2 * c + 1) * stride + f));
+            re = __ldcg(buf + (size_t)(2 * c) * stride + f); im = __ldcg(buf + (size_t)(2 * c + 1) * stride + f);
         }
+        p[c] = cx<T>(cr * re - ci * im, cr * im + ci * re);
     }
+}
+// coef * e^{+-i theta} of link k of the native backfield (BF 1: theta stored, BF 2: (cos, sin) stored; conj = -1: e^{-i theta})
+template <typename T, int BF>
+__device__ __forceinline__ void phase_coef(const T *__restrict__ bf, size_t k, T coef, T conj, T *cr, T *ci)
+{
+    if (BF == 0) { *cr = coef; *ci = (T)0; return; }
+    T sn, cs;
+    if (BF == 1) sincos_t(__ldcs(bf + k), &sn, &cs);
+    else { cs = __ldcs(bf + 2 * k); sn = __ldcs(bf + 2 * k + 1); }
+    *cr = coef * cs; *ci = coef * conj * sn;
 }

@@ -226,6 +226,12 @@ class SlabLattice:
         the backward x3 hop of the first owned slice reads U_3 of the slice below)."""
         return self.lat.pack_links(np.ascontiguousarray(self.geo.extract_full(U_global)))
 
+    def pack_backfield(self, theta_global):
+        """Global phases theta[V][4] -> this rank's native backfield (ghost slices included, like the links: the
+        backward x3 hop of the first owned slice carries the phase of the link in the slice below).  Attach it with
+        self.lat.set_backfield(...); both transports."""
+        return self.lat.pack_backfield(np.ascontiguousarray(self.geo.extract_full(theta_global)))
+
     def pack_spinor(self, phi_global, global_parity):
         """Global half vector -> native local vector; the ghost slices start out ZERO (they are
         filled by the halo exchange, never by the host)."""

@@ -184,6 +184,53 @@ def test_peer_fp32_cg_max_iter_and_zero_rhs():
     assert np.linalg.norm(b - oracle.mdagm(dims, U, 0.2, got)) / np.linalg.norm(b) < 2e-5
 
 
+@pytest.mark.parametrize("fmt", [0, 1])
+@pytest.mark.parametrize("world", [1, 2])
+def test_peer_backfield_dslash_and_solve(world, fmt):
+    """The backfield over the peer transport: the hops that leave the slab take their phase from the slab's own
+    (ghost-inclusive) phase field and their vector from the landing buffers."""
+    from paper_1701_00426_b200.slab import SlabLattice
+    dims = (8, 6, 4, 8)
+    rng = np.random.default_rng(76)
+    U = gen.smooth_links(dims, 0.3, rng)
+    psi = gen.gaussian_spinor(dims, rng)
+    theta = gen.uniform_backfield(dims, rng)
+    shifts = gen.rhmc_shifts(3)
+    b = oracle.full_to_half(dims, 0, psi)
+    ref = oracle.cg_multishift(dims, U, 0.1, shifts, b, 1e-10, 4000, theta=theta)
+    got = {0: np.zeros_like(b), 1: np.zeros_like(b)}
+    got_x = [np.zeros_like(b) for _ in shifts]
+    lock = threading.Lock()
+
+    def work(r, sl):
+        links = sl.pack_links(U)
+        sl.lat.set_backfield(sl.pack_backfield(theta))
+        outs = {}
+        for gp in (1, 0):
+            inp = sl.pack_spinor(oracle.full_to_half(dims, 1 - gp, psi), 1 - gp)
+            outs[gp] = sl.new_spinor()
+            sl.dslash(gp, outs[gp], inp, links)
+        be = sl.pack_spinor(b, 0)
+        xs = [sl.new_spinor() for _ in shifts]
+        res = sl.cg_multishift(xs, be, links, 0.1, shifts, 1e-10, 4000)
+        with lock:
+            for gp in (0, 1):
+                sl.unpack_spinor(outs[gp], gp, got[gp])
+            for i, x in enumerate(xs):
+                sl.unpack_spinor(x, 0, got_x[i])
+        return res
+
+    outs = run_peer_ranks(world, lambda r: SlabLattice(dims, world, r, transport="peer", options=dict(backfield_format=fmt)), work)
+    for gp in (0, 1):
+        want = oracle.dslash_half(dims, U, gp, oracle.full_to_half(dims, 1 - gp, psi), theta=theta)
+        assert rel(got[gp], want) < 1e-12, (world, fmt, gp)
+    for res in outs:
+        assert abs(res["iters"] - ref["iters"]) <= 2
+    for i, s in enumerate(shifts):
+        tr = np.linalg.norm(b - oracle.mdagm(dims, U, 0.1, got_x[i], sigma=s, theta=theta)) / np.linalg.norm(b)
+        assert tr < 1.5e-10, (i, tr)
+
+
 def test_peer_wait_gives_up_instead_of_hanging():
     """A rank whose neighbour never shows up (here: rank 0 of 2 runs alone, with a 50 ms limit) must not hang the GPU:
     the boundary tiles of its Dslash give up, the count is readable, and a solve returns LQCD_ERR_CUDA."""

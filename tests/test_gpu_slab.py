@@ -176,6 +176,49 @@ def test_slab_mdagm_and_multishift_cg(world):
     assert rel(got_y, y_ref) < bound
 
 
+@pytest.mark.parametrize("world", [1, 2])
+def test_slab_dslash_and_solve_with_backfield(world):
+    """The backfield in slab mode (hook transport): every rank packs the phases of its slab incl. the ghost slices,
+    like the links.  Dslash = global oracle with phases; a multi-shift solve by R16 with the oracle's phased operator."""
+    from paper_1701_00426_b200.slab import SlabLattice
+    dims = (8, 6, 4, 8)
+    rng = np.random.default_rng(33)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    theta = gen.uniform_backfield(dims, rng)
+    shifts = gen.rhmc_shifts(3)
+    want = oracle.dslash_half(dims, U, 1, b, theta=theta)
+    ref = oracle.cg_multishift(dims, U, 0.1, shifts, b, 1e-10, 4000, theta=theta)
+    got = np.zeros_like(want)
+    got_x = [np.zeros_like(b) for _ in shifts]
+    lock = threading.Lock()
+
+    def rank_fn(r, comm):
+        sl = SlabLattice(dims, world, r, comm=comm)
+        links = sl.pack_links(U)
+        sl.lat.set_backfield(sl.pack_backfield(theta))
+        be = sl.pack_spinor(b, 0)
+        out = sl.new_spinor()
+        sl.dslash(1, out, be, links)
+        xs = [sl.new_spinor() for _ in shifts]
+        res = sl.cg_multishift(xs, be, links, 0.1, shifts, 1e-10, 4000)
+        with lock:
+            sl.unpack_spinor(out, 1, got)
+            for i, x in enumerate(xs):
+                sl.unpack_spinor(x, 0, got_x[i])
+        sl.close()
+        return res
+
+    outs = run_ranks(world, rank_fn)
+    assert rel(got, want) < 1e-12
+    assert rel(oracle.dslash_half(dims, U, 1, b), want) > 0.1
+    for res in outs:
+        assert abs(res["iters"] - ref["iters"]) <= 2
+    for i, s in enumerate(shifts):
+        tr = np.linalg.norm(b - oracle.mdagm(dims, U, 0.1, got_x[i], sigma=s, theta=theta)) / np.linalg.norm(b)
+        assert tr < 1.5e-10, (i, tr)
+
+
 @pytest.mark.parametrize("prec", [0, 1])
 @pytest.mark.parametrize("layout", [0, 1])
 def test_single_face_halo_calls(prec, layout):
