@@ -348,6 +348,13 @@ int lqcd_peer_import(lqcd_ctx *ctx, int rank, const void *handle64, void **block
 int lqcd_peer_connect(lqcd_ctx *ctx, void *const *blocks);
 int lqcd_peer_disconnect(lqcd_ctx *ctx);
 int lqcd_set_phase_hook(lqcd_ctx *ctx, lqcd_phase_fn fn, void *user);
+/* Protocol self-test under real concurrency on ONE GPU: one cooperative kernel whose CTA r plays rank r of `nranks` on its
+ * own block -- the flags, slots and counters of the transport with ranks that really run at the same time, at uneven pace,
+ * and really wait for one another -- for `rounds` iterations of (halo exchange, two all-reduces).  *failures = wrong
+ * tokens / sums / waits that gave up (0 = pass).  sabotage = 1 makes the consumers skip their waits: the count must then
+ * be non-zero for more than a few ranks (the check that the test can fail).  Allocates and frees its own scratch memory;
+ * independent of lqcd_peer_init.  blocking. */
+int lqcd_peer_selftest(lqcd_ctx *ctx, int nranks, int rounds, int sabotage, int *failures);
 
 /*
  * After lqcd_cg / lqcd_cg_multishift: copy up to `n` entries of the per-iteration history

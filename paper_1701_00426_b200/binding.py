@@ -84,6 +84,7 @@ _sig = {
     "lqcd_peer_connect": (_i, [_vp, C.POINTER(_vp)]),
     "lqcd_peer_disconnect": (_i, [_vp]),
     "lqcd_set_phase_hook": (_i, [_vp, PHASE_FN, _vp]),
+    "lqcd_peer_selftest": (_i, [_vp, _i, _i, _i, _pi]),
     "lqcd_solver_history": (_i, [_vp, _i, _pd, _pd, _pd]),
     "lqcd_dslash_host": (_i, [_vp, _i, _vp, _vp, _vp]),
     "lqcd_dslash_host_vectors": (_i, [_vp, _i, _vp, _vp, _vp]),
@@ -298,6 +299,12 @@ class Lattice:
 
     def peer_disconnect(self):
         self._check(lib.lqcd_peer_disconnect(self._ctx))
+
+    def peer_selftest(self, nranks, rounds, sabotage=False):
+        """protocol self-test under real concurrency (one cooperative kernel, CTA r = rank r); returns failures."""
+        f = C.c_int(-1)
+        self._check(lib.lqcd_peer_selftest(self._ctx, nranks, rounds, int(bool(sabotage)), C.byref(f)))
+        return f.value
 
     def set_phase_hook(self, cb=None):
         """cb: a PHASE_FN instance (kept alive here) or None."""

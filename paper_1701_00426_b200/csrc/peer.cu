@@ -287,3 +287,109 @@ int launch_peer_allreduce(lqcd_ctx *ctx, double *vals, int nv, int which)
     launch_k(ctx, peer_gather_kernel, dim3(1), dim3(32), (const PeerDev *)ctx->d_peer, vals, nv, ctx->d_state, which);
     return lqcd_check_cuda(ctx, cudaGetLastError(), "peer gather");
 }
+
+// ---- protocol self-test under REAL concurrency on one GPU -----------------------------------------------------
+// The virtual-rank tests run the ranks in lock step (no kernel may wait for another LAUNCH on one GPU).  What they cannot
+// show -- the flag / slot / counter protocol of peer.cuh with ranks that really run at the same time and really wait for
+// one another -- is exercised here the way B200_PROFILING.md prescribes: ONE cooperative kernel whose CTA r plays rank r
+// on its own PeerBlock (co-residency is guaranteed by the cooperative launch).  Per round, as in a CG iteration:
+//   a "producer" phase   bump the counters, store a token into the two neighbours' landing buffers (kind = round & 1)
+//   signal + wait_halo   then check the two tokens that arrived
+//   publish + wait_red   (kind 0, then kind 1) and check the rank-ordered sum against the closed form
+// with deliberately uneven delays per rank and round so that fast ranks run ahead as far as the protocol lets them.
+// Any mismatch or timeout is counted.
+__global__ void __launch_bounds__(128) peer_selftest_kernel(const PeerDev *pds, int rounds, unsigned int *failures, int sabotage)
+{
+    const PeerDev &pd = pds[blockIdx.x];
+    const int P = pd.nranks, me = pd.rank, up = (me + 1) % P, down = (me + P - 1) % P;
+    for (int t = 0; t < rounds; ++t) {
+        // uneven pace: a rank- and round-dependent spin before each phase
+        const long long pause = 200LL * ((me * 7 + t * 13) % 11);
+        const long long t0 = clock64();
+        while (clock64() - t0 < pause) { }
+        const int kind = t & 1;
+        if (threadIdx.x == 0) {
+            // producer: faces = one token per direction (what a push kernel / fused push stores), then the counter
+            reinterpret_cast<volatile double *>(pd.land_up[kind])[0] = 1000.0 * t + me;          // to the rank above, "from down"
+            reinterpret_cast<volatile double *>(pd.land_down[kind])[0] = -(1000.0 * t + me);     // to the rank below, "from up"
+            __threadfence_system();     // stands for the kernel boundary between producer and consumer
+            peer_bump_halo(pd, kind);
+            peer_signal_halo(pd, kind);
+        }
+        __syncthreads();
+        if (!sabotage) peer_wait_halo(pd, kind);      // sabotage: the consumers do not wait -- the test must then FAIL
+        if (threadIdx.x == 0) {
+            const double a = __ldcg(reinterpret_cast<const double *>(pd.land_self[kind][0]));
+            const double b = __ldcg(reinterpret_cast<const double *>(pd.land_self[kind][1]));
+            if (a != 1000.0 * t + down) atomicAdd(failures, 1u);
+            if (b != -(1000.0 * t + up)) atomicAdd(failures, 1u);
+        }
+        for (int k = 0; k < 2; ++k) {            // the two all-reduces of an iteration
+            if (threadIdx.x == 0) {
+                const double v = (double)((me + 1) * (t + 1) + k);
+                peer_bump_red(pd, k);
+                peer_publish(pd, k, &v, 1);
+            }
+            __syncthreads();
+            const unsigned int n = sabotage ? *(volatile unsigned int *)&pd.self->cnt_red[k] : peer_wait_red(pd, k);
+            const double s = peer_sum(pd, k, n, 0);
+            const double want = (double)((t + 1) * (P * (P + 1) / 2) + k * P);
+            if (threadIdx.x == 0 && s != want) atomicAdd(failures, 1u);
+            __syncthreads();
+        }
+    }
+    if (threadIdx.x == 0 && pd.self->timeouts) atomicAdd(failures, pd.self->timeouts);
+}
+
+extern "C" int lqcd_peer_selftest(lqcd_ctx *ctx, int nranks, int rounds, int sabotage, int *failures)
+{
+    if (!ctx) return LQCD_ERR_ARG;
+    int rc = lqcd_check_cuda(ctx, cudaSetDevice(ctx->device), "cudaSetDevice");
+    if (rc) return rc;
+    if (nranks < 1 || nranks > LQCD_MAX_RANKS || rounds < 1 || !failures)
+        return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_peer_selftest: 1 <= nranks <= %d, rounds >= 1, failures != NULL", LQCD_MAX_RANKS);
+    int coop = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device);
+    if (!coop) return lqcd_fail(ctx, LQCD_ERR_UNSUPPORTED, "lqcd_peer_selftest: no cooperative launch on this device");
+    const size_t blk = align256(sizeof(PeerBlock)) + 4 * 256;       // one 256-byte "landing buffer" per (kind, direction)
+    char *mem = NULL;
+    PeerDev *d_pds = NULL;
+    unsigned int *d_fail = NULL;
+    cudaError_t e;
+    if ((e = cudaMalloc(&mem, blk * nranks)) != cudaSuccess || (e = cudaMalloc(&d_pds, sizeof(PeerDev) * nranks)) != cudaSuccess ||
+        (e = cudaMalloc(&d_fail, sizeof(unsigned int))) != cudaSuccess || (e = cudaMemset(mem, 0, blk * nranks)) != cudaSuccess ||
+        (e = cudaMemset(d_fail, 0, sizeof(unsigned int))) != cudaSuccess) {
+        cudaFree(mem); cudaFree(d_pds); cudaFree(d_fail);
+        return lqcd_check_cuda(ctx, e, "lqcd_peer_selftest");
+    }
+    PeerDev h[LQCD_MAX_RANKS];
+    memset(h, 0, sizeof(h));
+    int khz = 0;
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, ctx->device);
+    for (int r = 0; r < nranks; ++r) {
+        PeerDev &p = h[r];
+        p.nranks = nranks; p.rank = r;
+        p.self = (PeerBlock *)(mem + blk * r);
+        for (int q = 0; q < nranks; ++q) p.peer[q] = (PeerBlock *)(mem + blk * q);
+        p.up = p.peer[(r + 1) % nranks]; p.down = p.peer[(r + nranks - 1) % nranks];
+        p.sign_up = p.sign_down = 1.0;
+        p.wait_cycles = 3000LL * (khz > 0 ? khz : 1900000);
+        for (int k = 0; k < 2; ++k) {
+            for (int d = 0; d < 2; ++d) p.land_self[k][d] = (char *)p.self + align256(sizeof(PeerBlock)) + (k * 2 + d) * 256;
+            p.land_up[k] = (char *)p.up + align256(sizeof(PeerBlock)) + (k * 2 + 0) * 256;
+            p.land_down[k] = (char *)p.down + align256(sizeof(PeerBlock)) + (k * 2 + 1) * 256;
+        }
+    }
+    unsigned int hf = 0;
+    const PeerDev *arg_pds = d_pds;
+    void *args[] = { (void *)&arg_pds, (void *)&rounds, (void *)&d_fail, (void *)&sabotage };
+    if ((e = cudaMemcpy(d_pds, h, sizeof(PeerDev) * nranks, cudaMemcpyHostToDevice)) == cudaSuccess &&
+        (e = cudaLaunchCooperativeKernel((const void *)peer_selftest_kernel, dim3(nranks), dim3(128), args, 0, ctx->stream)) == cudaSuccess &&
+        (e = cudaStreamSynchronize(ctx->stream)) == cudaSuccess)
+        e = cudaMemcpy(&hf, d_fail, sizeof(hf), cudaMemcpyDeviceToHost);
+    ctx->launches++;
+    cudaFree(mem); cudaFree(d_pds); cudaFree(d_fail);
+    if (e != cudaSuccess) return lqcd_check_cuda(ctx, e, "lqcd_peer_selftest");
+    *failures = (int)hf;
+    return LQCD_OK;
+}

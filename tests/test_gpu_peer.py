@@ -231,6 +231,19 @@ def test_peer_backfield_dslash_and_solve(world, fmt):
         assert tr < 1.5e-10, (i, tr)
 
 
+@pytest.mark.parametrize("nranks", [1, 2, 3, 8, 16])
+def test_peer_protocol_selftest_under_real_concurrency(nranks):
+    """lqcd_peer_selftest: the flags / slots / counters of the transport with ranks that run AT THE SAME TIME (one
+    cooperative kernel, CTA r = rank r, uneven pace) and really wait for one another: 2000 rounds of (halo exchange,
+    two all-reduces), every token and every rank-ordered sum checked on the device."""
+    import paper_1701_00426_b200 as L
+    lat = L.Lattice((4, 4, 4, 4))
+    assert lat.peer_selftest(nranks, 2000) == 0
+    if nranks > 2:        # the test can fail: consumers that do not wait read stale tokens / incomplete sums
+        assert lat.peer_selftest(nranks, 2000, sabotage=True) > 0
+    lat.close()
+
+
 def test_peer_wait_gives_up_instead_of_hanging():
     """A rank whose neighbour never shows up (here: rank 0 of 2 runs alone, with a 50 ms limit) must not hang the GPU:
     the boundary tiles of its Dslash give up, the count is readable, and a solve returns LQCD_ERR_CUDA."""
