@@ -25,7 +25,8 @@
  *   - "dev" pointers are CUDA device pointers on the context's device, >= 16-byte aligned,
  *     owned by the caller (e.g. torch.empty(...).data_ptr()).  The library never allocates or
  *     frees field memory; it owns only the context (host struct, < 64 KiB of device scalars,
- *     one pinned flag word).  "host" pointers are ordinary host memory (pinned or not).
+ *     one pinned flag word), the staging buffers of the *_host* calls and, in slab mode over the
+ *     peer transport, the rank's communication block (flags, slots, four face-sized landing buffers).  "host" pointers are ordinary host memory (pinned or not).
  *   - All device work is enqueued on the CUDA stream given to lqcd_create.  Functions marked
  *     "async" return after enqueueing; functions marked "blocking" synchronise that stream.
  *   - out/in buffers of one call must not alias unless stated.
