@@ -215,7 +215,9 @@ int lqcd_rational_apply(lqcd_ctx *ctx, int nshift, const double *shifts, double 
  *            stored as 8 reals per link -- the paper's tamat_soa: F01, F02, F12 and
  *            (Im F00, Im F11); layout private, read it back with lqcd_unpack_tamat
  * The y_i are computed inside (nshift Dslash applications into the workspace of
- * lqcd_workspace_bytes(ctx, nshift)).  async.  LQCD_ERR_UNSUPPORTED in slab mode.
+ * lqcd_workspace_bytes(ctx, nshift)).  async.  In slab mode (either transport) xs_e are vectors of the context's
+ * solve_parity, the ghost slices of the x_i and y_i are filled by halo exchanges inside the call (those of the caller's
+ * x_i are overwritten), and only the owned links of `force` are written.
  */
 size_t lqcd_tamat_bytes(const lqcd_ctx *ctx); /* 8-real traceless anti-Hermitian field (fermion force)  */
 size_t lqcd_force_bytes(const lqcd_ctx *ctx); /* generic 3x3-complex-per-link field (gauge staples)          */
@@ -330,7 +332,8 @@ int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_parity, lqcd_ha
  *   lqcd_peer_disconnect  back to a single-rank context (frees the block, closes imported mappings).  blocking.
  * All ranks must issue the same sequence of calls (as with any collective).  With nranks = 1 the rank is its own
  * neighbour.  A backfield works as on one GPU (the slab's phases include the ghost slices, like its links);
- * lqcd_fermion_force and lqcd_gauge_staples are LQCD_ERR_UNSUPPORTED in this mode.
+ * lqcd_fermion_force works too (faces pushed and then pulled into the vectors' ghost slices);
+ * lqcd_gauge_staples is LQCD_ERR_UNSUPPORTED in this mode (it would need ghost depth 2).
  * A wait for another rank never lasts longer than a few seconds of SM clock: a wait that gives up is counted in the
  * rank's block, the solver calls then return LQCD_ERR_CUDA ("... waits for other ranks timed out"; the results are
  * meaningless), and lqcd_get_option(ctx, "peer_timeouts") reads the count (blocking) after lqcd_dslash / lqcd_mdagm.

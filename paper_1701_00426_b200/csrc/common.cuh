@@ -373,6 +373,7 @@ int peer_guard(lqcd_ctx *ctx, int kind);     // barrier before two exchanges of 
 int launch_halo(lqcd_ctx *ctx, int pack, void *buf, void *spinor, int x3, double sign);
 // peer transport (peer.cu): push both faces of `spinor` (a vector of local parity `parity`) to the neighbours
 int launch_peer_push(lqcd_ctx *ctx, const void *spinor, int parity, int gate);
+int launch_peer_pull(lqcd_ctx *ctx, void *spinor, int parity);   // the faces just exchanged -> the vector's own ghost slices
 int peer_phase(lqcd_ctx *ctx, int what);     // lock-step validation hook (no-op unless set)
 int launch_peer_allreduce(lqcd_ctx *ctx, double *vals, int nv, int which);
 int launch_peer_early_publish(lqcd_ctx *ctx, int kind, const double *partials, int n);   // lock-step validation only

@@ -30,14 +30,16 @@ struct ForceVecs {
 template <typename T, int LAYOUT, int RECON12, int STAGE>
 __global__ void __launch_bounds__(128, 5) force_kernel(const Geom g, const int parity, T *__restrict__ force,
                                                     const T *__restrict__ links, const ForceVecs fv,
-                                                    const T *__restrict__ bf, const int bf_fmt)
+                                                    const T *__restrict__ bf, const int bf_fmt, const int i_begin, const int i_end)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T *const own = reinterpret_cast<T *>(smem_raw);      // own[(s*6 + k)*128 + tid]
     pdl_wait();
     pdl_trigger();
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= g.Vh) return;
+    // sites [i_begin, i_end): the whole parity, or the owned x3 slices of a slab (the forward x3 neighbours of the top
+    // owned slice are then read from the vectors' ghost slice, which the caller's halo exchange has filled)
+    const int i = i_begin + blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= i_end) return;
     const size_t Vh = (size_t)g.Vh;
     const L2Pol pol = {0, 0};
     // site decode and forward neighbours as in dslash.cu (Eq. 9)
@@ -221,15 +223,16 @@ extern "C" size_t lqcd_force_bytes(const lqcd_ctx *ctx)
 template <typename T, int LAYOUT>
 static void launch_force_tl(lqcd_ctx *ctx, int parity, void *force, const void *links, const ForceVecs &fv)
 {
-    dim3 grid((ctx->g.Vh + 127) / 128), block(128);
+    const int i_begin = ctx->x3_lo * ctx->g.s3, i_end = ctx->x3_hi * ctx->g.s3;
+    dim3 grid((i_end - i_begin + 127) / 128), block(128);
     const size_t smem = (size_t)fv.n * 6 * 128 * sizeof(T);
     // measured at 32^4 (profiles/experiments_r1b.md section 7): fp64 -3 %, fp32 +20 % (the carve-out costs L1)
     if (smem <= 48 * 1024 && ctx->force_stage && sizeof(T) == 8) {
-        if (ctx->recon == LQCD_RECON_12) launch_k_smem(ctx, force_kernel<T, LAYOUT, 1, 1>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
-        else launch_k_smem(ctx, force_kernel<T, LAYOUT, 0, 1>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
+        if (ctx->recon == LQCD_RECON_12) launch_k_smem(ctx, force_kernel<T, LAYOUT, 1, 1>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format, i_begin, i_end);
+        else launch_k_smem(ctx, force_kernel<T, LAYOUT, 0, 1>, grid, block, smem, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format, i_begin, i_end);
     } else {
-        if (ctx->recon == LQCD_RECON_12) launch_k(ctx, force_kernel<T, LAYOUT, 1, 0>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
-        else launch_k(ctx, force_kernel<T, LAYOUT, 0, 0>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format);
+        if (ctx->recon == LQCD_RECON_12) launch_k(ctx, force_kernel<T, LAYOUT, 1, 0>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format, i_begin, i_end);
+        else launch_k(ctx, force_kernel<T, LAYOUT, 0, 0>, grid, block, ctx->g, parity, (T *)force, (const T *)links, fv, (const T *)ctx->backfield, ctx->backfield_format, i_begin, i_end);
     }
 }
 
@@ -245,28 +248,40 @@ extern "C" int lqcd_fermion_force(lqcd_ctx *ctx, int nshift, const double *coeff
         if (!xs_e[i]) return lqcd_fail(ctx, LQCD_ERR_ARG, "lqcd_fermion_force: solution %d is null", i);
         if (coeffs[i] != coeffs[i]) return lqcd_fail(ctx, LQCD_ERR_ARG, "coefficient %d is NaN", i);
     }
-    if (ctx->halo_fn || ctx->x3_lo != 0 || ctx->x3_hi != ctx->g.N3)
-        return lqcd_fail(ctx, LQCD_ERR_UNSUPPORTED, "lqcd_fermion_force: not available in slab mode");
+    const bool slab = ctx->halo_fn || ctx->peer_on;
+    if (!slab && (ctx->x3_lo != 0 || ctx->x3_hi != ctx->g.N3))
+        return lqcd_fail(ctx, LQCD_ERR_UNSUPPORTED, "lqcd_fermion_force: a slab context needs a transport (lqcd_set_slab hooks or lqcd_peer_connect)");
     if (!ctx->ws) return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "no workspace set");
     if (ctx->ws_bytes < lqcd_workspace_bytes(ctx, nshift))
         return lqcd_fail(ctx, LQCD_ERR_WORKSPACE, "workspace %zu bytes < %zu needed for %d shifts", ctx->ws_bytes, lqcd_workspace_bytes(ctx, nshift), nshift);
-    // y_i = D_oe x_i into the workspace slots the solver uses for its p_i
-    ForceVecs ev, od;
-    memset(&ev, 0, sizeof(ev));
-    memset(&od, 0, sizeof(od));
-    ev.n = od.n = nshift;
+    // y_i = D_oe x_i into the workspace slots the solver uses for its p_i.  In slab mode the solutions live on the local
+    // parity `par` (the paper's even sites), y_i on the other one, and the force kernel reads the forward x3
+    // neighbours of the top owned slice from the vectors' ghost slices: both x_i and y_i get their ghosts filled.
+    const int par = ctx->solve_parity;
+    auto ghosts = [&](void *v, int parity) -> int {
+        if (ctx->peer_on) { int e = launch_peer_push(ctx, v, parity, 0); return e ? e : launch_peer_pull(ctx, v, parity); }
+        if (ctx->halo_fn && ctx->halo_fn(ctx->comm_user, v, parity)) return lqcd_fail(ctx, LQCD_ERR_CUDA, "halo hook failed");
+        return LQCD_OK;
+    };
+    ForceVecs fx, fy;             // launches on the sites of parity par / 1 - par
+    memset(&fx, 0, sizeof(fx));
+    memset(&fy, 0, sizeof(fy));
+    fx.n = fy.n = nshift;
     for (int i = 0; i < nshift; ++i) {
         void *y = ws_vec(ctx, 4 + i);
-        if ((rc = launch_dslash(ctx, LQCD_ODD, y, xs_e[i], links, NULL, 0.0, 0, 0))) return rc;
-        ev.self[i] = xs_e[i]; ev.nbr[i] = y; ev.coef[i] = coeffs[i];        // x even: + c_i y_i(x+mu) x_i(x)^dagger
-        od.self[i] = y; od.nbr[i] = xs_e[i]; od.coef[i] = -coeffs[i];       // x odd:  - c_i x_i(x+mu) y_i(x)^dagger
+        if ((rc = ghosts(xs_e[i], par))) return rc;
+        if ((rc = launch_dslash(ctx, 1 - par, y, xs_e[i], links, NULL, 0.0, 0, 0))) return rc;
+        if (slab && (rc = ghosts(y, 1 - par))) return rc;
+        fx.self[i] = xs_e[i]; fx.nbr[i] = y; fx.coef[i] = coeffs[i];        // x even: + c_i y_i(x+mu) x_i(x)^dagger
+        fy.self[i] = y; fy.nbr[i] = xs_e[i]; fy.coef[i] = -coeffs[i];       // x odd:  - c_i x_i(x+mu) y_i(x)^dagger
     }
-    for (int par = 0; par < 2; ++par) {
-        const ForceVecs &fv = par ? od : ev;
+    for (int k = 0; k < 2; ++k) {
+        const int lp = k ? 1 - par : par;
+        const ForceVecs &fv = k ? fy : fx;
         if (ctx->prec == LQCD_F64) {
-            if (ctx->layout == 0) launch_force_tl<double, 0>(ctx, par, force, links, fv); else launch_force_tl<double, 1>(ctx, par, force, links, fv);
+            if (ctx->layout == 0) launch_force_tl<double, 0>(ctx, lp, force, links, fv); else launch_force_tl<double, 1>(ctx, lp, force, links, fv);
         } else {
-            if (ctx->layout == 0) launch_force_tl<float, 0>(ctx, par, force, links, fv); else launch_force_tl<float, 1>(ctx, par, force, links, fv);
+            if (ctx->layout == 0) launch_force_tl<float, 0>(ctx, lp, force, links, fv); else launch_force_tl<float, 1>(ctx, lp, force, links, fv);
         }
     }
     return lqcd_check_cuda(ctx, cudaGetLastError(), "fermion force");

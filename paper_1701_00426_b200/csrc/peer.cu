@@ -5,6 +5,7 @@
 
 #include "peer.cuh"
 #include "reduce.cuh"
+#include "su3.cuh"
 
 static size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
 static size_t land_bytes(const lqcd_ctx *ctx) { return align256(lqcd_halo_bytes(ctx)); }
@@ -254,6 +255,39 @@ int launch_peer_push(lqcd_ctx *ctx, const void *spinor, int parity, int gate)
 #undef CALL
     int rc = lqcd_check_cuda(ctx, cudaGetLastError(), "peer push");
     return rc ? rc : peer_after_producer(ctx, parity, gate);
+}
+
+// ---- face pull: the two faces of the exchange just pushed -> the vector's own ghost slices (for consumers that are not
+// the Dslash: the fermion-force kernel reads forward neighbours from the ghost slice).  Follows the push in the stream, so
+// its CTA (0,0) raises the neighbours' flags like the Dslash does; every CTA waits for the rank's own two flags.
+template <typename T, int LAYOUT>
+__global__ void __launch_bounds__(128) peer_pull_kernel(const Geom g, const PeerDev *__restrict__ pdp, const int kind,
+                                                        T *__restrict__ spinor, const int x3_lo, const int x3_hi)
+{
+    pdl_wait();
+    pdl_trigger();
+    const PeerDev &pd = *pdp;
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) peer_signal_halo(pd, kind);
+    peer_wait_halo(pd, kind);
+    const int up = blockIdx.y;                       // 0: ghost slice below (from down), 1: ghost slice above (from up)
+    const T *__restrict__ buf = reinterpret_cast<const T *>(pd.land_self[kind][up]);
+    const int x3 = up ? x3_hi : x3_lo - 1;
+    const int f = blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= g.s3) return;
+    Cx<T> p[3];
+    load_vec_cg<T, LAYOUT>(buf, (size_t)g.s3, (size_t)f, (T)1, (T)0, p);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) st_cx<T, LAYOUT, 0>(spinor, (size_t)c, (size_t)g.Vh, (size_t)x3 * g.s3 + f, p[c], L2Pol());
+}
+
+int launch_peer_pull(lqcd_ctx *ctx, void *spinor, int parity)
+{
+    dim3 grid((ctx->g.s3 + 127) / 128, 2), block(128);
+#define CALL(T, L) launch_k(ctx, peer_pull_kernel<T, L>, grid, block, ctx->g, (const PeerDev *)ctx->d_peer, parity, (T *)spinor, ctx->x3_lo, ctx->x3_hi)
+    if (ctx->prec == LQCD_F64) { if (ctx->layout == 0) CALL(double, 0); else CALL(double, 1); }
+    else { if (ctx->layout == 0) CALL(float, 0); else CALL(float, 1); }
+#undef CALL
+    return lqcd_check_cuda(ctx, cudaGetLastError(), "peer pull");
 }
 
 // ---- generic all-reduce of up to LQCD_MAX_SHIFTS doubles, as two one-CTA kernels (publish, then gather) ----------

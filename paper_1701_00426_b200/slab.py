@@ -308,6 +308,26 @@ class SlabLattice:
             self._halo_finish(inp.data_ptr(), handle)
             lat.dslash_slices(lp, out, inp, links, lo, hi)
 
+    def fermion_force(self, xs, links, coeffs):
+        """lqcd_fermion_force on the slab (both transports): xs = the solutions on the paper's even sites (native local
+        vectors; their ghost slices are overwritten by the halo exchange).  Returns the native (tamat) force field of
+        the LOCAL lattice; only the owned links are written -- collect them with unpack_tamat_owned."""
+        try:
+            return self.lat.fermion_force(xs, links, coeffs)
+        finally:
+            self._raise_hook_error()
+
+    def unpack_tamat_owned(self, native, out_global):
+        """Owned links of a native local tamat field (the fermion force) -> their place in the global canonical field
+        out_global[V][4][3][3]."""
+        loc = self.lat.unpack_tamat(native)
+        g = self.geo
+        s = g.slice_sites
+        gx3 = g.global_x3_of_local()
+        for k in range(g.x3_lo, g.x3_hi):
+            out_global[gx3[k] * s:(gx3[k] + 1) * s] = loc[k * s:(k + 1) * s]
+        return out_global
+
     def _raise_hook_error(self):
         if self.hook_error is not None:
             e, self.hook_error = self.hook_error, None

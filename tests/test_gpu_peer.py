@@ -244,6 +244,32 @@ def test_peer_protocol_selftest_under_real_concurrency(nranks):
     lat.close()
 
 
+@pytest.mark.parametrize("ap", [True, False])
+@pytest.mark.parametrize("world", [1, 2, 4])
+def test_peer_fermion_force_equals_global_oracle(world, ap):
+    """lqcd_fermion_force on slabs over the peer transport: every owned link against the oracle on the global lattice
+    (the antiperiodic sign crosses the slab boundary inside the ghost data; the (-1)^p(x) of R21 is the GLOBAL parity)."""
+    from paper_1701_00426_b200.slab import SlabLattice
+    dims = (4, 6, 4, 8)
+    rng = np.random.default_rng(77)
+    U = gen.haar_like_links(dims, rng)
+    n = 3
+    xs = np.stack([gen.gaussian_half_spinor(dims, rng) for _ in range(n)])
+    c = np.array([0.7, -1.1, 0.4])
+    want = oracle.fermion_force(dims, U, c, xs, antiperiodic_t=ap)
+    got = np.zeros_like(want)
+    lock = threading.Lock()
+
+    def work(r, sl):
+        links = sl.pack_links(U)
+        f = sl.fermion_force([sl.pack_spinor(x, 0) for x in xs], links, c)
+        with lock:
+            sl.unpack_tamat_owned(f, got)
+
+    run_peer_ranks(world, lambda r: SlabLattice(dims, world, r, antiperiodic_t=ap, transport="peer"), work)
+    assert rel(got, want) < 1e-12, (world, ap, rel(got, want))
+
+
 def test_peer_wait_gives_up_instead_of_hanging():
     """A rank whose neighbour never shows up (here: rank 0 of 2 runs alone, with a 50 ms limit) must not hang the GPU:
     the boundary tiles of its Dslash give up, the count is readable, and a solve returns LQCD_ERR_CUDA."""
@@ -278,7 +304,7 @@ def test_peer_errors_and_disconnect():
     links = sl.pack_links(U)
     with pytest.raises(L.LqcdError) as e:
         lat.gauge_staples(links)
-    assert e.value.code == L.ERR_UNSUPPORTED
+    assert e.value.code == L.ERR_UNSUPPORTED                 # ghost depth 2 would be needed
     with pytest.raises(L.LqcdError):
         lat.peer_init(17, 0, 1, 9, 1, 1.0, 1.0)            # more than 16 ranks
     with pytest.raises(L.LqcdError):

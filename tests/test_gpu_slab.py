@@ -219,6 +219,32 @@ def test_slab_dslash_and_solve_with_backfield(world):
         assert tr < 1.5e-10, (i, tr)
 
 
+@pytest.mark.parametrize("world", [1, 2])
+def test_slab_fermion_force_hook_transport(world):
+    """lqcd_fermion_force on slabs with the hook transport, fp32 included."""
+    from paper_1701_00426_b200.slab import SlabLattice
+    dims = (4, 6, 4, 8)
+    rng = np.random.default_rng(34)
+    U = gen.haar_like_links(dims, rng)
+    xs = np.stack([gen.gaussian_half_spinor(dims, rng) for _ in range(2)])
+    c = np.array([0.9, -0.3])
+    for prec in (0, 1):
+        Uu, xx = (U, xs) if prec == 0 else (U.astype(np.complex64).astype(np.complex128), xs.astype(np.complex64).astype(np.complex128))
+        want = oracle.fermion_force(dims, Uu, c, xx)
+        got = np.zeros_like(want)
+        lock = threading.Lock()
+
+        def rank_fn(r, comm):
+            sl = SlabLattice(dims, world, r, comm=comm, prec=prec)
+            f = sl.fermion_force([sl.pack_spinor(x, 0) for x in xx], sl.pack_links(Uu), c)
+            with lock:
+                sl.unpack_tamat_owned(f, got)
+            sl.close()
+
+        run_ranks(world, rank_fn)
+        assert rel(got, want) < (1e-12 if prec == 0 else 1e-5), (world, prec, rel(got, want))
+
+
 @pytest.mark.parametrize("prec", [0, 1])
 @pytest.mark.parametrize("layout", [0, 1])
 def test_single_face_halo_calls(prec, layout):
