@@ -8,8 +8,8 @@
 // rank's own writes is the KERNEL BOUNDARY (every kernel starts with griddepcontrol.wait), what orders them for
 // the peers is one release store per flag.
 //   dot products: the producer (Dslash with <p,q>, K1 with <r,r>) leaves per-CTA partials as on a single GPU;
-//     CTA 0 of the CONSUMER (K1, K2) adds them up and stores the rank's sum into every rank's slot, then raises
-//     the flags; every CTA of the consumer waits for the P flags and adds the P slots in rank order (every rank
+//     every CTA of the CONSUMER (K1, K2) adds them up for itself, CTA 0 stores the rank's sum into every rank's slot
+//     and raises the flags; every CTA waits for the OTHER ranks' flags and adds the P sums in rank order (every rank
 //     gets the bit-identical total, so every rank takes the same decisions);
 //   halo: the push kernel stores the two boundary slices of a vector straight into the neighbours' landing
 //     buffers; CTA 0 of the Dslash that follows it in the stream raises the neighbours' flags; only the tiles
@@ -81,6 +81,18 @@ __device__ __forceinline__ unsigned int peer_wait_red(const PeerDev &pd, int kin
     }
     __syncthreads();
     return n;
+}
+// The same for a consumer whose every CTA has already added up the rank's OWN partials (K1, K2: as on a single GPU, in
+// parallel and bit-identically): only the OTHER ranks' flags are waited for, and `local` takes the rank's own place in
+// the rank-ordered sum -- the rank never waits for its own publish / flag / poll round trip.
+__device__ __forceinline__ double peer_gather_with_local(const PeerDev &pd, int kind, double local)
+{
+    const unsigned int n = *(volatile unsigned int *)&pd.self->cnt_red[kind];
+    if (threadIdx.x < pd.nranks && threadIdx.x != pd.rank) peer_spin(pd, &pd.self->flag_red[kind][threadIdx.x], n);
+    __syncthreads();
+    double s = 0.0;
+    for (int r = 0; r < pd.nranks; ++r) s += r == pd.rank ? local : ld_slot(&pd.self->slot[kind][n & 1][r][0]);
+    return s;
 }
 // sum over the ranks, in rank order, of value v of reduction n (after peer_wait_red)
 __device__ __forceinline__ double peer_sum(const PeerDev &pd, int kind, unsigned int n, int v)

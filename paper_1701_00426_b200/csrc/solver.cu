@@ -164,13 +164,10 @@ __global__ void __launch_bounds__(256) k1_kernel(size_t npk, Seg sg, T *__restri
     if (comm == 1) alpha_d = st->alpha;
     else {
         double pq;
-        if (comm == 2) {     // peer transport: CTA 0 publishes this rank's sum of the Dslash partials, every CTA gathers
-            if (blockIdx.x == 0) {
-                const double local = sum_partials(part_in, n_in);
-                if (threadIdx.x == 0) peer_publish(*pdp, 0, &local, 1);
-            }
-            const unsigned int n = peer_wait_red(*pdp, 0);
-            pq = peer_sum(*pdp, 0, n, 0);
+        if (comm == 2) {     // peer transport: every CTA adds up this rank's Dslash partials (as on one GPU), CTA 0
+            const double local = sum_partials(part_in, n_in);      // publishes the sum, all gather the other ranks' sums
+            if (blockIdx.x == 0 && threadIdx.x == 0) peer_publish(*pdp, 0, &local, 1);
+            pq = peer_gather_with_local(*pdp, 0, local);
         } else pq = sum_partials(part_in, n_in);
         alpha_d = st->cur[ip].rho / pq;
         if (blockIdx.x == 0 && threadIdx.x == 0) solver_after_pq(st, pq, ip);
@@ -218,13 +215,10 @@ __global__ void __launch_bounds__(256) k2_kernel(size_t npk, Seg sg, const T *__
     double rho_new = 0.0, beta_d;
     if (comm == 1) beta_d = st->beta;
     else {
-        if (comm == 2) {     // peer transport: CTA 0 publishes this rank's sum of K1's partials, every CTA gathers
-            if (blockIdx.x == 0) {
-                const double local = sum_partials(part_in, n_in);
-                if (threadIdx.x == 0) peer_publish(*pdp, 1, &local, 1);
-            }
-            const unsigned int n = peer_wait_red(*pdp, 1);
-            rho_new = peer_sum(*pdp, 1, n, 0);
+        if (comm == 2) {     // peer transport: as in K1, with K1's partials
+            const double local = sum_partials(part_in, n_in);
+            if (blockIdx.x == 0 && threadIdx.x == 0) peer_publish(*pdp, 1, &local, 1);
+            rho_new = peer_gather_with_local(*pdp, 1, local);
         } else rho_new = sum_partials(part_in, n_in);
         beta_d = rho_new / st->cur[ip].rho;
     }
