@@ -365,8 +365,14 @@ __global__ void __launch_bounds__(128) peer_selftest_kernel(const PeerDev *pds, 
                 peer_publish(pd, k, &v, 1);
             }
             __syncthreads();
-            const unsigned int n = sabotage ? *(volatile unsigned int *)&pd.self->cnt_red[k] : peer_wait_red(pd, k);
-            const double s = peer_sum(pd, k, n, 0);
+            // kind 0 through the generic pair (wait for all P flags, sum the slots), kind 1 the way K1 / K2 do it (own
+            // value from registers, wait for the other ranks only)
+            double s;
+            if (k == 1 && !sabotage) s = peer_gather_with_local(pd, 1, (double)((me + 1) * (t + 1) + k));
+            else {
+                const unsigned int n = sabotage ? *(volatile unsigned int *)&pd.self->cnt_red[k] : peer_wait_red(pd, k);
+                s = peer_sum(pd, k, n, 0);
+            }
             const double want = (double)((t + 1) * (P * (P + 1) / 2) + k * P);
             if (threadIdx.x == 0 && s != want) atomicAdd(failures, 1u);
             __syncthreads();
