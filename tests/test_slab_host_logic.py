@@ -124,3 +124,55 @@ def test_slab_exchange_gloo_world2(tmp_path):
     for r, (p, o) in enumerate(zip(procs, outs)):
         assert p.returncode == 0, o
         assert f"rank {r} ok" in o
+
+
+_WORKER_IPC = r"""
+import os, sys
+sys.path.insert(0, %r)
+import torch.distributed as dist
+from paper_1701_00426_b200.slab import SlabLattice, SlabGeometry
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo", rank=rank, world_size=world)
+
+
+class FakeLat:                      # stands for the Lattice of a GPU box: records what the plumbing hands to the library
+    def __init__(self):
+        self.connected = None
+    def peer_export(self):
+        return bytes([rank]) * 64   # this rank's "IPC handle"
+    def peer_import(self, r, handle):
+        assert handle == bytes([r]) * 64, (r, handle)
+        return 1000 + r             # "device address" of rank r's block mapped into this process
+    def peer_connect(self, blocks):
+        self.connected = list(blocks)
+
+
+sl = SlabLattice.__new__(SlabLattice)        # no GPU here: only the connect_ipc plumbing is under test
+sl.geo = SlabGeometry((4, 4, 2, 8), world, rank)
+sl.lat = FakeLat()
+sl.peer_block = 7000 + rank
+sl.connect_ipc()
+want = [7000 + rank if r == rank else 1000 + r for r in range(world)]
+assert sl.lat.connected == want, (sl.lat.connected, want)
+dist.destroy_process_group()
+print("rank", rank, "ok")
+"""
+
+
+def test_peer_connect_ipc_plumbing_gloo_world2(tmp_path):
+    """SlabLattice.connect_ipc (the one-process-per-GPU set-up of the peer transport) under gloo with two CPU
+    processes and a stand-in for the GPU context: every rank gathers all handles, maps the OTHER ranks' blocks, keeps
+    its own, and connects with the blocks in rank order."""
+    script = tmp_path / "w_ipc.py"
+    script.write_text(_WORKER_IPC % ROOT)
+    port = 29870 + os.getpid() % 40
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE="2",
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.STDOUT, text=True))
+    outs = [p.communicate(timeout=180)[0] for p in procs]
+    for r, (p, o) in enumerate(zip(procs, outs)):
+        assert p.returncode == 0, o
+        assert f"rank {r} ok" in o
