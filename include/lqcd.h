@@ -151,6 +151,30 @@ int lqcd_mdagm(lqcd_ctx *ctx, void *out_e, const void *in_e, const void *links, 
                double sigma);
 
 /*
+ * lqcd_mdagm for callers that cannot supply a workspace because they cannot allocate device memory: a library
+ * embedded in a program whose own allocator has already claimed the GPU's memory, a service that bans
+ * cudaMalloc / cudaFree after start-up because both stall the whole device, a run planned to the last GB of HBM.
+ * Same arguments, same arithmetic, same two Dslash launches (Eq. 8); the odd-site temporary sits in a
+ * fixed array inside the library's device image instead of the caller's workspace, so no lqcd_set_workspace is
+ * needed and the call makes no cudaMalloc, cudaFree or other allocating call.  (lqcd_create, which every context
+ * needs once, does allocate < 1 MiB; do that at start-up.)
+ *   Limit   lqcd_spinor_bytes(ctx) <= LQCD_NOALLOC_SCRATCH_BYTES (8 MiB: up to 24^4 or 32^3 x 8 in fp64, 32^3 x 16
+ *           in fp32); beyond it LQCD_ERR_WORKSPACE with a message naming both sizes, nothing launched.
+ *   Cost    every GPU onto which the library's device code is loaded holds those 8 MiB until the process ends,
+ *           used or not.
+ *   First call per device: looks up the array's device address (cudaGetSymbolAddress, which may load the device
+ *           code); make that call during start-up, before any stream capture is begun.  Later calls only launch.
+ *   Sharing  one array per device and process, used by every context and every call.  Nothing in it needs
+ *           clearing (each call overwrites all it later reads), but it keeps the previous call's contents and
+ *           two calls that can overlap on the GPU (issued on different streams) race on it.  Calls on one
+ *           stream are safe.
+ * async.  Errors: as lqcd_mdagm, plus LQCD_ERR_WORKSPACE (too large) and LQCD_ERR_UNSUPPORTED (slab contexts).
+ */
+#define LQCD_NOALLOC_SCRATCH_BYTES (8u << 20)
+int lqcd_mdagm_noalloc(lqcd_ctx *ctx, void *out_e, const void *in_e, const void *links, double mass,
+                       double sigma);
+
+/*
  * Solve (mass^2 - D_eo D_oe) x_e = b_e by CG from x = 0 until ||r|| <= tol ||b|| (reading R10).
  *   x_e, b_e    native even-site vectors (device)
  *   iters       host, out: iterations performed (may be NULL)

@@ -17,6 +17,7 @@ F64, F32 = 0, 1
 RECON_18, RECON_12 = 0, 1
 EVEN, ODD = 0, 1
 MAX_SHIFTS = 32
+NOALLOC_SCRATCH_BYTES = 8 << 20   # LQCD_NOALLOC_SCRATCH_BYTES
 
 
 class LqcdError(RuntimeError):
@@ -60,6 +61,7 @@ _sig = {
     "lqcd_set_backfield": (_i, [_vp, _vp]),
     "lqcd_dslash_backfield": (_i, [_vp, _i, _vp, _vp, _vp, _vp]),
     "lqcd_mdagm": (_i, [_vp, _vp, _vp, _vp, _d, _d]),
+    "lqcd_mdagm_noalloc": (_i, [_vp, _vp, _vp, _vp, _d, _d]),
     "lqcd_cg": (_i, [_vp, _vp, _vp, _vp, _d, _d, _i, _pi, _pd]),
     "lqcd_cg_multishift": (_i, [_vp, _i, _pd, _vp, C.POINTER(_vp), _vp, _d, _d, _i, _pi, _pi, _pd]),
     "lqcd_rational_apply": (_i, [_vp, _i, _pd, _d, _pd, _vp, _vp, _vp, _d, _d, _i, _pi, _pi]),
@@ -314,6 +316,12 @@ class Lattice:
     def mdagm(self, out_e, in_e, links, mass, sigma=0.0):
         self.ensure_workspace(1)
         self._check(lib.lqcd_mdagm(self._ctx, _vp(out_e.data_ptr()), _vp(in_e.data_ptr()), _vp(links.data_ptr()), mass, sigma))
+
+    def mdagm_noalloc(self, out_e, in_e, links, mass, sigma=0.0):
+        """mdagm without a workspace: the temporary is the library's fixed 8 MiB device array (lqcd.h).  No torch
+        allocation happens here either; lattices whose half vector exceeds NOALLOC_SCRATCH_BYTES raise LqcdError."""
+        self._check(lib.lqcd_mdagm_noalloc(self._ctx, _vp(out_e.data_ptr()), _vp(in_e.data_ptr()), _vp(links.data_ptr()),
+                                           mass, sigma))
 
     def cg(self, x_e, b_e, links, mass, tol, max_iter, raise_on_max_iter=True):
         """blocking; returns dict(iters, rel_resid, converged)."""
