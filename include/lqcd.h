@@ -331,17 +331,31 @@ int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_parity, lqcd_ha
  * P2P stores into the neighbour's ghost slice", two all-reduces of one double per CG iteration) --------------------
  * No communication library and no host code between the kernels: every rank owns one block of device memory
  * (flags, P slots per reduction, four landing buffers for halo faces) that all ranks of the node map -- through
- * CUDA IPC with one process per GPU, or as plain pointers when the ranks share a process.  Per Dslash one small
- * kernel stores the two boundary slices of the input vector (times the boundary sign) straight into the
- * neighbours' landing buffers and raises their flags; the Dslash kernel waits for its two flags at its start and
- * reads the x3 hops that leave the slab from the landing buffers.  Dot products: the last CTA of the producing
- * kernel stores the local sum into every rank's slot and raises a flag; the consumer kernel (K1 after <p,q>, K2
- * after <r,r>) waits for the P flags and adds the P slots in rank order, so every rank gets the bit-identical
- * total and takes the same decisions.  The waits are inside the kernels: the CG loop stays one CUDA graph per
- * chunk of iterations.  Flags are monotone counters; re-use of slots and landing buffers is ordered by the two
- * all-reduces of every iteration and by the alternation of the two exchange kinds (even / odd input vector); where a
- * caller exchanges the same kind twice in a row (lqcd_dslash twice for one parity, a solve right after it) the
- * library puts a device-side barrier (a dummy all-reduce) in between by itself.
+ * CUDA IPC with one process per GPU, or as plain pointers when the ranks share a process.  The protocol as built
+ * (csrc/peer.cuh is the reference; this is its summary):
+ *   Halo.  The two boundary slices of a vector (times the boundary sign) are stored straight into the neighbours'
+ *     landing buffers by the kernel that PRODUCES the vector inside a solve (the init kernel and K2 for p, the first
+ *     Dslash of the iteration for D p); a stand-alone lqcd_dslash / lqcd_dslash_backfield / lqcd_mdagm uses one small
+ *     push kernel instead.  Thread 0 of the Dslash that follows in the stream raises the neighbours' flags (the kernel
+ *     boundary has completed the stores), and only the tiles of that Dslash that touch a boundary slice wait for the
+ *     rank's own two flags; they take the x3 hops that leave the slab from the landing buffers, the interior tiles
+ *     compute meanwhile.
+ *   Dot products.  The producer (Dslash with <p,q>, K1 with <r,r>) leaves per-CTA partials, as on one GPU.  Every CTA
+ *     of the CONSUMER kernel (K1, K2) adds them up for itself; its CTA 0 stores the rank's sum into every rank's slot
+ *     and raises the flags; every CTA waits for the OTHER ranks' flags only and adds the P sums in rank order, so
+ *     every rank gets the bit-identical total and takes the same decisions.
+ * The waits are inside the kernels: the CG loop stays one CUDA graph per chunk of iterations.  Flags are monotone
+ * counters; re-use of slots and landing buffers is ordered by the two all-reduces of every iteration and by the
+ * alternation of the two exchange kinds (even / odd input vector); where a caller exchanges the same kind twice in a
+ * row (lqcd_dslash twice for one parity, a solve right after it) the library puts a device-side barrier (a dummy
+ * all-reduce) in between by itself.
+ * STATUS: verified on ONE GPU only (virtual ranks in lock step, P = 1, 2, 4, and a cooperative-kernel self-test of
+ * the flag protocol under real concurrency).  With P >= 2 real devices the path has never executed: the assumption
+ * it rests on -- peer stores issued by kernel N are performed at the remote GPU before the st.release.sys that
+ * kernel N+1 issues after its griddepcontrol.wait -- is UNVERIFIED ON HARDWARE.
+ * Teardown: lqcd_peer_disconnect and lqcd_destroy free the rank's block after finishing only this rank's stream; a
+ * neighbour's last kernel may still be storing into it.  Every rank must finish its stream and meet the others at a
+ * host barrier before any rank disconnects or destroys (SlabLattice.close does).
  *   lqcd_peer_init      allocate the block; the context must have local extents (N0,N1,N2,L3+2) and antiperiodic_t
  *                       = 0 as described above; x3_lo/x3_hi/solve_parity as in lqcd_set_slab; sign_up / sign_down:
  *                       factor applied to the face sent to the rank above / below (-1 where the hop crosses an
@@ -358,9 +372,11 @@ int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_parity, lqcd_ha
  * neighbour.  A backfield works as on one GPU (the slab's phases include the ghost slices, like its links);
  * lqcd_fermion_force works too (faces pushed and then pulled into the vectors' ghost slices);
  * lqcd_gauge_staples is LQCD_ERR_UNSUPPORTED in this mode (it would need ghost depth 2).
- * A wait for another rank never lasts longer than a few seconds of SM clock: a wait that gives up is counted in the
- * rank's block, the solver calls then return LQCD_ERR_CUDA ("... waits for other ranks timed out"; the results are
- * meaningless), and lqcd_get_option(ctx, "peer_timeouts") reads the count (blocking) after lqcd_dslash / lqcd_mdagm.
+ * A wait for another rank never lasts longer than option peer_wait_ms (default 3000): a wait that gives up is counted
+ * in the rank's block and the rank's transport is then DEAD -- every later wait returns at once, a running solve stops
+ * at its next convergence poll, and this and every later solver call return LQCD_ERR_CUDA ("... waits for other ranks
+ * timed out"; the results are meaningless) until lqcd_peer_disconnect + lqcd_peer_init build a new block.
+ * lqcd_get_option(ctx, "peer_timeouts") reads the count (blocking) after lqcd_dslash / lqcd_mdagm.
  * The kernels of different ranks wait for one another: run each rank on its own GPU.  For validation on ONE GPU
  * lqcd_set_phase_hook installs a host callback that the library calls after every launch that publishes to the
  * peers (what = 0: face push, 1: generic all-reduce, 2: dot product); a test harness that synchronises its stream

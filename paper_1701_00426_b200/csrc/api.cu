@@ -357,6 +357,10 @@ extern "C" int lqcd_dslash_backfield(lqcd_ctx *ctx, int parity, void *out, const
     REQUIRE(out && in && links && backfield, "lqcd_dslash_backfield: null pointer");
     REQUIRE(parity == 0 || parity == 1, "lqcd_dslash_backfield: parity %d", parity);
     REQUIRE(out != in, "lqcd_dslash_backfield: out and in alias");
+    // peer transport: the faces of `in` go to the neighbours first, exactly as in lqcd_dslash (the kernel that follows
+    // raises the flags and reads the landing buffers; without the push it would find the flags of the PREVIOUS
+    // exchange already raised and read stale faces)
+    if (ctx->peer_on && (rc = launch_peer_push(ctx, in, 1 - parity, 0))) return rc;
     const void *saved = ctx->backfield;
     ctx->backfield = backfield;
     rc = launch_dslash(ctx, parity, out, in, links, NULL, 0.0, 0, 0);

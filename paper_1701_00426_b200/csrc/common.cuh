@@ -208,7 +208,8 @@ struct SolverState {
     unsigned int ticket;   // last-block-done counter of the reductions
     int comm;              // slab mode.  1 (hooks): reductions leave LOCAL sums in sum[] (0: <p,q>, 1: <r,r>, 2: <b,b>); the
     double sum[4];         // recurrences run in scalar_kernel after the caller's all-reduce.  2 (peer transport):
-                           // the last CTA publishes the local sum to every rank, the consumer kernel gathers (peer.cuh)
+                           // the producer leaves per-CTA partials; CTA 0 of the CONSUMER kernel publishes the rank's sum to
+                           // every rank, every CTA of the consumer gathers the other ranks' sums (peer.cuh)
     double resid[LQCD_MAX_SHIFTS];  // ||b - (A+sigma_i) x_i||^2 recomputed at exit
     double hist_alpha[LQCD_HIST], hist_beta[LQCD_HIST], hist_rnorm[LQCD_HIST];
 };

@@ -45,14 +45,20 @@ __device__ __forceinline__ double ld_slot(const double *p)
 }
 
 // Spin until *f >= n (wrap-safe), but never for more than pd.wait_cycles (option peer_wait_ms, default 3 s): a peer that died or
-// ran a different sequence of calls must not hang this GPU.  A wait that gives up counts itself in the rank's block;
-// the host turns a non-zero count into LQCD_ERR_CUDA at the end of the solve (the results are then meaningless).
+// ran a different sequence of calls must not hang this GPU.  A wait that gives up counts itself in the rank's block, and
+// from then on the transport of this rank is DEAD: every later wait (of this kernel's other CTAs, of every later kernel)
+// returns at once instead of spending the limit again -- the flags are monotone counters, so a peer that missed one sync
+// point misses all later ones, and 4 waits x 3 s per CG iteration would hold the GPU for hours.  The solver's host loop
+// reads the count with every convergence poll and stops enqueueing (solver.cu); every call over a dead transport
+// returns LQCD_ERR_CUDA (the results are meaningless) until lqcd_peer_disconnect + lqcd_peer_init build a new one.
 __device__ __forceinline__ void peer_spin(const PeerDev &pd, const unsigned int *f, unsigned int n)
 {
     if ((int)(ld_flag(f) - n) >= 0) return;
+    if (*(volatile unsigned int *)&pd.self->timeouts) return;
     const long long t0 = clock64();
     while ((int)(ld_flag(f) - n) < 0) {
         if (clock64() - t0 > pd.wait_cycles) { atomicAdd(&pd.self->timeouts, 1u); return; }
+        if (*(volatile unsigned int *)&pd.self->timeouts) return;      // another waiter of this rank gave up meanwhile
     }
 }
 

@@ -455,6 +455,7 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     const double msq = mass * mass + shifts[base];
     volatile int *flag = ctx->h_flag;
     flag[0] = flag[16 / 4] = 0;
+    flag[1] = flag[16 / 4 + 1] = 0;
     int enq = 0, chunk_id = 0, stop = 0;
     // one CG iteration = 4 kernels; all arguments are the same in every iteration
     // <p,q> partials (one per Dslash CTA) and <r,r> partials (one per K1 CTA) live in separate halves of
@@ -547,12 +548,14 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
         enq += n;
         int slot = chunk_id & 1;
         cudaMemcpyAsync((void *)(flag + slot * 4), &ctx->d_state->done, sizeof(int), cudaMemcpyDeviceToHost, s);
+        // peer transport: a wait that gave up (peer.cuh) ends the solve at the next poll, not after max_iter iterations
+        if (peer) cudaMemcpyAsync((void *)(flag + slot * 4 + 1), &((PeerBlock *)ctx->peer_mem)->timeouts, sizeof(int), cudaMemcpyDeviceToHost, s);
         cudaEventRecord(ctx->ev[slot], s);
         // look at the PREVIOUS chunk's flag, so that one chunk is always queued behind the GPU
         if (chunk_id > 0) {
             int prev = (chunk_id - 1) & 1;
             if ((rc = lqcd_check_cuda(ctx, cudaEventSynchronize(ctx->ev[prev]), "cg poll"))) return rc;
-            if (flag[prev * 4]) stop = 1;
+            if (flag[prev * 4] || (peer && flag[prev * 4 + 1])) stop = 1;
         }
         if (enq >= max_iter) stop = 1;
         ++chunk_id;
@@ -585,9 +588,9 @@ static int solve_t(lqcd_ctx *ctx, int nshift, const double *shifts, const void *
     memcpy(ctx->h_hist[2], h.hist_rnorm, sizeof(h.hist_rnorm));
     if (peer) {      // a wait for a peer gave up (dead or desynchronised rank): the results are meaningless
         const long nt = peer_timeouts(ctx);
-        if (nt != ctx->peer_timeouts_seen) {
+        if (nt != 0) {      // the transport stays dead (peer.cuh): every later solve reports it again
             ctx->peer_timeouts_seen = nt;
-            return lqcd_fail(ctx, LQCD_ERR_CUDA, "peer transport: %ld waits for other ranks timed out", nt);
+            return lqcd_fail(ctx, LQCD_ERR_CUDA, "peer transport: %ld waits for other ranks timed out; the transport is dead until lqcd_peer_disconnect + lqcd_peer_init", nt);
         }
     }
     if (!converged) return lqcd_fail(ctx, LQCD_ERR_NOT_CONVERGED, "not converged after %d iterations", h.iter);

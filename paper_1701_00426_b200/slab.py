@@ -184,6 +184,16 @@ class SlabLattice:
         self.lat.set_slab(self.geo.x3_lo, self.geo.x3_hi, self.geo.local_parity(0), self._halo_cb, self._allreduce_cb)
 
     def close(self):
+        """Peer transport between processes: a neighbour's last kernel may still be storing into this rank's block
+        (the faces K2 pushes after the final iteration have no reader), and freeing the block under it would fault the
+        neighbour's GPU.  So every rank finishes its own stream and meets the others before anyone frees (lqcd.h,
+        "Teardown").  Ranks that share a process (connect_local) are closed by one thread after all have finished."""
+        if getattr(self, "_ipc_connected", False) and self.lat._ctx:
+            import torch.distributed as dist
+            self.lat.synchronize()
+            if dist.is_initialized():
+                dist.barrier()
+            self._ipc_connected = False
         self.lat.close()
 
     # -- peer transport: hand every rank the other ranks' blocks ------------------------------------------
@@ -203,6 +213,7 @@ class SlabLattice:
         dist.all_gather_object(handles, self.lat.peer_export())
         blocks = [self.peer_block if r == g.rank else self.lat.peer_import(r, handles[r]) for r in range(g.world)]
         self.lat.peer_connect(blocks)
+        self._ipc_connected = True
         dist.barrier()
 
     def set_lockstep(self, barrier):

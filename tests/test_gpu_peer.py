@@ -231,6 +231,44 @@ def test_peer_backfield_dslash_and_solve(world, fmt):
         assert tr < 1.5e-10, (i, tr)
 
 
+@pytest.mark.parametrize("fmt", [0, 1])
+@pytest.mark.parametrize("world", [1, 2, 4])
+def test_peer_dslash_backfield_explicit_call(world, fmt):
+    """lqcd_dslash_backfield (the paper's four-argument acc_Deo, phases given per call, nothing attached to the
+    context) over the peer transport: the call must push the faces of ITS input before the kernel reads the landing
+    buffers.  Two calls in a row with different inputs: a missing push would leave the first call's faces (or none)
+    in the buffers and the boundary slices of the second result would be wrong."""
+    from paper_1701_00426_b200.slab import SlabLattice
+    dims = (8, 6, 4, 8)
+    rng = np.random.default_rng(77)
+    U = gen.smooth_links(dims, 0.3, rng)
+    theta = gen.uniform_backfield(dims, rng)
+    psis = [gen.gaussian_spinor(dims, rng), gen.gaussian_spinor(dims, rng)]
+    got = {(k, gp): None for k in range(2) for gp in (0, 1)}
+    for key in got:
+        got[key] = np.zeros((dims[0] * dims[1] * dims[2] * dims[3] // 2, 3), dtype=np.complex128)
+    lock = threading.Lock()
+
+    def work(r, sl):
+        links = sl.pack_links(U)
+        bf = sl.pack_backfield(theta)
+        outs = {}
+        for k, psi in enumerate(psis):
+            for gp in (1, 0):
+                inp = sl.pack_spinor(oracle.full_to_half(dims, 1 - gp, psi), 1 - gp)
+                outs[(k, gp)] = sl.new_spinor()
+                sl.lat.dslash_backfield(sl.geo.local_parity(gp), outs[(k, gp)], inp, links, bf)
+                sl._raise_hook_error()
+        with lock:
+            for key, buf in outs.items():
+                sl.unpack_spinor(buf, key[1], got[key])
+
+    run_peer_ranks(world, lambda r: SlabLattice(dims, world, r, transport="peer", options=dict(backfield_format=fmt)), work)
+    for (k, gp), g in got.items():
+        want = oracle.dslash_half(dims, U, gp, oracle.full_to_half(dims, 1 - gp, psis[k]), theta=theta)
+        assert rel(g, want) < 1e-12, (world, fmt, k, gp, rel(g, want))
+
+
 @pytest.mark.parametrize("nranks", [1, 2, 3, 8, 16])
 def test_peer_protocol_selftest_under_real_concurrency(nranks):
     """lqcd_peer_selftest: the flags / slots / counters of the transport with ranks that run AT THE SAME TIME (one
@@ -289,6 +327,37 @@ def test_peer_wait_gives_up_instead_of_hanging():
     with pytest.raises(L.LqcdError) as e:
         sl.cg_multishift([sl.new_spinor()], be, links, 0.2, [0.0], 1e-8, 8, raise_on_max_iter=False)
     assert e.value.code == L.ERR_CUDA and "timed out" in str(e.value)
+    for s in slabs:
+        s.close()
+
+
+def test_peer_timeout_ends_a_long_solve_at_once():
+    """A dead peer must cost ONE wait limit, not one per wait: with max_iter = 20000 and the chunk graph on (no lock-step
+    hook), rank 0 of 2 runs alone.  Before the first timeout made the transport dead, every one of the 4 waits of every
+    iteration spent the full limit again (here 4 x 0.1 s x 20000 iterations = over two hours of GPU time); now the first
+    wait gives up after 0.1 s, every later wait returns at once, the host sees the count at its next poll and the call
+    returns LQCD_ERR_CUDA within seconds -- and so does the next call over the same (dead) transport."""
+    import time
+    import paper_1701_00426_b200 as L
+    from paper_1701_00426_b200.slab import SlabLattice
+    dims = (4, 4, 4, 8)
+    rng = np.random.default_rng(78)
+    U = gen.smooth_links(dims, 0.3, rng)
+    b = gen.gaussian_half_spinor(dims, rng)
+    slabs = [SlabLattice(dims, 2, r, transport="peer", options=dict(peer_wait_ms=100)) for r in range(2)]
+    SlabLattice.connect_local(slabs)
+    sl = slabs[0]
+    links, be = sl.pack_links(U), sl.pack_spinor(b, 0)
+    xs = [sl.new_spinor(), sl.new_spinor()]
+    sl.lat.synchronize()
+    for attempt in range(2):
+        t0 = time.time()
+        with pytest.raises(L.LqcdError) as e:
+            sl.cg_multishift(xs, be, links, 0.01, [0.0, 0.1], 1e-12, 20000, raise_on_max_iter=False)
+        dt = time.time() - t0
+        assert e.value.code == L.ERR_CUDA and "timed out" in str(e.value)
+        assert dt < 20.0, (attempt, dt)
+    assert sl.lat.get_option("peer_timeouts") > 0
     for s in slabs:
         s.close()
 

@@ -138,6 +138,7 @@ dist.init_process_group("gloo", rank=rank, world_size=world)
 class FakeLat:                      # stands for the Lattice of a GPU box: records what the plumbing hands to the library
     def __init__(self):
         self.connected = None
+        self.events = []
     def peer_export(self):
         return bytes([rank]) * 64   # this rank's "IPC handle"
     def peer_import(self, r, handle):
@@ -145,6 +146,12 @@ class FakeLat:                      # stands for the Lattice of a GPU box: recor
         return 1000 + r             # "device address" of rank r's block mapped into this process
     def peer_connect(self, blocks):
         self.connected = list(blocks)
+    _ctx = 1
+    def synchronize(self):
+        self.events.append("sync")
+    def close(self):
+        self.events.append("close")
+        self._ctx = None
 
 
 sl = SlabLattice.__new__(SlabLattice)        # no GPU here: only the connect_ipc plumbing is under test
@@ -154,6 +161,16 @@ sl.peer_block = 7000 + rank
 sl.connect_ipc()
 want = [7000 + rank if r == rank else 1000 + r for r in range(world)]
 assert sl.lat.connected == want, (sl.lat.connected, want)
+# teardown: close() finishes the rank's stream, then meets the other ranks, then frees -- rank 1 arrives 1.5 s late and
+# rank 0 must not have freed its block before
+import time
+if rank == 1:
+    time.sleep(1.5)
+t0 = time.time()
+sl.close()
+waited = time.time() - t0
+assert sl.lat.events == ["sync", "close"], sl.lat.events
+assert rank == 1 or waited > 1.0, waited
 dist.destroy_process_group()
 print("rank", rank, "ok")
 """
@@ -162,7 +179,7 @@ print("rank", rank, "ok")
 def test_peer_connect_ipc_plumbing_gloo_world2(tmp_path):
     """SlabLattice.connect_ipc (the one-process-per-GPU set-up of the peer transport) under gloo with two CPU
     processes and a stand-in for the GPU context: every rank gathers all handles, maps the OTHER ranks' blocks, keeps
-    its own, and connects with the blocks in rank order."""
+    its own, and connects with the blocks in rank order; close() synchronises, waits for the other ranks, then frees."""
     script = tmp_path / "w_ipc.py"
     script.write_text(_WORKER_IPC % ROOT)
     port = 29870 + os.getpid() % 40
