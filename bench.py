@@ -15,7 +15,9 @@ from profiles/traffic.json, the ncu capture of the SAME kernel), e2e (same metri
 lqcd_dslash_host_vectors_batch with pinned host vectors, copies inside the timed region; links resident as the
 operator -- the all-inclusive lqcd_dslash_host figure is reported beside it as cold_links), cpu_baseline (the
 oracle on the host cores: Dslash, CG at 16^4, multi-shift CG at 24^3 x 48; bounded samples), clocks,
-gpu_launches, and `extra`: 12-real / fp32 Dslash, CG / multi-shift / rational iteration rates at 32^4,
+gpu_launches, parity (the last timed outputs against the oracle on sampled sites), solver (the CG / multi-shift /
+rational iteration rates, top level so that the driver's record keeps them), volume_ladder (Dslash and CG versus volume on
+the paper's Table-3 lattices), and `extra`: 12-real / fp32 Dslash, CG / multi-shift / rational iteration rates at 32^4,
 BASELINE.json configs[1], [3], [4] (16^4 CG and 24^3 x 48 / 32^4 multi-shift solves to tolerance, 48^4 and
 64^3 x 16 Dslash in fp64 and fp32), the fermion force, the gauge staples against the FP64 peak measured in
 this run, and the end-to-end multi-shift solve on host vectors.
@@ -349,6 +351,8 @@ def run_ours(args):
     ms = timed_loop(torch, step, args.steps, 0, world, D, device)
     launches = lat.launches - n0
     clocks = sampler.stop() if rank == 0 else None
+    # the outputs of the LAST timed applications, read back outside the timed region: checked against the oracle below
+    timed_out = {L.ODD: lat.unpack_spinor(d_out_o, L.ODD), L.EVEN: lat.unpack_spinor(d_out_e, L.EVEN)} if rank == 0 else None
     apps = 2 * k * args.steps
     ns_site = D.aggregate_ns_per_site(ms, k * args.steps, V, world)
     us_launch = ms * 1e3 / apps
@@ -505,7 +509,7 @@ def run_ours(args):
                                                "frac": f1 * V / (t_1 * 1e-3) / 1e12 / fp64_peak,
                                                "frac_by_definition_count": flop_def * V / (t_1 * 1e-3) / 1e12 / fp64_peak}
         del sbuf
-        cfg2 = cfg4 = None
+        cfg2 = cfg4 = ladder = None
         if not args.quick:
             # ---- BASELINE.json configs[1]: CG at 16^4 to tolerance (L2-resident: launch-latency bound) ----
             d2 = (16, 16, 16, 16)
@@ -553,6 +557,25 @@ def run_ours(args):
                                                    "GBs": by * (Vl // 2) / (ms_it * 1e-3) / 1e9,
                                                    "frac": by * (Vl // 2) / (ms_it * 1e-3) / 1e9 / peak}
                     lc.close()
+            # ---- BASELINE.json configs[4] "versus volume": the L2 -> HBM transition on the paper's Table-3 lattices
+            #      (32^2 x 8 x 32, 32^3 x 8, 24^4, 32^4, 32^3 x 36) and a few cubes around them; fp64 18-real
+            ladder = []
+            for dims_l in ((16, 16, 16, 16), (20, 20, 20, 20), (24, 24, 24, 24), (32, 32, 8, 32), (32, 32, 32, 8),
+                           (32, 32, 32, 36), (40, 40, 40, 40)):
+                Vl = gen.volume(dims_l)
+                Ul = U48[:Vl]
+                rs = np.random.default_rng(56)
+                ie, io = gen.gaussian_half_spinor(dims_l, rs), gen.gaussian_half_spinor(dims_l, rs)
+                dr = dslash_rate(torch, L, D, gen, dims_l, Ul, ie, io, L.F64, L.RECON_18, peak, device, n=100)
+                lc = L.Lattice(dims_l, device=local_rank)
+                ms_it = solver_iter_rate(torch, lc, L, lc.pack_links(Ul), lc.pack_spinor(ie, L.EVEN), [0.0], 0.01, n_lo=24, n_hi=120)
+                lc.close()
+                link_mb = Vl * 4 * 144 / 1e6
+                ladder.append({"dims": list(dims_l), "links_MB": round(link_mb, 1),
+                               "regime": "L2" if link_mb + 6 * Vl // 2 * 48 / 1e6 < 126 else "HBM",
+                               "dslash_ns_per_site": round(dr["ns_per_site"], 4), "dslash_frac": round(dr["frac"], 3),
+                               "cg_us_per_iter": round(ms_it * 1e3, 2),
+                               "cg_frac": round(CG_BYTES * (Vl // 2) / (ms_it * 1e-3) / 1e9 / peak, 3)})
             del U48
         # ---- CPU oracle beside it -------------------------------------------------------------
         psi = np.zeros((V, 3), dtype=np.complex128)
@@ -561,6 +584,17 @@ def run_ours(args):
         cpu_ns, reps, cores = cpu_oracle_dslash(U, psi, min_seconds=args.cpu_seconds)
         cpu = {"value": cpu_ns, "unit": "ns/site", "cores": cores, "kind": "oracle",
                "sample": f"{reps} full-lattice applications of oracle_dirac_full at 32^4"}
+        parity = check_timed_outputs(np, gen, U, psi, timed_out)
+        solver = {k2: {"iter_per_s": extra[k1]["iter_per_s"], "us_per_iter": extra[k1]["us_per_iter"], "frac": extra[k1]["frac"]}
+                  for k1, k2 in (("cg_f64", "cg"), ("multishift8_f64", "multishift8"), ("rational8_f64", "rational8"))}
+        solver["lattice"] = "32^4 fp64 18-real, all shifts active, per-iteration time by differencing two fixed-length solves"
+        s32 = extra["multishift_32x32x32x32"]
+        solver["multishift8_to_1e-10"] = {"iters": s32["iters"], "ms": s32["ms"], "max_true_rel_resid": s32["max_true_rel_resid"]}
+        for key in ("cg_48x48x48x48_f64", "cg_48x48x48x48_f32", "cg_64x64x64x16_f64", "cg_64x64x64x16_f32"):
+            if key in extra:
+                solver[key] = {"iter_per_s": extra[key]["iter_per_s"], "frac": extra[key]["frac"]}
+        solver["fermion_force8_ms"] = extra["fermion_force8_f64"]["ms"]
+        solver["gauge_staples_ns_per_site"] = extra["gauge_staples_f64"]["ns_per_site"]
         if cfg2 is not None:
             cpu["solver"] = cpu_oracle_solvers(gen, cfg2, cfg4, 40)
             cpu["solver"]["note"] = (f"same oracle, same inputs as extra.cg_16x16x16x16 / extra.multishift_24x24x24x48, {cores} threads "
@@ -594,6 +628,9 @@ def run_ours(args):
                                    "h2d_bytes_per_step": 2 * (U.nbytes + in_e.nbytes), "d2h_bytes_per_step": 2 * in_e.nbytes,
                                    "api": "lqcd_dslash_host x2 per step: the canonical link field is uploaded and packed in every call"}},
             "gpu_launches": launches,
+            "parity": parity,
+            "solver": solver,
+            "volume_ladder": ladder,
             "clocks": clocks,
             "cpu_baseline": cpu,
             "extra": extra,
@@ -660,6 +697,27 @@ def slab_strong_leg(torch, L, D, gen, U, rank, local_rank, world, device, plain_
     if plain_us is not None:
         out["dslash_overhead_us_vs_plain_context"] = us - plain_us
     return out
+
+
+def check_timed_outputs(np, gen, U, psi, timed_out, n_random=200, tol=1e-12):
+    """"last outputs vs oracle".  The vectors the LAST timed applications wrote (D_oe in_e on
+    the odd sites, D_eo in_o on the even sites) against oracle_dirac_site, one site at a time: the 16 corners, 20 random
+    sites in each x3 boundary slice, n_random random sites.  Outside every timed region; rank 0 only."""
+    import oracle
+    n0, n1, n2, n3 = DIMS
+    samp = np.random.default_rng(99)
+    picks = [(a * (n0 - 1), b * (n1 - 1), c * (n2 - 1), d * (n3 - 1)) for a in (0, 1) for b in (0, 1) for c in (0, 1) for d in (0, 1)]
+    for x3 in (0, n3 - 1):
+        picks += [(int(samp.integers(n0)), int(samp.integers(n1)), int(samp.integers(n2)), x3) for _ in range(20)]
+    picks += [tuple(int(samp.integers(n)) for n in DIMS) for _ in range(n_random)]
+    worst = 0.0
+    for x in picks:
+        lex = x[0] + n0 * (x[1] + n1 * (x[2] + n2 * x[3]))
+        want = oracle.dirac_site(DIMS, U, psi, x)
+        got = timed_out[sum(x) % 2][lex // 2]
+        worst = max(worst, float(np.abs(got - want).max() / np.abs(want).max()))
+    return {"max_rel_err": worst, "sites": len(picks), "tol": tol, "ok": bool(worst < tol),
+            "against": "oracle_dirac_site on the outputs of the last timed D_oe and D_eo applications"}
 
 
 def dslash_rate(torch, L, D, gen, dims, U, in_e, in_o, prec, recon, peak, device, n=100, theta=None, bf_format=0,
