@@ -377,13 +377,9 @@ int lqcd_set_slab(lqcd_ctx *ctx, int x3_lo, int x3_hi, int solve_parity, lqcd_ha
  * at its next convergence poll, and this and every later solver call return LQCD_ERR_CUDA ("... waits for other ranks
  * timed out"; the results are meaningless) until lqcd_peer_disconnect + lqcd_peer_init build a new block.
  * lqcd_get_option(ctx, "peer_timeouts") reads the count (blocking) after lqcd_dslash / lqcd_mdagm.
- * The kernels of different ranks wait for one another: run each rank on its own GPU.  For validation on ONE GPU
- * lqcd_set_phase_hook installs a host callback that the library calls after every launch that publishes to the
- * peers (what = 0: face push, 1: generic all-reduce, 2: dot product); a test harness that synchronises its stream
- * there and then meets the other ranks at a host barrier runs the ranks in lock step, so that no kernel ever
- * waits (the chunk graph is off while a hook is set).  Pass NULL to clear.
+ * The kernels of different ranks wait for one another: run each rank on its own GPU.  (Validation on ONE GPU: the
+ * lock-step hook and the protocol self-test of include/lqcd_diag.h.)
  */
-typedef int (*lqcd_phase_fn)(void *user, int what);
 size_t lqcd_peer_block_bytes(const lqcd_ctx *ctx);
 int lqcd_peer_init(lqcd_ctx *ctx, int nranks, int rank, int x3_lo, int x3_hi, int solve_parity,
                    double sign_up, double sign_down, void **block);
@@ -391,14 +387,6 @@ int lqcd_peer_export(lqcd_ctx *ctx, void *handle64);
 int lqcd_peer_import(lqcd_ctx *ctx, int rank, const void *handle64, void **block);
 int lqcd_peer_connect(lqcd_ctx *ctx, void *const *blocks);
 int lqcd_peer_disconnect(lqcd_ctx *ctx);
-int lqcd_set_phase_hook(lqcd_ctx *ctx, lqcd_phase_fn fn, void *user);
-/* Protocol self-test under real concurrency on ONE GPU: one cooperative kernel whose CTA r plays rank r of `nranks` on its
- * own block -- the flags, slots and counters of the transport with ranks that really run at the same time, at uneven pace,
- * and really wait for one another -- for `rounds` iterations of (halo exchange, two all-reduces).  *failures = wrong
- * tokens / sums / waits that gave up (0 = pass).  sabotage = 1 makes the consumers skip their waits: the count must then
- * be non-zero for more than a few ranks (the check that the test can fail).  Allocates and frees its own scratch memory;
- * independent of lqcd_peer_init.  blocking. */
-int lqcd_peer_selftest(lqcd_ctx *ctx, int nranks, int rounds, int sabotage, int *failures);
 
 /*
  * After lqcd_cg / lqcd_cg_multishift: copy up to `n` entries of the per-iteration history
@@ -442,16 +430,7 @@ int lqcd_cg_multishift_host(lqcd_ctx *ctx, int nshift, const double *shifts,
                             const void *links_host, double mass, double tol, int max_iter,
                             int *iters, int *conv_iter, double *rel_resid);
 
-/*
- * Measurement helper (no arithmetic of the method): attainable FP64 FMA rate of the device in TFLOP/s, from a
- * kernel of independent DFMA chains on the context's stream -- the roofline denominator of the ALU-bound
- * gauge-staples kernel (bench.py extra.fp64_peak_tflops).  tflops: host, out.  blocking.
- */
-int lqcd_measure_fp64_peak(lqcd_ctx *ctx, double *tflops);
-/* Measurement helper: attainable READ bandwidth in GB/s over the caller's device buffer (use one larger than L2, e.g.
- * the link field): 16-byte streaming loads, nothing written.  MEASURED_PEAKS.json's HBM figure is a copy (half
- * writes); the Dslash is 96 % reads (bench.py roofline.frac_of_read_rate).  buf: 16-byte aligned, >= 1 MiB.  blocking. */
-int lqcd_measure_hbm_read(lqcd_ctx *ctx, const void *buf_dev, size_t bytes, double *gbs);
+/* Validation and measurement helpers that are NOT part of the ABI of SURVEY.md section 8(b) live in lqcd_diag.h. */
 
 #ifdef __cplusplus
 }

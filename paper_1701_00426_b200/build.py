@@ -16,7 +16,8 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "liblqcd_b200.so")
 SOURCES = ["api.cu", "pack.cu", "dslash.cu", "solver.cu", "host.cu", "force.cu", "staples.cu", "diag.cu", "peer.cu", "noalloc.cu"]
-HEADERS = ["common.cuh", "reduce.cuh", "su3.cuh", "peer.cuh", os.path.join("..", "..", "include", "lqcd.h")]
+HEADERS = ["common.cuh", "reduce.cuh", "su3.cuh", "peer.cuh", os.path.join("..", "..", "include", "lqcd.h"),
+           os.path.join("..", "..", "include", "lqcd_diag.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

@@ -8,6 +8,7 @@
 #include <string.h>
 
 #include "../../include/lqcd.h"
+#include "../../include/lqcd_diag.h"
 
 // ------------------------------------------------------------------------------------------
 // Lattice geometry handed to kernels by value.

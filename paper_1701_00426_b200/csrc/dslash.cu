@@ -226,15 +226,16 @@ static void launch_t(lqcd_ctx *ctx, int parity, void *out, const void *in, const
         (const T *)ctx->backfield, (const PeerDev *)ctx->d_peer, push_out)
 #define GO(MB) do { if (ctx->l2_hints) GO1(MB, 1, 0); else GO1(MB, 0, 0); } while (0)
     // peer transport: the per-precision default variant, faces read from the landing buffers (halo_in)
+    // (DEF_MB is a compile-time constant so that only the variant a precision can launch is instantiated)
+    constexpr int DEF_MB = sizeof(T) == 8 ? 2 : 4;
     if (halo_in) {
         const int b = ctx->backfield ? 1 + ctx->backfield_format : 0;
-        if (sizeof(T) == 8) { if (b == 0) GO2(2, 0, 0, 1); else if (b == 1) GO2(2, 0, 1, 1); else GO2(2, 0, 2, 1); }
-        else { if (b == 0) GO2(4, 0, 0, 1); else if (b == 1) GO2(4, 0, 1, 1); else GO2(4, 0, 2, 1); }
+        if (b == 0) GO2(DEF_MB, 0, 0, 1); else if (b == 1) GO2(DEF_MB, 0, 1, 1); else GO2(DEF_MB, 0, 2, 1);
     } else
     // with a backfield: the per-precision default variant only (the tuning options dslash_minblocks and
     // l2_hints select nothing there)
-    if (ctx->backfield && ctx->backfield_format == 0) { if (sizeof(T) == 8) GO1(2, 0, 1); else GO1(4, 0, 1); }
-    else if (ctx->backfield) { if (sizeof(T) == 8) GO1(2, 0, 2); else GO1(4, 0, 2); }
+    if (ctx->backfield && ctx->backfield_format == 0) GO1(DEF_MB, 0, 1);
+    else if (ctx->backfield) GO1(DEF_MB, 0, 2);
     else if (minb <= 2) GO(2); else if (minb == 3) GO(3); else GO(4);
 #undef GO
 #undef GO1

@@ -4,6 +4,8 @@
     python sweep.py --multishift        # config 4: 24^3x48 and 32^4 solves
     python sweep.py --dims 16,16,16,16 --ladder
     python sweep.py --slab              # NEXT-2: slab path (torchrun for N > 1)
+    python sweep.py --backfield         # Dslash with the backfield, both storage formats, all precisions / link formats
+    python sweep.py --staples --dims 32,32,32,32 --variants 2 --options 'staples_minblocks=2;staples_minblocks=3'
 
 Prints one JSON line per measurement and, with --md FILE, appends a Markdown table.  Timing is by
 CUDA events on the launching stream after warm-up.  Volumes whose links fit the 126 MB L2 are
@@ -211,8 +213,45 @@ def slab(dims_list, out, transports=("peer", "hooks")):
     D.finalize(world)
 
 
-def staples(dims_list, out, variants=(0, 1, 2), precs=(0, 1), recons=(0, 1)):
-    """NEXT-4: gauge staples, the three algorithm variants, fp64 / fp32, 18- / 12-real links."""
+def backfield(dims_list, out):
+    """Dslash with the backfield (the paper's fourth acc_Deo argument): plain / theta stored (format 0) / (cos, sin) stored
+    (format 1), fp64 and fp32, 18- and 12-real links; us per launch over 500 alternating (D_oe, D_eo) pairs."""
+    import numpy as np
+    import torch
+    import lqcd_inputs as gen
+    import paper_1701_00426_b200 as L
+
+    for dims in dims_list:
+        rng = np.random.default_rng(5)
+        U = gen.smooth_links(dims, 0.5, rng)
+        ie, io = gen.gaussian_half_spinor(dims, rng), gen.gaussian_half_spinor(dims, rng)
+        theta = gen.uniform_backfield(dims, np.random.default_rng(33))
+        Vh = gen.volume(dims) // 2
+        for prec in (0, 1):
+            for recon in (0, 1):
+                rec = dict(kind="backfield", dims="x".join(map(str, dims)), prec=("f64", "f32")[prec], links=(18, 12)[recon])
+                for label, fmt, add in (("plain_us", None, 0), ("theta_us", 0, 64), ("cossin_us", 1, 128)):
+                    lat = L.Lattice(dims, prec=prec, recon=recon, options=dict(backfield_format=fmt or 0))
+                    links = lat.pack_links(U)
+                    if fmt is not None:
+                        lat.set_backfield(lat.pack_backfield(theta))
+                    a, b, oo, oe = lat.pack_spinor(ie, 0), lat.pack_spinor(io, 1), lat.new_spinor(), lat.new_spinor()
+
+                    def step():
+                        lat.dslash(1, oo, a, links)
+                        lat.dslash(0, oe, b, links)
+                    us = ev_time_us(torch, step, 500, 10) / 2
+                    rec[label] = round(us, 1)
+                    by = (BYTES[(prec, recon)] + add // (1 + prec)) * Vh
+                    rec[label.replace("_us", "_GBs")] = round(by / us / 1e3, 0)
+                    lat.close()
+                    del links, a, b, oo, oe
+                out(rec)
+
+
+def staples(dims_list, out, variants=(0, 1, 2), precs=(0, 1), recons=(0, 1), option_sets=({},)):
+    """NEXT-4: gauge staples, the three algorithm variants, fp64 / fp32, 18- / 12-real links; option_sets: extra
+    lqcd_set_option settings to sweep (e.g. staples_minblocks, staples_x2block), one run per set."""
     import numpy as np
     import torch
     import lqcd_inputs as gen
@@ -226,14 +265,17 @@ def staples(dims_list, out, variants=(0, 1, 2), precs=(0, 1), recons=(0, 1)):
         for prec in precs:
             for recon in recons:
                 for variant in variants:
-                    lat = L.Lattice(dims, prec=prec, recon=recon, options=dict(staples_variant=variant))
-                    links = lat.pack_links(U)
-                    buf = lat.gauge_staples(links)
-                    us = ev_time_us(torch, lambda: lat.gauge_staples(links, out=buf), 10, 2)
-                    out(dict(kind="staples", dims="x".join(map(str, dims)), prec=("f64", "f32")[prec], links=(18, 12)[recon],
-                             variant=variant, ran=lat.get_option("staples_ran"), us=round(us, 1), ns_per_site=round(us * 1e3 / V, 3),
-                             TFLOPs=round(flop_site * V / us / 1e6, 2)))
-                    lat.close()
+                    for opts in option_sets:
+                        lat = L.Lattice(dims, prec=prec, recon=recon, options=dict(opts, staples_variant=variant))
+                        links = lat.pack_links(U)
+                        buf = lat.gauge_staples(links)
+                        us = ev_time_us(torch, lambda: lat.gauge_staples(links, out=buf), 10, 2)
+                        out(dict(kind="staples", dims="x".join(map(str, dims)), prec=("f64", "f32")[prec], links=(18, 12)[recon],
+                                 variant=variant, options=",".join(f"{k}={v}" for k, v in opts.items()) or "-",
+                                 ran=lat.get_option("staples_ran"), us=round(us, 1), ns_per_site=round(us * 1e3 / V, 3),
+                                 TFLOPs=round(flop_site * V / us / 1e6, 2)))
+                        lat.close()
+                        del links, buf
 
 
 _UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
@@ -289,6 +331,9 @@ def main():
     ap.add_argument("--variants", default="0,1,2", help="with --staples: algorithm variants to time")
     ap.add_argument("--precs", default="0,1", help="with --staples: 0 = fp64, 1 = fp32")
     ap.add_argument("--recons", default="0,1", help="with --staples: 0 = 18-real, 1 = 12-real links")
+    ap.add_argument("--options", default="", help="with --staples: option sets to sweep, e.g. "
+                    "'staples_minblocks=2,staples_x2block=4;staples_minblocks=3,staples_x2block=0' (one run per ';' set)")
+    ap.add_argument("--backfield", action="store_true", help="Dslash with / without the backfield, both storage formats")
     ap.add_argument("--eps", type=float, default=0.5)
     ap.add_argument("--seed", type=int, default=5)
     ap.add_argument("--md", default=None)
@@ -311,12 +356,16 @@ def main():
         multishift(dims_list or [(24, 24, 24, 48), (32, 32, 32, 32)], out)
     if args.staples:
         ints = lambda t: tuple(int(v) for v in t.split(","))   # noqa: E731
-        staples(dims_list or [(16,) * 4, (32, 32, 32, 8), (32,) * 4], out, ints(args.variants), ints(args.precs), ints(args.recons))
+        sets = [dict((kv.split("=")[0], int(kv.split("=")[1])) for kv in st.split(",") if kv) for st in args.options.split(";")] \
+            if args.options else [{}]
+        staples(dims_list or [(16,) * 4, (32, 32, 32, 8), (32,) * 4], out, ints(args.variants), ints(args.precs), ints(args.recons), sets)
+    if args.backfield:
+        backfield(dims_list or [(32, 32, 32, 32)], out)
     if args.slab:
         slab(dims_list or [(32, 32, 32, 32)], out)
     if args.md:
         with open(args.md, "a") as f:
-            for kind in ("dslash", "cg", "multishift_solve", "slab_dslash", "slab_multishift8", "staples"):
+            for kind in ("dslash", "cg", "multishift_solve", "slab_dslash", "slab_multishift8", "staples", "backfield"):
                 sel = [r for r in rows if r["kind"] == kind]
                 if not sel:
                     continue
