@@ -469,11 +469,19 @@ def run_ours(args):
         xs8 = [lat.new_spinor() for _ in shifts]
         lat.cg_multishift(xs8, d_in_e, links, 0.0025, shifts, 1e-300, 8, raise_on_max_iter=False)
         fbuf = lat.fermion_force(xs8, links, [1.0] * 8)
-        t_f = timed_loop(torch, lambda: lat.fermion_force(xs8, links, [1.0] * 8, force=fbuf), 20, 3, 1, D, device) / 20
-        by = 8 * 1248 * Vh + V * (576 + 48 * 8 + 256)
+        # the method's own bytes: the y_i = D_oe x_i need every link of an odd site's 8 hops ONCE (1152 B) plus 96 B per
+        # shift (48 in, 48 out); the outer products 576 B of links + 48 B per shift + 256 B of 8-real force per site
+        by = Vh * (1152 + 96 * 8) + V * (576 + 48 * 8 + 256)
+        by_block = {}
+        for blk in (0, 4, 8):                 # one Dslash per shift (round 2) / two blocks of 4 / one block of 8 (default, last)
+            lat.set_option("force_block", blk)
+            t_b = timed_loop(torch, lambda: lat.fermion_force(xs8, links, [1.0] * 8, force=fbuf), 20, 3, 1, D, device) / 20
+            by_block[str(blk)] = {"ms": t_b, "frac_of_method_bytes": by / (t_b * 1e-3) / 1e9 / peak}
+        t_f = by_block["8"]["ms"]
         extra["fermion_force8_f64"] = {"ms": t_f, "ns_per_site": t_f * 1e6 / V, "bytes": by, "GBs": by / (t_f * 1e-3) / 1e9,
-                                       "frac": by / (t_f * 1e-3) / 1e9 / peak,
-                                       "note": "8 x D_oe (1248 B per odd site) + outer products (576 links + 48*8 vectors + 256 B of 8-real force per site)"}
+                                       "frac": by / (t_f * 1e-3) / 1e9 / peak, "by_force_block": by_block,
+                                       "note": "block Dslash for the 8 y_i (one launch, every link once: 1152 + 8 x 96 B per odd site) + outer products "
+                                               "(576 links + 48*8 vectors + 256 B of 8-real force per site)"}
         del xs8, fbuf
         # ---- NEXT-4: tree-level Symanzik gauge staples (ALU bound) against the FP64 rate measured here
         fp64_peak = lat.measure_fp64_peak()

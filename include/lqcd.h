@@ -119,6 +119,20 @@ int lqcd_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical_dev, const voi
 int lqcd_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links);
 
 /*
+ * Block Dslash: outs[r] = D ins[r] on the sites of `parity` for r = 0..n-1 (Eq. 7, same operator as
+ * lqcd_dslash).  Every thread loads each of its 8 links once per block of right-hand sides (option "force_block": 8,
+ * the default, or 4 per launch; a remainder runs in blocks of 4, 2 and 1) instead of once per vector: 1152 + 96 k bytes per
+ * site and block of k vectors in fp64 with 18-real links, against 1248 k.  Per vector the arithmetic and its order are
+ * those of lqcd_dslash: the results are bit-identical.  lqcd_fermion_force computes its y_i = D_oe x_i this way
+ * (PAPER.md:315).
+ *   outs, ins   host arrays of n device pointers (native half vectors); no output may alias any input
+ *   1 <= n <= LQCD_MAX_SHIFTS
+ * async.  Errors: LQCD_ERR_ARG; LQCD_ERR_UNSUPPORTED with a backfield attached or on a slab context (use lqcd_dslash).
+ */
+int lqcd_dslash_multi(lqcd_ctx *ctx, int parity, int n, void *const *outs, const void *const *ins,
+                      const void *links);
+
+/*
  * The `backfield` argument of the paper's acc_Deo(u, out, in, backfield) (Listing 2): one
  * real per link (the paper's double_soa), never explained in the text.  Reading R6 of DESIGN.md: an external
  * U(1) phase theta_mu(x); every link enters D as e^{i theta_mu(x)} U_mu(x), i.e. the forward hop out of x is

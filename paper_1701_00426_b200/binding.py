@@ -56,6 +56,7 @@ _sig = {
     "lqcd_pack_spinor": (_i, [_vp, _i, _vp, _vp]),
     "lqcd_unpack_spinor": (_i, [_vp, _i, _vp, _vp]),
     "lqcd_dslash": (_i, [_vp, _i, _vp, _vp, _vp]),
+    "lqcd_dslash_multi": (_i, [_vp, _i, _i, C.POINTER(_vp), C.POINTER(_vp), _vp]),
     "lqcd_backfield_bytes": (_sz, [_vp]),
     "lqcd_pack_backfield": (_i, [_vp, _vp, _vp]),
     "lqcd_set_backfield": (_i, [_vp, _vp]),
@@ -220,6 +221,14 @@ class Lattice:
     # -- the hot path (async unless stated) ---------------------------------------------------
     def dslash(self, parity, out, inp, links):
         self._check(lib.lqcd_dslash(self._ctx, parity, _vp(out.data_ptr()), _vp(inp.data_ptr()), _vp(links.data_ptr())))
+
+    def dslash_multi(self, parity, outs, inps, links):
+        """block Dslash: outs[r] = D inps[r]; every link loaded once per block of right-hand sides.  async."""
+        n = len(outs)
+        assert len(inps) == n
+        po = (_vp * n)(*[o.data_ptr() for o in outs])
+        pi = (_vp * n)(*[i.data_ptr() for i in inps])
+        self._check(lib.lqcd_dslash_multi(self._ctx, parity, n, po, pi, _vp(links.data_ptr())))
 
     def pack_backfield(self, theta):
         """theta: float64 [V][4] (numpy), the per-link U(1) phases -> native device buffer."""

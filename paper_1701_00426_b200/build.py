@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "liblqcd_b200.so")
-SOURCES = ["api.cu", "pack.cu", "dslash.cu", "solver.cu", "host.cu", "force.cu", "staples.cu", "diag.cu", "peer.cu", "noalloc.cu"]
+SOURCES = ["api.cu", "pack.cu", "dslash.cu", "solver.cu", "host.cu", "force.cu", "staples.cu", "diag.cu", "peer.cu", "noalloc.cu", "dslash_multi.cu"]
 HEADERS = ["common.cuh", "reduce.cuh", "su3.cuh", "peer.cuh", os.path.join("..", "..", "include", "lqcd.h"),
            os.path.join("..", "..", "include", "lqcd_diag.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

@@ -288,6 +288,7 @@ struct lqcd_ctx {
     int backfield_locked;  // a backfield was packed: the format can no longer change
     const void *backfield; // native U(1) phase field applied by every Dslash of this context (NULL: none; lqcd_set_backfield)
     int force_stage;       // 1: force_kernel stages the site's own vectors in shared memory when they fit
+    int force_block;       // right-hand sides per launch of the block Dslash that computes the y_i (0: one Dslash per shift; 4; 8)
     int staples_x2block;   // x2 block size of the staples' CTA order (0: plain idxh order)
     int staples_variant;   // 0: one product chain per path; 1: shared sub-products per (mu, nu); 2: two passes through
                            // stored 3-link staples (needs lqcd_staples_workspace_bytes of workspace, else 1 runs)
@@ -369,6 +370,8 @@ int launch_unpack_spinor(lqcd_ctx *ctx, int parity, void *canonical, const void 
 // landing buffers (the face push fused into the producer)
 int launch_dslash(lqcd_ctx *ctx, int parity, void *out, const void *in, const void *links,
                   const void *xpay_in, double coef, int dot_mode, int gate, int x3_lo = -1, int x3_hi = -1, int push_out = 0);
+// block Dslash (dslash_multi.cu): outs[r] = D ins[r], r < n, each link loaded once per block of `blk` (4 or 8) vectors
+int launch_dslash_multi(lqcd_ctx *ctx, int parity, int n, void *const *outs, const void *const *ins, const void *links, int blk);
 int peer_after_producer(lqcd_ctx *ctx, int kind, int gate);
 long peer_timeouts(lqcd_ctx *ctx);           // waits that gave up (blocking read of the rank's block)
 int peer_guard(lqcd_ctx *ctx, int kind);     // barrier before two exchanges of the same kind in a row (peer.cu)    // lock-step validation: signal kernel + host hook

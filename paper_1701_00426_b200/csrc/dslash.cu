@@ -18,33 +18,6 @@
 #include "peer.cuh"
 #include "su3.cuh"
 
-// acc += U p
-template <typename T> __device__ __forceinline__ void mv_acc(Cx<T> acc[3], const Su3<T> &u, const Cx<T> p[3])
-{
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b) {
-            acc[a].re = fma(u.e[a][b].re, p[b].re, acc[a].re);
-            acc[a].re = fma(-u.e[a][b].im, p[b].im, acc[a].re);
-            acc[a].im = fma(u.e[a][b].re, p[b].im, acc[a].im);
-            acc[a].im = fma(u.e[a][b].im, p[b].re, acc[a].im);
-        }
-}
-// acc += U^dagger p,  (U^dagger)_{ab} = conj(U_{ba})
-template <typename T> __device__ __forceinline__ void mvdag_acc(Cx<T> acc[3], const Su3<T> &u, const Cx<T> p[3])
-{
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b) {
-            acc[a].re = fma(u.e[b][a].re, p[b].re, acc[a].re);
-            acc[a].re = fma(u.e[b][a].im, p[b].im, acc[a].re);
-            acc[a].im = fma(u.e[b][a].re, p[b].im, acc[a].im);
-            acc[a].im = fma(-u.e[b][a].im, p[b].re, acc[a].im);
-        }
-}
-
 // MODE 0: out = D in;  1: out = coef*x - D in;  2: as 1, plus Re<x,out> -> solver_after_pq
 // BF != 0: every link enters as e^{i theta_mu(x)} U_mu(x) (the `backfield` argument of the paper's acc_Deo, Listing 2,
 // PAPER.md:320-326; reading R6), [parity][mu][idxh]; the phase multiplies the neighbour vector together with

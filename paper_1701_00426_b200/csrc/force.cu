@@ -267,11 +267,21 @@ extern "C" int lqcd_fermion_force(lqcd_ctx *ctx, int nshift, const double *coeff
     memset(&fx, 0, sizeof(fx));
     memset(&fy, 0, sizeof(fy));
     fx.n = fy.n = nshift;
+    // plain context: all y_i from the block Dslash, which loads every link once per block of right-hand sides instead
+    // of once per shift (dslash_multi.cu); slab contexts and a backfield keep one Dslash per shift
+    const bool block = !slab && !ctx->backfield && ctx->force_block >= 2 && nshift >= 2;
+    if (block) {
+        void *ys[LQCD_MAX_SHIFTS];
+        for (int i = 0; i < nshift; ++i) ys[i] = ws_vec(ctx, 4 + i);
+        if ((rc = launch_dslash_multi(ctx, 1 - par, nshift, ys, (const void *const *)xs_e, links, ctx->force_block))) return rc;
+    }
     for (int i = 0; i < nshift; ++i) {
         void *y = ws_vec(ctx, 4 + i);
-        if ((rc = ghosts(xs_e[i], par))) return rc;
-        if ((rc = launch_dslash(ctx, 1 - par, y, xs_e[i], links, NULL, 0.0, 0, 0))) return rc;
-        if (slab && (rc = ghosts(y, 1 - par))) return rc;
+        if (!block) {
+            if ((rc = ghosts(xs_e[i], par))) return rc;
+            if ((rc = launch_dslash(ctx, 1 - par, y, xs_e[i], links, NULL, 0.0, 0, 0))) return rc;
+            if (slab && (rc = ghosts(y, 1 - par))) return rc;
+        }
         fx.self[i] = xs_e[i]; fx.nbr[i] = y; fx.coef[i] = coeffs[i];        // x even: + c_i y_i(x+mu) x_i(x)^dagger
         fy.self[i] = y; fy.nbr[i] = xs_e[i]; fy.coef[i] = -coeffs[i];       // x odd:  - c_i x_i(x+mu) y_i(x)^dagger
     }

@@ -32,6 +32,33 @@ __device__ __forceinline__ Su3<T> load_link(const T *__restrict__ links, int par
     return u;
 }
 
+// acc += U p
+template <typename T> __device__ __forceinline__ void mv_acc(Cx<T> acc[3], const Su3<T> &u, const Cx<T> p[3])
+{
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            acc[a].re = fma(u.e[a][b].re, p[b].re, acc[a].re);
+            acc[a].re = fma(-u.e[a][b].im, p[b].im, acc[a].re);
+            acc[a].im = fma(u.e[a][b].re, p[b].im, acc[a].im);
+            acc[a].im = fma(u.e[a][b].im, p[b].re, acc[a].im);
+        }
+}
+// acc += U^dagger p,  (U^dagger)_{ab} = conj(U_{ba})
+template <typename T> __device__ __forceinline__ void mvdag_acc(Cx<T> acc[3], const Su3<T> &u, const Cx<T> p[3])
+{
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            acc[a].re = fma(u.e[b][a].re, p[b].re, acc[a].re);
+            acc[a].re = fma(u.e[b][a].im, p[b].im, acc[a].re);
+            acc[a].im = fma(u.e[b][a].re, p[b].im, acc[a].im);
+            acc[a].im = fma(-u.e[b][a].im, p[b].re, acc[a].im);
+        }
+}
+
 template <typename T, int LAYOUT, int POLICY>
 __device__ __forceinline__ void load_vec(const T *__restrict__ v, size_t Vh, size_t i, T coef, Cx<T> p[3], const L2Pol &pol)
 {

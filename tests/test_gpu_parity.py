@@ -741,3 +741,53 @@ def test_multishift_config4_32x4_properties_at_full_size():
     assert np.all(np.diff(res["conv_iter"]) <= 0)          # larger shifts freeze earlier
     assert res["conv_iter"][0] == res["iters"]
     lat.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# block Dslash (several right-hand sides per launch; dslash_multi.cu)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("layout", [0, 1])
+@pytest.mark.parametrize("recon", [0, 1])
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("dims,n,blk", [((4, 4, 4, 4), 1, 4), ((6, 4, 2, 8), 3, 4), ((12, 10, 6, 4), 7, 4), ((12, 10, 6, 4), 11, 8),
+                                        ((2, 2, 2, 2), 8, 8)])
+def test_dslash_multi_equals_oracle_and_single(dims, n, blk, prec, recon, layout):
+    """lqcd_dslash_multi: every right-hand side against oracle.dslash_half (both parities, ragged lattices, N = 2 wrap,
+    block remainders 8 + 2 + 1, 4 + 2 + 1, ...) and BIT-identical to n single lqcd_dslash applications."""
+    rng = np.random.default_rng(31)
+    U = gen.haar_like_links(dims, rng)
+    ins = [gen.gaussian_half_spinor(dims, rng) for _ in range(n)]
+    U, *ins = round_inputs(prec, U, *ins)
+    if recon == 1 and prec == 1:
+        U = oracle.reconstruct_row3(U)
+    lat = make_lattice(dims, prec, recon, True, layout=layout, force_block=blk)
+    links = lat.pack_links(U)
+    for out_parity in (0, 1):
+        d_in = [lat.pack_spinor(v, 1 - out_parity) for v in ins]
+        d_out = [lat.new_spinor() for _ in range(n)]
+        single = lat.new_spinor()
+        lat.dslash_multi(out_parity, d_out, d_in, links)
+        for r in range(n):
+            got = lat.unpack_spinor(d_out[r], out_parity)
+            assert rel(got, oracle.dslash_half(dims, U, out_parity, ins[r])) < TOL[prec], (dims, n, prec, recon, layout, out_parity, r)
+            lat.dslash(out_parity, single, d_in[r], links)
+            lat.synchronize()
+            assert bool((single == d_out[r]).all()), (dims, n, prec, recon, layout, out_parity, r)
+    lat.close()
+
+
+def test_dslash_multi_errors():
+    import paper_1701_00426_b200 as L
+    dims = (4, 4, 4, 4)
+    lat = make_lattice(dims)
+    links = lat.pack_links(gen.unit_links(dims))
+    a, b = lat.new_spinor(), lat.new_spinor()
+    with pytest.raises(L.LqcdError) as e:
+        lat.dslash_multi(0, [a, b], [b, b], links)            # output 1 aliases an input
+    assert e.value.code == L.ERR_ARG
+    theta = np.zeros((lat.V, 4))
+    lat.set_backfield(lat.pack_backfield(theta))
+    with pytest.raises(L.LqcdError) as e:
+        lat.dslash_multi(0, [a], [b], links)
+    assert e.value.code == L.ERR_UNSUPPORTED
+    lat.close()
