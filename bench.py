@@ -70,6 +70,11 @@ def ncu_traffic(kernel_name):
     if ent is None:
         raise SystemExit(f"bench.py: profiles/traffic.json has no entry for the kernel this run launches "
                          f"({kernel_name}); re-capture it (python sweep.py --traffic-from-ncu)")
+    # the capture must be of THIS build: traffic.json carries a hash of the kernel's sources (sweep.py writes it)
+    import sweep
+    ent = dict(ent)
+    ent["source_hash_now"] = sweep.kernel_source_hash()
+    ent["stale"] = ent.get("source_hash") != ent["source_hash_now"]
     return ent
 
 
@@ -615,9 +620,11 @@ def run_ours(args):
             "applications_timed": apps, "pairs_per_step": k,
             "GFLOPs": FLOP_PER_SITE * Vh * world / (us_launch * 1e-6) / 1e9,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": traffic["dram_bytes"], "traffic_source": traffic.get("source"),
-                         "traffic_commit": traffic.get("commit"),
-                         "frac_by_ncu_traffic": traffic["dram_bytes"] / (us_launch * 1e-6) / 1e9 / peak,
+                         # a capture of another build of the kernel's sources is not evidence for this one: null then
+                         "traffic": None if traffic["stale"] else traffic["dram_bytes"], "traffic_source": traffic.get("source"),
+                         "traffic_commit": traffic.get("commit"), "traffic_source_hash": traffic.get("source_hash"),
+                         "traffic_stale": traffic["stale"],
+                         "frac_by_ncu_traffic": None if traffic["stale"] else traffic["dram_bytes"] / (us_launch * 1e-6) / 1e9 / peak,
                          "peak_source": peak_src, "kernel": kernel,
                          "peak_note": "the peak is a 50 %-write copy; this kernel is 96 % reads, so frac may exceed 1",
                          "bytes_per_launch": BYTES_PER_SITE[("f64", 18)] * Vh, "us_per_launch": us_launch,

@@ -279,6 +279,50 @@ def staples(dims_list, out, variants=(0, 1, 2), precs=(0, 1), recons=(0, 1), opt
 
 
 _UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+_TIME_US = {"ns": 1e-3, "us": 1.0, "usecond": 1.0, "nsecond": 1e-3, "ms": 1e3, "msecond": 1e3, "s": 1e6, "second": 1e6}
+KERNEL_SOURCES = ("dslash.cu", "su3.cuh", "common.cuh")      # what the headline kernel is compiled from
+
+
+def kernel_source_hash():
+    """sha256 (first 16 hex digits) over the sources of the Dslash kernel: profiles/traffic.json carries the hash of the
+    build its ncu capture was taken from, bench.py compares it with the checkout it runs."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_1701_00426_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def launches_from_ncu(csv_path, md_path):
+    """Aggregate an `ncu --metrics gpu__time_duration.sum --csv --log-file X.csv` launch list into a Markdown table
+    (launches, total / avg / min / max us, share of the summed device time) per kernel and grid; appended to md_path."""
+    import csv
+    lines = open(csv_path, errors="replace").read().splitlines()
+    start = next(i for i, ln in enumerate(lines) if ln.startswith('"ID"'))
+    rows = list(csv.reader(lines[start:]))
+    hdr = rows[0]
+    col = {n: hdr.index(n) for n in ("Kernel Name", "Grid Size", "Metric Name", "Metric Unit", "Metric Value")}
+    acc, order = {}, []
+    for r in rows[1:]:
+        if len(r) <= col["Metric Value"] or r[col["Metric Name"]] != "gpu__time_duration.sum":
+            continue
+        key = (r[col["Kernel Name"]].split("(")[0].strip(), r[col["Grid Size"]])
+        us = float(r[col["Metric Value"]].replace(",", "")) * _TIME_US[r[col["Metric Unit"]]]
+        if key not in acc:
+            acc[key] = []
+            order.append(key)
+        acc[key].append(us)
+    total = sum(sum(v) for v in acc.values())
+    n_all = sum(len(v) for v in acc.values())
+    with open(md_path, "a") as f:
+        f.write(f"\n{n_all} launches, {total / 1e3:.1f} ms of summed device time\n\n"
+                "| launches | total us | avg us | min us | max us | share | kernel |\n|---|---|---|---|---|---|---|\n")
+        for key in order:
+            v = acc[key]
+            f.write(f"| {len(v)} | {sum(v):.1f} | {sum(v) / len(v):.2f} | {min(v):.2f} | {max(v):.2f} | "
+                    f"{100 * sum(v) / total:.1f} % | `{key[0]}` grid {key[1]} |\n")
+    print(json.dumps({"launches": n_all, "total_ms": total / 1e3, "kernels": len(acc)}))
 
 
 def traffic_from_ncu(csv_path, commit, source):
@@ -310,7 +354,8 @@ def traffic_from_ncu(csv_path, commit, source):
         n = len(v)
         table[name] = {"dram_bytes": sum(a + b for a, b, _ in v) / n, "dram_read_bytes": sum(a for a, _, _ in v) / n,
                        "dram_write_bytes": sum(b for _, b, _ in v) / n, "launches_captured": n,
-                       "ncu_duration_us": sum(t for _, _, t in v) / n, "commit": commit, "source": source}
+                       "ncu_duration_us": sum(t for _, _, t in v) / n, "commit": commit, "source": source,
+                       "source_hash": kernel_source_hash(), "hashed_files": list(KERNEL_SOURCES)}
     with open(path, "w") as f:
         json.dump(table, f, indent=1, sort_keys=True)
         f.write("\n")
@@ -323,6 +368,8 @@ def main():
                     help="write profiles/traffic.json from an `ncu --page raw --csv` export (no GPU needed)")
     ap.add_argument("--commit", default="", help="with --traffic-from-ncu: the commit the capture was taken at")
     ap.add_argument("--source", default="", help="with --traffic-from-ncu: the profiles/*.md that describes the capture")
+    ap.add_argument("--launches-from-ncu", default=None, metavar="LAUNCHES.csv",
+                    help="aggregate an `ncu --metrics gpu__time_duration.sum --csv` log into a table appended to --md (no GPU needed)")
     ap.add_argument("--ladder", action="store_true")
     ap.add_argument("--multishift", action="store_true")
     ap.add_argument("--staples", action="store_true", help="NEXT-4 gauge staples timing")
@@ -340,6 +387,9 @@ def main():
     args = ap.parse_args()
     if args.traffic_from_ncu:
         traffic_from_ncu(args.traffic_from_ncu, args.commit, args.source)
+        return
+    if args.launches_from_ncu:
+        launches_from_ncu(args.launches_from_ncu, args.md or os.path.join(ROOT, "profiles", "launches.md"))
         return
     dims_list = None
     if args.dims:
