@@ -281,6 +281,7 @@ def staples(dims_list, out, variants=(0, 1, 2), precs=(0, 1), recons=(0, 1), opt
 _UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
 _TIME_US = {"ns": 1e-3, "us": 1.0, "usecond": 1.0, "nsecond": 1e-3, "ms": 1e3, "msecond": 1e3, "s": 1e6, "second": 1e6}
 KERNEL_SOURCES = ("dslash.cu", "su3.cuh", "common.cuh")      # what the headline kernel is compiled from
+SRC_DIR = os.path.join(os.path.dirname(os.path.abspath(__file__)), "paper_1701_00426_b200", "csrc")
 
 
 def kernel_source_hash():
@@ -289,7 +290,7 @@ def kernel_source_hash():
     import hashlib
     h = hashlib.sha256()
     for f in KERNEL_SOURCES:
-        with open(os.path.join(ROOT, "paper_1701_00426_b200", "csrc", f), "rb") as fh:
+        with open(os.path.join(SRC_DIR, f), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()[:16]
 

@@ -240,6 +240,8 @@ def test_traffic_json_matches_the_kernel_bench_launches(tmp_path, monkeypatch):
     table = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
     assert name in table and table[name]["dram_bytes"] > 6e8
     assert bench.ncu_traffic(name)["dram_bytes"] == table[name]["dram_bytes"]
+    # the committed capture is of THIS checkout's kernel sources (else bench.py reports roofline.traffic = null)
+    assert table[name]["source_hash"] == sweep.kernel_source_hash() and bench.ncu_traffic(name)["stale"] is False
     with pytest.raises(SystemExit):
         bench.ncu_traffic("dslash_kernel<double,9,9>")
     # the parser, on a fabricated export, writing into a scratch root
@@ -253,5 +255,5 @@ def test_traffic_json_matches_the_kernel_bench_launches(tmp_path, monkeypatch):
     sweep.traffic_from_ncu(str(csvp), "abc1234", "test")
     got = json.load(open(tmp_path / "profiles" / "traffic.json"))
     ent = got[name]
-    assert ent["launches_captured"] == 2 and ent["commit"] == "abc1234"
+    assert ent["launches_captured"] == 2 and ent["commit"] == "abc1234" and ent["source_hash"] == sweep.kernel_source_hash()
     assert abs(ent["dram_bytes"] - (601.0e6 + 6.0e6)) < 1 and abs(ent["ncu_duration_us"] - 95.0) < 1e-9
